@@ -1,0 +1,108 @@
+"""oracle — TEST INFRASTRUCTURE ONLY.
+
+A plain, slow CPU oracle (768-bit cyclic Jacobi on MPFR, C source in zkd_oracle.c) for the result the hot path
+computes: the eigendecomposition of a dense complex Hermitian matrix at 768-bit precision (2.1).
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import this package.
+It imports nothing from paper_2402_11868_b200 (the CUDA path) and the CUDA path imports nothing from here.
+
+Parity status: pinned (tests/test_oracle_pins.py) — see the header of zkd_oracle.c for the list of pins.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libzkd_oracle.so")
+_SRCS = [os.path.join(_HERE, "zkd_oracle.c"), os.path.join(_HERE, "mpfr_abi.h")]
+
+PREC = 768
+GUARD_BITS = 128  # reading A6
+
+
+def build(force: bool = False) -> str:
+    if force or not os.path.exists(_SO) or any(os.path.getmtime(_SO) < os.path.getmtime(s) for s in _SRCS):
+        subprocess.check_call(
+            ["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", _SO, _SRCS[0], "-l:libmpfr.so.6", "-l:libgmp.so.10", "-lm"]
+        )
+    return _SO
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(build())
+        vp = ctypes.c_void_p
+        L.zkd_oracle_diag_herm.restype = ctypes.c_int
+        L.zkd_oracle_diag_herm.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                           ctypes.c_long, vp, vp, vp, vp]
+        L.zkd_oracle_compare.restype = ctypes.c_int
+        L.zkd_oracle_compare.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, vp, vp, vp, vp, vp, ctypes.c_int, vp]
+        L.zkd_oracle_api_to_double.restype = ctypes.c_double
+        L.zkd_oracle_api_to_double.argtypes = [vp, ctypes.c_int]
+        L.zkd_oracle_api_from_double.argtypes = [vp, ctypes.c_int, ctypes.c_double]
+        L.zkd_oracle_mpfr_version.restype = ctypes.c_char_p
+        L.zkd_oracle_max_threads.restype = ctypes.c_int
+        _lib = L
+    return _lib
+
+
+def real_bytes(prec: int = PREC) -> int:
+    return 16 + prec // 8
+
+
+def host_threads() -> int:
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:  # pragma: no cover
+        return os.cpu_count() or 1
+
+
+def diag_herm(A: np.ndarray, N: int, prec: int = PREC, ordering: str = "row-cyclic", guard_bits: int = GUARD_BITS,
+              threads: int | None = None, max_rotations: int = 0, want_vectors: bool = True):
+    """Cyclic Jacobi eigendecomposition of ONE N x N Hermitian matrix given in the API layout.
+    Returns (eigvals uint8[N*rb], eigvecs uint8[N*N*2*rb] or None, info dict)."""
+    rb = real_bytes(prec)
+    A = np.ascontiguousarray(A, dtype=np.uint8)
+    assert A.size == N * N * 2 * rb, (A.size, N)
+    lam = np.zeros(N * rb, dtype=np.uint8)
+    X = np.zeros(N * N * 2 * rb, dtype=np.uint8) if want_vectors else None
+    info = (ctypes.c_long * 3)()
+    o = {"row-cyclic": 0, "round-robin": 1}[ordering]
+    t = threads or (host_threads() if o == 1 else 1)
+    rc = lib().zkd_oracle_diag_herm(N, prec, guard_bits, o, t, max_rotations, A.ctypes.data, lam.ctypes.data,
+                                    X.ctypes.data if want_vectors else None, info)
+    return lam, X, {"status": rc, "sweeps": info[0], "rotations": info[1], "threads": t}
+
+
+def compare(A: np.ndarray, N: int, lam: np.ndarray, X: np.ndarray, lam0: np.ndarray | None = None,
+            X0: np.ndarray | None = None, cols=None, prec: int = PREC, threads: int | None = None) -> dict:
+    """Comparator of SURVEY.md 8(c): returns log2 error measures (see zkd_oracle_compare)."""
+    out = np.zeros(8, dtype=np.float64)
+    c = np.ascontiguousarray(cols, dtype=np.int32) if cols is not None else None
+    lib().zkd_oracle_compare(
+        N, prec, threads or host_threads(),
+        np.ascontiguousarray(A).ctypes.data, np.ascontiguousarray(lam).ctypes.data, np.ascontiguousarray(X).ctypes.data,
+        np.ascontiguousarray(lam0).ctypes.data if lam0 is not None else None,
+        np.ascontiguousarray(X0).ctypes.data if X0 is not None else None,
+        c.ctypes.data if c is not None else None, len(c) if c is not None else 0, out.ctypes.data)
+    return {"log2_dlam_rel": out[0], "log2_resid_rel": out[1], "log2_orth": out[2], "vec_margin_bits": out[3],
+            "log2_F": out[4], "groups": int(out[5]) if out[5] > -1e8 else 0,
+            "max_group": int(out[6]) if out[6] > -1e8 else 0, "log2_vec_err": out[7]}
+
+
+def api_to_double(buf, prec: int = PREC) -> float:
+    b = np.ascontiguousarray(np.frombuffer(bytes(buf), dtype=np.uint8))
+    return lib().zkd_oracle_api_to_double(b.ctypes.data, prec)
+
+
+def api_from_double(v: float, prec: int = PREC) -> bytes:
+    b = np.zeros(real_bytes(prec), dtype=np.uint8)
+    lib().zkd_oracle_api_from_double(b.ctypes.data, prec, v)
+    return bytes(b)

@@ -1,0 +1,78 @@
+/* oracle/mpfr_abi.h — TEST INFRASTRUCTURE ONLY (see oracle/README.md).
+ *
+ * The image ships libmpfr.so.6 (MPFR 4.2.1) and libgmp.so.10 but neither mpfr.h nor gmp.h.
+ * This file declares, by hand, the handful of MPFR entry points the oracle calls.  It is an
+ * interface declaration for linking against the system library (-l:libmpfr.so.6 -l:libgmp.so.10);
+ * it contains no arithmetic.  The struct layout is the documented public one
+ * ({precision, sign, exponent, limb pointer}; limbs little-endian, significand left-aligned,
+ * value = sign * 0.d[n-1]...d[0] * 2^exp, i.e. mantissa in [1/2,1)).
+ *
+ * Not shared with the CUDA path or with zkd_inputs/ (each side declares what it links against).
+ */
+#ifndef ZKD_ORACLE_MPFR_ABI_H
+#define ZKD_ORACLE_MPFR_ABI_H
+
+#include <limits.h>
+
+typedef long mpfr_prec_t;
+typedef int mpfr_sign_t;
+typedef long mpfr_exp_t;
+typedef unsigned long mp_limb_t;
+
+typedef struct {
+  mpfr_prec_t _mpfr_prec;
+  mpfr_sign_t _mpfr_sign;
+  mpfr_exp_t _mpfr_exp;
+  mp_limb_t *_mpfr_d;
+} __mpfr_struct;
+
+typedef __mpfr_struct mpfr_t[1];
+typedef __mpfr_struct *mpfr_ptr;
+typedef const __mpfr_struct *mpfr_srcptr;
+
+typedef enum { MPFR_RNDN = 0, MPFR_RNDZ, MPFR_RNDU, MPFR_RNDD, MPFR_RNDA } mpfr_rnd_t;
+
+#define ZKD_MPFR_EXP_ZERO (LONG_MIN + 1)
+
+const char *mpfr_get_version(void);
+void mpfr_init2(mpfr_ptr, mpfr_prec_t);
+void mpfr_clear(mpfr_ptr);
+void mpfr_free_cache(void);
+int mpfr_set(mpfr_ptr, mpfr_srcptr, mpfr_rnd_t);
+int mpfr_set_d(mpfr_ptr, double, mpfr_rnd_t);
+int mpfr_set_si(mpfr_ptr, long, mpfr_rnd_t);
+int mpfr_set_ui(mpfr_ptr, unsigned long, mpfr_rnd_t);
+void mpfr_set_zero(mpfr_ptr, int);
+int mpfr_set_si_2exp(mpfr_ptr, long, mpfr_exp_t, mpfr_rnd_t);
+double mpfr_get_d(mpfr_srcptr, mpfr_rnd_t);
+double mpfr_get_d_2exp(long *, mpfr_srcptr, mpfr_rnd_t);
+mpfr_exp_t mpfr_get_exp(mpfr_srcptr);
+int mpfr_add(mpfr_ptr, mpfr_srcptr, mpfr_srcptr, mpfr_rnd_t);
+int mpfr_sub(mpfr_ptr, mpfr_srcptr, mpfr_srcptr, mpfr_rnd_t);
+int mpfr_mul(mpfr_ptr, mpfr_srcptr, mpfr_srcptr, mpfr_rnd_t);
+int mpfr_sqr(mpfr_ptr, mpfr_srcptr, mpfr_rnd_t);
+int mpfr_div(mpfr_ptr, mpfr_srcptr, mpfr_srcptr, mpfr_rnd_t);
+int mpfr_sqrt(mpfr_ptr, mpfr_srcptr, mpfr_rnd_t);
+int mpfr_neg(mpfr_ptr, mpfr_srcptr, mpfr_rnd_t);
+int mpfr_abs(mpfr_ptr, mpfr_srcptr, mpfr_rnd_t);
+int mpfr_fma(mpfr_ptr, mpfr_srcptr, mpfr_srcptr, mpfr_srcptr, mpfr_rnd_t);
+int mpfr_fms(mpfr_ptr, mpfr_srcptr, mpfr_srcptr, mpfr_srcptr, mpfr_rnd_t);
+int mpfr_fmma(mpfr_ptr, mpfr_srcptr, mpfr_srcptr, mpfr_srcptr, mpfr_srcptr, mpfr_rnd_t);
+int mpfr_fmms(mpfr_ptr, mpfr_srcptr, mpfr_srcptr, mpfr_srcptr, mpfr_srcptr, mpfr_rnd_t);
+int mpfr_mul_2si(mpfr_ptr, mpfr_srcptr, long, mpfr_rnd_t);
+int mpfr_div_2si(mpfr_ptr, mpfr_srcptr, long, mpfr_rnd_t);
+int mpfr_mul_ui(mpfr_ptr, mpfr_srcptr, unsigned long, mpfr_rnd_t);
+int mpfr_div_ui(mpfr_ptr, mpfr_srcptr, unsigned long, mpfr_rnd_t);
+int mpfr_add_ui(mpfr_ptr, mpfr_srcptr, unsigned long, mpfr_rnd_t);
+int mpfr_sub_ui(mpfr_ptr, mpfr_srcptr, unsigned long, mpfr_rnd_t);
+int mpfr_ui_sub(mpfr_ptr, unsigned long, mpfr_srcptr, mpfr_rnd_t);
+int mpfr_ui_div(mpfr_ptr, unsigned long, mpfr_srcptr, mpfr_rnd_t);
+int mpfr_cmp(mpfr_srcptr, mpfr_srcptr);
+int mpfr_cmpabs(mpfr_srcptr, mpfr_srcptr);
+int mpfr_cmp_ui(mpfr_srcptr, unsigned long);
+int mpfr_cmp_si(mpfr_srcptr, long);
+int mpfr_sgn(mpfr_srcptr);
+int mpfr_zero_p(mpfr_srcptr);
+void mpfr_swap(mpfr_ptr, mpfr_ptr);
+
+#endif

@@ -1,0 +1,596 @@
+/* oracle/zkd_oracle.c — TEST INFRASTRUCTURE ONLY.
+ *
+ * Plain, slow, obviously-correct CPU oracle for the hot path of arxiv 2402.11868:
+ * "diagonalizing N x N Hermitian matrix with random elements. The 768-bit precision was used"
+ * (section 2.1; the routine is diag_H / zkcm_omp::diag_H / zkcm_cus::cus_diag_H).
+ * The paper gives no algorithm beyond one sentence on RQI; the GPU method reaches the
+ * plain result "real ascending lambda, unitary X with A X = X diag(lambda)" by a faster route, so the
+ * oracle is that definition computed by the textbook method BASELINE.json fixes: cyclic Jacobi on MPFR
+ * (followed here in that order and notation).
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may call this.
+ * It shares no code with paper_2402_11868_b200/ (the CUDA path) and does not include include/zkd.h:
+ * the number layout is restated below from DESIGN.md section "API number layout".
+ *
+ * API real number (little-endian, 16 + prec/8 bytes; 112 bytes at 768 bit):
+ *   int32 sign (-1, 0, +1); int32 flags (must be 0); int64 exp; uint64 limb[prec/64] (little-endian limbs)
+ *   value = sign * (sum_k limb[k] 2^(64k)) * 2^(exp - prec); nonzero => top bit of limb[L-1] set
+ *   (mantissa in [1/2,1), the MPFR convention); zero => all fields zero.
+ * Complex = (re, im) consecutive.  Matrices row-major A[i][j]; eigvecs[i][j] = component i of vector j.
+ *
+ * Pins (tests/test_oracle_pins.py, -m "not gpu"): 2x2 closed form, Hermitian tridiagonal Toeplitz spectrum and
+ * vectors, Q diag(lambda) Q^H with chosen lambda, trace / Frobenius identities, characteristic-polynomial
+ * roots at N <= 4, the paper's epsilon = 2^-(n-1) example, degenerate cases, ordering and
+ * guard-precision independence.  All pin values are computed in the tests with mpmath, not with this file.
+ */
+#include "mpfr_abi.h"
+
+#include <math.h>
+#include <omp.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define RN MPFR_RNDN
+
+/* ------------------------------------------------------------------------------------------------ */
+/* number format                                                                                    */
+/* ------------------------------------------------------------------------------------------------ */
+
+static size_t api_real_bytes(int prec) { return 16 + (size_t)prec / 8; }
+
+/* returns 0 ok, 3 malformed.  tmp must have precision exactly prec (a multiple of 64). */
+static int api_get(mpfr_ptr dst, const uint8_t *src, int prec, mpfr_ptr tmp) {
+  int32_t sign, flags;
+  int64_t e;
+  int L = prec / 64;
+  memcpy(&sign, src, 4);
+  memcpy(&flags, src + 4, 4);
+  memcpy(&e, src + 8, 8);
+  if (flags != 0 || sign < -1 || sign > 1) return 3;
+  if (sign == 0) {
+    mpfr_set_zero(dst, +1);
+    return 0;
+  }
+  uint64_t top;
+  memcpy(&top, src + 16 + 8 * (size_t)(L - 1), 8);
+  if (!(top >> 63)) return 3;
+  memcpy(tmp->_mpfr_d, src + 16, 8 * (size_t)L);
+  tmp->_mpfr_sign = sign;
+  tmp->_mpfr_exp = (mpfr_exp_t)e;
+  mpfr_set(dst, tmp, RN); /* exact when prec(dst) >= prec */
+  return 0;
+}
+
+/* rounds src to prec bits (RNDN) and writes the API layout. */
+static void api_put(uint8_t *dst, mpfr_srcptr src, int prec, mpfr_ptr tmp) {
+  int L = prec / 64;
+  memset(dst, 0, api_real_bytes(prec));
+  mpfr_set(tmp, src, RN);
+  if (mpfr_zero_p(tmp)) return;
+  int32_t sign = mpfr_sgn(tmp) < 0 ? -1 : 1;
+  int64_t e = (int64_t)mpfr_get_exp(tmp);
+  memcpy(dst, &sign, 4);
+  memcpy(dst + 8, &e, 8);
+  memcpy(dst + 16, tmp->_mpfr_d, 8 * (size_t)L);
+}
+
+/* ------------------------------------------------------------------------------------------------ */
+/* small helpers on arrays of mpfr                                                                  */
+/* ------------------------------------------------------------------------------------------------ */
+
+static __mpfr_struct *vec_alloc(size_t n, long prec) {
+  __mpfr_struct *v = (__mpfr_struct *)malloc(n * sizeof(__mpfr_struct));
+  for (size_t i = 0; i < n; ++i) {
+    mpfr_init2(&v[i], prec);
+    mpfr_set_zero(&v[i], +1);
+  }
+  return v;
+}
+static void vec_free(__mpfr_struct *v, size_t n) {
+  for (size_t i = 0; i < n; ++i) mpfr_clear(&v[i]);
+  free(v);
+}
+
+/* complex matrix: re and im planes, row-major */
+typedef struct {
+  int n;
+  __mpfr_struct *re, *im;
+} cmat;
+static cmat cmat_alloc(int n, long prec) {
+  cmat m;
+  m.n = n;
+  m.re = vec_alloc((size_t)n * n, prec);
+  m.im = vec_alloc((size_t)n * n, prec);
+  return m;
+}
+static void cmat_free(cmat *m) {
+  vec_free(m->re, (size_t)m->n * m->n);
+  vec_free(m->im, (size_t)m->n * m->n);
+}
+#define RE(m, i, j) (&(m).re[(size_t)(i) * (m).n + (j)])
+#define IM(m, i, j) (&(m).im[(size_t)(i) * (m).n + (j)])
+
+/* ------------------------------------------------------------------------------------------------ */
+/* one Jacobi rotation                                                       */
+/* ------------------------------------------------------------------------------------------------ */
+
+typedef struct {
+  mpfr_t c, sr, si; /* c real, sigma = sr + i si */
+  mpfr_t absb, zeta, t, w1, w2, w3, w4;
+  mpfr_t npr, npi, nqr, nqi; /* new values */
+  int active;
+} rot_t;
+
+static void rot_init(rot_t *r, long prec) {
+  mpfr_init2(r->c, prec); mpfr_init2(r->sr, prec); mpfr_init2(r->si, prec);
+  mpfr_init2(r->absb, prec); mpfr_init2(r->zeta, prec); mpfr_init2(r->t, prec);
+  mpfr_init2(r->w1, prec); mpfr_init2(r->w2, prec); mpfr_init2(r->w3, prec); mpfr_init2(r->w4, prec);
+  mpfr_init2(r->npr, prec); mpfr_init2(r->npi, prec); mpfr_init2(r->nqr, prec); mpfr_init2(r->nqi, prec);
+  r->active = 0;
+}
+static void rot_clear(rot_t *r) {
+  mpfr_clear(r->c); mpfr_clear(r->sr); mpfr_clear(r->si);
+  mpfr_clear(r->absb); mpfr_clear(r->zeta); mpfr_clear(r->t);
+  mpfr_clear(r->w1); mpfr_clear(r->w2); mpfr_clear(r->w3); mpfr_clear(r->w4);
+  mpfr_clear(r->npr); mpfr_clear(r->npi); mpfr_clear(r->nqr); mpfr_clear(r->nqi);
+}
+
+/* beta = a_pq, alpha = a_pp, gamma = a_qq.  Skip if |beta| <= thr.
+ * zeta = (gamma - alpha) / (2|beta|);  t = sgn(zeta) / (|zeta| + sqrt(1 + zeta^2)), sgn(0) = +1;
+ * c = 1/sqrt(1 + t^2);  s = t c;  sigma = s beta / |beta|. */
+static void rot_params(rot_t *r, const cmat *A, int p, int q, mpfr_srcptr thr) {
+  mpfr_srcptr br = RE(*A, p, q), bi = IM(*A, p, q);
+  mpfr_sqr(r->w1, br, RN);
+  mpfr_sqr(r->w2, bi, RN);
+  mpfr_add(r->w1, r->w1, r->w2, RN);
+  mpfr_sqrt(r->absb, r->w1, RN); /* |beta| */
+  if (mpfr_cmp(r->absb, thr) <= 0) {
+    r->active = 0;
+    return;
+  }
+  r->active = 1;
+  mpfr_sub(r->w1, RE(*A, q, q), RE(*A, p, p), RN); /* gamma - alpha */
+  mpfr_mul_2si(r->w2, r->absb, 1, RN);              /* 2|beta| */
+  mpfr_div(r->zeta, r->w1, r->w2, RN);
+  int neg = mpfr_sgn(r->zeta) < 0;
+  mpfr_sqr(r->w1, r->zeta, RN);
+  mpfr_add_ui(r->w1, r->w1, 1, RN);
+  mpfr_sqrt(r->w1, r->w1, RN); /* sqrt(1+zeta^2) */
+  mpfr_abs(r->w2, r->zeta, RN);
+  mpfr_add(r->w1, r->w1, r->w2, RN);
+  mpfr_ui_div(r->t, 1, r->w1, RN);
+  if (neg) mpfr_neg(r->t, r->t, RN);
+  mpfr_sqr(r->w1, r->t, RN);
+  mpfr_add_ui(r->w1, r->w1, 1, RN);
+  mpfr_sqrt(r->w1, r->w1, RN);
+  mpfr_ui_div(r->c, 1, r->w1, RN);    /* c = 1/sqrt(1+t^2) */
+  mpfr_mul(r->w2, r->t, r->c, RN);    /* s = t c */
+  mpfr_div(r->w2, r->w2, r->absb, RN);/* s/|beta| */
+  mpfr_mul(r->sr, r->w2, br, RN);
+  mpfr_mul(r->si, r->w2, bi, RN);
+}
+
+/* (x_p, x_q) <- (c x_p - conj(sg) x_q, sg x_p + c x_q), with sg = sr + i*sgn_i*si.
+ * sgn_i = +1: column form (A J, V J);  sgn_i = -1: row form (J^H A), i.e. sigma -> conj(sigma). */
+static void rot_apply(rot_t *r, mpfr_ptr pr, mpfr_ptr pi, mpfr_ptr qr, mpfr_ptr qi, int sgn_i) {
+  /* conj(sg) x_q = (sr qr + s' qi) + i (sr qi - s' qr),  s' = sgn_i * si */
+  /* sg x_p       = (sr pr - s' pi) + i (sr pi + s' pr) */
+  if (sgn_i > 0) {
+    mpfr_fmma(r->w1, r->sr, qr, r->si, qi, RN); /* Re conj(sg) x_q */
+    mpfr_fmms(r->w2, r->sr, qi, r->si, qr, RN); /* Im conj(sg) x_q */
+    mpfr_fmms(r->w3, r->sr, pr, r->si, pi, RN); /* Re sg x_p */
+    mpfr_fmma(r->w4, r->sr, pi, r->si, pr, RN); /* Im sg x_p */
+  } else {
+    mpfr_fmms(r->w1, r->sr, qr, r->si, qi, RN);
+    mpfr_fmma(r->w2, r->sr, qi, r->si, qr, RN);
+    mpfr_fmma(r->w3, r->sr, pr, r->si, pi, RN);
+    mpfr_fmms(r->w4, r->sr, pi, r->si, pr, RN);
+  }
+  mpfr_fms(r->npr, r->c, pr, r->w1, RN); /* c pr - w1 */
+  mpfr_fms(r->npi, r->c, pi, r->w2, RN);
+  mpfr_fma(r->nqr, r->c, qr, r->w3, RN); /* c qr + w3 */
+  mpfr_fma(r->nqi, r->c, qi, r->w4, RN);
+  mpfr_swap(pr, r->npr);
+  mpfr_swap(pi, r->npi);
+  mpfr_swap(qr, r->nqr);
+  mpfr_swap(qi, r->nqi);
+}
+
+static void rot_columns(rot_t *r, cmat *A, cmat *V, int p, int q) {
+  int n = A->n;
+  for (int k = 0; k < n; ++k) rot_apply(r, RE(*A, k, p), IM(*A, k, p), RE(*A, k, q), IM(*A, k, q), +1);
+  for (int k = 0; k < n; ++k) rot_apply(r, RE(*V, k, p), IM(*V, k, p), RE(*V, k, q), IM(*V, k, q), +1);
+}
+static void rot_rows(rot_t *r, cmat *A, int p, int q) {
+  int n = A->n;
+  for (int k = 0; k < n; ++k) rot_apply(r, RE(*A, p, k), IM(*A, p, k), RE(*A, q, k), IM(*A, q, k), -1);
+  mpfr_set_zero(RE(*A, p, q), +1); mpfr_set_zero(IM(*A, p, q), +1);
+  mpfr_set_zero(RE(*A, q, p), +1); mpfr_set_zero(IM(*A, q, p), +1);
+  mpfr_set_zero(IM(*A, p, p), +1); mpfr_set_zero(IM(*A, q, q), +1);
+}
+
+/* off(A)^2 = sum_{i != j} |a_ij|^2 */
+static void off_norm2(mpfr_ptr out, const cmat *A, mpfr_ptr w) {
+  int n = A->n;
+  mpfr_set_zero(out, +1);
+  for (int i = 0; i < n; ++i)
+    for (int j = 0; j < n; ++j) {
+      if (i == j) continue;
+      mpfr_sqr(w, RE(*A, i, j), RN); mpfr_add(out, out, w, RN);
+      mpfr_sqr(w, IM(*A, i, j), RN); mpfr_add(out, out, w, RN);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------------ */
+/* the oracle                                                                                       */
+/* ------------------------------------------------------------------------------------------------ */
+
+/* Cyclic Jacobi eigendecomposition of one Hermitian matrix.
+ *   ordering 0 = row-cyclic, serial;  1 = round-robin (tournament), OpenMP over the disjoint pairs of a round.
+ *   guard_bits: working precision P_o = prec + guard_bits (128 is the documented default, reading A6).
+ *   max_rotations > 0: stop after that many rotations (bench sampling hook; result then NOT converged).
+ *   info[0] = sweeps, info[1] = rotations applied, info[2] = status (0 ok, 2 not converged, 3 malformed input)
+ * Returns info[2]. */
+int zkd_oracle_diag_herm(int N, int prec, int guard_bits, int ordering, int nthreads, long max_rotations,
+                         const uint8_t *A_api, uint8_t *eigvals_api, uint8_t *eigvecs_api, long *info) {
+  const long Po = (long)prec + guard_bits;
+  const size_t rb = api_real_bytes(prec);
+  long sweeps = 0, rotations = 0;
+  int status = 0;
+  if (nthreads < 1) nthreads = 1;
+  if (info) info[0] = info[1] = info[2] = 0;
+  if (N < 1 || prec < 64 || prec % 64) { if (info) info[2] = 3; return 3; }
+
+  mpfr_t tmpP, F, thr, offtol, w, off2;
+  mpfr_init2(tmpP, prec); mpfr_init2(F, Po); mpfr_init2(thr, Po); mpfr_init2(offtol, Po);
+  mpfr_init2(w, Po); mpfr_init2(off2, Po);
+  cmat A = cmat_alloc(N, Po), V = cmat_alloc(N, Po);
+
+  /* step 1: copy A, upper triangle authoritative, a_ji = conj(a_ij), Im a_ii = 0; V = I; F = ||A||_F */
+  for (int i = 0; i < N && !status; ++i)
+    for (int j = i; j < N; ++j) {
+      const uint8_t *src = A_api + ((size_t)i * N + j) * 2 * rb;
+      if (api_get(RE(A, i, j), src, prec, tmpP) || api_get(IM(A, i, j), src + rb, prec, tmpP)) { status = 3; break; }
+      if (i == j) mpfr_set_zero(IM(A, i, j), +1);
+      else { mpfr_set(RE(A, j, i), RE(A, i, j), RN); mpfr_neg(IM(A, j, i), IM(A, i, j), RN); }
+    }
+  if (status) goto done;
+  for (int i = 0; i < N; ++i) mpfr_set_ui(RE(V, i, i), 1, RN);
+  mpfr_set_zero(F, +1);
+  for (int i = 0; i < N; ++i)
+    for (int j = 0; j < N; ++j) {
+      mpfr_sqr(w, RE(A, i, j), RN); mpfr_add(F, F, w, RN);
+      mpfr_sqr(w, IM(A, i, j), RN); mpfr_add(F, F, w, RN);
+    }
+  mpfr_sqrt(F, F, RN);
+  /* rotation skip threshold 2^-(Po+16) F / N; convergence off(A) <= 2^-(prec+64) F */
+  mpfr_div_2si(thr, F, Po + 16, RN); mpfr_div_ui(thr, thr, (unsigned long)N, RN);
+  mpfr_div_2si(offtol, F, prec + 64, RN);
+
+  {
+    int nt = ordering == 1 ? nthreads : 1;
+    int M = N + (N & 1); /* round-robin players (one dummy if N odd) */
+    rot_t *rots = (rot_t *)malloc(sizeof(rot_t) * (size_t)(M / 2 > 0 ? M / 2 : 1));
+    for (int i = 0; i < (M / 2 > 0 ? M / 2 : 1); ++i) rot_init(&rots[i], Po);
+    int *perm = (int *)malloc(sizeof(int) * (size_t)(M > 0 ? M : 1));
+    int *pp = (int *)malloc(sizeof(int) * (size_t)(M / 2 + 1)), *qq = (int *)malloc(sizeof(int) * (size_t)(M / 2 + 1));
+
+    /* step 2: sweeps until off(A) <= 2^-(P+64) F, or a sweep skipped every rotation; fail after 80 */
+    for (;;) {
+      off_norm2(off2, &A, w);
+      mpfr_sqrt(off2, off2, RN);
+      if (mpfr_cmp(off2, offtol) <= 0) break;
+      if (sweeps >= 80) { status = 2; break; }
+      if (max_rotations > 0 && rotations >= max_rotations) { status = 2; break; }
+      long applied = 0;
+      if (ordering == 0) {
+        /* step 3: row-cyclic sweep */
+        for (int p = 0; p < N - 1; ++p)
+          for (int q = p + 1; q < N; ++q) {
+            if (max_rotations > 0 && rotations + applied >= max_rotations) continue;
+            rot_params(&rots[0], &A, p, q, thr);
+            if (!rots[0].active) continue;
+            rot_columns(&rots[0], &A, &V, p, q);
+            rot_rows(&rots[0], &A, p, q);
+            ++applied;
+          }
+      } else {
+        /* step 5: round-robin ordering, M-1 rounds of M/2 disjoint pairs; column phase then row phase */
+        for (int i = 0; i < M; ++i) perm[i] = i;
+        for (int round = 0; round < M - 1; ++round) {
+          if (max_rotations > 0 && rotations + applied >= max_rotations) break;
+          int np = 0;
+          for (int i = 0; i < M / 2; ++i) {
+            int a = perm[i], b = perm[M - 1 - i];
+            if (a >= N || b >= N) continue;
+            pp[np] = a < b ? a : b; qq[np] = a < b ? b : a; ++np;
+          }
+#pragma omp parallel for num_threads(nt) schedule(dynamic, 1)
+          for (int i = 0; i < np; ++i) rot_params(&rots[i], &A, pp[i], qq[i], thr);
+#pragma omp parallel for num_threads(nt) schedule(dynamic, 1)
+          for (int i = 0; i < np; ++i) if (rots[i].active) rot_columns(&rots[i], &A, &V, pp[i], qq[i]);
+#pragma omp parallel for num_threads(nt) schedule(dynamic, 1)
+          for (int i = 0; i < np; ++i) if (rots[i].active) rot_rows(&rots[i], &A, pp[i], qq[i]);
+          for (int i = 0; i < np; ++i) applied += rots[i].active;
+          /* rotate players 1..M-1, player 0 fixed */
+          int last = perm[M - 1];
+          for (int i = M - 1; i > 1; --i) perm[i] = perm[i - 1];
+          if (M > 1) perm[1] = last;
+        }
+      }
+      rotations += applied;
+      ++sweeps;
+      if (applied == 0) break;
+    }
+    for (int i = 0; i < (M / 2 > 0 ? M / 2 : 1); ++i) rot_clear(&rots[i]);
+    free(rots); free(perm); free(pp); free(qq);
+  }
+
+  /* step 4: lambda_j = Re a_jj; stable ascending sort; permute V; renormalise; phase-normalise (A9); round */
+  {
+    int *ord = (int *)malloc(sizeof(int) * (size_t)N);
+    for (int i = 0; i < N; ++i) ord[i] = i;
+    for (int i = 1; i < N; ++i) { /* insertion sort: stable */
+      int k = ord[i], j = i - 1;
+      while (j >= 0 && mpfr_cmp(RE(A, ord[j], ord[j]), RE(A, k, k)) > 0) { ord[j + 1] = ord[j]; --j; }
+      ord[j + 1] = k;
+    }
+    mpfr_t nrm, best, m2, ur, ui, xr, xi;
+    mpfr_init2(nrm, Po); mpfr_init2(best, Po); mpfr_init2(m2, Po);
+    mpfr_init2(ur, Po); mpfr_init2(ui, Po); mpfr_init2(xr, Po); mpfr_init2(xi, Po);
+    for (int jj = 0; jj < N; ++jj) {
+      int j = ord[jj];
+      if (eigvals_api) api_put(eigvals_api + (size_t)jj * rb, RE(A, j, j), prec, tmpP);
+      if (!eigvecs_api) continue;
+      /* unit 2-norm */
+      mpfr_set_zero(nrm, +1);
+      int kstar = 0;
+      mpfr_set_si(best, -1, RN);
+      for (int k = 0; k < N; ++k) {
+        mpfr_sqr(m2, RE(V, k, j), RN); mpfr_sqr(w, IM(V, k, j), RN); mpfr_add(m2, m2, w, RN);
+        mpfr_add(nrm, nrm, m2, RN);
+        if (mpfr_cmp(m2, best) > 0) { mpfr_set(best, m2, RN); kstar = k; } /* first index attaining the max */
+      }
+      mpfr_sqrt(nrm, nrm, RN);
+      /* phase: multiply by conj(x_k*) / |x_k*|, and divide by the norm */
+      mpfr_sqrt(best, best, RN);
+      mpfr_mul(w, best, nrm, RN);
+      mpfr_div(ur, RE(V, kstar, j), w, RN);
+      mpfr_div(ui, IM(V, kstar, j), w, RN);
+      mpfr_neg(ui, ui, RN); /* u = conj(x_k*) / (|x_k*| ||x||) */
+      for (int k = 0; k < N; ++k) {
+        mpfr_fmms(xr, RE(V, k, j), ur, IM(V, k, j), ui, RN);
+        mpfr_fmma(xi, RE(V, k, j), ui, IM(V, k, j), ur, RN);
+        if (k == kstar) mpfr_set_zero(xi, +1);
+        uint8_t *dst = eigvecs_api + ((size_t)k * N + jj) * 2 * rb;
+        api_put(dst, xr, prec, tmpP);
+        api_put(dst + rb, xi, prec, tmpP);
+      }
+    }
+    mpfr_clear(nrm); mpfr_clear(best); mpfr_clear(m2);
+    mpfr_clear(ur); mpfr_clear(ui); mpfr_clear(xr); mpfr_clear(xi);
+    free(ord);
+  }
+
+done:
+  cmat_free(&A); cmat_free(&V);
+  mpfr_clear(tmpP); mpfr_clear(F); mpfr_clear(thr); mpfr_clear(offtol); mpfr_clear(w); mpfr_clear(off2);
+  if (info) { info[0] = sweeps; info[1] = rotations; info[2] = status; }
+  return status;
+}
+
+/* ------------------------------------------------------------------------------------------------ */
+/* comparator (SURVEY.md 8(c) "Comparator"; well-conditioned difference formulas only)               */
+/* ------------------------------------------------------------------------------------------------ */
+
+static void load_cmat(cmat *M, const uint8_t *api, int n, int prec, mpfr_ptr tmpP, int herm_upper) {
+  size_t rb = api_real_bytes(prec);
+  for (int i = 0; i < n; ++i)
+    for (int j = 0; j < n; ++j) {
+      const uint8_t *src = api + ((size_t)i * n + j) * 2 * rb;
+      api_get(RE(*M, i, j), src, prec, tmpP);
+      api_get(IM(*M, i, j), src + rb, prec, tmpP);
+    }
+  if (herm_upper)
+    for (int i = 0; i < n; ++i) {
+      mpfr_set_zero(IM(*M, i, i), +1);
+      for (int j = i + 1; j < n; ++j) { mpfr_set(RE(*M, j, i), RE(*M, i, j), RN); mpfr_neg(IM(*M, j, i), IM(*M, i, j), RN); }
+    }
+}
+
+static double log2_mpfr(mpfr_srcptr x) {
+  if (mpfr_zero_p(x)) return -1.0e9;
+  long e;
+  double m = mpfr_get_d_2exp(&e, x, RN);
+  return log2(fabs(m)) + (double)e;
+}
+
+/* Compare a candidate decomposition (lam, X) of A against invariants and (optionally) a reference (lam0, X0).
+ *  cols/ncols: columns on which residual and orthogonality are evaluated (NULL => all N).
+ *  lam0, X0 may be NULL (then (i)/(iv) are skipped).
+ *  out[0] = log2 max_j |lam_j - lam0_j| / F                          (i)
+ *  out[1] = log2 max_{j in cols} ||A x_j - lam_j x_j||_2 / F         (ii)
+ *  out[2] = log2 max_{j in cols, all i} |x_i^H x_j - delta_ij|       (iii)
+ *  out[3] = max over groups of  log2 ||E_G||_F - log2 (2^-730 F / gap_G)   (iv)  (<= 0 passes)
+ *  out[4] = log2 F;  out[5] = number of groups;  out[6] = largest group;  out[7] = log2 of worst ||E_G||_F
+ * Groups (reading A10): reference eigenvalues sorted ascending; a new group starts where the gap exceeds
+ * 2^-666 F.  gap_G = distance from the group's extreme members to the nearest eigenvalue outside.
+ * E_G = X_G - X0_G (X0_G^H X_G)  (= ||sin Theta||_F; for |G| = 1 the phase-aligned difference). */
+int zkd_oracle_compare(int N, int prec, int nthreads, const uint8_t *A_api, const uint8_t *lam_api,
+                       const uint8_t *X_api, const uint8_t *lam0_api, const uint8_t *X0_api, const int *cols,
+                       int ncols, double *out) {
+  const long Pc = (long)prec + 256;
+  const size_t rb = api_real_bytes(prec);
+  if (nthreads < 1) nthreads = 1;
+  mpfr_t tmpP, F, w, acc;
+  mpfr_init2(tmpP, prec); mpfr_init2(F, Pc); mpfr_init2(w, Pc); mpfr_init2(acc, Pc);
+  cmat A = cmat_alloc(N, Pc), X = cmat_alloc(N, Pc);
+  load_cmat(&A, A_api, N, prec, tmpP, 1);
+  load_cmat(&X, X_api, N, prec, tmpP, 0);
+  __mpfr_struct *lam = vec_alloc((size_t)N, Pc);
+  for (int j = 0; j < N; ++j) api_get(&lam[j], lam_api + (size_t)j * rb, prec, tmpP);
+  mpfr_set_zero(F, +1);
+  for (int i = 0; i < N; ++i)
+    for (int j = 0; j < N; ++j) {
+      mpfr_sqr(w, RE(A, i, j), RN); mpfr_add(F, F, w, RN);
+      mpfr_sqr(w, IM(A, i, j), RN); mpfr_add(F, F, w, RN);
+    }
+  mpfr_sqrt(F, F, RN);
+  double lF = log2_mpfr(F);
+  for (int i = 0; i < 8; ++i) out[i] = -1.0e9;
+  out[4] = lF;
+  int nc = cols ? ncols : N;
+
+  /* (ii) residuals and (iii) orthogonality on the chosen columns */
+  double *res = (double *)malloc(sizeof(double) * (size_t)nc), *orth = (double *)malloc(sizeof(double) * (size_t)nc);
+#pragma omp parallel num_threads(nthreads)
+  {
+    mpfr_t sr, si, t1, t2, r2, d;
+    mpfr_init2(sr, Pc); mpfr_init2(si, Pc); mpfr_init2(t1, Pc); mpfr_init2(t2, Pc); mpfr_init2(r2, Pc); mpfr_init2(d, Pc);
+#pragma omp for schedule(dynamic, 1)
+    for (int c = 0; c < nc; ++c) {
+      int j = cols ? cols[c] : c;
+      mpfr_set_zero(r2, +1);
+      for (int i = 0; i < N; ++i) {
+        mpfr_set_zero(sr, +1); mpfr_set_zero(si, +1);
+        for (int k = 0; k < N; ++k) { /* (A x_j)_i */
+          mpfr_fmms(t1, RE(A, i, k), RE(X, k, j), IM(A, i, k), IM(X, k, j), RN);
+          mpfr_fmma(t2, RE(A, i, k), IM(X, k, j), IM(A, i, k), RE(X, k, j), RN);
+          mpfr_add(sr, sr, t1, RN); mpfr_add(si, si, t2, RN);
+        }
+        mpfr_mul(t1, &lam[j], RE(X, i, j), RN); mpfr_sub(sr, sr, t1, RN);
+        mpfr_mul(t2, &lam[j], IM(X, i, j), RN); mpfr_sub(si, si, t2, RN);
+        mpfr_sqr(t1, sr, RN); mpfr_sqr(t2, si, RN);
+        mpfr_add(r2, r2, t1, RN); mpfr_add(r2, r2, t2, RN);
+      }
+      mpfr_sqrt(r2, r2, RN);
+      res[c] = log2_mpfr(r2) - lF;
+      double worst = -1.0e9;
+      for (int i = 0; i < N; ++i) { /* x_i^H x_j */
+        mpfr_set_zero(sr, +1); mpfr_set_zero(si, +1);
+        for (int k = 0; k < N; ++k) {
+          mpfr_fmma(t1, RE(X, k, i), RE(X, k, j), IM(X, k, i), IM(X, k, j), RN);
+          mpfr_fmms(t2, RE(X, k, i), IM(X, k, j), IM(X, k, i), RE(X, k, j), RN);
+          mpfr_add(sr, sr, t1, RN); mpfr_add(si, si, t2, RN);
+        }
+        if (i == j) mpfr_sub_ui(sr, sr, 1, RN);
+        mpfr_sqr(t1, sr, RN); mpfr_sqr(t2, si, RN); mpfr_add(d, t1, t2, RN); mpfr_sqrt(d, d, RN);
+        double l = log2_mpfr(d);
+        if (l > worst) worst = l;
+      }
+      orth[c] = worst;
+    }
+    mpfr_clear(sr); mpfr_clear(si); mpfr_clear(t1); mpfr_clear(t2); mpfr_clear(r2); mpfr_clear(d);
+  }
+  for (int c = 0; c < nc; ++c) { if (res[c] > out[1]) out[1] = res[c]; if (orth[c] > out[2]) out[2] = orth[c]; }
+  free(res); free(orth);
+
+  if (lam0_api) {
+    __mpfr_struct *lam0 = vec_alloc((size_t)N, Pc);
+    for (int j = 0; j < N; ++j) api_get(&lam0[j], lam0_api + (size_t)j * rb, prec, tmpP);
+    /* (i) */
+    for (int j = 0; j < N; ++j) {
+      mpfr_sub(w, &lam[j], &lam0[j], RN);
+      double l = log2_mpfr(w) - lF;
+      if (l > out[0]) out[0] = l;
+    }
+    if (X0_api) {
+      /* (iv) groups on the reference spectrum */
+      cmat X0 = cmat_alloc(N, Pc);
+      load_cmat(&X0, X0_api, N, prec, tmpP, 0);
+      mpfr_t gthr, gap, g2;
+      mpfr_init2(gthr, Pc); mpfr_init2(gap, Pc); mpfr_init2(g2, Pc);
+      mpfr_div_2si(gthr, F, 666, RN);
+      int *gstart = (int *)malloc(sizeof(int) * (size_t)(N + 1));
+      int ng = 0;
+      gstart[ng++] = 0;
+      for (int j = 0; j + 1 < N; ++j) {
+        mpfr_sub(w, &lam0[j + 1], &lam0[j], RN);
+        if (mpfr_cmp(w, gthr) > 0) gstart[ng++] = j + 1;
+      }
+      gstart[ng] = N;
+      out[5] = ng;
+      double *margin = (double *)malloc(sizeof(double) * (size_t)ng), *eabs = (double *)malloc(sizeof(double) * (size_t)ng);
+      int maxg = 0;
+      for (int g = 0; g < ng; ++g) if (gstart[g + 1] - gstart[g] > maxg) maxg = gstart[g + 1] - gstart[g];
+      out[6] = maxg;
+#pragma omp parallel num_threads(nthreads)
+      {
+        mpfr_t sr, si, t1, t2, e2, gp, g3;
+        mpfr_init2(sr, Pc); mpfr_init2(si, Pc); mpfr_init2(t1, Pc); mpfr_init2(t2, Pc); mpfr_init2(e2, Pc);
+        mpfr_init2(gp, Pc); mpfr_init2(g3, Pc);
+#pragma omp for schedule(dynamic, 1)
+        for (int g = 0; g < ng; ++g) {
+          int a = gstart[g], b = gstart[g + 1], m = b - a;
+          /* gap to the nearest eigenvalue outside */
+          int have = 0;
+          if (a > 0) { mpfr_sub(gp, &lam0[a], &lam0[a - 1], RN); have = 1; }
+          if (b < N) {
+            mpfr_sub(g3, &lam0[b], &lam0[b - 1], RN);
+            if (!have || mpfr_cmp(g3, gp) < 0) mpfr_set(gp, g3, RN);
+            have = 1;
+          }
+          /* M = X0_G^H X_G (m x m), E = X_G - X0_G M */
+          cmat Mm = cmat_alloc(m, Pc);
+          for (int p = 0; p < m; ++p)
+            for (int q = 0; q < m; ++q) {
+              mpfr_set_zero(sr, +1); mpfr_set_zero(si, +1);
+              for (int k = 0; k < N; ++k) {
+                mpfr_fmma(t1, RE(X0, k, a + p), RE(X, k, a + q), IM(X0, k, a + p), IM(X, k, a + q), RN);
+                mpfr_fmms(t2, RE(X0, k, a + p), IM(X, k, a + q), IM(X0, k, a + p), RE(X, k, a + q), RN);
+                mpfr_add(sr, sr, t1, RN); mpfr_add(si, si, t2, RN);
+              }
+              mpfr_set(RE(Mm, p, q), sr, RN); mpfr_set(IM(Mm, p, q), si, RN);
+            }
+          mpfr_set_zero(e2, +1);
+          for (int k = 0; k < N; ++k)
+            for (int q = 0; q < m; ++q) {
+              mpfr_set(sr, RE(X, k, a + q), RN); mpfr_set(si, IM(X, k, a + q), RN);
+              for (int p = 0; p < m; ++p) {
+                mpfr_fmms(t1, RE(X0, k, a + p), RE(Mm, p, q), IM(X0, k, a + p), IM(Mm, p, q), RN);
+                mpfr_fmma(t2, RE(X0, k, a + p), IM(Mm, p, q), IM(X0, k, a + p), RE(Mm, p, q), RN);
+                mpfr_sub(sr, sr, t1, RN); mpfr_sub(si, si, t2, RN);
+              }
+              mpfr_sqr(t1, sr, RN); mpfr_sqr(t2, si, RN);
+              mpfr_add(e2, e2, t1, RN); mpfr_add(e2, e2, t2, RN);
+            }
+          mpfr_sqrt(e2, e2, RN);
+          eabs[g] = log2_mpfr(e2);
+          double ltol = have ? (-730.0 + lF - log2_mpfr(gp)) : 1.0e9; /* single group spanning everything: any basis */
+          margin[g] = eabs[g] - ltol;
+          cmat_free(&Mm);
+        }
+        mpfr_clear(sr); mpfr_clear(si); mpfr_clear(t1); mpfr_clear(t2); mpfr_clear(e2); mpfr_clear(gp); mpfr_clear(g3);
+      }
+      for (int g = 0; g < ng; ++g) { if (margin[g] > out[3]) out[3] = margin[g]; if (eabs[g] > out[7]) out[7] = eabs[g]; }
+      free(margin); free(eabs); free(gstart);
+      mpfr_clear(gthr); mpfr_clear(gap); mpfr_clear(g2);
+      cmat_free(&X0);
+    }
+    vec_free(lam0, (size_t)N);
+  }
+  vec_free(lam, (size_t)N);
+  cmat_free(&A); cmat_free(&X);
+  mpfr_clear(tmpP); mpfr_clear(F); mpfr_clear(w); mpfr_clear(acc);
+  return 0;
+}
+
+/* number-format round trip helpers used by the tests */
+double zkd_oracle_api_to_double(const uint8_t *src, int prec) {
+  mpfr_t t, d;
+  mpfr_init2(t, prec); mpfr_init2(d, prec);
+  double r = NAN;
+  if (api_get(d, src, prec, t) == 0) r = mpfr_get_d(d, RN);
+  mpfr_clear(t); mpfr_clear(d);
+  return r;
+}
+void zkd_oracle_api_from_double(uint8_t *dst, int prec, double v) {
+  mpfr_t t, d;
+  mpfr_init2(t, prec); mpfr_init2(d, prec);
+  mpfr_set_d(d, v, RN);
+  api_put(dst, d, prec, t);
+  mpfr_clear(t); mpfr_clear(d);
+}
+const char *zkd_oracle_mpfr_version(void) { return mpfr_get_version(); }
+int zkd_oracle_max_threads(void) { return omp_get_max_threads(); }
