@@ -1,0 +1,215 @@
+"""paper_2402_11868_b200 — thin ctypes binding of libzkd (include/zkd.h).
+
+Argument marshalling only: every step of the hot path (S0 ingest .. S6 export) runs in the
+CUDA kernels of libzkd.so.  torch is used for device memory and streams, nothing else.  There is no CPU fallback:
+if libzkd.so is missing or fails to load, importing a function from here raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+SO_PATH = os.path.join(_HERE, "libzkd.so")
+
+PREC = 768
+REAL_BYTES = 16 + PREC // 8  # 112
+FX_DIGITS = 30
+FX_FRAC_BITS = 812
+
+ZKD_OK = 0
+
+
+class ZkdError(RuntimeError):
+    def __init__(self, code: int, what: str):
+        super().__init__(f"{what}: {strerror(code)} ({code})")
+        self.code = code
+
+
+class zkd_info(ctypes.Structure):
+    _fields_ = [("status", ctypes.c_int32), ("steps", ctypes.c_int32), ("n_clusters", ctypes.c_int32),
+                ("max_cluster", ctypes.c_int32), ("log2_resid", ctypes.c_float), ("log2_orth", ctypes.c_float)]
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libzkd.so (built in-tree by paper_2402_11868_b200.build).  Fails loudly when it is absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(SO_PATH):
+        raise ImportError(f"{SO_PATH} not found: run `python -m paper_2402_11868_b200.build` (no CPU fallback exists)")
+    L = ctypes.CDLL(SO_PATH)
+    vp, ci, cs, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t, ctypes.c_double
+    L.zkd_real_bytes.restype = cs
+    L.zkd_real_bytes.argtypes = [ci]
+    L.zkd_diag_herm_bufsize.argtypes = [ci, ci, ci, ctypes.POINTER(cs)]
+    L.zkd_diag_herm_ws.argtypes = [ci, ci, ci, vp, vp, vp, vp, cs, vp, vp]
+    L.zkd_diag_herm.argtypes = [ci, ci, ci, vp, vp, vp, vp]
+    L.zkd_diag_herm_host.argtypes = [ci, ci, ci, vp, vp, vp, vp]
+    L.zkd_set_option.argtypes = [ctypes.c_char_p, cd]
+    L.zkd_get_option.argtypes = [ctypes.c_char_p, ctypes.POINTER(cd)]
+    L.zkd_strerror.restype = ctypes.c_char_p
+    L.zkd_strerror.argtypes = [ci]
+    L.zkd_version.restype = ci
+    L.zkd_counters.restype = None
+    L.zkd_counters.argtypes = [ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint64)]
+    L.zkd_counters_reset.restype = None
+    L.zkd_pack.argtypes = [vp, ci, ci, ctypes.c_int64, vp]
+    L.zkd_unpack.argtypes = [vp, ci, ctypes.POINTER(ci), ctypes.POINTER(ctypes.c_int64), vp]
+    L.zkd_from_double.argtypes = [vp, ci, cd]
+    L.zkd_to_double.restype = cd
+    L.zkd_to_double.argtypes = [vp, ci]
+    L.zkd_fx_from_api.argtypes = [ci, ci, vp, vp, ci, vp]
+    L.zkd_fx_to_api.argtypes = [ci, ci, vp, vp, ci, vp]
+    L.zkd_gemm_fx_bufsize.argtypes = [ci, ci, ci, ci, ctypes.POINTER(cs)]
+    L.zkd_gemm_fx.argtypes = [ci, ci, ci, ci, ci, vp, ci, ci, vp, ci, ci, vp, ci, ci, ci, vp, cs, vp, vp, vp]
+    L.zkd_seed_fp64.argtypes = [ci, ci, vp, vp, vp, vp]
+    L.zkd_measure_imad_peak.argtypes = [cd, ctypes.POINTER(cd), vp]
+    _lib = L
+    return L
+
+
+def strerror(code: int) -> str:
+    return lib().zkd_strerror(code).decode()
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != ZKD_OK:
+        raise ZkdError(rc, what)
+
+
+def _stream_ptr(stream) -> int:
+    import torch
+
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return int(s.cuda_stream)
+
+
+def _dev_u8(t, nbytes: int, name: str) -> int:
+    import torch
+
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous()):
+        raise TypeError(f"{name} must be a contiguous CUDA tensor")
+    if t.numel() * t.element_size() < nbytes:
+        raise ValueError(f"{name} holds {t.numel() * t.element_size()} bytes, {nbytes} needed")
+    return t.data_ptr()
+
+
+def real_bytes(prec_bits: int = PREC) -> int:
+    return int(lib().zkd_real_bytes(prec_bits))
+
+
+def version() -> int:
+    return int(lib().zkd_version())
+
+
+def set_option(key: str, value: float) -> None:
+    _check(lib().zkd_set_option(key.encode(), float(value)), f"zkd_set_option({key})")
+
+
+def get_option(key: str) -> float:
+    v = ctypes.c_double()
+    _check(lib().zkd_get_option(key.encode(), ctypes.byref(v)), f"zkd_get_option({key})")
+    return v.value
+
+
+def counters() -> tuple[int, int]:
+    a, b = ctypes.c_uint64(), ctypes.c_uint64()
+    lib().zkd_counters(ctypes.byref(a), ctypes.byref(b))
+    return int(a.value), int(b.value)
+
+
+def counters_reset() -> None:
+    lib().zkd_counters_reset()
+
+
+def diag_herm_bufsize(N: int, batch: int, prec_bits: int = PREC) -> int:
+    n = ctypes.c_size_t()
+    _check(lib().zkd_diag_herm_bufsize(N, batch, prec_bits, ctypes.byref(n)), "zkd_diag_herm_bufsize")
+    return int(n.value)
+
+
+def diag_herm_ws(N: int, batch: int, A, eigvals, eigvecs, workspace, info=None, prec_bits: int = PREC, stream=None) -> None:
+    """zkd_diag_herm_ws on device tensors (uint8, API layout).  `info`: optional uint8/int32 CUDA tensor of
+    batch * sizeof(zkd_info) bytes."""
+    rb = REAL_BYTES
+    a = _dev_u8(A, batch * N * N * 2 * rb, "A")
+    lam = _dev_u8(eigvals, batch * N * rb, "eigvals")
+    x = _dev_u8(eigvecs, batch * N * N * 2 * rb, "eigvecs")
+    need = diag_herm_bufsize(N, batch, prec_bits)
+    w = _dev_u8(workspace, need, "workspace")
+    i = _dev_u8(info, batch * ctypes.sizeof(zkd_info), "info") if info is not None else None
+    _check(lib().zkd_diag_herm_ws(N, batch, prec_bits, a, lam, x, w, workspace.numel() * workspace.element_size(), i,
+                                  _stream_ptr(stream)), "zkd_diag_herm_ws")
+
+
+def diag_herm(N: int, batch: int, A, eigvals, eigvecs, prec_bits: int = PREC, stream=None) -> None:
+    rb = REAL_BYTES
+    a = _dev_u8(A, batch * N * N * 2 * rb, "A")
+    lam = _dev_u8(eigvals, batch * N * rb, "eigvals")
+    x = _dev_u8(eigvecs, batch * N * N * 2 * rb, "eigvecs")
+    _check(lib().zkd_diag_herm(N, batch, prec_bits, a, lam, x, _stream_ptr(stream)), "zkd_diag_herm")
+
+
+def diag_herm_host(N: int, batch: int, A_host, eigvals_host, eigvecs_host, info_host=None, prec_bits: int = PREC) -> None:
+    """zkd_diag_herm_host on HOST buffers (numpy uint8 arrays or pinned CPU torch tensors), copies included."""
+    def ptr(x):
+        return x.ctypes.data if hasattr(x, "ctypes") else x.data_ptr()
+    ip = ctypes.addressof(info_host) if info_host is not None else None
+    _check(lib().zkd_diag_herm_host(N, batch, prec_bits, ptr(A_host), ptr(eigvals_host), ptr(eigvecs_host), ip),
+           "zkd_diag_herm_host")
+
+
+def read_info(info_tensor, batch: int) -> list[dict]:
+    raw = bytes(info_tensor.cpu().numpy().tobytes())
+    arr = (zkd_info * batch).from_buffer_copy(raw[: batch * ctypes.sizeof(zkd_info)])
+    return [{f: getattr(a, f) for f, _ in zkd_info._fields_} for a in arr]
+
+
+# ---- building blocks -------------------------------------------------------------------------------------------
+
+def fx_from_api(count: int, src_api, dst_fx, scale_bits: int = 0, stream=None) -> None:
+    _check(lib().zkd_fx_from_api(count, PREC, _dev_u8(src_api, count * REAL_BYTES, "src_api"),
+                                 _dev_u8(dst_fx, count * FX_DIGITS * 4, "dst_fx"), scale_bits, _stream_ptr(stream)),
+           "zkd_fx_from_api")
+
+
+def fx_to_api(count: int, src_fx, dst_api, scale_bits: int = 0, stream=None) -> None:
+    _check(lib().zkd_fx_to_api(count, PREC, _dev_u8(src_fx, count * FX_DIGITS * 4, "src_fx"),
+                               _dev_u8(dst_api, count * REAL_BYTES, "dst_api"), scale_bits, _stream_ptr(stream)),
+           "zkd_fx_to_api")
+
+
+def gemm_fx_bufsize(M: int, N: int, K: int, batch: int) -> int:
+    n = ctypes.c_size_t()
+    _check(lib().zkd_gemm_fx_bufsize(M, N, K, batch, ctypes.byref(n)), "zkd_gemm_fx_bufsize")
+    return int(n.value)
+
+
+def gemm_fx(M, N, K, batch, op_a, A_fx, a_top_bit, a_digits, B_fx, b_top_bit, b_digits, C_fx, mode=0, out_cut_bit=-1,
+            path=0, workspace=None, err_flag=None, msb_out=None, stream=None) -> None:
+    import torch
+
+    if workspace is None:
+        workspace = torch.empty(gemm_fx_bufsize(M, N, K, batch), dtype=torch.uint8, device=A_fx.device)
+    per = 2 * FX_DIGITS * 4
+    _check(lib().zkd_gemm_fx(M, N, K, batch, op_a, _dev_u8(A_fx, batch * M * K * per, "A_fx"), a_top_bit, a_digits,
+                             _dev_u8(B_fx, batch * K * N * per, "B_fx"), b_top_bit, b_digits,
+                             _dev_u8(C_fx, batch * M * N * per, "C_fx"), mode, out_cut_bit, path, workspace.data_ptr(),
+                             workspace.numel() * workspace.element_size(),
+                             err_flag.data_ptr() if err_flag is not None else None,
+                             msb_out.data_ptr() if msb_out is not None else None, _stream_ptr(stream)), "zkd_gemm_fx")
+
+
+def seed_fp64(N: int, batch: int, A64, mu, V, stream=None) -> None:
+    _check(lib().zkd_seed_fp64(N, batch, _dev_u8(A64, batch * N * N * 16, "A64"), _dev_u8(mu, batch * N * 8, "mu"),
+                               _dev_u8(V, batch * N * N * 16, "V"), _stream_ptr(stream)), "zkd_seed_fp64")
+
+
+def measure_imad_peak(millis: float = 50.0, stream=None) -> float:
+    v = ctypes.c_double()
+    _check(lib().zkd_measure_imad_peak(millis, ctypes.byref(v), _stream_ptr(stream)), "zkd_measure_imad_peak")
+    return v.value

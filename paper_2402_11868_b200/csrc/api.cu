@@ -1,0 +1,316 @@
+// api.cu — the C ABI of libzkd (include/zkd.h): argument validation, options, counters, host-side number helpers,
+// and the measured integer-multiply peak.  No arithmetic of the method lives here.
+#include <atomic>
+#include <cmath>
+#include <cstring>
+
+#include "zkd_internal.h"
+
+namespace zkd {
+
+static std::atomic<uint64_t> g_launches{0}, g_macs{0};
+void count_launch(uint64_t n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+void count_macs(uint64_t n) { g_macs.fetch_add(n, std::memory_order_relaxed); }
+Options& options() {
+  static Options o;
+  return o;
+}
+
+static int check_device() {
+  static int cached = 1;  // 1 = unknown
+  if (cached != 1) return cached;
+  int dev = 0;
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+    (void)cudaGetLastError();
+    return ZKD_ERR_CUDA;
+  }
+  cached = (prop.major == 10) ? ZKD_OK : ZKD_ERR_ARCH;
+  return cached;
+}
+
+// ---- measured IMAD peak -------------------------------------------------------------------------------------------
+// Register-only loop of independent IMAD.WIDE.U32 (32x32+64 -> 64), 8 accumulators per thread, 1024 threads per SM.
+__global__ void __launch_bounds__(256) imad_peak_kernel(uint32_t* out, uint32_t a0, uint32_t b0, int iters) {
+  uint32_t a = a0 + threadIdx.x, b = b0 + blockIdx.x;
+  uint64_t acc[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) acc[i] = i + threadIdx.x;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) asm volatile("mad.wide.u32 %0, %1, %2, %0;" : "+l"(acc[i]) : "r"(a), "r"(b));
+    }
+  }
+  uint64_t s = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s += acc[i];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = (uint32_t)s ^ (uint32_t)(s >> 32);
+}
+
+int measure_imad_peak(double millis, double* per_sec, cudaStream_t s) {
+  int dev = 0, sms = 0;
+  ZKD_CUDA_TRY(cudaGetDevice(&dev));
+  ZKD_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const int blocks = sms * 4, threads = 256;
+  uint32_t* d = nullptr;
+  ZKD_CUDA_TRY(cudaMalloc(&d, sizeof(uint32_t) * blocks * threads));
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  int iters = 2000;
+  double best = 0;
+  imad_peak_kernel<<<blocks, threads, 0, s>>>(d, 3, 5, 200);  // warm-up
+  const int reps = millis > 20 ? 5 : 3;
+  // size one launch to about millis/reps
+  for (int r = 0; r < reps + 1; ++r) {
+    cudaEventRecord(e0, s);
+    imad_peak_kernel<<<blocks, threads, 0, s>>>(d, 3, 5, iters);
+    cudaEventRecord(e1, s);
+    if (cudaEventSynchronize(e1) != cudaSuccess) {
+      (void)cudaGetLastError();
+      cudaFree(d);
+      return ZKD_ERR_CUDA;
+    }
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double ops = (double)blocks * threads * (double)iters * 32.0;
+    if (r > 0 && ops / (ms * 1e-3) > best) best = ops / (ms * 1e-3);
+    if (r == 0 && ms > 0) {
+      double scale = (millis / reps) / ms;
+      if (scale > 50) scale = 50;
+      if (scale < 0.05) scale = 0.05;
+      iters = (int)(iters * scale) + 1;
+    }
+  }
+  count_launch(reps + 2);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(d);
+  *per_sec = best;
+  return ZKD_OK;
+}
+
+}  // namespace zkd
+
+using namespace zkd;
+
+extern "C" {
+
+size_t zkd_real_bytes(int prec_bits) { return prec_bits == kPrec ? (size_t)kApiRealBytes : 0; }
+
+const char* zkd_strerror(int code) {
+  switch (code) {
+    case ZKD_OK: return "ok";
+    case ZKD_ERR_INVALID_ARG: return "invalid argument";
+    case ZKD_ERR_UNSUPPORTED_PREC: return "unsupported precision (768 only)";
+    case ZKD_ERR_WORKSPACE: return "workspace too small or allocation failed";
+    case ZKD_ERR_CUDA: return "CUDA error";
+    case ZKD_ERR_ARCH: return "device is not sm_100";
+    case ZKD_ERR_INTERNAL: return "internal consistency check failed";
+    default: return "unknown error";
+  }
+}
+int zkd_version(void) { return 100; }
+
+void zkd_counters(uint64_t* kernel_launches, uint64_t* gemm_digit_macs) {
+  if (kernel_launches) *kernel_launches = g_launches.load();
+  if (gemm_digit_macs) *gemm_digit_macs = g_macs.load();
+}
+void zkd_counters_reset(void) {
+  g_launches.store(0);
+  g_macs.store(0);
+}
+
+static int* option_slot(const char* key) {
+  Options& o = options();
+  if (!key) return nullptr;
+  if (!strcmp(key, "tau_bits")) return &o.tau_bits;
+  if (!strcmp(key, "tol_bits")) return &o.tol_bits;
+  if (!strcmp(key, "max_steps")) return &o.max_steps;
+  if (!strcmp(key, "gemm_path")) return &o.gemm_path;
+  if (!strcmp(key, "min_split_ctas")) return &o.min_split_ctas;
+  if (!strcmp(key, "seed_sweeps")) return &o.seed_sweeps;
+  if (!strcmp(key, "verbose")) return &o.verbose;
+  return nullptr;
+}
+int zkd_set_option(const char* key, double value) {
+  int* s = option_slot(key);
+  if (!s || !std::isfinite(value)) return ZKD_ERR_INVALID_ARG;
+  *s = (int)value;
+  return ZKD_OK;
+}
+int zkd_get_option(const char* key, double* value) {
+  int* s = option_slot(key);
+  if (!s || !value) return ZKD_ERR_INVALID_ARG;
+  *value = *s;
+  return ZKD_OK;
+}
+
+// ---- host-side number helpers -------------------------------------------------------------------------------------
+int zkd_pack(void* dst, int prec_bits, int sign, int64_t exp, const uint64_t* limbs_le) {
+  if (!dst || prec_bits != kPrec || sign < -1 || sign > 1) return ZKD_ERR_INVALID_ARG;
+  unsigned char* o = (unsigned char*)dst;
+  memset(o, 0, kApiRealBytes);
+  if (sign == 0) return ZKD_OK;
+  if (!limbs_le || !(limbs_le[kPrec / 64 - 1] >> 63)) return ZKD_ERR_INVALID_ARG;
+  int32_t s32 = sign;
+  memcpy(o, &s32, 4);
+  memcpy(o + 8, &exp, 8);
+  memcpy(o + 16, limbs_le, kPrec / 8);
+  return ZKD_OK;
+}
+int zkd_unpack(const void* src, int prec_bits, int* sign, int64_t* exp, uint64_t* limbs_le) {
+  if (!src || prec_bits != kPrec) return ZKD_ERR_INVALID_ARG;
+  const unsigned char* s = (const unsigned char*)src;
+  int32_t s32, fl;
+  int64_t e;
+  memcpy(&s32, s, 4);
+  memcpy(&fl, s + 4, 4);
+  memcpy(&e, s + 8, 8);
+  if (fl != 0 || s32 < -1 || s32 > 1) return ZKD_ERR_INVALID_ARG;
+  uint64_t top;
+  memcpy(&top, s + 16 + kPrec / 8 - 8, 8);
+  if (s32 != 0 && !(top >> 63)) return ZKD_ERR_INVALID_ARG;
+  if (sign) *sign = s32;
+  if (exp) *exp = e;
+  if (limbs_le) memcpy(limbs_le, s + 16, kPrec / 8);
+  return ZKD_OK;
+}
+int zkd_from_double(void* dst, int prec_bits, double v) {
+  if (!dst || prec_bits != kPrec || !std::isfinite(v)) return ZKD_ERR_INVALID_ARG;
+  uint64_t limbs[kPrec / 64] = {0};
+  if (v == 0.0) return zkd_pack(dst, prec_bits, 0, 0, nullptr);
+  int e;
+  double m = frexp(fabs(v), &e);  // m in [1/2, 1)
+  limbs[kPrec / 64 - 1] = (uint64_t)ldexp(m, 64);  // exact: m has 53 bits
+  return zkd_pack(dst, prec_bits, v < 0 ? -1 : 1, e, limbs);
+}
+double zkd_to_double(const void* src, int prec_bits) {
+  int sign;
+  int64_t e;
+  uint64_t limbs[kPrec / 64];
+  if (zkd_unpack(src, prec_bits, &sign, &e, limbs) != ZKD_OK) return NAN;
+  if (sign == 0) return 0.0;
+  // round to nearest even on the top 64 bits + sticky
+  uint64_t top = limbs[kPrec / 64 - 1];
+  bool sticky = false;
+  for (int k = 0; k < kPrec / 64 - 1; ++k) sticky |= limbs[k] != 0;
+  uint64_t keep = top >> 11, rem = top & 0x7ff;
+  if (rem > 0x400 || (rem == 0x400 && (sticky || (keep & 1)))) keep += 1;
+  double m = ldexp((double)keep, -53);
+  double r = ldexp(m, (int)e);
+  return sign < 0 ? -r : r;
+}
+
+// ---- building blocks ----------------------------------------------------------------------------------------------
+int zkd_fx_from_api(int count, int prec_bits, const void* src_api, int32_t* dst_fx, int scale_bits, void* stream) {
+  if (prec_bits != kPrec) return ZKD_ERR_UNSUPPORTED_PREC;
+  if (count < 0 || !src_api || !dst_fx) return ZKD_ERR_INVALID_ARG;
+  ZKD_TRY(check_device());
+  return fx_from_api(count, src_api, dst_fx, scale_bits, (cudaStream_t)stream);
+}
+int zkd_fx_to_api(int count, int prec_bits, const int32_t* src_fx, void* dst_api, int scale_bits, void* stream) {
+  if (prec_bits != kPrec) return ZKD_ERR_UNSUPPORTED_PREC;
+  if (count < 0 || !src_fx || !dst_api) return ZKD_ERR_INVALID_ARG;
+  ZKD_TRY(check_device());
+  return fx_to_api(count, src_fx, dst_api, scale_bits, (cudaStream_t)stream);
+}
+int zkd_gemm_fx_bufsize(int M, int N, int K, int batch, size_t* workspace_bytes) {
+  if (M < 1 || N < 1 || K < 1 || batch < 1 || !workspace_bytes) return ZKD_ERR_INVALID_ARG;
+  *workspace_bytes = gemm_workspace_bytes(M, N, K, batch);
+  return ZKD_OK;
+}
+int zkd_gemm_fx(int M, int N, int K, int batch, int op_a, const int32_t* A_fx, int a_top_bit, int a_digits,
+                const int32_t* B_fx, int b_top_bit, int b_digits, int32_t* C_fx, int mode, int out_cut_bit, int path,
+                void* workspace, size_t workspace_bytes, int* err_flag, int* msb_out, void* stream) {
+  if (M < 1 || N < 1 || K < 1 || batch < 1 || !A_fx || !B_fx || !C_fx || !workspace || mode < 0 || mode > 2 ||
+      a_digits < 1 || a_digits > kND || b_digits < 1 || b_digits > kND)
+    return ZKD_ERR_INVALID_ARG;
+  ZKD_TRY(check_device());
+  GemmSide P, Q;
+  P.fx = A_fx; P.rows = op_a ? K : M; P.cols = op_a ? M : K; P.conj_transpose = op_a != 0; P.top_bit = a_top_bit; P.nw = a_digits;
+  Q.fx = B_fx; Q.rows = K; Q.cols = N; Q.top_bit = b_top_bit; Q.nw = b_digits;
+  return gemm_complex(M, N, K, batch, P, Q, C_fx, (GemmMode)mode, out_cut_bit, path, workspace, workspace_bytes, err_flag,
+                      msb_out, (cudaStream_t)stream);
+}
+int zkd_seed_fp64(int N, int batch, const double* A64, double* mu, double* V, void* stream) {
+  if (N < 1 || N > ZKD_MAX_N || batch < 1 || !A64 || !mu || !V) return ZKD_ERR_INVALID_ARG;
+  ZKD_TRY(check_device());
+  return seed_fp64(N, batch, A64, mu, V, options().seed_sweeps, (cudaStream_t)stream);
+}
+int zkd_measure_imad_peak(double millis, double* imad_wide_per_sec, void* stream) {
+  if (!imad_wide_per_sec || !(millis > 0)) return ZKD_ERR_INVALID_ARG;
+  ZKD_TRY(check_device());
+  return measure_imad_peak(millis, imad_wide_per_sec, (cudaStream_t)stream);
+}
+
+// ---- the hot path -------------------------------------------------------------------------------------------------
+static int check_diag_args(int N, int batch, int prec_bits) {
+  if (prec_bits != kPrec) return ZKD_ERR_UNSUPPORTED_PREC;
+  if (N < 1 || N > ZKD_MAX_N || batch < 1) return ZKD_ERR_INVALID_ARG;
+  return ZKD_OK;
+}
+int zkd_diag_herm_bufsize(int N, int batch, int prec_bits, size_t* workspace_bytes) {
+  ZKD_TRY(check_diag_args(N, batch, prec_bits));
+  if (!workspace_bytes) return ZKD_ERR_INVALID_ARG;
+  *workspace_bytes = diag_workspace_bytes(N, batch);
+  return ZKD_OK;
+}
+int zkd_diag_herm_ws(int N, int batch, int prec_bits, const void* A, void* eigvals, void* eigvecs, void* workspace,
+                     size_t workspace_bytes, zkd_info* info, void* stream) {
+  ZKD_TRY(check_diag_args(N, batch, prec_bits));
+  if (!A || !eigvals || !eigvecs || !workspace) return ZKD_ERR_INVALID_ARG;
+  if (((uintptr_t)A | (uintptr_t)eigvals | (uintptr_t)eigvecs | (uintptr_t)workspace) & 15) return ZKD_ERR_INVALID_ARG;
+  if (workspace_bytes < diag_workspace_bytes(N, batch)) return ZKD_ERR_WORKSPACE;
+  ZKD_TRY(check_device());
+  return diag_herm_device(N, batch, A, eigvals, eigvecs, workspace, workspace_bytes, info, (cudaStream_t)stream);
+}
+int zkd_diag_herm(int N, int batch, int prec_bits, const void* A, void* eigvals, void* eigvecs, void* stream) {
+  ZKD_TRY(check_diag_args(N, batch, prec_bits));
+  if (!A || !eigvals || !eigvecs) return ZKD_ERR_INVALID_ARG;
+  ZKD_TRY(check_device());
+  const size_t bytes = diag_workspace_bytes(N, batch);
+  void* ws = nullptr;
+  cudaStream_t s = (cudaStream_t)stream;
+  if (cudaMallocAsync(&ws, bytes, s) != cudaSuccess) {
+    (void)cudaGetLastError();
+    return ZKD_ERR_WORKSPACE;
+  }
+  int rc = zkd_diag_herm_ws(N, batch, prec_bits, A, eigvals, eigvecs, ws, bytes, nullptr, stream);
+  cudaFreeAsync(ws, s);
+  return rc;
+}
+int zkd_diag_herm_host(int N, int batch, int prec_bits, const void* A_host, void* eigvals_host, void* eigvecs_host,
+                       zkd_info* info_host) {
+  ZKD_TRY(check_diag_args(N, batch, prec_bits));
+  if (!A_host || !eigvals_host || !eigvecs_host) return ZKD_ERR_INVALID_ARG;
+  ZKD_TRY(check_device());
+  const size_t nA = (size_t)batch * N * N * 2 * kApiRealBytes, nL = (size_t)batch * N * kApiRealBytes;
+  const size_t wsb = diag_workspace_bytes(N, batch);
+  char* buf = nullptr;
+  const size_t offL = (nA + 255) / 256 * 256, offX = offL + (nL + 255) / 256 * 256, offI = offX + offL,
+               offW = offI + ((sizeof(zkd_info) * batch + 255) / 256 * 256);
+  if (cudaMalloc(&buf, offW + wsb) != cudaSuccess) {
+    (void)cudaGetLastError();
+    return ZKD_ERR_WORKSPACE;
+  }
+  int rc = ZKD_OK;
+  cudaStream_t s = 0;
+  if (cudaMemcpyAsync(buf, A_host, nA, cudaMemcpyHostToDevice, s) != cudaSuccess) rc = ZKD_ERR_CUDA;
+  if (rc == ZKD_OK)
+    rc = zkd_diag_herm_ws(N, batch, prec_bits, buf, buf + offL, buf + offX, buf + offW, wsb, (zkd_info*)(buf + offI), s);
+  if (rc == ZKD_OK) {
+    if (cudaMemcpyAsync(eigvals_host, buf + offL, nL, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+        cudaMemcpyAsync(eigvecs_host, buf + offX, nA, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+        (info_host && cudaMemcpyAsync(info_host, buf + offI, sizeof(zkd_info) * batch, cudaMemcpyDeviceToHost, s) != cudaSuccess) ||
+        cudaStreamSynchronize(s) != cudaSuccess)
+      rc = ZKD_ERR_CUDA;
+  }
+  if (rc == ZKD_ERR_CUDA) (void)cudaGetLastError();
+  cudaFree(buf);
+  return rc;
+}
+
+}  // extern "C"

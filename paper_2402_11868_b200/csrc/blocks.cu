@@ -1,0 +1,394 @@
+// blocks.cu — the O(N^2) and O(N^2 m) kernels of the refinement (SURVEY.md 8(a) S2, S3, S4c, S4d', S4f, S5, S6):
+// cluster detection, X := V, cluster-block Gram / Rayleigh-quotient matrices, block-diagonal applies (residual,
+// orthonormalisation, Rayleigh-Ritz rotation), the divided correction coefficients E_ij = C_ij / (theta_j - theta_i),
+// sorting, phase normalisation.  All multi-digit arithmetic is in-thread on FX digits (fx.cuh).
+#include "blocks.h"
+#include "fx.cuh"
+
+namespace zkd {
+
+// ---- FX -> complex double ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) fxc_to_c64_kernel(size_t count, const int32_t* __restrict__ src, double2* __restrict__ dst) {
+  const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= count) return;
+  int32_t d[ND];
+  fx_load(d, src, count, e);
+  const double re = fx_to_double(d);
+  fx_load(d, src + (size_t)ND * count, count, e);
+  dst[e] = make_double2(re, fx_to_double(d));
+}
+int fxc_to_c64(size_t count, const int32_t* src, double2* dst, cudaStream_t s) {
+  fxc_to_c64_kernel<<<(unsigned)((count + 255) / 256), 256, 0, s>>>(count, src, dst);
+  count_launch();
+  return launch_check();
+}
+
+// ---- S2: clusters ----------------------------------------------------------------------------------------------------
+// One CTA per matrix.  F = ||A64||_F; a new cluster starts at j when mu_j - mu_{j-1} > 2^-tau F.
+// cl[j] = first column of j's cluster, cle[j] = one past its last column.
+__global__ void __launch_bounds__(256) cluster_kernel(int n, const double2* __restrict__ A64, const double* __restrict__ mu,
+                                                      int tau_bits, int* __restrict__ cl, int* __restrict__ cle,
+                                                      int* __restrict__ stats /* [nb][2]: n_clusters, max_cluster */) {
+  __shared__ double s_red[8];
+  __shared__ double s_F;
+  const int b = blockIdx.x, tid = threadIdx.x;
+  const double2* Ab = A64 + (size_t)b * n * n;
+  double s = 0;
+  for (size_t e = tid; e < (size_t)n * n; e += blockDim.x) { const double2 a = Ab[e]; s += a.x * a.x + a.y * a.y; }
+  for (int off = 16; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+  if ((tid & 31) == 0) s_red[tid >> 5] = s;
+  __syncthreads();
+  if (tid == 0) {
+    double t = 0;
+    for (int w = 0; w < 8; ++w) t += s_red[w];
+    s_F = sqrt(t);
+  }
+  __syncthreads();
+  if (tid == 0) {
+    const double thr = ldexp(s_F, -tau_bits);
+    const double* m = mu + (size_t)b * n;
+    int* c = cl + (size_t)b * n;
+    int* ce = cle + (size_t)b * n;
+    int start = 0, ncl = 0, maxc = 0;
+    for (int j = 0; j < n; ++j) {
+      if (j > 0 && (m[j] - m[j - 1] > thr)) {
+        for (int k = start; k < j; ++k) ce[k] = j;
+        if (j - start > maxc) maxc = j - start;
+        ++ncl;
+        start = j;
+      }
+      c[j] = start;
+    }
+    for (int k = start; k < n; ++k) ce[k] = n;
+    if (n - start > maxc) maxc = n - start;
+    ++ncl;
+    stats[2 * b] = ncl;
+    stats[2 * b + 1] = maxc;
+  }
+}
+int cluster_detect(int n, int nb, const double2* A64, const double* mu, int tau_bits, int* cl, int* cle, int* stats, cudaStream_t s) {
+  cluster_kernel<<<nb, 256, 0, s>>>(n, A64, mu, tau_bits, cl, cle, stats);
+  count_launch();
+  return launch_check();
+}
+
+// ---- S3: X := V (exactly, truncated below FX bit 756 = digit 27) --------------------------------------------------------
+__global__ void __launch_bounds__(256) init_x_kernel(size_t count, const double2* __restrict__ V, int32_t* __restrict__ X) {
+  const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= count) return;
+  const double2 v = V[e];
+  int32_t d[ND];
+  fx_from_double(d, v.x);
+  // truncate toward -inf below digit 27 (keeps the value a short-window number: digits 27..29 only)
+#pragma unroll
+  for (int k = 0; k < 27; ++k) d[k] = 0;
+  fx_store(X, count, e, d);
+  fx_from_double(d, v.y);
+#pragma unroll
+  for (int k = 0; k < 27; ++k) d[k] = 0;
+  fx_store(X + (size_t)ND * count, count, e, d);
+}
+int init_x(size_t count, const double2* V, int32_t* X, cudaStream_t s) {
+  init_x_kernel<<<(unsigned)((count + 255) / 256), 256, 0, s>>>(count, V, X);
+  count_launch();
+  return launch_check();
+}
+
+// ---- cluster-block Gram matrices: G_ij = sum_k conj(x_ki) y_kj for cl(i) == cl(j) -------------------------------------
+// one warp per (b, i, j, part); lanes split k; exact digit products, one carry pass per MAC pair.
+__global__ void __launch_bounds__(128) gram_kernel(int n, int nb, const int32_t* __restrict__ X, const int32_t* __restrict__ Y,
+                                                   const int* __restrict__ cl, int32_t* __restrict__ G) {
+  const size_t w = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  const size_t per = (size_t)n * n;
+  if (w >= per * nb * 2) return;
+  const int part = (int)(w & 1);
+  const size_t e = w >> 1;
+  const int b = (int)(e / per);
+  const int i = (int)((e % per) / n), j = (int)(e % n);
+  if (cl[(size_t)b * n + i] != cl[(size_t)b * n + j]) return;
+  const size_t count = per * nb;
+  const int32_t* Xr = X;
+  const int32_t* Xi = X + (size_t)ND * count;
+  const int32_t* Yr = Y;
+  const int32_t* Yi = Y + (size_t)ND * count;
+  int64_t acc[FXP_NACC];
+  fxp_zero(acc);
+  for (int k = lane; k < n; k += 32) {
+    const size_t ei = (size_t)b * per + (size_t)k * n + i, ej = (size_t)b * per + (size_t)k * n + j;
+    int32_t a[ND], c[ND];
+    if (part == 0) {  // xr yr + xi yi
+      fx_load(a, Xr, count, ei); fx_load(c, Yr, count, ej); fx_mac<false>(acc, a, c);
+      fx_load(a, Xi, count, ei); fx_load(c, Yi, count, ej); fx_mac<false>(acc, a, c);
+    } else {          // xr yi - xi yr
+      fx_load(a, Xr, count, ei); fx_load(c, Yi, count, ej); fx_mac<false>(acc, a, c);
+      fx_load(a, Xi, count, ei); fx_load(c, Yr, count, ej); fx_mac<true>(acc, a, c);
+    }
+    fxp_relax(acc);
+  }
+  warp_sum_cols(acc);
+  if (lane == 0) {
+    int32_t r[ND];
+    fxp_finish(r, acc);
+    fx_store(G + (part ? (size_t)ND * count : 0), count, e, r);
+  }
+}
+int gram_blocks(int n, int nb, const int32_t* X, const int32_t* Y, const int* cl, int32_t* G, cudaStream_t s) {
+  const size_t warps = (size_t)n * n * nb * 2;
+  gram_kernel<<<(unsigned)((warps * 32 + 127) / 128), 128, 0, s>>>(n, nb, X, Y, cl, G);
+  count_launch();
+  return launch_check();
+}
+
+// ---- M := (I - G)/2 on cluster blocks (Newton-Schulz orthonormalisation step), msb of (G - I) ---------------------------
+__global__ void __launch_bounds__(256) ns_build_kernel(int n, int nb, const int* __restrict__ cl, int32_t* __restrict__ G,
+                                                       int* __restrict__ msb_out) {
+  const size_t per = (size_t)n * n, count = per * nb;
+  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= count * 2) return;
+  const int part = (int)(t / count);
+  const size_t e = t % count;
+  const int b = (int)(e / per), i = (int)((e % per) / n), j = (int)(e % n);
+  if (cl[(size_t)b * n + i] != cl[(size_t)b * n + j]) return;
+  int32_t* p = G + (part ? (size_t)ND * count : 0);
+  int32_t g[ND], r[ND];
+  fx_load(g, p, count, e);
+  if (part == 0 && i == j) g[ND - 1] -= 1;  // G - I
+  const int msb = fx_msb(g);
+  if (msb_out) atomicMax(msb_out, msb);
+  fx_neg(r, g);
+  fx_half(g, r);                            // (I - G)/2
+  fx_store(p, count, e, g);
+}
+int ns_build(int n, int nb, const int* cl, int32_t* G, int* msb_out, cudaStream_t s) {
+  const size_t t = (size_t)n * n * nb * 2;
+  ns_build_kernel<<<(unsigned)((t + 255) / 256), 256, 0, s>>>(n, nb, cl, G, msb_out);
+  count_launch();
+  return launch_check();
+}
+
+// ---- block-diagonal apply: dst_ij = base_ij + sgn * sum_{l in cluster(j)} Y_il M_lj -----------------------------------------
+// one thread per (b, i, j, part).  base may be null (treated as zero).  msb_out: atomicMax of msb(dst).
+__global__ void __launch_bounds__(128) block_apply_kernel(int n, int nb, const int32_t* __restrict__ base, const int32_t* __restrict__ Y,
+                                                          const int32_t* __restrict__ M, const int* __restrict__ cl,
+                                                          const int* __restrict__ cle, int negate, int32_t* __restrict__ dst,
+                                                          int* __restrict__ msb_out) {
+  const size_t per = (size_t)n * n, count = per * nb;
+  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= count * 2) return;
+  const int part = (int)(t / count);
+  const size_t e = t % count;
+  const int b = (int)(e / per), i = (int)((e % per) / n), j = (int)(e % n);
+  const int l0 = cl[(size_t)b * n + j], l1 = cle[(size_t)b * n + j];
+  const int32_t* Yr = Y;
+  const int32_t* Yi = Y + (size_t)ND * count;
+  const int32_t* Mr = M;
+  const int32_t* Mi = M + (size_t)ND * count;
+  int64_t acc[FXP_NACC];
+  fxp_zero(acc);
+  for (int l = l0; l < l1; ++l) {
+    const size_t ey = (size_t)b * per + (size_t)i * n + l, em = (size_t)b * per + (size_t)l * n + j;
+    int32_t a[ND], c[ND];
+    if (part == 0) {  // yr mr - yi mi
+      fx_load(a, Yr, count, ey); fx_load(c, Mr, count, em); fx_mac<false>(acc, a, c);
+      fx_load(a, Yi, count, ey); fx_load(c, Mi, count, em); fx_mac<true>(acc, a, c);
+    } else {          // yr mi + yi mr
+      fx_load(a, Yr, count, ey); fx_load(c, Mi, count, em); fx_mac<false>(acc, a, c);
+      fx_load(a, Yi, count, ey); fx_load(c, Mr, count, em); fx_mac<false>(acc, a, c);
+    }
+    fxp_relax(acc);
+  }
+  int32_t r[ND], o[ND];
+  fxp_finish(r, acc);
+  if (base) {
+    int32_t bs[ND];
+    fx_load(bs, base + (part ? (size_t)ND * count : 0), count, e);
+    if (negate) fx_sub(o, bs, r); else fx_add(o, bs, r);
+  } else {
+    if (negate) fx_neg(o, r);
+    else {
+#pragma unroll
+      for (int k = 0; k < ND; ++k) o[k] = r[k];
+    }
+  }
+  fx_store(dst + (part ? (size_t)ND * count : 0), count, e, o);
+  if (msb_out) {
+    const int msb = fx_msb(o);
+    // warp-level max first to keep the atomic traffic low
+    int m = msb;
+    for (int off = 16; off > 0; off >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, off));
+    if ((threadIdx.x & 31) == 0) atomicMax(msb_out, m);
+  }
+}
+int block_apply(int n, int nb, const int32_t* base, const int32_t* Y, const int32_t* M, const int* cl, const int* cle, bool negate,
+                int32_t* dst, int* msb_out, cudaStream_t s) {
+  const size_t t = (size_t)n * n * nb * 2;
+  block_apply_kernel<<<(unsigned)((t + 127) / 128), 128, 0, s>>>(n, nb, base, Y, M, cl, cle, negate ? 1 : 0, dst, msb_out);
+  count_launch();
+  return launch_check();
+}
+
+// ---- theta_j = Re S_jj ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) theta_kernel(int n, int nb, const int32_t* __restrict__ S, int32_t* __restrict__ theta) {
+  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (size_t)n * nb) return;
+  const int b = (int)(t / n), j = (int)(t % n);
+  const size_t count = (size_t)n * n * nb;
+  int32_t d[ND];
+  fx_load(d, S, count, (size_t)b * n * n + (size_t)j * n + j);
+  fx_store(theta, (size_t)n * nb, t, d);
+}
+int theta_from_diag(int n, int nb, const int32_t* S, int32_t* theta, cudaStream_t s) {
+  theta_kernel<<<(unsigned)(((size_t)n * nb + 127) / 128), 128, 0, s>>>(n, nb, S, theta);
+  count_launch();
+  return launch_check();
+}
+
+// ---- complex FX add: X += T ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) fx_add_kernel(size_t reals, int32_t* __restrict__ X, const int32_t* __restrict__ T) {
+  const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= reals) return;
+  // planes of re and im are laid out [2][ND][count]; treat as 2*count reals with plane stride `count`
+  const size_t count = reals / 2;
+  const size_t part = e / count, idx = e % count;
+  int32_t* xp = X + part * (size_t)ND * count;
+  const int32_t* tp = T + part * (size_t)ND * count;
+  int32_t a[ND], c[ND], r[ND];
+  fx_load(a, xp, count, idx);
+  fx_load(c, tp, count, idx);
+  fx_add(r, a, c);
+  fx_store(xp, count, idx, r);
+}
+int fxc_add_inplace(size_t count, int32_t* X, const int32_t* T, cudaStream_t s) {
+  fx_add_kernel<<<(unsigned)((2 * count + 255) / 256), 256, 0, s>>>(2 * count, X, T);
+  count_launch();
+  return launch_check();
+}
+
+// ---- E_ij = C_ij / (theta_j - theta_i) across clusters, 0 inside ---------------------------------------------------------------
+// One thread per pair i < j (and the diagonal, which is zeroed).  d = theta_j - theta_i is normalised to
+// d' = d 2^s in [1/4, 1/2) with a static barrel shifter, r = 1/d' by Newton from an fp64 start on W-digit fixed point
+// (r in (2,4], FX-like with 29 - (30-W) fractional digits), then E_ij = (C_ij r) 2^s, E_ji = -(C_ji r) 2^s.
+// r <- 1/d' for d' in [1/4,1/2] given as FX (only the top W digits below the binary point are used);
+// r returned as FX (value in [2,4]).  Newton: r <- r + r (1 - d' r), quadratic from an fp64 start.
+template <int W>
+__device__ __forceinline__ void fx_recip_quarter(int32_t (&r)[ND], const int32_t (&dq)[ND], int iters) {
+  // work on full FX digits but zero everything below digit ND-1-W so that products are short where it matters:
+  // the compiler removes multiplications by literal zeros only if the zeros are compile-time; so use W-digit arrays.
+  constexpr int LO = ND - 1 - W;  // first digit kept (FX digit index); fractional digits kept: 29 - LO = W...
+  int32_t dw[W + 1], rw[W + 1];   // digits LO..ND-1 of d' and r
+#pragma unroll
+  for (int k = 0; k <= W; ++k) dw[k] = dq[LO + k];
+  {
+    // fp64 start from the top three digits of d'
+    double dd = ((double)dw[W] * 268435456.0 + (double)dw[W - 1]) * 268435456.0 + (double)dw[W - 2];
+    dd = ldexp(dd, -3 * DB + DB);  // value: digit ND-1 is the integer digit -> dw[W] has weight 1
+    const double r0 = 1.0 / dd;     // in [2,4]
+    int32_t t[ND];
+    fx_from_double(t, r0);
+#pragma unroll
+    for (int k = 0; k <= W; ++k) rw[k] = t[LO + k];
+  }
+  // value(x) = sum_k x[k] 2^(28 (k - W)); product columns: x[a] y[b] has weight 2^(28 (a + b - 2W)); result digit k
+  // <- column k + W.  Keep columns >= W - 1 (guard).
+  for (int it = 0; it < iters; ++it) {
+    int64_t acc[W + 2];
+#pragma unroll
+    for (int k = 0; k < W + 2; ++k) acc[k] = 0;
+    mac_cols<W + 1, W + 1, W - 1, W + 2, false>(acc, dw, rw);  // columns W-1 .. 2W; the top one is signed digit W
+    carry_canon(acc);
+    // e = 1 - d' r : digits (acc[1 + k] is result digit k)
+    int32_t ew[W + 1];
+#pragma unroll
+    for (int k = 0; k <= W; ++k) ew[k] = -(int32_t)acc[1 + k];
+    ew[W] += 1;
+    carry_canon32(ew);
+    // r += r e
+    int64_t acc2[W + 2];
+#pragma unroll
+    for (int k = 0; k < W + 2; ++k) acc2[k] = 0;
+    // ew is canonical with signed top; rw canonical
+    mac_cols<W + 1, W + 1, W - 1, W + 2, false>(acc2, rw, ew);
+    carry_canon(acc2);
+#pragma unroll
+    for (int k = 0; k <= W; ++k) rw[k] += (int32_t)acc2[1 + k];
+    carry_canon32(rw);
+  }
+  fx_zero(r);
+#pragma unroll
+  for (int k = 0; k <= W; ++k) r[LO + k] = rw[k];
+}
+
+template <int W>
+__global__ void __launch_bounds__(128) ecalc_kernel(int n, int nb, const int32_t* __restrict__ theta, const int* __restrict__ cl,
+                                                    int32_t* __restrict__ C, int newton_iters, int* __restrict__ msb_out,
+                                                    int* __restrict__ err_flag) {
+  const size_t per = (size_t)n * n, count = per * nb;
+  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= count) return;
+  const int b = (int)(t / per), i = (int)((t % per) / n), j = (int)(t % n);
+  if (i > j) return;
+  int32_t* Cr = C;
+  int32_t* Ci = C + (size_t)ND * count;
+  const size_t eij = (size_t)b * per + (size_t)i * n + j, eji = (size_t)b * per + (size_t)j * n + i;
+  int32_t z[ND];
+  fx_zero(z);
+  if (cl[(size_t)b * n + i] == cl[(size_t)b * n + j]) {
+    fx_store(Cr, count, eij, z); fx_store(Ci, count, eij, z);
+    if (i != j) { fx_store(Cr, count, eji, z); fx_store(Ci, count, eji, z); }
+    return;
+  }
+  int32_t ti[ND], tj[ND], d[ND];
+  fx_load(ti, theta, (size_t)n * nb, (size_t)b * n + i);
+  fx_load(tj, theta, (size_t)n * nb, (size_t)b * n + j);
+  fx_sub(d, tj, ti);
+  const bool dneg = fx_is_neg(d);
+  if (dneg) { int32_t u[ND]; fx_neg(u, d);
+#pragma unroll
+    for (int k = 0; k < ND; ++k) d[k] = u[k]; }
+  const int msb = fx_msb(d);  // |d| in [2^(msb-1-812), 2^(msb-812))
+  if (msb < 812 - 200) {      // different clusters must be apart; anything this close is a planning error
+    if (err_flag) atomicOr(err_flag, 2);
+    fx_store(Cr, count, eij, z); fx_store(Ci, count, eij, z);
+    fx_store(Cr, count, eji, z); fx_store(Ci, count, eji, z);
+    return;
+  }
+  // d' = d 2^s with msb(d') = 811  (value in [1/4,1/2))
+  const int s = 811 - msb;  // may be negative when |d| >= 1/2
+  if (s >= 0) fx_shl(d, s); else fx_shr(d, -s);
+  int32_t r[ND];
+  fx_recip_quarter<W>(r, d, newton_iters);
+  // E = (C r) 2^s, with sign
+  int mymsb = 0;
+#pragma unroll 1
+  for (int which = 0; which < 4; ++which) {
+    int32_t* plane = (which & 1) ? Ci : Cr;
+    const size_t e = (which & 2) ? eji : eij;
+    const bool neg = dneg ^ ((which & 2) != 0);
+    int32_t c[ND], o[ND];
+    fx_load(c, plane, count, e);
+    fx_mul(o, c, r);
+    if (s >= 0) fx_shl(o, s); else fx_shr(o, -s);
+    if (neg) { int32_t u[ND]; fx_neg(u, o);
+#pragma unroll
+      for (int k = 0; k < ND; ++k) o[k] = u[k]; }
+    fx_store(plane, count, e, o);
+    mymsb = max(mymsb, fx_msb(o));
+  }
+  if (msb_out) atomicMax(msb_out, mymsb);
+}
+int ecalc(int n, int nb, const int32_t* theta, const int* cl, int32_t* C, int prec_bits, int* msb_out, int* err_flag, cudaStream_t s) {
+  const size_t t = (size_t)n * n * nb;
+  const unsigned blocks = (unsigned)((t + 127) / 128);
+  // Newton doubles the ~50 correct bits of the fp64 start each iteration
+  int iters = 0;
+  for (int have = 48; have < prec_bits; have *= 2) ++iters;
+  if (prec_bits <= 28 * 4 - 8) ecalc_kernel<4><<<blocks, 128, 0, s>>>(n, nb, theta, cl, C, iters, msb_out, err_flag);
+  else if (prec_bits <= 28 * 8 - 8) ecalc_kernel<8><<<blocks, 128, 0, s>>>(n, nb, theta, cl, C, iters, msb_out, err_flag);
+  else if (prec_bits <= 28 * 16 - 8) ecalc_kernel<16><<<blocks, 128, 0, s>>>(n, nb, theta, cl, C, iters, msb_out, err_flag);
+  else ecalc_kernel<29><<<blocks, 128, 0, s>>>(n, nb, theta, cl, C, iters, msb_out, err_flag);
+  count_launch();
+  return launch_check();
+}
+
+}  // namespace zkd

@@ -1,0 +1,34 @@
+// blocks.h — host entry points of the O(N^2) / O(N^2 m) kernels (blocks.cu, finalize.cu).
+#pragma once
+#include "zkd_internal.h"
+
+namespace zkd {
+
+int fxc_to_c64(size_t count, const int32_t* src, double2* dst, cudaStream_t s);
+int cluster_detect(int n, int nb, const double2* A64, const double* mu, int tau_bits, int* cl, int* cle, int* stats, cudaStream_t s);
+int init_x(size_t count, const double2* V, int32_t* X, cudaStream_t s);
+int gram_blocks(int n, int nb, const int32_t* X, const int32_t* Y, const int* cl, int32_t* G, cudaStream_t s);
+int ns_build(int n, int nb, const int* cl, int32_t* G, int* msb_out, cudaStream_t s);
+int block_apply(int n, int nb, const int32_t* base, const int32_t* Y, const int32_t* M, const int* cl, const int* cle, bool negate,
+                int32_t* dst, int* msb_out, cudaStream_t s);
+int theta_from_diag(int n, int nb, const int32_t* S, int32_t* theta, cudaStream_t s);
+int fxc_add_inplace(size_t count, int32_t* X, const int32_t* T, cudaStream_t s);
+int ecalc(int n, int nb, const int32_t* theta, const int* cl, int32_t* C, int prec_bits, int* msb_out, int* err_flag, cudaStream_t s);
+
+// finalize.cu
+// S0: per-matrix scale (max exponent over the upper triangle) and ingest with Hermitian mirroring
+int ingest_herm(int N, int batch, const void* A_api, int32_t* A_fx, int* scale /*[batch]*/, int* status /*[batch]*/, cudaStream_t s);
+// S5 plumbing: gather cluster blocks of S into a batch of m x m sub-problems scaled by 2^k, and back
+struct SubProblem { int b, col0; };  // matrix index and first column of the cluster
+int sub_gather(int n, int nb, int m, int nsub, const SubProblem* subs_dev, const int32_t* S, int32_t* H /*nsub m m*/,
+               int32_t* cbar /*FxR nsub*/, int* kshift /*nsub*/, int* degenerate /*nsub*/, int degenerate_msb,
+               const int* noise_parent /*nb, may be null*/, int* noise_child /*nsub*/, cudaStream_t s);
+int sub_scatter(int n, int nb, int m, int nsub, const SubProblem* subs_dev, const int32_t* U /*nsub m m*/, const int32_t* lam_sub,
+                const int32_t* cbar, const int* kshift, const int* degenerate, int32_t* Um /*nb n n*/, int32_t* theta, cudaStream_t s);
+int identity_blocks(int n, int nb, int32_t* Um, cudaStream_t s);
+// S6: sort ascending, phase-normalise, export
+int finalize_export(int N, int batch, const int32_t* X, const int32_t* lam, const int* scale, void* eigvals_api, void* eigvecs_api,
+                    int32_t* scratch /* FxC batch N N */, int32_t* lam_sorted /* FxR batch N */, int* rank /* batch N */,
+                    cudaStream_t s);
+
+}  // namespace zkd

@@ -1,0 +1,332 @@
+// gemm_digits.cu — complex FX matrix product on the IMAD path: operand preparation (window extraction, 3M
+// combinations, balanced digits), instance selection, and the combine epilogue (split-K sum, 3M recombination,
+// carry propagation, placement into the FX destination).
+//
+// Complex product by 3 real products (3M):  with P = pr + i pi and Q = qr + i qi,
+//     k1 = (pr + pi) qr,  k2 = pr (qi - qr),  k3 = pi (qr + qi);   Re = k1 - k3,  Im = k1 + k2.
+// In fixed point the operand sums are exact, so 3M costs nothing in accuracy.
+#include <vector>
+
+#include "gemm_digits.cuh"
+#include "zkd_internal.h"
+
+namespace zkd {
+
+#define ZKD_DECL_Q(n) \
+  extern const GemmInstance kGemmInstQ##n[]; \
+  extern const int kGemmInstQ##n##Count;
+ZKD_DECL_Q(3) ZKD_DECL_Q(4) ZKD_DECL_Q(5) ZKD_DECL_Q(6) ZKD_DECL_Q(8) ZKD_DECL_Q(10) ZKD_DECL_Q(12) ZKD_DECL_Q(15)
+ZKD_DECL_Q(18) ZKD_DECL_Q(22) ZKD_DECL_Q(30)
+
+static const std::vector<GemmInstance>& instances() {
+  static std::vector<GemmInstance> v;
+  if (v.empty()) {
+#define ZKD_ADD_Q(n) v.insert(v.end(), kGemmInstQ##n, kGemmInstQ##n + kGemmInstQ##n##Count);
+    ZKD_ADD_Q(3) ZKD_ADD_Q(4) ZKD_ADD_Q(5) ZKD_ADD_Q(6) ZKD_ADD_Q(8) ZKD_ADD_Q(10) ZKD_ADD_Q(12) ZKD_ADD_Q(15)
+    ZKD_ADD_Q(18) ZKD_ADD_Q(22) ZKD_ADD_Q(30)
+  }
+  return v;
+}
+
+static uint64_t inst_cost(const GemmInstance& in) {
+  // digit products per (i,j,k): pairs (a,b) with a + b >= low
+  uint64_t c = 0;
+  for (int a = 0; a < in.np; ++a)
+    for (int b = 0; b < in.nq; ++b)
+      if (a + b >= in.low) ++c;
+  return c;
+}
+
+// Cheapest instance with np >= nwP, nq >= nwQ and at least `ncols_needed` kept columns below the top.
+static const GemmInstance* pick_instance(int nwP, int nwQ) {
+  const GemmInstance* best = nullptr;
+  uint64_t bc = ~0ull;
+  for (const auto& in : instances()) {
+    if (in.np < nwP || in.nq < nwQ) continue;
+    // padding an operand at its low end shifts the needed columns up by the same amount, so the truncation rule
+    // LOW = NQ - 2 of the instance keeps at least the columns the request needs when nq_inst - nwQ <= np pad ...
+    uint64_t c = inst_cost(in);
+    if (c < bc) { bc = c; best = &in; }
+  }
+  return best;
+}
+
+// ---- operand preparation ----------------------------------------------------------------------------------------
+
+struct PrepArgs {
+  const int32_t* src;  // complex FX, batch * rows * cols
+  int32_t* dst;        // [3*batch][nw][R][C]
+  size_t src_count;    // batch * rows * cols
+  int R, C;            // destination dims (P: M x K, Q: K x N)
+  int batch;
+  int transpose;       // source stored C x R and conjugated
+  int side;            // 0: P-type planes (re+im, re, im); 1: Q-type planes (re, im-re, re+im)
+  int lsb_bit;         // FX bit position of digit 0 of the compact operand (may be negative)
+  int nw;              // digits written
+  int nw_src;          // digits taken from the source window (the rest, at the LOW end, are zero padding)
+  int* err_flag;
+};
+
+__device__ __forceinline__ int32_t fx_digit_get(const int32_t* __restrict__ planes, size_t count, size_t idx, int q, int32_t top) {
+  if (q < 0) return 0;
+  if (q < kND - 1) return planes[(size_t)q * count + idx];
+  if (q == kND - 1) return top & DMASK;
+  if (q == kND) return (top >> DB) & DMASK;
+  return top < 0 ? DMASK : 0;
+}
+
+__global__ void __launch_bounds__(256) prep_kernel(PrepArgs a) {
+  const size_t per = (size_t)a.R * a.C;
+  const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= per * a.batch) return;
+  const int b = (int)(e / per);
+  const size_t rc = e % per;
+  const int r = (int)(rc / a.C), c = (int)(rc % a.C);
+  const size_t sidx = a.transpose ? ((size_t)b * per + (size_t)c * a.R + r) : e;
+  const int32_t* re = a.src;
+  const int32_t* im = a.src + (size_t)kND * a.src_count;
+  const int32_t top_re = re[(size_t)(kND - 1) * a.src_count + sidx];
+  const int32_t top_im = im[(size_t)(kND - 1) * a.src_count + sidx];
+  const bool neg_re = top_re < 0, neg_im = top_im < 0;
+  const int pad = a.nw - a.nw_src;  // zero digits at the low end
+  const int lsb = a.lsb_bit + pad * DB;
+  // floor division of lsb by 28
+  int q0 = lsb >= 0 ? lsb / DB : -((-lsb + DB - 1) / DB);
+  const int sh = lsb - q0 * DB;  // 0..27
+
+  int64_t carry[3] = {0, 0, 0};
+  int32_t lo_re = fx_digit_get(re, a.src_count, sidx, q0, top_re);
+  int32_t lo_im = fx_digit_get(im, a.src_count, sidx, q0, top_im);
+  bool bad = false;
+  const size_t dplane = per;                      // elements per digit plane of one g
+  int32_t* dst0 = a.dst + ((size_t)(b * 3) * a.nw) * dplane + rc;
+  for (int d = 0; d < pad; ++d) {
+    dst0[((size_t)0 * a.nw + d) * dplane] = 0;
+    dst0[((size_t)1 * a.nw + d) * dplane] = 0;
+    dst0[((size_t)2 * a.nw + d) * dplane] = 0;
+  }
+  for (int d = 0; d < a.nw_src; ++d) {
+    const int32_t hi_re = fx_digit_get(re, a.src_count, sidx, q0 + d + 1, top_re);
+    const int32_t hi_im = fx_digit_get(im, a.src_count, sidx, q0 + d + 1, top_im);
+    int32_t wr = sh ? (((lo_re >> sh) | (hi_re << (DB - sh))) & DMASK) : lo_re;
+    int32_t wi = sh ? (((lo_im >> sh) | (hi_im << (DB - sh))) & DMASK) : lo_im;
+    lo_re = hi_re;
+    lo_im = hi_im;
+    const bool last = d == a.nw_src - 1;
+    if (last) {  // signed top digit of the window
+      if (neg_re) wr -= (1 << DB);
+      if (neg_im) wi -= (1 << DB);
+    }
+    if (a.transpose) wi = -wi;  // conjugate (window-level negate; the dropped low bits only move the truncation)
+    int64_t v[3];
+    if (a.side == 0) { v[0] = (int64_t)wr + wi; v[1] = wr; v[2] = wi; }
+    else             { v[0] = wr; v[1] = (int64_t)wi - wr; v[2] = (int64_t)wr + wi; }
+#pragma unroll
+    for (int pl = 0; pl < 3; ++pl) {
+      int64_t t = v[pl] + carry[pl];
+      int64_t out;
+      if (!last) {
+        int64_t cy = (t + DHALF) >> DB;
+        out = t - (cy << DB);
+        carry[pl] = cy;
+      } else {
+        out = t;
+        if (t < -(DHALF) || t > DHALF) bad = true;  // does not fit the window with the 3M headroom
+      }
+      dst0[((size_t)pl * a.nw + pad + d) * dplane] = (int32_t)out;
+    }
+  }
+  // bits above the window must be sign extension
+  {
+    const int tb = lsb + a.nw_src * DB;  // == top_bit
+    int q = tb >= 0 ? tb / DB : -((-tb + DB - 1) / DB);
+    const int s2 = tb - q * DB;
+    for (; q <= kND + 1; ++q) {
+      int32_t dr = fx_digit_get(re, a.src_count, sidx, q, top_re), di = fx_digit_get(im, a.src_count, sidx, q, top_im);
+      int32_t fr = neg_re ? DMASK : 0, fi = neg_im ? DMASK : 0;
+      int32_t mask = (q == (tb >= 0 ? tb / DB : -((-tb + DB - 1) / DB))) ? ((DMASK >> s2) << s2) : DMASK;
+      if (((dr ^ fr) & mask) || ((di ^ fi) & mask)) bad = true;
+    }
+  }
+  if (bad && a.err_flag) atomicOr(a.err_flag, 1);
+}
+
+// ---- combine ------------------------------------------------------------------------------------------------------
+
+struct CombineArgs {
+  const int32_t* raw;  // [split][3*batch][nc][M*N]
+  int32_t* dst;        // complex FX, batch*M*N
+  size_t mn;           // M*N
+  int batch, nc, nsplit;
+  int base_bit;        // FX bit position of raw column 0's LSB (may be negative)
+  int cut_bit;         // clear result bits below this FX bit (<= 0: none)
+  int mode;            // GemmMode
+  int* msb_out;
+};
+
+// one thread per (element, part); part 0 = Re = k1 - k3, part 1 = Im = k1 + k2
+__global__ void __launch_bounds__(256) combine_kernel(CombineArgs a) {
+  const size_t tot = a.mn * a.batch;
+  const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int part = blockIdx.y;
+  if (e >= tot) return;
+  const int b = (int)(e / a.mn);
+  const size_t ij = e % a.mn;
+  const int G = 3 * a.batch;
+  const size_t colstride = a.mn;
+  const size_t gstride = (size_t)a.nc * a.mn;
+  const size_t sstride = (size_t)G * gstride;
+  const int32_t* r1 = a.raw + (size_t)(b * 3 + 0) * gstride + ij;
+  const int32_t* r2 = a.raw + (size_t)(b * 3 + (part == 0 ? 2 : 1)) * gstride + ij;
+  const int sgn2 = part == 0 ? -1 : 1;
+
+  int q = a.base_bit >= 0 ? a.base_bit / DB : -((-a.base_bit + DB - 1) / DB);
+  const int sh = a.base_bit - q * DB;  // 0..27
+  int32_t* dst = a.dst + (part ? (size_t)kND * tot : 0) + e;
+
+  int64_t cy = 0;   // carry of the raw-column normalisation
+  int64_t cy2 = 0;  // carry of the destination addition
+  int msb_pos = 0, msb_neg = 0;  // candidates for the result's msb (if it ends up >= 0 / < 0)
+  const int cutq = a.cut_bit > 0 ? a.cut_bit / DB : 0, cutr = a.cut_bit > 0 ? a.cut_bit % DB : 0;
+
+  auto col = [&](int c) -> int64_t {
+    int64_t s1 = 0, s2 = 0;
+    for (int s = 0; s < a.nsplit; ++s) {
+      s1 += r1[(size_t)s * sstride + (size_t)c * colstride];
+      s2 += r2[(size_t)s * sstride + (size_t)c * colstride];
+    }
+    return (s1 + sgn2 * s2) << sh;
+  };
+  for (int c = 0;; ++c) {
+    const int k = q + c;
+    if (k > kND - 1) break;
+    int64_t v = cy + (c < a.nc ? col(c) : 0);
+    int32_t digit;
+    if (k < kND - 1) {
+      cy = v >> DB;
+      digit = (int32_t)(v & DMASK);
+    } else {
+      // everything that is left lands in the signed top digit (higher raw columns are sign extension unless the
+      // result overflows FX, which the callers' magnitude bounds exclude)
+      if (c + 1 < a.nc) v += col(c + 1) << DB;
+      digit = (int32_t)v;
+      cy = 0;
+    }
+    if (k < 0) continue;
+    if (k < cutq) digit = 0;
+    else if (k == cutq && cutr) digit &= ~((1 << cutr) - 1);
+    if (k < kND - 1) {
+      if (digit != 0) msb_pos = k * DB + (32 - __clz(digit));
+      if (digit != DMASK) msb_neg = k * DB + (32 - __clz((~digit) & DMASK));
+    } else {
+      if (digit > 0) msb_pos = k * DB + (32 - __clz(digit));
+      if (digit < -1) msb_neg = k * DB + (32 - __clz(~digit));
+      if (a.msb_out) atomicMax(a.msb_out, digit < 0 ? msb_neg : msb_pos);
+    }
+    int32_t* dp = dst + (size_t)k * tot;
+    if (a.mode == 0) {
+      *dp = digit;
+    } else {
+      int64_t t = (int64_t)*dp + (a.mode == 1 ? (int64_t)digit : -(int64_t)digit) + cy2;
+      if (k < kND - 1) {
+        cy2 = t >> DB;
+        *dp = (int32_t)(t & DMASK);
+      } else {
+        *dp = (int32_t)t;
+      }
+    }
+  }
+  // digits below the first written one (q > 0) are untouched in Add/Sub mode and must be zero in Assign mode
+  if (a.mode == 0)
+    for (int kk = 0; kk < q && kk < kND; ++kk) dst[(size_t)kk * tot] = 0;
+}
+
+// ---- host side ----------------------------------------------------------------------------------------------------
+
+static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+static int pick_splits(int M, int N, int K, int batch) {
+  const long tiles = (long)((M + GT - 1) / GT) * ((N + GT - 1) / GT) * 3 * batch;
+  const int want = options().min_split_ctas;
+  if (tiles >= want) return 1;
+  int s = (int)((want + tiles - 1) / tiles);
+  const int kmax = (K + GT - 1) / GT;
+  if (s > kmax) s = kmax;
+  if (s > 32) s = 32;
+  return s < 1 ? 1 : s;
+}
+
+size_t gemm_workspace_bytes(int M, int N, int K, int batch) {
+  const size_t pc = align_up(sizeof(int32_t) * 3 * (size_t)batch * kND * M * K);
+  const size_t qc = align_up(sizeof(int32_t) * 3 * (size_t)batch * kND * K * N);
+  const int sp = pick_splits(M, N, K, batch);
+  const size_t raw = align_up(sizeof(int32_t) * (size_t)sp * 3 * batch * (2 * kND + 3) * M * N);
+  return pc + qc + raw;
+}
+
+uint64_t gemm_complex_macs(int M, int N, int K, int batch, int nwP, int nwQ, int* inst_np, int* inst_nq) {
+  const GemmInstance* in = pick_instance(nwP, nwQ);
+  if (!in) return 0;
+  if (inst_np) *inst_np = in->np;
+  if (inst_nq) *inst_nq = in->nq;
+  return inst_cost(*in) * 3ull * (uint64_t)batch * M * N * K;
+}
+
+int gemm_complex(int M, int N, int K, int batch, const GemmSide& P, const GemmSide& Q, int32_t* dst_fx, GemmMode mode,
+                 int out_cut_bit, int /*path*/, void* workspace, size_t workspace_bytes, int* err_flag, int* msb_out,
+                 cudaStream_t stream) {
+  if (M < 1 || N < 1 || K < 1 || batch < 1 || P.nw < 1 || Q.nw < 1 || P.nw > kND || Q.nw > kND) return ZKD_ERR_INVALID_ARG;
+  // the instance needs NQ <= NP roles only through its truncation rule; pad whichever side is short
+  const GemmInstance* in = pick_instance(P.nw, Q.nw);
+  if (!in) return ZKD_ERR_INTERNAL;
+  if (workspace_bytes < gemm_workspace_bytes(M, N, K, batch)) return ZKD_ERR_WORKSPACE;
+  char* w = (char*)workspace;
+  int32_t* Pc = (int32_t*)w;
+  w += align_up(sizeof(int32_t) * 3 * (size_t)batch * kND * M * K);
+  int32_t* Qc = (int32_t*)w;
+  w += align_up(sizeof(int32_t) * 3 * (size_t)batch * kND * K * N);
+  int32_t* raw = (int32_t*)w;
+
+  // operand windows, padded at the LOW end up to the instance's digit counts
+  const int lsbP = P.top_bit - DB * in->np, lsbQ = Q.top_bit - DB * in->nq;
+  {
+    PrepArgs pa{};
+    pa.src = P.fx; pa.dst = Pc; pa.src_count = (size_t)batch * M * K; pa.R = M; pa.C = K; pa.batch = batch;
+    pa.transpose = P.conj_transpose ? 1 : 0; pa.side = 0; pa.lsb_bit = lsbP; pa.nw = in->np; pa.nw_src = P.nw; pa.err_flag = err_flag;
+    const size_t tot = (size_t)batch * M * K;
+    prep_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(pa);
+    count_launch();
+  }
+  {
+    PrepArgs pa{};
+    pa.src = Q.fx; pa.dst = Qc; pa.src_count = (size_t)batch * K * N; pa.R = K; pa.C = N; pa.batch = batch;
+    pa.transpose = 0; pa.side = 1; pa.lsb_bit = lsbQ; pa.nw = in->nq; pa.nw_src = Q.nw; pa.err_flag = err_flag;
+    const size_t tot = (size_t)batch * K * N;
+    prep_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(pa);
+    count_launch();
+  }
+  const int nsplit = pick_splits(M, N, K, batch);
+  int ksplit = (K + nsplit - 1) / nsplit;
+  ksplit = (ksplit + GT - 1) / GT * GT;
+  const int nsp = (K + ksplit - 1) / ksplit;
+  GemmKArgs ka{};
+  ka.P = Pc; ka.Q = Qc; ka.Out = raw;
+  ka.p_dstride = (size_t)M * K; ka.p_gstride = (size_t)in->np * M * K;
+  ka.q_dstride = (size_t)K * N; ka.q_gstride = (size_t)in->nq * K * N;
+  ka.M = M; ka.N = N; ka.K = K; ka.G = 3 * batch; ka.ksplit = ksplit; ka.nsplit = nsp;
+  dim3 grid((N + GT - 1) / GT, (M + GT - 1) / GT, (unsigned)(3 * batch * nsp));
+  if (in->launch(ka, grid, stream) != cudaSuccess) return ZKD_ERR_CUDA;
+  count_launch();
+  count_macs(inst_cost(*in) * 3ull * (uint64_t)batch * M * N * K);
+
+  CombineArgs ca{};
+  ca.raw = raw; ca.dst = dst_fx; ca.mn = (size_t)M * N; ca.batch = batch; ca.nc = in->nc; ca.nsplit = nsp;
+  ca.base_bit = lsbP + lsbQ + DB * in->low - kFRAC;
+  ca.cut_bit = out_cut_bit; ca.mode = (int)mode; ca.msb_out = msb_out;
+  const size_t tot = (size_t)batch * M * N;
+  combine_kernel<<<dim3((unsigned)((tot + 255) / 256), 2), 256, 0, stream>>>(ca);
+  count_launch();
+  return launch_check();
+}
+
+}  // namespace zkd

@@ -1,0 +1,107 @@
+// gemm_digits.cuh — the IMAD digit GEMM kernel template (S4a / S4d / S4e of SURVEY.md section 8(a)).
+//
+// Computes, for every plane g (3 real products of the 3M complex scheme x batch), the exact integer product
+//     S[g][i][j] = sum_k P[g][i][k] * Q[g][k][j]
+// of matrices whose entries are short multi-digit integers: NP (resp. NQ) balanced radix-2^28 digits in int32
+// words, digit-major planes.  Every digit product is one IMAD.WIDE into a 64-bit column accumulator
+// (column c = i_digit + j_digit); products whose column lies below LOW = NQ - 2 are skipped (truncated product:
+// their total is < 2^-17 of the lowest kept column after the guard column is dropped by the caller).
+// Carries are resolved once per 16-deep K tile, off the multiply loop.
+//
+// Roofline: compute-bound on the integer-multiply pipe (64 IMAD.WIDE / clk / SM measured); operands are staged
+// through shared memory, each tile word is reused by 16 threads.
+#pragma once
+#include "fx.cuh"
+
+namespace zkd {
+
+constexpr int GT = 16;  // output tile is GT x GT, K tile is GT deep
+
+template <int NP, int NQ>
+struct GemmShape {
+  static constexpr int LOW = NQ >= 2 ? NQ - 2 : 0;
+  static constexpr int NC = NP + NQ + 1 - LOW;  // kept columns LOW .. NP+NQ
+  static constexpr size_t SMEM = sizeof(int32_t) * (NP + NQ) * GT * GT;
+};
+
+struct GemmKArgs {
+  const int32_t* P;  // [g][d][M][K]
+  const int32_t* Q;  // [g][d][K][N]
+  int32_t* Out;      // [split][g][c][M][N]
+  size_t p_gstride, p_dstride, q_gstride, q_dstride;
+  int M, N, K, G, ksplit, nsplit;
+};
+
+template <int NP, int NQ>
+__global__ void __launch_bounds__(GT * GT) gemm_digits_kernel(GemmKArgs a) {
+  using S = GemmShape<NP, NQ>;
+  extern __shared__ int32_t smem[];
+  int32_t* Ps = smem;                    // [NP][GT][GT]   (i, k)
+  int32_t* Qs = smem + NP * GT * GT;     // [NQ][GT][GT]   (k, j)
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  const int g = blockIdx.z / a.nsplit, sp = blockIdx.z % a.nsplit;
+  const int i0 = blockIdx.y * GT, j0 = blockIdx.x * GT;
+  const int kbeg = sp * a.ksplit, kend = min(a.K, kbeg + a.ksplit);
+  const int32_t* Pg = a.P + (size_t)g * a.p_gstride;
+  const int32_t* Qg = a.Q + (size_t)g * a.q_gstride;
+
+  int64_t acc[S::NC];
+#pragma unroll
+  for (int c = 0; c < S::NC; ++c) acc[c] = 0;
+
+  for (int k0 = kbeg; k0 < kend; k0 += GT) {
+    // stage the tiles: thread (ty,tx) loads P[i0+ty][k0+tx] and Q[k0+ty][j0+tx] for every digit
+    {
+      const bool pin = (i0 + ty) < a.M && (k0 + tx) < kend;
+      const bool qin = (k0 + ty) < kend && (j0 + tx) < a.N;
+      const size_t po = (size_t)(i0 + ty) * a.K + (k0 + tx);
+      const size_t qo = (size_t)(k0 + ty) * a.N + (j0 + tx);
+#pragma unroll
+      for (int d = 0; d < NP; ++d) Ps[(d * GT + ty) * GT + tx] = pin ? Pg[(size_t)d * a.p_dstride + po] : 0;
+#pragma unroll
+      for (int d = 0; d < NQ; ++d) Qs[(d * GT + ty) * GT + tx] = qin ? Qg[(size_t)d * a.q_dstride + qo] : 0;
+    }
+    __syncthreads();
+#pragma unroll 1
+    for (int kk = 0; kk < GT; ++kk) {
+      int32_t p[NP], q[NQ];
+#pragma unroll
+      for (int d = 0; d < NQ; ++d) q[d] = Qs[(d * GT + kk) * GT + tx];
+#pragma unroll
+      for (int d = 0; d < NP; ++d) p[d] = Ps[(d * GT + ty) * GT + kk];
+      mac_cols<NP, NQ, S::LOW, S::NC, false>(acc, p, q);
+    }
+    carry_balanced(acc);  // <= 16 * min(NP,NQ) products of <= 2^54 per column since the last ripple: < 2^63
+    __syncthreads();
+  }
+  if (i0 + ty < a.M && j0 + tx < a.N) {
+    const size_t mn = (size_t)a.M * a.N;
+    int32_t* o = a.Out + ((size_t)(sp * a.G + g) * S::NC) * mn + (size_t)(i0 + ty) * a.N + (j0 + tx);
+#pragma unroll
+    for (int c = 0; c < S::NC; ++c) o[(size_t)c * mn] = (int32_t)acc[c];
+  }
+}
+
+using GemmLaunchFn = cudaError_t (*)(const GemmKArgs&, dim3 grid, cudaStream_t);
+
+template <int NP, int NQ>
+cudaError_t gemm_digits_launch(const GemmKArgs& a, dim3 grid, cudaStream_t s) {
+  using S = GemmShape<NP, NQ>;
+  static bool attr_done = false;
+  if (!attr_done) {
+    if (S::SMEM > 48 * 1024) {
+      cudaError_t e = cudaFuncSetAttribute(gemm_digits_kernel<NP, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::SMEM);
+      if (e != cudaSuccess) return e;
+    }
+    attr_done = true;
+  }
+  gemm_digits_kernel<NP, NQ><<<grid, dim3(GT, GT), S::SMEM, s>>>(a);
+  return cudaGetLastError();
+}
+
+struct GemmInstance {
+  int np, nq, low, nc;
+  GemmLaunchFn launch;
+};
+
+}  // namespace zkd

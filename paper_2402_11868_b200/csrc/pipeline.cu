@@ -1,0 +1,313 @@
+// pipeline.cu — host driver of the hot path: S0 ingest, then per level S1 seed -> S2 clusters -> S3 init ->
+// S4 refinement loop -> S5 cluster Rayleigh-Ritz (by recursion on the projected cluster matrices), and S6 export.
+//
+// The refinement ("Rayleigh quotient iteration ... to recover the
+// precision"), written for all eigenpairs at once with the current iterate as the preconditioner basis (S4g taken
+// every step, at a precision that doubles with the residual):
+//     G_c = X_c^H X_c ;  X_c, W_c <- (X_c, W_c)(I + (I - G_c)/2)            orthonormalise inside clusters (S4f)
+//     S_c = X_c^H W_c ;  theta_j = Re (S_c)_jj                               Rayleigh quotients (S4c)
+//     R_c = W_c - X_c S_c                                                    block residual (S4c)
+//     C = X^H R ;  E_ij = C_ij / (theta_j - theta_i), 0 inside a cluster     correction equation, deflated (S4d)
+//     T = X E ;  X <- X + T ;  W <- W + A T                                  update; W = A X kept incrementally (S4e, S4a)
+// Every product is a windowed digit GEMM: only the bits of R, E, T that matter at the current residual level take
+// part, and W = A X is never recomputed from scratch.  Exact solution of the correction equation is an RQI step;
+// with the basis equal to the iterate the error squares each step (50 -> 100 -> 200 -> 400 -> 800 bits).
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <map>
+#include <vector>
+
+#include "blocks.h"
+
+namespace zkd {
+
+namespace {
+
+struct Arena {
+  char* base = nullptr;
+  size_t size = 0, off = 0;
+  void* alloc(size_t bytes) {
+    const size_t a = (off + 255) / 256 * 256;
+    if (a + bytes > size) return nullptr;
+    off = a + bytes;
+    return base + a;
+  }
+  template <typename T>
+  T* get(size_t n) { return (T*)alloc(sizeof(T) * n); }
+};
+
+enum { S_ERR = 0, S_MSB_R = 1, S_MSB_G = 2, S_MSB_E = 3, S_MSB_T = 4, S_NUM = 8 };
+
+struct Ctx {
+  cudaStream_t s;
+  Arena ar;
+  void* gemm_ws;
+  size_t gemm_ws_bytes;
+  int* h_pin;  // pinned host staging, >= 4096 ints
+};
+
+struct LevelStats {
+  int steps = 0, status = 0, msb_r = 0, msb_g = 0;
+  std::vector<int> cl_stats;  // level 0 only: [nb][2]
+};
+
+int* pinned_staging() {
+  static thread_local int* p = nullptr;
+  if (!p) {
+    if (cudaMallocHost((void**)&p, sizeof(int) * 65536) != cudaSuccess) {
+      (void)cudaGetLastError();
+      p = nullptr;
+    }
+  }
+  return p;
+}
+
+inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
+inline int ilog2_ceil(int n) { int l = 0; while ((1 << l) < n) ++l; return l; }
+
+int read_scalars(Ctx& c, const int* dev, int n, int* out) {
+  ZKD_CUDA_TRY(cudaMemcpyAsync(c.h_pin, dev, sizeof(int) * n, cudaMemcpyDeviceToHost, c.s));
+  ZKD_CUDA_TRY(cudaStreamSynchronize(c.s));
+  for (int i = 0; i < n; ++i) out[i] = c.h_pin[i];
+  return ZKD_OK;
+}
+
+int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* lam, int depth, const int* noise, LevelStats* st) {
+  const Options& opt = options();
+  const size_t cnt = (size_t)n * n * nb;
+  const size_t fxc = FxC::bytes(cnt);
+  const size_t mark0 = c.ar.off;
+  cudaStream_t s = c.s;
+  if (depth > 48) return ZKD_ERR_INTERNAL;
+
+  // long-lived (needed by S5)
+  int* cl = c.ar.get<int>((size_t)n * nb);
+  int* cle = c.ar.get<int>((size_t)n * nb);
+  int* stats = c.ar.get<int>((size_t)2 * nb);
+  int32_t* Sm = (int32_t*)c.ar.alloc(fxc);
+  int32_t* theta = lam;
+  const size_t mark1 = c.ar.off;
+  // short-lived
+  double2* A64 = c.ar.get<double2>(cnt);
+  double* mu = c.ar.get<double>((size_t)n * nb);
+  double2* V = c.ar.get<double2>(cnt);
+  int32_t* W = (int32_t*)c.ar.alloc(fxc);
+  int32_t* R = (int32_t*)c.ar.alloc(fxc);
+  int32_t* Cm = (int32_t*)c.ar.alloc(fxc);
+  int32_t* T = (int32_t*)c.ar.alloc(fxc);
+  int32_t* Gm = (int32_t*)c.ar.alloc(fxc);
+  int* scal = c.ar.get<int>(S_NUM);
+  if (!cl || !cle || !stats || !Sm || !A64 || !mu || !V || !W || !R || !Cm || !T || !Gm || !scal) return ZKD_ERR_WORKSPACE;
+  if (gemm_workspace_bytes(n, n, n, nb) > c.gemm_ws_bytes) return ZKD_ERR_WORKSPACE;
+
+  // S1-S3
+  ZKD_TRY(fxc_to_c64(cnt, A, A64, s));
+  ZKD_TRY(seed_fp64(n, nb, (const double*)A64, mu, (double*)V, opt.seed_sweeps, s));
+  ZKD_TRY(cluster_detect(n, nb, A64, mu, opt.tau_bits, cl, cle, stats, s));
+  int32_t* Xc = X;  // current iterate (may end up in T's storage; copied back at the end)
+  int32_t* Tc = T;
+  int32_t* Wc = W;
+  int32_t* Cc = Cm;
+  ZKD_TRY(init_x(cnt, V, Xc, s));
+  ZKD_CUDA_TRY(cudaMemsetAsync(scal, 0, sizeof(int) * S_NUM, s));
+
+  const int topA = 812, topX = 815;
+  auto side = [&](const int32_t* fx, int top, int nw, bool ct) {
+    GemmSide g;
+    g.fx = fx; g.rows = n; g.cols = n; g.conj_transpose = ct; g.top_bit = top; g.nw = std::max(1, std::min(nw, kND));
+    return g;
+  };
+  // W = A X0 : X0 has digits 27..29 only
+  ZKD_TRY(gemm_complex(n, n, n, nb, side(A, topA, kND, false), side(Xc, topX, 3, false), Wc, GemmMode::Assign, -1, opt.gemm_path,
+                       c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s));
+
+  std::vector<int> h_cl;
+  int status = 2, steps = 0, prev_msb_r = 1 << 30;
+  int hs[S_NUM];
+  const int tol_msb = 812 - opt.tol_bits;
+  for (int step = 0; step < opt.max_steps; ++step) {
+    // S4f: orthonormalise inside clusters (Newton-Schulz step on the cluster Gram blocks)
+    ZKD_TRY(gram_blocks(n, nb, Xc, Xc, cl, Gm, s));
+    ZKD_TRY(ns_build(n, nb, cl, Gm, scal + S_MSB_G, s));
+    ZKD_TRY(block_apply(n, nb, Xc, Xc, Gm, cl, cle, false, Tc, nullptr, s));
+    ZKD_TRY(block_apply(n, nb, Wc, Wc, Gm, cl, cle, false, Cc, nullptr, s));
+    std::swap(Xc, Tc);
+    std::swap(Wc, Cc);
+    // S4c: Rayleigh quotients and block residual
+    ZKD_TRY(gram_blocks(n, nb, Xc, Wc, cl, Sm, s));
+    ZKD_TRY(theta_from_diag(n, nb, Sm, theta, s));
+    ZKD_TRY(block_apply(n, nb, Wc, Xc, Sm, cl, cle, true, R, scal + S_MSB_R, s));
+    if (step == 0) {
+      h_cl.resize((size_t)n * nb);
+      ZKD_CUDA_TRY(cudaMemcpyAsync(h_cl.data(), cl, sizeof(int) * n * nb, cudaMemcpyDeviceToHost, s));
+      if (st && depth == 0) {
+        st->cl_stats.resize((size_t)2 * nb);
+        ZKD_CUDA_TRY(cudaMemcpyAsync(st->cl_stats.data(), stats, sizeof(int) * 2 * nb, cudaMemcpyDeviceToHost, s));
+      }
+    }
+    ZKD_TRY(read_scalars(c, scal, S_NUM, hs));
+    const int msb_r = hs[S_MSB_R], msb_g = hs[S_MSB_G];
+    if (opt.verbose) fprintf(stderr, "[zkd] depth %d n %d nb %d step %d: msbR %d (2^%d) msbG %d err %d\n", depth, n, nb, step, msb_r, msb_r - 812, msb_g, hs[S_ERR]);
+    if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
+    steps = step;
+    if (st) { st->msb_r = msb_r; st->msb_g = msb_g; }
+    if (msb_r <= tol_msb && msb_g <= 812 - 400) { status = 0; break; }
+    if (step > 0 && msb_r > tol_msb && msb_r >= prev_msb_r - 2 && msb_g <= 812 - 400) { status = 1; break; }
+    if (step + 1 == opt.max_steps) break;
+    prev_msb_r = msb_r;
+    ZKD_CUDA_TRY(cudaMemsetAsync(scal, 0, sizeof(int) * S_NUM, s));
+    if (msb_r == 0) continue;  // residual exactly zero: only the orthonormalisation is still converging
+
+    // S4d: C = X^H R on windows sized for this step's gain
+    const int e = 812 - msb_r;                        // residual ~ 2^-e
+    const int pb = std::max(40, std::min(e + 40, msb_r + 30));  // relative bits worth computing for the correction
+    const int nwX = ceil_div(pb + 3, 28);
+    const int topR = msb_r + 2, nwR = ceil_div(pb + 2, 28);
+    ZKD_TRY(gemm_complex(n, n, n, nb, side(Xc, topX, nwX, true), side(R, topR, nwR, false), Cc, GemmMode::Assign, -1, opt.gemm_path,
+                         c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s));
+    ZKD_TRY(ecalc(n, nb, theta, cl, Cc, pb + 8, scal + S_MSB_E, scal + S_ERR, s));
+    ZKD_TRY(read_scalars(c, scal, S_NUM, hs));
+    if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
+    const int msb_e = hs[S_MSB_E];
+    if (msb_e == 0) continue;
+    // S4e: T = X E (bits below cutT cleared so that W += A T tracks A X exactly), X += T, W += A T
+    const int topE = msb_e + 2, nwE = ceil_div(pb + 2, 28);
+    const int cutT = std::max(0, msb_e - pb - 4);
+    ZKD_TRY(gemm_complex(n, n, n, nb, side(Xc, topX, nwX, false), side(Cc, topE, nwE, false), Tc, GemmMode::Assign, cutT, opt.gemm_path,
+                         c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s));
+    ZKD_TRY(fxc_add_inplace(cnt, Xc, Tc, s));
+    const int topT = msb_e + ilog2_ceil(n) + 2;
+    const int nwT = ceil_div(topT - cutT, 28);
+    const int nwA = std::min(kND, ceil_div(topT, 28));
+    ZKD_TRY(gemm_complex(n, n, n, nb, side(A, topA, nwA, false), side(Tc, topT, nwT, false), Wc, GemmMode::Add, -1, opt.gemm_path,
+                         c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s));
+  }
+  if (st) { st->steps = steps + 1; st->status = status; }
+  if (Xc != X) ZKD_CUDA_TRY(cudaMemcpyAsync(X, Xc, fxc, cudaMemcpyDeviceToDevice, s));
+
+  // S5: clusters with more than one member -> Rayleigh-Ritz on the projected matrix, by recursion
+  std::map<int, std::vector<SubProblem>> groups;
+  for (int b = 0; b < nb; ++b) {
+    int j = 0;
+    while (j < n) {
+      int k = j;
+      while (k + 1 < n && h_cl[(size_t)b * n + k + 1] == h_cl[(size_t)b * n + j]) ++k;
+      const int m = k - j + 1;
+      if (m > 1) groups[m].push_back(SubProblem{b, j});
+      j = k + 1;
+    }
+  }
+  if (!groups.empty()) {
+    ZKD_CUDA_TRY(cudaStreamSynchronize(s));  // short-lived buffers are about to be reused
+    c.ar.off = mark1;
+    int32_t* Um = (int32_t*)c.ar.alloc(fxc);
+    int32_t* Xn = (int32_t*)c.ar.alloc(fxc);
+    if (!Um || !Xn) return ZKD_ERR_WORKSPACE;
+    ZKD_TRY(identity_blocks(n, nb, Um, s));
+    const size_t mark2 = c.ar.off;
+    bool any = false;
+    for (auto& kv : groups) {
+      const int m = kv.first;
+      const int nsub = (int)kv.second.size();
+      c.ar.off = mark2;
+      SubProblem* subs_dev = c.ar.get<SubProblem>((size_t)nsub);
+      const size_t hc = (size_t)m * m * nsub;
+      int32_t* H = (int32_t*)c.ar.alloc(FxC::bytes(hc));
+      int32_t* U = (int32_t*)c.ar.alloc(FxC::bytes(hc));
+      int32_t* cbar = (int32_t*)c.ar.alloc(FxR::bytes((size_t)nsub));
+      int32_t* lam_sub = (int32_t*)c.ar.alloc(FxR::bytes((size_t)nsub * m));
+      int* kshift = c.ar.get<int>((size_t)nsub);
+      int* degen = c.ar.get<int>((size_t)nsub);
+      int* noise_sub = c.ar.get<int>((size_t)nsub);
+      if (!subs_dev || !H || !U || !cbar || !lam_sub || !kshift || !degen || !noise_sub) return ZKD_ERR_WORKSPACE;
+      ZKD_CUDA_TRY(cudaMemcpyAsync(subs_dev, kv.second.data(), sizeof(SubProblem) * nsub, cudaMemcpyHostToDevice, s));
+      ZKD_TRY(sub_gather(n, nb, m, nsub, subs_dev, Sm, H, cbar, kshift, degen, tol_msb + 6, noise, noise_sub, s));
+      std::vector<int> hdeg((size_t)nsub);
+      ZKD_CUDA_TRY(cudaMemcpyAsync(hdeg.data(), degen, sizeof(int) * nsub, cudaMemcpyDeviceToHost, s));
+      ZKD_CUDA_TRY(cudaStreamSynchronize(s));
+      bool all_deg = true;
+      for (int v : hdeg) all_deg = all_deg && v;
+      if (all_deg) continue;
+      LevelStats sub;
+      ZKD_TRY(solve_level(c, m, nsub, H, U, lam_sub, depth + 1, noise_sub, &sub));
+      if (st && sub.status > st->status) st->status = sub.status;
+      ZKD_TRY(sub_scatter(n, nb, m, nsub, subs_dev, U, lam_sub, cbar, kshift, degen, Um, theta, s));
+      any = true;
+    }
+    if (any) {
+      ZKD_TRY(block_apply(n, nb, nullptr, X, Um, cl, cle, false, Xn, nullptr, s));
+      ZKD_CUDA_TRY(cudaMemcpyAsync(X, Xn, fxc, cudaMemcpyDeviceToDevice, s));
+    }
+    ZKD_CUDA_TRY(cudaStreamSynchronize(s));
+  }
+  c.ar.off = mark0;
+  return ZKD_OK;
+}
+
+__global__ void info_kernel(int batch, const int* __restrict__ status_in, int level_status, int steps, int msb_r, int msb_g,
+                            const int* __restrict__ cl_stats, zkd_info* __restrict__ info) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= batch) return;
+  zkd_info o;
+  o.status = status_in[b] ? 3 : level_status;
+  o.steps = steps;
+  o.n_clusters = cl_stats ? cl_stats[2 * b] : 0;
+  o.max_cluster = cl_stats ? cl_stats[2 * b + 1] : 0;
+  o.log2_resid = (float)(msb_r - 812);
+  o.log2_orth = (float)(msb_g - 812);
+  info[b] = o;
+}
+
+size_t level_bytes(int N, int batch) {
+  const size_t cnt = (size_t)N * N * batch;
+  return 12 * (FxC::bytes(cnt) + 4096) + 3 * 16 * cnt + 64 * (size_t)N * batch + (1 << 20);
+}
+
+}  // namespace
+
+size_t diag_workspace_bytes(int N, int batch) {
+  return level_bytes(N, batch) + gemm_workspace_bytes(N, N, N, batch) + (32u << 20);
+}
+
+int diag_herm_device(int N, int batch, const void* A_api, void* eigvals_api, void* eigvecs_api, void* ws, size_t ws_bytes,
+                     zkd_info* info, cudaStream_t s) {
+  Ctx c;
+  c.s = s;
+  c.ar.base = (char*)ws;
+  c.ar.size = ws_bytes;
+  c.h_pin = pinned_staging();
+  if (!c.h_pin) return ZKD_ERR_CUDA;
+  c.gemm_ws_bytes = gemm_workspace_bytes(N, N, N, batch) + (32u << 20);
+  c.gemm_ws = c.ar.alloc(c.gemm_ws_bytes);
+  const size_t cnt = (size_t)N * N * batch;
+  int32_t* A = (int32_t*)c.ar.alloc(FxC::bytes(cnt));
+  int32_t* X = (int32_t*)c.ar.alloc(FxC::bytes(cnt));
+  int32_t* lam = (int32_t*)c.ar.alloc(FxR::bytes((size_t)N * batch));
+  int32_t* lam_sorted = (int32_t*)c.ar.alloc(FxR::bytes((size_t)N * batch));
+  int* scale = c.ar.get<int>((size_t)batch);
+  int* status = c.ar.get<int>((size_t)batch);
+  int* rank = c.ar.get<int>((size_t)N * batch);
+  int* cl_stats_dev = c.ar.get<int>((size_t)2 * batch);
+  if (!c.gemm_ws || !A || !X || !lam || !lam_sorted || !scale || !status || !rank || !cl_stats_dev) return ZKD_ERR_WORKSPACE;
+
+  ZKD_TRY(ingest_herm(N, batch, A_api, A, scale, status, s));
+  LevelStats st;
+  ZKD_TRY(solve_level(c, N, batch, A, X, lam, 0, nullptr, &st));
+  ZKD_TRY(finalize_export(N, batch, X, lam, scale, eigvals_api, eigvecs_api, A /* scratch: A is dead */, lam_sorted, rank, s));
+  if (info) {
+    const int* cs = nullptr;
+    if (!st.cl_stats.empty()) {
+      ZKD_CUDA_TRY(cudaMemcpyAsync(cl_stats_dev, st.cl_stats.data(), sizeof(int) * 2 * batch, cudaMemcpyHostToDevice, s));
+      cs = cl_stats_dev;
+    }
+    info_kernel<<<(batch + 127) / 128, 128, 0, s>>>(batch, status, st.status, st.steps, st.msb_r, st.msb_g, cs, info);
+    count_launch();
+    ZKD_TRY(launch_check());
+    // st.cl_stats must outlive the async copy
+    ZKD_CUDA_TRY(cudaStreamSynchronize(s));
+  }
+  return ZKD_OK;
+}
+
+}  // namespace zkd

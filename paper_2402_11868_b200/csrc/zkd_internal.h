@@ -1,0 +1,106 @@
+// zkd_internal.h — declarations shared between the translation units of libzkd (not part of the public ABI).
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "../../include/zkd.h"
+
+namespace zkd {
+
+constexpr int kND = ZKD_FX_DIGITS;   // 30
+constexpr int kDB = 28;
+constexpr int kFRAC = ZKD_FX_FRAC_BITS;
+constexpr int kFxBits = kND * kDB;   // 840 (the top digit really has 32 bits)
+constexpr int kPrec = 768;
+constexpr int kApiRealBytes = 16 + kPrec / 8;  // 112
+
+// ---- error plumbing ---------------------------------------------------------------------------------------------
+#define ZKD_CUDA_TRY(expr)                         \
+  do {                                             \
+    cudaError_t _e = (expr);                       \
+    if (_e != cudaSuccess) {                       \
+      (void)cudaGetLastError();                    \
+      return ZKD_ERR_CUDA;                         \
+    }                                              \
+  } while (0)
+#define ZKD_TRY(expr)          \
+  do {                         \
+    int _rc = (expr);          \
+    if (_rc != ZKD_OK) return _rc; \
+  } while (0)
+
+void count_launch(uint64_t n = 1);
+void count_macs(uint64_t n);
+inline int launch_check() {
+  cudaError_t e = cudaGetLastError();
+  return e == cudaSuccess ? ZKD_OK : ZKD_ERR_CUDA;
+}
+
+struct Options {
+  int tau_bits = 20;
+  int tol_bits = 770;
+  int max_steps = 40;
+  int gemm_path = 0;
+  int min_split_ctas = 296;
+  int seed_sweeps = 12;
+  int verbose = 0;
+};
+Options& options();
+
+// ---- complex FX matrices in device memory ------------------------------------------------------------------------
+// A complex FX array with `count` elements: int32[2][kND][count] (re planes then im planes).
+struct FxC {
+  int32_t* p = nullptr;
+  size_t count = 0;
+  __host__ __device__ int32_t* re() const { return p; }
+  __host__ __device__ int32_t* im() const { return p + (size_t)kND * count; }
+  static size_t bytes(size_t count) { return sizeof(int32_t) * 2 * kND * count; }
+};
+struct FxR {
+  int32_t* p = nullptr;
+  size_t count = 0;
+  static size_t bytes(size_t count) { return sizeof(int32_t) * kND * count; }
+};
+
+// ---- digit GEMM (gemm_digits.cu) ---------------------------------------------------------------------------------
+// One side of a complex product C = op(P) * Q.  The window of the FX operand that takes part is
+// bits [top_bit - 28*nw, top_bit) (FX bit 0 = 2^-812); bits above must be sign extension (checked on device).
+struct GemmSide {
+  const int32_t* fx = nullptr;  // complex FX array of batch*rows*cols elements, row-major
+  int rows = 0, cols = 0;       // as stored
+  bool conj_transpose = false;  // P only: use A^H (stored K x M)
+  int top_bit = 0;
+  int nw = 0;
+};
+enum class GemmMode : int { Assign = 0, Add = 1, Sub = 2 };
+
+size_t gemm_workspace_bytes(int M, int N, int K, int batch);
+// dst (+)= op(P) * Q ; bits of the product below out_cut_bit are cleared (use a negative value for none).
+// err_flag (device int, may be null) receives bit 1 when an operand does not fit its window.
+// msb_out (device int, may be null): atomicMax of the msb position of |result| elements.
+int gemm_complex(int M, int N, int K, int batch, const GemmSide& P, const GemmSide& Q, int32_t* dst_fx, GemmMode mode,
+                 int out_cut_bit, int path, void* workspace, size_t workspace_bytes, int* err_flag, int* msb_out,
+                 cudaStream_t stream);
+// number of 28x28-bit digit products one call performs (algorithmic, after instance selection)
+uint64_t gemm_complex_macs(int M, int N, int K, int batch, int nwP, int nwQ, int* inst_np, int* inst_nq);
+
+// ---- pipeline pieces --------------------------------------------------------------------------------------------
+int fx_from_api(int count, const void* src_api, int32_t* dst_fx, int scale_bits, cudaStream_t s);
+int fx_to_api(int count, const int32_t* src_fx, void* dst_api, int scale_bits, cudaStream_t s);
+int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int max_sweeps, cudaStream_t s);
+
+size_t diag_workspace_bytes(int N, int batch);
+int diag_herm_device(int N, int batch, const void* A_api, void* eigvals_api, void* eigvecs_api, void* ws, size_t ws_bytes,
+                     zkd_info* info, cudaStream_t s);
+
+}  // namespace zkd
+
+namespace zkd {
+int fx_from_api_scaled(size_t count, const void* src_api, int32_t* dst_fx, int scale_bits, const int* scale_dev,
+                       int scale_stride, size_t per_scale, int* status, cudaStream_t s);
+int fx_to_api_scaled(size_t count, const int32_t* src_fx, void* dst_api, int scale_bits, const int* scale_dev, int scale_stride,
+                     size_t per_scale, cudaStream_t s);
+int fxc_to_api(size_t count, const int32_t* src_fxc, void* dst_api, cudaStream_t s);
+int measure_imad_peak(double millis, double* per_sec, cudaStream_t s);
+}  // namespace zkd
