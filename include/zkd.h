@@ -94,6 +94,13 @@ int zkd_version(void);
 void zkd_counters(uint64_t *kernel_launches, uint64_t *gemm_digit_macs);
 void zkd_counters_reset(void);
 
+/* Per-launch device timing of the dominant kernel (the digit GEMM), for roofline reporting: zkd_kernel_timing(1)
+ * resets and arms it (every digit-GEMM launch is then bracketed by a CUDA event pair on its own stream, up to 16384
+ * launches), zkd_kernel_timing(0) disarms; zkd_kernel_timing_read waits for the recorded events and returns the summed
+ * kernel time in ms, the number of timed launches and the digit products they performed.  Host calls. */
+int zkd_kernel_timing(int enable);
+int zkd_kernel_timing_read(double *gemm_ms, uint64_t *gemm_launches, uint64_t *gemm_digit_macs);
+
 /* ---- host-side helpers (no CUDA): one real between the API layout and (sign, exp, limbs) / double ---- */
 int zkd_pack(void *dst, int prec_bits, int sign, int64_t exp, const uint64_t *limbs_le);
 int zkd_unpack(const void *src, int prec_bits, int *sign, int64_t *exp, uint64_t *limbs_le);

@@ -57,6 +57,8 @@ def lib() -> ctypes.CDLL:
     L.zkd_counters.restype = None
     L.zkd_counters.argtypes = [ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint64)]
     L.zkd_counters_reset.restype = None
+    L.zkd_kernel_timing.argtypes = [ci]
+    L.zkd_kernel_timing_read.argtypes = [ctypes.POINTER(cd), ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint64)]
     L.zkd_pack.argtypes = [vp, ci, ci, ctypes.c_int64, vp]
     L.zkd_unpack.argtypes = [vp, ci, ctypes.POINTER(ci), ctypes.POINTER(ctypes.c_int64), vp]
     L.zkd_from_double.argtypes = [vp, ci, cd]
@@ -124,6 +126,17 @@ def counters() -> tuple[int, int]:
 
 def counters_reset() -> None:
     lib().zkd_counters_reset()
+
+
+def kernel_timing(enable: bool) -> None:
+    _check(lib().zkd_kernel_timing(1 if enable else 0), "zkd_kernel_timing")
+
+
+def kernel_timing_read() -> tuple[float, int, int]:
+    """(summed digit-GEMM kernel time in ms, timed launches, digit products of those launches)"""
+    ms, n, m = ctypes.c_double(), ctypes.c_uint64(), ctypes.c_uint64()
+    _check(lib().zkd_kernel_timing_read(ctypes.byref(ms), ctypes.byref(n), ctypes.byref(m)), "zkd_kernel_timing_read")
+    return ms.value, int(n.value), int(m.value)
 
 
 def diag_herm_bufsize(N: int, batch: int, prec_bits: int = PREC) -> int:

@@ -246,6 +246,14 @@ int zkd_measure_imad_peak(double millis, double* imad_wide_per_sec, void* stream
   return measure_imad_peak(millis, imad_wide_per_sec, (cudaStream_t)stream);
 }
 
+int zkd_kernel_timing(int enable) {
+  kernel_timing_enable(enable != 0);
+  return ZKD_OK;
+}
+int zkd_kernel_timing_read(double* gemm_ms, uint64_t* gemm_launches, uint64_t* gemm_digit_macs) {
+  return kernel_timing_read(gemm_ms, gemm_launches, gemm_digit_macs);
+}
+
 // ---- the hot path -------------------------------------------------------------------------------------------------
 static int check_diag_args(int N, int batch, int prec_bits) {
   if (prec_bits != kPrec) return ZKD_ERR_UNSUPPORTED_PREC;

@@ -243,6 +243,59 @@ __global__ void __launch_bounds__(256) combine_kernel(CombineArgs a) {
 
 // ---- host side ----------------------------------------------------------------------------------------------------
 
+// Optional per-launch timing of the digit GEMM kernel (zkd_kernel_timing): event pairs on the launching stream.
+namespace {
+struct KernelTimer {
+  bool enabled = false;
+  std::vector<cudaEvent_t> ev;   // pairs
+  std::vector<uint64_t> macs;    // per timed launch
+  size_t used = 0;               // pairs used
+  uint64_t untimed = 0;
+};
+KernelTimer g_kt;
+constexpr size_t kMaxTimedLaunches = 16384;
+}  // namespace
+
+void kernel_timing_enable(bool on) {
+  g_kt.enabled = on;
+  g_kt.used = 0;
+  g_kt.untimed = 0;
+  g_kt.macs.clear();
+}
+int kernel_timing_read(double* ms, uint64_t* launches, uint64_t* macs) {
+  double tot = 0;
+  uint64_t m = 0;
+  for (size_t i = 0; i < g_kt.used; ++i) {
+    float t = 0;
+    if (cudaEventSynchronize(g_kt.ev[2 * i + 1]) != cudaSuccess || cudaEventElapsedTime(&t, g_kt.ev[2 * i], g_kt.ev[2 * i + 1]) != cudaSuccess) {
+      (void)cudaGetLastError();
+      return ZKD_ERR_CUDA;
+    }
+    tot += t;
+    m += g_kt.macs[i];
+  }
+  if (ms) *ms = tot;
+  if (launches) *launches = g_kt.used;
+  if (macs) *macs = m;
+  return ZKD_OK;
+}
+static bool kt_begin(cudaStream_t s) {
+  if (!g_kt.enabled) return false;
+  if (g_kt.used >= kMaxTimedLaunches) { ++g_kt.untimed; return false; }
+  while (g_kt.ev.size() < 2 * (g_kt.used + 1)) {
+    cudaEvent_t e;
+    if (cudaEventCreate(&e) != cudaSuccess) { (void)cudaGetLastError(); return false; }
+    g_kt.ev.push_back(e);
+  }
+  cudaEventRecord(g_kt.ev[2 * g_kt.used], s);
+  return true;
+}
+static void kt_end(cudaStream_t s, uint64_t macs) {
+  cudaEventRecord(g_kt.ev[2 * g_kt.used + 1], s);
+  g_kt.macs.push_back(macs);
+  ++g_kt.used;
+}
+
 static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 static int pick_splits(int M, int N, int K, int batch) {
@@ -315,9 +368,12 @@ int gemm_complex(int M, int N, int K, int batch, const GemmSide& P, const GemmSi
   ka.q_dstride = (size_t)K * N; ka.q_gstride = (size_t)in->nq * K * N;
   ka.M = M; ka.N = N; ka.K = K; ka.G = 3 * batch; ka.ksplit = ksplit; ka.nsplit = nsp;
   dim3 grid((N + GT - 1) / GT, (M + GT - 1) / GT, (unsigned)(3 * batch * nsp));
+  const uint64_t nmacs = inst_cost(*in) * 3ull * (uint64_t)batch * M * N * K;
+  const bool timed = kt_begin(stream);
   if (in->launch(ka, grid, stream) != cudaSuccess) return ZKD_ERR_CUDA;
+  if (timed) kt_end(stream, nmacs);
   count_launch();
-  count_macs(inst_cost(*in) * 3ull * (uint64_t)batch * M * N * K);
+  count_macs(nmacs);
 
   CombineArgs ca{};
   ca.raw = raw; ca.dst = dst_fx; ca.mn = (size_t)M * N; ca.batch = batch; ca.nc = in->nc; ca.nsplit = nsp;

@@ -24,17 +24,39 @@ namespace zkd {
 
 namespace {
 
+// Stack allocator over the caller's workspace.  The workspace from zkd_diag_herm_bufsize covers the top level and
+// one full-size level of cluster recursion; deeper recursion (rare: every level must split or shrink its clusters)
+// overflows into the stream-ordered CUDA allocator, released when the level that asked for it returns.
 struct Arena {
   char* base = nullptr;
   size_t size = 0, off = 0;
+  cudaStream_t stream = nullptr;
+  std::vector<void*> overflow;
   void* alloc(size_t bytes) {
     const size_t a = (off + 255) / 256 * 256;
-    if (a + bytes > size) return nullptr;
-    off = a + bytes;
-    return base + a;
+    if (a + bytes <= size) {
+      off = a + bytes;
+      return base + a;
+    }
+    void* p = nullptr;
+    if (cudaMallocAsync(&p, bytes ? bytes : 256, stream) != cudaSuccess) {
+      (void)cudaGetLastError();
+      return nullptr;
+    }
+    overflow.push_back(p);
+    return p;
   }
   template <typename T>
   T* get(size_t n) { return (T*)alloc(sizeof(T) * n); }
+  struct Mark { size_t off, nover; };
+  Mark mark() const { return Mark{off, overflow.size()}; }
+  void release(const Mark& m) {
+    off = m.off;
+    while (overflow.size() > m.nover) {
+      cudaFreeAsync(overflow.back(), stream);
+      overflow.pop_back();
+    }
+  }
 };
 
 enum { S_ERR = 0, S_MSB_R = 1, S_MSB_G = 2, S_MSB_E = 3, S_MSB_T = 4, S_NUM = 8 };
@@ -77,7 +99,7 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
   const Options& opt = options();
   const size_t cnt = (size_t)n * n * nb;
   const size_t fxc = FxC::bytes(cnt);
-  const size_t mark0 = c.ar.off;
+  const Arena::Mark mark0 = c.ar.mark();
   cudaStream_t s = c.s;
   if (depth > 48) return ZKD_ERR_INTERNAL;
 
@@ -87,7 +109,7 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
   int* stats = c.ar.get<int>((size_t)2 * nb);
   int32_t* Sm = (int32_t*)c.ar.alloc(fxc);
   int32_t* theta = lam;
-  const size_t mark1 = c.ar.off;
+  const Arena::Mark mark1 = c.ar.mark();
   // short-lived
   double2* A64 = c.ar.get<double2>(cnt);
   double* mu = c.ar.get<double>((size_t)n * nb);
@@ -200,17 +222,17 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
   }
   if (!groups.empty()) {
     ZKD_CUDA_TRY(cudaStreamSynchronize(s));  // short-lived buffers are about to be reused
-    c.ar.off = mark1;
+    c.ar.release(mark1);
     int32_t* Um = (int32_t*)c.ar.alloc(fxc);
     int32_t* Xn = (int32_t*)c.ar.alloc(fxc);
     if (!Um || !Xn) return ZKD_ERR_WORKSPACE;
     ZKD_TRY(identity_blocks(n, nb, Um, s));
-    const size_t mark2 = c.ar.off;
+    const Arena::Mark mark2 = c.ar.mark();
     bool any = false;
     for (auto& kv : groups) {
       const int m = kv.first;
       const int nsub = (int)kv.second.size();
-      c.ar.off = mark2;
+      c.ar.release(mark2);
       SubProblem* subs_dev = c.ar.get<SubProblem>((size_t)nsub);
       const size_t hc = (size_t)m * m * nsub;
       int32_t* H = (int32_t*)c.ar.alloc(FxC::bytes(hc));
@@ -241,7 +263,7 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
     }
     ZKD_CUDA_TRY(cudaStreamSynchronize(s));
   }
-  c.ar.off = mark0;
+  c.ar.release(mark0);
   return ZKD_OK;
 }
 
@@ -267,7 +289,7 @@ size_t level_bytes(int N, int batch) {
 }  // namespace
 
 size_t diag_workspace_bytes(int N, int batch) {
-  return level_bytes(N, batch) + gemm_workspace_bytes(N, N, N, batch) + (32u << 20);
+  return 2 * level_bytes(N, batch) + gemm_workspace_bytes(N, N, N, batch) + (32u << 20);
 }
 
 int diag_herm_device(int N, int batch, const void* A_api, void* eigvals_api, void* eigvecs_api, void* ws, size_t ws_bytes,
@@ -276,6 +298,7 @@ int diag_herm_device(int N, int batch, const void* A_api, void* eigvals_api, voi
   c.s = s;
   c.ar.base = (char*)ws;
   c.ar.size = ws_bytes;
+  c.ar.stream = s;
   c.h_pin = pinned_staging();
   if (!c.h_pin) return ZKD_ERR_CUDA;
   c.gemm_ws_bytes = gemm_workspace_bytes(N, N, N, batch) + (32u << 20);
@@ -293,7 +316,13 @@ int diag_herm_device(int N, int batch, const void* A_api, void* eigvals_api, voi
 
   ZKD_TRY(ingest_herm(N, batch, A_api, A, scale, status, s));
   LevelStats st;
-  ZKD_TRY(solve_level(c, N, batch, A, X, lam, 0, nullptr, &st));
+  {
+    const int rc = solve_level(c, N, batch, A, X, lam, 0, nullptr, &st);
+    if (rc != ZKD_OK) {
+      c.ar.release(Arena::Mark{c.ar.off, 0});  // an error return may have left overflow allocations behind
+      return rc;
+    }
+  }
   ZKD_TRY(finalize_export(N, batch, X, lam, scale, eigvals_api, eigvecs_api, A /* scratch: A is dead */, lam_sorted, rank, s));
   if (info) {
     const int* cs = nullptr;
