@@ -30,23 +30,31 @@ static int check_device() {
 }
 
 // ---- measured IMAD peak -------------------------------------------------------------------------------------------
-// Register-only loop of independent IMAD.WIDE.U32 (32x32+64 -> 64), 8 accumulators per thread, 1024 threads per SM.
-__global__ void __launch_bounds__(256) imad_peak_kernel(uint32_t* out, uint32_t a0, uint32_t b0, int iters) {
-  uint32_t a = a0 + threadIdx.x, b = b0 + blockIdx.x;
-  uint64_t acc[8];
+// Register-only loop of independent signed IMAD.WIDE (32x32+64 -> 64), the instruction the digit GEMM is made of:
+// 8 accumulators x 4 multipliers per thread, 1024 threads per SM.  Every product of an iteration has distinct
+// operands and the multipliers change every iteration (one IADD on the ALU pipe per 8 multiplies), so ptxas can
+// neither merge nor hoist the multiplies: the SASS loop body holds exactly 32 IMAD.WIDE (checked with cuobjdump,
+// profiles/r01_imad_peak.md).
+__global__ void __launch_bounds__(256) imad_peak_kernel(uint32_t* out, int32_t a0, int32_t b0, int iters) {
+  int32_t a[8], b[4];
+  int64_t acc[8];
 #pragma unroll
-  for (int i = 0; i < 8; ++i) acc[i] = i + threadIdx.x;
+  for (int i = 0; i < 8; ++i) { a[i] = a0 + 3 * i + (int)threadIdx.x; acc[i] = i; }
+#pragma unroll
+  for (int u = 0; u < 4; ++u) b[u] = b0 + 5 * u + (int)blockIdx.x;
+#pragma unroll 1
   for (int it = 0; it < iters; ++it) {
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
 #pragma unroll
-      for (int i = 0; i < 8; ++i) asm volatile("mad.wide.u32 %0, %1, %2, %0;" : "+l"(acc[i]) : "r"(a), "r"(b));
+      for (int i = 0; i < 8; ++i) acc[i] += (int64_t)a[i] * (int64_t)b[u];
+      b[u] += it;
     }
   }
-  uint64_t s = 0;
+  int64_t s = 0;
 #pragma unroll
   for (int i = 0; i < 8; ++i) s += acc[i];
-  out[blockIdx.x * blockDim.x + threadIdx.x] = (uint32_t)s ^ (uint32_t)(s >> 32);
+  out[blockIdx.x * blockDim.x + threadIdx.x] = (uint32_t)s ^ (uint32_t)((uint64_t)s >> 32);
 }
 
 int measure_imad_peak(double millis, double* per_sec, cudaStream_t s) {

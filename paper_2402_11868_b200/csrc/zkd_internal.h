@@ -40,7 +40,7 @@ inline int launch_check() {
 struct Options {
   int tau_bits = 20;
   int tol_bits = 770;
-  int max_steps = 40;
+  int max_steps = 120;
   int gemm_path = 0;
   int min_split_ctas = 296;
   int seed_sweeps = 12;
