@@ -140,6 +140,8 @@ static int* option_slot(const char* key) {
   if (!strcmp(key, "gemm_path")) return &o.gemm_path;
   if (!strcmp(key, "min_split_ctas")) return &o.min_split_ctas;
   if (!strcmp(key, "seed_sweeps")) return &o.seed_sweeps;
+  if (!strcmp(key, "seed_path")) return &o.seed_path;
+  if (!strcmp(key, "seed_cluster")) return &o.seed_cluster;
   if (!strcmp(key, "verbose")) return &o.verbose;
   return nullptr;
 }
@@ -305,12 +307,20 @@ int zkd_diag_herm_host(int N, int batch, int prec_bits, const void* A_host, void
   ZKD_TRY(check_device());
   const size_t nA = (size_t)batch * N * N * 2 * kApiRealBytes, nL = (size_t)batch * N * kApiRealBytes;
   const size_t wsb = diag_workspace_bytes(N, batch);
-  char* buf = nullptr;
   const size_t offL = (nA + 255) / 256 * 256, offX = offL + (nL + 255) / 256 * 256, offI = offX + offL,
                offW = offI + ((sizeof(zkd_info) * batch + 255) / 256 * 256);
-  if (cudaMalloc(&buf, offW + wsb) != cudaSuccess) {
-    (void)cudaGetLastError();
-    return ZKD_ERR_WORKSPACE;
+  // grow-only device buffer kept between calls (cudaMalloc/cudaFree cost more than a whole N=64 decomposition)
+  static thread_local char* buf = nullptr;
+  static thread_local size_t buf_bytes = 0;
+  if (offW + wsb > buf_bytes) {
+    if (buf) cudaFree(buf);
+    buf = nullptr;
+    buf_bytes = 0;
+    if (cudaMalloc(&buf, offW + wsb) != cudaSuccess) {
+      (void)cudaGetLastError();
+      return ZKD_ERR_WORKSPACE;
+    }
+    buf_bytes = offW + wsb;
   }
   int rc = ZKD_OK;
   cudaStream_t s = 0;
@@ -325,7 +335,6 @@ int zkd_diag_herm_host(int N, int batch, int prec_bits, const void* A_host, void
       rc = ZKD_ERR_CUDA;
   }
   if (rc == ZKD_ERR_CUDA) (void)cudaGetLastError();
-  cudaFree(buf);
   return rc;
 }
 

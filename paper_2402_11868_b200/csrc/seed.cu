@@ -9,10 +9,10 @@
 // Only column operations occur, so a round of n/2 disjoint pairs is embarrassingly parallel: one warp per pair,
 // round-robin (tournament) ordering, one barrier per round.
 //
-//   n <= 256 : thread-block CLUSTER per matrix (1, 2, 4 or 8 CTAs).  G lives in distributed shared memory, column j in
-//              the shared memory of CTA j / cpc; a warp pulls its two columns through DSMEM into registers, rotates, and
-//              writes them back; rounds are separated by the hardware cluster barrier (about 0.2 us) instead of a grid
-//              barrier through L2.  With many matrices in the batch the cluster size drops to 1 CTA (one SM per matrix).
+//   n <= 256 : thread-block CLUSTER per matrix (1 .. 16 CTAs), systolic ring: every warp owns one pair of columns per round and
+//              hands each rotated column to a neighbouring warp's shared-memory slot, so only the columns at CTA boundaries
+//              cross distributed shared memory; rounds are separated by the hardware cluster barrier.  With many matrices
+//              in the batch the cluster shrinks to 1 CTA (one SM per matrix, plain CTA kernel).
 //   n  > 256 : cooperative grid, G in global memory (L2 resident), grid.sync between rounds.
 // The seed only has to be good to ~2^-40 (the refinement squares the error every step).
 #include <cooperative_groups.h>
@@ -62,40 +62,266 @@ __device__ __forceinline__ void rr_pair(int M, int r, int i, int& p, int& q) {
   if (p > q) { int t = p; p = q; q = t; }
 }
 
-// ---- n <= 256: one thread-block cluster per matrix, G in distributed shared memory -------------------------------------
-// EPL = elements of a column per lane (n <= 32 EPL).  Dynamic shared memory: cpc columns of n complex doubles.
+// ---- n <= 256, systolic ring (Brent-Luk): processor k = warp k % wpc of CTA k / wpc holds the pair (top_k, bot_k) -------------
+// After every round top_0 stays, bot_0 -> top_1, top_k -> top_{k+1}, top_{P-1} -> bot_{P-1}, bot_k -> bot_{k-1}: in M - 1 rounds
+// every pair of columns meets once, and a rotated column is written straight into the slot where it is needed next, which is
+// a neighbouring warp: only the two columns at each CTA boundary cross distributed shared memory per round (DSMEM moves about
+// 17 B/clk/SM, so a design in which every warp fetches both of its columns from their home CTA is bandwidth-bound: it measured
+// 8.6 us per round at n = 256, 21 ms per call; profiles/r01b_seed.md).
+// One slot buffer, two cluster-barrier phases per round: "all slots read" (its wait hidden behind the arithmetic) and "all
+// slots written".
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+
 template <int EPL>
 __global__ void __launch_bounds__(EPL >= 8 ? 512 : 1024)
-seed_cluster_kernel(int n, int cpc, const double2* __restrict__ A, double* __restrict__ mu, double2* __restrict__ V,
-                    int max_sweeps, double tol2) {
-  extern __shared__ double2 Gl[];                 // [cpc][n] : columns rank*cpc .. rank*cpc + cpc - 1
-  __shared__ double s_mu[256];                    // full copy of the unsorted eigenvalues (every CTA)
-  __shared__ unsigned long long s_cmax[2];        // per-sweep max cos^2 of this CTA (bits of a non-negative double)
-  __shared__ double s_rmax;                       // this CTA's largest Gershgorin row sum
+seed_ring_kernel(int n, int wpc, const double2* __restrict__ A, double* __restrict__ mu, double2* __restrict__ V, int max_sweeps,
+                 double tol2) {
+  extern __shared__ double2 slots[];              // [wpc][2][n]
+  __shared__ int s_id[32][2];                     // column ids held by the local slots
+  __shared__ double s_mu[258];                    // by position 2k + which (every CTA holds a full copy)
+  __shared__ int s_pid[258];
+  __shared__ unsigned long long s_cmax[2];
+  __shared__ double s_rmax;
   __shared__ double s_red[32];
   cg::cluster_group cluster = cg::this_cluster();
   const int csize = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
   const int b = blockIdx.x / csize;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const double2* Ab = A + (size_t)b * n * n;
+  const int M = n + (n & 1), P = M / 2;
+  const int k = rank * wpc + warp;                // processor index; processors >= P idle but keep the barriers
+  const bool act = k < P;
+  double2* my_top = slots + (size_t)(warp * 2 + 0) * n;
+  double2* my_bot = slots + (size_t)(warp * 2 + 1) * n;
+
+  // own two columns of the Hermitian matrix (upper triangle authoritative), Gershgorin radius
+  double rmax = 0;
+  if (act) {
+    for (int which = 0; which < 2; ++which) {
+      const int j = 2 * k + which;
+      double2* g = which ? my_bot : my_top;
+      double rs = 0;
+      for (int i = lane; i < n; i += 32) {
+        double2 a = make_double2(0, 0);
+        if (j < n) {
+          a = (i <= j) ? Ab[(size_t)i * n + j] : Ab[(size_t)j * n + i];
+          if (i > j) a.y = -a.y;
+          if (i == j) a.y = 0;
+        }
+        g[i] = a;
+        rs += (i == j) ? fabs(a.x) : sqrt(a.x * a.x + a.y * a.y);
+      }
+      rmax = fmax(rmax, warp_sum(rs));
+      if (lane == 0) s_id[warp][which] = j;
+    }
+  }
+  if (lane == 0) s_red[warp] = rmax;
+  if (tid == 0) { s_cmax[0] = 0ull; s_cmax[1] = 0ull; }
+  __syncthreads();
+  if (tid == 0) {
+    double m = 0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) m = fmax(m, s_red[w]);
+    s_rmax = m;
+  }
+  cluster.sync();
+  double sigma = 0;
+  for (int r = 0; r < csize; ++r) sigma = fmax(sigma, *cluster.map_shared_rank(&s_rmax, r));
+  sigma *= 1.5;
+  if (act && lane == 0) {
+    if (2 * k < n) my_top[2 * k].x += sigma;
+    if (2 * k + 1 < n) my_bot[2 * k + 1].x += sigma;
+  }
+  // destinations of this processor's rotated columns (fixed for the whole run)
+  double2* dst_top = my_top;
+  double2* dst_bot = my_bot;
+  int* dst_top_id = &s_id[warp][0];
+  int* dst_bot_id = &s_id[warp][1];
+  if (act && P > 1) {
+    auto slot_of = [&](int kk, int which) -> double2* {
+      double2* local = slots + (size_t)((kk % wpc) * 2 + which) * n;
+      return (kk / wpc == rank) ? local : cluster.map_shared_rank(local, kk / wpc);
+    };
+    auto id_of = [&](int kk, int which) -> int* {
+      int* local = &s_id[kk % wpc][which];
+      return (kk / wpc == rank) ? local : cluster.map_shared_rank(local, kk / wpc);
+    };
+    if (k == 0) { dst_top = my_top; dst_top_id = &s_id[warp][0]; dst_bot = slot_of(1, 0); dst_bot_id = id_of(1, 0); }
+    else {
+      if (k < P - 1) { dst_top = slot_of(k + 1, 0); dst_top_id = id_of(k + 1, 0); }
+      else { dst_top = my_bot; dst_top_id = &s_id[warp][1]; }
+      dst_bot = slot_of(k - 1, 1); dst_bot_id = id_of(k - 1, 1);
+    }
+  }
+  cluster.sync();
+
+  if (n > 1 && sigma > 0) {
+    for (int sweep = 0; sweep < max_sweeps; ++sweep) {
+      double cmax = 0;
+      for (int r = 0; r < M - 1; ++r) {
+        double2 a[EPL], bb[EPL];
+        int ida = 0, idb = 0;
+        if (act) {
+#pragma unroll
+          for (int q = 0; q < EPL; ++q) {
+            const int i2 = lane + 32 * q;
+            a[q] = i2 < n ? my_top[i2] : make_double2(0, 0);
+            bb[q] = i2 < n ? my_bot[i2] : make_double2(0, 0);
+          }
+          ida = s_id[warp][0];
+          idb = s_id[warp][1];
+        }
+        cluster_arrive();  // slots read
+        if (act) {
+          double al = 0, be = 0, gr = 0, gi = 0;
+#pragma unroll
+          for (int q = 0; q < EPL; ++q) {
+            al = fma(a[q].x, a[q].x, fma(a[q].y, a[q].y, al));
+            be = fma(bb[q].x, bb[q].x, fma(bb[q].y, bb[q].y, be));
+            gr = fma(a[q].x, bb[q].x, fma(a[q].y, bb[q].y, gr));
+            gi = fma(a[q].x, bb[q].y, fma(-a[q].y, bb[q].x, gi));
+          }
+          al = warp_sum(al); be = warp_sum(be); gr = warp_sum(gr); gi = warp_sum(gi);
+          double c, sr, si, cos2;
+          if (rot_params(al, be, gr, gi, tol2, c, sr, si, cos2)) {
+            cmax = fmax(cmax, cos2);
+#pragma unroll
+            for (int q = 0; q < EPL; ++q) {
+              const double2 x = a[q], y = bb[q];
+              a[q] = make_double2(c * x.x - (sr * y.x + si * y.y), c * x.y - (sr * y.y - si * y.x));
+              bb[q] = make_double2(sr * x.x - si * x.y + c * y.x, sr * x.y + si * x.x + c * y.y);
+            }
+          }
+        }
+        cluster_wait();    // everybody has read: slots may be overwritten
+        if (act) {
+#pragma unroll
+          for (int q = 0; q < EPL; ++q) {
+            const int i2 = lane + 32 * q;
+            if (i2 < n) { dst_top[i2] = a[q]; dst_bot[i2] = bb[q]; }
+          }
+          if (lane == 0) { *dst_top_id = ida; *dst_bot_id = idb; }
+        }
+        if (r == M - 2 && lane == 0 && cmax > 0) atomicMax(&s_cmax[sweep & 1], (unsigned long long)__double_as_longlong(cmax));
+        cluster_arrive();
+        cluster_wait();    // slots written
+      }
+      double worst = 0;
+      for (int r = 0; r < csize; ++r)
+        worst = fmax(worst, __longlong_as_double((long long)*cluster.map_shared_rank(&s_cmax[sweep & 1], r)));
+      if (tid == 0) s_cmax[(sweep + 1) & 1] = 0ull;  // last read by the other CTAs one sweep (many barriers) ago
+      __syncthreads();
+      if (!(worst > kSeedStopCos2)) break;
+    }
+  }
+  cluster.sync();
+
+  // mu = ||g|| - sigma per position, broadcast to every CTA; normalise in place
+  if (act) {
+    for (int which = 0; which < 2; ++which) {
+      double2* g = which ? my_bot : my_top;
+      double sq = 0;
+      for (int i = lane; i < n; i += 32) { const double2 x = g[i]; sq += x.x * x.x + x.y * x.y; }
+      sq = warp_sum(sq);
+      const double nrm = sqrt(sq);
+      const double inv = nrm > 0 ? 1.0 / nrm : 0.0;
+      const int id = s_id[warp][which];
+      for (int i = lane; i < n; i += 32) {
+        double2 x = g[i];
+        if (nrm > 0) { x.x *= inv; x.y *= inv; } else { x = make_double2(i == id ? 1.0 : 0.0, 0.0); }
+        g[i] = x;
+      }
+      if (lane < csize) {
+        *cluster.map_shared_rank(&s_mu[2 * k + which], lane) = nrm - sigma;
+        *cluster.map_shared_rank(&s_pid[2 * k + which], lane) = id;
+      }
+    }
+  }
+  cluster.sync();
+  if (act) {
+    for (int which = 0; which < 2; ++which) {
+      const int pos = 2 * k + which;
+      const int id = s_pid[pos];
+      if (id >= n) continue;  // the padding column of an odd n
+      const double mj = s_mu[pos];
+      int rk = 0;
+      for (int i = lane; i < M; i += 32) {
+        const double mi = s_mu[i];
+        const int idi = s_pid[i];
+        rk += (idi < n) && ((mi < mj) || (mi == mj && idi < id));
+      }
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) rk += __shfl_xor_sync(0xffffffffu, rk, off);
+      if (lane == 0) mu[(size_t)b * n + rk] = mj;
+      const double2* g = which ? my_bot : my_top;
+      for (int i = lane; i < n; i += 32) V[(size_t)b * n * n + (size_t)i * n + rk] = g[i];
+    }
+  }
+  cluster.sync();
+}
+
+template <int EPL>
+static int launch_ring(int N, int batch, int csize, const double2* A, double* mu, double2* V, int max_sweeps, double tol2,
+                       cudaStream_t s) {
+  const int P = (N + 1) / 2;
+  const int wpc = (P + csize - 1) / csize;
+  const size_t smem = sizeof(double2) * (size_t)wpc * 2 * N;
+  static size_t attr_smem = 0;
+  static bool np_done = false;
+  if (smem > 48 * 1024 && smem > attr_smem) {
+    ZKD_CUDA_TRY(cudaFuncSetAttribute(seed_ring_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_smem = smem;
+  }
+  if (csize > 8 && !np_done) {
+    ZKD_CUDA_TRY(cudaFuncSetAttribute(seed_ring_kernel<EPL>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    np_done = true;
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(batch * csize));
+  cfg.blockDim = dim3((unsigned)(32 * wpc));
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = (unsigned)csize;
+  at[0].val.clusterDim.y = 1;
+  at[0].val.clusterDim.z = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  ZKD_CUDA_TRY(cudaLaunchKernelEx(&cfg, seed_ring_kernel<EPL>, N, wpc, A, mu, V, max_sweeps, tol2));
+  count_launch();
+  return launch_check();
+}
+
+// ---- n <= 96: one CTA per matrix, G in this CTA's shared memory -----------------------------------------------------------
+// One warp per pair of a round (npairs <= 48 warps would not fit, so a warp takes ceil(npairs / nwarps) pairs), one
+// __syncthreads per round: no cluster barrier and no DSMEM latency on the critical path, and a batch uses one SM per matrix.
+template <int EPL>
+__global__ void __launch_bounds__(1024)
+seed_cta_kernel(int n, const double2* __restrict__ A, double* __restrict__ mu, double2* __restrict__ V, int max_sweeps, double tol2) {
+  extern __shared__ double2 Gl[];                 // [n][n], column j at Gl + j n
+  __shared__ double s_mu[96];
+  __shared__ unsigned long long s_cmax[2];
+  __shared__ double s_red[32];
+  __shared__ double s_sigma;
+  const int b = blockIdx.x;
   const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = nthr >> 5;
   const double2* Ab = A + (size_t)b * n * n;
-  const int j0 = rank * cpc, j1 = min(n, j0 + cpc);
-
-  // own columns of the Hermitian matrix built from the upper triangle (unshifted), and their absolute sums
-  for (int e = tid; e < (j1 - j0) * n; e += nthr) {
-    const int jl = e / n, i = e - jl * n, j = j0 + jl;
+  for (int e = tid; e < n * n; e += nthr) {
+    const int j = e / n, i = e - j * n;
     double2 a = (i <= j) ? Ab[(size_t)i * n + j] : Ab[(size_t)j * n + i];
     if (i > j) a.y = -a.y;
     if (i == j) a.y = 0;
-    Gl[(size_t)jl * n + i] = a;
+    Gl[e] = a;
   }
   if (tid == 0) { s_cmax[0] = 0ull; s_cmax[1] = 0ull; }
   __syncthreads();
   double rmax = 0;
-  for (int jl = warp; jl < j1 - j0; jl += nwarps) {
+  for (int j = warp; j < n; j += nwarps) {
     double rs = 0;
     for (int i = lane; i < n; i += 32) {
-      const double2 a = Gl[(size_t)jl * n + i];
-      rs += (i == j0 + jl) ? fabs(a.x) : sqrt(a.x * a.x + a.y * a.y);
+      const double2 a = Gl[(size_t)j * n + i];
+      rs += (i == j) ? fabs(a.x) : sqrt(a.x * a.x + a.y * a.y);
     }
     rmax = fmax(rmax, warp_sum(rs));
   }
@@ -104,27 +330,24 @@ seed_cluster_kernel(int n, int cpc, const double2* __restrict__ A, double* __res
   if (tid == 0) {
     double m = 0;
     for (int w = 0; w < nwarps; ++w) m = fmax(m, s_red[w]);
-    s_rmax = m;
+    s_sigma = 1.5 * m;
   }
-  cluster.sync();
-  double sigma = 0;
-  for (int r = 0; r < csize; ++r) sigma = fmax(sigma, *cluster.map_shared_rank(&s_rmax, r));
-  sigma *= 1.5;
-  for (int jl = tid; jl < j1 - j0; jl += nthr) Gl[(size_t)jl * n + (j0 + jl)].x += sigma;
-  cluster.sync();
+  __syncthreads();
+  const double sigma = s_sigma;
+  for (int j = tid; j < n; j += nthr) Gl[(size_t)j * n + j].x += sigma;
+  __syncthreads();
 
   const int M = n + (n & 1), npairs = M / 2;
-  const int gwarp = rank * nwarps + warp, gwarps = csize * nwarps;
   if (n > 1 && sigma > 0) {
     for (int sweep = 0; sweep < max_sweeps; ++sweep) {
       double cmax = 0;
       for (int r = 0; r < M - 1; ++r) {
-        for (int i = gwarp; i < npairs; i += gwarps) {
+        for (int i = warp; i < npairs; i += nwarps) {
           int p, q;
           rr_pair(M, r, i, p, q);
           if (q >= n) continue;
-          double2* gp = cluster.map_shared_rank(Gl + (size_t)(p % cpc) * n, p / cpc);
-          double2* gq = cluster.map_shared_rank(Gl + (size_t)(q % cpc) * n, q / cpc);
+          double2* gp = Gl + (size_t)p * n;
+          double2* gq = Gl + (size_t)q * n;
           double2 a[EPL], bb[EPL];
           double al = 0, be = 0, gr = 0, gi = 0;
 #pragma unroll
@@ -137,7 +360,7 @@ seed_cluster_kernel(int n, int cpc, const double2* __restrict__ A, double* __res
           for (int k = 0; k < EPL; ++k) {
             al = fma(a[k].x, a[k].x, fma(a[k].y, a[k].y, al));
             be = fma(bb[k].x, bb[k].x, fma(bb[k].y, bb[k].y, be));
-            gr = fma(a[k].x, bb[k].x, fma(a[k].y, bb[k].y, gr));  // conj(a) b
+            gr = fma(a[k].x, bb[k].x, fma(a[k].y, bb[k].y, gr));
             gi = fma(a[k].x, bb[k].y, fma(-a[k].y, bb[k].x, gi));
           }
           al = warp_sum(al); be = warp_sum(be); gr = warp_sum(gr); gi = warp_sum(gi);
@@ -154,37 +377,30 @@ seed_cluster_kernel(int n, int cpc, const double2* __restrict__ A, double* __res
           }
         }
         if (r == M - 2 && lane == 0 && cmax > 0) atomicMax(&s_cmax[sweep & 1], (unsigned long long)__double_as_longlong(cmax));
-        cluster.sync();
+        __syncthreads();
       }
-      // A sweep whose largest |cos| was below 2^-22 leaves every pair below ~2^-44 (quadratic convergence): stop there.
-      double worst = 0;
-      for (int r = 0; r < csize; ++r)
-        worst = fmax(worst, __longlong_as_double((long long)*cluster.map_shared_rank(&s_cmax[sweep & 1], r)));
-      if (tid == 0) s_cmax[(sweep + 1) & 1] = 0ull;  // last read by the other CTAs one sweep (many barriers) ago
+      const double worst = __longlong_as_double((long long)s_cmax[sweep & 1]);
       __syncthreads();
+      if (tid == 0) s_cmax[(sweep + 1) & 1] = 0ull;
       if (!(worst > kSeedStopCos2)) break;
     }
   }
-  cluster.sync();  // nobody may leave (or overwrite s_cmax) while a neighbour still reads its shared memory
-
-  // mu_j = ||g_j|| - sigma for own columns, broadcast to every CTA of the cluster; normalise own columns in place
-  for (int jl = warp; jl < j1 - j0; jl += nwarps) {
+  __syncthreads();
+  for (int j = warp; j < n; j += nwarps) {
     double s = 0;
-    for (int i = lane; i < n; i += 32) { const double2 a = Gl[(size_t)jl * n + i]; s += a.x * a.x + a.y * a.y; }
+    for (int i = lane; i < n; i += 32) { const double2 a = Gl[(size_t)j * n + i]; s += a.x * a.x + a.y * a.y; }
     s = warp_sum(s);
     const double nrm = sqrt(s);
     const double inv = nrm > 0 ? 1.0 / nrm : 0.0;
     for (int i = lane; i < n; i += 32) {
-      double2 a = Gl[(size_t)jl * n + i];
-      if (nrm > 0) { a.x *= inv; a.y *= inv; } else { a = make_double2(i == j0 + jl ? 1.0 : 0.0, 0.0); }
-      Gl[(size_t)jl * n + i] = a;
+      double2 a = Gl[(size_t)j * n + i];
+      if (nrm > 0) { a.x *= inv; a.y *= inv; } else { a = make_double2(i == j ? 1.0 : 0.0, 0.0); }
+      Gl[(size_t)j * n + i] = a;
     }
-    if (lane < csize) *cluster.map_shared_rank(&s_mu[j0 + jl], lane) = nrm - sigma;
+    if (lane == 0) s_mu[j] = nrm - sigma;
   }
-  cluster.sync();
-  // stable rank sort ascending; V[i][rank] = column j
-  for (int jl = warp; jl < j1 - j0; jl += nwarps) {
-    const int j = j0 + jl;
+  __syncthreads();
+  for (int j = warp; j < n; j += nwarps) {
     const double mj = s_mu[j];
     int rk = 0;
     for (int i = lane; i < n; i += 32) {
@@ -194,39 +410,21 @@ seed_cluster_kernel(int n, int cpc, const double2* __restrict__ A, double* __res
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) rk += __shfl_xor_sync(0xffffffffu, rk, off);
     if (lane == 0) mu[(size_t)b * n + rk] = mj;
-    for (int i = lane; i < n; i += 32) V[(size_t)b * n * n + (size_t)i * n + rk] = Gl[(size_t)jl * n + i];
+    for (int i = lane; i < n; i += 32) V[(size_t)b * n * n + (size_t)i * n + rk] = Gl[(size_t)j * n + i];
   }
-  cluster.sync();
 }
 
 template <int EPL>
-static int launch_cluster(int N, int batch, int csize, const double2* A, double* mu, double2* V, int max_sweeps, double tol2,
-                          cudaStream_t s) {
-  const int M = N + (N & 1), npairs = M / 2;
-  const int cpc = (N + csize - 1) / csize;
-  int warps = (npairs + csize - 1) / csize;
-  const int maxw = EPL >= 8 ? 16 : 32;
-  if (warps > maxw) warps = maxw;
-  if (warps < 1) warps = 1;
-  const size_t smem = sizeof(double2) * (size_t)cpc * N;
+static int launch_cta(int N, int batch, const double2* A, double* mu, double2* V, int max_sweeps, double tol2, cudaStream_t s) {
+  const int npairs = (N + 1) / 2;
+  int warps = npairs < 1 ? 1 : (npairs > 32 ? (npairs + 1) / 2 : npairs);
+  const size_t smem = sizeof(double2) * (size_t)N * N;
   static size_t attr_smem = 0;
-  if (smem > attr_smem) {
-    ZKD_CUDA_TRY(cudaFuncSetAttribute(seed_cluster_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem > 48 * 1024 ? smem : 48 * 1024)));
-    attr_smem = smem > 48 * 1024 ? smem : 48 * 1024;
+  if (smem > 48 * 1024 && smem > attr_smem) {
+    ZKD_CUDA_TRY(cudaFuncSetAttribute(seed_cta_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_smem = smem;
   }
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3((unsigned)(batch * csize));
-  cfg.blockDim = dim3((unsigned)(32 * warps));
-  cfg.dynamicSmemBytes = smem;
-  cfg.stream = s;
-  cudaLaunchAttribute at[1];
-  at[0].id = cudaLaunchAttributeClusterDimension;
-  at[0].val.clusterDim.x = (unsigned)csize;
-  at[0].val.clusterDim.y = 1;
-  at[0].val.clusterDim.z = 1;
-  cfg.attrs = at;
-  cfg.numAttrs = 1;
-  ZKD_CUDA_TRY(cudaLaunchKernelEx(&cfg, seed_cluster_kernel<EPL>, N, cpc, A, mu, V, max_sweeps, tol2));
+  seed_cta_kernel<EPL><<<batch, 32 * warps, smem, s>>>(N, A, mu, V, max_sweeps, tol2);
   count_launch();
   return launch_check();
 }
@@ -349,18 +547,34 @@ int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int ma
   ZKD_CUDA_TRY(cudaGetDevice(&dev));
   ZKD_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   if (N <= 256) {
-    // cluster size: enough CTAs to give every pair of a round its own warp (4 warps per CTA at least), shrunk while the
-    // batch alone fills the machine, grown while a CTA's columns do not fit its shared memory
-    const int npairs = (N + 1) / 2;
-    int csize = 1;
-    while (csize < 8 && npairs > 4 * csize) csize *= 2;
-    while (csize > 1 && (long)batch * csize > 2L * sms) csize /= 2;
-    while (csize < 8 && sizeof(double2) * (size_t)((N + csize - 1) / csize) * N > 200 * 1024) csize *= 2;
+    // ring: as many CTAs as give every processor (pair of columns) its own warp, with at most 16 (n > 128) or 32 warps per CTA;
+    // fewer CTAs when the batch alone fills the machine.  A cluster of 16 is "non-portable": fall back to 8 when refused.
+    const int P = (N + 1) / 2;
+    const int maxw = N > 128 ? 16 : 32;
     const double2* A = (const double2*)A64;
     double2* Vv = (double2*)V;
-    if (N <= 64) return launch_cluster<2>(N, batch, csize, A, mu, Vv, max_sweeps, tol2, s);
-    if (N <= 128) return launch_cluster<4>(N, batch, csize, A, mu, Vv, max_sweeps, tol2, s);
-    return launch_cluster<8>(N, batch, csize, A, mu, Vv, max_sweeps, tol2, s);
+    static int max_cluster = 16;
+    const int want = options().seed_cluster > 0 ? options().seed_cluster : max_cluster;
+    for (;;) {
+      int csize = 1;
+      while (csize < want && csize < max_cluster && P > 4 * csize) csize *= 2;
+      while (csize > 1 && (long)batch * csize > 2L * sms) csize /= 2;
+      while ((P + csize - 1) / csize > maxw) csize *= 2;
+      int rc;
+      if (csize == 1 && N <= 96 && options().seed_path != 2) {
+        // a whole matrix per SM: plain CTA kernel (__syncthreads instead of cluster barriers)
+        if (N <= 32) rc = launch_cta<1>(N, batch, A, mu, Vv, max_sweeps, tol2, s);
+        else if (N <= 64) rc = launch_cta<2>(N, batch, A, mu, Vv, max_sweeps, tol2, s);
+        else rc = launch_cta<3>(N, batch, A, mu, Vv, max_sweeps, tol2, s);
+        return rc;
+      }
+      if (N <= 32) rc = launch_ring<1>(N, batch, csize, A, mu, Vv, max_sweeps, tol2, s);
+      else if (N <= 64) rc = launch_ring<2>(N, batch, csize, A, mu, Vv, max_sweeps, tol2, s);
+      else if (N <= 128) rc = launch_ring<4>(N, batch, csize, A, mu, Vv, max_sweeps, tol2, s);
+      else rc = launch_ring<8>(N, batch, csize, A, mu, Vv, max_sweeps, tol2, s);
+      if (rc == ZKD_ERR_CUDA && csize > 8 && max_cluster > 8) { max_cluster = 8; continue; }
+      return rc;
+    }
   }
   // large: cooperative grid, one matrix at a time
   const int M = N + (N & 1);

@@ -44,6 +44,8 @@ struct Options {
   int gemm_path = 0;
   int min_split_ctas = 296;
   int seed_sweeps = 12;
+  int seed_cluster = 0;  // ring seed: largest cluster size to use (0 = 16, falling back to 8 when refused)
+  int seed_path = 0;     // 0: auto; 2: always the ring kernel for N <= 256
   int verbose = 0;
 };
 Options& options();
