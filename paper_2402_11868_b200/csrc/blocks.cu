@@ -265,6 +265,145 @@ int fxc_add_inplace(size_t count, int32_t* X, const int32_t* T, cudaStream_t s) 
   return launch_check();
 }
 
+// ---- fused S4f + S4c for levels whose clusters are all singletons (the common case: c1, c2, c3) ---------------------------------
+// One CTA per column j:  g = ||x_j||^2 ;  f = 1 + (1 - g)/2 ;  x_j <- f x_j ;  w_j <- f w_j   (Newton-Schulz step = normalisation)
+//                        s = x_j^H w_j ;  theta_j = Re s ;  r_j = w_j - x_j s                  (Rayleigh quotient, residual)
+// X and W are updated in place (a CTA touches only its own column).  Replaces gram, ns_build, 2 x block_apply, gram, theta,
+// block_apply of the general path (7 launches) by one launch whose critical path is 14 digit products per element.
+template <int NACC2>
+__device__ __forceinline__ void block_sum_cols(int64_t (&acc)[NACC2], int64_t* s_part /*[nwarps][NACC2]*/, int nwarps) {
+  warp_sum_cols(acc);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  __syncthreads();  // s_part may still be read from the previous reduction
+  if (lane == 0) {
+#pragma unroll
+    for (int k = 0; k < NACC2; ++k) s_part[warp * NACC2 + k] = acc[k];
+  }
+  __syncthreads();
+#pragma unroll
+  for (int k = 0; k < NACC2; ++k) {
+    int64_t t = 0;
+    for (int w = 0; w < nwarps; ++w) t += s_part[w * NACC2 + k];
+    acc[k] = t;
+  }
+}
+
+__global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int32_t* __restrict__ X, int32_t* __restrict__ W,
+                                                             int32_t* __restrict__ R, int32_t* __restrict__ S,
+                                                             int32_t* __restrict__ theta, int* __restrict__ msb_g_out,
+                                                             int* __restrict__ msb_r_out) {
+  __shared__ int64_t s_part[8 * FXP_NACC];
+  __shared__ int s_msb;
+  const int b = blockIdx.x / n, j = blockIdx.x % n;
+  const int tid = threadIdx.x, nwarps = blockDim.x >> 5;
+  const size_t per = (size_t)n * n, count = per * nb;
+  int32_t* Xr = X;  int32_t* Xi = X + (size_t)ND * count;
+  int32_t* Wr = W;  int32_t* Wi = W + (size_t)ND * count;
+  int32_t* Rr = R;  int32_t* Ri = R + (size_t)ND * count;
+  if (tid == 0) s_msb = 0;
+
+  // g = sum_k |x_kj|^2
+  int64_t acc[FXP_NACC];
+  fxp_zero(acc);
+  for (int k = tid; k < n; k += blockDim.x) {
+    const size_t e = (size_t)b * per + (size_t)k * n + j;
+    int32_t a[ND];
+    fx_load(a, Xr, count, e); fx_mac<false>(acc, a, a);
+    fx_load(a, Xi, count, e); fx_mac<false>(acc, a, a);
+    fxp_relax(acc);
+  }
+  block_sum_cols(acc, s_part, nwarps);
+  int32_t g[ND], m[ND];
+  fxp_finish(g, acc);
+  g[ND - 1] -= 1;                      // g - 1
+  if (tid == 0 && msb_g_out) atomicMax(msb_g_out, fx_msb(g));
+  {
+    int32_t t[ND];
+    fx_neg(t, g);
+    fx_half(m, t);                     // m = (1 - g)/2
+  }
+
+  // x <- x + x m, w <- w + w m   (one plane at a time: at most three digit arrays and one accumulator set are live)
+#pragma unroll 1
+  for (int pl = 0; pl < 4; ++pl) {
+    int32_t* P = pl == 0 ? Xr : pl == 1 ? Xi : pl == 2 ? Wr : Wi;
+#pragma unroll 1
+    for (int k = tid; k < n; k += blockDim.x) {
+      const size_t e = (size_t)b * per + (size_t)k * n + j;
+      int32_t u[ND], t[ND];
+      fx_load(u, P, count, e);
+      fx_mul(t, u, m);
+      int32_t o[ND];
+      fx_add(o, u, t);
+      fx_store(P, count, e, o);
+    }
+  }
+  // s = x^H w : real part, then imaginary part
+  int32_t sr[ND], si[ND];
+#pragma unroll 1
+  for (int part = 0; part < 2; ++part) {
+    fxp_zero(acc);
+#pragma unroll 1
+    for (int k = tid; k < n; k += blockDim.x) {
+      const size_t e = (size_t)b * per + (size_t)k * n + j;
+      int32_t a[ND], c[ND];
+      if (part == 0) {  // xr wr + xi wi
+        fx_load(a, Xr, count, e); fx_load(c, Wr, count, e); fx_mac<false>(acc, a, c);
+        fx_load(a, Xi, count, e); fx_load(c, Wi, count, e); fx_mac<false>(acc, a, c);
+      } else {          // xr wi - xi wr
+        fx_load(a, Xr, count, e); fx_load(c, Wi, count, e); fx_mac<false>(acc, a, c);
+        fx_load(a, Xi, count, e); fx_load(c, Wr, count, e); fx_mac<true>(acc, a, c);
+      }
+      fxp_relax(acc);
+    }
+    block_sum_cols(acc, s_part, nwarps);
+    if (part == 0) fxp_finish(sr, acc); else fxp_finish(si, acc);
+  }
+  if (tid == 0) {
+    fx_store(theta, (size_t)n * nb, (size_t)b * n + j, sr);
+    const size_t ejj = (size_t)b * per + (size_t)j * n + j;
+    fx_store(S, count, ejj, sr);
+    fx_store(S + (size_t)ND * count, count, ejj, si);
+  }
+
+  // r = w - x s
+  int mymsb = 0;
+#pragma unroll 1
+  for (int part = 0; part < 2; ++part) {
+#pragma unroll 1
+    for (int k = tid; k < n; k += blockDim.x) {
+      const size_t e = (size_t)b * per + (size_t)k * n + j;
+      int32_t a[ND], t[ND];
+      fxp_zero(acc);
+      if (part == 0) {  // xr sr - xi si
+        fx_load(a, Xr, count, e); fx_mac<false>(acc, a, sr);
+        fx_load(a, Xi, count, e); fx_mac<true>(acc, a, si);
+      } else {          // xr si + xi sr
+        fx_load(a, Xr, count, e); fx_mac<false>(acc, a, si);
+        fx_load(a, Xi, count, e); fx_mac<false>(acc, a, sr);
+      }
+      fxp_finish(t, acc);
+      fx_load(a, part ? Wi : Wr, count, e);
+      int32_t o[ND];
+      fx_sub(o, a, t);
+      fx_store(part ? Ri : Rr, count, e, o);
+      mymsb = max(mymsb, fx_msb(o));
+    }
+  }
+  for (int off = 16; off > 0; off >>= 1) mymsb = max(mymsb, __shfl_xor_sync(0xffffffffu, mymsb, off));
+  if ((tid & 31) == 0 && mymsb) atomicMax(&s_msb, mymsb);
+  __syncthreads();
+  if (tid == 0 && msb_r_out) atomicMax(msb_r_out, s_msb);
+}
+int singleton_step(int n, int nb, int32_t* X, int32_t* W, int32_t* R, int32_t* S, int32_t* theta, int* msb_g_out, int* msb_r_out,
+                   cudaStream_t s) {
+  int threads = (n + 31) / 32 * 32;
+  if (threads > 256) threads = 256;
+  singleton_step_kernel<<<(unsigned)((size_t)n * nb), threads, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out);
+  count_launch();
+  return launch_check();
+}
+
 // ---- E_ij = C_ij / (theta_j - theta_i) across clusters, 0 inside ---------------------------------------------------------------
 // One thread per pair i < j (and the diagonal, which is zeroed).  d = theta_j - theta_i is normalised to
 // d' = d 2^s in [1/4, 1/2) with a static barrel shifter, r = 1/d' by Newton from an fp64 start on W-digit fixed point

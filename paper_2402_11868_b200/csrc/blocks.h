@@ -11,6 +11,9 @@ int gram_blocks(int n, int nb, const int32_t* X, const int32_t* Y, const int* cl
 int ns_build(int n, int nb, const int* cl, int32_t* G, int* msb_out, cudaStream_t s);
 int block_apply(int n, int nb, const int32_t* base, const int32_t* Y, const int32_t* M, const int* cl, const int* cle, bool negate,
                 int32_t* dst, int* msb_out, cudaStream_t s);
+// fused S4f + S4c when every cluster of the level is a singleton: X, W updated in place, R, diag(S), theta written
+int singleton_step(int n, int nb, int32_t* X, int32_t* W, int32_t* R, int32_t* S, int32_t* theta, int* msb_g_out, int* msb_r_out,
+                   cudaStream_t s);
 int theta_from_diag(int n, int nb, const int32_t* S, int32_t* theta, cudaStream_t s);
 int fxc_add_inplace(size_t count, int32_t* X, const int32_t* T, cudaStream_t s);
 int ecalc(int n, int nb, const int32_t* theta, const int* cl, int32_t* C, int prec_bits, int* msb_out, int* err_flag, cudaStream_t s);

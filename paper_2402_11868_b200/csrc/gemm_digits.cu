@@ -75,7 +75,15 @@ __device__ __forceinline__ int32_t fx_digit_get(const int32_t* __restrict__ plan
   return top < 0 ? DMASK : 0;
 }
 
-__global__ void __launch_bounds__(256) prep_kernel(PrepArgs a) {
+struct PrepArgs2 { PrepArgs side[2]; };
+
+// One launch prepares both operands (blockIdx.y = 0: P, 1: Q).  All digits of the element's window are fetched up front
+// by an unrolled, predicated loop (independent loads in flight together); the window extraction, the 3M sums and the
+// balanced-digit carry chain then run on registers.
+constexpr int kPrepMaxDigits = kND + 2;  // window digits + the one above, at most
+
+__global__ void __launch_bounds__(256) prep_kernel(PrepArgs2 both) {
+  const PrepArgs& a = both.side[blockIdx.y];
   const size_t per = (size_t)a.R * a.C;
   const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= per * a.batch) return;
@@ -83,68 +91,73 @@ __global__ void __launch_bounds__(256) prep_kernel(PrepArgs a) {
   const size_t rc = e % per;
   const int r = (int)(rc / a.C), c = (int)(rc % a.C);
   const size_t sidx = a.transpose ? ((size_t)b * per + (size_t)c * a.R + r) : e;
-  const int32_t* re = a.src;
-  const int32_t* im = a.src + (size_t)kND * a.src_count;
+  const int32_t* __restrict__ re = a.src;
+  const int32_t* __restrict__ im = a.src + (size_t)kND * a.src_count;
   const int32_t top_re = re[(size_t)(kND - 1) * a.src_count + sidx];
   const int32_t top_im = im[(size_t)(kND - 1) * a.src_count + sidx];
   const bool neg_re = top_re < 0, neg_im = top_im < 0;
   const int pad = a.nw - a.nw_src;  // zero digits at the low end
   const int lsb = a.lsb_bit + pad * DB;
-  // floor division of lsb by 28
-  int q0 = lsb >= 0 ? lsb / DB : -((-lsb + DB - 1) / DB);
-  const int sh = lsb - q0 * DB;  // 0..27
+  int q0 = lsb >= 0 ? lsb / DB : -((-lsb + DB - 1) / DB);  // floor(lsb / 28)
+  const int sh = lsb - q0 * DB;                             // 0..27
+  const int nsrc = a.nw_src;
+
+  int32_t lr[kPrepMaxDigits], li[kPrepMaxDigits];
+#pragma unroll
+  for (int t = 0; t < kPrepMaxDigits; ++t) {
+    const bool need = t <= nsrc;
+    lr[t] = need ? fx_digit_get(re, a.src_count, sidx, q0 + t, top_re) : 0;
+    li[t] = need ? fx_digit_get(im, a.src_count, sidx, q0 + t, top_im) : 0;
+  }
 
   int64_t carry[3] = {0, 0, 0};
-  int32_t lo_re = fx_digit_get(re, a.src_count, sidx, q0, top_re);
-  int32_t lo_im = fx_digit_get(im, a.src_count, sidx, q0, top_im);
   bool bad = false;
   const size_t dplane = per;                      // elements per digit plane of one g
-  int32_t* dst0 = a.dst + ((size_t)(b * 3) * a.nw) * dplane + rc;
+  int32_t* __restrict__ dst0 = a.dst + ((size_t)(b * 3) * a.nw) * dplane + rc;
   for (int d = 0; d < pad; ++d) {
     dst0[((size_t)0 * a.nw + d) * dplane] = 0;
     dst0[((size_t)1 * a.nw + d) * dplane] = 0;
     dst0[((size_t)2 * a.nw + d) * dplane] = 0;
   }
-  for (int d = 0; d < a.nw_src; ++d) {
-    const int32_t hi_re = fx_digit_get(re, a.src_count, sidx, q0 + d + 1, top_re);
-    const int32_t hi_im = fx_digit_get(im, a.src_count, sidx, q0 + d + 1, top_im);
-    int32_t wr = sh ? (((lo_re >> sh) | (hi_re << (DB - sh))) & DMASK) : lo_re;
-    int32_t wi = sh ? (((lo_im >> sh) | (hi_im << (DB - sh))) & DMASK) : lo_im;
-    lo_re = hi_re;
-    lo_im = hi_im;
-    const bool last = d == a.nw_src - 1;
-    if (last) {  // signed top digit of the window
-      if (neg_re) wr -= (1 << DB);
-      if (neg_im) wi -= (1 << DB);
-    }
-    if (a.transpose) wi = -wi;  // conjugate (window-level negate; the dropped low bits only move the truncation)
-    int64_t v[3];
-    if (a.side == 0) { v[0] = (int64_t)wr + wi; v[1] = wr; v[2] = wi; }
-    else             { v[0] = wr; v[1] = (int64_t)wi - wr; v[2] = (int64_t)wr + wi; }
 #pragma unroll
-    for (int pl = 0; pl < 3; ++pl) {
-      int64_t t = v[pl] + carry[pl];
-      int64_t out;
-      if (!last) {
-        int64_t cy = (t + DHALF) >> DB;
-        out = t - (cy << DB);
-        carry[pl] = cy;
-      } else {
-        out = t;
-        if (t < -(DHALF) || t > DHALF) bad = true;  // does not fit the window with the 3M headroom
+  for (int d = 0; d < kND; ++d) {
+    if (d < nsrc) {
+      int32_t wr = sh ? (((lr[d] >> sh) | (lr[d + 1] << (DB - sh))) & DMASK) : lr[d];
+      int32_t wi = sh ? (((li[d] >> sh) | (li[d + 1] << (DB - sh))) & DMASK) : li[d];
+      const bool last = d == nsrc - 1;
+      if (last) {  // signed top digit of the window
+        if (neg_re) wr -= (1 << DB);
+        if (neg_im) wi -= (1 << DB);
       }
-      dst0[((size_t)pl * a.nw + pad + d) * dplane] = (int32_t)out;
+      if (a.transpose) wi = -wi;  // conjugate (window-level negate; the dropped low bits only move the truncation)
+      int64_t v[3];
+      if (a.side == 0) { v[0] = (int64_t)wr + wi; v[1] = wr; v[2] = wi; }
+      else             { v[0] = wr; v[1] = (int64_t)wi - wr; v[2] = (int64_t)wr + wi; }
+#pragma unroll
+      for (int pl = 0; pl < 3; ++pl) {
+        int64_t t = v[pl] + carry[pl];
+        int64_t out;
+        if (!last) {
+          int64_t cy = (t + DHALF) >> DB;
+          out = t - (cy << DB);
+          carry[pl] = cy;
+        } else {
+          out = t;
+          if (t < -(DHALF) || t > DHALF) bad = true;  // does not fit the window with the 3M headroom
+        }
+        dst0[((size_t)pl * a.nw + pad + d) * dplane] = (int32_t)out;
+      }
     }
   }
   // bits above the window must be sign extension
   {
-    const int tb = lsb + a.nw_src * DB;  // == top_bit
-    int q = tb >= 0 ? tb / DB : -((-tb + DB - 1) / DB);
-    const int s2 = tb - q * DB;
-    for (; q <= kND + 1; ++q) {
+    const int tb = lsb + nsrc * DB;  // == top_bit
+    const int qt = tb >= 0 ? tb / DB : -((-tb + DB - 1) / DB);
+    const int s2 = tb - qt * DB;
+    for (int q = qt; q <= kND + 1; ++q) {
       int32_t dr = fx_digit_get(re, a.src_count, sidx, q, top_re), di = fx_digit_get(im, a.src_count, sidx, q, top_im);
       int32_t fr = neg_re ? DMASK : 0, fi = neg_im ? DMASK : 0;
-      int32_t mask = (q == (tb >= 0 ? tb / DB : -((-tb + DB - 1) / DB))) ? ((DMASK >> s2) << s2) : DMASK;
+      int32_t mask = (q == qt) ? ((DMASK >> s2) << s2) : DMASK;
       if (((dr ^ fr) & mask) || ((di ^ fi) & mask)) bad = true;
     }
   }
@@ -189,50 +202,80 @@ __global__ void __launch_bounds__(256) combine_kernel(CombineArgs a) {
   int msb_pos = 0, msb_neg = 0;  // candidates for the result's msb (if it ends up >= 0 / < 0)
   const int cutq = a.cut_bit > 0 ? a.cut_bit / DB : 0, cutr = a.cut_bit > 0 ? a.cut_bit % DB : 0;
 
+  const int32_t* __restrict__ q1 = r1;
+  const int32_t* __restrict__ q2 = r2;
   auto col = [&](int c) -> int64_t {
     int64_t s1 = 0, s2 = 0;
     for (int s = 0; s < a.nsplit; ++s) {
-      s1 += r1[(size_t)s * sstride + (size_t)c * colstride];
-      s2 += r2[(size_t)s * sstride + (size_t)c * colstride];
+      s1 += q1[(size_t)s * sstride + (size_t)c * colstride];
+      s2 += q2[(size_t)s * sstride + (size_t)c * colstride];
     }
     return (s1 + sgn2 * s2) << sh;
   };
-  for (int c = 0;; ++c) {
-    const int k = q + c;
-    if (k > kND - 1) break;
-    int64_t v = cy + (c < a.nc ? col(c) : 0);
-    int32_t digit;
-    if (k < kND - 1) {
-      cy = v >> DB;
-      digit = (int32_t)(v & DMASK);
-    } else {
-      // everything that is left lands in the signed top digit (higher raw columns are sign extension unless the
-      // result overflows FX, which the callers' magnitude bounds exclude)
-      if (c + 1 < a.nc) v += col(c + 1) << DB;
-      digit = (int32_t)v;
-      cy = 0;
+  // columns are fetched eight at a time (independent loads in flight together); the carry chains run on registers
+  constexpr int CH = 8;
+  for (int c0 = 0; q + c0 <= kND - 1; c0 += CH) {
+    int64_t s1[CH], s2[CH];
+    int32_t old[CH];
+#pragma unroll
+    for (int u = 0; u < CH; ++u) { s1[u] = 0; s2[u] = 0; old[u] = 0; }
+    for (int s = 0; s < a.nsplit; ++s) {
+#pragma unroll
+      for (int u = 0; u < CH; ++u) {
+        if (c0 + u < a.nc) {
+          s1[u] += q1[(size_t)s * sstride + (size_t)(c0 + u) * colstride];
+          s2[u] += q2[(size_t)s * sstride + (size_t)(c0 + u) * colstride];
+        }
+      }
     }
-    if (k < 0) continue;
-    if (k < cutq) digit = 0;
-    else if (k == cutq && cutr) digit &= ~((1 << cutr) - 1);
-    if (k < kND - 1) {
-      if (digit != 0) msb_pos = k * DB + (32 - __clz(digit));
-      if (digit != DMASK) msb_neg = k * DB + (32 - __clz((~digit) & DMASK));
-    } else {
-      if (digit > 0) msb_pos = k * DB + (32 - __clz(digit));
-      if (digit < -1) msb_neg = k * DB + (32 - __clz(~digit));
-      if (a.msb_out) atomicMax(a.msb_out, digit < 0 ? msb_neg : msb_pos);
+    if (a.mode != 0) {
+#pragma unroll
+      for (int u = 0; u < CH; ++u) {
+        const int k = q + c0 + u;
+        if (k >= 0 && k <= kND - 1) old[u] = dst[(size_t)k * tot];
+      }
     }
-    int32_t* dp = dst + (size_t)k * tot;
-    if (a.mode == 0) {
-      *dp = digit;
-    } else {
-      int64_t t = (int64_t)*dp + (a.mode == 1 ? (int64_t)digit : -(int64_t)digit) + cy2;
-      if (k < kND - 1) {
-        cy2 = t >> DB;
-        *dp = (int32_t)(t & DMASK);
-      } else {
-        *dp = (int32_t)t;
+#pragma unroll
+    for (int u = 0; u < CH; ++u) {
+      const int c = c0 + u;
+      const int k = q + c;
+      if (k <= kND - 1) {
+        int64_t v = cy + ((s1[u] + sgn2 * s2[u]) << sh);
+        int32_t digit;
+        if (k < kND - 1) {
+          cy = v >> DB;
+          digit = (int32_t)(v & DMASK);
+        } else {
+          // everything that is left lands in the signed top digit (higher raw columns are sign extension unless the
+          // result overflows FX, which the callers' magnitude bounds exclude)
+          if (c + 1 < a.nc) v += col(c + 1) << DB;
+          digit = (int32_t)v;
+          cy = 0;
+        }
+        if (k >= 0) {
+          if (k < cutq) digit = 0;
+          else if (k == cutq && cutr) digit &= ~((1 << cutr) - 1);
+          if (k < kND - 1) {
+            if (digit != 0) msb_pos = k * DB + (32 - __clz(digit));
+            if (digit != DMASK) msb_neg = k * DB + (32 - __clz((~digit) & DMASK));
+          } else {
+            if (digit > 0) msb_pos = k * DB + (32 - __clz(digit));
+            if (digit < -1) msb_neg = k * DB + (32 - __clz(~digit));
+            if (a.msb_out) atomicMax(a.msb_out, digit < 0 ? msb_neg : msb_pos);
+          }
+          int32_t* dp = dst + (size_t)k * tot;
+          if (a.mode == 0) {
+            *dp = digit;
+          } else {
+            int64_t t = (int64_t)old[u] + (a.mode == 1 ? (int64_t)digit : -(int64_t)digit) + cy2;
+            if (k < kND - 1) {
+              cy2 = t >> DB;
+              *dp = (int32_t)(t & DMASK);
+            } else {
+              *dp = (int32_t)t;
+            }
+          }
+        }
       }
     }
   }
@@ -343,19 +386,15 @@ int gemm_complex(int M, int N, int K, int batch, const GemmSide& P, const GemmSi
   // operand windows, padded at the LOW end up to the instance's digit counts
   const int lsbP = P.top_bit - DB * in->np, lsbQ = Q.top_bit - DB * in->nq;
   {
-    PrepArgs pa{};
+    PrepArgs2 both{};
+    PrepArgs& pa = both.side[0];
     pa.src = P.fx; pa.dst = Pc; pa.src_count = (size_t)batch * M * K; pa.R = M; pa.C = K; pa.batch = batch;
     pa.transpose = P.conj_transpose ? 1 : 0; pa.side = 0; pa.lsb_bit = lsbP; pa.nw = in->np; pa.nw_src = P.nw; pa.err_flag = err_flag;
-    const size_t tot = (size_t)batch * M * K;
-    prep_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(pa);
-    count_launch();
-  }
-  {
-    PrepArgs pa{};
-    pa.src = Q.fx; pa.dst = Qc; pa.src_count = (size_t)batch * K * N; pa.R = K; pa.C = N; pa.batch = batch;
-    pa.transpose = 0; pa.side = 1; pa.lsb_bit = lsbQ; pa.nw = in->nq; pa.nw_src = Q.nw; pa.err_flag = err_flag;
-    const size_t tot = (size_t)batch * K * N;
-    prep_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(pa);
+    PrepArgs& qa = both.side[1];
+    qa.src = Q.fx; qa.dst = Qc; qa.src_count = (size_t)batch * K * N; qa.R = K; qa.C = N; qa.batch = batch;
+    qa.transpose = 0; qa.side = 1; qa.lsb_bit = lsbQ; qa.nw = in->nq; qa.nw_src = Q.nw; qa.err_flag = err_flag;
+    const size_t tot = (size_t)batch * K * (size_t)(M > N ? M : N);
+    prep_kernel<<<dim3((unsigned)((tot + 255) / 256), 2), 256, 0, stream>>>(both);
     count_launch();
   }
   const int nsplit = pick_splits(M, N, K, batch);

@@ -144,29 +144,37 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
   ZKD_TRY(gemm_complex(n, n, n, nb, side(A, topA, kND, false), side(Xc, topX, 3, false), Wc, GemmMode::Assign, -1, opt.gemm_path,
                        c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s));
 
-  std::vector<int> h_cl;
+  // cluster table to the host (needed for S5 and to pick the singleton fast path)
+  std::vector<int> h_cl((size_t)n * nb);
+  ZKD_CUDA_TRY(cudaMemcpyAsync(h_cl.data(), cl, sizeof(int) * n * nb, cudaMemcpyDeviceToHost, s));
+  if (st && depth == 0) {
+    st->cl_stats.resize((size_t)2 * nb);
+    ZKD_CUDA_TRY(cudaMemcpyAsync(st->cl_stats.data(), stats, sizeof(int) * 2 * nb, cudaMemcpyDeviceToHost, s));
+  }
+  ZKD_CUDA_TRY(cudaStreamSynchronize(s));
+  bool singletons = true;
+  for (int b = 0; b < nb && singletons; ++b)
+    for (int j = 1; j < n; ++j)
+      if (h_cl[(size_t)b * n + j] != j) { singletons = false; break; }
   int status = 2, steps = 0, prev_msb_r = 1 << 30;
   int hs[S_NUM];
   const int tol_msb = 812 - opt.tol_bits;
   for (int step = 0; step < opt.max_steps; ++step) {
-    // S4f: orthonormalise inside clusters (Newton-Schulz step on the cluster Gram blocks)
-    ZKD_TRY(gram_blocks(n, nb, Xc, Xc, cl, Gm, s));
-    ZKD_TRY(ns_build(n, nb, cl, Gm, scal + S_MSB_G, s));
-    ZKD_TRY(block_apply(n, nb, Xc, Xc, Gm, cl, cle, false, Tc, nullptr, s));
-    ZKD_TRY(block_apply(n, nb, Wc, Wc, Gm, cl, cle, false, Cc, nullptr, s));
-    std::swap(Xc, Tc);
-    std::swap(Wc, Cc);
-    // S4c: Rayleigh quotients and block residual
-    ZKD_TRY(gram_blocks(n, nb, Xc, Wc, cl, Sm, s));
-    ZKD_TRY(theta_from_diag(n, nb, Sm, theta, s));
-    ZKD_TRY(block_apply(n, nb, Wc, Xc, Sm, cl, cle, true, R, scal + S_MSB_R, s));
-    if (step == 0) {
-      h_cl.resize((size_t)n * nb);
-      ZKD_CUDA_TRY(cudaMemcpyAsync(h_cl.data(), cl, sizeof(int) * n * nb, cudaMemcpyDeviceToHost, s));
-      if (st && depth == 0) {
-        st->cl_stats.resize((size_t)2 * nb);
-        ZKD_CUDA_TRY(cudaMemcpyAsync(st->cl_stats.data(), stats, sizeof(int) * 2 * nb, cudaMemcpyDeviceToHost, s));
-      }
+    if (singletons) {
+      // S4f + S4c fused: normalise columns, Rayleigh quotients, residual (X, W in place)
+      ZKD_TRY(singleton_step(n, nb, Xc, Wc, R, Sm, theta, scal + S_MSB_G, scal + S_MSB_R, s));
+    } else {
+      // S4f: orthonormalise inside clusters (Newton-Schulz step on the cluster Gram blocks)
+      ZKD_TRY(gram_blocks(n, nb, Xc, Xc, cl, Gm, s));
+      ZKD_TRY(ns_build(n, nb, cl, Gm, scal + S_MSB_G, s));
+      ZKD_TRY(block_apply(n, nb, Xc, Xc, Gm, cl, cle, false, Tc, nullptr, s));
+      ZKD_TRY(block_apply(n, nb, Wc, Wc, Gm, cl, cle, false, Cc, nullptr, s));
+      std::swap(Xc, Tc);
+      std::swap(Wc, Cc);
+      // S4c: Rayleigh quotients and block residual
+      ZKD_TRY(gram_blocks(n, nb, Xc, Wc, cl, Sm, s));
+      ZKD_TRY(theta_from_diag(n, nb, Sm, theta, s));
+      ZKD_TRY(block_apply(n, nb, Wc, Xc, Sm, cl, cle, true, R, scal + S_MSB_R, s));
     }
     ZKD_TRY(read_scalars(c, scal, S_NUM, hs));
     const int msb_r = hs[S_MSB_R], msb_g = hs[S_MSB_G];
