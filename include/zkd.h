@@ -81,7 +81,8 @@ int zkd_diag_herm_host(int N, int batch, int prec_bits, const void *A_host, void
 
 /* Tunables (process-wide; call before zkd_diag_herm*).  Keys: "tau_bits" (cluster threshold 2^-tau ||A||_F,
  * default 20), "tol_bits" (stop when max|R_ij| <= 2^-tol, default 770), "max_steps" (default 40),
- * "gemm_path" (0 = IMAD digit GEMM [default], 1 = int8 tcgen05 sliced GEMM where available),
+ * "gemm_path" (engine of the digit GEMM: 0 = automatic [default]: limb-sliced int8 tcgen05 MMAs when M, N, K >= 128,
+ * the IMAD kernel otherwise; 1 = IMAD only; 2 = int8 tcgen05 wherever its tiles can be formed),
  * "min_split_ctas" (split-K target, default 296).  Returns ZKD_ERR_INVALID_ARG for an unknown key. */
 int zkd_set_option(const char *key, double value);
 int zkd_get_option(const char *key, double *value);
@@ -100,6 +101,9 @@ void zkd_counters_reset(void);
  * kernel time in ms, the number of timed launches and the digit products they performed.  Host calls. */
 int zkd_kernel_timing(int enable);
 int zkd_kernel_timing_read(double *gemm_ms, uint64_t *gemm_launches, uint64_t *gemm_digit_macs);
+/* The same for the int8 tcgen05 engine (S4b): summed kernel time, timed launches, and the s8 x s8 multiply-accumulates
+ * its tcgen05.mma instructions performed (full 128 x 128 x 128 blocks, padding included). */
+int zkd_kernel_timing_read_i8(double *gemm_ms, uint64_t *gemm_launches, uint64_t *int8_macs);
 
 /* ---- host-side helpers (no CUDA): one real between the API layout and (sign, exp, limbs) / double ---- */
 int zkd_pack(void *dst, int prec_bits, int sign, int64_t exp, const uint64_t *limbs_le);

@@ -59,6 +59,7 @@ def lib() -> ctypes.CDLL:
     L.zkd_counters_reset.restype = None
     L.zkd_kernel_timing.argtypes = [ci]
     L.zkd_kernel_timing_read.argtypes = [ctypes.POINTER(cd), ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint64)]
+    L.zkd_kernel_timing_read_i8.argtypes = [ctypes.POINTER(cd), ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint64)]
     L.zkd_pack.argtypes = [vp, ci, ci, ctypes.c_int64, vp]
     L.zkd_unpack.argtypes = [vp, ci, ctypes.POINTER(ci), ctypes.POINTER(ctypes.c_int64), vp]
     L.zkd_from_double.argtypes = [vp, ci, cd]
@@ -136,6 +137,13 @@ def kernel_timing_read() -> tuple[float, int, int]:
     """(summed digit-GEMM kernel time in ms, timed launches, digit products of those launches)"""
     ms, n, m = ctypes.c_double(), ctypes.c_uint64(), ctypes.c_uint64()
     _check(lib().zkd_kernel_timing_read(ctypes.byref(ms), ctypes.byref(n), ctypes.byref(m)), "zkd_kernel_timing_read")
+    return ms.value, int(n.value), int(m.value)
+
+
+def kernel_timing_read_i8() -> tuple[float, int, int]:
+    """(summed int8 tcgen05 GEMM kernel time in ms, timed launches, s8 x s8 MACs of those launches)"""
+    ms, n, m = ctypes.c_double(), ctypes.c_uint64(), ctypes.c_uint64()
+    _check(lib().zkd_kernel_timing_read_i8(ctypes.byref(ms), ctypes.byref(n), ctypes.byref(m)), "zkd_kernel_timing_read_i8")
     return ms.value, int(n.value), int(m.value)
 
 

@@ -4,13 +4,15 @@
 #include <cmath>
 #include <cstring>
 
+#include "gemm_i8.h"
 #include "zkd_internal.h"
 
 namespace zkd {
 
-static std::atomic<uint64_t> g_launches{0}, g_macs{0};
+static std::atomic<uint64_t> g_launches{0}, g_macs{0}, g_i8_macs{0};
 void count_launch(uint64_t n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 void count_macs(uint64_t n) { g_macs.fetch_add(n, std::memory_order_relaxed); }
+void count_i8_macs(uint64_t n) { g_i8_macs.fetch_add(n, std::memory_order_relaxed); }
 Options& options() {
   static Options o;
   return o;
@@ -129,6 +131,7 @@ void zkd_counters(uint64_t* kernel_launches, uint64_t* gemm_digit_macs) {
 void zkd_counters_reset(void) {
   g_launches.store(0);
   g_macs.store(0);
+  g_i8_macs.store(0);
 }
 
 static int* option_slot(const char* key) {
@@ -262,6 +265,9 @@ int zkd_kernel_timing(int enable) {
 }
 int zkd_kernel_timing_read(double* gemm_ms, uint64_t* gemm_launches, uint64_t* gemm_digit_macs) {
   return kernel_timing_read(gemm_ms, gemm_launches, gemm_digit_macs);
+}
+int zkd_kernel_timing_read_i8(double* gemm_ms, uint64_t* gemm_launches, uint64_t* int8_macs) {
+  return kernel_timing_read_i8(gemm_ms, gemm_launches, int8_macs);
 }
 
 // ---- the hot path -------------------------------------------------------------------------------------------------

@@ -8,6 +8,7 @@
 #include <vector>
 
 #include "gemm_digits.cuh"
+#include "gemm_i8.h"
 #include "zkd_internal.h"
 
 namespace zkd {
@@ -300,6 +301,7 @@ constexpr size_t kMaxTimedLaunches = 16384;
 }  // namespace
 
 void kernel_timing_enable(bool on) {
+  kernel_timing_enable_i8(on);
   g_kt.enabled = on;
   g_kt.used = 0;
   g_kt.untimed = 0;
@@ -357,7 +359,8 @@ size_t gemm_workspace_bytes(int M, int N, int K, int batch) {
   const size_t qc = align_up(sizeof(int32_t) * 3 * (size_t)batch * kND * K * N);
   const int sp = pick_splits(M, N, K, batch);
   const size_t raw = align_up(sizeof(int32_t) * (size_t)sp * 3 * batch * (2 * kND + 3) * M * N);
-  return pc + qc + raw;
+  const size_t i8 = gemm_i8_eligible(options().gemm_path, M, N, K, batch) ? gemm_i8_workspace_bytes(M, N, K, batch) : 0;
+  return pc + qc + (raw > i8 ? raw : i8);
 }
 
 uint64_t gemm_complex_macs(int M, int N, int K, int batch, int nwP, int nwQ, int* inst_np, int* inst_nq) {
@@ -369,7 +372,7 @@ uint64_t gemm_complex_macs(int M, int N, int K, int batch, int nwP, int nwQ, int
 }
 
 int gemm_complex(int M, int N, int K, int batch, const GemmSide& P, const GemmSide& Q, int32_t* dst_fx, GemmMode mode,
-                 int out_cut_bit, int /*path*/, void* workspace, size_t workspace_bytes, int* err_flag, int* msb_out,
+                 int out_cut_bit, int path, void* workspace, size_t workspace_bytes, int* err_flag, int* msb_out,
                  cudaStream_t stream) {
   if (M < 1 || N < 1 || K < 1 || batch < 1 || P.nw < 1 || Q.nw < 1 || P.nw > kND || Q.nw > kND) return ZKD_ERR_INVALID_ARG;
   // the instance needs NQ <= NP roles only through its truncation rule; pad whichever side is short
@@ -383,20 +386,29 @@ int gemm_complex(int M, int N, int K, int batch, const GemmSide& P, const GemmSi
   w += align_up(sizeof(int32_t) * 3 * (size_t)batch * kND * K * N);
   int32_t* raw = (int32_t*)w;
 
-  // operand windows, padded at the LOW end up to the instance's digit counts
-  const int lsbP = P.top_bit - DB * in->np, lsbQ = Q.top_bit - DB * in->nq;
+  // the int8 tcgen05 engine takes the windows as they are; the IMAD instances need them padded at the LOW end up to
+  // the instance's digit counts
+  const bool use_i8 = gemm_i8_eligible(path, M, N, K, batch) &&
+                      workspace_bytes >= align_up(sizeof(int32_t) * 3 * (size_t)batch * kND * M * K) +
+                                             align_up(sizeof(int32_t) * 3 * (size_t)batch * kND * K * N) +
+                                             gemm_i8_workspace_bytes(M, N, K, batch);
+  const int npad = use_i8 ? P.nw : in->np, nqad = use_i8 ? Q.nw : in->nq;
+  const int lsbP = P.top_bit - DB * npad, lsbQ = Q.top_bit - DB * nqad;
   {
     PrepArgs2 both{};
     PrepArgs& pa = both.side[0];
     pa.src = P.fx; pa.dst = Pc; pa.src_count = (size_t)batch * M * K; pa.R = M; pa.C = K; pa.batch = batch;
-    pa.transpose = P.conj_transpose ? 1 : 0; pa.side = 0; pa.lsb_bit = lsbP; pa.nw = in->np; pa.nw_src = P.nw; pa.err_flag = err_flag;
+    pa.transpose = P.conj_transpose ? 1 : 0; pa.side = 0; pa.lsb_bit = lsbP; pa.nw = npad; pa.nw_src = P.nw; pa.err_flag = err_flag;
     PrepArgs& qa = both.side[1];
     qa.src = Q.fx; qa.dst = Qc; qa.src_count = (size_t)batch * K * N; qa.R = K; qa.C = N; qa.batch = batch;
-    qa.transpose = 0; qa.side = 1; qa.lsb_bit = lsbQ; qa.nw = in->nq; qa.nw_src = Q.nw; qa.err_flag = err_flag;
+    qa.transpose = 0; qa.side = 1; qa.lsb_bit = lsbQ; qa.nw = nqad; qa.nw_src = Q.nw; qa.err_flag = err_flag;
     const size_t tot = (size_t)batch * K * (size_t)(M > N ? M : N);
     prep_kernel<<<dim3((unsigned)((tot + 255) / 256), 2), 256, 0, stream>>>(both);
     count_launch();
   }
+  if (use_i8)
+    return gemm_i8_finish(M, N, K, batch, Pc, Qc, npad, nqad, lsbP, lsbQ, dst_fx, (int)mode, out_cut_bit, raw,
+                          workspace_bytes - (size_t)((char*)raw - (char*)workspace), err_flag, msb_out, stream);
   const int nsplit = pick_splits(M, N, K, batch);
   int ksplit = (K + nsplit - 1) / nsplit;
   ksplit = (ksplit + GT - 1) / GT * GT;

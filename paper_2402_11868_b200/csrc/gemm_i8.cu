@@ -1,0 +1,611 @@
+// gemm_i8.cu — S4b of SURVEY.md 8(a): the digit GEMM's contraction as limb-sliced int8 tcgen05 MMAs with exact int32
+// accumulation (north_star (e): "the residual/update GEMM A*Y ... run as limb-sliced int8 tcgen05 MMAs with exact int32
+// accumulation and carry propagation wherever that beats the IMAD path").
+//
+// The operands arrive as the compact balanced radix-2^28 digit planes the IMAD path uses (prep_kernel).  Here every
+// entry is re-sliced into balanced radix-2^8 digits ("slices", s8 in [-128,127]); with P = sum_a P_a 2^(8a) and
+// Q = sum_b Q_b 2^(8b) the product is  sum_d 2^(8d) S_d,  S_d = sum_{a+b=d} P_a Q_b  (a convolution of int8 GEMMs).
+// One CTA owns a 128 x 128 output tile and D = 4 consecutive columns d: four int32 accumulators in TMEM (512 columns).
+// For each 128-deep K block it walks a upward; the slices Q_b it needs form a window sliding downward, so every step
+// brings in one P tile and one Q tile (TMA, 128B swizzle) and issues D x 4 tcgen05.mma.kind::i8 (128x128x32).
+// |S_d| <= K * min(nsP,nsQ) * 2^14 < 2^31 is enforced by splitting K.  Columns below dcut (the IMAD path's truncation
+// point) are not computed.  The epilogue stores raw S_d; combine_i8_kernel folds the radix-2^8 columns into FX digits
+// (3M recombination, carries, cut, add/sub into the destination) exactly like combine_kernel does for radix 2^28.
+#include <cuda.h>
+
+#include <vector>
+
+#include "fx.cuh"
+#include "gemm_i8.h"
+
+namespace zkd {
+
+namespace {
+
+constexpr int I8_BM = 128, I8_BN = 128, I8_BK = 128;  // BK in int8 elements = bytes = one 128B swizzle row
+constexpr int I8_D = 4;                               // accumulators (columns d) per CTA: 4 x 128 TMEM columns
+constexpr int I8_RP = 3, I8_RQ = 6;                   // ring depths (tiles of 16 KB)
+constexpr int I8_TILE_BYTES = I8_BM * I8_BK;          // 16384
+constexpr int I8_THREADS = 192;                       // warps 0-3 epilogue, 4 TMA producer, 5 MMA issuer
+constexpr size_t I8_SMEM = (size_t)(I8_RP + I8_RQ) * I8_TILE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+
+// ---- PTX wrappers --------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void* smem_dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(
+          smem_u32(smem_dst)),
+      "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
+      : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint64_t* bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
+      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// K-major, 128B-swizzled operand tile (rows of 128 bytes, 8-row groups 1024 B apart); sm_100 descriptor version 1
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
+  uint64_t d = 0;
+  d |= (uint64_t)((smem_addr & 0x3FFFF) >> 4);  // start address
+  d |= (uint64_t)1 << 16;                       // leading byte offset (unused for swizzled K-major)
+  d |= (uint64_t)(1024 >> 4) << 32;             // stride byte offset: 8 rows x 128 B
+  d |= (uint64_t)1 << 46;                       // descriptor version (sm_100)
+  d |= (uint64_t)2 << 61;                       // SWIZZLE_128B
+  return d;
+}
+__device__ __forceinline__ void tmem_ld_32x32b_x32(uint32_t taddr, uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+        "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]),
+        "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]),
+        "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+      : "r"(taddr));
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+}  // namespace
+
+namespace {
+
+// ---- re-slicing: compact balanced radix-2^28 planes -> balanced radix-2^8 planes, K-major, K padded to 128 ----------
+struct SliceArgs {
+  const int32_t* src;  // [G][nw][R][C]
+  int8_t* dst;         // [G][ns][rows][Kp]   (P: rows = R, k = c;  Q: rows = C, k = r)
+  int R, C, G, nw, ns, rows, K, Kp, transpose;
+  int* err_flag;
+};
+
+__global__ void __launch_bounds__(256) slice_i8_kernel(SliceArgs a) {
+  const size_t per = (size_t)a.rows * a.Kp;
+  const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= per * a.G) return;
+  const int g = (int)(e / per);
+  const size_t rk = e % per;
+  const int row = (int)(rk / a.Kp), kk = (int)(rk % a.Kp);
+  int8_t* __restrict__ dst = a.dst + (size_t)g * a.ns * per + rk;
+  if (kk >= a.K) {
+    for (int j = 0; j < a.ns; ++j) dst[(size_t)j * per] = 0;
+    return;
+  }
+  const size_t RC = (size_t)a.R * a.C;
+  const size_t sidx = a.transpose ? ((size_t)kk * a.C + row) : ((size_t)row * a.C + kk);
+  const int32_t* __restrict__ src = a.src + (size_t)g * a.nw * RC + sidx;
+  int64_t acc = 0;
+  int pos = 0, j = 0;
+  bool bad = false;
+  for (int k = 0; k < a.nw; ++k) {
+    const int32_t d = src[(size_t)k * RC];
+    acc += (int64_t)d << (DB * k - pos);
+    const int limit = (k == a.nw - 1) ? a.ns * 8 : DB * (k + 1);
+    while (pos + 8 <= limit) {
+      int64_t cy = (acc + 128) >> 8;
+      int64_t byte = acc - (cy << 8);
+      if (j == a.ns - 1) {
+        byte = acc;
+        cy = 0;
+        if (acc < -128 || acc > 127) bad = true;
+      }
+      dst[(size_t)j * per] = (int8_t)byte;
+      acc = cy;
+      pos += 8;
+      ++j;
+    }
+  }
+  if (bad && a.err_flag) atomicOr(a.err_flag, 4);
+}
+
+}  // namespace
+
+namespace {
+
+// ---- the tcgen05 kernel ----------------------------------------------------------------------------------------------
+struct I8Args {
+  int32_t* out;  // [nsplit][G][ncol][M][N]
+  int M, N, G, nsP, nsQ, dcut, ncol, ngroups, nkb, kb_per_split, nsplit;
+  uint32_t p_tile_bytes, q_tile_bytes;  // bytes one TMA box delivers (rows may be < 128 for small matrices)
+};
+
+// the slice ranges of one column group [d0, d0 + D)
+struct GroupRange {
+  int d0, a_min, a_max, b_min, b_max, nA, nQ;
+};
+__device__ __forceinline__ GroupRange group_range(const I8Args& a, int dg) {
+  GroupRange r;
+  r.d0 = a.dcut + I8_D * dg;
+  const int dhi = min(r.d0 + I8_D - 1, a.nsP + a.nsQ - 2);
+  r.a_min = max(0, r.d0 - (a.nsQ - 1));
+  r.a_max = min(a.nsP - 1, dhi);
+  r.b_max = min(a.nsQ - 1, dhi - r.a_min);
+  r.b_min = max(0, r.d0 - r.a_max);
+  r.nA = r.a_max - r.a_min + 1;
+  r.nQ = r.b_max - r.b_min + 1;
+  return r;
+}
+
+__global__ void __launch_bounds__(I8_THREADS, 1)
+gemm_i8_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ CUtensorMap mapQ, const I8Args a) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  uint8_t* p_tiles = smem;                                  // [RP][16 KB]
+  uint8_t* q_tiles = smem + (size_t)I8_RP * I8_TILE_BYTES;  // [RQ][16 KB]
+  uint64_t* bars = (uint64_t*)(smem + (size_t)(I8_RP + I8_RQ) * I8_TILE_BYTES);
+  uint64_t* full_p = bars;
+  uint64_t* empty_p = bars + I8_RP;
+  uint64_t* full_q = bars + 2 * I8_RP;
+  uint64_t* empty_q = bars + 2 * I8_RP + I8_RQ;
+  uint64_t* tmem_full = bars + 2 * I8_RP + 2 * I8_RQ;
+  uint32_t* tmem_base_slot = (uint32_t*)(tmem_full + 1);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int j0 = blockIdx.x * I8_BN, i0 = blockIdx.y * I8_BM;
+  int z = blockIdx.z;
+  const int dg = z % a.ngroups;
+  z /= a.ngroups;
+  const int sp = z % a.nsplit;
+  const int g = z / a.nsplit;
+  const GroupRange gr = group_range(a, dg);
+  const int kb0 = sp * a.kb_per_split, kb1 = min(a.nkb, kb0 + a.kb_per_split);
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < I8_RP; ++i) { mbar_init(full_p + i, 1); mbar_init(empty_p + i, 1); }
+    for (int i = 0; i < I8_RQ; ++i) { mbar_init(full_q + i, 1); mbar_init(empty_q + i, 1); }
+    mbar_init(tmem_full, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  if (warp == 5) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_base_slot)), "n"(512));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t tmem_base = *tmem_base_slot;
+
+  if (warp == 4) {
+    // ===== TMA producer =====
+    if (lane == 0) {
+      uint32_t pseq = 0, qseq = 0;
+      for (int kb = kb0; kb < kb1; ++kb) {
+        int q_next = gr.b_max;
+        for (int aa = gr.a_min; aa <= gr.a_max; ++aa) {
+          const int lowest = max(gr.b_min, gr.d0 - aa);
+          while (q_next >= lowest) {
+            const uint32_t s = qseq % I8_RQ, ph = (qseq / I8_RQ) & 1;
+            mbar_wait(empty_q + s, ph ^ 1);
+            mbar_expect_tx(full_q + s, a.q_tile_bytes);
+            tma_load_3d(q_tiles + (size_t)s * I8_TILE_BYTES, &mapQ, full_q + s, kb * I8_BK, j0, g * a.nsQ + q_next);
+            ++qseq;
+            --q_next;
+          }
+          const uint32_t s = pseq % I8_RP, ph = (pseq / I8_RP) & 1;
+          mbar_wait(empty_p + s, ph ^ 1);
+          mbar_expect_tx(full_p + s, a.p_tile_bytes);
+          tma_load_3d(p_tiles + (size_t)s * I8_TILE_BYTES, &mapP, full_p + s, kb * I8_BK, i0, g * a.nsP + aa);
+          ++pseq;
+        }
+      }
+    }
+  } else if (warp == 5) {
+    // ===== MMA issuer =====
+    if (lane == 0) {
+      // S32 accumulate, S8 x S8, both K-major, M = 128, N = 128
+      constexpr uint32_t idesc = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(I8_BN >> 3) << 17) | ((uint32_t)(I8_BM >> 4) << 24);
+      uint32_t started = 0;
+      uint32_t pseq = 0;
+      for (int kb = kb0; kb < kb1; ++kb) {
+        const uint32_t qbase = (uint32_t)(kb - kb0) * gr.nQ;  // sequence number of tile b_max of this K block
+        int q_next = gr.b_max;
+        for (int aa = gr.a_min; aa <= gr.a_max; ++aa) {
+          const int lowest = max(gr.b_min, gr.d0 - aa);
+          while (q_next >= lowest) {
+            const uint32_t qs = qbase + (gr.b_max - q_next);
+            mbar_wait(full_q + qs % I8_RQ, (qs / I8_RQ) & 1);
+            --q_next;
+          }
+          const uint32_t s = pseq % I8_RP;
+          mbar_wait(full_p + s, (pseq / I8_RP) & 1);
+          asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+          const uint32_t pa = smem_u32(p_tiles + (size_t)s * I8_TILE_BYTES);
+#pragma unroll
+          for (int dd = 0; dd < I8_D; ++dd) {
+            const int b = gr.d0 + dd - aa;
+            if (b < gr.b_min || b > gr.b_max) continue;
+            const uint32_t qs = qbase + (gr.b_max - b);
+            const uint32_t qa = smem_u32(q_tiles + (size_t)(qs % I8_RQ) * I8_TILE_BYTES);
+#pragma unroll
+            for (int k = 0; k < I8_BK / 32; ++k) {
+              umma_i8(tmem_base + dd * I8_BN, umma_desc_sw128(pa + k * 32), umma_desc_sw128(qa + k * 32), idesc,
+                      ((started >> dd) & 1) | (k > 0));
+            }
+            started |= 1u << dd;
+          }
+          umma_commit(empty_p + s);
+          ++pseq;
+          // Q tiles that no later step of this K block uses
+          const int dead_hi = gr.d0 + I8_D - 1 - aa;
+          const int dead_lo = (aa == gr.a_max) ? gr.b_min : dead_hi;
+          for (int b = min(dead_hi, gr.b_max); b >= max(dead_lo, gr.b_min); --b) {
+            const uint32_t qs = qbase + (gr.b_max - b);
+            umma_commit(empty_q + qs % I8_RQ);
+          }
+        }
+      }
+      umma_commit(tmem_full);
+    }
+  } else {
+    // ===== epilogue: warps 0-3, TMEM lanes 32*warp .. +31 = output rows =====
+    mbar_wait(tmem_full, 0);
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const int i = i0 + warp * 32 + lane;
+    const size_t mn = (size_t)a.M * a.N;
+    for (int dd = 0; dd < I8_D; ++dd) {
+      const int c = I8_D * dg + dd;  // column index relative to dcut
+      if (c >= a.ncol) break;
+      int32_t* o = a.out + ((size_t)(sp * a.G + g) * a.ncol + c) * mn + (size_t)i * a.N + j0;
+      const bool has = true;  // every kept column d <= nsP + nsQ - 2 receives at least one slice pair
+#pragma unroll 1
+      for (int cc = 0; cc < I8_BN; cc += 32) {
+        uint32_t v[32];
+        if (has) {
+          tmem_ld_32x32b_x32(tmem_base + ((uint32_t)(warp * 32) << 16) + dd * I8_BN + cc, v);
+        } else {
+#pragma unroll
+          for (int t = 0; t < 32; ++t) v[t] = 0;
+        }
+        if (i < a.M) {
+          if (j0 + cc + 32 <= a.N && (a.N & 3) == 0) {
+#pragma unroll
+            for (int t = 0; t < 32; t += 4) *(int4*)(o + cc + t) = make_int4((int)v[t], (int)v[t + 1], (int)v[t + 2], (int)v[t + 3]);
+          } else {
+#pragma unroll
+            for (int t = 0; t < 32; ++t)
+              if (j0 + cc + t < a.N) o[cc + t] = (int32_t)v[t];
+          }
+        }
+      }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  }
+  __syncthreads();
+  if (warp == 5) {
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(512));
+  }
+}
+
+}  // namespace
+
+namespace {
+
+// ---- combine: radix-2^8 column sums -> FX digits ------------------------------------------------------------------------
+struct CombineI8Args {
+  const int32_t* raw;  // [nsplit][3*batch][ncol][M*N]
+  int32_t* dst;        // complex FX, batch*M*N
+  size_t mn;
+  int batch, ncol, nsplit;
+  int base_bit;  // FX bit position of column 0's LSB (may be negative)
+  int cut_bit;   // clear result bits below this FX bit (<= 0: none)
+  int mode;      // 0 assign, 1 add, 2 sub
+  int* msb_out;
+};
+
+// one thread per (element, part); part 0 = Re = k1 - k3, part 1 = Im = k1 + k2
+__global__ void __launch_bounds__(256) combine_i8_kernel(CombineI8Args a) {
+  const size_t tot = a.mn * a.batch;
+  const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int part = blockIdx.y;
+  if (e >= tot) return;
+  const int b = (int)(e / a.mn);
+  const size_t ij = e % a.mn;
+  const size_t gstride = (size_t)a.ncol * a.mn;
+  const size_t sstride = (size_t)3 * a.batch * gstride;
+  const int32_t* __restrict__ r1 = a.raw + (size_t)(b * 3 + 0) * gstride + ij;
+  const int32_t* __restrict__ r2 = a.raw + (size_t)(b * 3 + (part == 0 ? 2 : 1)) * gstride + ij;
+  const int sgn2 = part == 0 ? -1 : 1;
+  int32_t* dst = a.dst + (part ? (size_t)ND * tot : 0) + e;
+
+  auto col = [&](int c) -> int64_t {
+    int64_t s1 = 0, s2 = 0;
+    for (int s = 0; s < a.nsplit; ++s) {
+      s1 += r1[(size_t)s * sstride + (size_t)c * a.mn];
+      s2 += r2[(size_t)s * sstride + (size_t)c * a.mn];
+    }
+    return s1 + sgn2 * s2;
+  };
+  // FX digit k covers bits [28k, 28k+28); walk k upward from the digit holding column 0, feeding each digit the
+  // columns whose LSB falls inside it
+  const int kstart = a.base_bit >= 0 ? a.base_bit / DB : -((-a.base_bit + DB - 1) / DB);
+  const int cutq = a.cut_bit > 0 ? a.cut_bit / DB : 0, cutr = a.cut_bit > 0 ? a.cut_bit % DB : 0;
+  int64_t acc = 0, cy2 = 0;
+  int c = 0;
+  int msb_pos = 0, msb_neg = 0;
+  for (int k = kstart; k <= ND - 1; ++k) {
+    const int lo = k * DB;
+    if (k < ND - 1) {
+      while (c < a.ncol && a.base_bit + 8 * c < lo + DB) {
+        acc += col(c) << (a.base_bit + 8 * c - lo);
+        ++c;
+      }
+    } else {
+      // the signed top digit takes everything that is left (sign extension unless the result overflows FX, which the
+      // callers' magnitude bounds exclude)
+      while (c < a.ncol) {
+        const int sh = a.base_bit + 8 * c - lo;
+        if (sh < 40) acc += col(c) << sh;
+        ++c;
+      }
+    }
+    int32_t digit;
+    if (k < ND - 1) {
+      digit = (int32_t)(acc & DMASK);
+      acc >>= DB;
+    } else {
+      digit = (int32_t)acc;
+    }
+    if (k < 0) continue;
+    if (k < cutq) digit = 0;
+    else if (k == cutq && cutr) digit &= ~((1 << cutr) - 1);
+    if (k < ND - 1) {
+      if (digit != 0) msb_pos = k * DB + (32 - __clz(digit));
+      if (digit != DMASK) msb_neg = k * DB + (32 - __clz((~digit) & DMASK));
+    } else {
+      if (digit > 0) msb_pos = k * DB + (32 - __clz(digit));
+      if (digit < -1) msb_neg = k * DB + (32 - __clz(~digit));
+      if (a.msb_out) atomicMax(a.msb_out, digit < 0 ? msb_neg : msb_pos);
+    }
+    int32_t* dp = dst + (size_t)k * tot;
+    if (a.mode == 0) {
+      *dp = digit;
+    } else {
+      const int64_t t = (int64_t)*dp + (a.mode == 1 ? (int64_t)digit : -(int64_t)digit) + cy2;
+      if (k < ND - 1) {
+        cy2 = t >> DB;
+        *dp = (int32_t)(t & DMASK);
+      } else {
+        *dp = (int32_t)t;
+      }
+    }
+  }
+  if (a.mode == 0)
+    for (int kk = 0; kk < kstart && kk < ND; ++kk) dst[(size_t)kk * tot] = 0;
+}
+
+}  // namespace
+
+// ---- host side -----------------------------------------------------------------------------------------------------
+
+namespace {
+
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)p;
+    else
+      (void)cudaGetLastError();
+  }
+  return fn;
+}
+
+// int8 planes [planes][rows][Kp] -> 3D map (k, row, plane), box 128 x min(128, rows) x 1, 128B swizzle
+int make_map(CUtensorMap* map, const int8_t* base, int Kp, int rows, int planes, int box_rows) {
+  EncodeTiledFn fn = encode_tiled_fn();
+  if (!fn) return ZKD_ERR_CUDA;
+  const cuuint64_t dims[3] = {(cuuint64_t)Kp, (cuuint64_t)rows, (cuuint64_t)planes};
+  const cuuint64_t strides[2] = {(cuuint64_t)Kp, (cuuint64_t)Kp * rows};
+  const cuuint32_t box[3] = {(cuuint32_t)I8_BK, (cuuint32_t)box_rows, 1};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  const CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, (void*)base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                        CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? ZKD_OK : ZKD_ERR_CUDA;
+}
+
+inline size_t align_up(size_t x, size_t a = 1024) { return (x + a - 1) / a * a; }
+inline int slices_for(int nw) { return (DB * nw + 8) / 8; }
+constexpr int kMaxSlices = (DB * ND + 8) / 8;  // 106
+constexpr int kMaxCols = 128;                  // kept columns: <= nsP + nsQ - 1 - dcut <= 106 + 8 + ... (checked at run time)
+
+struct Timer {
+  bool enabled = false;
+  std::vector<cudaEvent_t> ev;
+  std::vector<uint64_t> macs;
+  size_t used = 0;
+};
+Timer g_t;
+
+int pick_nsplit(int K, int nsmin) {
+  // |S_d| <= Ksplit * nsmin * 2^14 must stay below 2^31
+  const int nkb = (K + I8_BK - 1) / I8_BK;
+  int kb_per = nkb;
+  while (kb_per > 1 && (long)kb_per * I8_BK * nsmin >= 131072) --kb_per;
+  return (nkb + kb_per - 1) / kb_per;
+}
+
+}  // namespace
+
+void kernel_timing_enable_i8(bool on) {
+  g_t.enabled = on;
+  g_t.used = 0;
+  g_t.macs.clear();
+}
+int kernel_timing_read_i8(double* ms, uint64_t* launches, uint64_t* macs) {
+  double tot = 0;
+  uint64_t m = 0;
+  for (size_t i = 0; i < g_t.used; ++i) {
+    float t = 0;
+    if (cudaEventSynchronize(g_t.ev[2 * i + 1]) != cudaSuccess ||
+        cudaEventElapsedTime(&t, g_t.ev[2 * i], g_t.ev[2 * i + 1]) != cudaSuccess) {
+      (void)cudaGetLastError();
+      return ZKD_ERR_CUDA;
+    }
+    tot += t;
+    m += g_t.macs[i];
+  }
+  if (ms) *ms = tot;
+  if (launches) *launches = g_t.used;
+  if (macs) *macs = m;
+  return ZKD_OK;
+}
+
+bool gemm_i8_eligible(int path, int M, int N, int K, int batch) {
+  (void)batch;
+  if (path == 1) return false;                              // IMAD only
+  if (path == 2) return M >= 8 && N >= 8 && K >= 1;         // forced (tests)
+  return M >= 128 && N >= 128 && K >= 128;                  // auto: where one matrix fills 128 x 128 tiles
+}
+
+size_t gemm_i8_workspace_bytes(int M, int N, int K, int batch) {
+  const size_t Kp = (size_t)(K + I8_BK - 1) / I8_BK * I8_BK;
+  const size_t G = 3 * (size_t)batch;
+  const size_t p8 = align_up(G * kMaxSlices * (size_t)M * Kp);
+  const size_t q8 = align_up(G * kMaxSlices * (size_t)N * Kp);
+  const int nsplit = pick_nsplit(K, kMaxSlices);
+  const size_t raw = align_up(sizeof(int32_t) * (size_t)nsplit * G * kMaxCols * (size_t)M * N);
+  return p8 + q8 + raw;
+}
+
+int gemm_i8_finish(int M, int N, int K, int batch, const int32_t* Pc, const int32_t* Qc, int np, int nq, int lsbP, int lsbQ,
+                   int32_t* dst_fx, int mode, int cut_bit, void* ws, size_t ws_bytes, int* err_flag, int* msb_out,
+                   cudaStream_t stream) {
+  if (ws_bytes < gemm_i8_workspace_bytes(M, N, K, batch)) return ZKD_ERR_WORKSPACE;
+  const int Kp = (K + I8_BK - 1) / I8_BK * I8_BK;
+  const int G = 3 * batch;
+  const int nsP = slices_for(np), nsQ = slices_for(nq);
+  const int low28 = nq >= 2 ? nq - 2 : 0;  // the IMAD instances' truncation rule (gemm_digits.cuh)
+  const int dcut = DB * low28 / 8;
+  const int ncol = nsP + nsQ - 1 - dcut;
+  if (ncol < 1 || ncol > kMaxCols) return ZKD_ERR_INTERNAL;
+  char* w = (char*)ws;
+  int8_t* P8 = (int8_t*)w;
+  w += align_up((size_t)G * kMaxSlices * M * Kp);
+  int8_t* Q8 = (int8_t*)w;
+  w += align_up((size_t)G * kMaxSlices * N * Kp);
+  int32_t* raw = (int32_t*)w;
+
+  {
+    SliceArgs sa{};
+    sa.src = Pc; sa.dst = P8; sa.R = M; sa.C = K; sa.G = G; sa.nw = np; sa.ns = nsP; sa.rows = M; sa.K = K; sa.Kp = Kp;
+    sa.transpose = 0; sa.err_flag = err_flag;
+    size_t tot = (size_t)G * M * Kp;
+    slice_i8_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(sa);
+    count_launch();
+    sa.src = Qc; sa.dst = Q8; sa.R = K; sa.C = N; sa.nw = nq; sa.ns = nsQ; sa.rows = N; sa.transpose = 1;
+    tot = (size_t)G * N * Kp;
+    slice_i8_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(sa);
+    count_launch();
+  }
+  CUtensorMap mapP, mapQ;
+  const int boxP = M < I8_BM ? M : I8_BM, boxQ = N < I8_BN ? N : I8_BN;
+  ZKD_TRY(make_map(&mapP, P8, Kp, M, G * nsP, boxP));
+  ZKD_TRY(make_map(&mapQ, Q8, Kp, N, G * nsQ, boxQ));
+
+  I8Args ka{};
+  ka.out = raw; ka.M = M; ka.N = N; ka.G = G; ka.nsP = nsP; ka.nsQ = nsQ; ka.dcut = dcut; ka.ncol = ncol;
+  ka.ngroups = (ncol + I8_D - 1) / I8_D;
+  ka.nkb = Kp / I8_BK;
+  ka.nsplit = pick_nsplit(K, nsP < nsQ ? nsP : nsQ);
+  ka.kb_per_split = (ka.nkb + ka.nsplit - 1) / ka.nsplit;
+  ka.nsplit = (ka.nkb + ka.kb_per_split - 1) / ka.kb_per_split;
+  ka.p_tile_bytes = (uint32_t)boxP * I8_BK;
+  ka.q_tile_bytes = (uint32_t)boxQ * I8_BK;
+  static bool attr_done = false;
+  if (!attr_done) {
+    ZKD_CUDA_TRY(cudaFuncSetAttribute(gemm_i8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)I8_SMEM));
+    attr_done = true;
+  }
+  const dim3 grid((N + I8_BN - 1) / I8_BN, (M + I8_BM - 1) / I8_BM, (unsigned)(G * ka.nsplit * ka.ngroups));
+  if (grid.z > 65535) return ZKD_ERR_INTERNAL;
+  // int8 MACs actually issued: every (a, b) pair with a + b >= dcut, on full 128 x 128 x 128 blocks
+  uint64_t pairs = 0;
+  for (int x = 0; x < nsP; ++x)
+    for (int y = 0; y < nsQ; ++y)
+      if (x + y >= dcut) ++pairs;
+  const uint64_t macs = pairs * (uint64_t)G * grid.x * grid.y * ka.nkb * I8_BM * I8_BN * I8_BK;
+  bool timed = false;
+  if (g_t.enabled && g_t.used < 16384) {
+    while (g_t.ev.size() < 2 * (g_t.used + 1)) {
+      cudaEvent_t ev;
+      if (cudaEventCreate(&ev) != cudaSuccess) { (void)cudaGetLastError(); break; }
+      g_t.ev.push_back(ev);
+    }
+    if (g_t.ev.size() >= 2 * (g_t.used + 1)) {
+      cudaEventRecord(g_t.ev[2 * g_t.used], stream);
+      timed = true;
+    }
+  }
+  gemm_i8_kernel<<<grid, I8_THREADS, I8_SMEM, stream>>>(mapP, mapQ, ka);
+  if (timed) {
+    cudaEventRecord(g_t.ev[2 * g_t.used + 1], stream);
+    g_t.macs.push_back(macs);
+    ++g_t.used;
+  }
+  count_launch();
+  count_i8_macs(macs);
+  ZKD_TRY(launch_check());
+
+  CombineI8Args ca{};
+  ca.raw = raw; ca.dst = dst_fx; ca.mn = (size_t)M * N; ca.batch = batch; ca.ncol = ncol; ca.nsplit = ka.nsplit;
+  ca.base_bit = lsbP + lsbQ - FRAC + 8 * dcut;
+  ca.cut_bit = cut_bit; ca.mode = mode; ca.msb_out = msb_out;
+  const size_t tot = (size_t)batch * M * N;
+  combine_i8_kernel<<<dim3((unsigned)((tot + 255) / 256), 2), 256, 0, stream>>>(ca);
+  count_launch();
+  return launch_check();
+}
+
+}  // namespace zkd

@@ -85,8 +85,36 @@ GEMM_CASES = [
 ]
 
 
+# the same contraction through the int8 tcgen05 engine (S4b): forced on small ragged shapes (partial TMA boxes), and
+# shapes spanning several 128-tiles, K blocks and a ragged tail
+GEMM_I8_CASES = [
+    (16, 16, 16, 2, 0, (812, 30), (815, 30), 0, -1),
+    (33, 18, 37, 1, 0, (812, 30), (815, 30), 0, -1),
+    (20, 20, 20, 1, 1, (815, 5), (700, 5), 0, -1),
+    (20, 20, 20, 3, 0, (815, 6), (650, 6), 0, 480),
+    (24, 9, 40, 1, 0, (812, 24), (660, 8), 1, -1),
+    (24, 9, 40, 1, 0, (812, 24), (660, 8), 2, -1),
+    (130, 70, 150, 1, 0, (812, 30), (815, 3), 0, -1),
+    (140, 136, 260, 1, 1, (815, 9), (600, 9), 0, -1),
+    (128, 128, 128, 1, 0, (812, 30), (815, 30), 0, -1),
+]
+
+
+@pytest.mark.parametrize("case", GEMM_I8_CASES)
+def test_gemm_fx_int8_tcgen05_matches_python_integers(zkd, case):
+    zkd.set_option("gemm_path", 2)
+    try:
+        zkd.kernel_timing(True)
+        test_gemm_fx_matches_python_integers(zkd, case, path=2)
+        ms, launches, macs = zkd.kernel_timing_read_i8()
+        assert launches == 1 and macs > 0, "the int8 tcgen05 kernel did not run"
+    finally:
+        zkd.kernel_timing(False)
+        zkd.set_option("gemm_path", 0)
+
+
 @pytest.mark.parametrize("case", GEMM_CASES)
-def test_gemm_fx_matches_python_integers(zkd, case):
+def test_gemm_fx_matches_python_integers(zkd, case, path=1):
     import torch
 
     M, N, K, batch, op_a, (a_top, a_dig), (b_top, b_dig), mode, cut = case
@@ -110,7 +138,7 @@ def test_gemm_fx_matches_python_integers(zkd, case):
     dC = _dev(fxc_from_ints(C0re, C0im))
     err = torch.zeros(1, dtype=torch.int32, device="cuda")
     msb = torch.zeros(1, dtype=torch.int32, device="cuda")
-    zkd.gemm_fx(M, N, K, batch, op_a, dA, a_top, a_dig, dB, b_top, b_dig, dC, mode, cut, 0, None, err, msb)
+    zkd.gemm_fx(M, N, K, batch, op_a, dA, a_top, a_dig, dB, b_top, b_dig, dC, mode, cut, path, None, err, msb)
     torch.cuda.synchronize()
     assert int(err.item()) == 0
     gre, gim = ints_from_fxc(dC.cpu().numpy())
