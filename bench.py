@@ -154,6 +154,20 @@ class Runner:
         return self.lam_host.numel() + self.X_host.numel()
 
 
+def aggregate(world: int, batch: int, steps: int, seconds: float, device: str = "cuda") -> tuple[float, float]:
+    """Whole-job throughput of `world` independent replicas ("replicas only"): every rank processed
+    batch*steps matrices in `seconds` of its own device time; the job's time is the MAX over ranks (one all_reduce of a
+    scalar, outside the timed region - there is no collective on the data path).  Returns (matrices/s, max seconds)."""
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([seconds], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    tmax = float(t.item())
+    return world * batch * steps / tmax, tmax
+
+
 def timed_steps(torch, runner_step, steps, flush):
     """per-step CUDA-event times (ms) on the current stream; L2 is flushed between steps outside the event pairs"""
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
@@ -276,11 +290,8 @@ def main():
     z.kernel_timing(False)
     clocks = sampler.stop()
     total_ms = sum(times)
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms_max = float(t.item())
-    value = world * b * args.steps / (total_ms_max * 1e-3)
+    value, tmax = aggregate(world, b, args.steps, total_ms * 1e-3)
+    total_ms_max = tmax * 1e3
 
     # ---- e2e: host buffers through zkd_diag_herm_host -------------------------------------------------------------
     for _ in range(2):
@@ -291,10 +302,7 @@ def main():
         run.step_e2e()  # synchronous: returns after the D2H copies completed
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = world * b * args.steps / float(te.item())
+    e2e_value, _ = aggregate(world, b, args.steps, e2e_s)
 
     if rank != 0:
         if world > 1:

@@ -234,3 +234,31 @@ def measure_imad_peak(millis: float = 50.0, stream=None) -> float:
     v = ctypes.c_double()
     _check(lib().zkd_measure_imad_peak(millis, ctypes.byref(v), _stream_ptr(stream)), "zkd_measure_imad_peak")
     return v.value
+
+
+# ---- host-side number helpers (no CUDA) --------------------------------------------------------------------------
+
+def pack(sign: int, exp: int, limbs_le, prec_bits: int = PREC) -> bytes:
+    """one real in the API layout from (sign, exp, 64-bit limbs little-endian)"""
+    n = prec_bits // 64
+    buf = ctypes.create_string_buffer(16 + prec_bits // 8)
+    arr = (ctypes.c_uint64 * n)(*[int(x) for x in limbs_le])
+    _check(lib().zkd_pack(buf, prec_bits, sign, ctypes.c_int64(exp), arr), "zkd_pack")
+    return buf.raw
+
+
+def unpack(src: bytes, prec_bits: int = PREC) -> tuple[int, int, list[int]]:
+    n = prec_bits // 64
+    s, e, out = ctypes.c_int(), ctypes.c_int64(), (ctypes.c_uint64 * n)()
+    _check(lib().zkd_unpack(ctypes.c_char_p(bytes(src)), prec_bits, ctypes.byref(s), ctypes.byref(e), out), "zkd_unpack")
+    return s.value, e.value, [int(x) for x in out]
+
+
+def from_double(v: float, prec_bits: int = PREC) -> bytes:
+    buf = ctypes.create_string_buffer(16 + prec_bits // 8)
+    _check(lib().zkd_from_double(buf, prec_bits, float(v)), "zkd_from_double")
+    return buf.raw
+
+
+def to_double(src: bytes, prec_bits: int = PREC) -> float:
+    return float(lib().zkd_to_double(ctypes.c_char_p(bytes(src)), prec_bits))
