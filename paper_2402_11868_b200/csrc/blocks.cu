@@ -27,7 +27,8 @@ int fxc_to_c64(size_t count, const int32_t* src, double2* dst, cudaStream_t s) {
 // One CTA per matrix.  F = ||A64||_F; a new cluster starts at j when mu_j - mu_{j-1} > 2^-tau F.
 // cl[j] = first column of j's cluster, cle[j] = one past its last column.
 __global__ void __launch_bounds__(256) cluster_kernel(int n, const double2* __restrict__ A64, const double* __restrict__ mu,
-                                                      int tau_bits, int* __restrict__ cl, int* __restrict__ cle,
+                                                      int tau_bits, const int* __restrict__ floor_msb /* [nb] or null */,
+                                                      int* __restrict__ cl, int* __restrict__ cle,
                                                       int* __restrict__ stats /* [nb][2]: n_clusters, max_cluster */) {
   __shared__ double s_red[8];
   __shared__ double s_F;
@@ -45,7 +46,9 @@ __global__ void __launch_bounds__(256) cluster_kernel(int n, const double2* __re
   }
   __syncthreads();
   if (tid == 0) {
-    const double thr = ldexp(s_F, -tau_bits);
+    // differences below 2^(floor_msb - 812) are noise of the matrix entries themselves (early splits, S4h): never split there
+    double thr = ldexp(s_F, -tau_bits);
+    if (floor_msb) thr = fmax(thr, ldexp(1.0, floor_msb[b] - 812));
     const double* m = mu + (size_t)b * n;
     int* c = cl + (size_t)b * n;
     int* ce = cle + (size_t)b * n;
@@ -66,8 +69,9 @@ __global__ void __launch_bounds__(256) cluster_kernel(int n, const double2* __re
     stats[2 * b + 1] = maxc;
   }
 }
-int cluster_detect(int n, int nb, const double2* A64, const double* mu, int tau_bits, int* cl, int* cle, int* stats, cudaStream_t s) {
-  cluster_kernel<<<nb, 256, 0, s>>>(n, A64, mu, tau_bits, cl, cle, stats);
+int cluster_detect(int n, int nb, const double2* A64, const double* mu, int tau_bits, const int* floor_msb, int* cl, int* cle,
+                   int* stats, cudaStream_t s) {
+  cluster_kernel<<<nb, 256, 0, s>>>(n, A64, mu, tau_bits, floor_msb, cl, cle, stats);
   count_launch();
   return launch_check();
 }

@@ -5,7 +5,8 @@
 namespace zkd {
 
 int fxc_to_c64(size_t count, const int32_t* src, double2* dst, cudaStream_t s);
-int cluster_detect(int n, int nb, const double2* A64, const double* mu, int tau_bits, int* cl, int* cle, int* stats, cudaStream_t s);
+int cluster_detect(int n, int nb, const double2* A64, const double* mu, int tau_bits, const int* floor_msb /*[nb], may be null*/,
+                   int* cl, int* cle, int* stats, cudaStream_t s);
 int init_x(size_t count, const double2* V, int32_t* X, cudaStream_t s);
 int gram_blocks(int n, int nb, const int32_t* X, const int32_t* Y, const int* cl, int32_t* G, cudaStream_t s);
 int ns_build(int n, int nb, const int* cl, int32_t* G, int* msb_out, cudaStream_t s);
@@ -25,7 +26,13 @@ int ingest_herm(int N, int batch, const void* A_api, int32_t* A_fx, int* scale /
 struct SubProblem { int b, col0; };  // matrix index and first column of the cluster
 int sub_gather(int n, int nb, int m, int nsub, const SubProblem* subs_dev, const int32_t* S, int32_t* H /*nsub m m*/,
                int32_t* cbar /*FxR nsub*/, int* kshift /*nsub*/, int* degenerate /*nsub*/, int degenerate_msb,
-               const int* noise_parent /*nb, may be null*/, int* noise_child /*nsub*/, cudaStream_t s);
+               const int* noise_parent /*nb, may be null*/, int* noise_child /*nsub*/, int* floor_child /*nsub, may be null*/,
+               int min_split_msb /* S4h: blocks with a smaller spread are reported degenerate; 0 for S5 */, cudaStream_t s);
+// S4h (early split): U := V64 (fp64 eigenvectors of the scaled cluster blocks) placed on the diagonal blocks of Um, and the
+// cluster table refined by the sub-problems' own clusters; degenerate sub-problems keep the identity and their cluster
+int split_scatter(int n, int nb, int m, int nsub, const SubProblem* subs_dev, const double2* V64 /*nsub m m*/,
+                  const int* sub_cl, const int* sub_cle, const int* degenerate, int32_t* Um /*nb n n*/, int* cl, int* cle,
+                  cudaStream_t s);
 int sub_scatter(int n, int nb, int m, int nsub, const SubProblem* subs_dev, const int32_t* U /*nsub m m*/, const int32_t* lam_sub,
                 const int32_t* cbar, const int* kshift, const int* degenerate, int32_t* Um /*nb n n*/, int32_t* theta, cudaStream_t s);
 int identity_blocks(int n, int nb, int32_t* Um, cudaStream_t s);

@@ -90,14 +90,15 @@ __global__ void __launch_bounds__(128) sub_gather_kernel(int n, int nb, int m, c
                                                          int32_t* __restrict__ cbar, int* __restrict__ kshift,
                                                          int* __restrict__ degenerate, int degenerate_msb_base,
                                                          const int* __restrict__ noise_parent, int* __restrict__ noise_child,
-                                                         int nsub) {
+                                                         int* __restrict__ floor_child, int min_split_msb, int nsub) {
   __shared__ int32_t s_c[ND];
   __shared__ int s_msb;
   const int p = blockIdx.x;
   const SubProblem sp = subs[p];
   // entries of S are known to ~2^-812 in the units of depth 0, i.e. to 2^(noise - 812) in the units of this level
   const int noise = noise_parent ? noise_parent[sp.b] : 0;
-  const int degenerate_msb = degenerate_msb_base + noise;
+  // blocks whose spread is below min_split_msb are also reported "degenerate" (S4h: not worth splitting now)
+  const int degenerate_msb = max(degenerate_msb_base + noise, min_split_msb - 1);
   const size_t per = (size_t)n * n, count = per * nb;
   const size_t hcount = (size_t)m * m * nsub;
   const int32_t* Sr = S;
@@ -171,12 +172,14 @@ __global__ void __launch_bounds__(128) sub_gather_kernel(int n, int nb, int m, c
     kshift[p] = 810 - s_msb;
     degenerate[p] = s_msb <= degenerate_msb ? 1 : 0;
     noise_child[p] = noise + max(0, 810 - s_msb);
+    if (floor_child) floor_child[p] = degenerate_msb + (810 - s_msb);  // the same noise level in the scaled units of H
   }
 }
 int sub_gather(int n, int nb, int m, int nsub, const SubProblem* subs_dev, const int32_t* S, int32_t* H, int32_t* cbar, int* kshift,
-               int* degenerate, int degenerate_msb, const int* noise_parent, int* noise_child, cudaStream_t s) {
+               int* degenerate, int degenerate_msb, const int* noise_parent, int* noise_child, int* floor_child, int min_split_msb,
+               cudaStream_t s) {
   sub_gather_kernel<<<nsub, 128, 0, s>>>(n, nb, m, subs_dev, S, H, cbar, kshift, degenerate, degenerate_msb, noise_parent,
-                                         noise_child, nsub);
+                                         noise_child, floor_child, min_split_msb, nsub);
   count_launch();
   return launch_check();
 }
@@ -228,6 +231,37 @@ __global__ void __launch_bounds__(128) sub_scatter_kernel(int n, int nb, int m, 
 int sub_scatter(int n, int nb, int m, int nsub, const SubProblem* subs_dev, const int32_t* U, const int32_t* lam_sub,
                 const int32_t* cbar, const int* kshift, const int* degenerate, int32_t* Um, int32_t* theta, cudaStream_t s) {
   sub_scatter_kernel<<<nsub, 128, 0, s>>>(n, nb, m, nsub, subs_dev, U, lam_sub, cbar, kshift, degenerate, Um, theta);
+  count_launch();
+  return launch_check();
+}
+
+// S4h: one CTA per sub-problem
+__global__ void __launch_bounds__(128) split_scatter_kernel(int n, int nb, int m, int nsub, const SubProblem* __restrict__ subs,
+                                                            const double2* __restrict__ V64, const int* __restrict__ sub_cl,
+                                                            const int* __restrict__ sub_cle, const int* __restrict__ degenerate,
+                                                            int32_t* __restrict__ Um, int* __restrict__ cl, int* __restrict__ cle) {
+  const int p = blockIdx.x;
+  if (degenerate[p]) return;
+  const SubProblem sp = subs[p];
+  const size_t per = (size_t)n * n, count = per * nb;
+  for (int e = threadIdx.x; e < m * m; e += blockDim.x) {
+    const int i = e / m, j = e % m;
+    const double2 v = V64[(size_t)p * m * m + e];
+    const size_t dst = (size_t)sp.b * per + (size_t)(sp.col0 + i) * n + (sp.col0 + j);
+    int32_t d[ND];
+    fx_from_double(d, v.x);
+    fx_store(Um, count, dst, d);
+    fx_from_double(d, v.y);
+    fx_store(Um + (size_t)ND * count, count, dst, d);
+  }
+  for (int j = threadIdx.x; j < m; j += blockDim.x) {
+    cl[(size_t)sp.b * n + sp.col0 + j] = sp.col0 + sub_cl[(size_t)p * m + j];
+    cle[(size_t)sp.b * n + sp.col0 + j] = sp.col0 + sub_cle[(size_t)p * m + j];
+  }
+}
+int split_scatter(int n, int nb, int m, int nsub, const SubProblem* subs_dev, const double2* V64, const int* sub_cl,
+                  const int* sub_cle, const int* degenerate, int32_t* Um, int* cl, int* cle, cudaStream_t s) {
+  split_scatter_kernel<<<nsub, 128, 0, s>>>(n, nb, m, nsub, subs_dev, V64, sub_cl, sub_cle, degenerate, Um, cl, cle);
   count_launch();
   return launch_check();
 }

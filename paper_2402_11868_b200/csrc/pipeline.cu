@@ -95,6 +95,107 @@ int read_scalars(Ctx& c, const int* dev, int n, int* out) {
   return ZKD_OK;
 }
 
+using Groups = std::map<int, std::vector<SubProblem>>;
+
+// clusters with more than one member, grouped by size (one batched sub-problem set per size)
+Groups build_groups(const std::vector<int>& h_cl, int n, int nb) {
+  Groups groups;
+  for (int b = 0; b < nb; ++b) {
+    int j = 0;
+    while (j < n) {
+      int k = j;
+      while (k + 1 < n && h_cl[(size_t)b * n + k + 1] == h_cl[(size_t)b * n + j]) ++k;
+      if (k > j) groups[k - j + 1].push_back(SubProblem{b, j});
+      j = k + 1;
+    }
+  }
+  return groups;
+}
+
+// S4h, early cluster split.  Inside a cluster the correction is deflated, so its convergence is only linear, at
+// (spread of the cluster / gap to the outside)^2 per step, when the cluster has internal structure (c4: the 29-dimensional
+// cluster holds 2^-21 .. 2^-60 and 24 zeros).  As soon as that structure stands above the noise of S_c = X_c^H W_c
+// (Ritz-value error ~ |R|^2 / gap), the scaled block 2^k (S_c - mean) is diagonalised in fp64 by the seed kernel, the
+// cluster basis is rotated by those eigenvectors (X_c, W_c <- X_c U, W_c U) and the cluster table is refined by the block's
+// own clusters.  U is unitary to fp64 only; the S4f Newton-Schulz step of the following passes repairs that quadratically.
+// Blocks whose structure is below the noise (true multiplicities) are left alone.  Sets *changed when any cluster split.
+int try_split(Ctx& c, int n, int nb, const int32_t* Sm, int msb_r, int tol_msb, const int* noise, const int32_t* Xc,
+              const int32_t* Wc, int32_t* Xo, int32_t* Wo, int32_t* Um, int* cl, int* cle, std::vector<int>& h_cl, bool* changed) {
+  const Options& opt = options();
+  cudaStream_t s = c.s;
+  *changed = false;
+  const Groups groups = build_groups(h_cl, n, nb);
+  if (groups.empty()) return ZKD_OK;
+  // eigenvalues of a block are told apart only when they differ by more than (a) the Ritz-value noise ~ |R|^2 / gap and
+  // (b) 2^16 |R|: the correction E_ij = C_ij / (theta_j - theta_i) between the new clusters must stay small
+  // and (c) 2^-190: ecalc's reciprocal range.
+  const int noise_msb = std::max(std::max(tol_msb + 6, 812 - 190), std::max(2 * msb_r - 812 + opt.split_margin_bits, msb_r + 16));
+  // Worth it?  Unsplit, the cluster gains 2 log2(gap / spread) bits per step with gap >= 2^-tau |A|_F ~ 2^(790-812); split
+  // (or with no structure) the step gains about e + 40 bits (windowed quadratic convergence), and no more than what is
+  // left to the tolerance is needed.  Split only blocks whose spread makes the linear rate the slower one (c4), not those
+  // whose structure is far below the gap (c5: 2^-200 spacing, left to S5).
+  const int want = std::min(812 - msb_r + 40, msb_r - tol_msb + 10);
+  const int min_split_msb = 812 - opt.tau_bits - 2 - want / 2;
+  const Arena::Mark mark = c.ar.mark();
+  bool any = false, first = true;
+  for (const auto& kv : groups) {
+    const int m = kv.first;
+    const int nsub = (int)kv.second.size();
+    c.ar.release(mark);
+    const size_t hc = (size_t)m * m * nsub;
+    SubProblem* subs_dev = c.ar.get<SubProblem>((size_t)nsub);
+    int32_t* H = (int32_t*)c.ar.alloc(FxC::bytes(hc));
+    int32_t* cbar = (int32_t*)c.ar.alloc(FxR::bytes((size_t)nsub));
+    double2* H64 = c.ar.get<double2>(hc);
+    double2* V64 = c.ar.get<double2>(hc);
+    double* mu = c.ar.get<double>((size_t)m * nsub);
+    int* ints = c.ar.get<int>((size_t)nsub * (6 + 2 * (size_t)m));
+    if (!subs_dev || !H || !cbar || !H64 || !V64 || !mu || !ints) return ZKD_ERR_WORKSPACE;
+    int *kshift = ints, *degen = ints + nsub, *noise_sub = ints + 2 * nsub, *floor_sub = ints + 3 * nsub, *sstats = ints + 4 * nsub;
+    int *scl = ints + 6 * nsub, *scle = scl + (size_t)m * nsub;
+    ZKD_CUDA_TRY(cudaMemcpyAsync(subs_dev, kv.second.data(), sizeof(SubProblem) * nsub, cudaMemcpyHostToDevice, s));
+    ZKD_TRY(sub_gather(n, nb, m, nsub, subs_dev, Sm, H, cbar, kshift, degen, noise_msb, noise, noise_sub, floor_sub, min_split_msb, s));
+    std::vector<int> hdeg((size_t)nsub);
+    ZKD_CUDA_TRY(cudaMemcpyAsync(hdeg.data(), degen, sizeof(int) * nsub, cudaMemcpyDeviceToHost, s));
+    ZKD_CUDA_TRY(cudaStreamSynchronize(s));  // also keeps kv.second alive for the copy above
+    bool all_deg = true;
+    for (int v : hdeg) all_deg = all_deg && v;
+    if (all_deg) continue;
+    if (first) { ZKD_TRY(identity_blocks(n, nb, Um, s)); first = false; }
+    ZKD_TRY(fxc_to_c64(hc, H, H64, s));
+    ZKD_TRY(seed_fp64(m, nsub, (const double*)H64, mu, (double*)V64, opt.seed_sweeps, s));
+    ZKD_TRY(cluster_detect(m, nsub, H64, mu, opt.tau_bits, floor_sub, scl, scle, sstats, s));
+    ZKD_TRY(split_scatter(n, nb, m, nsub, subs_dev, V64, scl, scle, degen, Um, cl, cle, s));
+    any = true;
+  }
+  if (any) {
+    // rotate with the OLD cluster table (the blocks of Um), then adopt the refined one
+    std::vector<int> h_new((size_t)n * nb), h_cle_old((size_t)n * nb);
+    int* cl_old = c.ar.get<int>((size_t)n * nb);
+    int* cle_old = c.ar.get<int>((size_t)n * nb);
+    if (!cl_old || !cle_old) return ZKD_ERR_WORKSPACE;
+    ZKD_CUDA_TRY(cudaMemcpyAsync(h_new.data(), cl, sizeof(int) * n * nb, cudaMemcpyDeviceToHost, s));
+    ZKD_CUDA_TRY(cudaMemcpyAsync(cl_old, h_cl.data(), sizeof(int) * n * nb, cudaMemcpyHostToDevice, s));
+    for (int b = 0; b < nb; ++b) {
+      int j = 0;
+      while (j < n) {
+        int k = j;
+        while (k + 1 < n && h_cl[(size_t)b * n + k + 1] == h_cl[(size_t)b * n + j]) ++k;
+        for (int t = j; t <= k; ++t) h_cle_old[(size_t)b * n + t] = k + 1;
+        j = k + 1;
+      }
+    }
+    ZKD_CUDA_TRY(cudaMemcpyAsync(cle_old, h_cle_old.data(), sizeof(int) * n * nb, cudaMemcpyHostToDevice, s));
+    ZKD_TRY(block_apply(n, nb, nullptr, Xc, Um, cl_old, cle_old, false, Xo, nullptr, s));
+    ZKD_TRY(block_apply(n, nb, nullptr, Wc, Um, cl_old, cle_old, false, Wo, nullptr, s));
+    ZKD_CUDA_TRY(cudaStreamSynchronize(s));
+    *changed = h_new != h_cl;
+    h_cl.swap(h_new);
+  }
+  c.ar.release(mark);
+  return ZKD_OK;
+}
+
 int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* lam, int depth, const int* noise, LevelStats* st) {
   const Options& opt = options();
   const size_t cnt = (size_t)n * n * nb;
@@ -109,6 +210,9 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
   int* stats = c.ar.get<int>((size_t)2 * nb);
   int32_t* Sm = (int32_t*)c.ar.alloc(fxc);
   int32_t* theta = lam;
+  int* cl0 = c.ar.get<int>((size_t)n * nb);   // the clusters as detected (S4h refines cl / cle)
+  int* cle0 = c.ar.get<int>((size_t)n * nb);
+  bool split_done = false;
   const Arena::Mark mark1 = c.ar.mark();
   // short-lived
   double2* A64 = c.ar.get<double2>(cnt);
@@ -120,13 +224,14 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
   int32_t* T = (int32_t*)c.ar.alloc(fxc);
   int32_t* Gm = (int32_t*)c.ar.alloc(fxc);
   int* scal = c.ar.get<int>(S_NUM);
+  if (!cl0 || !cle0) return ZKD_ERR_WORKSPACE;
   if (!cl || !cle || !stats || !Sm || !A64 || !mu || !V || !W || !R || !Cm || !T || !Gm || !scal) return ZKD_ERR_WORKSPACE;
   if (gemm_workspace_bytes(n, n, n, nb) > c.gemm_ws_bytes) return ZKD_ERR_WORKSPACE;
 
   // S1-S3
   ZKD_TRY(fxc_to_c64(cnt, A, A64, s));
   ZKD_TRY(seed_fp64(n, nb, (const double*)A64, mu, (double*)V, opt.seed_sweeps, s));
-  ZKD_TRY(cluster_detect(n, nb, A64, mu, opt.tau_bits, cl, cle, stats, s));
+  ZKD_TRY(cluster_detect(n, nb, A64, mu, opt.tau_bits, nullptr, cl, cle, stats, s));
   int32_t* Xc = X;  // current iterate (may end up in T's storage; copied back at the end)
   int32_t* Tc = T;
   int32_t* Wc = W;
@@ -144,6 +249,8 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
   ZKD_TRY(gemm_complex(n, n, n, nb, side(A, topA, kND, false), side(Xc, topX, 3, false), Wc, GemmMode::Assign, -1, opt.gemm_path,
                        c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s));
 
+  ZKD_CUDA_TRY(cudaMemcpyAsync(cl0, cl, sizeof(int) * n * nb, cudaMemcpyDeviceToDevice, s));
+  ZKD_CUDA_TRY(cudaMemcpyAsync(cle0, cle, sizeof(int) * n * nb, cudaMemcpyDeviceToDevice, s));
   // cluster table to the host (needed for S5 and to pick the singleton fast path)
   std::vector<int> h_cl((size_t)n * nb);
   ZKD_CUDA_TRY(cudaMemcpyAsync(h_cl.data(), cl, sizeof(int) * n * nb, cudaMemcpyDeviceToHost, s));
@@ -189,6 +296,21 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
     ZKD_CUDA_TRY(cudaMemsetAsync(scal, 0, sizeof(int) * S_NUM, s));
     if (msb_r == 0) continue;  // residual exactly zero: only the orthonormalisation is still converging
 
+    // S4h: split clusters whose internal structure stands above the noise of S_c
+    if (!singletons && opt.early_split && msb_g <= 812 - 45) {
+      bool changed = false;
+      ZKD_TRY(try_split(c, n, nb, Sm, msb_r, tol_msb, noise, Xc, Wc, Tc, Cc, Gm, cl, cle, h_cl, &changed));
+      if (changed) {
+        split_done = true;
+        std::swap(Xc, Tc);
+        std::swap(Wc, Cc);
+        singletons = true;
+        for (size_t t = 0; t < h_cl.size() && singletons; ++t) singletons = h_cl[t] == (int)(t % n);
+        prev_msb_r = 1 << 30;
+        continue;  // S4f / S4c again with the rotated basis and the finer clusters
+      }
+    }
+
     // S4d: C = X^H R on windows sized for this step's gain
     const int e = 812 - msb_r;                        // residual ~ 2^-e
     const int pb = std::max(40, std::min(e + 40, msb_r + 30));  // relative bits worth computing for the correction
@@ -214,20 +336,20 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
                          c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s));
   }
   if (st) { st->steps = steps + 1; st->status = status; }
+  if (split_done) {
+    // Vectors of clusters that were split apart are orthogonal only to residual / gap, and the gaps inside a detected
+    // cluster can be tiny (c4: 2^-61).  One symmetric (Loewdin / Newton-Schulz) orthonormalisation over the clusters AS
+    // DETECTED squares that error; it moves the vectors by the same residual / gap inside a cluster whose spread is
+    // <= 2^-tau, i.e. the residual grows by less than itself.
+    ZKD_TRY(gram_blocks(n, nb, Xc, Xc, cl0, Gm, s));
+    ZKD_TRY(ns_build(n, nb, cl0, Gm, nullptr, s));
+    ZKD_TRY(block_apply(n, nb, Xc, Xc, Gm, cl0, cle0, false, Tc, nullptr, s));
+    std::swap(Xc, Tc);
+  }
   if (Xc != X) ZKD_CUDA_TRY(cudaMemcpyAsync(X, Xc, fxc, cudaMemcpyDeviceToDevice, s));
 
   // S5: clusters with more than one member -> Rayleigh-Ritz on the projected matrix, by recursion
-  std::map<int, std::vector<SubProblem>> groups;
-  for (int b = 0; b < nb; ++b) {
-    int j = 0;
-    while (j < n) {
-      int k = j;
-      while (k + 1 < n && h_cl[(size_t)b * n + k + 1] == h_cl[(size_t)b * n + j]) ++k;
-      const int m = k - j + 1;
-      if (m > 1) groups[m].push_back(SubProblem{b, j});
-      j = k + 1;
-    }
-  }
+  Groups groups = build_groups(h_cl, n, nb);
   if (!groups.empty()) {
     ZKD_CUDA_TRY(cudaStreamSynchronize(s));  // short-lived buffers are about to be reused
     c.ar.release(mark1);
@@ -252,7 +374,7 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
       int* noise_sub = c.ar.get<int>((size_t)nsub);
       if (!subs_dev || !H || !U || !cbar || !lam_sub || !kshift || !degen || !noise_sub) return ZKD_ERR_WORKSPACE;
       ZKD_CUDA_TRY(cudaMemcpyAsync(subs_dev, kv.second.data(), sizeof(SubProblem) * nsub, cudaMemcpyHostToDevice, s));
-      ZKD_TRY(sub_gather(n, nb, m, nsub, subs_dev, Sm, H, cbar, kshift, degen, tol_msb + 6, noise, noise_sub, s));
+      ZKD_TRY(sub_gather(n, nb, m, nsub, subs_dev, Sm, H, cbar, kshift, degen, tol_msb + 6, noise, noise_sub, nullptr, 0, s));
       std::vector<int> hdeg((size_t)nsub);
       ZKD_CUDA_TRY(cudaMemcpyAsync(hdeg.data(), degen, sizeof(int) * nsub, cudaMemcpyDeviceToHost, s));
       ZKD_CUDA_TRY(cudaStreamSynchronize(s));
