@@ -168,6 +168,37 @@ def aggregate(world: int, batch: int, steps: int, seconds: float, device: str = 
     return world * batch * steps / tmax, tmax
 
 
+def measured_peaks() -> dict:
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f)
+    except (OSError, ValueError):
+        return {}
+
+
+def roofline_object(gemm_ms, gemm_launches, gemm_macs, i8_ms, i8_launches, i8_macs, imad_peak, steps, total_ms) -> dict:
+    """The engine that carries most of the GEMM time.  IMAD path: digit products (IMAD.WIDE) per second against the live
+    microbenchmark.  int8 path: s8 x s8 MACs per second, x2 = op/s, against 2 x the measured dense bf16 peak of
+    MEASURED_PEAKS.json (int8 is nominally 2 x bf16 on B200; fallback: the profiling guide's nominal 4.5 PFLOP/s int8)."""
+    if i8_ms > gemm_ms:
+        mp = measured_peaks()
+        if "bf16_tflops" in mp:
+            peak_tops, src = 2.0 * float(mp["bf16_tflops"]), "2 x MEASURED_PEAKS.json bf16_tflops (burst; kernel timed alone per launch)"
+        else:
+            peak_tops, src = 4500.0, "fallback: nominal dense int8 4.5 POP/s (B200_PROFILING.md); MEASURED_PEAKS.json absent"
+        achieved = 2.0 * i8_macs / (i8_ms * 1e-3) / 1e12
+        return {"bound": "tensor", "kernel": "gemm_i8_kernel", "achieved": achieved, "peak": peak_tops, "unit": "TOP/s (int8)",
+                "frac": achieved / peak_tops, "traffic": None, "launches": i8_launches, "kernel_ms_per_step": i8_ms / steps,
+                "share_of_step": i8_ms / total_ms, "int8_macs_per_step": i8_macs / steps, "peak_source": src,
+                "imad_gemm_ms_per_step": gemm_ms / steps}
+    achieved = gemm_macs / (gemm_ms * 1e-3) if gemm_ms > 0 else 0.0
+    return {"bound": "alu", "kernel": "gemm_digits_kernel", "achieved": achieved / 1e12, "peak": imad_peak / 1e12, "unit": "TIMAD/s",
+            "frac": achieved / imad_peak if imad_peak else None, "traffic": None, "launches": gemm_launches,
+            "kernel_ms_per_step": gemm_ms / steps, "share_of_step": gemm_ms / total_ms, "digit_macs_per_step": gemm_macs / steps,
+            "peak_source": "measured live (zkd_measure_imad_peak): IMAD.WIDE with 64-bit accumulate; nominal 32-bit IMAD rate "
+                           "148 SM x 64 lanes/clk x 1.965 GHz = 18.6"}
+
+
 def timed_steps(torch, runner_step, steps, flush):
     """per-step CUDA-event times (ms) on the current stream; L2 is flushed between steps outside the event pairs"""
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
@@ -287,6 +318,7 @@ def main():
     barrier()
     launches, macs = z.counters()
     gemm_ms, gemm_launches, gemm_macs = z.kernel_timing_read()
+    i8_ms, i8_launches, i8_macs = z.kernel_timing_read_i8()
     z.kernel_timing(False)
     clocks = sampler.stop()
     total_ms = sum(times)
@@ -310,16 +342,9 @@ def main():
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (digit GEMM; bound: integer-multiply pipe) --------------------------------
-    peak = z.measure_imad_peak(60.0)  # measured, register-only IMAD.WIDE loop on all SMs (DESIGN.md "Peaks")
-    achieved = gemm_macs / (gemm_ms * 1e-3) if gemm_ms > 0 else 0.0
-    roofline = {
-        "bound": "alu", "kernel": "gemm_digits_kernel", "achieved": achieved / 1e12, "peak": peak / 1e12, "unit": "TIMAD/s",
-        "frac": achieved / peak if peak else None, "traffic": None,
-        "launches": gemm_launches, "kernel_ms_per_step": gemm_ms / args.steps, "share_of_step": gemm_ms / total_ms,
-        "digit_macs_per_step": gemm_macs / args.steps,
-        "peak_source": "measured live (zkd_measure_imad_peak); nominal 148 SM x 64 lanes/clk x 1.965 GHz = 18.6",
-    }
+    # ---- roofline of the dominant GEMM engine: IMAD digit GEMM (integer-multiply pipe) or int8 tcgen05 (tensor pipe) ----
+    peak = z.measure_imad_peak(60.0)  # measured, register-only IMAD.WIDE loop on all SMs (DESIGN.md 6.1)
+    roofline = roofline_object(gemm_ms, gemm_launches, gemm_macs, i8_ms, i8_launches, i8_macs, peak, args.steps, total_ms)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -338,7 +363,7 @@ def main():
     # ---- context rows: the other configs and a saturating batch (not the headline) --------------------------------
     if not args.no_extra and world == 1:
         extra = {}
-        for nm, bb, k in (("c1", 1, 5), ("c2", 256, 3), ("c3", 1, 3), ("c4", 512, 2)):
+        for nm, bb, k in (("c1", 1, 5), ("c2", 1, 5), ("c2", 256, 3), ("c3", 1, 3), ("c4", 512, 2), ("c5", 1, 2)):
             if nm == args.workload and bb == b:
                 continue
             try:
@@ -349,10 +374,12 @@ def main():
                 z.kernel_timing(True)
                 ts = timed_steps(torch, r2.step, k, flush)
                 gms, gl, gm = z.kernel_timing_read()
+                g8 = z.kernel_timing_read_i8()
                 z.kernel_timing(False)
                 ms = sum(ts) / len(ts)
-                extra[f"{nm}x{b2}"] = {"matrices_per_s": b2 / (ms * 1e-3), "ms_per_step": ms,
-                                       "gemm_share": gms / sum(ts), "gemm_frac_of_peak": (gm / (gms * 1e-3) / peak) if gms > 0 else None}
+                rf = roofline_object(gms, gl, gm, g8[0], g8[1], g8[2], peak, k, sum(ts))
+                extra[f"{nm}x{b2}"] = {"matrices_per_s": b2 / (ms * 1e-3), "ms_per_step": ms, "gemm_engine": rf["kernel"],
+                                       "gemm_share": rf["share_of_step"], "gemm_frac_of_peak": rf["frac"]}
                 del r2
                 torch.cuda.empty_cache()
             except Exception as e:  # context only; never fails the bench line
