@@ -145,8 +145,8 @@ int gram_blocks(int n, int nb, const int32_t* X, const int32_t* Y, const int* cl
 }
 
 // ---- M := (I - G)/2 on cluster blocks (Newton-Schulz orthonormalisation step), msb of (G - I) ---------------------------
-__global__ void __launch_bounds__(256) ns_build_kernel(int n, int nb, const int* __restrict__ cl, int32_t* __restrict__ G,
-                                                       int* __restrict__ msb_out) {
+__global__ void __launch_bounds__(256) ns_build_kernel(int n, int nb, const int* __restrict__ cl, const int* __restrict__ cle_skip1,
+                                                       int32_t* __restrict__ G, int* __restrict__ msb_out) {
   const size_t per = (size_t)n * n, count = per * nb;
   const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= count * 2) return;
@@ -154,6 +154,7 @@ __global__ void __launch_bounds__(256) ns_build_kernel(int n, int nb, const int*
   const size_t e = t % count;
   const int b = (int)(e / per), i = (int)((e % per) / n), j = (int)(e % n);
   if (cl[(size_t)b * n + i] != cl[(size_t)b * n + j]) return;
+  if (cle_skip1 && cle_skip1[(size_t)b * n + j] - cl[(size_t)b * n + j] == 1) return;  // singletons are handled elsewhere
   int32_t* p = G + (part ? (size_t)ND * count : 0);
   int32_t g[ND], r[ND];
   fx_load(g, p, count, e);
@@ -164,9 +165,9 @@ __global__ void __launch_bounds__(256) ns_build_kernel(int n, int nb, const int*
   fx_half(g, r);                            // (I - G)/2
   fx_store(p, count, e, g);
 }
-int ns_build(int n, int nb, const int* cl, int32_t* G, int* msb_out, cudaStream_t s) {
+int ns_build(int n, int nb, const int* cl, int32_t* G, int* msb_out, cudaStream_t s, const int* cle_skip1) {
   const size_t t = (size_t)n * n * nb * 2;
-  ns_build_kernel<<<(unsigned)((t + 255) / 256), 256, 0, s>>>(n, nb, cl, G, msb_out);
+  ns_build_kernel<<<(unsigned)((t + 255) / 256), 256, 0, s>>>(n, nb, cl, cle_skip1, G, msb_out);
   count_launch();
   return launch_check();
 }
@@ -248,6 +249,27 @@ int theta_from_diag(int n, int nb, const int32_t* S, int32_t* theta, cudaStream_
   return launch_check();
 }
 
+// ---- smallest gap between neighbouring clusters: gap_inv_out <- max(1024 - msb(theta_{j+1} - theta_j)) over cluster borders ----
+// (columns are in ascending order of theta, so the closest pair of eigenvalues of different clusters is a neighbouring pair)
+__global__ void __launch_bounds__(128) min_gap_kernel(int n, int nb, const int32_t* __restrict__ theta, const int* __restrict__ cl,
+                                                      int* __restrict__ gap_inv_out) {
+  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (size_t)n * nb) return;
+  const int j = (int)(t % n);
+  if (j + 1 >= n || cl[t] == cl[t + 1]) return;
+  int32_t a[ND], c[ND], d[ND];
+  fx_load(a, theta, (size_t)n * nb, t);
+  fx_load(c, theta, (size_t)n * nb, t + 1);
+  fx_sub(d, c, a);
+  if (fx_is_neg(d)) { fx_neg(a, d); atomicMax(gap_inv_out, 1024 - fx_msb(a)); }
+  else atomicMax(gap_inv_out, 1024 - fx_msb(d));
+}
+int min_gap(int n, int nb, const int32_t* theta, const int* cl, int* gap_inv_out, cudaStream_t s) {
+  min_gap_kernel<<<(unsigned)(((size_t)n * nb + 127) / 128), 128, 0, s>>>(n, nb, theta, cl, gap_inv_out);
+  count_launch();
+  return launch_check();
+}
+
 // ---- complex FX add: X += T ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) fx_add_kernel(size_t reals, int32_t* __restrict__ X, const int32_t* __restrict__ T) {
   const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -295,10 +317,12 @@ __device__ __forceinline__ void block_sum_cols(int64_t (&acc)[NACC2], int64_t* s
 __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int32_t* __restrict__ X, int32_t* __restrict__ W,
                                                              int32_t* __restrict__ R, int32_t* __restrict__ S,
                                                              int32_t* __restrict__ theta, int* __restrict__ msb_g_out,
-                                                             int* __restrict__ msb_r_out) {
+                                                             int* __restrict__ msb_r_out, const int* __restrict__ cl,
+                                                             const int* __restrict__ cle) {
   __shared__ int64_t s_part[8 * FXP_NACC];
   __shared__ int s_msb;
   const int b = blockIdx.x / n, j = blockIdx.x % n;
+  if (cl && cle[blockIdx.x] - cl[blockIdx.x] > 1) return;  // mixed levels: columns of larger clusters take the GEMM path
   const int tid = threadIdx.x, nwarps = blockDim.x >> 5;
   const size_t per = (size_t)n * n, count = per * nb;
   int32_t* Xr = X;  int32_t* Xi = X + (size_t)ND * count;
@@ -400,10 +424,10 @@ __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int3
   if (tid == 0 && msb_r_out) atomicMax(msb_r_out, s_msb);
 }
 int singleton_step(int n, int nb, int32_t* X, int32_t* W, int32_t* R, int32_t* S, int32_t* theta, int* msb_g_out, int* msb_r_out,
-                   cudaStream_t s) {
+                   cudaStream_t s, const int* cl, const int* cle) {
   int threads = (n + 31) / 32 * 32;
   if (threads > 256) threads = 256;
-  singleton_step_kernel<<<(unsigned)((size_t)n * nb), threads, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out);
+  singleton_step_kernel<<<(unsigned)((size_t)n * nb), threads, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
   count_launch();
   return launch_check();
 }
@@ -490,7 +514,7 @@ __global__ void __launch_bounds__(128) ecalc_kernel(int n, int nb, const int32_t
 #pragma unroll
     for (int k = 0; k < ND; ++k) d[k] = u[k]; }
   const int msb = fx_msb(d);  // |d| in [2^(msb-1-812), 2^(msb-812))
-  if (msb < 812 - 200) {      // different clusters must be apart; anything this close is a planning error
+  if (msb < 812 - 400) {      // different clusters must be apart; anything this close is a planning error
     if (err_flag) atomicOr(err_flag, 2);
     fx_store(Cr, count, eij, z); fx_store(Ci, count, eij, z);
     fx_store(Cr, count, eji, z); fx_store(Ci, count, eji, z);

@@ -57,7 +57,9 @@ static const GemmInstance* pick_instance(int nwP, int nwQ) {
 struct PrepArgs {
   const int32_t* src;  // complex FX, batch * rows * cols
   int32_t* dst;        // [3*batch][nw][R][C]
-  size_t src_count;    // batch * rows * cols
+  size_t src_count;    // complex elements per plane of the source array
+  int ld;              // row stride of the stored matrix
+  const int* off;      // per batch element start (null: b * R * C)
   int R, C;            // destination dims (P: M x K, Q: K x N)
   int batch;
   int transpose;       // source stored C x R and conjugated
@@ -91,7 +93,8 @@ __global__ void __launch_bounds__(256) prep_kernel(PrepArgs2 both) {
   const int b = (int)(e / per);
   const size_t rc = e % per;
   const int r = (int)(rc / a.C), c = (int)(rc % a.C);
-  const size_t sidx = a.transpose ? ((size_t)b * per + (size_t)c * a.R + r) : e;
+  const size_t base = a.off ? (size_t)a.off[b] : (size_t)b * per;
+  const size_t sidx = base + (a.transpose ? ((size_t)c * a.ld + r) : ((size_t)r * a.ld + c));
   const int32_t* __restrict__ re = a.src;
   const int32_t* __restrict__ im = a.src + (size_t)kND * a.src_count;
   const int32_t top_re = re[(size_t)(kND - 1) * a.src_count + sidx];
@@ -171,6 +174,9 @@ struct CombineArgs {
   const int32_t* raw;  // [split][3*batch][nc][M*N]
   int32_t* dst;        // complex FX, batch*M*N
   size_t mn;           // M*N
+  int N, ld;           // destination view: element (i, j) of batch element b at off[b] + i * ld + j
+  const int* off;      // null: b * mn
+  size_t plane_count;  // complex elements per destination plane
   int batch, nc, nsplit;
   int base_bit;        // FX bit position of raw column 0's LSB (may be negative)
   int cut_bit;         // clear result bits below this FX bit (<= 0: none)
@@ -178,7 +184,9 @@ struct CombineArgs {
   int* msb_out;
 };
 
-// one thread per (element, part); part 0 = Re = k1 - k3, part 1 = Im = k1 + k2
+// one thread per (element, part); part 0 = Re = k1 - k3, part 1 = Im = k1 + k2.
+// NS: compile-time bound of the split count (0: any), so that the loads of all splits of a column chunk are in flight together
+template <int NS>
 __global__ void __launch_bounds__(256) combine_kernel(CombineArgs a) {
   const size_t tot = a.mn * a.batch;
   const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -196,7 +204,9 @@ __global__ void __launch_bounds__(256) combine_kernel(CombineArgs a) {
 
   int q = a.base_bit >= 0 ? a.base_bit / DB : -((-a.base_bit + DB - 1) / DB);
   const int sh = a.base_bit - q * DB;  // 0..27
-  int32_t* dst = a.dst + (part ? (size_t)kND * tot : 0) + e;
+  const size_t tot_d = a.plane_count;
+  int32_t* dst = a.dst + (part ? (size_t)kND * tot_d : 0) + (a.off ? (size_t)a.off[b] : (size_t)b * a.mn) +
+                 (size_t)(ij / a.N) * a.ld + (ij % a.N);
 
   int64_t cy = 0;   // carry of the raw-column normalisation
   int64_t cy2 = 0;  // carry of the destination addition
@@ -220,20 +230,39 @@ __global__ void __launch_bounds__(256) combine_kernel(CombineArgs a) {
     int32_t old[CH];
 #pragma unroll
     for (int u = 0; u < CH; ++u) { s1[u] = 0; s2[u] = 0; old[u] = 0; }
-    for (int s = 0; s < a.nsplit; ++s) {
-#pragma unroll
-      for (int u = 0; u < CH; ++u) {
-        if (c0 + u < a.nc) {
-          s1[u] += q1[(size_t)s * sstride + (size_t)(c0 + u) * colstride];
-          s2[u] += q2[(size_t)s * sstride + (size_t)(c0 + u) * colstride];
-        }
-      }
-    }
     if (a.mode != 0) {
 #pragma unroll
       for (int u = 0; u < CH; ++u) {
         const int k = q + c0 + u;
-        if (k >= 0 && k <= kND - 1) old[u] = dst[(size_t)k * tot];
+        if (k >= 0 && k <= kND - 1) old[u] = dst[(size_t)k * tot_d];
+      }
+    }
+    if (NS > 0) {
+      constexpr int NSA = NS > 0 ? NS : 1;
+      int32_t l1[NSA][CH], l2[NSA][CH];
+#pragma unroll
+      for (int s = 0; s < NS; ++s) {
+#pragma unroll
+        for (int u = 0; u < CH; ++u) {
+          const bool in = s < a.nsplit && c0 + u < a.nc;
+          l1[s][u] = in ? q1[(size_t)s * sstride + (size_t)(c0 + u) * colstride] : 0;
+          l2[s][u] = in ? q2[(size_t)s * sstride + (size_t)(c0 + u) * colstride] : 0;
+        }
+      }
+#pragma unroll
+      for (int s = 0; s < NS; ++s) {
+#pragma unroll
+        for (int u = 0; u < CH; ++u) { s1[u] += l1[s][u]; s2[u] += l2[s][u]; }
+      }
+    } else {
+      for (int s = 0; s < a.nsplit; ++s) {
+#pragma unroll
+        for (int u = 0; u < CH; ++u) {
+          if (c0 + u < a.nc) {
+            s1[u] += q1[(size_t)s * sstride + (size_t)(c0 + u) * colstride];
+            s2[u] += q2[(size_t)s * sstride + (size_t)(c0 + u) * colstride];
+          }
+        }
       }
     }
 #pragma unroll
@@ -256,25 +285,26 @@ __global__ void __launch_bounds__(256) combine_kernel(CombineArgs a) {
         if (k >= 0) {
           if (k < cutq) digit = 0;
           else if (k == cutq && cutr) digit &= ~((1 << cutr) - 1);
-          if (k < kND - 1) {
-            if (digit != 0) msb_pos = k * DB + (32 - __clz(digit));
-            if (digit != DMASK) msb_neg = k * DB + (32 - __clz((~digit) & DMASK));
-          } else {
-            if (digit > 0) msb_pos = k * DB + (32 - __clz(digit));
-            if (digit < -1) msb_neg = k * DB + (32 - __clz(~digit));
-            if (a.msb_out) atomicMax(a.msb_out, digit < 0 ? msb_neg : msb_pos);
-          }
-          int32_t* dp = dst + (size_t)k * tot;
-          if (a.mode == 0) {
-            *dp = digit;
-          } else {
+          int32_t* dp = dst + (size_t)k * tot_d;
+          int32_t outd = digit;
+          if (a.mode != 0) {
             int64_t t = (int64_t)old[u] + (a.mode == 1 ? (int64_t)digit : -(int64_t)digit) + cy2;
             if (k < kND - 1) {
               cy2 = t >> DB;
-              *dp = (int32_t)(t & DMASK);
+              outd = (int32_t)(t & DMASK);
             } else {
-              *dp = (int32_t)t;
+              outd = (int32_t)t;
             }
+          }
+          *dp = outd;
+          // msb of the value that ends up in the destination
+          if (k < kND - 1) {
+            if (outd != 0) msb_pos = k * DB + (32 - __clz(outd));
+            if (outd != DMASK) msb_neg = k * DB + (32 - __clz((~outd) & DMASK));
+          } else {
+            if (outd > 0) msb_pos = k * DB + (32 - __clz(outd));
+            if (outd < -1) msb_neg = k * DB + (32 - __clz(~outd));
+            if (a.msb_out) atomicMax(a.msb_out, outd < 0 ? msb_neg : msb_pos);
           }
         }
       }
@@ -282,7 +312,7 @@ __global__ void __launch_bounds__(256) combine_kernel(CombineArgs a) {
   }
   // digits below the first written one (q > 0) are untouched in Add/Sub mode and must be zero in Assign mode
   if (a.mode == 0)
-    for (int kk = 0; kk < q && kk < kND; ++kk) dst[(size_t)kk * tot] = 0;
+    for (int kk = 0; kk < q && kk < kND; ++kk) dst[(size_t)kk * tot_d] = 0;
 }
 
 // ---- host side ----------------------------------------------------------------------------------------------------
@@ -373,7 +403,7 @@ uint64_t gemm_complex_macs(int M, int N, int K, int batch, int nwP, int nwQ, int
 
 int gemm_complex(int M, int N, int K, int batch, const GemmSide& P, const GemmSide& Q, int32_t* dst_fx, GemmMode mode,
                  int out_cut_bit, int path, void* workspace, size_t workspace_bytes, int* err_flag, int* msb_out,
-                 cudaStream_t stream) {
+                 cudaStream_t stream, const GemmDstView* dv) {
   if (M < 1 || N < 1 || K < 1 || batch < 1 || P.nw < 1 || Q.nw < 1 || P.nw > kND || Q.nw > kND) return ZKD_ERR_INVALID_ARG;
   // the instance needs NQ <= NP roles only through its truncation rule; pad whichever side is short
   const GemmInstance* in = pick_instance(P.nw, Q.nw);
@@ -397,10 +427,12 @@ int gemm_complex(int M, int N, int K, int batch, const GemmSide& P, const GemmSi
   {
     PrepArgs2 both{};
     PrepArgs& pa = both.side[0];
-    pa.src = P.fx; pa.dst = Pc; pa.src_count = (size_t)batch * M * K; pa.R = M; pa.C = K; pa.batch = batch;
+    pa.src = P.fx; pa.dst = Pc; pa.src_count = P.plane_count ? P.plane_count : (size_t)batch * M * K; pa.R = M; pa.C = K; pa.batch = batch;
+    pa.ld = P.ld ? P.ld : (P.conj_transpose ? M : K); pa.off = P.off;
     pa.transpose = P.conj_transpose ? 1 : 0; pa.side = 0; pa.lsb_bit = lsbP; pa.nw = npad; pa.nw_src = P.nw; pa.err_flag = err_flag;
     PrepArgs& qa = both.side[1];
-    qa.src = Q.fx; qa.dst = Qc; qa.src_count = (size_t)batch * K * N; qa.R = K; qa.C = N; qa.batch = batch;
+    qa.src = Q.fx; qa.dst = Qc; qa.src_count = Q.plane_count ? Q.plane_count : (size_t)batch * K * N; qa.R = K; qa.C = N; qa.batch = batch;
+    qa.ld = Q.ld ? Q.ld : N; qa.off = Q.off;
     qa.transpose = 0; qa.side = 1; qa.lsb_bit = lsbQ; qa.nw = nqad; qa.nw_src = Q.nw; qa.err_flag = err_flag;
     const size_t tot = (size_t)batch * K * (size_t)(M > N ? M : N);
     prep_kernel<<<dim3((unsigned)((tot + 255) / 256), 2), 256, 0, stream>>>(both);
@@ -408,7 +440,7 @@ int gemm_complex(int M, int N, int K, int batch, const GemmSide& P, const GemmSi
   }
   if (use_i8)
     return gemm_i8_finish(M, N, K, batch, Pc, Qc, npad, nqad, lsbP, lsbQ, dst_fx, (int)mode, out_cut_bit, raw,
-                          workspace_bytes - (size_t)((char*)raw - (char*)workspace), err_flag, msb_out, stream);
+                          workspace_bytes - (size_t)((char*)raw - (char*)workspace), err_flag, msb_out, stream, dv);
   const int nsplit = pick_splits(M, N, K, batch);
   int ksplit = (K + nsplit - 1) / nsplit;
   ksplit = (ksplit + GT - 1) / GT * GT;
@@ -428,10 +460,16 @@ int gemm_complex(int M, int N, int K, int batch, const GemmSide& P, const GemmSi
 
   CombineArgs ca{};
   ca.raw = raw; ca.dst = dst_fx; ca.mn = (size_t)M * N; ca.batch = batch; ca.nc = in->nc; ca.nsplit = nsp;
+  ca.N = N; ca.ld = dv && dv->ld ? dv->ld : N; ca.off = dv ? dv->off : nullptr;
+  ca.plane_count = dv && dv->plane_count ? dv->plane_count : (size_t)batch * M * N;
   ca.base_bit = lsbP + lsbQ + DB * in->low - kFRAC;
   ca.cut_bit = out_cut_bit; ca.mode = (int)mode; ca.msb_out = msb_out;
   const size_t tot = (size_t)batch * M * N;
-  combine_kernel<<<dim3((unsigned)((tot + 255) / 256), 2), 256, 0, stream>>>(ca);
+  const dim3 cgrid((unsigned)((tot + 255) / 256), 2);
+  if (nsp == 1) combine_kernel<1><<<cgrid, 256, 0, stream>>>(ca);
+  else if (nsp == 2) combine_kernel<2><<<cgrid, 256, 0, stream>>>(ca);
+  else if (nsp <= 4) combine_kernel<4><<<cgrid, 256, 0, stream>>>(ca);
+  else combine_kernel<0><<<cgrid, 256, 0, stream>>>(ca);
   count_launch();
   return launch_check();
 }

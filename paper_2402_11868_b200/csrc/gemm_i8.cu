@@ -328,6 +328,9 @@ struct CombineI8Args {
   const int32_t* raw;  // [nsplit][3*batch][ncol][M*N]
   int32_t* dst;        // complex FX, batch*M*N
   size_t mn;
+  int N, ld;           // destination view (see combine_kernel)
+  const int* off;
+  size_t plane_count;
   int batch, ncol, nsplit;
   int base_bit;  // FX bit position of column 0's LSB (may be negative)
   int cut_bit;   // clear result bits below this FX bit (<= 0: none)
@@ -348,7 +351,9 @@ __global__ void __launch_bounds__(256) combine_i8_kernel(CombineI8Args a) {
   const int32_t* __restrict__ r1 = a.raw + (size_t)(b * 3 + 0) * gstride + ij;
   const int32_t* __restrict__ r2 = a.raw + (size_t)(b * 3 + (part == 0 ? 2 : 1)) * gstride + ij;
   const int sgn2 = part == 0 ? -1 : 1;
-  int32_t* dst = a.dst + (part ? (size_t)ND * tot : 0) + e;
+  const size_t tot_d = a.plane_count;
+  int32_t* dst = a.dst + (part ? (size_t)ND * tot_d : 0) + (a.off ? (size_t)a.off[b] : (size_t)b * a.mn) +
+                 (size_t)(ij / a.N) * a.ld + (ij % a.N);
 
   auto col = [&](int c) -> int64_t {
     int64_t s1 = 0, s2 = 0;
@@ -391,29 +396,29 @@ __global__ void __launch_bounds__(256) combine_i8_kernel(CombineI8Args a) {
     if (k < 0) continue;
     if (k < cutq) digit = 0;
     else if (k == cutq && cutr) digit &= ~((1 << cutr) - 1);
-    if (k < ND - 1) {
-      if (digit != 0) msb_pos = k * DB + (32 - __clz(digit));
-      if (digit != DMASK) msb_neg = k * DB + (32 - __clz((~digit) & DMASK));
-    } else {
-      if (digit > 0) msb_pos = k * DB + (32 - __clz(digit));
-      if (digit < -1) msb_neg = k * DB + (32 - __clz(~digit));
-      if (a.msb_out) atomicMax(a.msb_out, digit < 0 ? msb_neg : msb_pos);
-    }
-    int32_t* dp = dst + (size_t)k * tot;
-    if (a.mode == 0) {
-      *dp = digit;
-    } else {
+    int32_t* dp = dst + (size_t)k * tot_d;
+    int32_t outd = digit;
+    if (a.mode != 0) {
       const int64_t t = (int64_t)*dp + (a.mode == 1 ? (int64_t)digit : -(int64_t)digit) + cy2;
       if (k < ND - 1) {
         cy2 = t >> DB;
-        *dp = (int32_t)(t & DMASK);
+        outd = (int32_t)(t & DMASK);
       } else {
-        *dp = (int32_t)t;
+        outd = (int32_t)t;
       }
+    }
+    *dp = outd;
+    if (k < ND - 1) {
+      if (outd != 0) msb_pos = k * DB + (32 - __clz(outd));
+      if (outd != DMASK) msb_neg = k * DB + (32 - __clz((~outd) & DMASK));
+    } else {
+      if (outd > 0) msb_pos = k * DB + (32 - __clz(outd));
+      if (outd < -1) msb_neg = k * DB + (32 - __clz(~outd));
+      if (a.msb_out) atomicMax(a.msb_out, outd < 0 ? msb_neg : msb_pos);
     }
   }
   if (a.mode == 0)
-    for (int kk = 0; kk < kstart && kk < ND; ++kk) dst[(size_t)kk * tot] = 0;
+    for (int kk = 0; kk < kstart && kk < ND; ++kk) dst[(size_t)kk * tot_d] = 0;
 }
 
 }  // namespace
@@ -521,7 +526,7 @@ size_t gemm_i8_workspace_bytes(int M, int N, int K, int batch) {
 
 int gemm_i8_finish(int M, int N, int K, int batch, const int32_t* Pc, const int32_t* Qc, int np, int nq, int lsbP, int lsbQ,
                    int32_t* dst_fx, int mode, int cut_bit, void* ws, size_t ws_bytes, int* err_flag, int* msb_out,
-                   cudaStream_t stream) {
+                   cudaStream_t stream, const GemmDstView* dv) {
   if (ws_bytes < gemm_i8_workspace_bytes(M, N, K, batch)) return ZKD_ERR_WORKSPACE;
   const int Kp = (K + I8_BK - 1) / I8_BK * I8_BK;
   const int G = 3 * batch;
@@ -600,6 +605,8 @@ int gemm_i8_finish(int M, int N, int K, int batch, const int32_t* Pc, const int3
 
   CombineI8Args ca{};
   ca.raw = raw; ca.dst = dst_fx; ca.mn = (size_t)M * N; ca.batch = batch; ca.ncol = ncol; ca.nsplit = ka.nsplit;
+  ca.N = N; ca.ld = dv && dv->ld ? dv->ld : N; ca.off = dv ? dv->off : nullptr;
+  ca.plane_count = dv && dv->plane_count ? dv->plane_count : (size_t)batch * M * N;
   ca.base_bit = lsbP + lsbQ - FRAC + 8 * dcut;
   ca.cut_bit = cut_bit; ca.mode = mode; ca.msb_out = msb_out;
   const size_t tot = (size_t)batch * M * N;

@@ -59,7 +59,7 @@ struct Arena {
   }
 };
 
-enum { S_ERR = 0, S_MSB_R = 1, S_MSB_G = 2, S_MSB_E = 3, S_MSB_T = 4, S_NUM = 8 };
+enum { S_ERR = 0, S_MSB_R = 1, S_MSB_G = 2, S_MSB_E = 3, S_MSB_T = 4, S_GAP_INV = 5, S_NUM = 8 };
 
 struct Ctx {
   cudaStream_t s;
@@ -112,6 +112,105 @@ Groups build_groups(const std::vector<int>& h_cl, int n, int nb) {
   return groups;
 }
 
+// ---- S4f / S4c of a level that has clusters with more than one member, as windowed GEMMs over cluster views -----------------
+// For every cluster size m > 1 the clusters of that size form one batched product over views into X, W, S (column slices
+// X_c = X[:, c0:c0+m] and diagonal blocks); singleton columns go through the fused singleton kernel.  All products carry
+// only the bits above `cut` (an absolute FX bit position chosen from the previous pass's error level).
+struct ClusterGroup { int m, nsub; const int* offX; const int* offB; };
+struct ClusterPlan {
+  std::vector<ClusterGroup> groups;
+  bool has_singletons = false;
+  int max_m = 1, max_nsub = 0;
+};
+
+int build_plan(Ctx& c, int n, int nb, const std::vector<int>& h_cl, int* plan_dev /* 2 n nb ints */, ClusterPlan* plan) {
+  const Groups groups = build_groups(h_cl, n, nb);
+  plan->groups.clear();
+  plan->max_m = 1;
+  plan->max_nsub = 0;
+  std::vector<int> h;
+  size_t clustered = 0;
+  for (const auto& kv : groups) {
+    ClusterGroup g;
+    g.m = kv.first;
+    g.nsub = (int)kv.second.size();
+    g.offX = plan_dev + h.size();
+    for (const SubProblem& sp : kv.second) h.push_back(sp.b * n * n + sp.col0);
+    g.offB = plan_dev + h.size();
+    for (const SubProblem& sp : kv.second) h.push_back(sp.b * n * n + sp.col0 * n + sp.col0);
+    plan->groups.push_back(g);
+    plan->max_m = std::max(plan->max_m, g.m);
+    plan->max_nsub = std::max(plan->max_nsub, g.nsub);
+    clustered += (size_t)g.m * g.nsub;
+  }
+  plan->has_singletons = clustered < (size_t)n * nb;
+  if (!h.empty()) {
+    ZKD_CUDA_TRY(cudaMemcpyAsync(plan_dev, h.data(), sizeof(int) * h.size(), cudaMemcpyHostToDevice, c.s));
+    ZKD_CUDA_TRY(cudaStreamSynchronize(c.s));  // h is a local
+  }
+  return ZKD_OK;
+}
+
+inline int digits_for(int top, int cut) { return std::max(2, std::min(kND, ceil_div(top - cut, kDB) + 1)); }
+
+// X, W <- (X, W)(I + (I - G)/2) on clusters;  S = X_c^H W_c;  theta = diag S;  R = W - X_c S_c.  msb(G - I) and msb(R) are
+// accumulated into scal[S_MSB_G] / scal[S_MSB_R] (singleton columns included).
+int cluster_pass(Ctx& c, int n, int nb, const ClusterPlan& plan, const int* cl, const int* cle, int32_t* X, int32_t* W, int32_t* R,
+                 int32_t* Sm, int32_t* Gm, int32_t* theta, int* scal, int cut, size_t fxc) {
+  const Options& opt = options();
+  cudaStream_t s = c.s;
+  const size_t cnt = (size_t)n * n * nb;
+  const int topX = 815, topW = std::min(812 + ilog2_ceil(n) + 1, 840);
+  auto view = [&](const int32_t* fx, int rows, int cols, bool ct, int top, int nw, const int* off) {
+    GemmSide g;
+    g.fx = fx; g.rows = rows; g.cols = cols; g.conj_transpose = ct; g.top_bit = top; g.nw = std::max(1, std::min(nw, kND));
+    g.ld = n; g.off = off; g.plane_count = cnt;
+    return g;
+  };
+  auto gemm = [&](int M, int N, int K, int batch, const GemmSide& P, const GemmSide& Q, int32_t* dst, GemmMode mode,
+                  const int* dst_off, int* msb_out, int out_cut = -1) {
+    GemmDstView dv;
+    dv.ld = n; dv.off = dst_off; dv.plane_count = cnt;
+    return gemm_complex(M, N, K, batch, P, Q, dst, mode, out_cut, opt.gemm_path, c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, msb_out, s,
+                        &dv);
+  };
+  const int nwX = digits_for(topX, cut), nwW = digits_for(topW, cut);
+  // S4f: G_c = X_c^H X_c, bits below cutG cleared so that M = (I - G)/2 is a short number
+  const int cutG = std::max(1, cut);
+  for (const ClusterGroup& g : plan.groups)
+    ZKD_TRY(gemm(g.m, g.m, n, g.nsub, view(X, n, g.m, true, topX, nwX, g.offX), view(X, n, g.m, false, topX, nwX, g.offX), Gm,
+                 GemmMode::Assign, g.offB, nullptr, cutG));
+  ZKD_TRY(ns_build(n, nb, cl, Gm, scal + S_MSB_G, s, cle));
+  int hs[S_NUM];
+  ZKD_TRY(read_scalars(c, scal, S_NUM, hs));
+  if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
+  const int msb_m = hs[S_MSB_G];  // |M| = |(I - G)/2| < 2^(msb_m - 813)
+  if (msb_m > 0) {
+    // X_c += X_c M_c, W_c += W_c M_c in place (the operands are copied into compact planes before the product runs).
+    // These two must be exact to the FX floor, whatever the pass's precision: W = A X is kept incrementally, so an error
+    // made here would stay in W for good.  Exact = all digits of X / W times all nonzero digits of M (those above cutG - 1).
+    const int topM = msb_m + 1, nwM = std::max(1, std::min(kND, ceil_div(topM - (cutG - 1), kDB)));
+    const int nwXm = kND, nwWm = kND;
+    for (const ClusterGroup& g : plan.groups) {
+      ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(X, n, g.m, false, topX, nwXm, g.offX), view(Gm, g.m, g.m, false, topM, nwM, g.offB), X,
+                   GemmMode::Add, g.offX, nullptr));
+      ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(W, n, g.m, false, topW, nwWm, g.offX), view(Gm, g.m, g.m, false, topM, nwM, g.offB), W,
+                   GemmMode::Add, g.offX, nullptr));
+    }
+  }
+  // S4c
+  ZKD_CUDA_TRY(cudaMemcpyAsync(R, W, fxc, cudaMemcpyDeviceToDevice, s));
+  if (plan.has_singletons) ZKD_TRY(singleton_step(n, nb, X, W, R, Sm, theta, scal + S_MSB_G, scal + S_MSB_R, s, cl, cle));
+  for (const ClusterGroup& g : plan.groups)
+    ZKD_TRY(gemm(g.m, g.m, n, g.nsub, view(X, n, g.m, true, topX, nwX, g.offX), view(W, n, g.m, false, topW, nwW, g.offX), Sm,
+                 GemmMode::Assign, g.offB, nullptr));
+  ZKD_TRY(theta_from_diag(n, nb, Sm, theta, s));
+  for (const ClusterGroup& g : plan.groups)
+    ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(X, n, g.m, false, topX, nwX, g.offX), view(Sm, g.m, g.m, false, topW, nwW, g.offB), R,
+                 GemmMode::Sub, g.offX, scal + S_MSB_R));
+  return ZKD_OK;
+}
+
 // S4h, early cluster split.  Inside a cluster the correction is deflated, so its convergence is only linear, at
 // (spread of the cluster / gap to the outside)^2 per step, when the cluster has internal structure (c4: the 29-dimensional
 // cluster holds 2^-21 .. 2^-60 and 24 zeros).  As soon as that structure stands above the noise of S_c = X_c^H W_c
@@ -119,8 +218,9 @@ Groups build_groups(const std::vector<int>& h_cl, int n, int nb) {
 // cluster basis is rotated by those eigenvectors (X_c, W_c <- X_c U, W_c U) and the cluster table is refined by the block's
 // own clusters.  U is unitary to fp64 only; the S4f Newton-Schulz step of the following passes repairs that quadratically.
 // Blocks whose structure is below the noise (true multiplicities) are left alone.  Sets *changed when any cluster split.
-int try_split(Ctx& c, int n, int nb, const int32_t* Sm, int msb_r, int tol_msb, const int* noise, const int32_t* Xc,
-              const int32_t* Wc, int32_t* Xo, int32_t* Wo, int32_t* Um, int* cl, int* cle, std::vector<int>& h_cl, bool* changed) {
+int try_split(Ctx& c, int n, int nb, const ClusterPlan& plan, const int32_t* Sm, int msb_r, int tol_msb, const int* noise, int32_t* X,
+              int32_t* W, int32_t* Um, int32_t* G2 /* scratch, FxC n n nb */, int* scal, int* cl, int* cle, std::vector<int>& h_cl,
+              bool* changed) {
   const Options& opt = options();
   cudaStream_t s = c.s;
   *changed = false;
@@ -128,14 +228,13 @@ int try_split(Ctx& c, int n, int nb, const int32_t* Sm, int msb_r, int tol_msb, 
   if (groups.empty()) return ZKD_OK;
   // eigenvalues of a block are told apart only when they differ by more than (a) the Ritz-value noise ~ |R|^2 / gap and
   // (b) 2^16 |R|: the correction E_ij = C_ij / (theta_j - theta_i) between the new clusters must stay small
-  // and (c) 2^-190: ecalc's reciprocal range.
-  const int noise_msb = std::max(std::max(tol_msb + 6, 812 - 190), std::max(2 * msb_r - 812 + opt.split_margin_bits, msb_r + 16));
-  // Worth it?  Unsplit, the cluster gains 2 log2(gap / spread) bits per step with gap >= 2^-tau |A|_F ~ 2^(790-812); split
-  // (or with no structure) the step gains about e + 40 bits (windowed quadratic convergence), and no more than what is
-  // left to the tolerance is needed.  Split only blocks whose spread makes the linear rate the slower one (c4), not those
-  // whose structure is far below the gap (c5: 2^-200 spacing, left to S5).
-  const int want = std::min(812 - msb_r + 40, msb_r - tol_msb + 10);
-  const int min_split_msb = 812 - opt.tau_bits - 2 - want / 2;
+  // and (c) 2^-390: ecalc's reciprocal range.
+  const int noise_msb = std::max(std::max(tol_msb + 6, 812 - 390), std::max(2 * msb_r - 812 + opt.split_margin_bits, msb_r + 16));
+  // Worth it?  Unsplit, the cluster gains about log2(gap / spread) bits per pass (measured: c4 ~20 bits, c5 ~195 bits),
+  // with gap >= 2^-tau |A|_F ~ 2^(790-812).  A split resets the error inside the cluster to that of the fp64 eigenvectors
+  // of the block (2^-50), i.e. costs about 5 passes of quadratic convergence.  Split only the blocks that would need more
+  // passes than that at their linear rate (c4), not those whose structure is far below the gap (c5: left to S5).
+  const int min_split_msb = 812 - opt.tau_bits - 2 - (msb_r - tol_msb) / 5;
   const Arena::Mark mark = c.ar.mark();
   bool any = false, first = true;
   for (const auto& kv : groups) {
@@ -160,6 +259,12 @@ int try_split(Ctx& c, int n, int nb, const int32_t* Sm, int msb_r, int tol_msb, 
     ZKD_CUDA_TRY(cudaStreamSynchronize(s));  // also keeps kv.second alive for the copy above
     bool all_deg = true;
     for (int v : hdeg) all_deg = all_deg && v;
+    if (opt.verbose) {
+      std::vector<int> hk((size_t)nsub);
+      cudaMemcpy(hk.data(), kshift, sizeof(int) * nsub, cudaMemcpyDeviceToHost);
+      fprintf(stderr, "[zkd]   split? m %d nsub %d noise_msb %d min_split_msb %d: spread msb %d deg %d (first block)\n", m, nsub,
+              noise_msb, min_split_msb, 810 - hk[0], hdeg[0]);
+    }
     if (all_deg) continue;
     if (first) { ZKD_TRY(identity_blocks(n, nb, Um, s)); first = false; }
     ZKD_TRY(fxc_to_c64(hc, H, H64, s));
@@ -169,7 +274,7 @@ int try_split(Ctx& c, int n, int nb, const int32_t* Sm, int msb_r, int tol_msb, 
     any = true;
   }
   if (any) {
-    // rotate with the OLD cluster table (the blocks of Um), then adopt the refined one
+    // cl / cle now hold the refined table; cl_old / cle_old the one the blocks of Um belong to
     std::vector<int> h_new((size_t)n * nb), h_cle_old((size_t)n * nb);
     int* cl_old = c.ar.get<int>((size_t)n * nb);
     int* cle_old = c.ar.get<int>((size_t)n * nb);
@@ -186,10 +291,58 @@ int try_split(Ctx& c, int n, int nb, const int32_t* Sm, int msb_r, int tol_msb, 
       }
     }
     ZKD_CUDA_TRY(cudaMemcpyAsync(cle_old, h_cle_old.data(), sizeof(int) * n * nb, cudaMemcpyHostToDevice, s));
-    ZKD_TRY(block_apply(n, nb, nullptr, Xc, Um, cl_old, cle_old, false, Xo, nullptr, s));
-    ZKD_TRY(block_apply(n, nb, nullptr, Wc, Um, cl_old, cle_old, false, Wo, nullptr, s));
+    const size_t cnt = (size_t)n * n * nb;
+    auto view = [&](const int32_t* fx, int rows, int cols, bool ct, int top, const int* off) {
+      GemmSide g;
+      g.fx = fx; g.rows = rows; g.cols = cols; g.conj_transpose = ct; g.top_bit = top; g.nw = kND;
+      g.ld = n; g.off = off; g.plane_count = cnt;
+      return g;
+    };
+    auto gemm = [&](int M, int N, int K, int batch, const GemmSide& P, const GemmSide& Q, int32_t* dst, GemmMode mode, const int* dst_off) {
+      GemmDstView dv;
+      dv.ld = n; dv.off = dst_off; dv.plane_count = cnt;
+      return gemm_complex(M, N, K, batch, P, Q, dst, mode, -1, opt.gemm_path, c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s, &dv);
+    };
+    // U is unitary to fp64 only.  Newton-Schulz on the blocks, U <- U (I + (I - U^H U)/2), squares that error each time
+    // (2^-50 -> 2^-100 -> ... -> FX floor): X_c U then stays orthonormal and the Rayleigh quotients stay meaningful
+    // against gaps far below 2^-50; what is left of the fp64 eigenvectors' error is a pure rotation, which S4d removes.
+    // Iteration `it` starts from an error of about 2^-(48 2^it): U^H U is needed to twice that many bits only, and the
+    // correction M = (I - U^H U)/2 is then a short number (bits below the cut cleared).
+    for (int it = 0; it < 6; ++it) {
+      const int cutU = std::max(1, 812 - (100 << it) - 30);
+      const int nwU = digits_for(815, cutU);
+      for (const ClusterGroup& g : plan.groups) {
+        GemmSide P = view(Um, g.m, g.m, true, 815, g.offB), Q = view(Um, g.m, g.m, false, 815, g.offB);
+        P.nw = Q.nw = nwU;
+        GemmDstView dv;
+        dv.ld = n; dv.off = g.offB; dv.plane_count = cnt;
+        ZKD_TRY(gemm_complex(g.m, g.m, g.m, g.nsub, P, Q, G2, GemmMode::Assign, cutU, opt.gemm_path, c.gemm_ws, c.gemm_ws_bytes,
+                             scal + S_ERR, nullptr, s, &dv));
+      }
+      ZKD_CUDA_TRY(cudaMemsetAsync(scal + S_MSB_T, 0, sizeof(int), s));
+      ZKD_TRY(ns_build(n, nb, cl_old, G2, scal + S_MSB_T, s, cle_old));
+      int hs[S_NUM];
+      ZKD_TRY(read_scalars(c, scal, S_NUM, hs));
+      if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
+      const int msb_m = hs[S_MSB_T];
+      if (msb_m <= 20 && cutU <= 1) break;  // |U^H U - I| < 2^-792
+      if (msb_m == 0) continue;
+      for (const ClusterGroup& g : plan.groups) {
+        GemmSide Q = view(G2, g.m, g.m, false, msb_m + 1, g.offB);
+        Q.nw = std::max(1, std::min(kND, ceil_div(msb_m + 1 - (cutU - 1), kDB)));
+        ZKD_TRY(gemm(g.m, g.m, g.m, g.nsub, view(Um, g.m, g.m, false, 815, g.offB), Q, Um, GemmMode::Add, g.offB));
+      }
+    }
+    // X_c <- X_c U_c, W_c <- W_c U_c in place (operands are staged before the product runs)
+    const int topW = std::min(812 + ilog2_ceil(n) + 1, 840);
+    for (const ClusterGroup& g : plan.groups) {
+      ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(X, n, g.m, false, 815, g.offX), view(Um, g.m, g.m, false, 815, g.offB), X,
+                   GemmMode::Assign, g.offX));
+      ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(W, n, g.m, false, topW, g.offX), view(Um, g.m, g.m, false, 815, g.offB), W,
+                   GemmMode::Assign, g.offX));
+    }
     ZKD_CUDA_TRY(cudaStreamSynchronize(s));
-    *changed = h_new != h_cl;
+    *changed = true;
     h_cl.swap(h_new);
   }
   c.ar.release(mark);
@@ -212,6 +365,7 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
   int32_t* theta = lam;
   int* cl0 = c.ar.get<int>((size_t)n * nb);   // the clusters as detected (S4h refines cl / cle)
   int* cle0 = c.ar.get<int>((size_t)n * nb);
+  int* plan_dev = c.ar.get<int>((size_t)2 * n * nb);
   bool split_done = false;
   const Arena::Mark mark1 = c.ar.mark();
   // short-lived
@@ -224,7 +378,7 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
   int32_t* T = (int32_t*)c.ar.alloc(fxc);
   int32_t* Gm = (int32_t*)c.ar.alloc(fxc);
   int* scal = c.ar.get<int>(S_NUM);
-  if (!cl0 || !cle0) return ZKD_ERR_WORKSPACE;
+  if (!cl0 || !cle0 || !plan_dev) return ZKD_ERR_WORKSPACE;
   if (!cl || !cle || !stats || !Sm || !A64 || !mu || !V || !W || !R || !Cm || !T || !Gm || !scal) return ZKD_ERR_WORKSPACE;
   if (gemm_workspace_bytes(n, n, n, nb) > c.gemm_ws_bytes) return ZKD_ERR_WORKSPACE;
 
@@ -263,7 +417,10 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
   for (int b = 0; b < nb && singletons; ++b)
     for (int j = 1; j < n; ++j)
       if (h_cl[(size_t)b * n + j] != j) { singletons = false; break; }
+  ClusterPlan plan;
+  if (!singletons) ZKD_TRY(build_plan(c, n, nb, h_cl, plan_dev, &plan));
   int status = 2, steps = 0, prev_msb_r = 1 << 30;
+  int e_prev = 15, last_cut = 0;  // error level of the previous pass (2^-e_prev), precision of the current one
   int hs[S_NUM];
   const int tol_msb = 812 - opt.tol_bits;
   for (int step = 0; step < opt.max_steps; ++step) {
@@ -271,26 +428,23 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
       // S4f + S4c fused: normalise columns, Rayleigh quotients, residual (X, W in place)
       ZKD_TRY(singleton_step(n, nb, Xc, Wc, R, Sm, theta, scal + S_MSB_G, scal + S_MSB_R, s));
     } else {
-      // S4f: orthonormalise inside clusters (Newton-Schulz step on the cluster Gram blocks)
-      ZKD_TRY(gram_blocks(n, nb, Xc, Xc, cl, Gm, s));
-      ZKD_TRY(ns_build(n, nb, cl, Gm, scal + S_MSB_G, s));
-      ZKD_TRY(block_apply(n, nb, Xc, Xc, Gm, cl, cle, false, Tc, nullptr, s));
-      ZKD_TRY(block_apply(n, nb, Wc, Wc, Gm, cl, cle, false, Cc, nullptr, s));
-      std::swap(Xc, Tc);
-      std::swap(Wc, Cc);
-      // S4c: Rayleigh quotients and block residual
-      ZKD_TRY(gram_blocks(n, nb, Xc, Wc, cl, Sm, s));
-      ZKD_TRY(theta_from_diag(n, nb, Sm, theta, s));
-      ZKD_TRY(block_apply(n, nb, Wc, Xc, Sm, cl, cle, true, R, scal + S_MSB_R, s));
+      // S4f + S4c on cluster views.  Results are needed to about 2^-(2 e_now + 40) and e_now <= 2 e_prev + 45.
+      last_cut = 812 - (4 * e_prev + 130);
+      ZKD_TRY(cluster_pass(c, n, nb, plan, cl, cle, Xc, Wc, R, Sm, Gm, theta, scal, last_cut, fxc));
     }
+    if (split_done) ZKD_TRY(min_gap(n, nb, theta, cl, scal + S_GAP_INV, s));
     ZKD_TRY(read_scalars(c, scal, S_NUM, hs));
     const int msb_r = hs[S_MSB_R], msb_g = hs[S_MSB_G];
+    // clusters that S4h split apart can be much closer than 2^-tau |A|_F: C_ij / gap needs that many more bits of C, E, T
+    const int gap_extra = (split_done && hs[S_GAP_INV]) ? std::max(0, (812 - opt.tau_bits - 2) - (1024 - hs[S_GAP_INV])) : 0;
     if (opt.verbose) fprintf(stderr, "[zkd] depth %d n %d nb %d step %d: msbR %d (2^%d) msbG %d err %d\n", depth, n, nb, step, msb_r, msb_r - 812, msb_g, hs[S_ERR]);
     if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
     steps = step;
     if (st) { st->msb_r = msb_r; st->msb_g = msb_g; }
-    if (msb_r <= tol_msb && msb_g <= 812 - 400) { status = 0; break; }
-    if (step > 0 && msb_r > tol_msb && msb_r >= prev_msb_r - 2 && msb_g <= 812 - 400) { status = 1; break; }
+    const bool exact_pass = singletons || last_cut <= 0;  // a windowed pass cannot certify convergence
+    if (exact_pass && msb_r <= tol_msb && msb_g <= 812 - 400) { status = 0; break; }
+    if (exact_pass && step > 0 && msb_r > tol_msb && msb_r >= prev_msb_r - 2 && msb_g <= 812 - 400) { status = 1; break; }
+    e_prev = std::max(15, 812 - msb_r);
     if (step + 1 == opt.max_steps) break;
     prev_msb_r = msb_r;
     ZKD_CUDA_TRY(cudaMemsetAsync(scal, 0, sizeof(int) * S_NUM, s));
@@ -299,13 +453,13 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
     // S4h: split clusters whose internal structure stands above the noise of S_c
     if (!singletons && opt.early_split && msb_g <= 812 - 45) {
       bool changed = false;
-      ZKD_TRY(try_split(c, n, nb, Sm, msb_r, tol_msb, noise, Xc, Wc, Tc, Cc, Gm, cl, cle, h_cl, &changed));
+      ZKD_TRY(try_split(c, n, nb, plan, Sm, msb_r, tol_msb, noise, Xc, Wc, Gm, R, scal, cl, cle, h_cl, &changed));
       if (changed) {
         split_done = true;
-        std::swap(Xc, Tc);
-        std::swap(Wc, Cc);
+        ZKD_CUDA_TRY(cudaMemsetAsync(scal, 0, sizeof(int) * S_NUM, s));
         singletons = true;
         for (size_t t = 0; t < h_cl.size() && singletons; ++t) singletons = h_cl[t] == (int)(t % n);
+        if (!singletons) ZKD_TRY(build_plan(c, n, nb, h_cl, plan_dev, &plan));
         prev_msb_r = 1 << 30;
         continue;  // S4f / S4c again with the rotated basis and the finer clusters
       }
@@ -313,7 +467,7 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
 
     // S4d: C = X^H R on windows sized for this step's gain
     const int e = 812 - msb_r;                        // residual ~ 2^-e
-    const int pb = std::max(40, std::min(e + 40, msb_r + 30));  // relative bits worth computing for the correction
+    const int pb = std::max(40, std::min(e + 40, msb_r + 30)) + gap_extra;  // relative bits worth computing for the correction
     const int nwX = ceil_div(pb + 3, 28);
     const int topR = msb_r + 2, nwR = ceil_div(pb + 2, 28);
     ZKD_TRY(gemm_complex(n, n, n, nb, side(Xc, topX, nwX, true), side(R, topR, nwR, false), Cc, GemmMode::Assign, -1, opt.gemm_path,

@@ -76,6 +76,16 @@ struct GemmSide {
   bool conj_transpose = false;  // P only: use A^H (stored K x M)
   int top_bit = 0;
   int nw = 0;
+  // optional view: batch element v is the rows x cols sub-matrix that starts at complex element off[v] of an array of
+  // plane_count complex elements with row stride ld (cluster blocks and column slices of X, W, S)
+  int ld = 0;                // 0: cols
+  const int* off = nullptr;  // device, [batch]; null: v * rows * cols
+  size_t plane_count = 0;    // 0: batch * rows * cols
+};
+struct GemmDstView {         // the same for the destination (M x N per batch element)
+  int ld = 0;
+  const int* off = nullptr;
+  size_t plane_count = 0;
 };
 enum class GemmMode : int { Assign = 0, Add = 1, Sub = 2 };
 
@@ -85,7 +95,7 @@ size_t gemm_workspace_bytes(int M, int N, int K, int batch);
 // msb_out (device int, may be null): atomicMax of the msb position of |result| elements.
 int gemm_complex(int M, int N, int K, int batch, const GemmSide& P, const GemmSide& Q, int32_t* dst_fx, GemmMode mode,
                  int out_cut_bit, int path, void* workspace, size_t workspace_bytes, int* err_flag, int* msb_out,
-                 cudaStream_t stream);
+                 cudaStream_t stream, const GemmDstView* dst_view = nullptr);
 // number of 28x28-bit digit products one call performs (algorithmic, after instance selection)
 uint64_t gemm_complex_macs(int M, int N, int K, int batch, int nwP, int nwQ, int* inst_np, int* inst_nq);
 
