@@ -24,54 +24,60 @@ int fxc_to_c64(size_t count, const int32_t* src, double2* dst, cudaStream_t s) {
 }
 
 // ---- S2: clusters ----------------------------------------------------------------------------------------------------
-// One CTA per matrix.  F = ||A64||_F; a new cluster starts at j when mu_j - mu_{j-1} > 2^-tau F.
+// One CTA per matrix.  F = ||A64||_F = (sum_j mu_j^2)^(1/2) (the Frobenius norm of a Hermitian matrix from its eigenvalues: no
+// pass over the n^2 entries); a new cluster starts at j when mu_j - mu_{j-1} > 2^-tau F.
 // cl[j] = first column of j's cluster, cle[j] = one past its last column.
 __global__ void __launch_bounds__(256) cluster_kernel(int n, const double2* __restrict__ A64, const double* __restrict__ mu,
                                                       int tau_bits, const int* __restrict__ floor_msb /* [nb] or null */,
                                                       int* __restrict__ cl, int* __restrict__ cle,
                                                       int* __restrict__ stats /* [nb][2]: n_clusters, max_cluster */) {
+  extern __shared__ int s_flag[];  // [n + 1]: 1 where a cluster starts; s_flag[n] = 1
   __shared__ double s_red[8];
-  __shared__ double s_F;
+  __shared__ double s_thr;
+  __shared__ int s_ncl, s_maxc;
+  (void)A64;
   const int b = blockIdx.x, tid = threadIdx.x;
-  const double2* Ab = A64 + (size_t)b * n * n;
+  const double* m = mu + (size_t)b * n;
   double s = 0;
-  for (size_t e = tid; e < (size_t)n * n; e += blockDim.x) { const double2 a = Ab[e]; s += a.x * a.x + a.y * a.y; }
+  for (int j = tid; j < n; j += blockDim.x) s += m[j] * m[j];
   for (int off = 16; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
   if ((tid & 31) == 0) s_red[tid >> 5] = s;
   __syncthreads();
   if (tid == 0) {
     double t = 0;
     for (int w = 0; w < 8; ++w) t += s_red[w];
-    s_F = sqrt(t);
+    // differences below 2^(floor_msb - 812) are noise of the matrix entries themselves (early splits, S4h): never split there
+    double thr = ldexp(sqrt(t), -tau_bits);
+    if (floor_msb) thr = fmax(thr, ldexp(1.0, floor_msb[b] - 812));
+    s_thr = thr;
+    s_ncl = 0;
+    s_maxc = 0;
+    s_flag[n] = 1;
+  }
+  __syncthreads();
+  const double thr = s_thr;
+  for (int j = tid; j < n; j += blockDim.x) s_flag[j] = (j == 0 || (m[j] - m[j - 1] > thr)) ? 1 : 0;
+  __syncthreads();
+  for (int j = tid; j < n; j += blockDim.x) {
+    int lo = j, hi = j + 1;
+    while (!s_flag[lo]) --lo;
+    while (!s_flag[hi]) ++hi;
+    cl[(size_t)b * n + j] = lo;
+    cle[(size_t)b * n + j] = hi;
+    if (lo == j) {
+      atomicAdd(&s_ncl, 1);
+      atomicMax(&s_maxc, hi - lo);
+    }
   }
   __syncthreads();
   if (tid == 0) {
-    // differences below 2^(floor_msb - 812) are noise of the matrix entries themselves (early splits, S4h): never split there
-    double thr = ldexp(s_F, -tau_bits);
-    if (floor_msb) thr = fmax(thr, ldexp(1.0, floor_msb[b] - 812));
-    const double* m = mu + (size_t)b * n;
-    int* c = cl + (size_t)b * n;
-    int* ce = cle + (size_t)b * n;
-    int start = 0, ncl = 0, maxc = 0;
-    for (int j = 0; j < n; ++j) {
-      if (j > 0 && (m[j] - m[j - 1] > thr)) {
-        for (int k = start; k < j; ++k) ce[k] = j;
-        if (j - start > maxc) maxc = j - start;
-        ++ncl;
-        start = j;
-      }
-      c[j] = start;
-    }
-    for (int k = start; k < n; ++k) ce[k] = n;
-    if (n - start > maxc) maxc = n - start;
-    ++ncl;
-    stats[2 * b] = ncl;
-    stats[2 * b + 1] = maxc;
+    stats[2 * b] = s_ncl;
+    stats[2 * b + 1] = s_maxc;
   }
 }
 int cluster_detect(int n, int nb, const double2* A64, const double* mu, int tau_bits, const int* floor_msb, int* cl, int* cle,
                    int* stats, cudaStream_t s) {
-  cluster_kernel<<<nb, 256, 0, s>>>(n, A64, mu, tau_bits, floor_msb, cl, cle, stats);
+  cluster_kernel<<<nb, 256, sizeof(int) * (n + 1), s>>>(n, A64, mu, tau_bits, floor_msb, cl, cle, stats);
   count_launch();
   return launch_check();
 }

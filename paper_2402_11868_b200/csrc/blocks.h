@@ -25,7 +25,7 @@ int ecalc(int n, int nb, const int32_t* theta, const int* cl, int32_t* C, int pr
 
 // finalize.cu
 // S0: per-matrix scale (max exponent over the upper triangle) and ingest with Hermitian mirroring
-int ingest_herm(int N, int batch, const void* A_api, int32_t* A_fx, int* scale /*[batch]*/, int* status /*[batch]*/, cudaStream_t s);
+int ingest_herm(int N, int batch, const void* A_api, int32_t* A_fx, int* scale /*[2 * batch]: scales, then scratch*/, int* status /*[batch]*/, cudaStream_t s);
 // S5 plumbing: gather cluster blocks of S into a batch of m x m sub-problems scaled by 2^k, and back
 struct SubProblem { int b, col0; };  // matrix index and first column of the cluster
 int sub_gather(int n, int nb, int m, int nsub, const SubProblem* subs_dev, const int32_t* S, int32_t* H /*nsub m m*/,

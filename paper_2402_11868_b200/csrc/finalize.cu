@@ -1,45 +1,49 @@
 // finalize.cu — S0 (scale + Hermitian ingest), S5 plumbing (cluster sub-problems in and out) and S6 (sort,
 // phase-normalise, export).  Readings A5/A9/A15 of DESIGN.md: upper triangle authoritative; ascending order; unit
 // 2-norm; the first component of largest modulus is made real positive.
+#include <algorithm>
+
 #include "blocks.h"
 #include "fx_api.cuh"
 
 namespace zkd {
 
 // ---- S0 ------------------------------------------------------------------------------------------------------------
-// per matrix: scale = -(max exponent over the upper triangle) - 2, so that max |a_ij| 2^scale lies in [1/8, 1/4)
-__global__ void __launch_bounds__(256) maxexp_kernel(int N, const uint8_t* __restrict__ A, int* __restrict__ scale, int* __restrict__ status) {
-  __shared__ long long s_max;
-  __shared__ int s_bad, s_any;
-  const int b = blockIdx.x;
-  if (threadIdx.x == 0) { s_max = LLONG_MIN; s_bad = 0; s_any = 0; }
+// per matrix: scale = -(max exponent over the upper triangle) - 2, so that max |a_ij| 2^scale lies in [1/8, 1/4).
+// Pass 1 (grid: chunks x batch): rawmax[b] <- max exponent (clamped to +-2^30; kNoExp when every entry is zero),
+// status[b] |= 3 on a malformed number.  The ingest kernel turns rawmax into the scale.
+constexpr int kNoExp = (int)0x80808080;  // what cudaMemsetAsync(.., 0x80, ..) leaves: below every clamped exponent
+__global__ void __launch_bounds__(256) maxexp_kernel(int N, const uint8_t* __restrict__ A, int* __restrict__ rawmax, int* __restrict__ status) {
+  __shared__ int s_max, s_bad;
+  const int b = blockIdx.y;
+  if (threadIdx.x == 0) { s_max = kNoExp; s_bad = 0; }
   __syncthreads();
   const uint8_t* Ab = A + (size_t)b * N * N * 2 * kApiRealBytes;
-  long long mx = LLONG_MIN;
-  bool bad = false, any = false;
-  for (size_t e = threadIdx.x; e < (size_t)N * N; e += blockDim.x) {
+  int mx = kNoExp;
+  bool bad = false;
+  for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < (size_t)N * N; e += (size_t)gridDim.x * blockDim.x) {
     const int i = (int)(e / N), j = (int)(e % N);
     if (i > j) continue;
     int64_t ex;
-    if (api_real_exp(Ab + e * 2 * kApiRealBytes, &ex, &bad)) { any = true; if (ex > mx) mx = ex; }
-    if (i < j) {
-      if (api_real_exp(Ab + e * 2 * kApiRealBytes + kApiRealBytes, &ex, &bad)) { any = true; if (ex > mx) mx = ex; }
+    for (int part = 0; part < (i < j ? 2 : 1); ++part) {
+      if (api_real_exp(Ab + (e * 2 + part) * kApiRealBytes, &ex, &bad)) {
+        const int ec = ex > (1 << 30) ? (1 << 30) : ex < -(1 << 30) ? -(1 << 30) : (int)ex;
+        if (ec > mx) mx = ec;
+      }
     }
   }
-  if (any) { atomicMax(&s_max, mx); s_any = 1; }
+  if (mx != kNoExp) atomicMax(&s_max, mx);
   if (bad) s_bad = 1;
   __syncthreads();
   if (threadIdx.x == 0) {
-    long long sc = s_any ? -(s_max)-2 : 0;
-    if (sc > (1 << 30)) sc = 1 << 30;
-    if (sc < -(1 << 30)) sc = -(1 << 30);
-    scale[b] = (int)sc;
-    status[b] = s_bad ? 3 : 0;
+    if (s_max != kNoExp) atomicMax(&rawmax[b], s_max);
+    if (s_bad) atomicOr(&status[b], 3);
   }
 }
+__device__ __forceinline__ int scale_from_rawmax(int rawmax) { return rawmax == kNoExp ? 0 : -rawmax - 2; }
 
-__global__ void __launch_bounds__(128) ingest_kernel(int N, int batch, const uint8_t* __restrict__ A, const int* __restrict__ scale,
-                                                     int32_t* __restrict__ dst, int* __restrict__ status) {
+__global__ void __launch_bounds__(128) ingest_kernel(int N, int batch, const uint8_t* __restrict__ A, const int* __restrict__ rawmax,
+                                                     int* __restrict__ scale, int32_t* __restrict__ dst, int* __restrict__ status) {
   const size_t per = (size_t)N * N, count = per * batch;
   const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= 2 * count) return;
@@ -48,19 +52,27 @@ __global__ void __launch_bounds__(128) ingest_kernel(int N, int batch, const uin
   const int b = (int)(e / per), i = (int)((e % per) / N), j = (int)(e % N);
   int32_t d[ND];
   fx_zero(d);
+  const int sc = scale_from_rawmax(rawmax[b]);
+  if (part == 0 && e == (size_t)b * per) scale[b] = sc;  // for the export
   if (!(part == 1 && i == j) && status[b] == 0) {
     const int si = i <= j ? i : j, sj = i <= j ? j : i;
     const uint8_t* s = A + (((size_t)b * per + (size_t)si * N + sj) * 2 + part) * kApiRealBytes;
-    const int st = api_real_to_fx(s, scale[b], part == 1 && i > j, d);
+    const int st = api_real_to_fx(s, sc, part == 1 && i > j, d);
     if (st) { atomicOr(&status[b], 3); fx_zero(d); }
   }
   fx_store(dst + (part ? (size_t)ND * count : 0), count, e, d);
 }
 
-int ingest_herm(int N, int batch, const void* A_api, int32_t* A_fx, int* scale, int* status, cudaStream_t s) {
-  maxexp_kernel<<<batch, 256, 0, s>>>(N, (const uint8_t*)A_api, scale, status);
+int ingest_herm(int N, int batch, const void* A_api, int32_t* A_fx, int* scale /* 2 * batch ints */, int* status, cudaStream_t s) {
+  int* rawmax = scale + batch;
+  ZKD_CUDA_TRY(cudaMemsetAsync(rawmax, 0x80, sizeof(int) * batch, s));
+  ZKD_CUDA_TRY(cudaMemsetAsync(status, 0, sizeof(int) * batch, s));
+  // enough CTAs per matrix to fill the machine when the batch is small
+  const size_t per = (size_t)N * N;
+  unsigned chunks = (unsigned)std::min<size_t>((per + 255) / 256, (size_t)std::max(1, 592 / batch));
+  maxexp_kernel<<<dim3(chunks, batch), 256, 0, s>>>(N, (const uint8_t*)A_api, rawmax, status);
   const size_t t = 2 * (size_t)N * N * batch;
-  ingest_kernel<<<(unsigned)((t + 127) / 128), 128, 0, s>>>(N, batch, (const uint8_t*)A_api, scale, A_fx, status);
+  ingest_kernel<<<(unsigned)((t + 127) / 128), 128, 0, s>>>(N, batch, (const uint8_t*)A_api, rawmax, scale, A_fx, status);
   count_launch(2);
   return launch_check();
 }

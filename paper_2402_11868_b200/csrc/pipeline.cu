@@ -592,7 +592,7 @@ int diag_herm_device(int N, int batch, const void* A_api, void* eigvals_api, voi
   int32_t* X = (int32_t*)c.ar.alloc(FxC::bytes(cnt));
   int32_t* lam = (int32_t*)c.ar.alloc(FxR::bytes((size_t)N * batch));
   int32_t* lam_sorted = (int32_t*)c.ar.alloc(FxR::bytes((size_t)N * batch));
-  int* scale = c.ar.get<int>((size_t)batch);
+  int* scale = c.ar.get<int>((size_t)2 * batch);  // [batch] scales, then [batch] raw maxima of the ingest
   int* status = c.ar.get<int>((size_t)batch);
   int* rank = c.ar.get<int>((size_t)N * batch);
   int* cl_stats_dev = c.ar.get<int>((size_t)2 * batch);
