@@ -514,6 +514,141 @@ __global__ void __launch_bounds__(128) seed_large_kernel(int n, const double2* _
   }
 }
 
+// ---- large matrices, blocked: a CTA holds two blocks of W columns in shared memory -------------------------------------------
+// Same one-sided Jacobi, but the round-robin tournament runs over BLOCKS of W columns: per round a CTA loads its two blocks
+// (2 W n double2, <= 200 KB), rotates every cross pair (W sub-rounds of W disjoint pairs, one warp per pair; in round 0 of a
+// sweep also the pairs inside each block) and writes the blocks back.  Every pair of columns still meets once per sweep, but
+// there are (n / W - 1) rounds (grid syncs, passes over G in L2) per sweep instead of (n - 1).
+__device__ __forceinline__ double rotate_pair_smem(double2* __restrict__ gp, double2* __restrict__ gq, int n, int lane, double tol2) {
+  double al = 0, be = 0, gr = 0, gi = 0;
+  for (int i = lane; i < n; i += 32) {
+    const double2 a = gp[i], b = gq[i];
+    al = fma(a.x, a.x, fma(a.y, a.y, al));
+    be = fma(b.x, b.x, fma(b.y, b.y, be));
+    gr = fma(a.x, b.x, fma(a.y, b.y, gr));
+    gi = fma(a.x, b.y, fma(-a.y, b.x, gi));
+  }
+  al = warp_sum(al); be = warp_sum(be); gr = warp_sum(gr); gi = warp_sum(gi);
+  double c, sr, si, cos2;
+  if (!rot_params(al, be, gr, gi, tol2, c, sr, si, cos2)) return cos2;
+  for (int i = lane; i < n; i += 32) {
+    const double2 a = gp[i], b = gq[i];
+    gp[i] = make_double2(c * a.x - (sr * b.x + si * b.y), c * a.y - (sr * b.y - si * b.x));
+    gq[i] = make_double2(sr * a.x - si * a.y + c * b.x, sr * a.y + si * a.x + c * b.y);
+  }
+  return cos2;
+}
+
+template <int W>
+__global__ void __launch_bounds__(256) seed_block_kernel(int n, const double2* __restrict__ A, double2* __restrict__ G,
+                                                         const double* __restrict__ sigma_p, int* __restrict__ rot_flags,
+                                                         double* __restrict__ mu_unsorted, int max_sweeps, double tol2) {
+  extern __shared__ double2 s_cols[];  // [2 W][n]
+  cg::grid_group grid = cg::this_grid();
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int gwarp = (blockIdx.x * blockDim.x + tid) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
+  const size_t gtid = (size_t)blockIdx.x * blockDim.x + tid, gthr = (size_t)gridDim.x * blockDim.x;
+  const double sigma = *sigma_p;
+  for (size_t e = gtid; e < (size_t)n * n; e += gthr) {
+    const int i = (int)(e % n), j = (int)(e / n);
+    double2 a = (i <= j) ? A[(size_t)i * n + j] : A[(size_t)j * n + i];
+    if (i > j) a.y = -a.y;
+    if (i == j) { a.y = 0; a.x += sigma; }
+    G[e] = a;
+  }
+  if (gtid < (size_t)max_sweeps) rot_flags[gtid] = 0;
+  grid.sync();
+  const int NB = (n + W - 1) / W, MB = NB + (NB & 1), npairs = MB / 2;
+  if (sigma > 0) {
+    for (int sweep = 0; sweep < max_sweeps; ++sweep) {
+      double cmax = 0;
+      for (int r = 0; r < MB - 1; ++r) {
+        for (int pi = blockIdx.x; pi < npairs; pi += gridDim.x) {
+          int bp, bq;
+          rr_pair(MB, r, pi, bp, bq);
+          // load (absent columns, beyond n or in the padding block, are zero: rot_params leaves zero columns alone)
+          for (int c = 0; c < 2 * W; ++c) {
+            const int col = (c < W ? bp : bq) * W + (c % W);
+            double2* dst = s_cols + (size_t)c * n;
+            if (col < n) {
+              const double2* src = G + (size_t)col * n;
+              for (int i = tid; i < n; i += blockDim.x) dst[i] = __ldcg(src + i);
+            } else {
+              for (int i = tid; i < n; i += blockDim.x) dst[i] = make_double2(0.0, 0.0);
+            }
+          }
+          __syncthreads();
+          if (r == 0 && W > 1) {
+            // pairs inside each block, once per sweep: round-robin over W columns, both blocks at once
+            for (int t = 0; t < W - 1; ++t) {
+              if (warp < W) {
+                const int blk = warp / (W / 2), i = warp % (W / 2);
+                int p, q;
+                rr_pair(W, t, i, p, q);
+                cmax = fmax(cmax, rotate_pair_smem(s_cols + (size_t)(blk * W + p) * n, s_cols + (size_t)(blk * W + q) * n, n, lane, tol2));
+              }
+              __syncthreads();
+            }
+          }
+          for (int t = 0; t < W; ++t) {
+            if (warp < W) {
+              const int p = warp, q = W + (warp + t) % W;
+              cmax = fmax(cmax, rotate_pair_smem(s_cols + (size_t)p * n, s_cols + (size_t)q * n, n, lane, tol2));
+            }
+            __syncthreads();
+          }
+          for (int c = 0; c < 2 * W; ++c) {
+            const int col = (c < W ? bp : bq) * W + (c % W);
+            if (col < n) {
+              const double2* src = s_cols + (size_t)c * n;
+              double2* dst = G + (size_t)col * n;
+              for (int i = tid; i < n; i += blockDim.x) __stcg(dst + i, src[i]);
+            }
+          }
+          __syncthreads();
+        }
+        if (r == MB - 2 && cmax > kSeedStopCos2 && lane == 0) rot_flags[sweep] = 1;
+        grid.sync();
+      }
+      if (!rot_flags[sweep]) break;
+    }
+  }
+  for (int j = gwarp; j < n; j += nwarps) {
+    double s = 0;
+    for (int i = lane; i < n; i += 32) { const double2 a = G[(size_t)j * n + i]; s += a.x * a.x + a.y * a.y; }
+    s = warp_sum(s);
+    if (lane == 0) mu_unsorted[j] = sqrt(s) - sigma;
+  }
+}
+
+template <int W>
+static int launch_block(int n, int sms, const double2* Ab, double2* G, double* sigma, int* flags, double* mu_uns, int ms, double t2,
+                        cudaStream_t s) {
+  const size_t smem = sizeof(double2) * 2 * W * (size_t)n;
+  static bool attr_done = false;
+  if (!attr_done) {
+    if (cudaFuncSetAttribute(seed_block_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) {
+      (void)cudaGetLastError();
+      return ZKD_ERR_CUDA;
+    }
+    attr_done = true;
+  }
+  int maxb = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&maxb, seed_block_kernel<W>, 256, smem) != cudaSuccess || maxb < 1) {
+    (void)cudaGetLastError();
+    return ZKD_ERR_CUDA;
+  }
+  const int NB = (n + W - 1) / W, MB = NB + (NB & 1);
+  int nblocks = MB / 2;
+  if (nblocks > maxb * sms) nblocks = maxb * sms;
+  void* args[] = {&n, (void*)&Ab, &G, &sigma, &flags, &mu_uns, &ms, &t2};
+  if (cudaLaunchCooperativeKernel((void*)seed_block_kernel<W>, dim3(nblocks), dim3(256), args, smem, s) != cudaSuccess) {
+    (void)cudaGetLastError();
+    return ZKD_ERR_CUDA;
+  }
+  return ZKD_OK;
+}
+
 // V[i][rank(j)] = g_j[i] / ||g_j||, mu[rank(j)] = mu_j; one CTA per group of source columns, coalesced on the source
 __global__ void __launch_bounds__(256) seed_sort_kernel(int n, const double* __restrict__ mu_unsorted, const double2* __restrict__ G,
                                                         const double* __restrict__ sigma_p, double* __restrict__ mu,
@@ -598,12 +733,20 @@ int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int ma
     double2* Vb = (double2*)V + (size_t)b * nn;
     int n = N, ms = max_sweeps > 64 ? 64 : max_sweeps;
     double t2 = tol2;
-    void* args[] = {&n, (void*)&Ab, &G, &sigma, &flags, &mu_uns, &ms, &t2};
-    if (cudaLaunchCooperativeKernel((void*)seed_large_kernel, dim3(nblocks), dim3(128), args, 0, s) != cudaSuccess) {
-      (void)cudaGetLastError();
-      rc = ZKD_ERR_CUDA;
-      break;
+    // blocked kernel with the widest column blocks whose pair fits shared memory; plain kernel beyond that
+    const size_t col_bytes = sizeof(double2) * (size_t)n;
+    const size_t smem_budget = 200 * 1024;
+    if (options().seed_path != 3 && 16 * col_bytes <= smem_budget) rc = launch_block<8>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, s);
+    else if (options().seed_path != 3 && 8 * col_bytes <= smem_budget) rc = launch_block<4>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, s);
+    else if (options().seed_path != 3 && 4 * col_bytes <= smem_budget) rc = launch_block<2>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, s);
+    else {
+      void* args[] = {&n, (void*)&Ab, &G, &sigma, &flags, &mu_uns, &ms, &t2};
+      if (cudaLaunchCooperativeKernel((void*)seed_large_kernel, dim3(nblocks), dim3(128), args, 0, s) != cudaSuccess) {
+        (void)cudaGetLastError();
+        rc = ZKD_ERR_CUDA;
+      }
     }
+    if (rc != ZKD_OK) break;
     seed_sort_kernel<<<sms, 256, 0, s>>>(N, mu_uns, G, sigma, mub, Vb);
     count_launch(3);
     rc = launch_check();

@@ -194,7 +194,7 @@ def test_gemm_fx_flags_window_overflow(zkd):
     assert int(err.item()) & 1
 
 
-@pytest.mark.parametrize("N,batch", [(1, 2), (2, 3), (7, 2), (16, 4), (33, 2), (64, 3), (96, 1), (200, 1)])
+@pytest.mark.parametrize("N,batch", [(1, 2), (2, 3), (7, 2), (16, 4), (33, 2), (64, 3), (96, 1), (200, 1), (300, 1), (515, 2), (1000, 1)])
 def test_seed_fp64_vs_lapack(zkd, N, batch):
     import torch
 
