@@ -302,34 +302,47 @@ int fxc_add_inplace(size_t count, int32_t* X, const int32_t* T, cudaStream_t s) 
 //                        s = x_j^H w_j ;  theta_j = Re s ;  r_j = w_j - x_j s                  (Rayleigh quotient, residual)
 // X and W are updated in place (a CTA touches only its own column).  Replaces gram, ns_build, 2 x block_apply, gram, theta,
 // block_apply of the general path (7 launches) by one launch whose critical path is 14 digit products per element.
-template <int NACC2>
-__device__ __forceinline__ void block_sum_cols(int64_t (&acc)[NACC2], int64_t* s_part /*[nwarps][NACC2]*/, int nwarps) {
-  warp_sum_cols(acc);
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  __syncthreads();  // s_part may still be read from the previous reduction
-  if (lane == 0) {
+// Sum of column accumulators over the threads of the CTA that own the same matrix column.  Thread layout: tx = tid % CPB is
+// the matrix column inside the CTA's group of CPB columns, the other bits of tid index rows; lanes with equal tx are
+// lane % CPB apart, so the warp stage uses xor offsets 16 .. CPB only.  Every thread returns its column's total.
+template <int CPB, int NACC2>
+__device__ __forceinline__ void block_sum_cols(int64_t (&acc)[NACC2], int64_t* s_part /*[nwarps][CPB][NACC2]*/, int nwarps) {
 #pragma unroll
-    for (int k = 0; k < NACC2; ++k) s_part[warp * NACC2 + k] = acc[k];
+  for (int off = 16; off >= CPB; off >>= 1) {
+#pragma unroll
+    for (int k = 0; k < NACC2; ++k) acc[k] += __shfl_down_sync(0xffffffffu, acc[k], off);
+  }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, tx = threadIdx.x % CPB;
+  __syncthreads();  // s_part may still be read from the previous reduction
+  if (lane < CPB) {
+#pragma unroll
+    for (int k = 0; k < NACC2; ++k) s_part[(warp * CPB + lane) * NACC2 + k] = acc[k];
   }
   __syncthreads();
 #pragma unroll
   for (int k = 0; k < NACC2; ++k) {
     int64_t t = 0;
-    for (int w = 0; w < nwarps; ++w) t += s_part[w * NACC2 + k];
+    for (int w = 0; w < nwarps; ++w) t += s_part[(w * CPB + tx) * NACC2 + k];
     acc[k] = t;
   }
 }
 
+// CPB matrix columns per CTA: a warp reads CPB consecutive columns of 32 / CPB rows, i.e. CPB * 4 contiguous bytes per row
+// (row-major X: a single column per CTA touches one 32-byte sector per element and digit).
+template <int CPB>
 __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int32_t* __restrict__ X, int32_t* __restrict__ W,
                                                              int32_t* __restrict__ R, int32_t* __restrict__ S,
                                                              int32_t* __restrict__ theta, int* __restrict__ msb_g_out,
                                                              int* __restrict__ msb_r_out, const int* __restrict__ cl,
                                                              const int* __restrict__ cle) {
-  __shared__ int64_t s_part[8 * FXP_NACC];
+  __shared__ int64_t s_part[8 * CPB * FXP_NACC];
   __shared__ int s_msb;
-  const int b = blockIdx.x / n, j = blockIdx.x % n;
-  if (cl && cle[blockIdx.x] - cl[blockIdx.x] > 1) return;  // mixed levels: columns of larger clusters take the GEMM path
-  const int tid = threadIdx.x, nwarps = blockDim.x >> 5;
+  const int groups = (n + CPB - 1) / CPB;
+  const int b = blockIdx.x / groups;
+  const int tid = threadIdx.x, nwarps = blockDim.x >> 5, tx = tid % CPB, ty = tid / CPB, rows = blockDim.x / CPB;
+  const int j = (blockIdx.x % groups) * CPB + tx;
+  // mixed levels: columns of larger clusters take the GEMM path
+  const bool act = j < n && !(cl && cle[(size_t)b * n + j] - cl[(size_t)b * n + j] > 1);
   const size_t per = (size_t)n * n, count = per * nb;
   int32_t* Xr = X;  int32_t* Xi = X + (size_t)ND * count;
   int32_t* Wr = W;  int32_t* Wi = W + (size_t)ND * count;
@@ -339,18 +352,20 @@ __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int3
   // g = sum_k |x_kj|^2
   int64_t acc[FXP_NACC];
   fxp_zero(acc);
-  for (int k = tid; k < n; k += blockDim.x) {
-    const size_t e = (size_t)b * per + (size_t)k * n + j;
-    int32_t a[ND];
-    fx_load(a, Xr, count, e); fx_mac<false>(acc, a, a);
-    fx_load(a, Xi, count, e); fx_mac<false>(acc, a, a);
-    fxp_relax(acc);
+  if (act) {
+    for (int k = ty; k < n; k += rows) {
+      const size_t e = (size_t)b * per + (size_t)k * n + j;
+      int32_t a[ND];
+      fx_load(a, Xr, count, e); fx_mac<false>(acc, a, a);
+      fx_load(a, Xi, count, e); fx_mac<false>(acc, a, a);
+      fxp_relax(acc);
+    }
   }
-  block_sum_cols(acc, s_part, nwarps);
+  block_sum_cols<CPB>(acc, s_part, nwarps);
   int32_t g[ND], m[ND];
   fxp_finish(g, acc);
   g[ND - 1] -= 1;                      // g - 1
-  if (tid == 0 && msb_g_out) atomicMax(msb_g_out, fx_msb(g));
+  if (act && ty == 0 && msb_g_out) atomicMax(msb_g_out, fx_msb(g));
   {
     int32_t t[ND];
     fx_neg(t, g);
@@ -358,18 +373,20 @@ __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int3
   }
 
   // x <- x + x m, w <- w + w m   (one plane at a time: at most three digit arrays and one accumulator set are live)
+  if (act) {
 #pragma unroll 1
-  for (int pl = 0; pl < 4; ++pl) {
-    int32_t* P = pl == 0 ? Xr : pl == 1 ? Xi : pl == 2 ? Wr : Wi;
+    for (int pl = 0; pl < 4; ++pl) {
+      int32_t* P = pl == 0 ? Xr : pl == 1 ? Xi : pl == 2 ? Wr : Wi;
 #pragma unroll 1
-    for (int k = tid; k < n; k += blockDim.x) {
-      const size_t e = (size_t)b * per + (size_t)k * n + j;
-      int32_t u[ND], t[ND];
-      fx_load(u, P, count, e);
-      fx_mul(t, u, m);
-      int32_t o[ND];
-      fx_add(o, u, t);
-      fx_store(P, count, e, o);
+      for (int k = ty; k < n; k += rows) {
+        const size_t e = (size_t)b * per + (size_t)k * n + j;
+        int32_t u[ND], t[ND];
+        fx_load(u, P, count, e);
+        fx_mul(t, u, m);
+        int32_t o[ND];
+        fx_add(o, u, t);
+        fx_store(P, count, e, o);
+      }
     }
   }
   // s = x^H w : real part, then imaginary part
@@ -377,23 +394,25 @@ __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int3
 #pragma unroll 1
   for (int part = 0; part < 2; ++part) {
     fxp_zero(acc);
+    if (act) {
 #pragma unroll 1
-    for (int k = tid; k < n; k += blockDim.x) {
-      const size_t e = (size_t)b * per + (size_t)k * n + j;
-      int32_t a[ND], c[ND];
-      if (part == 0) {  // xr wr + xi wi
-        fx_load(a, Xr, count, e); fx_load(c, Wr, count, e); fx_mac<false>(acc, a, c);
-        fx_load(a, Xi, count, e); fx_load(c, Wi, count, e); fx_mac<false>(acc, a, c);
-      } else {          // xr wi - xi wr
-        fx_load(a, Xr, count, e); fx_load(c, Wi, count, e); fx_mac<false>(acc, a, c);
-        fx_load(a, Xi, count, e); fx_load(c, Wr, count, e); fx_mac<true>(acc, a, c);
+      for (int k = ty; k < n; k += rows) {
+        const size_t e = (size_t)b * per + (size_t)k * n + j;
+        int32_t a[ND], c[ND];
+        if (part == 0) {  // xr wr + xi wi
+          fx_load(a, Xr, count, e); fx_load(c, Wr, count, e); fx_mac<false>(acc, a, c);
+          fx_load(a, Xi, count, e); fx_load(c, Wi, count, e); fx_mac<false>(acc, a, c);
+        } else {          // xr wi - xi wr
+          fx_load(a, Xr, count, e); fx_load(c, Wi, count, e); fx_mac<false>(acc, a, c);
+          fx_load(a, Xi, count, e); fx_load(c, Wr, count, e); fx_mac<true>(acc, a, c);
+        }
+        fxp_relax(acc);
       }
-      fxp_relax(acc);
     }
-    block_sum_cols(acc, s_part, nwarps);
+    block_sum_cols<CPB>(acc, s_part, nwarps);
     if (part == 0) fxp_finish(sr, acc); else fxp_finish(si, acc);
   }
-  if (tid == 0) {
+  if (act && ty == 0) {
     fx_store(theta, (size_t)n * nb, (size_t)b * n + j, sr);
     const size_t ejj = (size_t)b * per + (size_t)j * n + j;
     fx_store(S, count, ejj, sr);
@@ -402,38 +421,54 @@ __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int3
 
   // r = w - x s
   int mymsb = 0;
+  if (act) {
 #pragma unroll 1
-  for (int part = 0; part < 2; ++part) {
+    for (int part = 0; part < 2; ++part) {
 #pragma unroll 1
-    for (int k = tid; k < n; k += blockDim.x) {
-      const size_t e = (size_t)b * per + (size_t)k * n + j;
-      int32_t a[ND], t[ND];
-      fxp_zero(acc);
-      if (part == 0) {  // xr sr - xi si
-        fx_load(a, Xr, count, e); fx_mac<false>(acc, a, sr);
-        fx_load(a, Xi, count, e); fx_mac<true>(acc, a, si);
-      } else {          // xr si + xi sr
-        fx_load(a, Xr, count, e); fx_mac<false>(acc, a, si);
-        fx_load(a, Xi, count, e); fx_mac<false>(acc, a, sr);
+      for (int k = ty; k < n; k += rows) {
+        const size_t e = (size_t)b * per + (size_t)k * n + j;
+        int32_t a[ND], t[ND];
+        fxp_zero(acc);
+        if (part == 0) {  // xr sr - xi si
+          fx_load(a, Xr, count, e); fx_mac<false>(acc, a, sr);
+          fx_load(a, Xi, count, e); fx_mac<true>(acc, a, si);
+        } else {          // xr si + xi sr
+          fx_load(a, Xr, count, e); fx_mac<false>(acc, a, si);
+          fx_load(a, Xi, count, e); fx_mac<false>(acc, a, sr);
+        }
+        fxp_finish(t, acc);
+        fx_load(a, part ? Wi : Wr, count, e);
+        int32_t o[ND];
+        fx_sub(o, a, t);
+        fx_store(part ? Ri : Rr, count, e, o);
+        mymsb = max(mymsb, fx_msb(o));
       }
-      fxp_finish(t, acc);
-      fx_load(a, part ? Wi : Wr, count, e);
-      int32_t o[ND];
-      fx_sub(o, a, t);
-      fx_store(part ? Ri : Rr, count, e, o);
-      mymsb = max(mymsb, fx_msb(o));
     }
   }
   for (int off = 16; off > 0; off >>= 1) mymsb = max(mymsb, __shfl_xor_sync(0xffffffffu, mymsb, off));
   if ((tid & 31) == 0 && mymsb) atomicMax(&s_msb, mymsb);
   __syncthreads();
-  if (tid == 0 && msb_r_out) atomicMax(msb_r_out, s_msb);
+  if (tid == 0 && msb_r_out && s_msb) atomicMax(msb_r_out, s_msb);
 }
 int singleton_step(int n, int nb, int32_t* X, int32_t* W, int32_t* R, int32_t* S, int32_t* theta, int* msb_g_out, int* msb_r_out,
                    cudaStream_t s, const int* cl, const int* cle) {
-  int threads = (n + 31) / 32 * 32;
-  if (threads > 256) threads = 256;
-  singleton_step_kernel<<<(unsigned)((size_t)n * nb), threads, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
+  // columns per CTA: as many as keep about one CTA per SM (sector efficiency of the row-major loads against parallelism)
+  const size_t cols = (size_t)n * nb;
+  const int forced = options().sstep_cpb;
+  const int cpb = (forced == 1 || forced == 2 || forced == 4 || forced == 8) ? forced
+                  : cols >= 8 * 128 ? 8 : cols >= 4 * 96 ? 4 : cols >= 2 * 96 ? 2 : 1;
+  const unsigned grid = (unsigned)((size_t)((n + cpb - 1) / cpb) * nb);
+  if (cpb == 1) {
+    int threads = (n + 31) / 32 * 32;
+    if (threads > 256) threads = 256;
+    singleton_step_kernel<1><<<grid, threads, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
+  } else if (cpb == 2) {
+    singleton_step_kernel<2><<<grid, 256, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
+  } else if (cpb == 4) {
+    singleton_step_kernel<4><<<grid, 256, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
+  } else {
+    singleton_step_kernel<8><<<grid, 256, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
+  }
   count_launch();
   return launch_check();
 }
