@@ -87,6 +87,28 @@ def test_parity_small_configs(zkd, name, batch):
             check_sorted_and_phase(lam[i], X[i], N)
 
 
+@pytest.mark.parametrize("name,opt,val", [("c4small", "early_split", 0), ("c5small", "split_margin_bits", 20),
+                                          ("c4small", "tau_bits", 12), ("c5small", "tau_bits", 30), ("c4small", "sstep_cpb", 8),
+                                          ("c2", "sstep_cpb", 4), ("c1", "sstep_cpb", 2)])
+def test_parity_alternative_paths(zkd, name, opt, val):
+    """The same results through the other routes of the method: clusters left to the S5 recursion (S4h off), a different
+    cluster threshold (other cluster tables, splits and recursion depths), several matrix columns per CTA in the fused
+    singleton kernel."""
+    cfg = zi.config(name, batch=2 if name == "c4small" else None)
+    N, b = cfg["N"], cfg["batch"]
+    old = zkd.get_option(opt)
+    zkd.set_option(opt, val)
+    try:
+        lam, X, info = gpu_diag(zkd, cfg["A"], N, b)
+    finally:
+        zkd.set_option(opt, old)
+    A = cfg["A"].reshape(b, -1)
+    for i in range(b):
+        assert info[i]["status"] == 0, info[i]
+        l0, X0, _ = oracle.diag_herm(A[i], N)
+        check(oracle.compare(A[i], N, lam[i], X[i], l0, X0), (name, opt, val, i))
+
+
 @pytest.mark.parametrize("N", [1, 2, 3, 5, 17, 31, 33, 48, 65, 100])
 def test_parity_ragged_sizes(zkd, N):
     A = zi.random_hermitian(N, 4242 + N)
