@@ -151,6 +151,36 @@ def test_paper_epsilon_example(zkd):
     check(oracle.compare(A, N, lam[0], X[0]), "eps")
 
 
+def test_mixed_batch_different_cluster_tables(zkd):
+    """One batch whose matrices have different cluster structures (a c4-shaped one, a random one, exact multiplicities in
+    the middle of the spectrum, two near-degenerate pairs at 2^-300, a spectrum spanning 2^-1 .. 2^-700): the cluster
+    groups of a pass mix sizes and matrices, and splits / recursion happen for some matrices only."""
+    N = 16
+    mats = [zi.config("c4small", batch=1)["A"], zi.random_hermitian(N, 9001)]
+    half = Fraction(1, 2)
+    spectra = [
+        [Fraction(-3, 4)] * 3 + [Fraction(1, 8)] * 5 + [Fraction(k, 16) for k in range(3, 11)],                  # multiplicities
+        [Fraction(k, 20) for k in range(-7, 5)] + [half, half + Fraction(1, 2 ** 300), Fraction(7, 10),
+                                                   Fraction(7, 10) + Fraction(3, 2 ** 300)],                   # 2^-300 pairs
+        [Fraction(1, 2 ** (1 + 46 * k)) for k in range(N)],                                                       # 2^-1 .. 2^-691
+    ]
+    for t, vals in enumerate(spectra):
+        mats.append(zi.qdq(N, 9100 + t, 0, 4, zi._lam_array(sorted(vals))))
+    A = np.concatenate([np.asarray(m).reshape(-1) for m in mats])
+    b = len(mats)
+    lam, X, info = gpu_diag(zkd, A, N, b)
+    A = A.reshape(b, -1)
+    for i in range(b):
+        assert info[i]["status"] == 0, (i, info[i])
+        l0, X0, oi = oracle.diag_herm(A[i], N)
+        assert oi["status"] == 0
+        check(oracle.compare(A[i], N, lam[i], X[i], l0, X0), ("mixed", i))
+    # the spectrum of matrix 4 is known by construction: every eigenvalue, down to 2^-691, to absolute 2^-740 ||A||_F
+    got = [zi.to_fraction(lam[4].reshape(N, -1)[j]) for j in range(N)]
+    for g, w in zip(got, sorted(spectra[2])):
+        assert abs(g - w) <= Fraction(1, 2 ** 740), (float(g), float(w))
+
+
 # ---- degenerate inputs (P9) ------------------------------------------------------------------------------------------
 
 def _api_matrix(N, fn):
