@@ -338,10 +338,7 @@ struct CombineI8Args {
   int* msb_out;
 };
 
-// one thread per (element, part); part 0 = Re = k1 - k3, part 1 = Im = k1 + k2.
-// Column-driven: the radix-2^8 columns are fetched 14 at a time (= 112 bits = four FX digits; all loads of a chunk in
-// flight together) and fed upward into a running accumulator; whenever a column's LSB passes the next 28-bit boundary the
-// finished FX digit is emitted (cut, accumulate into the destination, msb tracking, store).
+// one thread per (element, part); part 0 = Re = k1 - k3, part 1 = Im = k1 + k2
 __global__ void __launch_bounds__(256) combine_i8_kernel(CombineI8Args a) {
   const size_t tot = a.mn * a.batch;
   const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -358,21 +355,52 @@ __global__ void __launch_bounds__(256) combine_i8_kernel(CombineI8Args a) {
   int32_t* dst = a.dst + (part ? (size_t)ND * tot_d : 0) + (a.off ? (size_t)a.off[b] : (size_t)b * a.mn) +
                  (size_t)(ij / a.N) * a.ld + (ij % a.N);
 
+  auto col = [&](int c) -> int64_t {
+    int64_t s1 = 0, s2 = 0;
+    for (int s = 0; s < a.nsplit; ++s) {
+      s1 += r1[(size_t)s * sstride + (size_t)c * a.mn];
+      s2 += r2[(size_t)s * sstride + (size_t)c * a.mn];
+    }
+    return s1 + sgn2 * s2;
+  };
+  // FX digit k covers bits [28k, 28k+28); walk k upward from the digit holding column 0, feeding each digit the
+  // columns whose LSB falls inside it
   const int kstart = a.base_bit >= 0 ? a.base_bit / DB : -((-a.base_bit + DB - 1) / DB);
   const int cutq = a.cut_bit > 0 ? a.cut_bit / DB : 0, cutr = a.cut_bit > 0 ? a.cut_bit % DB : 0;
   int64_t acc = 0, cy2 = 0;
+  int c = 0;
   int msb_pos = 0, msb_neg = 0;
-  int k = kstart;
-
-  auto emit = [&](int kk, int32_t digit) {
-    if (kk < 0) return;
-    if (kk < cutq) digit = 0;
-    else if (kk == cutq && cutr) digit &= ~((1 << cutr) - 1);
-    int32_t* dp = dst + (size_t)kk * tot_d;
+  for (int k = kstart; k <= ND - 1; ++k) {
+    const int lo = k * DB;
+    if (k < ND - 1) {
+      while (c < a.ncol && a.base_bit + 8 * c < lo + DB) {
+        acc += col(c) << (a.base_bit + 8 * c - lo);
+        ++c;
+      }
+    } else {
+      // the signed top digit takes everything that is left (sign extension unless the result overflows FX, which the
+      // callers' magnitude bounds exclude)
+      while (c < a.ncol) {
+        const int sh = a.base_bit + 8 * c - lo;
+        if (sh < 40) acc += col(c) << sh;
+        ++c;
+      }
+    }
+    int32_t digit;
+    if (k < ND - 1) {
+      digit = (int32_t)(acc & DMASK);
+      acc >>= DB;
+    } else {
+      digit = (int32_t)acc;
+    }
+    if (k < 0) continue;
+    if (k < cutq) digit = 0;
+    else if (k == cutq && cutr) digit &= ~((1 << cutr) - 1);
+    int32_t* dp = dst + (size_t)k * tot_d;
     int32_t outd = digit;
     if (a.mode != 0) {
       const int64_t t = (int64_t)*dp + (a.mode == 1 ? (int64_t)digit : -(int64_t)digit) + cy2;
-      if (kk < ND - 1) {
+      if (k < ND - 1) {
         cy2 = t >> DB;
         outd = (int32_t)(t & DMASK);
       } else {
@@ -380,55 +408,15 @@ __global__ void __launch_bounds__(256) combine_i8_kernel(CombineI8Args a) {
       }
     }
     *dp = outd;
-    if (kk < ND - 1) {
-      if (outd != 0) msb_pos = kk * DB + (32 - __clz(outd));
-      if (outd != DMASK) msb_neg = kk * DB + (32 - __clz((~outd) & DMASK));
+    if (k < ND - 1) {
+      if (outd != 0) msb_pos = k * DB + (32 - __clz(outd));
+      if (outd != DMASK) msb_neg = k * DB + (32 - __clz((~outd) & DMASK));
     } else {
-      if (outd > 0) msb_pos = kk * DB + (32 - __clz(outd));
-      if (outd < -1) msb_neg = kk * DB + (32 - __clz(~outd));
+      if (outd > 0) msb_pos = k * DB + (32 - __clz(outd));
+      if (outd < -1) msb_neg = k * DB + (32 - __clz(~outd));
       if (a.msb_out) atomicMax(a.msb_out, outd < 0 ? msb_neg : msb_pos);
     }
-  };
-
-  constexpr int CH = 14;
-  for (int c0 = 0; c0 < a.ncol; c0 += CH) {
-    int64_t v[CH];
-#pragma unroll
-    for (int u = 0; u < CH; ++u) v[u] = 0;
-    for (int s = 0; s < a.nsplit; ++s) {
-      int32_t l1[CH], l2[CH];
-#pragma unroll
-      for (int u = 0; u < CH; ++u) {
-        const bool in = c0 + u < a.ncol;
-        l1[u] = in ? r1[(size_t)s * sstride + (size_t)(c0 + u) * a.mn] : 0;
-        l2[u] = in ? r2[(size_t)s * sstride + (size_t)(c0 + u) * a.mn] : 0;
-      }
-#pragma unroll
-      for (int u = 0; u < CH; ++u) v[u] += (int64_t)l1[u] + sgn2 * (int64_t)l2[u];
-    }
-#pragma unroll
-    for (int u = 0; u < CH; ++u) {
-      const int c = c0 + u;
-      if (c < a.ncol) {
-        const int pos = a.base_bit + 8 * c;
-        if (k < ND - 1 && pos >= (k + 1) * DB) {  // columns advance by 8 bits: at most one boundary per column
-          emit(k, (int32_t)(acc & DMASK));
-          acc >>= DB;
-          ++k;
-        }
-        const int sh = pos - k * DB;
-        // the signed top digit takes everything that is left (sign extension unless the result overflows FX, which the
-        // callers' magnitude bounds exclude)
-        if (sh < 40) acc += v[u] << sh;
-      }
-    }
   }
-  while (k < ND - 1) {
-    emit(k, (int32_t)(acc & DMASK));
-    acc >>= DB;
-    ++k;
-  }
-  emit(ND - 1, (int32_t)acc);
   if (a.mode == 0)
     for (int kk = 0; kk < kstart && kk < ND; ++kk) dst[(size_t)kk * tot_d] = 0;
 }
