@@ -52,7 +52,8 @@ typedef struct {
   int32_t n_clusters;  /* clusters (incl. singletons) found by S2 at the top level */
   int32_t max_cluster; /* size of the largest cluster */
   float log2_resid;    /* log2 of max_ij |(A X - X diag(lambda))_ij| in units where max|a_ij| is in [1/8,1/4) */
-  float log2_orth;     /* log2 of max |X_c^H X_c - I| over cluster blocks before the last orthonormalisation */
+  float log2_orth;     /* log2 of max |X_c^H X_c - I| over cluster blocks after the last orthonormalisation: twice the
+                          log2 measured before that Newton-Schulz step (which squares it), not below -800 */
 } zkd_info;
 
 /* ---- the hot path ------------------------------------------------------------- */

@@ -561,7 +561,8 @@ __global__ void info_kernel(int batch, const int* __restrict__ status_in, int le
   o.n_clusters = cl_stats ? cl_stats[2 * b] : 0;
   o.max_cluster = cl_stats ? cl_stats[2 * b + 1] : 0;
   o.log2_resid = (float)(msb_r - 812);
-  o.log2_orth = (float)(msb_g - 812);
+  // msb_g is measured before the pass's Newton-Schulz step, which squares the deviation from orthonormality
+  o.log2_orth = fmaxf(2.0f * (float)(msb_g - 812), -800.0f);
   info[b] = o;
 }
 

@@ -261,6 +261,23 @@ def _sample_cols(N, k, seed):
     return np.sort(rng.choice(N, size=min(k, N), replace=False)).astype(np.int32)
 
 
+def test_large_ragged_sampled(zkd):
+    """N = 777 (not a multiple of any tile: ragged 128-tiles of the int8 engine, ragged column blocks of the blocked seed):
+    status, residual and orthogonality of sampled columns against ALL columns (properties that need no oracle), and the
+    trace identity over all eigenvalues."""
+    N = 777
+    A = zi.random_hermitian(N, 7777)
+    lam, X, info = gpu_diag(zkd, A, N, 1)
+    assert info[0]["status"] == 0, info
+    c = oracle.compare(A, N, lam[0], X[0], cols=_sample_cols(N, 8, 3))
+    assert c["log2_resid_rel"] <= TOL and c["log2_orth"] <= TOL, c
+    Ar = A.reshape(N, N, 2, -1)
+    tr = sum(zi.to_fraction(Ar[i, i, 0]) for i in range(N))
+    sl = sum(zi.to_fraction(lam[0].reshape(N, -1)[j]) for j in range(N))
+    F = Fraction(2) ** int(np.ceil(c["log2_F"]))
+    assert abs(tr - sl) <= N * F / 2 ** 740
+
+
 def test_full_c3_sampled(zkd):
     """c3 (N=256): residual and orthogonality (properties that need no oracle) on sampled columns, all eigenvalues
     against trace / Frobenius identities, and full parity against the round-robin oracle when the box has the cores."""
