@@ -300,11 +300,17 @@ __global__ void __launch_bounds__(128) rank_kernel(int N, int batch, const int32
   fx_load(lj, lam, cnt, t);
   int r = 0;
   for (int i = 0; i < N; ++i) {
-    int32_t li[ND];
-    fx_load(li, lam, cnt, (size_t)b * N + i);
-    const bool lt = fx_less(li, lj);
-    const bool eq = !lt && !fx_less(lj, li);
-    r += lt || (eq && i < j);
+    // compare from the top digit down and stop loading at the first difference (almost always the top digit or the next)
+    const int32_t* pi = lam + (size_t)b * N + i;
+    int cmp = 0;  // sign of (lambda_i - lambda_j)
+#pragma unroll
+    for (int k = ND - 1; k >= 0; --k) {
+      if (cmp == 0) {
+        const int32_t d = pi[(size_t)k * cnt];
+        cmp = d < lj[k] ? -1 : d > lj[k] ? 1 : 0;
+      }
+    }
+    r += cmp < 0 || (cmp == 0 && i < j);
   }
   rank[t] = r;
   fx_store(lam_sorted, cnt, (size_t)b * N + r, lj);

@@ -432,11 +432,12 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
       last_cut = 812 - (4 * e_prev + 130);
       ZKD_TRY(cluster_pass(c, n, nb, plan, cl, cle, Xc, Wc, R, Sm, Gm, theta, scal, last_cut, fxc));
     }
-    if (split_done) ZKD_TRY(min_gap(n, nb, theta, cl, scal + S_GAP_INV, s));
+    ZKD_TRY(min_gap(n, nb, theta, cl, scal + S_GAP_INV, s));
     ZKD_TRY(read_scalars(c, scal, S_NUM, hs));
     const int msb_r = hs[S_MSB_R], msb_g = hs[S_MSB_G];
     // clusters that S4h split apart can be much closer than 2^-tau |A|_F: C_ij / gap needs that many more bits of C, E, T
-    const int gap_extra = (split_done && hs[S_GAP_INV]) ? std::max(0, (812 - opt.tau_bits - 2) - (1024 - hs[S_GAP_INV])) : 0;
+    const int gap_msb = hs[S_GAP_INV] ? 1024 - hs[S_GAP_INV] : 0;  // 0: one cluster only, nothing to correct between clusters
+    const int gap_extra = (split_done && gap_msb) ? std::max(0, (812 - opt.tau_bits - 2) - gap_msb) : 0;
     if (opt.verbose) fprintf(stderr, "[zkd] depth %d n %d nb %d step %d: msbR %d (2^%d) msbG %d err %d\n", depth, n, nb, step, msb_r, msb_r - 812, msb_g, hs[S_ERR]);
     if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
     steps = step;
@@ -465,6 +466,8 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
       }
     }
 
+    if (gap_msb == 0) continue;  // a single cluster per matrix: no correction between clusters
+
     // S4d: C = X^H R on windows sized for this step's gain
     const int e = 812 - msb_r;                        // residual ~ 2^-e
     const int pb = std::max(40, std::min(e + 40, msb_r + 30)) + gap_extra;  // relative bits worth computing for the correction
@@ -473,13 +476,14 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
     ZKD_TRY(gemm_complex(n, n, n, nb, side(Xc, topX, nwX, true), side(R, topR, nwR, false), Cc, GemmMode::Assign, -1, opt.gemm_path,
                          c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s));
     ZKD_TRY(ecalc(n, nb, theta, cl, Cc, pb + 8, scal + S_MSB_E, scal + S_ERR, s));
-    ZKD_TRY(read_scalars(c, scal, S_NUM, hs));
-    if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
-    const int msb_e = hs[S_MSB_E];
-    if (msb_e == 0) continue;
+    // No host read of msb(E): a rigorous bound sizes the windows instead.  |C_ij| = |x_i^H r_j| <= |x_i| |r_j| <= sqrt(n) max|R|
+    // (columns are normalised), and |theta_j - theta_i| >= the smallest gap between neighbouring clusters, which the same
+    // read as msb(R) delivered.  The bound is a few bits loose; the E / T windows get those bits back (pbE).
+    const int msb_e = std::min(838, msb_r + (ilog2_ceil(n) + 1) / 2 + 1 + 813 - gap_msb);
+    const int pbE = pb + 8;
     // S4e: T = X E (bits below cutT cleared so that W += A T tracks A X exactly), X += T, W += A T
-    const int topE = msb_e + 2, nwE = ceil_div(pb + 2, 28);
-    const int cutT = std::max(0, msb_e - pb - 4);
+    const int topE = msb_e + 2, nwE = ceil_div(pbE + 2, 28);
+    const int cutT = std::max(0, msb_e - pbE - 4);
     ZKD_TRY(gemm_complex(n, n, n, nb, side(Xc, topX, nwX, false), side(Cc, topE, nwE, false), Tc, GemmMode::Assign, cutT, opt.gemm_path,
                          c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s));
     ZKD_TRY(fxc_add_inplace(cnt, Xc, Tc, s));
