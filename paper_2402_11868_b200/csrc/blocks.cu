@@ -352,12 +352,17 @@ __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int3
   // g = sum_k |x_kj|^2
   int64_t acc[FXP_NACC];
   fxp_zero(acc);
+  // (every product phase below has ONE inlined multiply site, looped over planes / terms with run-time operand and sign
+  // selection: the unrolled 30 x 30 digit product is ~500 IMAD.WIDE, and 14 copies of it thrashed the instruction cache)
   if (act) {
     for (int k = ty; k < n; k += rows) {
       const size_t e = (size_t)b * per + (size_t)k * n + j;
-      int32_t a[ND];
-      fx_load(a, Xr, count, e); fx_mac<false>(acc, a, a);
-      fx_load(a, Xi, count, e); fx_mac<false>(acc, a, a);
+#pragma unroll 1
+      for (int pl = 0; pl < 2; ++pl) {
+        int32_t a[ND];
+        fx_load(a, pl ? Xi : Xr, count, e);
+        fx_mac<false>(acc, a, a);
+      }
       fxp_relax(acc);
     }
   }
@@ -398,13 +403,17 @@ __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int3
 #pragma unroll 1
       for (int k = ty; k < n; k += rows) {
         const size_t e = (size_t)b * per + (size_t)k * n + j;
-        int32_t a[ND], c[ND];
-        if (part == 0) {  // xr wr + xi wi
-          fx_load(a, Xr, count, e); fx_load(c, Wr, count, e); fx_mac<false>(acc, a, c);
-          fx_load(a, Xi, count, e); fx_load(c, Wi, count, e); fx_mac<false>(acc, a, c);
-        } else {          // xr wi - xi wr
-          fx_load(a, Xr, count, e); fx_load(c, Wi, count, e); fx_mac<false>(acc, a, c);
-          fx_load(a, Xi, count, e); fx_load(c, Wr, count, e); fx_mac<true>(acc, a, c);
+        // part 0: xr wr + xi wi ;  part 1: xr wi - xi wr
+#pragma unroll 1
+        for (int term = 0; term < 2; ++term) {
+          int32_t a[ND], c[ND];
+          fx_load(a, term ? Xi : Xr, count, e);
+          fx_load(c, (term ^ part) ? Wi : Wr, count, e);
+          if (part == 1 && term == 1) {
+#pragma unroll
+            for (int q = 0; q < ND; ++q) a[q] = -a[q];  // digit-wise negation: a valid (non-canonical) operand of fx_mac
+          }
+          fx_mac<false>(acc, a, c);
         }
         fxp_relax(acc);
       }
@@ -429,12 +438,18 @@ __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int3
         const size_t e = (size_t)b * per + (size_t)k * n + j;
         int32_t a[ND], t[ND];
         fxp_zero(acc);
-        if (part == 0) {  // xr sr - xi si
-          fx_load(a, Xr, count, e); fx_mac<false>(acc, a, sr);
-          fx_load(a, Xi, count, e); fx_mac<true>(acc, a, si);
-        } else {          // xr si + xi sr
-          fx_load(a, Xr, count, e); fx_mac<false>(acc, a, si);
-          fx_load(a, Xi, count, e); fx_mac<false>(acc, a, sr);
+        // part 0: xr sr - xi si ;  part 1: xr si + xi sr
+#pragma unroll 1
+        for (int term = 0; term < 2; ++term) {
+          int32_t mm[ND];
+          const bool use_si = (term ^ part) != 0, neg = part == 0 && term == 1;
+#pragma unroll
+          for (int q = 0; q < ND; ++q) {
+            const int32_t v = use_si ? si[q] : sr[q];
+            mm[q] = neg ? -v : v;
+          }
+          fx_load(a, term ? Xi : Xr, count, e);
+          fx_mac<false>(acc, a, mm);
         }
         fxp_finish(t, acc);
         fx_load(a, part ? Wi : Wr, count, e);
