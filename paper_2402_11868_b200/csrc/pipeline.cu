@@ -349,7 +349,12 @@ int try_split(Ctx& c, int n, int nb, const ClusterPlan& plan, const int32_t* Sm,
   return ZKD_OK;
 }
 
-int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* lam, int depth, const int* noise, LevelStats* st) {
+int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* lam, int depth, const int* noise, LevelStats* st);
+
+// One level of the path.  allow_split = false leaves every cluster to the S5 recursion (slower on spectra like c4's, but it
+// has no heuristics to go wrong); *split_used tells the caller whether S4h took part in a failed attempt.
+int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* lam, int depth, const int* noise, LevelStats* st,
+                     bool allow_split, bool* split_used) {
   const Options& opt = options();
   const size_t cnt = (size_t)n * n * nb;
   const size_t fxc = FxC::bytes(cnt);
@@ -452,11 +457,13 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
     if (msb_r == 0) continue;  // residual exactly zero: only the orthonormalisation is still converging
 
     // S4h: split clusters whose internal structure stands above the noise of S_c
-    if (!singletons && opt.early_split && msb_g <= 812 - 45) {
+    if (split_done && step >= 48) return ZKD_ERR_INTERNAL;  // S4h is not getting anywhere: the caller retries without it
+    if (!singletons && allow_split && opt.early_split && msb_g <= 812 - 45) {
       bool changed = false;
       ZKD_TRY(try_split(c, n, nb, plan, Sm, msb_r, tol_msb, noise, Xc, Wc, Gm, R, scal, cl, cle, h_cl, &changed));
       if (changed) {
         split_done = true;
+        *split_used = true;
         ZKD_CUDA_TRY(cudaMemsetAsync(scal, 0, sizeof(int) * S_NUM, s));
         singletons = true;
         for (size_t t = 0; t < h_cl.size() && singletons; ++t) singletons = h_cl[t] == (int)(t % n);
@@ -553,6 +560,25 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
   }
   c.ar.release(mark0);
   return ZKD_OK;
+}
+
+// S4h (early cluster split) is a heuristic accelerator: when a level that used it fails (a window overflow, no convergence),
+// the level is redone from its seed with every cluster left to the S5 recursion.
+int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* lam, int depth, const int* noise, LevelStats* st) {
+  const Arena::Mark mark = c.ar.mark();
+  bool split_used = false;
+  LevelStats tmp;
+  int rc = solve_level_impl(c, n, nb, A, X, lam, depth, noise, st ? st : &tmp, true, &split_used);
+  const bool failed = rc == ZKD_ERR_INTERNAL || (rc == ZKD_OK && (st ? st->status : tmp.status) == 2);
+  if (failed && split_used) {
+    if (options().verbose) fprintf(stderr, "[zkd] depth %d n %d: retry without early splits\n", depth, n);
+    ZKD_CUDA_TRY(cudaStreamSynchronize(c.s));
+    c.ar.release(mark);
+    if (st) *st = LevelStats();
+    bool dummy = false;
+    rc = solve_level_impl(c, n, nb, A, X, lam, depth, noise, st ? st : &tmp, false, &dummy);
+  }
+  return rc;
 }
 
 __global__ void info_kernel(int batch, const int* __restrict__ status_in, int level_status, int steps, int msb_r, int msb_g,

@@ -181,6 +181,21 @@ def test_mixed_batch_different_cluster_tables(zkd):
         assert abs(g - w) <= Fraction(1, 2 ** 740), (float(g), float(w))
 
 
+@pytest.mark.parametrize("N,step", [(96, 11), (64, 3), (48, 30)])
+def test_geometric_cascade(zkd, N, step):
+    """Spectra +-2^-(1 + step i), i = 0 .. N-1 (zero once the exponent passes 760): every 2^-20 window of the cascade is a
+    cluster with internal structure, level after level.  Exercises repeated early splits, deep S5 recursion and the
+    retry-without-splits path; eigenvalues are known by construction."""
+    vals = sorted(Fraction((-1) ** i, 2 ** (1 + step * i)) if 1 + step * i < 760 else Fraction(0) for i in range(N))
+    A = zi.qdq(N, 31000 + step, 0, 3, zi._lam_array(vals))
+    lam, X, info = gpu_diag(zkd, A, N, 1)
+    assert info[0]["status"] == 0, info
+    c = oracle.compare(A, N, lam[0], X[0], cols=_sample_cols(N, 10, step))
+    assert c["log2_resid_rel"] <= TOL and c["log2_orth"] <= TOL, c
+    got = [zi.to_fraction(lam[0].reshape(N, -1)[j]) for j in range(N)]
+    assert all(abs(g - w) <= Fraction(1, 2 ** 740) for g, w in zip(got, vals))
+
+
 # ---- degenerate inputs (P9) ------------------------------------------------------------------------------------------
 
 def _api_matrix(N, fn):
