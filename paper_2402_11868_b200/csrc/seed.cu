@@ -519,9 +519,15 @@ __global__ void __launch_bounds__(128) seed_large_kernel(int n, const double2* _
 // (2 W n double2, <= 200 KB), rotates every cross pair (W sub-rounds of W disjoint pairs, one warp per pair; in round 0 of a
 // sweep also the pairs inside each block) and writes the blocks back.  Every pair of columns still meets once per sweep, but
 // there are (n / W - 1) rounds (grid syncs, passes over G in L2) per sweep instead of (n - 1).
-__device__ __forceinline__ double rotate_pair_smem(double2* __restrict__ gp, double2* __restrict__ gq, int n, int lane, double tol2) {
+// WPP warps per pair: warp `part` of the pair owns the rows [part * chunk, (part + 1) * chunk); the four partial sums meet in
+// shared memory (s_red: [4 * WPP] doubles of this pair).  Contains one __syncthreads when WPP > 1: every warp of the CTA calls it.
+template <int WPP>
+__device__ __forceinline__ double rotate_pair_smem(double2* __restrict__ gp, double2* __restrict__ gq, int n, int lane, int part,
+                                                   double* __restrict__ s_red, double tol2) {
+  const int chunk = (n + WPP - 1) / WPP;
+  const int i0 = part * chunk, i1 = min(n, i0 + chunk);
   double al = 0, be = 0, gr = 0, gi = 0;
-  for (int i = lane; i < n; i += 32) {
+  for (int i = i0 + lane; i < i1; i += 32) {
     const double2 a = gp[i], b = gq[i];
     al = fma(a.x, a.x, fma(a.y, a.y, al));
     be = fma(b.x, b.x, fma(b.y, b.y, be));
@@ -529,9 +535,16 @@ __device__ __forceinline__ double rotate_pair_smem(double2* __restrict__ gp, dou
     gi = fma(a.x, b.y, fma(-a.y, b.x, gi));
   }
   al = warp_sum(al); be = warp_sum(be); gr = warp_sum(gr); gi = warp_sum(gi);
+  if (WPP > 1) {
+    if (lane == 0) { s_red[4 * part + 0] = al; s_red[4 * part + 1] = be; s_red[4 * part + 2] = gr; s_red[4 * part + 3] = gi; }
+    __syncthreads();
+    al = be = gr = gi = 0;
+#pragma unroll
+    for (int p = 0; p < WPP; ++p) { al += s_red[4 * p + 0]; be += s_red[4 * p + 1]; gr += s_red[4 * p + 2]; gi += s_red[4 * p + 3]; }
+  }
   double c, sr, si, cos2;
   if (!rot_params(al, be, gr, gi, tol2, c, sr, si, cos2)) return cos2;
-  for (int i = lane; i < n; i += 32) {
+  for (int i = i0 + lane; i < i1; i += 32) {
     const double2 a = gp[i], b = gq[i];
     gp[i] = make_double2(c * a.x - (sr * b.x + si * b.y), c * a.y - (sr * b.y - si * b.x));
     gq[i] = make_double2(sr * a.x - si * a.y + c * b.x, sr * a.y + si * a.x + c * b.y);
@@ -544,8 +557,11 @@ __global__ void __launch_bounds__(256) seed_block_kernel(int n, const double2* _
                                                          const double* __restrict__ sigma_p, int* __restrict__ rot_flags,
                                                          double* __restrict__ mu_unsorted, int max_sweeps, double tol2) {
   extern __shared__ double2 s_cols[];  // [2 W][n]
+  constexpr int WPP = 8 / W;           // warps per pair: all 8 warps of the CTA rotate in every sub-round
+  __shared__ double s_red[W][4 * WPP];
   cg::grid_group grid = cg::this_grid();
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int pr = warp % W, part = warp / W;
   const int gwarp = (blockIdx.x * blockDim.x + tid) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
   const size_t gtid = (size_t)blockIdx.x * blockDim.x + tid, gthr = (size_t)gridDim.x * blockDim.x;
   const double sigma = *sigma_p;
@@ -581,20 +597,17 @@ __global__ void __launch_bounds__(256) seed_block_kernel(int n, const double2* _
           if (r == 0 && W > 1) {
             // pairs inside each block, once per sweep: round-robin over W columns, both blocks at once
             for (int t = 0; t < W - 1; ++t) {
-              if (warp < W) {
-                const int blk = warp / (W / 2), i = warp % (W / 2);
-                int p, q;
-                rr_pair(W, t, i, p, q);
-                cmax = fmax(cmax, rotate_pair_smem(s_cols + (size_t)(blk * W + p) * n, s_cols + (size_t)(blk * W + q) * n, n, lane, tol2));
-              }
+              const int blk = pr / (W / 2), i = pr % (W / 2);
+              int p, q;
+              rr_pair(W, t, i, p, q);
+              cmax = fmax(cmax, rotate_pair_smem<WPP>(s_cols + (size_t)(blk * W + p) * n, s_cols + (size_t)(blk * W + q) * n, n, lane,
+                                                      part, s_red[pr], tol2));
               __syncthreads();
             }
           }
           for (int t = 0; t < W; ++t) {
-            if (warp < W) {
-              const int p = warp, q = W + (warp + t) % W;
-              cmax = fmax(cmax, rotate_pair_smem(s_cols + (size_t)p * n, s_cols + (size_t)q * n, n, lane, tol2));
-            }
+            const int p = pr, q = W + (pr + t) % W;
+            cmax = fmax(cmax, rotate_pair_smem<WPP>(s_cols + (size_t)p * n, s_cols + (size_t)q * n, n, lane, part, s_red[pr], tol2));
             __syncthreads();
           }
           for (int c = 0; c < 2 * W; ++c) {
@@ -627,7 +640,7 @@ static int launch_block(int n, int sms, const double2* Ab, double2* G, double* s
   const size_t smem = sizeof(double2) * 2 * W * (size_t)n;
   static bool attr_done = false;
   if (!attr_done) {
-    if (cudaFuncSetAttribute(seed_block_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) {
+    if (cudaFuncSetAttribute(seed_block_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess) {
       (void)cudaGetLastError();
       return ZKD_ERR_CUDA;
     }
