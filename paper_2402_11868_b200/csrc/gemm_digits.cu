@@ -315,6 +315,178 @@ __global__ void __launch_bounds__(256) combine_kernel(CombineArgs a) {
     for (int kk = 0; kk < q && kk < kND; ++kk) dst[(size_t)kk * tot_d] = 0;
 }
 
+// Warp-cooperative combine: one warp per (8 consecutive elements, part).  Lane k owns FX digit k of those elements (lanes
+// 0..29), lane 30 the raw columns that lie below digit 0 (only their carry matters).  All raw columns of an element are
+// fetched in one round trip (each lane reads 8 consecutive words = one sector per column and split), and the carries are
+// resolved by parallel relaxation: every lane hands the overflow of its digit to the lane above until no lane overflows
+// (3 - 5 rounds; a full ripple is 30).  The canonical digits of an integer are unique, so the result is bit-identical to
+// the digit-serial kernel above.
+constexpr int EPW = 8;
+
+__device__ __forceinline__ void relax_digits(int64_t (&lo)[EPW], int64_t (&hi)[EPW], int lane) {
+  for (;;) {
+    bool pending = false;
+#pragma unroll
+    for (int u = 0; u < EPW; ++u) {
+      int64_t inc = __shfl_up_sync(0xffffffffu, hi[u], 1);
+      if (lane == 0 || lane > kND - 1) inc = 0;
+      const int64_t t = lo[u] + inc;
+      if (lane < kND - 1) {
+        hi[u] = t >> DB;
+        lo[u] = t & DMASK;
+      } else {
+        hi[u] = 0;   // the top digit keeps the (signed) rest; lanes 30, 31 hold nothing
+        lo[u] = t;
+      }
+      pending |= hi[u] != 0;
+    }
+    if (!__any_sync(0xffffffffu, pending)) break;
+  }
+}
+
+__global__ void __launch_bounds__(256) combine_warp_kernel(CombineArgs a) {
+  const int lane = threadIdx.x & 31;
+  const size_t w = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int part = blockIdx.y;
+  const size_t gpb = (a.mn + EPW - 1) / EPW;  // groups per batch element
+  if (w >= gpb * a.batch) return;             // the whole warp leaves together
+  const int b = (int)(w / gpb);
+  const size_t ij0 = (w % gpb) * EPW;
+  const int nvalid = (int)(a.mn - ij0 < (size_t)EPW ? a.mn - ij0 : (size_t)EPW);
+  const int G = 3 * a.batch;
+  const size_t gstride = (size_t)a.nc * a.mn;
+  const size_t sstride = (size_t)G * gstride;
+  const int32_t* __restrict__ r1 = a.raw + (size_t)(b * 3 + 0) * gstride + ij0;
+  const int32_t* __restrict__ r2 = a.raw + (size_t)(b * 3 + (part == 0 ? 2 : 1)) * gstride + ij0;
+  const int sgn2 = part == 0 ? -1 : 1;
+  const int q = a.base_bit >= 0 ? a.base_bit / DB : -((-a.base_bit + DB - 1) / DB);
+  const int sh = a.base_bit - q * DB;  // 0..27
+  const int k = lane;                  // FX digit of this lane (lanes 0..29)
+  const size_t tot_d = a.plane_count;
+
+  // destination addresses of the 8 elements (views: rows of ld words)
+  size_t daddr[EPW];
+#pragma unroll
+  for (int u = 0; u < EPW; ++u) {
+    const size_t ij = ij0 + (u < nvalid ? u : 0);
+    daddr[u] = (part ? (size_t)kND * tot_d : 0) + (a.off ? (size_t)a.off[b] : (size_t)b * a.mn) + (ij / a.N) * a.ld + (ij % a.N);
+  }
+  int32_t old[EPW];
+#pragma unroll
+  for (int u = 0; u < EPW; ++u) old[u] = 0;
+  if (a.mode != 0 && k < kND) {
+#pragma unroll
+    for (int u = 0; u < EPW; ++u)
+      if (u < nvalid) old[u] = a.dst[daddr[u] + (size_t)k * tot_d];
+  }
+
+  // column sums of this lane's digit
+  int64_t v[EPW];
+#pragma unroll
+  for (int u = 0; u < EPW; ++u) v[u] = 0;
+  auto add_col = [&](int c, int shift) {
+    for (int s = 0; s < a.nsplit; ++s) {
+      int32_t l1[EPW], l2[EPW];
+#pragma unroll
+      for (int u = 0; u < EPW; ++u) {
+        const bool in = u < nvalid;
+        l1[u] = in ? r1[(size_t)s * sstride + (size_t)c * a.mn + u] : 0;
+        l2[u] = in ? r2[(size_t)s * sstride + (size_t)c * a.mn + u] : 0;
+      }
+#pragma unroll
+      for (int u = 0; u < EPW; ++u) v[u] += ((int64_t)l1[u] + sgn2 * (int64_t)l2[u]) << shift;
+    }
+  };
+  if (k < kND) {
+    const int c = k - q;
+    if (c >= 0 && c < a.nc) add_col(c, sh);
+    // everything that is left lands in the signed top digit (higher raw columns are sign extension unless the result
+    // overflows FX, which the callers' magnitude bounds exclude)
+    if (k == kND - 1 && c >= 0 && c + 1 < a.nc) add_col(c + 1, sh + DB);
+  } else if (k == kND) {
+    // raw columns below digit 0: serial carry chain (a handful of columns), delivered to digit 0
+    const int nlow = -q < a.nc ? -q : a.nc;
+    int64_t cy[EPW];
+#pragma unroll
+    for (int u = 0; u < EPW; ++u) cy[u] = 0;
+    for (int c = 0; c < nlow; ++c) {
+#pragma unroll
+      for (int u = 0; u < EPW; ++u) v[u] = 0;
+      add_col(c, sh);
+#pragma unroll
+      for (int u = 0; u < EPW; ++u) cy[u] = (cy[u] + v[u]) >> DB;
+    }
+    // digits between the last low column and digit 0 only pass the carry on: cy >> 28 per skipped digit
+    for (int kk = q + nlow; kk < 0; ++kk) {
+#pragma unroll
+      for (int u = 0; u < EPW; ++u) cy[u] >>= DB;
+    }
+#pragma unroll
+    for (int u = 0; u < EPW; ++u) v[u] = cy[u];
+  }
+  // carry of the low columns into digit 0
+#pragma unroll
+  for (int u = 0; u < EPW; ++u) {
+    const int64_t cin = __shfl_sync(0xffffffffu, v[u], kND);
+    if (k == 0) v[u] += cin;
+    if (k >= kND) v[u] = 0;
+  }
+  int64_t lo[EPW], hi[EPW];
+#pragma unroll
+  for (int u = 0; u < EPW; ++u) {
+    if (k < kND - 1) { lo[u] = v[u] & DMASK; hi[u] = v[u] >> DB; }
+    else { lo[u] = v[u]; hi[u] = 0; }
+  }
+  relax_digits(lo, hi, lane);
+
+  // cut, accumulate
+  const int cutq = a.cut_bit > 0 ? a.cut_bit / DB : 0, cutr = a.cut_bit > 0 ? a.cut_bit % DB : 0;
+  int32_t outd[EPW];
+#pragma unroll
+  for (int u = 0; u < EPW; ++u) {
+    int32_t digit = (int32_t)lo[u];
+    if (k < cutq) digit = 0;
+    else if (k == cutq && cutr) digit &= ~((1 << cutr) - 1);
+    outd[u] = digit;
+  }
+  if (a.mode != 0) {
+#pragma unroll
+    for (int u = 0; u < EPW; ++u) {
+      const int64_t t = (int64_t)old[u] + (a.mode == 1 ? (int64_t)outd[u] : -(int64_t)outd[u]);
+      if (k < kND - 1) { lo[u] = t & DMASK; hi[u] = t >> DB; }
+      else { lo[u] = (k == kND - 1) ? t : 0; hi[u] = 0; }
+    }
+    relax_digits(lo, hi, lane);
+#pragma unroll
+    for (int u = 0; u < EPW; ++u) outd[u] = (int32_t)lo[u];
+  }
+  // store (accumulate modes leave the digits below the product's lowest one untouched: they cannot change)
+  if (k < kND && (a.mode == 0 || k >= q)) {
+#pragma unroll
+    for (int u = 0; u < EPW; ++u)
+      if (u < nvalid) a.dst[daddr[u] + (size_t)k * tot_d] = outd[u];
+  }
+  // msb of the stored values
+  if (a.msb_out) {
+    int best = 0;
+#pragma unroll
+    for (int u = 0; u < EPW; ++u) {
+      const int32_t top = __shfl_sync(0xffffffffu, outd[u], kND - 1);
+      int cand = 0;
+      if (k < kND - 1) {
+        if (top < 0) { if (outd[u] != DMASK) cand = k * DB + (32 - __clz((~outd[u]) & DMASK)); }
+        else if (outd[u] != 0) cand = k * DB + (32 - __clz(outd[u]));
+      } else if (k == kND - 1) {
+        if (outd[u] > 0) cand = k * DB + (32 - __clz(outd[u]));
+        if (outd[u] < -1) cand = k * DB + (32 - __clz(~outd[u]));
+      }
+      if (u < nvalid && cand > best) best = cand;
+    }
+    for (int o = 16; o > 0; o >>= 1) best = max(best, __shfl_xor_sync(0xffffffffu, best, o));
+    if (lane == 0 && best) atomicMax(a.msb_out, best);
+  }
+}
+
 // ---- host side ----------------------------------------------------------------------------------------------------
 
 // Optional per-launch timing of the digit GEMM kernel (zkd_kernel_timing): event pairs on the launching stream.
@@ -466,7 +638,13 @@ int gemm_complex(int M, int N, int K, int batch, const GemmSide& P, const GemmSi
   ca.cut_bit = out_cut_bit; ca.mode = (int)mode; ca.msb_out = msb_out;
   const size_t tot = (size_t)batch * M * N;
   const dim3 cgrid((unsigned)((tot + 255) / 256), 2);
-  if (nsp == 1) combine_kernel<1><<<cgrid, 256, 0, stream>>>(ca);
+  // the warp-cooperative kernel wins only while the digit-serial one cannot fill the machine (measured: c2 2.47 -> 2.40 ms,
+  // but c4 244 -> 316 ms when forced)
+  const int cpath = options().combine_path;
+  if (cpath == 2 || (cpath == 0 && tot <= 32768)) {
+    const size_t warps = ((size_t)M * N + EPW - 1) / EPW * batch;
+    combine_warp_kernel<<<dim3((unsigned)((warps * 32 + 255) / 256), 2), 256, 0, stream>>>(ca);
+  } else if (nsp == 1) combine_kernel<1><<<cgrid, 256, 0, stream>>>(ca);
   else if (nsp == 2) combine_kernel<2><<<cgrid, 256, 0, stream>>>(ca);
   else if (nsp <= 4) combine_kernel<4><<<cgrid, 256, 0, stream>>>(ca);
   else combine_kernel<0><<<cgrid, 256, 0, stream>>>(ca);

@@ -114,6 +114,17 @@ def test_gemm_fx_int8_tcgen05_matches_python_integers(zkd, case):
 
 
 @pytest.mark.parametrize("case", GEMM_CASES)
+@pytest.mark.parametrize("combine", [1, 2])
+def test_gemm_fx_epilogues_match_python_integers(zkd, case, combine):
+    """both epilogues of the IMAD engine (digit-serial and warp-cooperative carry resolution) are bit-identical"""
+    zkd.set_option("combine_path", combine)
+    try:
+        test_gemm_fx_matches_python_integers(zkd, case, path=1)
+    finally:
+        zkd.set_option("combine_path", 0)
+
+
+@pytest.mark.parametrize("case", GEMM_CASES)
 def test_gemm_fx_matches_python_integers(zkd, case, path=1):
     import torch
 
