@@ -323,24 +323,48 @@ __global__ void __launch_bounds__(256) combine_kernel(CombineArgs a) {
 // the digit-serial kernel above.
 constexpr int EPW = 8;
 
+// lo: this lane's digit value (any int64), hi: what it owes the lane above (0 on entry is fine).  Two relaxation rounds bring
+// every debt down to {-1, 0, +1} (|v| < 2^63 -> |hi| < 2^35 -> < 2^8 -> <= 1); the remaining unit carries and borrows may
+// ripple through runs of 2^28-1 / 0 digits (a small negative result borrows through ALL its higher digits), so they are
+// resolved by carry look-ahead on warp ballots instead of 30 more rounds: with G = lanes that emit a unit and P = lanes that
+// would pass one on, the lanes that receive one are ((P + (G << 1)) ^ P ^ (G << 1)) | (G << 1).
 __device__ __forceinline__ void relax_digits(int64_t (&lo)[EPW], int64_t (&hi)[EPW], int lane) {
-  for (;;) {
-    bool pending = false;
+  const bool low = lane < kND - 1;        // digits 0..28 are reduced mod 2^28
+  const bool top = lane == kND - 1;       // digit 29 keeps the signed rest
+  constexpr unsigned kLowMask = (1u << (kND - 1)) - 1;
+#pragma unroll
+  for (int round = 0; round < 2; ++round) {
 #pragma unroll
     for (int u = 0; u < EPW; ++u) {
       int64_t inc = __shfl_up_sync(0xffffffffu, hi[u], 1);
       if (lane == 0 || lane > kND - 1) inc = 0;
       const int64_t t = lo[u] + inc;
-      if (lane < kND - 1) {
-        hi[u] = t >> DB;
-        lo[u] = t & DMASK;
-      } else {
-        hi[u] = 0;   // the top digit keeps the (signed) rest; lanes 30, 31 hold nothing
-        lo[u] = t;
-      }
-      pending |= hi[u] != 0;
+      if (low) { hi[u] = t >> DB; lo[u] = t & DMASK; }
+      else { hi[u] = 0; lo[u] = t; }
     }
-    if (!__any_sync(0xffffffffu, pending)) break;
+  }
+#pragma unroll
+  for (int u = 0; u < EPW; ++u) {
+    int64_t inc = __shfl_up_sync(0xffffffffu, hi[u], 1);  // -1, 0 or +1
+    if (lane == 0 || lane > kND - 1) inc = 0;
+    int64_t t = lo[u] + inc;
+    bool gp = false, gm = false;
+    if (low) {
+      if (t == (int64_t)DMASK + 1) { t = 0; gp = true; }
+      else if (t < 0) { t = DMASK; gm = true; }
+    }
+    // carries
+    unsigned G = __ballot_sync(0xffffffffu, gp) & kLowMask;
+    unsigned P = __ballot_sync(0xffffffffu, low && t == DMASK) & kLowMask;
+    unsigned C = (((P + (G << 1)) ^ P ^ (G << 1)) | (G << 1));
+    if ((C >> lane) & 1) t = low ? ((t + 1) & DMASK) : (top ? t + 1 : t);
+    // borrows
+    G = __ballot_sync(0xffffffffu, gm) & kLowMask;
+    P = __ballot_sync(0xffffffffu, low && t == 0) & kLowMask;
+    C = (((P + (G << 1)) ^ P ^ (G << 1)) | (G << 1));
+    if ((C >> lane) & 1) t = low ? ((t - 1) & DMASK) : (top ? t - 1 : t);
+    lo[u] = t;
+    hi[u] = 0;
   }
 }
 
