@@ -5,6 +5,7 @@
 // Complex product by 3 real products (3M):  with P = pr + i pi and Q = qr + i qi,
 //     k1 = (pr + pi) qr,  k2 = pr (qi - qr),  k3 = pi (qr + qi);   Re = k1 - k3,  Im = k1 + k2.
 // In fixed point the operand sums are exact, so 3M costs nothing in accuracy.
+#include <cstdio>
 #include <vector>
 
 #include "gemm_digits.cuh"
@@ -347,19 +348,24 @@ __device__ __forceinline__ void relax_digits(int64_t (&lo)[EPW], int64_t (&hi)[E
   for (int u = 0; u < EPW; ++u) {
     int64_t inc = __shfl_up_sync(0xffffffffu, hi[u], 1);  // -1, 0 or +1
     if (lane == 0 || lane > kND - 1) inc = 0;
-    int64_t t = lo[u] + inc;
-    bool gp = false, gm = false;
-    if (low) {
-      if (t == (int64_t)DMASK + 1) { t = 0; gp = true; }
-      else if (t < 0) { t = DMASK; gm = true; }
+    int64_t t = lo[u];
+    // First all the +1 units, then all the -1 units: within one sign a lane that emits a unit (it wrapped to 0, resp. to
+    // 2^28-1) can never also pass one on, so every lane receives at most one unit per phase - which is all a bit mask can say.
+    bool gen = false;
+    if (inc == 1) {
+      t += 1;
+      if (low && t == (int64_t)DMASK + 1) { t = 0; gen = true; }
     }
-    // carries
-    unsigned G = __ballot_sync(0xffffffffu, gp) & kLowMask;
+    unsigned G = __ballot_sync(0xffffffffu, gen) & kLowMask;
     unsigned P = __ballot_sync(0xffffffffu, low && t == DMASK) & kLowMask;
     unsigned C = (((P + (G << 1)) ^ P ^ (G << 1)) | (G << 1));
     if ((C >> lane) & 1) t = low ? ((t + 1) & DMASK) : (top ? t + 1 : t);
-    // borrows
-    G = __ballot_sync(0xffffffffu, gm) & kLowMask;
+    gen = false;
+    if (inc == -1) {
+      t -= 1;
+      if (low && t < 0) { t = DMASK; gen = true; }
+    }
+    G = __ballot_sync(0xffffffffu, gen) & kLowMask;
     P = __ballot_sync(0xffffffffu, low && t == 0) & kLowMask;
     C = (((P + (G << 1)) ^ P ^ (G << 1)) | (G << 1));
     if ((C >> lane) & 1) t = low ? ((t - 1) & DMASK) : (top ? t - 1 : t);

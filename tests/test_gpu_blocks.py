@@ -190,6 +190,62 @@ def test_gemm_fx_matches_python_integers(zkd, case, path=1):
     assert maxmag.bit_length() - 1 <= int(msb.item()) <= maxmag.bit_length() + 1
 
 
+@pytest.mark.parametrize("combine", [1, 2])
+@pytest.mark.parametrize("mode", [0, 1, 2])
+def test_gemm_fx_near_identity_carry_chains(zkd, combine, mode):
+    """Products of near-identity matrices (G = X^H X, X (I + M)): results like 1 - 2^-300 or -2^-500, whose canonical digits
+    are long runs of 2^28-1 and 0 with carries and borrows meeting in them - the case that random operands never produce
+    (a look-ahead bug of the warp-cooperative epilogue passed every random test and was caught by a soak of the pipeline)."""
+    import torch
+
+    M = N = K = 13
+    batch = 2
+    rng = random.Random(1234 + mode)
+    one = 1 << FRAC
+
+    def near_identity():
+        re, im = [], []
+        for b in range(batch):
+            for i in range(M):
+                for j in range(M):
+                    e = rng.choice([1, -1]) * (1 << rng.randint(0, 780)) if rng.random() < 0.8 else 0
+                    f = rng.choice([1, -1]) * (1 << rng.randint(0, 780)) if rng.random() < 0.5 else 0
+                    re.append((one if i == j else 0) + e)
+                    im.append(f if i != j else 0)
+        return re, im
+
+    Are, Aim = near_identity()
+    Bre, Bim = near_identity()
+    C0re = [(one if (e % (M * N)) // N == e % N else 0) - rng.getrandbits(rng.randint(1, 700)) for e in range(batch * M * N)]
+    C0im = [rng.choice([1, -1]) * (1 << rng.randint(0, 700)) for _ in range(batch * M * N)]
+    dA, dB, dC = _dev(fxc_from_ints(Are, Aim)), _dev(fxc_from_ints(Bre, Bim)), _dev(fxc_from_ints(C0re, C0im))
+    err = torch.zeros(1, dtype=torch.int32, device="cuda")
+    zkd.set_option("combine_path", combine)
+    try:
+        zkd.gemm_fx(M, N, K, batch, 1, dA, 815, 30, dB, 815, 30, dC, mode, -1, 1, None, err, None)
+        torch.cuda.synchronize()
+    finally:
+        zkd.set_option("combine_path", 0)
+    assert int(err.item()) == 0
+    gre, gim = ints_from_fxc(dC.cpu().numpy())
+    worst = 0
+    for b in range(batch):
+        for i in range(M):
+            for j in range(N):
+                sre = sim = 0
+                for k in range(K):
+                    ia, ib = b * M * K + k * M + i, b * K * N + k * N + j
+                    are, aim = Are[ia], -Aim[ia]  # op_a = 1: conjugate transpose
+                    sre += are * Bre[ib] - aim * Bim[ib]
+                    sim += are * Bim[ib] + aim * Bre[ib]
+                e = b * M * N + i * N + j
+                for s_, g, c0 in ((sre, gre[e], C0re[e]), (sim, gim[e], C0im[e])):
+                    p_ = s_ >> FRAC
+                    want = p_ if mode == 0 else (c0 + p_ if mode == 1 else c0 - p_)
+                    worst = max(worst, abs(g - want))
+    assert worst <= 2 + (1 << max(0, -25 + 815 - 837 + 4)), worst
+
+
 def test_gemm_fx_flags_window_overflow(zkd):
     import torch
 
