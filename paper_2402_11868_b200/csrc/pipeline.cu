@@ -360,7 +360,7 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
   const size_t fxc = FxC::bytes(cnt);
   const Arena::Mark mark0 = c.ar.mark();
   cudaStream_t s = c.s;
-  if (depth > 48) return ZKD_ERR_INTERNAL;
+  if (depth > 512) return ZKD_ERR_INTERNAL;  // every level strictly shrinks its clusters; a cascade peeled one eigenvalue per level is slow, not wrong
 
   // long-lived (needed by S5)
   int* cl = c.ar.get<int>((size_t)n * nb);
