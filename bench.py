@@ -349,6 +349,7 @@ def main():
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": total_ms_max / args.steps, "ms_per_step_std": statistics.pstdev(times) if len(times) > 1 else 0.0,
+        "ms_per_step_all": [round(t, 4) for t in times],
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32x30 (28-bit digits, 840-bit fixed point)",
         "data": "synthetic",
         "config": {"workload": WORKLOADS[args.workload], "N": N, "batch": b, "prec_bits": 768, "parallelism": "replicas only",

@@ -733,7 +733,21 @@ int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int ma
   char* buf = nullptr;
   const size_t nn = (size_t)N * N;
   const size_t bytes = sizeof(double2) * nn + sizeof(double) * (N + 8) + sizeof(int) * 64;
-  ZKD_CUDA_TRY(cudaMallocAsync((void**)&buf, bytes, s));
+  // grow-only scratch of the calling thread (N^2 double2: 16 MB at N = 1024): a stream-ordered allocation here costs a pool
+  // re-growth after every synchronisation of the caller (the default pool trims at sync points)
+  {
+    static thread_local char* cached = nullptr;
+    static thread_local size_t cached_bytes = 0;
+    if (cached_bytes < bytes) {
+      ZKD_CUDA_TRY(cudaStreamSynchronize(s));
+      if (cached) cudaFree(cached);
+      cached = nullptr;
+      cached_bytes = 0;
+      ZKD_CUDA_TRY(cudaMalloc((void**)&cached, bytes));
+      cached_bytes = bytes;
+    }
+    buf = cached;
+  }
   double2* G = (double2*)buf;
   double* sigma = (double*)(G + nn);
   double* mu_uns = sigma + 8;
@@ -764,7 +778,6 @@ int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int ma
     count_launch(3);
     rc = launch_check();
   }
-  cudaFreeAsync(buf, s);
   return rc;
 }
 
