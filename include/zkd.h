@@ -81,10 +81,16 @@ int zkd_diag_herm_host(int N, int batch, int prec_bits, const void *A_host, void
                        zkd_info *info_host);
 
 /* Tunables (process-wide; call before zkd_diag_herm*).  Keys: "tau_bits" (cluster threshold 2^-tau ||A||_F,
- * default 20), "tol_bits" (stop when max|R_ij| <= 2^-tol, default 770), "max_steps" (default 40),
+ * default 20), "tol_bits" (stop when max|R_ij| <= 2^-tol, default 770), "max_steps" (default 120),
  * "gemm_path" (engine of the digit GEMM: 0 = automatic [default]: limb-sliced int8 tcgen05 MMAs when M, N, K >= 128,
  * the IMAD kernel otherwise; 1 = IMAD only; 2 = int8 tcgen05 wherever its tiles can be formed),
- * "min_split_ctas" (split-K target, default 296).  Returns ZKD_ERR_INVALID_ARG for an unknown key. */
+ * "min_split_ctas" (split-K target, default 296), "early_split" (S4h: split clusters whose internal structure stands
+ * above the noise of the projected matrix; default 1; 0 leaves every cluster to the S5 recursion),
+ * "split_margin_bits" (that margin, default 40), "seed_sweeps" (cap on the fp64 Jacobi sweeps, default 12),
+ * "seed_path" / "seed_cluster" (seed kernel selection), "combine_path" (epilogue of the IMAD GEMM: 0 automatic,
+ * 1 digit-serial, 2 warp-cooperative), "sstep_cpb" (matrix columns per CTA of the fused singleton step, 0 automatic),
+ * "verbose" (1: one line per refinement pass on stderr).  All routes give the same results to the stated tolerances;
+ * the defaults are the measured-fastest ones.  Returns ZKD_ERR_INVALID_ARG for an unknown key. */
 int zkd_set_option(const char *key, double value);
 int zkd_get_option(const char *key, double *value);
 
