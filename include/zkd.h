@@ -84,7 +84,7 @@ int zkd_diag_herm_host(int N, int batch, int prec_bits, const void *A_host, void
  * default 20), "tol_bits" (stop when max|R_ij| <= 2^-tol, default 770), "max_steps" (default 120),
  * "gemm_path" (engine of the digit GEMM: 0 = automatic [default]: limb-sliced int8 tcgen05 MMAs when M, N, K >= 128,
  * the IMAD kernel otherwise; 1 = IMAD only; 2 = int8 tcgen05 wherever its tiles can be formed),
- * "min_split_ctas" (split-K target, default 296), "early_split" (S4h: split clusters whose internal structure stands
+ * "min_split_ctas" (split-K target, default 296; every split keeps at least 32 of K), "early_split" (S4h: split clusters whose internal structure stands
  * above the noise of the projected matrix; default 1; 0 leaves every cluster to the S5 recursion),
  * "split_margin_bits" (that margin, default 40), "seed_sweeps" (cap on the fp64 Jacobi sweeps, default 12),
  * "seed_path" / "seed_cluster" (seed kernel selection), "combine_path" (epilogue of the IMAD GEMM: 0 automatic,

@@ -576,11 +576,14 @@ static void kt_end(cudaStream_t s, uint64_t macs) {
 static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 static int pick_splits(int M, int N, int K, int batch) {
+  // Split K until the product has about min_split_ctas CTAs, but leave every split at least two 16-deep K tiles: a CTA
+  // that does a single tile is all prologue and epilogue, and every split adds a raw plane for the epilogue to sum
+  // (measured: N = 64, K = 64: 2 splits 2.27 ms per matrix, 4 splits 2.37, none 2.46; K = 1024 wants its splits).
   const long tiles = (long)((M + GT - 1) / GT) * ((N + GT - 1) / GT) * 3 * batch;
   const int want = options().min_split_ctas;
   if (tiles >= want) return 1;
   int s = (int)((want + tiles - 1) / tiles);
-  const int kmax = (K + GT - 1) / GT;
+  const int kmax = ((K + GT - 1) / GT) / 2;
   if (s > kmax) s = kmax;
   if (s > 32) s = 32;
   return s < 1 ? 1 : s;

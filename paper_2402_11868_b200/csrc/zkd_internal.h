@@ -42,7 +42,7 @@ struct Options {
   int tol_bits = 770;
   int max_steps = 120;
   int gemm_path = 0;
-  int min_split_ctas = 296;
+  int min_split_ctas = 296;  // split K until a product has about this many CTAs (two per SM), see pick_splits
   int seed_sweeps = 12;
   int seed_cluster = 0;  // ring seed: largest cluster size to use (0 = 16, falling back to 8 when refused)
   int seed_path = 0;     // 0: auto; 2: always the ring kernel for N <= 256; 3: unblocked cooperative kernel for N > 256
