@@ -148,6 +148,7 @@ static int* option_slot(const char* key) {
   if (!strcmp(key, "early_split")) return &o.early_split;
   if (!strcmp(key, "split_margin_bits")) return &o.split_margin_bits;
   if (!strcmp(key, "sstep_cpb")) return &o.sstep_cpb;
+  if (!strcmp(key, "sstep_cache")) return &o.sstep_cache;
   if (!strcmp(key, "combine_path")) return &o.combine_path;
   if (!strcmp(key, "verbose")) return &o.verbose;
   return nullptr;

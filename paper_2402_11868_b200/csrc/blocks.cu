@@ -329,7 +329,10 @@ __device__ __forceinline__ void block_sum_cols(int64_t (&acc)[NACC2], int64_t* s
 
 // CPB matrix columns per CTA: a warp reads CPB consecutive columns of 32 / CPB rows, i.e. CPB * 4 contiguous bytes per row
 // (row-major X: a single column per CTA touches one 32-byte sector per element and digit).
-template <int CPB>
+// CACHE (CPB = 1, small n): the column's x and w digits (4 planes x 30 digits x n words) are staged in shared memory once;
+// the five phases then read and update them there, and x, w go back to global memory at the end - instead of ~26
+// dependent round trips to L2 per element.
+template <int CPB, bool CACHE>
 __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int32_t* __restrict__ X, int32_t* __restrict__ W,
                                                              int32_t* __restrict__ R, int32_t* __restrict__ S,
                                                              int32_t* __restrict__ theta, int* __restrict__ msb_g_out,
@@ -337,6 +340,7 @@ __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int3
                                                              const int* __restrict__ cle) {
   __shared__ int64_t s_part[8 * CPB * FXP_NACC];
   __shared__ int s_msb;
+  extern __shared__ int32_t s_cache[];  // CACHE: [4][ND][n]
   const int groups = (n + CPB - 1) / CPB;
   const int b = blockIdx.x / groups;
   const int tid = threadIdx.x, nwarps = blockDim.x >> 5, tx = tid % CPB, ty = tid / CPB, rows = blockDim.x / CPB;
@@ -344,10 +348,25 @@ __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int3
   // mixed levels: columns of larger clusters take the GEMM path
   const bool act = j < n && !(cl && cle[(size_t)b * n + j] - cl[(size_t)b * n + j] > 1);
   const size_t per = (size_t)n * n, count = per * nb;
-  int32_t* Xr = X;  int32_t* Xi = X + (size_t)ND * count;
-  int32_t* Wr = W;  int32_t* Wi = W + (size_t)ND * count;
+  int32_t* const gplane[4] = {X, X + (size_t)ND * count, W, W + (size_t)ND * count};  // xr, xi, wr, wi
   int32_t* Rr = R;  int32_t* Ri = R + (size_t)ND * count;
+  // plane pl of row k: base pointer, digit stride and index, in shared or global memory
+  const size_t stride = CACHE ? (size_t)n : count;
+  auto base = [&](int pl) -> int32_t* { return CACHE ? s_cache + (size_t)pl * ND * n : gplane[pl]; };
+  auto idx = [&](int k) -> size_t { return CACHE ? (size_t)k : (size_t)b * per + (size_t)k * n + j; };
   if (tid == 0) s_msb = 0;
+  if (CACHE && act) {
+    for (int k = ty; k < n; k += rows) {
+      const size_t e = (size_t)b * per + (size_t)k * n + j;
+#pragma unroll 1
+      for (int pl = 0; pl < 4; ++pl) {
+        int32_t a[ND];
+        fx_load(a, gplane[pl], count, e);
+        fx_store(s_cache + (size_t)pl * ND * n, (size_t)n, (size_t)k, a);
+      }
+    }
+  }
+  // (a thread only ever touches the cache entries of its own rows: no barrier needed for the cache itself)
 
   // g = sum_k |x_kj|^2
   int64_t acc[FXP_NACC];
@@ -356,11 +375,10 @@ __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int3
   // selection: the unrolled 30 x 30 digit product is ~500 IMAD.WIDE, and 14 copies of it thrashed the instruction cache)
   if (act) {
     for (int k = ty; k < n; k += rows) {
-      const size_t e = (size_t)b * per + (size_t)k * n + j;
 #pragma unroll 1
       for (int pl = 0; pl < 2; ++pl) {
         int32_t a[ND];
-        fx_load(a, pl ? Xi : Xr, count, e);
+        fx_load(a, base(pl), stride, idx(k));
         fx_mac<false>(acc, a, a);
       }
       fxp_relax(acc);
@@ -381,16 +399,15 @@ __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int3
   if (act) {
 #pragma unroll 1
     for (int pl = 0; pl < 4; ++pl) {
-      int32_t* P = pl == 0 ? Xr : pl == 1 ? Xi : pl == 2 ? Wr : Wi;
 #pragma unroll 1
       for (int k = ty; k < n; k += rows) {
-        const size_t e = (size_t)b * per + (size_t)k * n + j;
         int32_t u[ND], t[ND];
-        fx_load(u, P, count, e);
+        fx_load(u, base(pl), stride, idx(k));
         fx_mul(t, u, m);
         int32_t o[ND];
         fx_add(o, u, t);
-        fx_store(P, count, e, o);
+        fx_store(base(pl), stride, idx(k), o);
+        if (CACHE) fx_store(gplane[pl], count, (size_t)b * per + (size_t)k * n + j, o);
       }
     }
   }
@@ -402,13 +419,12 @@ __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int3
     if (act) {
 #pragma unroll 1
       for (int k = ty; k < n; k += rows) {
-        const size_t e = (size_t)b * per + (size_t)k * n + j;
         // part 0: xr wr + xi wi ;  part 1: xr wi - xi wr
 #pragma unroll 1
         for (int term = 0; term < 2; ++term) {
           int32_t a[ND], c[ND];
-          fx_load(a, term ? Xi : Xr, count, e);
-          fx_load(c, (term ^ part) ? Wi : Wr, count, e);
+          fx_load(a, base(term), stride, idx(k));
+          fx_load(c, base(2 + (term ^ part)), stride, idx(k));
           if (part == 1 && term == 1) {
 #pragma unroll
             for (int q = 0; q < ND; ++q) a[q] = -a[q];  // digit-wise negation: a valid (non-canonical) operand of fx_mac
@@ -448,11 +464,11 @@ __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int3
             const int32_t v = use_si ? si[q] : sr[q];
             mm[q] = neg ? -v : v;
           }
-          fx_load(a, term ? Xi : Xr, count, e);
+          fx_load(a, base(term), stride, idx(k));
           fx_mac<false>(acc, a, mm);
         }
         fxp_finish(t, acc);
-        fx_load(a, part ? Wi : Wr, count, e);
+        fx_load(a, base(2 + part), stride, idx(k));
         int32_t o[ND];
         fx_sub(o, a, t);
         fx_store(part ? Ri : Rr, count, e, o);
@@ -476,13 +492,17 @@ int singleton_step(int n, int nb, int32_t* X, int32_t* W, int32_t* R, int32_t* S
   if (cpb == 1) {
     int threads = (n + 31) / 32 * 32;
     if (threads > 256) threads = 256;
-    singleton_step_kernel<1><<<grid, threads, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
+    const size_t cache = sizeof(int32_t) * 4 * ND * (size_t)n;  // 480 n bytes
+    if (cache + 8 * FXP_NACC * sizeof(int64_t) + 64 <= 48 * 1024 && options().sstep_cache)
+      singleton_step_kernel<1, true><<<grid, threads, cache, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
+    else
+      singleton_step_kernel<1, false><<<grid, threads, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
   } else if (cpb == 2) {
-    singleton_step_kernel<2><<<grid, 256, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
+    singleton_step_kernel<2, false><<<grid, 256, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
   } else if (cpb == 4) {
-    singleton_step_kernel<4><<<grid, 256, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
+    singleton_step_kernel<4, false><<<grid, 256, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
   } else {
-    singleton_step_kernel<8><<<grid, 256, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
+    singleton_step_kernel<8, false><<<grid, 256, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
   }
   count_launch();
   return launch_check();
