@@ -88,7 +88,8 @@ int zkd_diag_herm_host(int N, int batch, int prec_bits, const void *A_host, void
  * above the noise of the projected matrix; default 1; 0 leaves every cluster to the S5 recursion),
  * "split_margin_bits" (that margin, default 40), "seed_sweeps" (cap on the fp64 Jacobi sweeps, default 12),
  * "seed_path" / "seed_cluster" (seed kernel selection), "combine_path" (epilogue of the IMAD GEMM: 0 automatic,
- * 1 digit-serial, 2 warp-cooperative), "sstep_cpb" (matrix columns per CTA of the fused singleton step, 0 automatic),
+ * 1 digit-serial, 2 warp-cooperative), "sstep_cpb" (matrix columns per CTA of the fused singleton step, 0 automatic), "sstep_warp" (1: its
+ * warp-per-element variant for N <= 64, default 0), "sstep_cache" (shared-memory staging of the column, default 1),
  * "verbose" (1: one line per refinement pass on stderr).  All routes give the same results to the stated tolerances;
  * the defaults are the measured-fastest ones.  Returns ZKD_ERR_INVALID_ARG for an unknown key. */
 int zkd_set_option(const char *key, double value);

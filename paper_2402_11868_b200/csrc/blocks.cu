@@ -481,6 +481,233 @@ __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int3
   __syncthreads();
   if (tid == 0 && msb_r_out && s_msb) atomicMax(msb_r_out, s_msb);
 }
+// ---- warp-cooperative variant for small n (north_star (b): "warp-cooperative limb add, multiply, normalise ... carry chains
+// via warp shuffles") -------------------------------------------------------------------------------------------------------
+// One CTA per matrix column, one WARP per element: lane L holds digit L of an FX number (lanes 0..29) and, in a product,
+// column 28 + L (lanes 0..30: the 31 kept columns).  A 30 x 30 digit product is 30 x (shuffle + IMAD.WIDE) per lane instead of
+// ~500 IMAD.WIDE in one thread; carries are resolved across lanes by two relaxation rounds and a ballot look-ahead.  Each
+// warp keeps the x, w digits of its (at most 4) rows in registers through all phases.  Exact integer sums and one rounding
+// at the guard column, as in the thread-per-element kernel: the results are bit-identical.
+template <int TOP>
+__device__ __forceinline__ int64_t wcanon(int64_t v, int lane) {
+  const bool low = lane < TOP, top = lane == TOP;
+  constexpr unsigned kLowMask = (1u << TOP) - 1;
+  int64_t lo = low ? (v & DMASK) : (top ? v : 0), hi = low ? (v >> DB) : 0;
+#pragma unroll
+  for (int round = 0; round < 2; ++round) {
+    int64_t inc = __shfl_up_sync(0xffffffffu, hi, 1);
+    if (lane == 0 || lane > TOP) inc = 0;
+    const int64_t t = lo + inc;
+    if (low) { hi = t >> DB; lo = t & DMASK; }
+    else { hi = 0; lo = t; }
+  }
+  int64_t inc = __shfl_up_sync(0xffffffffu, hi, 1);  // -1, 0 or +1
+  if (lane == 0 || lane > TOP) inc = 0;
+  int64_t t = lo;
+  bool gen = false;
+  if (inc == 1) {
+    t += 1;
+    if (low && t == (int64_t)DMASK + 1) { t = 0; gen = true; }
+  }
+  unsigned G = __ballot_sync(0xffffffffu, gen) & kLowMask;
+  unsigned P = __ballot_sync(0xffffffffu, low && t == DMASK) & kLowMask;
+  unsigned C = (((P + (G << 1)) ^ P ^ (G << 1)) | (G << 1));
+  if ((C >> lane) & 1) t = low ? ((t + 1) & DMASK) : (top ? t + 1 : t);
+  gen = false;
+  if (inc == -1) {
+    t -= 1;
+    if (low && t < 0) { t = DMASK; gen = true; }
+  }
+  G = __ballot_sync(0xffffffffu, gen) & kLowMask;
+  P = __ballot_sync(0xffffffffu, low && t == 0) & kLowMask;
+  C = (((P + (G << 1)) ^ P ^ (G << 1)) | (G << 1));
+  if ((C >> lane) & 1) t = low ? ((t - 1) & DMASK) : (top ? t - 1 : t);
+  return t;
+}
+// acc (column 28 + lane) += sign * sum_i a_i b_{28 + lane - i}:  a uniform (every lane holds all digits), b one digit per lane
+__device__ __forceinline__ void wmac_u(int64_t& acc, const int32_t (&a)[ND], int32_t b, int lane, bool neg) {
+#pragma unroll
+  for (int i = 0; i < ND; ++i) {
+    const int src = FXP_LOW + lane - i;
+    int32_t bv = __shfl_sync(0xffffffffu, b, src & 31);
+    if (src < 0 || src > ND - 1) bv = 0;
+    const int64_t p = (int64_t)a[i] * (int64_t)bv;
+    acc += neg ? -p : p;
+  }
+}
+// both operands one digit per lane
+__device__ __forceinline__ void wmac_l(int64_t& acc, int32_t a, int32_t b, int lane, bool neg) {
+#pragma unroll
+  for (int i = 0; i < ND; ++i) {
+    const int32_t ai = __shfl_sync(0xffffffffu, a, i);
+    const int src = FXP_LOW + lane - i;
+    int32_t bv = __shfl_sync(0xffffffffu, b, src & 31);
+    if (src < 0 || src > ND - 1) bv = 0;
+    const int64_t p = (int64_t)ai * (int64_t)bv;
+    acc += neg ? -p : p;
+  }
+}
+// keep a running column accumulator small: pass the overflow of every column to the lane above (lane 30 keeps the rest)
+__device__ __forceinline__ void wrelax1(int64_t& acc, int lane) {
+  const bool low = lane < ND;
+  const int64_t hi = low ? (acc >> DB) : 0;
+  int64_t inc = __shfl_up_sync(0xffffffffu, hi, 1);
+  if (lane == 0 || lane > ND) inc = 0;
+  acc = (low ? (acc & DMASK) : acc) + inc;
+}
+// product columns -> FX digits (rounded at the guard column): digit r ends up in lane r
+__device__ __forceinline__ int32_t wfinish(int64_t acc, int lane) {
+  if (lane == 0) acc += DHALF;
+  if (lane > ND) acc = 0;
+  const int64_t t = wcanon<ND>(acc, lane);  // 31 columns: lanes 0..30, the rest in lane 30
+  const int64_t d = __shfl_down_sync(0xffffffffu, t, 1);
+  return lane < ND ? (int32_t)d : 0;
+}
+// all 30 digits of a digit-per-lane number into every lane
+__device__ __forceinline__ void wbroadcast(int32_t (&all)[ND], int32_t d) {
+#pragma unroll
+  for (int i = 0; i < ND; ++i) all[i] = __shfl_sync(0xffffffffu, d, i);
+}
+__device__ __forceinline__ int wmsb(int32_t d, int lane) {
+  const int32_t top = __shfl_sync(0xffffffffu, d, ND - 1);
+  int cand = 0;
+  if (lane < ND - 1) {
+    if (top < 0) { if (d != DMASK) cand = lane * DB + (32 - __clz((~d) & DMASK)); }
+    else if (d != 0) cand = lane * DB + (32 - __clz(d));
+  } else if (lane == ND - 1) {
+    if (d > 0) cand = lane * DB + (32 - __clz(d));
+    if (d < -1) cand = lane * DB + (32 - __clz(~d));
+  }
+  for (int o = 16; o > 0; o >>= 1) cand = max(cand, __shfl_xor_sync(0xffffffffu, cand, o));
+  return cand;
+}
+
+constexpr int SW_RPW = 4;  // rows per warp
+
+__global__ void __launch_bounds__(512) singleton_step_warp_kernel(int n, int nb, int32_t* __restrict__ X, int32_t* __restrict__ W,
+                                                                   int32_t* __restrict__ R, int32_t* __restrict__ S,
+                                                                   int32_t* __restrict__ theta, int* __restrict__ msb_g_out,
+                                                                   int* __restrict__ msb_r_out, const int* __restrict__ cl,
+                                                                   const int* __restrict__ cle) {
+  __shared__ int64_t s_red[2][16][32];
+  __shared__ int s_msb;
+  const int b = blockIdx.x / n, j = blockIdx.x % n;
+  if (cl && cle[blockIdx.x] - cl[blockIdx.x] > 1) return;  // columns of larger clusters take the GEMM path
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  const size_t per = (size_t)n * n, count = per * nb;
+  const bool dl = lane < ND;  // lanes that hold a digit
+  int32_t* const gplane[4] = {X, X + (size_t)ND * count, W, W + (size_t)ND * count};
+  if (threadIdx.x == 0) s_msb = 0;
+
+  // this warp's rows: k = warp + t * nw
+  int32_t v[4][SW_RPW];
+#pragma unroll
+  for (int t = 0; t < SW_RPW; ++t) {
+    const int k = warp + t * nw;
+#pragma unroll
+    for (int pl = 0; pl < 4; ++pl)
+      v[pl][t] = (k < n && dl) ? gplane[pl][(size_t)lane * count + (size_t)b * per + (size_t)k * n + j] : 0;
+  }
+  auto block_sum = [&](int64_t a, int slot) -> int64_t {
+    s_red[slot][warp][lane] = a;
+    __syncthreads();
+    int64_t t = 0;
+    for (int w = 0; w < nw; ++w) t += s_red[slot][w][lane];
+    return t;
+  };
+
+  // g = sum_k |x_kj|^2
+  int64_t acc = 0;
+#pragma unroll
+  for (int t = 0; t < SW_RPW; ++t) {
+    if (warp + t * nw < n) {
+      wmac_l(acc, v[0][t], v[0][t], lane, false);
+      wmac_l(acc, v[1][t], v[1][t], lane, false);
+      wrelax1(acc, lane);
+    }
+  }
+  acc = block_sum(acc, 0);
+  int32_t g = wfinish(acc, lane);
+  if (lane == ND - 1) g -= 1;  // g - 1
+  {
+    const int mg = wmsb(g, lane);
+    if (threadIdx.x == 0 && msb_g_out) atomicMax(msb_g_out, mg);
+  }
+  // m = (1 - g)/2: negate, canonicalise, shift right by one bit
+  int32_t m;
+  {
+    const int64_t ng = wcanon<ND - 1>(dl ? -(int64_t)g : 0, lane);
+    const int64_t up = __shfl_down_sync(0xffffffffu, ng, 1);
+    m = lane < ND - 1 ? (int32_t)(((ng >> 1) | (up << (DB - 1))) & DMASK) : (lane == ND - 1 ? (int32_t)(ng >> 1) : 0);
+  }
+  int32_t all[ND];
+  wbroadcast(all, m);
+  // x <- x + x m, w <- w + w m
+#pragma unroll
+  for (int t = 0; t < SW_RPW; ++t) {
+    const int k = warp + t * nw;
+    if (k < n) {
+#pragma unroll
+      for (int pl = 0; pl < 4; ++pl) {
+        int64_t a2 = 0;
+        wmac_u(a2, all, v[pl][t], lane, false);
+        const int32_t tt = wfinish(a2, lane);
+        const int32_t o = (int32_t)wcanon<ND - 1>(dl ? (int64_t)v[pl][t] + tt : 0, lane);
+        v[pl][t] = o;
+        if (dl) gplane[pl][(size_t)lane * count + (size_t)b * per + (size_t)k * n + j] = o;
+      }
+    }
+  }
+  // s = x^H w
+  int64_t are = 0, aim = 0;
+#pragma unroll
+  for (int t = 0; t < SW_RPW; ++t) {
+    if (warp + t * nw < n) {
+      wmac_l(are, v[0][t], v[2][t], lane, false);  // xr wr
+      wmac_l(are, v[1][t], v[3][t], lane, false);  // xi wi
+      wmac_l(aim, v[0][t], v[3][t], lane, false);  // xr wi
+      wmac_l(aim, v[1][t], v[2][t], lane, true);   // - xi wr
+      wrelax1(are, lane);
+      wrelax1(aim, lane);
+    }
+  }
+  __syncthreads();  // s_red[0] is still being read by slower warps
+  are = block_sum(are, 1);
+  aim = block_sum(aim, 0);
+  const int32_t sr = wfinish(are, lane), si = wfinish(aim, lane);
+  if (warp == 0 && dl) {
+    theta[(size_t)lane * n * nb + (size_t)b * n + j] = sr;
+    const size_t ejj = (size_t)b * per + (size_t)j * n + j;
+    S[(size_t)lane * count + ejj] = sr;
+    S[((size_t)ND + lane) * count + ejj] = si;
+  }
+  // r = w - x s
+  int32_t sall[ND];
+  int mymsb = 0;
+#pragma unroll 1
+  for (int part = 0; part < 2; ++part) {
+    // part 0: xr sr - xi si ;  part 1: xr si + xi sr
+#pragma unroll
+    for (int t = 0; t < SW_RPW; ++t) {
+      const int k = warp + t * nw;
+      if (k < n) {
+        int64_t a2 = 0;
+        wbroadcast(sall, part ? si : sr);
+        wmac_u(a2, sall, v[0][t], lane, false);
+        wbroadcast(sall, part ? sr : si);
+        wmac_u(a2, sall, v[1][t], lane, part == 0);
+        const int32_t tt = wfinish(a2, lane);
+        const int32_t o = (int32_t)wcanon<ND - 1>(dl ? (int64_t)v[2 + part][t] - tt : 0, lane);
+        if (dl) R[((size_t)part * ND + lane) * count + (size_t)b * per + (size_t)k * n + j] = o;
+        mymsb = max(mymsb, wmsb(o, lane));
+      }
+    }
+  }
+  if (lane == 0 && mymsb) atomicMax(&s_msb, mymsb);
+  __syncthreads();
+  if (threadIdx.x == 0 && msb_r_out && s_msb) atomicMax(msb_r_out, s_msb);
+}
+
 int singleton_step(int n, int nb, int32_t* X, int32_t* W, int32_t* R, int32_t* S, int32_t* theta, int* msb_g_out, int* msb_r_out,
                    cudaStream_t s, const int* cl, const int* cle) {
   // columns per CTA: as many as keep about one CTA per SM (sector efficiency of the row-major loads against parallelism)
@@ -489,7 +716,10 @@ int singleton_step(int n, int nb, int32_t* X, int32_t* W, int32_t* R, int32_t* S
   const int cpb = (forced == 1 || forced == 2 || forced == 4 || forced == 8) ? forced
                   : cols >= 8 * 128 ? 8 : cols >= 4 * 96 ? 4 : cols >= 2 * 96 ? 2 : 1;
   const unsigned grid = (unsigned)((size_t)((n + cpb - 1) / cpb) * nb);
-  if (cpb == 1) {
+  if (cpb == 1 && n <= 16 * SW_RPW && options().sstep_warp) {
+    const int nw = (n + SW_RPW - 1) / SW_RPW;
+    singleton_step_warp_kernel<<<grid, 32 * nw, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
+  } else if (cpb == 1) {
     int threads = (n + 31) / 32 * 32;
     if (threads > 256) threads = 256;
     const size_t cache = sizeof(int32_t) * 4 * ND * (size_t)n;  // 480 n bytes
