@@ -144,6 +144,7 @@ static int* option_slot(const char* key) {
   if (!strcmp(key, "min_split_ctas")) return &o.min_split_ctas;
   if (!strcmp(key, "seed_sweeps")) return &o.seed_sweeps;
   if (!strcmp(key, "seed_path")) return &o.seed_path;
+  if (!strcmp(key, "seed_dbuf")) return &o.seed_dbuf;
   if (!strcmp(key, "seed_cluster")) return &o.seed_cluster;
   if (!strcmp(key, "early_split")) return &o.early_split;
   if (!strcmp(key, "split_margin_bits")) return &o.split_margin_bits;

@@ -76,9 +76,10 @@ __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.w
 template <int EPL>
 __global__ void __launch_bounds__(EPL >= 8 ? 512 : 1024)
 seed_ring_kernel(int n, int wpc, const double2* __restrict__ A, double* __restrict__ mu, double2* __restrict__ V, int max_sweeps,
-                 double tol2) {
-  extern __shared__ double2 slots[];              // [wpc][2][n]
-  __shared__ int s_id[32][2];                     // column ids held by the local slots
+                 double tol2, int dbuf) {
+  extern __shared__ double2 slots[];              // [1 + dbuf][wpc][2][n]
+  __shared__ int s_id2[2][32][2];                 // column ids held by the local slots (per buffer)
+  int (*s_id)[2] = s_id2[0];
   __shared__ double s_mu[258];                    // by position 2k + which (every CTA holds a full copy)
   __shared__ int s_pid[258];
   __shared__ unsigned long long s_cmax[2];
@@ -94,6 +95,11 @@ seed_ring_kernel(int n, int wpc, const double2* __restrict__ A, double* __restri
   const bool act = k < P;
   double2* my_top = slots + (size_t)(warp * 2 + 0) * n;
   double2* my_bot = slots + (size_t)(warp * 2 + 1) * n;
+  // dbuf: a second set of slots.  Round r reads set r % 2 and writes the rotated columns into set (r + 1) % 2 of their
+  // destinations, so the "all slots read" barrier of the single-buffer scheme is not needed: one cluster barrier per round.
+  const size_t bufstride = (size_t)wpc * 2 * n;   // double2 elements between the two slot sets
+  constexpr int kIdStride = 32 * 2;               // ints between the two id sets
+  int cur = 0;
 
   // own two columns of the Hermitian matrix (upper triangle authoritative), Gershgorin radius
   double rmax = 0;
@@ -162,16 +168,18 @@ seed_ring_kernel(int n, int wpc, const double2* __restrict__ A, double* __restri
         double2 a[EPL], bb[EPL];
         int ida = 0, idb = 0;
         if (act) {
+          const double2* rt = my_top + (size_t)cur * bufstride;
+          const double2* rb = my_bot + (size_t)cur * bufstride;
 #pragma unroll
           for (int q = 0; q < EPL; ++q) {
             const int i2 = lane + 32 * q;
-            a[q] = i2 < n ? my_top[i2] : make_double2(0, 0);
-            bb[q] = i2 < n ? my_bot[i2] : make_double2(0, 0);
+            a[q] = i2 < n ? rt[i2] : make_double2(0, 0);
+            bb[q] = i2 < n ? rb[i2] : make_double2(0, 0);
           }
-          ida = s_id[warp][0];
-          idb = s_id[warp][1];
+          ida = s_id2[cur][warp][0];
+          idb = s_id2[cur][warp][1];
         }
-        cluster_arrive();  // slots read
+        if (!dbuf) cluster_arrive();  // slots read
         if (act) {
           double al = 0, be = 0, gr = 0, gi = 0;
 #pragma unroll
@@ -193,15 +201,19 @@ seed_ring_kernel(int n, int wpc, const double2* __restrict__ A, double* __restri
             }
           }
         }
-        cluster_wait();    // everybody has read: slots may be overwritten
+        if (!dbuf) cluster_wait();    // everybody has read: slots may be overwritten
+        const int nxt = dbuf ? (cur ^ 1) : 0;
         if (act) {
+          double2* wt = dst_top + (size_t)nxt * bufstride;
+          double2* wb = dst_bot + (size_t)nxt * bufstride;
 #pragma unroll
           for (int q = 0; q < EPL; ++q) {
             const int i2 = lane + 32 * q;
-            if (i2 < n) { dst_top[i2] = a[q]; dst_bot[i2] = bb[q]; }
+            if (i2 < n) { wt[i2] = a[q]; wb[i2] = bb[q]; }
           }
-          if (lane == 0) { *dst_top_id = ida; *dst_bot_id = idb; }
+          if (lane == 0) { dst_top_id[nxt * kIdStride] = ida; dst_bot_id[nxt * kIdStride] = idb; }
         }
+        cur = nxt;
         if (r == M - 2 && lane == 0 && cmax > 0) atomicMax(&s_cmax[sweep & 1], (unsigned long long)__double_as_longlong(cmax));
         cluster_arrive();
         cluster_wait();    // slots written
@@ -215,6 +227,10 @@ seed_ring_kernel(int n, int wpc, const double2* __restrict__ A, double* __restri
     }
   }
   cluster.sync();
+  // the final columns sit in slot set `cur`
+  my_top += (size_t)cur * bufstride;
+  my_bot += (size_t)cur * bufstride;
+  s_id = s_id2[cur];
 
   // mu = ||g|| - sigma per position, broadcast to every CTA; normalise in place
   if (act) {
@@ -265,7 +281,9 @@ static int launch_ring(int N, int batch, int csize, const double2* A, double* mu
                        cudaStream_t s) {
   const int P = (N + 1) / 2;
   const int wpc = (P + csize - 1) / csize;
-  const size_t smem = sizeof(double2) * (size_t)wpc * 2 * N;
+  const size_t smem1 = sizeof(double2) * (size_t)wpc * 2 * N;
+  int dbuf = (2 * smem1 <= 200 * 1024 && options().seed_dbuf) ? 1 : 0;
+  const size_t smem = smem1 * (1 + dbuf);
   static size_t attr_smem = 0;
   static bool np_done = false;
   if (smem > 48 * 1024 && smem > attr_smem) {
@@ -288,7 +306,7 @@ static int launch_ring(int N, int batch, int csize, const double2* A, double* mu
   at[0].val.clusterDim.z = 1;
   cfg.attrs = at;
   cfg.numAttrs = 1;
-  ZKD_CUDA_TRY(cudaLaunchKernelEx(&cfg, seed_ring_kernel<EPL>, N, wpc, A, mu, V, max_sweeps, tol2));
+  ZKD_CUDA_TRY(cudaLaunchKernelEx(&cfg, seed_ring_kernel<EPL>, N, wpc, A, mu, V, max_sweeps, tol2, dbuf));
   count_launch();
   return launch_check();
 }
