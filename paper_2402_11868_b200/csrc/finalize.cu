@@ -299,18 +299,36 @@ __global__ void __launch_bounds__(128) rank_kernel(int N, int batch, const int32
   int32_t lj[ND];
   fx_load(lj, lam, cnt, t);
   int r = 0;
-  for (int i = 0; i < N; ++i) {
-    // compare from the top digit down and stop loading at the first difference (almost always the top digit or the next)
-    const int32_t* pi = lam + (size_t)b * N + i;
-    int cmp = 0;  // sign of (lambda_i - lambda_j)
+  // The top three digits (integer part and 56 fractional bits) decide almost every comparison: fetch them for four
+  // candidates at a time (independent loads), and walk the remaining digits only on a tie.
+  const int32_t* base = lam + (size_t)b * N;
+  for (int i0 = 0; i0 < N; i0 += 4) {
+    int32_t d2[4], d1[4], d0[4];
 #pragma unroll
-    for (int k = ND - 1; k >= 0; --k) {
-      if (cmp == 0) {
-        const int32_t d = pi[(size_t)k * cnt];
-        cmp = d < lj[k] ? -1 : d > lj[k] ? 1 : 0;
-      }
+    for (int u = 0; u < 4; ++u) {
+      const int i = i0 + u < N ? i0 + u : N - 1;
+      d2[u] = base[(size_t)(ND - 1) * cnt + i];
+      d1[u] = base[(size_t)(ND - 2) * cnt + i];
+      d0[u] = base[(size_t)(ND - 3) * cnt + i];
     }
-    r += cmp < 0 || (cmp == 0 && i < j);
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int i = i0 + u;
+      if (i >= N) continue;
+      int cmp = d2[u] < lj[ND - 1] ? -1 : d2[u] > lj[ND - 1] ? 1 : 0;  // sign of (lambda_i - lambda_j)
+      if (cmp == 0) cmp = d1[u] < lj[ND - 2] ? -1 : d1[u] > lj[ND - 2] ? 1 : 0;
+      if (cmp == 0) cmp = d0[u] < lj[ND - 3] ? -1 : d0[u] > lj[ND - 3] ? 1 : 0;
+      if (cmp == 0) {
+#pragma unroll
+        for (int k = ND - 4; k >= 0; --k) {
+          if (cmp == 0) {
+            const int32_t d = base[(size_t)k * cnt + i];
+            cmp = d < lj[k] ? -1 : d > lj[k] ? 1 : 0;
+          }
+        }
+      }
+      r += cmp < 0 || (cmp == 0 && i < j);
+    }
   }
   rank[t] = r;
   fx_store(lam_sorted, cnt, (size_t)b * N + r, lj);
