@@ -831,6 +831,10 @@ __global__ void __launch_bounds__(128) ecalc_kernel(int n, int nb, const int32_t
   if (s >= 0) fx_shl(d, s); else fx_shr(d, -s);
   int32_t r[ND];
   fx_recip_quarter<W>(r, d, newton_iters);
+  constexpr int LO = ND - 1 - W;
+  int32_t rw[W + 1];
+#pragma unroll
+  for (int k = 0; k <= W; ++k) rw[k] = r[LO + k];
   // E = (C r) 2^s, with sign
   int mymsb = 0;
 #pragma unroll 1
@@ -840,7 +844,14 @@ __global__ void __launch_bounds__(128) ecalc_kernel(int n, int nb, const int32_t
     const bool neg = dneg ^ ((which & 2) != 0);
     int32_t c[ND], o[ND];
     fx_load(c, plane, count, e);
-    fx_mul(o, c, r);
+    {
+      // r has W + 1 nonzero digits (LO .. 29): the product needs 30 (W + 1) digit products, not 30 x 30; the kept columns
+      // and the rounding are those of fx_mul
+      int64_t acc[FXP_NACC];
+      fxp_zero(acc);
+      mac_cols<ND, W + 1, FXP_LOW - LO, FXP_NACC, false>(acc, c, rw);
+      fxp_finish(o, acc);
+    }
     if (s >= 0) fx_shl(o, s); else fx_shr(o, -s);
     if (neg) { int32_t u[ND]; fx_neg(u, o);
 #pragma unroll
