@@ -411,13 +411,14 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
   ZKD_CUDA_TRY(cudaMemcpyAsync(cl0, cl, sizeof(int) * n * nb, cudaMemcpyDeviceToDevice, s));
   ZKD_CUDA_TRY(cudaMemcpyAsync(cle0, cle, sizeof(int) * n * nb, cudaMemcpyDeviceToDevice, s));
   // cluster table to the host (needed for S5 and to pick the singleton fast path)
-  std::vector<int> h_cl((size_t)n * nb);
+  std::vector<int> h_cl((size_t)n * nb), h_cl0;
   ZKD_CUDA_TRY(cudaMemcpyAsync(h_cl.data(), cl, sizeof(int) * n * nb, cudaMemcpyDeviceToHost, s));
   if (st && depth == 0) {
     st->cl_stats.resize((size_t)2 * nb);
     ZKD_CUDA_TRY(cudaMemcpyAsync(st->cl_stats.data(), stats, sizeof(int) * 2 * nb, cudaMemcpyDeviceToHost, s));
   }
   ZKD_CUDA_TRY(cudaStreamSynchronize(s));
+  h_cl0 = h_cl;  // the clusters as detected (S4h refines h_cl)
   bool singletons = true;
   for (int b = 0; b < nb && singletons; ++b)
     for (int j = 1; j < n; ++j)
@@ -506,10 +507,38 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
     // cluster can be tiny (c4: 2^-61).  One symmetric (Loewdin / Newton-Schulz) orthonormalisation over the clusters AS
     // DETECTED squares that error; it moves the vectors by the same residual / gap inside a cluster whose spread is
     // <= 2^-tau, i.e. the residual grows by less than itself.
-    ZKD_TRY(gram_blocks(n, nb, Xc, Xc, cl0, Gm, s));
-    ZKD_TRY(ns_build(n, nb, cl0, Gm, nullptr, s));
-    ZKD_TRY(block_apply(n, nb, Xc, Xc, Gm, cl0, cle0, false, Tc, nullptr, s));
-    std::swap(Xc, Tc);
+    // As GEMMs over the views of the detected clusters: G at full width, M = (I - G)/2 is tiny (|M| ~ residual / gap), so
+    // X_c += X_c M_c is a 30 x 3-digit product.
+    ClusterPlan plan0;
+    ZKD_TRY(build_plan(c, n, nb, h_cl0, plan_dev, &plan0));
+    {
+      const size_t cnt0 = (size_t)n * n * nb;
+      auto view = [&](const int32_t* fx, int rows, int cols, bool ct, int top, int nw, const int* off) {
+        GemmSide g;
+        g.fx = fx; g.rows = rows; g.cols = cols; g.conj_transpose = ct; g.top_bit = top; g.nw = std::max(1, std::min(nw, kND));
+        g.ld = n; g.off = off; g.plane_count = cnt0;
+        return g;
+      };
+      auto gemm = [&](int M, int N, int K, int batch, const GemmSide& P, const GemmSide& Q, int32_t* dst, GemmMode mode, const int* dst_off) {
+        GemmDstView dv;
+        dv.ld = n; dv.off = dst_off; dv.plane_count = cnt0;
+        return gemm_complex(M, N, K, batch, P, Q, dst, mode, -1, opt.gemm_path, c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s, &dv);
+      };
+      ZKD_CUDA_TRY(cudaMemsetAsync(scal, 0, sizeof(int) * S_NUM, s));
+      for (const ClusterGroup& g : plan0.groups)
+        ZKD_TRY(gemm(g.m, g.m, n, g.nsub, view(Xc, n, g.m, true, topX, kND, g.offX), view(Xc, n, g.m, false, topX, kND, g.offX), Gm,
+                     GemmMode::Assign, g.offB));
+      ZKD_TRY(ns_build(n, nb, cl0, Gm, scal + S_MSB_G, s, cle0));
+      ZKD_TRY(read_scalars(c, scal, S_NUM, hs));
+      if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
+      const int msb_m = hs[S_MSB_G];
+      if (msb_m > 0) {
+        const int topM = msb_m + 1, nwM = std::max(1, std::min(kND, ceil_div(topM, kDB)));
+        for (const ClusterGroup& g : plan0.groups)
+          ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(Xc, n, g.m, false, topX, kND, g.offX), view(Gm, g.m, g.m, false, topM, nwM, g.offB), Xc,
+                       GemmMode::Add, g.offX));
+      }
+    }
   }
   if (Xc != X) ZKD_CUDA_TRY(cudaMemcpyAsync(X, Xc, fxc, cudaMemcpyDeviceToDevice, s));
 
