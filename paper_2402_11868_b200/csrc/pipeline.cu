@@ -582,8 +582,19 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
       any = true;
     }
     if (any) {
-      ZKD_TRY(block_apply(n, nb, nullptr, X, Um, cl, cle, false, Xn, nullptr, s));
-      ZKD_CUDA_TRY(cudaMemcpyAsync(X, Xn, fxc, cudaMemcpyDeviceToDevice, s));
+      // X_c <- X_c U_c in place, as batched GEMMs over the cluster views (operands are staged before the product runs)
+      ClusterPlan planf;
+      ZKD_TRY(build_plan(c, n, nb, h_cl, plan_dev, &planf));
+      const size_t cntf = (size_t)n * n * nb;
+      for (const ClusterGroup& g : planf.groups) {
+        GemmSide P, Q;
+        P.fx = X; P.rows = n; P.cols = g.m; P.conj_transpose = false; P.top_bit = topX; P.nw = kND; P.ld = n; P.off = g.offX; P.plane_count = cntf;
+        Q.fx = Um; Q.rows = g.m; Q.cols = g.m; Q.conj_transpose = false; Q.top_bit = topX; Q.nw = kND; Q.ld = n; Q.off = g.offB; Q.plane_count = cntf;
+        GemmDstView dv;
+        dv.ld = n; dv.off = g.offX; dv.plane_count = cntf;
+        ZKD_TRY(gemm_complex(n, g.m, g.m, g.nsub, P, Q, X, GemmMode::Assign, -1, opt.gemm_path, c.gemm_ws, c.gemm_ws_bytes, nullptr, nullptr,
+                             s, &dv));
+      }
     }
     ZKD_CUDA_TRY(cudaStreamSynchronize(s));
   }
