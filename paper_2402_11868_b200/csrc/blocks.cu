@@ -104,52 +104,6 @@ int init_x(size_t count, const double2* V, int32_t* X, cudaStream_t s) {
   return launch_check();
 }
 
-// ---- cluster-block Gram matrices: G_ij = sum_k conj(x_ki) y_kj for cl(i) == cl(j) -------------------------------------
-// one warp per (b, i, j, part); lanes split k; exact digit products, one carry pass per MAC pair.
-__global__ void __launch_bounds__(128) gram_kernel(int n, int nb, const int32_t* __restrict__ X, const int32_t* __restrict__ Y,
-                                                   const int* __restrict__ cl, int32_t* __restrict__ G) {
-  const size_t w = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  const int lane = threadIdx.x & 31;
-  const size_t per = (size_t)n * n;
-  if (w >= per * nb * 2) return;
-  const int part = (int)(w & 1);
-  const size_t e = w >> 1;
-  const int b = (int)(e / per);
-  const int i = (int)((e % per) / n), j = (int)(e % n);
-  if (cl[(size_t)b * n + i] != cl[(size_t)b * n + j]) return;
-  const size_t count = per * nb;
-  const int32_t* Xr = X;
-  const int32_t* Xi = X + (size_t)ND * count;
-  const int32_t* Yr = Y;
-  const int32_t* Yi = Y + (size_t)ND * count;
-  int64_t acc[FXP_NACC];
-  fxp_zero(acc);
-  for (int k = lane; k < n; k += 32) {
-    const size_t ei = (size_t)b * per + (size_t)k * n + i, ej = (size_t)b * per + (size_t)k * n + j;
-    int32_t a[ND], c[ND];
-    if (part == 0) {  // xr yr + xi yi
-      fx_load(a, Xr, count, ei); fx_load(c, Yr, count, ej); fx_mac<false>(acc, a, c);
-      fx_load(a, Xi, count, ei); fx_load(c, Yi, count, ej); fx_mac<false>(acc, a, c);
-    } else {          // xr yi - xi yr
-      fx_load(a, Xr, count, ei); fx_load(c, Yi, count, ej); fx_mac<false>(acc, a, c);
-      fx_load(a, Xi, count, ei); fx_load(c, Yr, count, ej); fx_mac<true>(acc, a, c);
-    }
-    fxp_relax(acc);
-  }
-  warp_sum_cols(acc);
-  if (lane == 0) {
-    int32_t r[ND];
-    fxp_finish(r, acc);
-    fx_store(G + (part ? (size_t)ND * count : 0), count, e, r);
-  }
-}
-int gram_blocks(int n, int nb, const int32_t* X, const int32_t* Y, const int* cl, int32_t* G, cudaStream_t s) {
-  const size_t warps = (size_t)n * n * nb * 2;
-  gram_kernel<<<(unsigned)((warps * 32 + 127) / 128), 128, 0, s>>>(n, nb, X, Y, cl, G);
-  count_launch();
-  return launch_check();
-}
-
 // ---- M := (I - G)/2 on cluster blocks (Newton-Schulz orthonormalisation step), msb of (G - I) ---------------------------
 __global__ void __launch_bounds__(256) ns_build_kernel(int n, int nb, const int* __restrict__ cl, const int* __restrict__ cle_skip1,
                                                        int32_t* __restrict__ G, int* __restrict__ msb_out) {
@@ -174,67 +128,6 @@ __global__ void __launch_bounds__(256) ns_build_kernel(int n, int nb, const int*
 int ns_build(int n, int nb, const int* cl, int32_t* G, int* msb_out, cudaStream_t s, const int* cle_skip1) {
   const size_t t = (size_t)n * n * nb * 2;
   ns_build_kernel<<<(unsigned)((t + 255) / 256), 256, 0, s>>>(n, nb, cl, cle_skip1, G, msb_out);
-  count_launch();
-  return launch_check();
-}
-
-// ---- block-diagonal apply: dst_ij = base_ij + sgn * sum_{l in cluster(j)} Y_il M_lj -----------------------------------------
-// one thread per (b, i, j, part).  base may be null (treated as zero).  msb_out: atomicMax of msb(dst).
-__global__ void __launch_bounds__(128) block_apply_kernel(int n, int nb, const int32_t* __restrict__ base, const int32_t* __restrict__ Y,
-                                                          const int32_t* __restrict__ M, const int* __restrict__ cl,
-                                                          const int* __restrict__ cle, int negate, int32_t* __restrict__ dst,
-                                                          int* __restrict__ msb_out) {
-  const size_t per = (size_t)n * n, count = per * nb;
-  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= count * 2) return;
-  const int part = (int)(t / count);
-  const size_t e = t % count;
-  const int b = (int)(e / per), i = (int)((e % per) / n), j = (int)(e % n);
-  const int l0 = cl[(size_t)b * n + j], l1 = cle[(size_t)b * n + j];
-  const int32_t* Yr = Y;
-  const int32_t* Yi = Y + (size_t)ND * count;
-  const int32_t* Mr = M;
-  const int32_t* Mi = M + (size_t)ND * count;
-  int64_t acc[FXP_NACC];
-  fxp_zero(acc);
-  for (int l = l0; l < l1; ++l) {
-    const size_t ey = (size_t)b * per + (size_t)i * n + l, em = (size_t)b * per + (size_t)l * n + j;
-    int32_t a[ND], c[ND];
-    if (part == 0) {  // yr mr - yi mi
-      fx_load(a, Yr, count, ey); fx_load(c, Mr, count, em); fx_mac<false>(acc, a, c);
-      fx_load(a, Yi, count, ey); fx_load(c, Mi, count, em); fx_mac<true>(acc, a, c);
-    } else {          // yr mi + yi mr
-      fx_load(a, Yr, count, ey); fx_load(c, Mi, count, em); fx_mac<false>(acc, a, c);
-      fx_load(a, Yi, count, ey); fx_load(c, Mr, count, em); fx_mac<false>(acc, a, c);
-    }
-    fxp_relax(acc);
-  }
-  int32_t r[ND], o[ND];
-  fxp_finish(r, acc);
-  if (base) {
-    int32_t bs[ND];
-    fx_load(bs, base + (part ? (size_t)ND * count : 0), count, e);
-    if (negate) fx_sub(o, bs, r); else fx_add(o, bs, r);
-  } else {
-    if (negate) fx_neg(o, r);
-    else {
-#pragma unroll
-      for (int k = 0; k < ND; ++k) o[k] = r[k];
-    }
-  }
-  fx_store(dst + (part ? (size_t)ND * count : 0), count, e, o);
-  if (msb_out) {
-    const int msb = fx_msb(o);
-    // warp-level max first to keep the atomic traffic low
-    int m = msb;
-    for (int off = 16; off > 0; off >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, off));
-    if ((threadIdx.x & 31) == 0) atomicMax(msb_out, m);
-  }
-}
-int block_apply(int n, int nb, const int32_t* base, const int32_t* Y, const int32_t* M, const int* cl, const int* cle, bool negate,
-                int32_t* dst, int* msb_out, cudaStream_t s) {
-  const size_t t = (size_t)n * n * nb * 2;
-  block_apply_kernel<<<(unsigned)((t + 127) / 128), 128, 0, s>>>(n, nb, base, Y, M, cl, cle, negate ? 1 : 0, dst, msb_out);
   count_launch();
   return launch_check();
 }
@@ -300,8 +193,8 @@ int fxc_add_inplace(size_t count, int32_t* X, const int32_t* T, cudaStream_t s) 
 // ---- fused S4f + S4c for levels whose clusters are all singletons (the common case: c1, c2, c3) ---------------------------------
 // One CTA per column j:  g = ||x_j||^2 ;  f = 1 + (1 - g)/2 ;  x_j <- f x_j ;  w_j <- f w_j   (Newton-Schulz step = normalisation)
 //                        s = x_j^H w_j ;  theta_j = Re s ;  r_j = w_j - x_j s                  (Rayleigh quotient, residual)
-// X and W are updated in place (a CTA touches only its own column).  Replaces gram, ns_build, 2 x block_apply, gram, theta,
-// block_apply of the general path (7 launches) by one launch whose critical path is 14 digit products per element.
+// X and W are updated in place (a CTA touches only its own column).  One launch in place of the seven products of the cluster path
+// (Gram, Newton-Schulz build, two applies, Rayleigh-Ritz, theta, residual); its critical path is 14 digit products per element.
 // Sum of column accumulators over the threads of the CTA that own the same matrix column.  Thread layout: tx = tid % CPB is
 // the matrix column inside the CTA's group of CPB columns, the other bits of tid index rows; lanes with equal tx are
 // lane % CPB apart, so the warp stage uses xor offsets 16 .. CPB only.  Every thread returns its column's total.

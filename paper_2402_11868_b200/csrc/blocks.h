@@ -8,11 +8,8 @@ int fxc_to_c64(size_t count, const int32_t* src, double2* dst, cudaStream_t s);
 int cluster_detect(int n, int nb, const double2* A64, const double* mu, int tau_bits, const int* floor_msb /*[nb], may be null*/,
                    int* cl, int* cle, int* stats, cudaStream_t s);
 int init_x(size_t count, const double2* V, int32_t* X, cudaStream_t s);
-int gram_blocks(int n, int nb, const int32_t* X, const int32_t* Y, const int* cl, int32_t* G, cudaStream_t s);
 // cle_skip1 != null: blocks of singleton clusters are left untouched
 int ns_build(int n, int nb, const int* cl, int32_t* G, int* msb_out, cudaStream_t s, const int* cle_skip1 = nullptr);
-int block_apply(int n, int nb, const int32_t* base, const int32_t* Y, const int32_t* M, const int* cl, const int* cle, bool negate,
-                int32_t* dst, int* msb_out, cudaStream_t s);
 // fused S4f + S4c when every cluster of the level is a singleton: X, W updated in place, R, diag(S), theta written
 // cl / cle != null: only the columns whose cluster is a singleton are processed
 int singleton_step(int n, int nb, int32_t* X, int32_t* W, int32_t* R, int32_t* S, int32_t* theta, int* msb_g_out, int* msb_r_out,

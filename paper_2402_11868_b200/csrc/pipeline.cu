@@ -548,8 +548,7 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
     ZKD_CUDA_TRY(cudaStreamSynchronize(s));  // short-lived buffers are about to be reused
     c.ar.release(mark1);
     int32_t* Um = (int32_t*)c.ar.alloc(fxc);
-    int32_t* Xn = (int32_t*)c.ar.alloc(fxc);
-    if (!Um || !Xn) return ZKD_ERR_WORKSPACE;
+    if (!Um) return ZKD_ERR_WORKSPACE;
     ZKD_TRY(identity_blocks(n, nb, Um, s));
     const Arena::Mark mark2 = c.ar.mark();
     bool any = false;
