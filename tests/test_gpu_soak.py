@@ -113,9 +113,11 @@ def test_random_structures(zkd, seed, opts):
                     failures.append((tag, {k: round(float(v), 1) for k, v in c.items()}))
                     continue
                 if specs[i] is not None:
+                    # north_star: |dlam| <= 2^-740 ||A||_F, with ||A||_F^2 = sum lambda^2 exactly (A = Q diag(lambda) Q^H
+                    # up to the 2^-768 rounding of its entries): compared squared, in exact rationals
                     got = [zi.to_fraction(lam[i].reshape(N, -1)[j]) for j in range(N)]
-                    F = Fraction(2) ** int(np.ceil(c["log2_F"]))
-                    if not all(abs(g - w) <= F / 2 ** 738 for g, w in zip(got, specs[i])):
+                    F2 = sum(w * w for w in specs[i])
+                    if not all((g - w) ** 2 * 4 ** 740 <= F2 for g, w in zip(got, specs[i])):
                         failures.append((tag, "eigenvalue mismatch"))
     finally:
         for k, v in old.items():

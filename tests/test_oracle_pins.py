@@ -339,3 +339,138 @@ def test_clustered_spectrum_small(mp):
     c = oracle.compare(cfg["A"], N, lam, X, cfg["lam"], cfg["Q"])
     assert c["log2_dlam_rel"] <= -758 and c["log2_resid_rel"] <= -758 and c["log2_orth"] <= -758
     assert c["groups"] == N and c["vec_margin_bits"] <= -10
+
+
+# ------------------------------------------------------------------------------------------------------------
+# P11: the comparator's multi-member branch (SURVEY.md 8(c) comparator (iv), reading A10) — the part that certifies
+# exact multiplicities and near-degenerate groups.  Every expected value is evaluated in mpmath from the definition
+# E_G = X_G - X0_G (X0_G^H X_G), gap_G = distance from the group's extreme members to the nearest eigenvalue outside.
+def _random_unitary(mp, m, seed):
+    import random
+
+    rng = random.Random(seed)
+    Z = mp.matrix(m, m)
+    for i in range(m):
+        for j in range(m):
+            Z[i, j] = mp.mpc(rng.uniform(-1, 1), rng.uniform(-1, 1))
+    Qm, _ = mp.qr(Z)
+    return Qm
+
+
+def _groups_mp(mp, lam0, F):
+    """reading A10: a new group starts where the gap to the previous eigenvalue exceeds 2^-666 F"""
+    starts = [0]
+    for j in range(len(lam0) - 1):
+        if lam0[j + 1] - lam0[j] > mp.ldexp(F, -666):
+            starts.append(j + 1)
+    return starts + [len(lam0)]
+
+
+def _group_measures_mp(mp, lam0, X0, X, F):
+    """per group: (log2 ||E_G||_F, margin in bits against 2^-730 F / gap_G), definitions written out"""
+    N = len(lam0)
+    st = _groups_mp(mp, lam0, F)
+    out = []
+    for g in range(len(st) - 1):
+        a, b = st[g], st[g + 1]
+        m = b - a
+        M = mp.matrix(m, m)
+        for p in range(m):
+            for q in range(m):
+                M[p, q] = sum(mp.conj(X0[k, a + p]) * X[k, a + q] for k in range(N))
+        e2 = mp.mpf(0)
+        for k in range(N):
+            for q in range(m):
+                e2 += abs(X[k, a + q] - sum(X0[k, a + p] * M[p, q] for p in range(m))) ** 2
+        gaps = []
+        if a > 0:
+            gaps.append(lam0[a] - lam0[a - 1])
+        if b < N:
+            gaps.append(lam0[b] - lam0[b - 1])
+        le = log2abs(mp, mp.sqrt(e2))
+        out.append((le, le - (-730 + float(mp.log(F, 2)) - float(mp.log(min(gaps), 2))) if gaps else -1e9))
+    return out
+
+
+def test_P11_comparator_multi_member_groups(mp):
+    N = 8
+    t = Fraction(1, 2 ** 700)
+    vals = [Fraction(-1, 4), Fraction(0), t, 2 * t, Fraction(1, 2), Fraction(1, 2), Fraction(3, 4), Fraction(1)]
+    lamb = zi._lam_array(vals)
+    Ab, Qb = zi.qdq(N, 1111, 0, 3, lamb, want_q=True)
+    A = herm_from_upper(mp, zi.cmatrix_to_mp(Ab, N), N)
+    F = fro(mp, A)
+    Q = zi.cmatrix_to_mp(Qb, N)
+    lam0 = [mp.mpf(v.numerator) / v.denominator for v in vals]
+    assert _groups_mp(mp, lam0, F) == [0, 1, 4, 6, 7, 8]  # {-1/4} {0, t, 2t} {1/2, 1/2} {3/4} {1}
+
+    def run(Xm, cols=None):
+        Xb = zi.cmatrix_from_mp(Xm, N)
+        c = oracle.compare(Ab, N, lamb.reshape(-1), Xb, lamb.reshape(-1), Qb, cols=cols)
+        return c, zi.cmatrix_to_mp(Xb, N)  # the rounded candidate the comparator actually saw
+
+    # (a) a unitary remix inside each multi-member group (non-symmetric, complex: a transposed or conjugated index in
+    #     M = X0_G^H X_G would leave an O(1) error) changes nothing: E stays at the rounding level of the inputs
+    R = mp.eye(N)
+    U3, U2 = _random_unitary(mp, 3, 5), _random_unitary(mp, 2, 6)
+    for p in range(3):
+        for q in range(3):
+            R[1 + p, 1 + q] = U3[p, q]
+    for p in range(2):
+        for q in range(2):
+            R[4 + p, 4 + q] = U2[p, q]
+    X1 = Q * R
+    c, X1r = run(X1)
+    meas = _group_measures_mp(mp, lam0, Q, X1r, F)
+    assert c["groups"] == 5 and c["max_group"] == 3
+    assert c["log2_vec_err"] <= -760
+    assert abs(c["log2_vec_err"] - max(m[0] for m in meas)) < 0.01
+    assert abs(c["vec_margin_bits"] - max(m[1] for m in meas)) < 0.01
+    # without the remix the same measure is at the same level: the remix is invisible
+    c0, _ = run(Q)
+    assert c0["log2_vec_err"] <= -760
+
+    # (b) a 2^-700 leak out of the 3-member group (a component along an eigenvector outside it) is reported at 2^-700,
+    #     against the gap of that group's extreme members: min(0 - (-1/4), 1/2 - 2t) = 1/4
+    X2 = X1.copy()
+    for k in range(N):
+        X2[k, 2] += Q[k, 6] * mp.ldexp(mp.mpf(1), -700)
+    c, X2r = run(X2)
+    meas = _group_measures_mp(mp, lam0, Q, X2r, F)
+    assert abs(c["log2_vec_err"] - (-700)) < 0.01
+    assert abs(c["log2_vec_err"] - max(m[0] for m in meas)) < 0.01
+    want_margin = -700 - (-730 + float(mp.log(F, 2)) - (-2))
+    assert abs(c["vec_margin_bits"] - want_margin) < 0.01 and c["vec_margin_bits"] > 0
+    assert abs(c["vec_margin_bits"] - max(m[1] for m in meas)) < 0.01
+    # a leak INSIDE the group (along another member of the same group) is not an error of the subspace
+    X3 = X1.copy()
+    for k in range(N):
+        X3[k, 2] += Q[k, 3] * mp.ldexp(mp.mpf(1), -700)
+    c, X3r = run(X3)
+    assert c["log2_vec_err"] <= -760 and c["log2_orth"] > -702  # only orthonormality sees it
+
+    # (c) cols = [...]: residual and orthogonality are those of the chosen columns only (the leak sits in column 2)
+    lam_mp = lam0
+
+    def col_measures(Xm, j):
+        r = mp.sqrt(sum(abs(sum(A[i, k] * Xm[k, j] for k in range(N)) - lam_mp[j] * Xm[i, j]) ** 2 for i in range(N)))
+        o = max(abs(sum(mp.conj(Xm[k, i]) * Xm[k, j] for k in range(N)) - (1 if i == j else 0)) for i in range(N))
+        return log2abs(mp, r / F), log2abs(mp, o)
+
+    cfull, _ = run(X2)
+    for cols in ([2], [0, 5], [1, 2, 7]):
+        cc, _ = run(X2, cols=cols)
+        want_r = max(col_measures(X2r, j)[0] for j in cols)
+        want_o = max(col_measures(X2r, j)[1] for j in cols)
+        assert abs(cc["log2_resid_rel"] - want_r) < 0.01 and abs(cc["log2_orth"] - want_o) < 0.01, cols
+        # the group part is independent of cols
+        assert abs(cc["vec_margin_bits"] - cfull["vec_margin_bits"]) < 1e-9
+    assert abs(cfull["log2_resid_rel"] - max(col_measures(X2r, j)[0] for j in range(N))) < 0.01
+
+    # (d) one group spanning the whole spectrum (A = c I): any unitary X is correct, no gap exists
+    cI = zi.cmatrix_from_mp(mp.eye(5) * (mp.mpf(5) / 8), 5)
+    lamI = zi._lam_array([Fraction(5, 8)] * 5).reshape(-1)
+    XI = zi.cmatrix_from_mp(_random_unitary(mp, 5, 9), 5)
+    c = oracle.compare(cI, 5, lamI, XI, lamI, zi.cmatrix_from_mp(mp.eye(5), 5))
+    assert c["groups"] == 1 and c["max_group"] == 5 and c["vec_margin_bits"] < -1e8
+    assert c["log2_resid_rel"] <= -760 and c["log2_orth"] <= -760
