@@ -4,8 +4,9 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2] [--impl reference]
 
 One "step" = one pass of the whole hot path (S0 ingest .. S6 export) over one batch of seeded
-synthetic input through the C ABI (zkd_diag_herm_ws).  Default workload: BASELINE.json configs[1] = c2, one random
-Hermitian N=64 matrix at 768 bit (the paper's random-matrix timing, Fig. 1).  Prints ONE JSON line (rank 0).
+synthetic input through the C ABI (zkd_diag_herm_ws).  Default workload: c5 (BASELINE.json configs[4], N=1024, the
+largest single-GPU configuration of the metric "matrices/sec vs N": N=1024 is the largest N and one step carries the
+most digit products of the five configs); c1-c4 are reported as context rows.  Prints ONE JSON line (rank 0).
 
 Multi-GPU (torchrun): the path does not shard ("replicas only"): every rank runs the same workload on its
 own GPU with a different seed stream, no collective on the data path; value = matrices of all ranks / max-over-ranks
@@ -44,7 +45,7 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)  # the paper's 10-trial convention
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="c2", choices=sorted(WORKLOADS))
+    ap.add_argument("--workload", default="c5", choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="zkd", choices=["zkd", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the context rows (other configs, saturating batch)")
@@ -176,27 +177,74 @@ def measured_peaks() -> dict:
         return {}
 
 
-def roofline_object(gemm_ms, gemm_launches, gemm_macs, i8_ms, i8_launches, i8_macs, imad_peak, steps, total_ms) -> dict:
-    """The engine that carries most of the GEMM time.  IMAD path: digit products (IMAD.WIDE) per second against the live
-    microbenchmark.  int8 path: s8 x s8 MACs per second, x2 = op/s, against 2 x the measured dense bf16 peak of
-    MEASURED_PEAKS.json (int8 is nominally 2 x bf16 on B200; fallback: the profiling guide's nominal 4.5 PFLOP/s int8)."""
-    if i8_ms > gemm_ms:
-        mp = measured_peaks()
-        if "bf16_tflops" in mp:
-            peak_tops, src = 2.0 * float(mp["bf16_tflops"]), "2 x MEASURED_PEAKS.json bf16_tflops (burst; kernel timed alone per launch)"
+HBM_UNITS = ("prep_kernel", "combine_kernel", "slice_i8_kernel", "combine_i8_kernel", "ingest_export")
+IMAD_UNITS = ("gemm_digits_kernel", "singleton_step_kernel", "ecalc_kernel", "lu_kernels")
+
+
+def load_traffic(workload: str) -> dict:
+    """DRAM bytes per launch from the committed `ncu --set full` captures (profiles/traffic.json, written by hand from
+    the raw pages named there); {} when absent."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f).get(workload, {})
+    except (OSError, ValueError):
+        return {}
+
+
+def roofline_objects(cats: dict, seed_elems, imad_peak, dfma_peak, steps, total_ms, workload) -> list[dict]:
+    """One roofline object per kernel category that took part, largest share of the step first.
+    achieved = ALGORITHMIC work of the launches / their summed CUDA-event time; achieved_executed = the same with the
+    work the launches executed (instance / tile padding included).
+      digit kernels : 28x28-bit digit products (IMAD.WIDE) vs the live register-only IMAD.WIDE peak ("alu")
+      gemm_i8_kernel: s8 MACs x 2 = op/s vs 2 x the measured dense bf16 peak of MEASURED_PEAKS.json ("tensor")
+      seed_fp64     : fp64 flops (8 DFMA per element of a checked column pair + 12 per rotated one) vs the live DFMA peak
+      byte movers   : bytes vs the measured HBM copy bandwidth (they run out of L2 at these sizes: frac can exceed 1)"""
+    mp = measured_peaks()
+    traffic = load_traffic(workload)
+    out = []
+    for name, (ms, n, wexec, walg) in cats.items():
+        if n == 0 or ms <= 0:
+            continue
+        o = {"kernel": name, "launches_per_step": n / steps, "kernel_ms_per_step": ms / steps, "share_of_step": ms / total_ms,
+             "traffic": traffic.get(name)}
+        sec = ms * 1e-3
+        if name in IMAD_UNITS:
+            o.update({"bound": "alu", "unit": "TIMAD/s", "achieved": walg / sec / 1e12, "achieved_executed": wexec / sec / 1e12,
+                      "peak": imad_peak / 1e12, "work_per_step": walg / steps,
+                      "peak_source": "measured live (zkd_measure_imad_peak): register-only IMAD.WIDE loop, 64-bit accumulate"})
+        elif name == "gemm_i8_kernel":
+            if "bf16_tflops" in mp:
+                peak, src = 2.0 * float(mp["bf16_tflops"]), "2 x MEASURED_PEAKS.json bf16_tflops (burst; kernel timed alone per launch)"
+            else:
+                peak, src = 4500.0, "fallback: nominal dense int8 4.5 POP/s (B200_PROFILING.md); MEASURED_PEAKS.json absent"
+            o.update({"bound": "tensor", "unit": "TOP/s (int8)", "achieved": 2.0 * walg / sec / 1e12,
+                      "achieved_executed": 2.0 * wexec / sec / 1e12, "peak": peak, "work_per_step": walg / steps, "peak_source": src})
+        elif name == "seed_fp64":
+            chk, rot = seed_elems
+            flops = 2.0 * (8.0 * chk + 12.0 * rot)
+            # every checked pair also moves both columns through shared memory / L2 once in and (if rotated) once out
+            gbs = 16.0 * (2.0 * chk + 2.0 * rot) / sec / 1e9
+            o.update({"bound": "alu", "unit": "TFLOP/s (fp64)", "achieved": flops / sec / 1e12, "achieved_executed": flops / sec / 1e12,
+                      "peak": dfma_peak / 1e12, "work_per_step": flops / steps, "column_traffic_gbs": gbs,
+                      "hbm_gbs_peak": mp.get("hbm_gbs"),
+                      "peak_source": "measured live (zkd_measure_dfma_peak): register-only DFMA loop; column_traffic_gbs = bytes of "
+                                     "the column pairs read + written (shared memory / L2, not HBM) per second"})
+        elif name in HBM_UNITS:
+            peak = float(mp.get("hbm_gbs", 7700.0))
+            o.update({"bound": "hbm", "unit": "GB/s", "achieved": walg / sec / 1e9, "achieved_executed": wexec / sec / 1e9, "peak": peak,
+                      "work_per_step": walg / steps,
+                      "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in mp else "fallback 7700 GB/s nominal"})
         else:
-            peak_tops, src = 4500.0, "fallback: nominal dense int8 4.5 POP/s (B200_PROFILING.md); MEASURED_PEAKS.json absent"
-        achieved = 2.0 * i8_macs / (i8_ms * 1e-3) / 1e12
-        return {"bound": "tensor", "kernel": "gemm_i8_kernel", "achieved": achieved, "peak": peak_tops, "unit": "TOP/s (int8)",
-                "frac": achieved / peak_tops, "traffic": None, "launches": i8_launches, "kernel_ms_per_step": i8_ms / steps,
-                "share_of_step": i8_ms / total_ms, "int8_macs_per_step": i8_macs / steps, "peak_source": src,
-                "imad_gemm_ms_per_step": gemm_ms / steps}
-    achieved = gemm_macs / (gemm_ms * 1e-3) if gemm_ms > 0 else 0.0
-    return {"bound": "alu", "kernel": "gemm_digits_kernel", "achieved": achieved / 1e12, "peak": imad_peak / 1e12, "unit": "TIMAD/s",
-            "frac": achieved / imad_peak if imad_peak else None, "traffic": None, "launches": gemm_launches,
-            "kernel_ms_per_step": gemm_ms / steps, "share_of_step": gemm_ms / total_ms, "digit_macs_per_step": gemm_macs / steps,
-            "peak_source": "measured live (zkd_measure_imad_peak): IMAD.WIDE with 64-bit accumulate; nominal 32-bit IMAD rate "
-                           "148 SM x 64 lanes/clk x 1.965 GHz = 18.6"}
+            o.update({"bound": "latency", "unit": None, "achieved": None, "peak": None})
+        if o.get("achieved") is not None and o.get("peak"):
+            o["frac"] = o["achieved"] / o["peak"]
+            if "achieved_executed" in o:
+                o["frac_executed"] = o["achieved_executed"] / o["peak"]
+        else:
+            o["frac"] = None
+        out.append(o)
+    out.sort(key=lambda x: -x["share_of_step"])
+    return out
 
 
 def timed_steps(torch, runner_step, steps, flush):
@@ -273,6 +321,35 @@ def run_reference(args):
 # ---------------------------------------------------------------------------------------------------------------
 # main
 # ---------------------------------------------------------------------------------------------------------------
+def measure(torch, z, run, steps, flush, barrier, world, with_e2e=True):
+    """K timed steps (CUDA events on the launching stream, L2 flushed before every step outside the event pair, per-kernel
+    event pairs armed inside the library) and, under the same conditions, K steps through zkd_diag_herm_host."""
+    z.counters_reset()
+    z.seed_stats(reset=True)
+    z.kernel_timing(True)
+    barrier()
+    times = timed_steps(torch, run.step, steps, flush)
+    barrier()
+    launches, _ = z.counters()
+    cats = z.kernel_timing_read_all()
+    seed_elems = z.seed_stats(reset=True)
+    z.kernel_timing(False)
+    e2e_times = []
+    if with_e2e:
+        for _ in range(2):
+            run.step_e2e()
+        z.kernel_timing(True)  # same conditions as the device-timed loop: events armed, L2 flushed before every step
+        barrier()
+        for _ in range(steps):
+            flush.add_(1)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            run.step_e2e()  # synchronous: returns after the D2H copies completed
+            e2e_times.append(time.perf_counter() - t0)
+        z.kernel_timing(False)
+    return times, launches, cats, seed_elems, e2e_times
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
@@ -302,8 +379,8 @@ def main():
     N, b, A = make_workload(args.workload, rank)
     run = Runner(z, N, b, A)
     flush = torch.zeros(192 << 20, dtype=torch.uint8, device="cuda")  # 192 MiB > 126 MB L2
-
-    for _ in range(max(args.warmup, 3)):
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
         run.step()
     torch.cuda.synchronize()
 
@@ -311,30 +388,12 @@ def main():
     sampler = ClockSampler(local)
     sampler.start()
     time.sleep(0.3)
-    z.counters_reset()
-    z.kernel_timing(True)
-    barrier()
-    times = timed_steps(torch, run.step, args.steps, flush)
-    barrier()
-    launches, macs = z.counters()
-    gemm_ms, gemm_launches, gemm_macs = z.kernel_timing_read()
-    i8_ms, i8_launches, i8_macs = z.kernel_timing_read_i8()
-    z.kernel_timing(False)
+    times, launches, cats, seed_elems, e2e_times = measure(torch, z, run, args.steps, flush, barrier, world)
     clocks = sampler.stop()
     total_ms = sum(times)
     value, tmax = aggregate(world, b, args.steps, total_ms * 1e-3)
     total_ms_max = tmax * 1e3
-
-    # ---- e2e: host buffers through zkd_diag_herm_host -------------------------------------------------------------
-    for _ in range(2):
-        run.step_e2e()
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        run.step_e2e()  # synchronous: returns after the D2H copies completed
-    torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    e2e_value, _ = aggregate(world, b, args.steps, e2e_s)
+    e2e_value, _ = aggregate(world, b, args.steps, sum(e2e_times))
 
     if rank != 0:
         if world > 1:
@@ -342,45 +401,52 @@ def main():
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant GEMM engine: IMAD digit GEMM (integer-multiply pipe) or int8 tcgen05 (tensor pipe) ----
-    peak = z.measure_imad_peak(60.0)  # measured, register-only IMAD.WIDE loop on all SMs
-    roofline = roofline_object(gemm_ms, gemm_launches, gemm_macs, i8_ms, i8_launches, i8_macs, peak, args.steps, total_ms)
+    # ---- rooflines: every kernel category of the step, measured peaks ------------------------------------------------
+    imad_peak = z.measure_imad_peak(60.0)  # register-only IMAD.WIDE loop on all SMs
+    dfma_peak = z.measure_dfma_peak(40.0)  # register-only DFMA loop on all SMs
+    roofs = roofline_objects(cats, seed_elems, imad_peak, dfma_peak, args.steps, total_ms, args.workload)
+    listed = [r for r in roofs if r["share_of_step"] >= 0.02]
 
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warm,
         "ms_per_step": total_ms_max / args.steps, "ms_per_step_std": statistics.pstdev(times) if len(times) > 1 else 0.0,
         "ms_per_step_all": [round(t, 4) for t in times],
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32x30 (28-bit digits, 840-bit fixed point)",
         "data": "synthetic",
         "config": {"workload": WORKLOADS[args.workload], "N": N, "batch": b, "prec_bits": 768, "parallelism": "replicas only",
-                   "l2": "flushed between steps (192 MiB write)"},
+                   "l2": "flushed before every step (192 MiB write), device-timed and e2e legs alike",
+                   "kernel_events": "armed in both legs (one CUDA event pair per kernel launch inside the library)"},
         "eigenpairs_per_s": value * N,
         "clocks": clocks,
-        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": run.h2d_bytes, "d2h_bytes_per_step": run.d2h_bytes},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": run.h2d_bytes, "d2h_bytes_per_step": run.d2h_bytes,
+                "ms_per_step": 1e3 * sum(e2e_times) / max(1, len(e2e_times))},
         "gpu_launches": launches,
-        "roofline": roofline,
+        "roofline": listed[0] if listed else None,
+        "roofline_others": listed[1:],
+        "roofline_share_listed": sum(r["share_of_step"] for r in listed),
+        "whole_step_frac_of_imad_peak": (sum(r.get("work_per_step", 0) for r in roofs if r["kernel"] in IMAD_UNITS) * args.steps
+                                         / (total_ms * 1e-3) / imad_peak),
     }
 
     # ---- context rows: the other configs and a saturating batch (not the headline) --------------------------------
     if not args.no_extra and world == 1:
         extra = {}
-        for nm, bb, k in (("c1", 1, 5), ("c2", 1, 5), ("c2", 256, 3), ("c3", 1, 3), ("c4", 512, 2), ("c5", 1, 2)):
+        for nm, bb, k in (("c1", 1, 5), ("c2", 1, 5), ("c2", 256, 3), ("c3", 1, 5), ("c4", 512, 3), ("c5", 1, 3)):
             if nm == args.workload and bb == b:
                 continue
             try:
                 n2, b2, A2 = make_workload(nm, 0, batch=bb)
                 r2 = Runner(z, n2, b2, A2)
-                r2.step()
+                for _ in range(2):
+                    r2.step()
                 torch.cuda.synchronize()
-                z.kernel_timing(True)
-                ts = timed_steps(torch, r2.step, k, flush)
-                gms, gl, gm = z.kernel_timing_read()
-                g8 = z.kernel_timing_read_i8()
-                z.kernel_timing(False)
-                ms = sum(ts) / len(ts)
-                rf = roofline_object(gms, gl, gm, g8[0], g8[1], g8[2], peak, k, sum(ts))
-                extra[f"{nm}x{b2}"] = {"matrices_per_s": b2 / (ms * 1e-3), "ms_per_step": ms, "gemm_engine": rf["kernel"],
-                                       "gemm_share": rf["share_of_step"], "gemm_frac_of_peak": rf["frac"]}
+                ts0 = timed_steps(torch, r2.step, k, flush)  # kernel events disarmed: the row's own time
+                ts, _, c2, se2, _ = measure(torch, z, r2, k, flush, barrier, 1, with_e2e=False)
+                ms = sum(ts0) / len(ts0)
+                rf = [r for r in roofline_objects(c2, se2, imad_peak, dfma_peak, k, sum(ts), nm) if r["share_of_step"] >= 0.1]
+                extra[f"{nm}x{b2}"] = {"matrices_per_s": b2 / (ms * 1e-3), "ms_per_step": ms, "ms_per_step_events_armed": sum(ts) / len(ts),
+                                       "kernels": [{"kernel": r["kernel"], "share_of_step": round(r["share_of_step"], 4),
+                                                    "frac": r["frac"], "bound": r["bound"]} for r in rf]}
                 del r2
                 torch.cuda.empty_cache()
             except Exception as e:  # context only; never fails the bench line

@@ -113,6 +113,19 @@ int zkd_kernel_timing_read(double *gemm_ms, uint64_t *gemm_launches, uint64_t *g
  * its tcgen05.mma instructions performed (full 128 x 128 x 128 blocks, padding included). */
 int zkd_kernel_timing_read_i8(double *gemm_ms, uint64_t *gemm_launches, uint64_t *int8_macs);
 
+/* Per-category timing of EVERY kernel of the hot path (same arming as above): category indices 0 .. categories-1, each
+ * with a name (the kernel or kernel family), the summed device time of its launches, their number, and two work counts in
+ * the category's unit - "executed" (what the launches performed, tile and instance padding included) and "algorithmic"
+ * (what the requests needed).  Units: gemm_digits_kernel, singleton_step_kernel, ecalc_kernel, lu_kernels: 28x28-bit digit
+ * products; gemm_i8_kernel: s8 x s8 multiply-accumulates; prep / combine / slice / combine_i8 / ingest_export: bytes
+ * moved (algorithmic = executed); seed_fp64: 0 (use zkd_seed_stats).  Host calls. */
+int zkd_kernel_timing_categories(void);
+const char *zkd_kernel_timing_name(int category);
+int zkd_kernel_timing_read_cat(int category, double *ms, uint64_t *launches, uint64_t *work_executed, uint64_t *work_algorithmic);
+/* Work of the fp64 seed kernels (S1) since the last reset: column elements whose pair of columns was checked (three dot
+ * products = 8 DFMA per element) and elements whose pair was also rotated (12 more DFMA per element).  Synchronises. */
+int zkd_seed_stats(uint64_t *elems_checked, uint64_t *elems_rotated, int reset);
+
 /* ---- host-side helpers (no CUDA): one real between the API layout and (sign, exp, limbs) / double ---- */
 int zkd_pack(void *dst, int prec_bits, int sign, int64_t exp, const uint64_t *limbs_le);
 int zkd_unpack(const void *src, int prec_bits, int *sign, int64_t *exp, uint64_t *limbs_le);
@@ -151,6 +164,8 @@ int zkd_seed_fp64(int N, int batch, const double *A64, double *mu, double *V, vo
 /* Measured integer-multiply peak: runs a register-only IMAD.WIDE loop on every SM for about `millis`
  * milliseconds and returns wide (32x32+64) multiply-adds per second (host double). */
 int zkd_measure_imad_peak(double millis, double *imad_wide_per_sec, void *stream);
+/* Measured fp64 peak (roofline denominator of the seed): register-only DFMA loop on every SM; returns flop/s (2 per FMA). */
+int zkd_measure_dfma_peak(double millis, double *fp64_flops_per_sec, void *stream);
 
 #ifdef __cplusplus
 }

@@ -71,6 +71,13 @@ def lib() -> ctypes.CDLL:
     L.zkd_gemm_fx.argtypes = [ci, ci, ci, ci, ci, vp, ci, ci, vp, ci, ci, vp, ci, ci, ci, vp, cs, vp, vp, vp]
     L.zkd_seed_fp64.argtypes = [ci, ci, vp, vp, vp, vp]
     L.zkd_measure_imad_peak.argtypes = [cd, ctypes.POINTER(cd), vp]
+    L.zkd_measure_dfma_peak.argtypes = [cd, ctypes.POINTER(cd), vp]
+    L.zkd_seed_stats.argtypes = [ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint64), ci]
+    L.zkd_kernel_timing_categories.restype = ci
+    L.zkd_kernel_timing_name.restype = ctypes.c_char_p
+    L.zkd_kernel_timing_name.argtypes = [ci]
+    L.zkd_kernel_timing_read_cat.argtypes = [ci, ctypes.POINTER(cd), ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint64),
+                                             ctypes.POINTER(ctypes.c_uint64)]
     _lib = L
     return L
 
@@ -145,6 +152,34 @@ def kernel_timing_read_i8() -> tuple[float, int, int]:
     ms, n, m = ctypes.c_double(), ctypes.c_uint64(), ctypes.c_uint64()
     _check(lib().zkd_kernel_timing_read_i8(ctypes.byref(ms), ctypes.byref(n), ctypes.byref(m)), "zkd_kernel_timing_read_i8")
     return ms.value, int(n.value), int(m.value)
+
+
+def kernel_timing_categories() -> int:
+    return int(lib().zkd_kernel_timing_categories())
+
+
+def kernel_timing_name(category: int) -> str:
+    return lib().zkd_kernel_timing_name(category).decode()
+
+
+def kernel_timing_read_cat(category: int) -> tuple[float, int, int, int]:
+    """(summed kernel time in ms, timed launches, work executed, work algorithmic) of one kernel category"""
+    ms, n, we, wa = ctypes.c_double(), ctypes.c_uint64(), ctypes.c_uint64(), ctypes.c_uint64()
+    _check(lib().zkd_kernel_timing_read_cat(category, ctypes.byref(ms), ctypes.byref(n), ctypes.byref(we), ctypes.byref(wa)),
+           "zkd_kernel_timing_read_cat")
+    return ms.value, int(n.value), int(we.value), int(wa.value)
+
+
+def kernel_timing_read_all() -> dict:
+    """{category name: (ms, launches, work executed, work algorithmic)} for every kernel category of the library"""
+    return {kernel_timing_name(c): kernel_timing_read_cat(c) for c in range(kernel_timing_categories())}
+
+
+def seed_stats(reset: bool = False) -> tuple[int, int]:
+    """(column elements checked, column elements rotated) by the fp64 seed kernels since the last reset"""
+    a, b = ctypes.c_uint64(), ctypes.c_uint64()
+    _check(lib().zkd_seed_stats(ctypes.byref(a), ctypes.byref(b), 1 if reset else 0), "zkd_seed_stats")
+    return int(a.value), int(b.value)
 
 
 def diag_herm_bufsize(N: int, batch: int, prec_bits: int = PREC) -> int:
@@ -233,6 +268,12 @@ def seed_fp64(N: int, batch: int, A64, mu, V, stream=None) -> None:
 def measure_imad_peak(millis: float = 50.0, stream=None) -> float:
     v = ctypes.c_double()
     _check(lib().zkd_measure_imad_peak(millis, ctypes.byref(v), _stream_ptr(stream)), "zkd_measure_imad_peak")
+    return v.value
+
+
+def measure_dfma_peak(millis: float = 50.0, stream=None) -> float:
+    v = ctypes.c_double()
+    _check(lib().zkd_measure_dfma_peak(millis, ctypes.byref(v), _stream_ptr(stream)), "zkd_measure_dfma_peak")
     return v.value
 
 

@@ -5,6 +5,7 @@
 #include <cstring>
 
 #include "gemm_i8.h"
+#include "timing.h"
 #include "zkd_internal.h"
 
 namespace zkd {
@@ -99,6 +100,70 @@ int measure_imad_peak(double millis, double* per_sec, cudaStream_t s) {
   cudaEventDestroy(e1);
   cudaFree(d);
   *per_sec = best;
+  return ZKD_OK;
+}
+
+// ---- measured fp64 FMA peak (roofline denominator of the fp64 seed) -------------------------------------------------
+// Register-only loop of independent DFMA chains: 8 accumulators per thread, 1024 threads per SM.
+__global__ void __launch_bounds__(256) dfma_peak_kernel(double* out, double a0, double b0, int iters) {
+  double acc[8], a[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) { acc[i] = (double)i + (double)threadIdx.x; a[i] = a0 + 1e-9 * (double)(i + blockIdx.x); }
+  double b = b0;
+#pragma unroll 1
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) acc[i] = fma(acc[i], a[i], b);
+    }
+    b += 1e-12;
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s += acc[i];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+int measure_dfma_peak(double millis, double* flops_per_sec, cudaStream_t s) {
+  int dev = 0, sms = 0;
+  ZKD_CUDA_TRY(cudaGetDevice(&dev));
+  ZKD_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const int blocks = sms * 4, threads = 256;
+  double* d = nullptr;
+  ZKD_CUDA_TRY(cudaMalloc(&d, sizeof(double) * blocks * threads));
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  int iters = 2000;
+  double best = 0;
+  dfma_peak_kernel<<<blocks, threads, 0, s>>>(d, 0.999999, 1e-3, 200);  // warm-up
+  const int reps = millis > 20 ? 5 : 3;
+  for (int r = 0; r < reps + 1; ++r) {
+    cudaEventRecord(e0, s);
+    dfma_peak_kernel<<<blocks, threads, 0, s>>>(d, 0.999999, 1e-3, iters);
+    cudaEventRecord(e1, s);
+    if (cudaEventSynchronize(e1) != cudaSuccess) {
+      (void)cudaGetLastError();
+      cudaFree(d);
+      return ZKD_ERR_CUDA;
+    }
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double flops = (double)blocks * threads * (double)iters * 32.0 * 2.0;
+    if (r > 0 && flops / (ms * 1e-3) > best) best = flops / (ms * 1e-3);
+    if (r == 0 && ms > 0) {
+      double scale = (millis / reps) / ms;
+      if (scale > 50) scale = 50;
+      if (scale < 0.05) scale = 0.05;
+      iters = (int)(iters * scale) + 1;
+    }
+  }
+  count_launch(reps + 2);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(d);
+  *flops_per_sec = best;
   return ZKD_OK;
 }
 
@@ -264,6 +329,21 @@ int zkd_measure_imad_peak(double millis, double* imad_wide_per_sec, void* stream
   if (!imad_wide_per_sec || !(millis > 0)) return ZKD_ERR_INVALID_ARG;
   ZKD_TRY(check_device());
   return measure_imad_peak(millis, imad_wide_per_sec, (cudaStream_t)stream);
+}
+
+int zkd_measure_dfma_peak(double millis, double* fp64_flops_per_sec, void* stream) {
+  if (!fp64_flops_per_sec || !(millis > 0)) return ZKD_ERR_INVALID_ARG;
+  ZKD_TRY(check_device());
+  return measure_dfma_peak(millis, fp64_flops_per_sec, (cudaStream_t)stream);
+}
+int zkd_seed_stats(uint64_t* elems_checked, uint64_t* elems_rotated, int reset) {
+  ZKD_TRY(check_device());
+  return seed_stats(elems_checked, elems_rotated, reset != 0);
+}
+int zkd_kernel_timing_categories(void) { return KC_NUM; }
+const char* zkd_kernel_timing_name(int category) { return kcat_name(category); }
+int zkd_kernel_timing_read_cat(int category, double* ms, uint64_t* launches, uint64_t* work_executed, uint64_t* work_algorithmic) {
+  return kt_read(category, ms, launches, work_executed, work_algorithmic);
 }
 
 int zkd_kernel_timing(int enable) {

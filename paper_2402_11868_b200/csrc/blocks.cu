@@ -4,6 +4,7 @@
 // sorting, phase normalisation.  All multi-digit arithmetic is in-thread on FX digits (fx.cuh).
 #include "blocks.h"
 #include "fx.cuh"
+#include "timing.h"
 
 namespace zkd {
 
@@ -18,6 +19,7 @@ __global__ void __launch_bounds__(256) fxc_to_c64_kernel(size_t count, const int
   dst[e] = make_double2(re, fx_to_double(d));
 }
 int fxc_to_c64(size_t count, const int32_t* src, double2* dst, cudaStream_t s) {
+  KtScope kt_scope(KC_IO, s);
   fxc_to_c64_kernel<<<(unsigned)((count + 255) / 256), 256, 0, s>>>(count, src, dst);
   count_launch();
   return launch_check();
@@ -77,6 +79,7 @@ __global__ void __launch_bounds__(256) cluster_kernel(int n, const double2* __re
 }
 int cluster_detect(int n, int nb, const double2* A64, const double* mu, int tau_bits, const int* floor_msb, int* cl, int* cle,
                    int* stats, cudaStream_t s) {
+  KtScope kt_scope(KC_OTHER, s);
   cluster_kernel<<<nb, 256, sizeof(int) * (n + 1), s>>>(n, A64, mu, tau_bits, floor_msb, cl, cle, stats);
   count_launch();
   return launch_check();
@@ -99,6 +102,7 @@ __global__ void __launch_bounds__(256) init_x_kernel(size_t count, const double2
   fx_store(X + (size_t)ND * count, count, e, d);
 }
 int init_x(size_t count, const double2* V, int32_t* X, cudaStream_t s) {
+  KtScope kt_scope(KC_IO, s);
   init_x_kernel<<<(unsigned)((count + 255) / 256), 256, 0, s>>>(count, V, X);
   count_launch();
   return launch_check();
@@ -126,6 +130,7 @@ __global__ void __launch_bounds__(256) ns_build_kernel(int n, int nb, const int*
   fx_store(p, count, e, g);
 }
 int ns_build(int n, int nb, const int* cl, int32_t* G, int* msb_out, cudaStream_t s, const int* cle_skip1) {
+  KtScope kt_scope(KC_OTHER, s);
   const size_t t = (size_t)n * n * nb * 2;
   ns_build_kernel<<<(unsigned)((t + 255) / 256), 256, 0, s>>>(n, nb, cl, cle_skip1, G, msb_out);
   count_launch();
@@ -143,6 +148,7 @@ __global__ void __launch_bounds__(128) theta_kernel(int n, int nb, const int32_t
   fx_store(theta, (size_t)n * nb, t, d);
 }
 int theta_from_diag(int n, int nb, const int32_t* S, int32_t* theta, cudaStream_t s) {
+  KtScope kt_scope(KC_OTHER, s);
   theta_kernel<<<(unsigned)(((size_t)n * nb + 127) / 128), 128, 0, s>>>(n, nb, S, theta);
   count_launch();
   return launch_check();
@@ -164,6 +170,7 @@ __global__ void __launch_bounds__(128) min_gap_kernel(int n, int nb, const int32
   else atomicMax(gap_inv_out, 1024 - fx_msb(d));
 }
 int min_gap(int n, int nb, const int32_t* theta, const int* cl, int* gap_inv_out, cudaStream_t s) {
+  KtScope kt_scope(KC_OTHER, s);
   min_gap_kernel<<<(unsigned)(((size_t)n * nb + 127) / 128), 128, 0, s>>>(n, nb, theta, cl, gap_inv_out);
   count_launch();
   return launch_check();
@@ -185,6 +192,7 @@ __global__ void __launch_bounds__(256) fx_add_kernel(size_t reals, int32_t* __re
   fx_store(xp, count, idx, r);
 }
 int fxc_add_inplace(size_t count, int32_t* X, const int32_t* T, cudaStream_t s) {
+  KtScope kt_scope(KC_OTHER, s);
   fx_add_kernel<<<(unsigned)((2 * count + 255) / 256), 256, 0, s>>>(2 * count, X, T);
   count_launch();
   return launch_check();
@@ -603,6 +611,7 @@ __global__ void __launch_bounds__(512) singleton_step_warp_kernel(int n, int nb,
 
 int singleton_step(int n, int nb, int32_t* X, int32_t* W, int32_t* R, int32_t* S, int32_t* theta, int* msb_g_out, int* msb_r_out,
                    cudaStream_t s, const int* cl, const int* cle) {
+  KtScope kt_scope(KC_SSTEP, s, 14ull * 494ull * (uint64_t)n * n * nb);
   // columns per CTA: as many as keep about one CTA per SM (sector efficiency of the row-major loads against parallelism)
   const size_t cols = (size_t)n * nb;
   const int forced = options().sstep_cpb;
@@ -760,6 +769,9 @@ int ecalc(int n, int nb, const int32_t* theta, const int* cl, int32_t* C, int pr
   // Newton doubles the ~50 correct bits of the fp64 start each iteration
   int iters = 0;
   for (int have = 48; have < prec_bits; have *= 2) ++iters;
+  // digit products per pair i < j: two (W+1)^2-digit products per Newton iteration (half of them kept) and four 30 x (W+1) products
+  const uint64_t Wd = prec_bits <= 28 * 4 - 8 ? 5 : prec_bits <= 28 * 8 - 8 ? 9 : prec_bits <= 28 * 16 - 8 ? 17 : 30;
+  KtScope kt_scope(KC_ECALC, s, (uint64_t)n * (n - 1) / 2 * nb * ((uint64_t)iters * Wd * (Wd + 3) + 4ull * ND * Wd));
   if (prec_bits <= 28 * 4 - 8) ecalc_kernel<4><<<blocks, 128, 0, s>>>(n, nb, theta, cl, C, iters, msb_out, err_flag);
   else if (prec_bits <= 28 * 8 - 8) ecalc_kernel<8><<<blocks, 128, 0, s>>>(n, nb, theta, cl, C, iters, msb_out, err_flag);
   else if (prec_bits <= 28 * 16 - 8) ecalc_kernel<16><<<blocks, 128, 0, s>>>(n, nb, theta, cl, C, iters, msb_out, err_flag);

@@ -5,6 +5,7 @@
 
 #include "blocks.h"
 #include "fx_api.cuh"
+#include "timing.h"
 
 namespace zkd {
 
@@ -64,6 +65,7 @@ __global__ void __launch_bounds__(128) ingest_kernel(int N, int batch, const uin
 }
 
 int ingest_herm(int N, int batch, const void* A_api, int32_t* A_fx, int* scale /* 2 * batch ints */, int* status, cudaStream_t s) {
+  KtScope kt_scope(KC_IO, s);
   int* rawmax = scale + batch;
   ZKD_CUDA_TRY(cudaMemsetAsync(rawmax, 0x80, sizeof(int) * batch, s));
   ZKD_CUDA_TRY(cudaMemsetAsync(status, 0, sizeof(int) * batch, s));
@@ -190,6 +192,7 @@ __global__ void __launch_bounds__(128) sub_gather_kernel(int n, int nb, int m, c
 int sub_gather(int n, int nb, int m, int nsub, const SubProblem* subs_dev, const int32_t* S, int32_t* H, int32_t* cbar, int* kshift,
                int* degenerate, int degenerate_msb, const int* noise_parent, int* noise_child, int* floor_child, int min_split_msb,
                cudaStream_t s) {
+  KtScope kt_scope(KC_OTHER, s);
   sub_gather_kernel<<<nsub, 128, 0, s>>>(n, nb, m, subs_dev, S, H, cbar, kshift, degenerate, degenerate_msb, noise_parent,
                                          noise_child, floor_child, min_split_msb, nsub);
   count_launch();
@@ -209,6 +212,7 @@ __global__ void __launch_bounds__(256) identity_blocks_kernel(size_t count, int 
   fx_store(Um + (part ? (size_t)ND * count : 0), count, e, d);
 }
 int identity_blocks(int n, int nb, int32_t* Um, cudaStream_t s) {
+  KtScope kt_scope(KC_OTHER, s);
   const size_t count = (size_t)n * n * nb;
   identity_blocks_kernel<<<(unsigned)((2 * count + 255) / 256), 256, 0, s>>>(count, n, Um);
   count_launch();
@@ -242,6 +246,7 @@ __global__ void __launch_bounds__(128) sub_scatter_kernel(int n, int nb, int m, 
 }
 int sub_scatter(int n, int nb, int m, int nsub, const SubProblem* subs_dev, const int32_t* U, const int32_t* lam_sub,
                 const int32_t* cbar, const int* kshift, const int* degenerate, int32_t* Um, int32_t* theta, cudaStream_t s) {
+  KtScope kt_scope(KC_OTHER, s);
   sub_scatter_kernel<<<nsub, 128, 0, s>>>(n, nb, m, nsub, subs_dev, U, lam_sub, cbar, kshift, degenerate, Um, theta);
   count_launch();
   return launch_check();
@@ -273,6 +278,7 @@ __global__ void __launch_bounds__(128) split_scatter_kernel(int n, int nb, int m
 }
 int split_scatter(int n, int nb, int m, int nsub, const SubProblem* subs_dev, const double2* V64, const int* sub_cl,
                   const int* sub_cle, const int* degenerate, int32_t* Um, int* cl, int* cle, cudaStream_t s) {
+  KtScope kt_scope(KC_OTHER, s);
   split_scatter_kernel<<<nsub, 128, 0, s>>>(n, nb, m, nsub, subs_dev, V64, sub_cl, sub_cle, degenerate, Um, cl, cle);
   count_launch();
   return launch_check();
@@ -442,6 +448,7 @@ __global__ void __launch_bounds__(128) phase_kernel(int N, int batch, const int3
 
 int finalize_export(int N, int batch, const int32_t* X, const int32_t* lam, const int* scale, void* eigvals_api, void* eigvecs_api,
                     int32_t* scratch, int32_t* lam_sorted, int* rank, cudaStream_t s) {
+  KtScope kt_scope(KC_IO, s);
   const size_t nl = (size_t)N * batch;
   rank_kernel<<<(unsigned)((nl + 127) / 128), 128, 0, s>>>(N, batch, lam, rank, lam_sorted);
   phase_kernel<<<(unsigned)((nl * 32 + 127) / 128), 128, 0, s>>>(N, batch, X, rank, scratch);

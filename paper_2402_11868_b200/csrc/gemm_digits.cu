@@ -10,6 +10,7 @@
 
 #include "gemm_digits.cuh"
 #include "gemm_i8.h"
+#include "timing.h"
 #include "zkd_internal.h"
 
 namespace zkd {
@@ -36,6 +37,16 @@ static uint64_t inst_cost(const GemmInstance& in) {
   for (int a = 0; a < in.np; ++a)
     for (int b = 0; b < in.nq; ++b)
       if (a + b >= in.low) ++c;
+  return c;
+}
+
+// digit products per (i,j,k) the REQUEST needs: its own windows with the truncation rule applied to them (no instance padding)
+static uint64_t request_cost(int nwP, int nwQ) {
+  const int low = nwQ >= 2 ? nwQ - 2 : 0;
+  uint64_t c = 0;
+  for (int a = 0; a < nwP; ++a)
+    for (int b = 0; b < nwQ; ++b)
+      if (a + b >= low) ++c;
   return c;
 }
 
@@ -519,59 +530,8 @@ __global__ void __launch_bounds__(256) combine_warp_kernel(CombineArgs a) {
 
 // ---- host side ----------------------------------------------------------------------------------------------------
 
-// Optional per-launch timing of the digit GEMM kernel (zkd_kernel_timing): event pairs on the launching stream.
-namespace {
-struct KernelTimer {
-  bool enabled = false;
-  std::vector<cudaEvent_t> ev;   // pairs
-  std::vector<uint64_t> macs;    // per timed launch
-  size_t used = 0;               // pairs used
-  uint64_t untimed = 0;
-};
-KernelTimer g_kt;
-constexpr size_t kMaxTimedLaunches = 16384;
-}  // namespace
-
-void kernel_timing_enable(bool on) {
-  kernel_timing_enable_i8(on);
-  g_kt.enabled = on;
-  g_kt.used = 0;
-  g_kt.untimed = 0;
-  g_kt.macs.clear();
-}
-int kernel_timing_read(double* ms, uint64_t* launches, uint64_t* macs) {
-  double tot = 0;
-  uint64_t m = 0;
-  for (size_t i = 0; i < g_kt.used; ++i) {
-    float t = 0;
-    if (cudaEventSynchronize(g_kt.ev[2 * i + 1]) != cudaSuccess || cudaEventElapsedTime(&t, g_kt.ev[2 * i], g_kt.ev[2 * i + 1]) != cudaSuccess) {
-      (void)cudaGetLastError();
-      return ZKD_ERR_CUDA;
-    }
-    tot += t;
-    m += g_kt.macs[i];
-  }
-  if (ms) *ms = tot;
-  if (launches) *launches = g_kt.used;
-  if (macs) *macs = m;
-  return ZKD_OK;
-}
-static bool kt_begin(cudaStream_t s) {
-  if (!g_kt.enabled) return false;
-  if (g_kt.used >= kMaxTimedLaunches) { ++g_kt.untimed; return false; }
-  while (g_kt.ev.size() < 2 * (g_kt.used + 1)) {
-    cudaEvent_t e;
-    if (cudaEventCreate(&e) != cudaSuccess) { (void)cudaGetLastError(); return false; }
-    g_kt.ev.push_back(e);
-  }
-  cudaEventRecord(g_kt.ev[2 * g_kt.used], s);
-  return true;
-}
-static void kt_end(cudaStream_t s, uint64_t macs) {
-  cudaEventRecord(g_kt.ev[2 * g_kt.used + 1], s);
-  g_kt.macs.push_back(macs);
-  ++g_kt.used;
-}
+void kernel_timing_enable(bool on) { kt_enable(on); }
+int kernel_timing_read(double* ms, uint64_t* launches, uint64_t* macs) { return kt_read(KC_GEMM_DIGITS, ms, launches, macs, nullptr); }
 
 static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
@@ -640,7 +600,12 @@ int gemm_complex(int M, int N, int K, int batch, const GemmSide& P, const GemmSi
     qa.ld = Q.ld ? Q.ld : N; qa.off = Q.off;
     qa.transpose = 0; qa.side = 1; qa.lsb_bit = lsbQ; qa.nw = nqad; qa.nw_src = Q.nw; qa.err_flag = err_flag;
     const size_t tot = (size_t)batch * K * (size_t)(M > N ? M : N);
-    prep_kernel<<<dim3((unsigned)((tot + 255) / 256), 2), 256, 0, stream>>>(both);
+    {
+      // bytes: the source windows read (re + im) and the three compact planes written, both operands
+      const uint64_t bytes = 4ull * batch * ((uint64_t)M * K * (2 * (P.nw + 1) + 3 * npad) + (uint64_t)K * N * (2 * (Q.nw + 1) + 3 * nqad));
+      KtScope kt(KC_PREP, stream, bytes);
+      prep_kernel<<<dim3((unsigned)((tot + 255) / 256), 2), 256, 0, stream>>>(both);
+    }
     count_launch();
   }
   if (use_i8)
@@ -657,9 +622,10 @@ int gemm_complex(int M, int N, int K, int batch, const GemmSide& P, const GemmSi
   ka.M = M; ka.N = N; ka.K = K; ka.G = 3 * batch; ka.ksplit = ksplit; ka.nsplit = nsp;
   dim3 grid((N + GT - 1) / GT, (M + GT - 1) / GT, (unsigned)(3 * batch * nsp));
   const uint64_t nmacs = inst_cost(*in) * 3ull * (uint64_t)batch * M * N * K;
-  const bool timed = kt_begin(stream);
-  if (in->launch(ka, grid, stream) != cudaSuccess) return ZKD_ERR_CUDA;
-  if (timed) kt_end(stream, nmacs);
+  {
+    KtScope kt(KC_GEMM_DIGITS, stream, nmacs, request_cost(P.nw, Q.nw) * 3ull * (uint64_t)batch * M * N * K);
+    if (in->launch(ka, grid, stream) != cudaSuccess) return ZKD_ERR_CUDA;
+  }
   count_launch();
   count_macs(nmacs);
 
@@ -674,6 +640,8 @@ int gemm_complex(int M, int N, int K, int batch, const GemmSide& P, const GemmSi
   // the warp-cooperative kernel wins only while the digit-serial one cannot fill the machine (measured: c2 2.47 -> 2.40 ms,
   // but c4 244 -> 316 ms when forced)
   const int cpath = options().combine_path;
+  // bytes: raw columns read (two of the three planes per part, every split) + the FX digits written (+ read when accumulating)
+  KtScope kt(KC_COMBINE, stream, 4ull * batch * M * N * ((uint64_t)nsp * 3 * in->nc + 2ull * kND * (mode == GemmMode::Assign ? 1 : 2)));
   if (cpath == 2 || (cpath == 0 && tot <= 32768)) {
     const size_t warps = ((size_t)M * N + EPW - 1) / EPW * batch;
     combine_warp_kernel<<<dim3((unsigned)((warps * 32 + 255) / 256), 2), 256, 0, stream>>>(ca);

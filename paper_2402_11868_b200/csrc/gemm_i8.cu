@@ -17,6 +17,7 @@
 
 #include "fx.cuh"
 #include "gemm_i8.h"
+#include "timing.h"
 
 namespace zkd {
 
@@ -465,14 +466,6 @@ inline int slices_for(int nw) { return (DB * nw + 8) / 8; }
 constexpr int kMaxSlices = (DB * ND + 8) / 8;  // 106
 constexpr int kMaxCols = 128;                  // kept columns: <= nsP + nsQ - 1 - dcut <= 106 + 8 + ... (checked at run time)
 
-struct Timer {
-  bool enabled = false;
-  std::vector<cudaEvent_t> ev;
-  std::vector<uint64_t> macs;
-  size_t used = 0;
-};
-Timer g_t;
-
 int pick_nsplit(int K, int nsmin) {
   // |S_d| <= Ksplit * nsmin * 2^14 must stay below 2^31
   const int nkb = (K + I8_BK - 1) / I8_BK;
@@ -483,29 +476,8 @@ int pick_nsplit(int K, int nsmin) {
 
 }  // namespace
 
-void kernel_timing_enable_i8(bool on) {
-  g_t.enabled = on;
-  g_t.used = 0;
-  g_t.macs.clear();
-}
-int kernel_timing_read_i8(double* ms, uint64_t* launches, uint64_t* macs) {
-  double tot = 0;
-  uint64_t m = 0;
-  for (size_t i = 0; i < g_t.used; ++i) {
-    float t = 0;
-    if (cudaEventSynchronize(g_t.ev[2 * i + 1]) != cudaSuccess ||
-        cudaEventElapsedTime(&t, g_t.ev[2 * i], g_t.ev[2 * i + 1]) != cudaSuccess) {
-      (void)cudaGetLastError();
-      return ZKD_ERR_CUDA;
-    }
-    tot += t;
-    m += g_t.macs[i];
-  }
-  if (ms) *ms = tot;
-  if (launches) *launches = g_t.used;
-  if (macs) *macs = m;
-  return ZKD_OK;
-}
+void kernel_timing_enable_i8(bool on) { (void)on; }
+int kernel_timing_read_i8(double* ms, uint64_t* launches, uint64_t* macs) { return kt_read(KC_GEMM_I8, ms, launches, macs, nullptr); }
 
 bool gemm_i8_eligible(int path, int M, int N, int K, int batch) {
   (void)batch;
@@ -547,11 +519,17 @@ int gemm_i8_finish(int M, int N, int K, int batch, const int32_t* Pc, const int3
     sa.src = Pc; sa.dst = P8; sa.R = M; sa.C = K; sa.G = G; sa.nw = np; sa.ns = nsP; sa.rows = M; sa.K = K; sa.Kp = Kp;
     sa.transpose = 0; sa.err_flag = err_flag;
     size_t tot = (size_t)G * M * Kp;
-    slice_i8_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(sa);
+    {
+      KtScope kt(KC_SLICE_I8, stream, (uint64_t)G * M * K * 4ull * np + (uint64_t)tot * nsP);
+      slice_i8_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(sa);
+    }
     count_launch();
     sa.src = Qc; sa.dst = Q8; sa.R = K; sa.C = N; sa.nw = nq; sa.ns = nsQ; sa.rows = N; sa.transpose = 1;
     tot = (size_t)G * N * Kp;
-    slice_i8_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(sa);
+    {
+      KtScope kt(KC_SLICE_I8, stream, (uint64_t)G * N * K * 4ull * nq + (uint64_t)tot * nsQ);
+      slice_i8_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(sa);
+    }
     count_launch();
   }
   CUtensorMap mapP, mapQ;
@@ -581,23 +559,10 @@ int gemm_i8_finish(int M, int N, int K, int batch, const int32_t* Pc, const int3
     for (int y = 0; y < nsQ; ++y)
       if (x + y >= dcut) ++pairs;
   const uint64_t macs = pairs * (uint64_t)G * grid.x * grid.y * ka.nkb * I8_BM * I8_BN * I8_BK;
-  bool timed = false;
-  if (g_t.enabled && g_t.used < 16384) {
-    while (g_t.ev.size() < 2 * (g_t.used + 1)) {
-      cudaEvent_t ev;
-      if (cudaEventCreate(&ev) != cudaSuccess) { (void)cudaGetLastError(); break; }
-      g_t.ev.push_back(ev);
-    }
-    if (g_t.ev.size() >= 2 * (g_t.used + 1)) {
-      cudaEventRecord(g_t.ev[2 * g_t.used], stream);
-      timed = true;
-    }
-  }
-  gemm_i8_kernel<<<grid, I8_THREADS, I8_SMEM, stream>>>(mapP, mapQ, ka);
-  if (timed) {
-    cudaEventRecord(g_t.ev[2 * g_t.used + 1], stream);
-    g_t.macs.push_back(macs);
-    ++g_t.used;
+  {
+    // algorithmic: the same slice pairs on the matrices as they are (no padding of M, N, K to 128)
+    KtScope kt(KC_GEMM_I8, stream, macs, pairs * (uint64_t)G * M * N * K);
+    gemm_i8_kernel<<<grid, I8_THREADS, I8_SMEM, stream>>>(mapP, mapQ, ka);
   }
   count_launch();
   count_i8_macs(macs);
@@ -610,6 +575,7 @@ int gemm_i8_finish(int M, int N, int K, int batch, const int32_t* Pc, const int3
   ca.base_bit = lsbP + lsbQ - FRAC + 8 * dcut;
   ca.cut_bit = cut_bit; ca.mode = mode; ca.msb_out = msb_out;
   const size_t tot = (size_t)batch * M * N;
+  KtScope kt(KC_COMBINE_I8, stream, 4ull * tot * ((uint64_t)ka.nsplit * 3 * ncol + 2ull * ND * (mode == 0 ? 1 : 2)));
   combine_i8_kernel<<<dim3((unsigned)((tot + 255) / 256), 2), 256, 0, stream>>>(ca);
   count_launch();
   return launch_check();

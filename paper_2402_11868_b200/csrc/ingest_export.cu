@@ -4,6 +4,7 @@
 // FX real: 30 digits of 28 bits, value = int * 2^-812 (fx.cuh).  One thread per number; the AoS side is read /
 // written with 16-byte accesses, the SoA side is coalesced across threads.
 #include "fx_api.cuh"
+#include "timing.h"
 
 namespace zkd {
 
@@ -105,6 +106,7 @@ __global__ void __launch_bounds__(128) fx_to_api_kernel(size_t count, const int3
 
 int fx_from_api_scaled(size_t count, const void* src_api, int32_t* dst_fx, int scale_bits, const int* scale_dev,
                        int scale_stride, size_t per_scale, int* status, cudaStream_t s) {
+  KtScope kt_scope(KC_IO, s);
   if (count == 0) return ZKD_OK;
   fx_from_api_kernel<<<(unsigned)((count + 127) / 128), 128, 0, s>>>(count, (const uint8_t*)src_api, dst_fx, scale_bits,
                                                                      scale_dev, scale_stride, per_scale ? per_scale : 1, status);
@@ -113,6 +115,7 @@ int fx_from_api_scaled(size_t count, const void* src_api, int32_t* dst_fx, int s
 }
 int fx_to_api_scaled(size_t count, const int32_t* src_fx, void* dst_api, int scale_bits, const int* scale_dev, int scale_stride,
                      size_t per_scale, cudaStream_t s) {
+  KtScope kt_scope(KC_IO, s);
   if (count == 0) return ZKD_OK;
   fx_to_api_kernel<<<(unsigned)((count + 127) / 128), 128, 0, s>>>(count, src_fx, (uint8_t*)dst_api, 1, 0, scale_bits, scale_dev,
                                                                    scale_stride, per_scale ? per_scale : 1);
@@ -121,6 +124,7 @@ int fx_to_api_scaled(size_t count, const int32_t* src_fx, void* dst_api, int sca
 }
 // complex FX array (re planes, im planes) -> interleaved (re, im) API numbers
 int fxc_to_api(size_t count, const int32_t* src_fxc, void* dst_api, cudaStream_t s) {
+  KtScope kt_scope(KC_IO, s);
   if (count == 0) return ZKD_OK;
   for (int part = 0; part < 2; ++part)
     fx_to_api_kernel<<<(unsigned)((count + 127) / 128), 128, 0, s>>>(count, src_fxc + (size_t)part * ND * count, (uint8_t*)dst_api,

@@ -17,6 +17,7 @@
 // The seed only has to be good to ~2^-40 (the refinement squares the error every step).
 #include <cooperative_groups.h>
 
+#include "timing.h"
 #include "zkd_internal.h"
 
 namespace cg = cooperative_groups;
@@ -24,6 +25,14 @@ namespace cg = cooperative_groups;
 namespace zkd {
 
 constexpr double kSeedStopCos2 = 8.8817841970012523e-16;  // 2^-50
+
+// Work counters for the roofline of the seed (zkd_seed_stats): column ELEMENTS whose pair was checked (three dot products:
+// 8 DFMA per element) and elements whose pair was also rotated (12 more), summed over all launches since the last reset.
+__device__ unsigned long long g_seed_stats[2];
+__device__ __forceinline__ void seed_count(unsigned long long chk, unsigned long long rot) {
+  if (chk) atomicAdd(&g_seed_stats[0], chk);
+  if (rot) atomicAdd(&g_seed_stats[1], rot);
+}
 
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
@@ -162,6 +171,7 @@ seed_ring_kernel(int n, int wpc, const double2* __restrict__ A, double* __restri
   cluster.sync();
 
   if (n > 1 && sigma > 0) {
+    unsigned long long nchk = 0, nrot = 0;
     for (int sweep = 0; sweep < max_sweeps; ++sweep) {
       double cmax = 0;
       for (int r = 0; r < M - 1; ++r) {
@@ -191,7 +201,9 @@ seed_ring_kernel(int n, int wpc, const double2* __restrict__ A, double* __restri
           }
           al = warp_sum(al); be = warp_sum(be); gr = warp_sum(gr); gi = warp_sum(gi);
           double c, sr, si, cos2;
+          nchk += n;
           if (rot_params(al, be, gr, gi, tol2, c, sr, si, cos2)) {
+            nrot += n;
             cmax = fmax(cmax, cos2);
 #pragma unroll
             for (int q = 0; q < EPL; ++q) {
@@ -225,6 +237,7 @@ seed_ring_kernel(int n, int wpc, const double2* __restrict__ A, double* __restri
       __syncthreads();
       if (!(worst > kSeedStopCos2)) break;
     }
+    if (lane == 0) seed_count(nchk, nrot);
   }
   cluster.sync();
   // the final columns sit in slot set `cur`
@@ -306,7 +319,10 @@ static int launch_ring(int N, int batch, int csize, const double2* A, double* mu
   at[0].val.clusterDim.z = 1;
   cfg.attrs = at;
   cfg.numAttrs = 1;
-  ZKD_CUDA_TRY(cudaLaunchKernelEx(&cfg, seed_ring_kernel<EPL>, N, wpc, A, mu, V, max_sweeps, tol2, dbuf));
+  {
+    KtScope kt(KC_SEED, s);
+    ZKD_CUDA_TRY(cudaLaunchKernelEx(&cfg, seed_ring_kernel<EPL>, N, wpc, A, mu, V, max_sweeps, tol2, dbuf));
+  }
   count_launch();
   return launch_check();
 }
@@ -357,6 +373,7 @@ seed_cta_kernel(int n, const double2* __restrict__ A, double* __restrict__ mu, d
 
   const int M = n + (n & 1), npairs = M / 2;
   if (n > 1 && sigma > 0) {
+    unsigned long long nchk = 0, nrot = 0;
     for (int sweep = 0; sweep < max_sweeps; ++sweep) {
       double cmax = 0;
       for (int r = 0; r < M - 1; ++r) {
@@ -383,7 +400,9 @@ seed_cta_kernel(int n, const double2* __restrict__ A, double* __restrict__ mu, d
           }
           al = warp_sum(al); be = warp_sum(be); gr = warp_sum(gr); gi = warp_sum(gi);
           double c, sr, si, cos2;
+          nchk += n;
           if (!rot_params(al, be, gr, gi, tol2, c, sr, si, cos2)) continue;
+          nrot += n;
           cmax = fmax(cmax, cos2);
 #pragma unroll
           for (int k = 0; k < EPL; ++k) {
@@ -402,6 +421,7 @@ seed_cta_kernel(int n, const double2* __restrict__ A, double* __restrict__ mu, d
       if (tid == 0) s_cmax[(sweep + 1) & 1] = 0ull;
       if (!(worst > kSeedStopCos2)) break;
     }
+    if (lane == 0) seed_count(nchk, nrot);
   }
   __syncthreads();
   for (int j = warp; j < n; j += nwarps) {
@@ -442,7 +462,10 @@ static int launch_cta(int N, int batch, const double2* A, double* mu, double2* V
     ZKD_CUDA_TRY(cudaFuncSetAttribute(seed_cta_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     attr_smem = smem;
   }
-  seed_cta_kernel<EPL><<<batch, 32 * warps, smem, s>>>(N, A, mu, V, max_sweeps, tol2);
+  {
+    KtScope kt(KC_SEED, s);
+    seed_cta_kernel<EPL><<<batch, 32 * warps, smem, s>>>(N, A, mu, V, max_sweeps, tol2);
+  }
   count_launch();
   return launch_check();
 }
@@ -471,7 +494,8 @@ __global__ void seed_sigma_kernel(int n, const double2* __restrict__ A, double* 
 }
 
 // one warp: orthogonalise columns p, q of G (length n, global memory)
-__device__ __forceinline__ double rotate_pair_global(double2* __restrict__ gp, double2* __restrict__ gq, int n, int lane, double tol2) {
+__device__ __forceinline__ double rotate_pair_global(double2* __restrict__ gp, double2* __restrict__ gq, int n, int lane, double tol2,
+                                                     unsigned long long& nchk, unsigned long long& nrot) {
   double al = 0, be = 0, gr = 0, gi = 0;
   for (int i = lane; i < n; i += 32) {
     const double2 a = __ldcg(gp + i), b = __ldcg(gq + i);
@@ -482,7 +506,9 @@ __device__ __forceinline__ double rotate_pair_global(double2* __restrict__ gp, d
   }
   al = warp_sum(al); be = warp_sum(be); gr = warp_sum(gr); gi = warp_sum(gi);
   double c, sr, si, cos2;
+  nchk += n;
   if (!rot_params(al, be, gr, gi, tol2, c, sr, si, cos2)) return cos2;
+  nrot += n;
   for (int i = lane; i < n; i += 32) {
     const double2 a = __ldcg(gp + i), b = __ldcg(gq + i);
     __stcg(gp + i, make_double2(c * a.x - (sr * b.x + si * b.y), c * a.y - (sr * b.y - si * b.x)));
@@ -509,6 +535,7 @@ __global__ void __launch_bounds__(128) seed_large_kernel(int n, const double2* _
   if (gtid < (size_t)max_sweeps) rot_flags[gtid] = 0;
   grid.sync();
   const int M = n + (n & 1), npairs = M / 2;
+  unsigned long long nchk = 0, nrot = 0;
   if (sigma > 0) {
     for (int sweep = 0; sweep < max_sweeps; ++sweep) {
       double cmax = 0;
@@ -516,7 +543,7 @@ __global__ void __launch_bounds__(128) seed_large_kernel(int n, const double2* _
         for (int i = gwarp; i < npairs; i += nwarps) {
           int p, q;
           rr_pair(M, r, i, p, q);
-          if (q < n) cmax = fmax(cmax, rotate_pair_global(G + (size_t)p * n, G + (size_t)q * n, n, lane, tol2));
+          if (q < n) cmax = fmax(cmax, rotate_pair_global(G + (size_t)p * n, G + (size_t)q * n, n, lane, tol2, nchk, nrot));
         }
         if (r == M - 2 && cmax > kSeedStopCos2 && lane == 0) rot_flags[sweep] = 1;
         grid.sync();
@@ -524,6 +551,7 @@ __global__ void __launch_bounds__(128) seed_large_kernel(int n, const double2* _
       if (!rot_flags[sweep]) break;
     }
   }
+  if (lane == 0) seed_count(nchk, nrot);
   for (int j = gwarp; j < n; j += nwarps) {
     double s = 0;
     for (int i = lane; i < n; i += 32) { const double2 a = G[(size_t)j * n + i]; s += a.x * a.x + a.y * a.y; }
@@ -541,7 +569,8 @@ __global__ void __launch_bounds__(128) seed_large_kernel(int n, const double2* _
 // shared memory (s_red: [4 * WPP] doubles of this pair).  Contains one __syncthreads when WPP > 1: every warp of the CTA calls it.
 template <int WPP>
 __device__ __forceinline__ double rotate_pair_smem(double2* __restrict__ gp, double2* __restrict__ gq, int n, int lane, int part,
-                                                   double* __restrict__ s_red, double tol2) {
+                                                   double* __restrict__ s_red, double tol2, unsigned long long& nchk,
+                                                   unsigned long long& nrot) {
   const int chunk = (n + WPP - 1) / WPP;
   const int i0 = part * chunk, i1 = min(n, i0 + chunk);
   double al = 0, be = 0, gr = 0, gi = 0;
@@ -561,7 +590,9 @@ __device__ __forceinline__ double rotate_pair_smem(double2* __restrict__ gp, dou
     for (int p = 0; p < WPP; ++p) { al += s_red[4 * p + 0]; be += s_red[4 * p + 1]; gr += s_red[4 * p + 2]; gi += s_red[4 * p + 3]; }
   }
   double c, sr, si, cos2;
-  if (!rot_params(al, be, gr, gi, tol2, c, sr, si, cos2)) return cos2;
+  const bool rot = rot_params(al, be, gr, gi, tol2, c, sr, si, cos2);
+  if (part == 0) { nchk += n; if (rot) nrot += n; }
+  if (!rot) return cos2;
   for (int i = i0 + lane; i < i1; i += 32) {
     const double2 a = gp[i], b = gq[i];
     gp[i] = make_double2(c * a.x - (sr * b.x + si * b.y), c * a.y - (sr * b.y - si * b.x));
@@ -593,6 +624,7 @@ __global__ void __launch_bounds__(256) seed_block_kernel(int n, const double2* _
   if (gtid < (size_t)max_sweeps) rot_flags[gtid] = 0;
   grid.sync();
   const int NB = (n + W - 1) / W, MB = NB + (NB & 1), npairs = MB / 2;
+  unsigned long long nchk = 0, nrot = 0;
   if (sigma > 0) {
     for (int sweep = 0; sweep < max_sweeps; ++sweep) {
       double cmax = 0;
@@ -619,13 +651,13 @@ __global__ void __launch_bounds__(256) seed_block_kernel(int n, const double2* _
               int p, q;
               rr_pair(W, t, i, p, q);
               cmax = fmax(cmax, rotate_pair_smem<WPP>(s_cols + (size_t)(blk * W + p) * n, s_cols + (size_t)(blk * W + q) * n, n, lane,
-                                                      part, s_red[pr], tol2));
+                                                      part, s_red[pr], tol2, nchk, nrot));
               __syncthreads();
             }
           }
           for (int t = 0; t < W; ++t) {
             const int p = pr, q = W + (pr + t) % W;
-            cmax = fmax(cmax, rotate_pair_smem<WPP>(s_cols + (size_t)p * n, s_cols + (size_t)q * n, n, lane, part, s_red[pr], tol2));
+            cmax = fmax(cmax, rotate_pair_smem<WPP>(s_cols + (size_t)p * n, s_cols + (size_t)q * n, n, lane, part, s_red[pr], tol2, nchk, nrot));
             __syncthreads();
           }
           for (int c = 0; c < 2 * W; ++c) {
@@ -644,6 +676,7 @@ __global__ void __launch_bounds__(256) seed_block_kernel(int n, const double2* _
       if (!rot_flags[sweep]) break;
     }
   }
+  if (lane == 0) seed_count(nchk, nrot);
   for (int j = gwarp; j < n; j += nwarps) {
     double s = 0;
     for (int i = lane; i < n; i += 32) { const double2 a = G[(size_t)j * n + i]; s += a.x * a.x + a.y * a.y; }
@@ -773,6 +806,7 @@ int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int ma
   int rc = ZKD_OK;
   for (int b = 0; b < batch && rc == ZKD_OK; ++b) {
     const double2* Ab = (const double2*)A64 + (size_t)b * nn;
+    KtScope kt(KC_SEED, s);
     seed_sigma_kernel<<<1, 1024, 0, s>>>(N, Ab, sigma);
     double* mub = mu + (size_t)b * N;
     double2* Vb = (double2*)V + (size_t)b * nn;
@@ -797,6 +831,18 @@ int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int ma
     rc = launch_check();
   }
   return rc;
+}
+
+int seed_stats(uint64_t* elems_checked, uint64_t* elems_rotated, bool reset) {
+  unsigned long long h[2] = {0, 0};
+  ZKD_CUDA_TRY(cudaMemcpyFromSymbol(h, g_seed_stats, sizeof(h)));
+  if (elems_checked) *elems_checked = h[0];
+  if (elems_rotated) *elems_rotated = h[1];
+  if (reset) {
+    const unsigned long long z[2] = {0, 0};
+    ZKD_CUDA_TRY(cudaMemcpyToSymbol(g_seed_stats, z, sizeof(z)));
+  }
+  return ZKD_OK;
 }
 
 }  // namespace zkd

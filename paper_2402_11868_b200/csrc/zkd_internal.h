@@ -122,6 +122,8 @@ int fx_to_api_scaled(size_t count, const int32_t* src_fx, void* dst_api, int sca
                      size_t per_scale, cudaStream_t s);
 int fxc_to_api(size_t count, const int32_t* src_fxc, void* dst_api, cudaStream_t s);
 int measure_imad_peak(double millis, double* per_sec, cudaStream_t s);
+int measure_dfma_peak(double millis, double* flops_per_sec, cudaStream_t s);
+int seed_stats(uint64_t* elems_checked, uint64_t* elems_rotated, bool reset);
 void kernel_timing_enable(bool on);
 int kernel_timing_read(double* ms, uint64_t* launches, uint64_t* macs);
 }  // namespace zkd
