@@ -45,26 +45,41 @@ extern "C" {
 
 #define ZKD_MAX_N 2048
 
-/* per-matrix outcome, written to device memory by the call */
+/* Per-matrix outcome, written to device memory by the call (one record per matrix of the batch).
+ * status, n_clusters, max_cluster, log2_resid and log2_orth are per matrix.  `steps` is per CALL: the refinement loop runs
+ * the whole batch until its slowest matrix stops, so every matrix of a call reports the same number.  A matrix whose own
+ * residual is at or below the tolerance reports status 0 even when another matrix of the batch hit the floor (1) or the
+ * step limit (2).  Failures that are not data-dependent outcomes (a window overflow the retry could not repair, a CUDA
+ * error) fail the whole call through its return code. */
 typedef struct {
   int32_t status;      /* 0 converged; 1 stopped at the precision floor above tolerance; 2 max steps; 3 malformed input */
-  int32_t steps;       /* refinement steps taken at the top level (S4) */
+  int32_t steps;       /* refinement passes of the top level (S4), the same for every matrix of the call */
   int32_t n_clusters;  /* clusters (incl. singletons) found by S2 at the top level */
   int32_t max_cluster; /* size of the largest cluster */
-  float log2_resid;    /* log2 of max_ij |(A X - X diag(lambda))_ij| in units where max|a_ij| is in [1/8,1/4) */
-  float log2_orth;     /* log2 of max |X_c^H X_c - I| over cluster blocks after the last orthonormalisation: twice the
-                          log2 measured before that Newton-Schulz step (which squares it), not below -800 */
+  float log2_resid;    /* log2 of max_ij |(A X - X S)_ij| of THIS matrix (S = the cluster-block Rayleigh quotients; the
+                          residuals of the S5 sub-problems of its clusters folded in), in units where max|a_ij| is in
+                          [1/8,1/4); -812 when the residual is exactly zero */
+  float log2_orth;     /* log2 of max |X_c^H X_c - I| over the cluster blocks of THIS matrix after the last
+                          orthonormalisation: twice the log2 measured before that Newton-Schulz step (which squares it),
+                          not below -800 */
 } zkd_info;
 
 /* ---- the hot path ------------------------------------------------------------- */
 
-/* bytes of one real in the API layout; 0 if prec_bits is unsupported */
+/* Bytes of one real in the API layout at `prec_bits` of significand ("The 768-bit precision was used", PAPER.md:41,
+ * section 2.1; 256 bit: section 3.1; 128 bit: section 3.2): 16 + prec_bits/8.  Returns 0 if
+ * prec_bits is unsupported.  Host call, no CUDA work, no error state. */
 size_t zkd_real_bytes(int prec_bits);
 
-/* Size of the device workspace zkd_diag_herm_ws needs for (N, batch).  Host call, no CUDA work. */
+/* Size in bytes of the device workspace zkd_diag_herm_ws needs for (N, batch); *workspace_bytes is a
+ * host pointer.  Host call, no CUDA work.  Errors: ZKD_ERR_INVALID_ARG (N < 1, N > ZKD_MAX_N, batch < 1 or > 65535,
+ * NULL), ZKD_ERR_UNSUPPORTED_PREC. */
 int zkd_diag_herm_bufsize(int N, int batch, int prec_bits, size_t *workspace_bytes);
 
-/* Eigendecomposition of `batch` Hermitian N x N matrices (S0 ingest .. S6 export, all on `stream`).
+/* The operation of the paper's diag_H / zkcm_cus::cus_diag_H: "diagonalizing N x N Hermitian matrix" at multiprecision
+ * (section 2.1) by "the Rayleigh quotient iteration ... to recover the precision from the result of
+ * double-precision calculations" (section 2).
+ * Eigendecomposition of `batch` Hermitian N x N matrices (S0 ingest .. S6 export, all on `stream`).
  *   A, eigvals, eigvecs, workspace, info: DEVICE pointers (info may be NULL).  A is not modified and may not
  *   alias the outputs.  The call synchronises `stream` internally a few times (cluster table and one
  *   convergence scalar per refinement step) and returns after all work has been enqueued; outputs are valid
@@ -72,15 +87,21 @@ int zkd_diag_herm_bufsize(int N, int batch, int prec_bits, size_t *workspace_byt
 int zkd_diag_herm_ws(int N, int batch, int prec_bits, const void *A, void *eigvals, void *eigvecs, void *workspace,
                      size_t workspace_bytes, zkd_info *info, void *stream);
 
-/* Same with a workspace obtained from (and returned to) the stream-ordered CUDA allocator. */
+/* The same operation (PAPER.md:41 / :33; north_star's example call) with a workspace obtained from, and returned to, the
+ * stream-ordered CUDA allocator.  A, eigvals, eigvecs: DEVICE pointers, caller-owned, 16-byte aligned.  Same errors as
+ * zkd_diag_herm_ws plus ZKD_ERR_WORKSPACE when the allocation fails. */
 int zkd_diag_herm(int N, int batch, int prec_bits, const void *A, void *eigvals, void *eigvecs, void *stream);
 
-/* End-to-end convenience: HOST buffers in the API layout; copies H2D, runs zkd_diag_herm, copies D2H, and
- * synchronises.  info_host may be NULL. */
+/* End-to-end convenience for the same operation (PAPER.md:41 / :33): HOST buffers in the API layout (pageable or pinned,
+ * caller-owned); copies H2D, runs zkd_diag_herm_ws on the legacy default stream, copies D2H, and synchronises.
+ * info_host (host, `batch` records) may be NULL.  Keeps one grow-only device buffer per calling thread between calls. */
 int zkd_diag_herm_host(int N, int batch, int prec_bits, const void *A_host, void *eigvals_host, void *eigvecs_host,
                        zkd_info *info_host);
 
-/* Tunables (process-wide; call before zkd_diag_herm*).  Keys: "tau_bits" (cluster threshold 2^-tau ||A||_F,
+/* Tunables.  PROCESS-WIDE and unsynchronised: set them before, not during, calls of zkd_diag_herm* from
+ * other threads; the library may be used from several host threads with distinct workspaces as long as the options, the
+ * counters and the kernel timing are left alone meanwhile, and it serves ONE device per process (the device current at
+ * the first call).  Keys: "tau_bits" (cluster threshold 2^-tau ||A||_F,
  * default 20), "tol_bits" (stop when max|R_ij| <= 2^-tol, default 770), "max_steps" (default 120),
  * "gemm_path" (engine of the digit GEMM: 0 = automatic [default]: limb-sliced int8 tcgen05 MMAs when M, N, K >= 128,
  * the IMAD kernel otherwise; 1 = IMAD only; 2 = int8 tcgen05 wherever its tiles can be formed),
@@ -95,6 +116,7 @@ int zkd_diag_herm_host(int N, int batch, int prec_bits, const void *A_host, void
 int zkd_set_option(const char *key, double value);
 int zkd_get_option(const char *key, double *value);
 
+/* Text of a ZKD_ERR_* code (static storage); library version (major * 100 + minor).  SURVEY.md 8(b). */
 const char *zkd_strerror(int code);
 int zkd_version(void);
 
@@ -126,7 +148,10 @@ int zkd_kernel_timing_read_cat(int category, double *ms, uint64_t *launches, uin
  * products = 8 DFMA per element) and elements whose pair was also rotated (12 more DFMA per element).  Synchronises. */
 int zkd_seed_stats(uint64_t *elems_checked, uint64_t *elems_rotated, int reset);
 
-/* ---- host-side helpers (no CUDA): one real between the API layout and (sign, exp, limbs) / double ---- */
+/* ---- host-side helpers (no CUDA): one real between the API layout and (sign, exp, limbs) / double (the
+ * layout follows MPFR's, the library the paper's ZKCM is built on).  dst / src: host pointers to
+ * zkd_real_bytes(prec_bits) bytes; limbs_le: prec_bits/64 words, least significant first.  ZKD_ERR_INVALID_ARG for NULL,
+ * an unsupported precision, a sign outside -1..1, an unnormalised mantissa or a non-finite double. ---- */
 int zkd_pack(void *dst, int prec_bits, int sign, int64_t exp, const uint64_t *limbs_le);
 int zkd_unpack(const void *src, int prec_bits, int *sign, int64_t *exp, uint64_t *limbs_le);
 int zkd_from_double(void *dst, int prec_bits, double v);
@@ -144,6 +169,28 @@ double zkd_to_double(const void *src, int prec_bits);
 int zkd_fx_from_api(int count, int prec_bits, const void *src_api, int32_t *dst_fx, int scale_bits, void *stream);
 int zkd_fx_to_api(int count, int prec_bits, const int32_t *src_fx, void *dst_api, int scale_bits, void *stream);
 
+/* Element-wise multi-digit primitives on real FX arrays of `count` numbers (north_star (b); SURVEY.md 8(a) "MP
+ * primitives"): out[e] = a[e] (op) b[e].  The hot path uses the same device functions inside its kernels; this entry exists
+ * so that each primitive can be checked against exact integer arithmetic.  a, b, out: DEVICE pointers to int32[30][count]
+ * (b may be NULL for the unary ones; out may alias a or b).
+ *   ADD, SUB : exact modulo 2^840 (wraps like the top digit).      HALF : floor(a / 2).
+ *   MUL      : sum of the digit products a_i b_j with i + j >= 28, + 2^(28*28 + 27), shifted right by 28*29 bits (floor):
+ *              the exact product rounded at the guard column, minus the digit columns below the guard column, i.e.
+ *              within [-28, +1/2] units of 2^-812 of the exact product for non-negative low digits.
+ *   RECIP    : a in [1/4, 1/2] -> 1/a in [2, 4] by Newton from an fp64 start (error <= 64 units of 2^-812).
+ *   RSQRT    : a > 0 -> 1/sqrt(a) (error <= 64 units of 2^-812 times max(1, 1/sqrt(a))); a <= 0 -> 0.
+ *   MSB      : digit 0 of out = 1 + position of the highest bit of a that differs from its sign (0 for 0 and -1).
+ *   FROM_DOUBLE : out = fx(double(a)): the FX -> fp64 -> FX round trip used by the seed (S1 / S3). */
+#define ZKD_PRIM_ADD 0
+#define ZKD_PRIM_SUB 1
+#define ZKD_PRIM_MUL 2
+#define ZKD_PRIM_RECIP 3
+#define ZKD_PRIM_RSQRT 4
+#define ZKD_PRIM_MSB 5
+#define ZKD_PRIM_HALF 6
+#define ZKD_PRIM_FROM_DOUBLE 7
+int zkd_fx_prim(int op, int count, const int32_t *a_fx, const int32_t *b_fx, int32_t *out_fx, void *stream);
+
 /* C (+)= op(A) * B for complex FX matrices (S4a/S4d/S4e), A: M x K, B: K x N, C: M x N (row-major element order,
  * `batch` problems stored consecutively).  op_a: 0 = A, 1 = A^H (then A is stored K x M).  mode: 0 assign, 1 add,
  * 2 subtract.  Only the window [top_bit - 28*digits, top_bit) of each operand takes part (FX bit 0 = 2^-812; every
@@ -157,7 +204,8 @@ int zkd_gemm_fx(int M, int N, int K, int batch, int op_a, const int32_t *A_fx, i
                 const int32_t *B_fx, int b_top_bit, int b_digits, int32_t *C_fx, int mode, int out_cut_bit, int path,
                 void *workspace, size_t workspace_bytes, int *err_flag, int *msb_out, void *stream);
 
-/* fp64 seed (S1): Hermitian eigendecomposition of batch N x N matrices given as complex doubles (row-major,
+/* fp64 seed (S1; the "double-precision calculations" RQI starts from, PAPER.md:33 - hand-written, no cuSOLVER):
+ * Hermitian eigendecomposition of batch N x N matrices given as complex doubles (row-major,
  * interleaved re/im); mu ascending, V[i][j] = component i of vector j. */
 int zkd_seed_fp64(int N, int batch, const double *A64, double *mu, double *V, void *stream);
 

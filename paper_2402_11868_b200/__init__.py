@@ -67,6 +67,7 @@ def lib() -> ctypes.CDLL:
     L.zkd_to_double.argtypes = [vp, ci]
     L.zkd_fx_from_api.argtypes = [ci, ci, vp, vp, ci, vp]
     L.zkd_fx_to_api.argtypes = [ci, ci, vp, vp, ci, vp]
+    L.zkd_fx_prim.argtypes = [ci, ci, vp, vp, vp, vp]
     L.zkd_gemm_fx_bufsize.argtypes = [ci, ci, ci, ci, ctypes.POINTER(cs)]
     L.zkd_gemm_fx.argtypes = [ci, ci, ci, ci, ci, vp, ci, ci, vp, ci, ci, vp, ci, ci, ci, vp, cs, vp, vp, vp]
     L.zkd_seed_fp64.argtypes = [ci, ci, vp, vp, vp, vp]
@@ -237,6 +238,16 @@ def fx_to_api(count: int, src_fx, dst_api, scale_bits: int = 0, stream=None) -> 
     _check(lib().zkd_fx_to_api(count, PREC, _dev_u8(src_fx, count * FX_DIGITS * 4, "src_fx"),
                                _dev_u8(dst_api, count * REAL_BYTES, "dst_api"), scale_bits, _stream_ptr(stream)),
            "zkd_fx_to_api")
+
+
+PRIM = {"add": 0, "sub": 1, "mul": 2, "recip": 3, "rsqrt": 4, "msb": 5, "half": 6, "from_double": 7}
+
+
+def fx_prim(op: str, count: int, a_fx, b_fx, out_fx, stream=None) -> None:
+    """element-wise multi-digit primitive on real FX arrays (int32[30][count] device tensors)"""
+    nb = count * FX_DIGITS * 4
+    _check(lib().zkd_fx_prim(PRIM[op], count, _dev_u8(a_fx, nb, "a_fx"), _dev_u8(b_fx, nb, "b_fx") if b_fx is not None else None,
+                             _dev_u8(out_fx, nb, "out_fx"), _stream_ptr(stream)), "zkd_fx_prim")
 
 
 def gemm_fx_bufsize(M: int, N: int, K: int, batch: int) -> int:

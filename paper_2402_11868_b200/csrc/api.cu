@@ -36,8 +36,7 @@ static int check_device() {
 // Register-only loop of independent signed IMAD.WIDE (32x32+64 -> 64), the instruction the digit GEMM is made of:
 // 8 accumulators x 4 multipliers per thread, 1024 threads per SM.  Every product of an iteration has distinct
 // operands and the multipliers change every iteration (one IADD on the ALU pipe per 8 multiplies), so ptxas can
-// neither merge nor hoist the multiplies: the SASS loop body holds exactly 32 IMAD.WIDE (checked with cuobjdump,
-// profiles/r01_imad_peak.md).
+// neither merge nor hoist the multiplies: the SASS loop body holds exactly 32 IMAD.WIDE (cuobjdump -sass).
 __global__ void __launch_bounds__(256) imad_peak_kernel(uint32_t* out, int32_t a0, int32_t b0, int iters) {
   int32_t a[8], b[4];
   int64_t acc[8];
@@ -302,6 +301,12 @@ int zkd_fx_to_api(int count, int prec_bits, const int32_t* src_fx, void* dst_api
   ZKD_TRY(check_device());
   return fx_to_api(count, src_fx, dst_api, scale_bits, (cudaStream_t)stream);
 }
+int zkd_fx_prim(int op, int count, const int32_t* a_fx, const int32_t* b_fx, int32_t* out_fx, void* stream) {
+  if (count < 0 || !a_fx || !out_fx || op < 0 || op > ZKD_PRIM_FROM_DOUBLE) return ZKD_ERR_INVALID_ARG;
+  if (!b_fx && (op == ZKD_PRIM_ADD || op == ZKD_PRIM_SUB || op == ZKD_PRIM_MUL)) return ZKD_ERR_INVALID_ARG;
+  ZKD_TRY(check_device());
+  return fx_prim(op, (size_t)count, a_fx, b_fx, out_fx, (cudaStream_t)stream);
+}
 int zkd_gemm_fx_bufsize(int M, int N, int K, int batch, size_t* workspace_bytes) {
   if (M < 1 || N < 1 || K < 1 || batch < 1 || !workspace_bytes) return ZKD_ERR_INVALID_ARG;
   *workspace_bytes = gemm_workspace_bytes(M, N, K, batch);
@@ -360,7 +365,7 @@ int zkd_kernel_timing_read_i8(double* gemm_ms, uint64_t* gemm_launches, uint64_t
 // ---- the hot path -------------------------------------------------------------------------------------------------
 static int check_diag_args(int N, int batch, int prec_bits) {
   if (prec_bits != kPrec) return ZKD_ERR_UNSUPPORTED_PREC;
-  if (N < 1 || N > ZKD_MAX_N || batch < 1) return ZKD_ERR_INVALID_ARG;
+  if (N < 1 || N > ZKD_MAX_N || batch < 1 || batch > 65535) return ZKD_ERR_INVALID_ARG;  // batch is a grid dimension (y / z)
   return ZKD_OK;
 }
 int zkd_diag_herm_bufsize(int N, int batch, int prec_bits, size_t* workspace_bytes) {

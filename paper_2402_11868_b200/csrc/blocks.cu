@@ -4,6 +4,7 @@
 // sorting, phase normalisation.  All multi-digit arithmetic is in-thread on FX digits (fx.cuh).
 #include "blocks.h"
 #include "fx.cuh"
+#include "fx_funcs.cuh"
 #include "timing.h"
 
 namespace zkd {
@@ -110,7 +111,7 @@ int init_x(size_t count, const double2* V, int32_t* X, cudaStream_t s) {
 
 // ---- M := (I - G)/2 on cluster blocks (Newton-Schulz orthonormalisation step), msb of (G - I) ---------------------------
 __global__ void __launch_bounds__(256) ns_build_kernel(int n, int nb, const int* __restrict__ cl, const int* __restrict__ cle_skip1,
-                                                       int32_t* __restrict__ G, int* __restrict__ msb_out) {
+                                                       int32_t* __restrict__ G, int* __restrict__ msb_out, int* __restrict__ msb_b) {
   const size_t per = (size_t)n * n, count = per * nb;
   const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= count * 2) return;
@@ -125,14 +126,15 @@ __global__ void __launch_bounds__(256) ns_build_kernel(int n, int nb, const int*
   if (part == 0 && i == j) g[ND - 1] -= 1;  // G - I
   const int msb = fx_msb(g);
   if (msb_out) atomicMax(msb_out, msb);
+  if (msb_b && msb) atomicMax(msb_b + b, msb);
   fx_neg(r, g);
   fx_half(g, r);                            // (I - G)/2
   fx_store(p, count, e, g);
 }
-int ns_build(int n, int nb, const int* cl, int32_t* G, int* msb_out, cudaStream_t s, const int* cle_skip1) {
+int ns_build(int n, int nb, const int* cl, int32_t* G, int* msb_out, cudaStream_t s, const int* cle_skip1, int* msb_b) {
   KtScope kt_scope(KC_OTHER, s);
   const size_t t = (size_t)n * n * nb * 2;
-  ns_build_kernel<<<(unsigned)((t + 255) / 256), 256, 0, s>>>(n, nb, cl, cle_skip1, G, msb_out);
+  ns_build_kernel<<<(unsigned)((t + 255) / 256), 256, 0, s>>>(n, nb, cl, cle_skip1, G, msb_out, msb_b);
   count_launch();
   return launch_check();
 }
@@ -172,6 +174,36 @@ __global__ void __launch_bounds__(128) min_gap_kernel(int n, int nb, const int32
 int min_gap(int n, int nb, const int32_t* theta, const int* cl, int* gap_inv_out, cudaStream_t s) {
   KtScope kt_scope(KC_OTHER, s);
   min_gap_kernel<<<(unsigned)(((size_t)n * nb + 127) / 128), 128, 0, s>>>(n, nb, theta, cl, gap_inv_out);
+  count_launch();
+  return launch_check();
+}
+
+// ---- per-matrix residual level (zkd_info.log2_resid / status): max msb over the elements of each matrix of R ---------------------
+__global__ void __launch_bounds__(256) resid_per_matrix_kernel(int n, int nb, const int32_t* __restrict__ R, int* __restrict__ msb_r_b) {
+  const size_t per = (size_t)n * n, count = per * nb;
+  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int m = 0;
+  int b = 0;
+  if (t < 2 * count) {
+    const size_t e = t % count;
+    b = (int)(e / per);
+    int32_t d[ND];
+    fx_load(d, R + (t / count) * (size_t)ND * count, count, e);
+    m = fx_msb(d);
+  }
+  // a warp usually lies inside one matrix: one atomic per warp then
+  const int b0 = __shfl_sync(0xffffffffu, b, 0);
+  if (__all_sync(0xffffffffu, b == b0 || m == 0)) {
+    for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0 && m) atomicMax(msb_r_b + b0, m);
+  } else if (m) {
+    atomicMax(msb_r_b + b, m);
+  }
+}
+int resid_per_matrix(int n, int nb, const int32_t* R, int* msb_r_b, cudaStream_t s) {
+  KtScope kt_scope(KC_OTHER, s);
+  const size_t t = 2 * (size_t)n * n * nb;
+  resid_per_matrix_kernel<<<(unsigned)((t + 255) / 256), 256, 0, s>>>(n, nb, R, msb_r_b);
   count_launch();
   return launch_check();
 }
@@ -238,7 +270,7 @@ __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int3
                                                              int32_t* __restrict__ R, int32_t* __restrict__ S,
                                                              int32_t* __restrict__ theta, int* __restrict__ msb_g_out,
                                                              int* __restrict__ msb_r_out, const int* __restrict__ cl,
-                                                             const int* __restrict__ cle) {
+                                                             const int* __restrict__ cle, int* __restrict__ msb_g_b) {
   __shared__ int64_t s_part[8 * CPB * FXP_NACC];
   __shared__ int s_msb;
   extern __shared__ int32_t s_cache[];  // CACHE: [4][ND][n]
@@ -289,7 +321,11 @@ __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int3
   int32_t g[ND], m[ND];
   fxp_finish(g, acc);
   g[ND - 1] -= 1;                      // g - 1
-  if (act && ty == 0 && msb_g_out) atomicMax(msb_g_out, fx_msb(g));
+  if (act && ty == 0 && msb_g_out) {
+    const int mg = fx_msb(g);
+    atomicMax(msb_g_out, mg);
+    if (msb_g_b && mg) atomicMax(msb_g_b + b, mg);
+  }
   {
     int32_t t[ND];
     fx_neg(t, g);
@@ -489,7 +525,7 @@ __global__ void __launch_bounds__(512) singleton_step_warp_kernel(int n, int nb,
                                                                    int32_t* __restrict__ R, int32_t* __restrict__ S,
                                                                    int32_t* __restrict__ theta, int* __restrict__ msb_g_out,
                                                                    int* __restrict__ msb_r_out, const int* __restrict__ cl,
-                                                                   const int* __restrict__ cle) {
+                                                                   const int* __restrict__ cle, int* __restrict__ msb_g_b) {
   __shared__ int64_t s_red[2][16][32];
   __shared__ int s_msb;
   const int b = blockIdx.x / n, j = blockIdx.x % n;
@@ -533,6 +569,7 @@ __global__ void __launch_bounds__(512) singleton_step_warp_kernel(int n, int nb,
   {
     const int mg = wmsb(g, lane);
     if (threadIdx.x == 0 && msb_g_out) atomicMax(msb_g_out, mg);
+    if (threadIdx.x == 0 && msb_g_b && mg) atomicMax(msb_g_b + b, mg);
   }
   // m = (1 - g)/2: negate, canonicalise, shift right by one bit
   int32_t m;
@@ -610,7 +647,7 @@ __global__ void __launch_bounds__(512) singleton_step_warp_kernel(int n, int nb,
 }
 
 int singleton_step(int n, int nb, int32_t* X, int32_t* W, int32_t* R, int32_t* S, int32_t* theta, int* msb_g_out, int* msb_r_out,
-                   cudaStream_t s, const int* cl, const int* cle) {
+                   cudaStream_t s, const int* cl, const int* cle, int* msb_g_b) {
   KtScope kt_scope(KC_SSTEP, s, 14ull * 494ull * (uint64_t)n * n * nb);
   // columns per CTA: as many as keep about one CTA per SM (sector efficiency of the row-major loads against parallelism)
   const size_t cols = (size_t)n * nb;
@@ -620,21 +657,21 @@ int singleton_step(int n, int nb, int32_t* X, int32_t* W, int32_t* R, int32_t* S
   const unsigned grid = (unsigned)((size_t)((n + cpb - 1) / cpb) * nb);
   if (cpb == 1 && n <= 16 * SW_RPW && options().sstep_warp) {
     const int nw = (n + SW_RPW - 1) / SW_RPW;
-    singleton_step_warp_kernel<<<grid, 32 * nw, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
+    singleton_step_warp_kernel<<<grid, 32 * nw, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle, msb_g_b);
   } else if (cpb == 1) {
     int threads = (n + 31) / 32 * 32;
     if (threads > 256) threads = 256;
     const size_t cache = sizeof(int32_t) * 4 * ND * (size_t)n;  // 480 n bytes
     if (cache + 8 * FXP_NACC * sizeof(int64_t) + 64 <= 48 * 1024 && options().sstep_cache)
-      singleton_step_kernel<1, true><<<grid, threads, cache, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
+      singleton_step_kernel<1, true><<<grid, threads, cache, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle, msb_g_b);
     else
-      singleton_step_kernel<1, false><<<grid, threads, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
+      singleton_step_kernel<1, false><<<grid, threads, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle, msb_g_b);
   } else if (cpb == 2) {
-    singleton_step_kernel<2, false><<<grid, 256, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
+    singleton_step_kernel<2, false><<<grid, 256, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle, msb_g_b);
   } else if (cpb == 4) {
-    singleton_step_kernel<4, false><<<grid, 256, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
+    singleton_step_kernel<4, false><<<grid, 256, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle, msb_g_b);
   } else {
-    singleton_step_kernel<8, false><<<grid, 256, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle);
+    singleton_step_kernel<8, false><<<grid, 256, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle, msb_g_b);
   }
   count_launch();
   return launch_check();
@@ -644,56 +681,6 @@ int singleton_step(int n, int nb, int32_t* X, int32_t* W, int32_t* R, int32_t* S
 // One thread per pair i < j (and the diagonal, which is zeroed).  d = theta_j - theta_i is normalised to
 // d' = d 2^s in [1/4, 1/2) with a static barrel shifter, r = 1/d' by Newton from an fp64 start on W-digit fixed point
 // (r in (2,4], FX-like with 29 - (30-W) fractional digits), then E_ij = (C_ij r) 2^s, E_ji = -(C_ji r) 2^s.
-// r <- 1/d' for d' in [1/4,1/2] given as FX (only the top W digits below the binary point are used);
-// r returned as FX (value in [2,4]).  Newton: r <- r + r (1 - d' r), quadratic from an fp64 start.
-template <int W>
-__device__ __forceinline__ void fx_recip_quarter(int32_t (&r)[ND], const int32_t (&dq)[ND], int iters) {
-  // work on full FX digits but zero everything below digit ND-1-W so that products are short where it matters:
-  // the compiler removes multiplications by literal zeros only if the zeros are compile-time; so use W-digit arrays.
-  constexpr int LO = ND - 1 - W;  // first digit kept (FX digit index); fractional digits kept: 29 - LO = W...
-  int32_t dw[W + 1], rw[W + 1];   // digits LO..ND-1 of d' and r
-#pragma unroll
-  for (int k = 0; k <= W; ++k) dw[k] = dq[LO + k];
-  {
-    // fp64 start from the top three digits of d'
-    double dd = ((double)dw[W] * 268435456.0 + (double)dw[W - 1]) * 268435456.0 + (double)dw[W - 2];
-    dd = ldexp(dd, -3 * DB + DB);  // value: digit ND-1 is the integer digit -> dw[W] has weight 1
-    const double r0 = 1.0 / dd;     // in [2,4]
-    int32_t t[ND];
-    fx_from_double(t, r0);
-#pragma unroll
-    for (int k = 0; k <= W; ++k) rw[k] = t[LO + k];
-  }
-  // value(x) = sum_k x[k] 2^(28 (k - W)); product columns: x[a] y[b] has weight 2^(28 (a + b - 2W)); result digit k
-  // <- column k + W.  Keep columns >= W - 1 (guard).
-  for (int it = 0; it < iters; ++it) {
-    int64_t acc[W + 2];
-#pragma unroll
-    for (int k = 0; k < W + 2; ++k) acc[k] = 0;
-    mac_cols<W + 1, W + 1, W - 1, W + 2, false>(acc, dw, rw);  // columns W-1 .. 2W; the top one is signed digit W
-    carry_canon(acc);
-    // e = 1 - d' r : digits (acc[1 + k] is result digit k)
-    int32_t ew[W + 1];
-#pragma unroll
-    for (int k = 0; k <= W; ++k) ew[k] = -(int32_t)acc[1 + k];
-    ew[W] += 1;
-    carry_canon32(ew);
-    // r += r e
-    int64_t acc2[W + 2];
-#pragma unroll
-    for (int k = 0; k < W + 2; ++k) acc2[k] = 0;
-    // ew is canonical with signed top; rw canonical
-    mac_cols<W + 1, W + 1, W - 1, W + 2, false>(acc2, rw, ew);
-    carry_canon(acc2);
-#pragma unroll
-    for (int k = 0; k <= W; ++k) rw[k] += (int32_t)acc2[1 + k];
-    carry_canon32(rw);
-  }
-  fx_zero(r);
-#pragma unroll
-  for (int k = 0; k <= W; ++k) r[LO + k] = rw[k];
-}
-
 template <int W>
 __global__ void __launch_bounds__(128) ecalc_kernel(int n, int nb, const int32_t* __restrict__ theta, const int* __restrict__ cl,
                                                     int32_t* __restrict__ C, int newton_iters, int* __restrict__ msb_out,

@@ -9,11 +9,14 @@ int cluster_detect(int n, int nb, const double2* A64, const double* mu, int tau_
                    int* cl, int* cle, int* stats, cudaStream_t s);
 int init_x(size_t count, const double2* V, int32_t* X, cudaStream_t s);
 // cle_skip1 != null: blocks of singleton clusters are left untouched
-int ns_build(int n, int nb, const int* cl, int32_t* G, int* msb_out, cudaStream_t s, const int* cle_skip1 = nullptr);
+// msb_b != null: the same maximum per matrix (atomicMax into msb_b[b])
+int ns_build(int n, int nb, const int* cl, int32_t* G, int* msb_out, cudaStream_t s, const int* cle_skip1 = nullptr, int* msb_b = nullptr);
 // fused S4f + S4c when every cluster of the level is a singleton: X, W updated in place, R, diag(S), theta written
 // cl / cle != null: only the columns whose cluster is a singleton are processed
 int singleton_step(int n, int nb, int32_t* X, int32_t* W, int32_t* R, int32_t* S, int32_t* theta, int* msb_g_out, int* msb_r_out,
-                   cudaStream_t s, const int* cl = nullptr, const int* cle = nullptr);
+                   cudaStream_t s, const int* cl = nullptr, const int* cle = nullptr, int* msb_g_b = nullptr /* [nb], per matrix */);
+// per-matrix outcome (zkd_info): msb_r_b[b] <- max msb over the elements of matrix b of the residual array R
+int resid_per_matrix(int n, int nb, const int32_t* R, int* msb_r_b, cudaStream_t s);
 // gap_inv_out (device int, zeroed by the caller) <- max over neighbouring columns of different clusters of 1024 - msb(gap)
 int min_gap(int n, int nb, const int32_t* theta, const int* cl, int* gap_inv_out, cudaStream_t s);
 int theta_from_diag(int n, int nb, const int32_t* S, int32_t* theta, cudaStream_t s);
@@ -37,6 +40,10 @@ int split_scatter(int n, int nb, int m, int nsub, const SubProblem* subs_dev, co
 int sub_scatter(int n, int nb, int m, int nsub, const SubProblem* subs_dev, const int32_t* U /*nsub m m*/, const int32_t* lam_sub,
                 const int32_t* cbar, const int* kshift, const int* degenerate, int32_t* Um /*nb n n*/, int32_t* theta, cudaStream_t s);
 int identity_blocks(int n, int nb, int32_t* Um, cudaStream_t s);
+// per-matrix outcome: residual / orthonormality levels of the sub-problems (pm_sub: [2 nsub], in the sub-level's scaled units)
+// folded into their parent matrices (pm_parent: [2 nb_parent]): resid msb - kshift, orth msb as it is
+int fold_sub_stats(int nsub, const SubProblem* subs_dev, const int* kshift, const int* degenerate, const int* pm_sub, int* pm_parent,
+                   int nb_parent, cudaStream_t s);
 // S6: sort ascending, phase-normalise, export
 int finalize_export(int N, int batch, const int32_t* X, const int32_t* lam, const int* scale, void* eigvals_api, void* eigvecs_api,
                     int32_t* scratch /* FxC batch N N */, int32_t* lam_sorted /* FxR batch N */, int* rank /* batch N */,

@@ -5,6 +5,7 @@
 
 #include "blocks.h"
 #include "fx_api.cuh"
+#include "fx_funcs.cuh"
 #include "timing.h"
 
 namespace zkd {
@@ -252,6 +253,24 @@ int sub_scatter(int n, int nb, int m, int nsub, const SubProblem* subs_dev, cons
   return launch_check();
 }
 
+__global__ void __launch_bounds__(128) fold_sub_stats_kernel(int nsub, const SubProblem* __restrict__ subs, const int* __restrict__ kshift,
+                                                             const int* __restrict__ degenerate, const int* __restrict__ pm_sub,
+                                                             int* __restrict__ pm_parent, int nb_parent) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= nsub || degenerate[p]) return;
+  const int b = subs[p].b;
+  const int r = pm_sub[p] - kshift[p];  // the sub-problem was scaled by 2^kshift
+  if (r > 0) atomicMax(pm_parent + b, r);
+  if (pm_sub[nsub + p] > 0) atomicMax(pm_parent + nb_parent + b, pm_sub[nsub + p]);
+}
+int fold_sub_stats(int nsub, const SubProblem* subs_dev, const int* kshift, const int* degenerate, const int* pm_sub, int* pm_parent,
+                   int nb_parent, cudaStream_t s) {
+  KtScope kt_scope(KC_OTHER, s);
+  fold_sub_stats_kernel<<<(nsub + 127) / 128, 128, 0, s>>>(nsub, subs_dev, kshift, degenerate, pm_sub, pm_parent, nb_parent);
+  count_launch();
+  return launch_check();
+}
+
 // S4h: one CTA per sub-problem
 __global__ void __launch_bounds__(128) split_scatter_kernel(int n, int nb, int m, int nsub, const SubProblem* __restrict__ subs,
                                                             const double2* __restrict__ V64, const int* __restrict__ sub_cl,
@@ -395,24 +414,8 @@ __global__ void __launch_bounds__(128) phase_kernel(int N, int batch, const int3
     if (msb == 0) {  // zero column (cannot happen for a unit vector): leave it alone
       fx_zero(ur); fx_zero(ui); ur[ND - 1] = 1;
     } else {
-      // s' = s 4^t with msb(s') in {811, 812}  (s' in [1/4, 1))
-      int t2 = 812 - msb;
-      t2 -= (t2 & 1);
-      if (t2 < 0) t2 = 0;
-      fx_shl(s2, t2);
       int32_t y[ND];
-      fx_from_double(y, rsqrt(fx_to_double(s2)));  // y in (1, 2]
-      for (int it = 0; it < 5; ++it) {
-        int32_t yy[ND], syy[ND], corr[ND], three[ND], h[ND];
-        fx_mul(yy, y, y);
-        fx_mul(syy, s2, yy);
-        fx_zero(three); three[ND - 1] = 3;
-        fx_sub(corr, three, syy);  // 3 - s y^2
-        fx_mul(h, y, corr);
-        fx_half(y, h);
-      }
-      // 1/sqrt(s) = y 2^(t2/2)
-      fx_shl(y, t2 / 2);
+      fx_rsqrt(y, s2);  // 1/|x_k*|
       const size_t e = (size_t)b * per + (size_t)bestk * N + j;
       int32_t zr[ND], zi[ND], nzi[ND];
       fx_load(zr, Xr, count, e); fx_load(zi, Xi, count, e);

@@ -6,10 +6,11 @@
 // i.e. a radix-2^28 two's-complement expansion.  Arrays are digit-major planes: plane d of a real array with
 // `count` elements is int32[count], so consecutive threads read consecutive words of one plane.
 //
-// Why 28-bit digits in 32-bit words: IMAD.WIDE (32x32+64 -> 64) issues at the full 64 lanes/clk/SM on sm_100a
-// (measured, profiles/r01_imad_microbench.md) but a carry chain (IMAD.WIDE.X with predicate carries) reached
-// only 44 % of that.  With 28-bit digits a 64-bit column accumulator absorbs >= 128 products before it can
-// overflow, so products are independent IMAD.WIDEs and carries are resolved once per tile, off the hot loop.
+// Why 28-bit digits in 32-bit words: independent IMAD.WIDE (32x32+64 -> 64) issue at 30.5 per clock per SM on sm_100a
+// (zkd_measure_imad_peak, the register-only loop in api.cu: 8.86e12 /s at 1965 MHz; half the 32-bit IMAD rate), but a
+// carry chain (IMAD.WIDE.X with predicate carries) reached only 44 % of that in the same loop.  With 28-bit digits a 64-bit
+// column accumulator absorbs >= 128 products before it can overflow, so products are independent IMAD.WIDEs and carries are
+// resolved once per tile, off the hot loop.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>

@@ -8,8 +8,8 @@
 // their total is < 2^-17 of the lowest kept column after the guard column is dropped by the caller).
 // Carries are resolved once per 16-deep K tile, off the multiply loop.
 //
-// Roofline: compute-bound on the integer-multiply pipe (64 IMAD.WIDE / clk / SM measured); operands are staged
-// through shared memory, each tile word is reused by 16 threads.
+// Roofline: compute-bound on the integer-multiply pipe (30.5 IMAD.WIDE / clk / SM measured by zkd_measure_imad_peak);
+// operands are staged through shared memory, each tile word is reused by 16 threads.
 #pragma once
 #include "fx.cuh"
 
@@ -87,13 +87,9 @@ using GemmLaunchFn = cudaError_t (*)(const GemmKArgs&, dim3 grid, cudaStream_t);
 template <int NP, int NQ>
 cudaError_t gemm_digits_launch(const GemmKArgs& a, dim3 grid, cudaStream_t s) {
   using S = GemmShape<NP, NQ>;
-  static bool attr_done = false;
-  if (!attr_done) {
-    if (S::SMEM > 48 * 1024) {
-      cudaError_t e = cudaFuncSetAttribute(gemm_digits_kernel<NP, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::SMEM);
-      if (e != cudaSuccess) return e;
-    }
-    attr_done = true;
+  if (S::SMEM > 48 * 1024) {  // per device and cheap: set on every launch rather than cached in a process-wide flag
+    cudaError_t e = cudaFuncSetAttribute(gemm_digits_kernel<NP, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::SMEM);
+    if (e != cudaSuccess) return e;
   }
   gemm_digits_kernel<NP, NQ><<<grid, dim3(GT, GT), S::SMEM, s>>>(a);
   return cudaGetLastError();

@@ -546,11 +546,7 @@ int gemm_i8_finish(int M, int N, int K, int batch, const int32_t* Pc, const int3
   ka.nsplit = (ka.nkb + ka.kb_per_split - 1) / ka.kb_per_split;
   ka.p_tile_bytes = (uint32_t)boxP * I8_BK;
   ka.q_tile_bytes = (uint32_t)boxQ * I8_BK;
-  static bool attr_done = false;
-  if (!attr_done) {
-    ZKD_CUDA_TRY(cudaFuncSetAttribute(gemm_i8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)I8_SMEM));
-    attr_done = true;
-  }
+  ZKD_CUDA_TRY(cudaFuncSetAttribute(gemm_i8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)I8_SMEM));  // per device, cheap
   const dim3 grid((N + I8_BN - 1) / I8_BN, (M + I8_BM - 1) / I8_BM, (unsigned)(G * ka.nsplit * ka.ngroups));
   if (grid.z > 65535) return ZKD_ERR_INTERNAL;
   // int8 MACs actually issued: every (a, b) pair with a + b >= dcut, on full 128 x 128 x 128 blocks

@@ -19,6 +19,7 @@
 #include <vector>
 
 #include "blocks.h"
+#include "timing.h"
 
 namespace zkd {
 
@@ -156,7 +157,7 @@ inline int digits_for(int top, int cut) { return std::max(2, std::min(kND, ceil_
 // X, W <- (X, W)(I + (I - G)/2) on clusters;  S = X_c^H W_c;  theta = diag S;  R = W - X_c S_c.  msb(G - I) and msb(R) are
 // accumulated into scal[S_MSB_G] / scal[S_MSB_R] (singleton columns included).
 int cluster_pass(Ctx& c, int n, int nb, const ClusterPlan& plan, const int* cl, const int* cle, int32_t* X, int32_t* W, int32_t* R,
-                 int32_t* Sm, int32_t* Gm, int32_t* theta, int* scal, int cut, size_t fxc) {
+                 int32_t* Sm, int32_t* Gm, int32_t* theta, int* scal, int cut, size_t fxc, int* pm_orth /* [nb], may be null */) {
   const Options& opt = options();
   cudaStream_t s = c.s;
   const size_t cnt = (size_t)n * n * nb;
@@ -180,7 +181,7 @@ int cluster_pass(Ctx& c, int n, int nb, const ClusterPlan& plan, const int* cl, 
   for (const ClusterGroup& g : plan.groups)
     ZKD_TRY(gemm(g.m, g.m, n, g.nsub, view(X, n, g.m, true, topX, nwX, g.offX), view(X, n, g.m, false, topX, nwX, g.offX), Gm,
                  GemmMode::Assign, g.offB, nullptr, cutG));
-  ZKD_TRY(ns_build(n, nb, cl, Gm, scal + S_MSB_G, s, cle));
+  ZKD_TRY(ns_build(n, nb, cl, Gm, scal + S_MSB_G, s, cle, pm_orth));
   int hs[S_NUM];
   ZKD_TRY(read_scalars(c, scal, S_NUM, hs));
   if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
@@ -199,8 +200,11 @@ int cluster_pass(Ctx& c, int n, int nb, const ClusterPlan& plan, const int* cl, 
     }
   }
   // S4c
-  ZKD_CUDA_TRY(cudaMemcpyAsync(R, W, fxc, cudaMemcpyDeviceToDevice, s));
-  if (plan.has_singletons) ZKD_TRY(singleton_step(n, nb, X, W, R, Sm, theta, scal + S_MSB_G, scal + S_MSB_R, s, cl, cle));
+  {
+    KtScope kt(KC_OTHER, s);
+    ZKD_CUDA_TRY(cudaMemcpyAsync(R, W, fxc, cudaMemcpyDeviceToDevice, s));
+  }
+  if (plan.has_singletons) ZKD_TRY(singleton_step(n, nb, X, W, R, Sm, theta, scal + S_MSB_G, scal + S_MSB_R, s, cl, cle, pm_orth));
   for (const ClusterGroup& g : plan.groups)
     ZKD_TRY(gemm(g.m, g.m, n, g.nsub, view(X, n, g.m, true, topX, nwX, g.offX), view(W, n, g.m, false, topW, nwW, g.offX), Sm,
                  GemmMode::Assign, g.offB, nullptr));
@@ -341,7 +345,11 @@ int try_split(Ctx& c, int n, int nb, const ClusterPlan& plan, const int32_t* Sm,
       ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(W, n, g.m, false, topW, g.offX), view(Um, g.m, g.m, false, 815, g.offB), W,
                    GemmMode::Assign, g.offX));
     }
-    ZKD_CUDA_TRY(cudaStreamSynchronize(s));
+    {
+      int hs[S_NUM];
+      ZKD_TRY(read_scalars(c, scal, S_NUM, hs));  // synchronises; the rotation GEMMs' operand checks land in S_ERR
+      if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
+    }
     *changed = true;
     h_cl.swap(h_new);
   }
@@ -349,12 +357,14 @@ int try_split(Ctx& c, int n, int nb, const ClusterPlan& plan, const int32_t* Sm,
   return ZKD_OK;
 }
 
-int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* lam, int depth, const int* noise, LevelStats* st);
+// pm: device int[2 nb], per-matrix outcome of the level (zkd_info): [b] msb of the final residual of matrix b (sub-levels folded
+// in), [nb + b] msb of G - I measured by the last pass.  Zeroed here.
+int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* lam, int depth, const int* noise, LevelStats* st, int* pm);
 
 // One level of the path.  allow_split = false leaves every cluster to the S5 recursion (slower on spectra like c4's, but it
 // has no heuristics to go wrong); *split_used tells the caller whether S4h took part in a failed attempt.
 int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* lam, int depth, const int* noise, LevelStats* st,
-                     bool allow_split, bool* split_used) {
+                     bool allow_split, bool* split_used, int* pm) {
   const Options& opt = options();
   const size_t cnt = (size_t)n * n * nb;
   const size_t fxc = FxC::bytes(cnt);
@@ -397,6 +407,7 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
   int32_t* Cc = Cm;
   ZKD_TRY(init_x(cnt, V, Xc, s));
   ZKD_CUDA_TRY(cudaMemsetAsync(scal, 0, sizeof(int) * S_NUM, s));
+  ZKD_CUDA_TRY(cudaMemsetAsync(pm, 0, sizeof(int) * 2 * nb, s));
 
   const int topA = 812, topX = 815;
   auto side = [&](const int32_t* fx, int top, int nw, bool ct) {
@@ -432,11 +443,11 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
   for (int step = 0; step < opt.max_steps; ++step) {
     if (singletons) {
       // S4f + S4c fused: normalise columns, Rayleigh quotients, residual (X, W in place)
-      ZKD_TRY(singleton_step(n, nb, Xc, Wc, R, Sm, theta, scal + S_MSB_G, scal + S_MSB_R, s));
+      ZKD_TRY(singleton_step(n, nb, Xc, Wc, R, Sm, theta, scal + S_MSB_G, scal + S_MSB_R, s, nullptr, nullptr, pm + nb));
     } else {
       // S4f + S4c on cluster views.  Results are needed to about 2^-(2 e_now + 40) and e_now <= 2 e_prev + 45.
       last_cut = 812 - (4 * e_prev + 130);
-      ZKD_TRY(cluster_pass(c, n, nb, plan, cl, cle, Xc, Wc, R, Sm, Gm, theta, scal, last_cut, fxc));
+      ZKD_TRY(cluster_pass(c, n, nb, plan, cl, cle, Xc, Wc, R, Sm, Gm, theta, scal, last_cut, fxc, pm + nb));
     }
     ZKD_TRY(min_gap(n, nb, theta, cl, scal + S_GAP_INV, s));
     ZKD_TRY(read_scalars(c, scal, S_NUM, hs));
@@ -455,6 +466,7 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
     if (step + 1 == opt.max_steps) break;
     prev_msb_r = msb_r;
     ZKD_CUDA_TRY(cudaMemsetAsync(scal, 0, sizeof(int) * S_NUM, s));
+    ZKD_CUDA_TRY(cudaMemsetAsync(pm + nb, 0, sizeof(int) * nb, s));
     if (msb_r == 0) continue;  // residual exactly zero: only the orthonormalisation is still converging
 
     // S4h: split clusters whose internal structure stands above the noise of S_c
@@ -502,6 +514,7 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
                          c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s));
   }
   if (st) { st->steps = steps + 1; st->status = status; }
+  ZKD_TRY(resid_per_matrix(n, nb, R, pm, s));  // R is the residual of the last pass
   if (split_done) {
     // Vectors of clusters that were split apart are orthogonal only to residual / gap, and the gaps inside a detected
     // cluster can be tiny (c4: 2^-61).  One symmetric (Loewdin / Newton-Schulz) orthonormalisation over the clusters AS
@@ -565,7 +578,8 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
       int* kshift = c.ar.get<int>((size_t)nsub);
       int* degen = c.ar.get<int>((size_t)nsub);
       int* noise_sub = c.ar.get<int>((size_t)nsub);
-      if (!subs_dev || !H || !U || !cbar || !lam_sub || !kshift || !degen || !noise_sub) return ZKD_ERR_WORKSPACE;
+      int* pm_sub = c.ar.get<int>((size_t)2 * nsub);
+      if (!subs_dev || !H || !U || !cbar || !lam_sub || !kshift || !degen || !noise_sub || !pm_sub) return ZKD_ERR_WORKSPACE;
       ZKD_CUDA_TRY(cudaMemcpyAsync(subs_dev, kv.second.data(), sizeof(SubProblem) * nsub, cudaMemcpyHostToDevice, s));
       ZKD_TRY(sub_gather(n, nb, m, nsub, subs_dev, Sm, H, cbar, kshift, degen, tol_msb + 6, noise, noise_sub, nullptr, 0, s));
       std::vector<int> hdeg((size_t)nsub);
@@ -575,8 +589,9 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
       for (int v : hdeg) all_deg = all_deg && v;
       if (all_deg) continue;
       LevelStats sub;
-      ZKD_TRY(solve_level(c, m, nsub, H, U, lam_sub, depth + 1, noise_sub, &sub));
+      ZKD_TRY(solve_level(c, m, nsub, H, U, lam_sub, depth + 1, noise_sub, &sub, pm_sub));
       if (st && sub.status > st->status) st->status = sub.status;
+      ZKD_TRY(fold_sub_stats(nsub, subs_dev, kshift, degen, pm_sub, pm, nb, s));
       ZKD_TRY(sub_scatter(n, nb, m, nsub, subs_dev, U, lam_sub, cbar, kshift, degen, Um, theta, s));
       any = true;
     }
@@ -603,11 +618,11 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
 
 // S4h (early cluster split) is a heuristic accelerator: when a level that used it fails (a window overflow, no convergence),
 // the level is redone from its seed with every cluster left to the S5 recursion.
-int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* lam, int depth, const int* noise, LevelStats* st) {
+int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* lam, int depth, const int* noise, LevelStats* st, int* pm) {
   const Arena::Mark mark = c.ar.mark();
   bool split_used = false;
   LevelStats tmp;
-  int rc = solve_level_impl(c, n, nb, A, X, lam, depth, noise, st ? st : &tmp, true, &split_used);
+  int rc = solve_level_impl(c, n, nb, A, X, lam, depth, noise, st ? st : &tmp, true, &split_used, pm);
   const bool failed = rc == ZKD_ERR_INTERNAL || (rc == ZKD_OK && (st ? st->status : tmp.status) == 2);
   if (failed && split_used) {
     if (options().verbose) fprintf(stderr, "[zkd] depth %d n %d: retry without early splits\n", depth, n);
@@ -615,17 +630,21 @@ int solve_level(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_t* la
     c.ar.release(mark);
     if (st) *st = LevelStats();
     bool dummy = false;
-    rc = solve_level_impl(c, n, nb, A, X, lam, depth, noise, st ? st : &tmp, false, &dummy);
+    rc = solve_level_impl(c, n, nb, A, X, lam, depth, noise, st ? st : &tmp, false, &dummy, pm);
   }
   return rc;
 }
 
-__global__ void info_kernel(int batch, const int* __restrict__ status_in, int level_status, int steps, int msb_r, int msb_g,
-                            const int* __restrict__ cl_stats, zkd_info* __restrict__ info) {
+// zkd_info per matrix.  pm[b] = msb of the final residual of matrix b (S5 sub-levels folded in), pm[batch + b] = msb of G - I
+// measured by its last pass.  The refinement loop runs the whole batch until its worst matrix stops, so `steps` is the same
+// for every matrix of a call; status 1 / 2 is given only to the matrices whose own residual is still above the tolerance.
+__global__ void info_kernel(int batch, const int* __restrict__ status_in, int level_status, int steps, int tol_msb,
+                            const int* __restrict__ pm, const int* __restrict__ cl_stats, zkd_info* __restrict__ info) {
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b >= batch) return;
   zkd_info o;
-  o.status = status_in[b] ? 3 : level_status;
+  const int msb_r = pm[b], msb_g = pm[batch + b];
+  o.status = status_in[b] ? 3 : (msb_r <= tol_msb ? 0 : (level_status ? level_status : 1));
   o.steps = steps;
   o.n_clusters = cl_stats ? cl_stats[2 * b] : 0;
   o.max_cluster = cl_stats ? cl_stats[2 * b + 1] : 0;
@@ -666,12 +685,13 @@ int diag_herm_device(int N, int batch, const void* A_api, void* eigvals_api, voi
   int* status = c.ar.get<int>((size_t)batch);
   int* rank = c.ar.get<int>((size_t)N * batch);
   int* cl_stats_dev = c.ar.get<int>((size_t)2 * batch);
-  if (!c.gemm_ws || !A || !X || !lam || !lam_sorted || !scale || !status || !rank || !cl_stats_dev) return ZKD_ERR_WORKSPACE;
+  int* pm = c.ar.get<int>((size_t)2 * batch);
+  if (!c.gemm_ws || !A || !X || !lam || !lam_sorted || !scale || !status || !rank || !cl_stats_dev || !pm) return ZKD_ERR_WORKSPACE;
 
   ZKD_TRY(ingest_herm(N, batch, A_api, A, scale, status, s));
   LevelStats st;
   {
-    const int rc = solve_level(c, N, batch, A, X, lam, 0, nullptr, &st);
+    const int rc = solve_level(c, N, batch, A, X, lam, 0, nullptr, &st, pm);
     if (rc != ZKD_OK) {
       c.ar.release(Arena::Mark{c.ar.off, 0});  // an error return may have left overflow allocations behind
       return rc;
@@ -684,7 +704,7 @@ int diag_herm_device(int N, int batch, const void* A_api, void* eigvals_api, voi
       ZKD_CUDA_TRY(cudaMemcpyAsync(cl_stats_dev, st.cl_stats.data(), sizeof(int) * 2 * batch, cudaMemcpyHostToDevice, s));
       cs = cl_stats_dev;
     }
-    info_kernel<<<(batch + 127) / 128, 128, 0, s>>>(batch, status, st.status, st.steps, st.msb_r, st.msb_g, cs, info);
+    info_kernel<<<(batch + 127) / 128, 128, 0, s>>>(batch, status, st.status, st.steps, 812 - options().tol_bits, pm, cs, info);
     count_launch();
     ZKD_TRY(launch_check());
     // st.cl_stats must outlive the async copy

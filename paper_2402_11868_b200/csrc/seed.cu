@@ -76,7 +76,7 @@ __device__ __forceinline__ void rr_pair(int M, int r, int i, int& p, int& q) {
 // every pair of columns meets once, and a rotated column is written straight into the slot where it is needed next, which is
 // a neighbouring warp: only the two columns at each CTA boundary cross distributed shared memory per round (DSMEM moves about
 // 17 B/clk/SM, so a design in which every warp fetches both of its columns from their home CTA is bandwidth-bound: it measured
-// 8.6 us per round at n = 256, 21 ms per call; profiles/r01b_seed.md).
+// 8.6 us per round at n = 256, 21 ms per call).
 // One slot buffer, two cluster-barrier phases per round: "all slots read" (its wait hidden behind the arithmetic) and "all
 // slots written".
 __device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
@@ -297,16 +297,9 @@ static int launch_ring(int N, int batch, int csize, const double2* A, double* mu
   const size_t smem1 = sizeof(double2) * (size_t)wpc * 2 * N;
   int dbuf = (2 * smem1 <= 200 * 1024 && options().seed_dbuf) ? 1 : 0;
   const size_t smem = smem1 * (1 + dbuf);
-  static size_t attr_smem = 0;
-  static bool np_done = false;
-  if (smem > 48 * 1024 && smem > attr_smem) {
-    ZKD_CUDA_TRY(cudaFuncSetAttribute(seed_ring_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_smem = smem;
-  }
-  if (csize > 8 && !np_done) {
-    ZKD_CUDA_TRY(cudaFuncSetAttribute(seed_ring_kernel<EPL>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-    np_done = true;
-  }
+  // function attributes are per device: set on every launch (cheap) rather than cached in process-wide flags
+  if (smem > 48 * 1024) ZKD_CUDA_TRY(cudaFuncSetAttribute(seed_ring_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  if (csize > 8) ZKD_CUDA_TRY(cudaFuncSetAttribute(seed_ring_kernel<EPL>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)(batch * csize));
   cfg.blockDim = dim3((unsigned)(32 * wpc));
@@ -457,11 +450,7 @@ static int launch_cta(int N, int batch, const double2* A, double* mu, double2* V
   const int npairs = (N + 1) / 2;
   int warps = npairs < 1 ? 1 : (npairs > 32 ? (npairs + 1) / 2 : npairs);
   const size_t smem = sizeof(double2) * (size_t)N * N;
-  static size_t attr_smem = 0;
-  if (smem > 48 * 1024 && smem > attr_smem) {
-    ZKD_CUDA_TRY(cudaFuncSetAttribute(seed_cta_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_smem = smem;
-  }
+  if (smem > 48 * 1024) ZKD_CUDA_TRY(cudaFuncSetAttribute(seed_cta_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   {
     KtScope kt(KC_SEED, s);
     seed_cta_kernel<EPL><<<batch, 32 * warps, smem, s>>>(N, A, mu, V, max_sweeps, tol2);
@@ -689,13 +678,9 @@ template <int W>
 static int launch_block(int n, int sms, const double2* Ab, double2* G, double* sigma, int* flags, double* mu_uns, int ms, double t2,
                         cudaStream_t s) {
   const size_t smem = sizeof(double2) * 2 * W * (size_t)n;
-  static bool attr_done = false;
-  if (!attr_done) {
-    if (cudaFuncSetAttribute(seed_block_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess) {
-      (void)cudaGetLastError();
-      return ZKD_ERR_CUDA;
-    }
-    attr_done = true;
+  if (cudaFuncSetAttribute(seed_block_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess) {
+    (void)cudaGetLastError();
+    return ZKD_ERR_CUDA;
   }
   int maxb = 0;
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&maxb, seed_block_kernel<W>, 256, smem) != cudaSuccess || maxb < 1) {

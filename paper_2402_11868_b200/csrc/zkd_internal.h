@@ -121,6 +121,7 @@ int fx_from_api_scaled(size_t count, const void* src_api, int32_t* dst_fx, int s
 int fx_to_api_scaled(size_t count, const int32_t* src_fx, void* dst_api, int scale_bits, const int* scale_dev, int scale_stride,
                      size_t per_scale, cudaStream_t s);
 int fxc_to_api(size_t count, const int32_t* src_fxc, void* dst_api, cudaStream_t s);
+int fx_prim(int op, size_t count, const int32_t* a, const int32_t* b, int32_t* out, cudaStream_t s);
 int measure_imad_peak(double millis, double* per_sec, cudaStream_t s);
 int measure_dfma_peak(double millis, double* flops_per_sec, cudaStream_t s);
 int seed_stats(uint64_t* elems_checked, uint64_t* elems_rotated, bool reset);

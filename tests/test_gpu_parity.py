@@ -297,6 +297,29 @@ def test_malformed_number_sets_status(zkd):
     assert info[0]["status"] == 3 and info[1]["status"] == 0
 
 
+def test_info_is_per_matrix(zkd):
+    """zkd_info: status, n_clusters, max_cluster, log2_resid and log2_orth belong to the matrix, `steps` to the call.  A batch of
+    a diagonal matrix (its residual is exactly zero from the first pass), a random one and a c4-shaped one must report three
+    different records; with max_steps = 2 the diagonal one is converged (0) while the others report the step limit (2)."""
+    N = 16
+    diag = _api_matrix(N, lambda i, j: (Fraction((i * 5) % N - 4, 7) if i == j else 0, 0))
+    mats = [diag, zi.random_hermitian(N, 777), zi.config("c4small", batch=1)["A"]]
+    A = np.concatenate([np.asarray(m).reshape(-1) for m in mats])
+    lam, X, info = gpu_diag(zkd, A, N, 3)
+    assert [r["status"] for r in info] == [0, 0, 0], info
+    assert len({r["steps"] for r in info}) == 1
+    assert info[0]["log2_resid"] == -812.0 and -812.0 < info[1]["log2_resid"] <= -770.0, info
+    assert info[2]["max_cluster"] > 1 and info[0]["max_cluster"] == 1 and info[1]["max_cluster"] == 1, info
+    assert info[2]["log2_resid"] <= -770.0 and info[2]["log2_orth"] <= -760.0, info
+    zkd.set_option("max_steps", 2)
+    try:
+        lam, X, info = gpu_diag(zkd, A, N, 3)
+    finally:
+        zkd.set_option("max_steps", 120)
+    assert info[0]["status"] == 0 and info[1]["status"] == 2 and info[2]["status"] == 2, info
+    assert info[1]["log2_resid"] > -770.0 and info[0]["log2_resid"] == -812.0, info
+
+
 def test_argument_errors(zkd):
     import torch
 
