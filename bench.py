@@ -107,7 +107,7 @@ class ClockSampler:
 # ---------------------------------------------------------------------------------------------------------------
 # workloads
 # ---------------------------------------------------------------------------------------------------------------
-def make_workload(name: str, rank: int, batch: int | None = None):
+def make_workload(name: str, rank: int, batch: int | None = None, prec: int = 768):
     import numpy as np
 
     import zkd_inputs as zi
@@ -116,35 +116,35 @@ def make_workload(name: str, rank: int, batch: int | None = None):
         N = {"c1": 16, "c2": 64, "c3": 256}[name]
         b = batch or 1
         # rank r takes seed streams r*b .. r*b+b-1 (rank 0 = the config's own matrix)
-        A = np.concatenate([zi.random_hermitian(N, zi.CONFIG_SEEDS[name], rank * b + s) for s in range(b)])
+        A = np.concatenate([zi.random_hermitian(N, zi.CONFIG_SEEDS[name], rank * b + s, prec) for s in range(b)])
         return N, b, A
-    cfg = zi.config(name, batch=batch)
+    cfg = zi.config(name, batch=batch, prec=prec)
     return cfg["N"], cfg["batch"], cfg["A"]
 
 
 class Runner:
     """Device-resident buffers for one workload + the call through the C ABI."""
 
-    def __init__(self, z, N, batch, A_np):
+    def __init__(self, z, N, batch, A_np, prec: int = 768):
         import torch
 
-        self.z, self.N, self.b = z, N, batch
-        rb = z.REAL_BYTES
+        self.z, self.N, self.b, self.prec = z, N, batch, prec
+        rb = z.real_bytes(prec)
         self.A_host = torch.from_numpy(A_np).pin_memory()
         self.A = self.A_host.cuda()
         self.lam = torch.zeros(batch * N * rb, dtype=torch.uint8, device="cuda")
         self.X = torch.zeros(batch * N * N * 2 * rb, dtype=torch.uint8, device="cuda")
-        self.ws = torch.empty(z.diag_herm_bufsize(N, batch), dtype=torch.uint8, device="cuda")
+        self.ws = torch.empty(z.diag_herm_bufsize(N, batch, prec), dtype=torch.uint8, device="cuda")
         self.info = torch.zeros(batch * 24, dtype=torch.uint8, device="cuda")
         self.lam_host = torch.zeros(batch * N * rb, dtype=torch.uint8).pin_memory()
         self.X_host = torch.zeros(batch * N * N * 2 * rb, dtype=torch.uint8).pin_memory()
 
     def step(self):
-        self.z.diag_herm_ws(self.N, self.b, self.A, self.lam, self.X, self.ws, self.info)
+        self.z.diag_herm_ws(self.N, self.b, self.A, self.lam, self.X, self.ws, self.info, prec_bits=self.prec)
 
     def step_e2e(self):
         # HOST buffers in, HOST buffers out, copies inside (zkd_diag_herm_host allocates, copies, runs, copies back)
-        self.z.diag_herm_host(self.N, self.b, self.A_host, self.lam_host, self.X_host)
+        self.z.diag_herm_host(self.N, self.b, self.A_host, self.lam_host, self.X_host, prec_bits=self.prec)
 
     @property
     def h2d_bytes(self):
@@ -431,12 +431,14 @@ def main():
     # ---- context rows: the other configs and a saturating batch (not the headline) --------------------------------
     if not args.no_extra and world == 1:
         extra = {}
-        for nm, bb, k in (("c1", 1, 5), ("c2", 1, 5), ("c2", 256, 3), ("c3", 1, 5), ("c4", 512, 3), ("c5", 1, 3)):
-            if nm == args.workload and bb == b:
+        # (the last two rows: the paper's other precisions, 256 bit = Deutsch-Jozsa runs PAPER.md:61, 128 bit = Shor runs :65)
+        for nm, bb, k, pr in (("c1", 1, 5, 768), ("c2", 1, 5, 768), ("c2", 256, 3, 768), ("c3", 1, 5, 768), ("c4", 512, 3, 768),
+                              ("c5", 1, 3, 768), ("c4", 512, 3, 256), ("c4", 512, 3, 128)):
+            if nm == args.workload and bb == b and pr == 768:
                 continue
             try:
-                n2, b2, A2 = make_workload(nm, 0, batch=bb)
-                r2 = Runner(z, n2, b2, A2)
+                n2, b2, A2 = make_workload(nm, 0, batch=bb, prec=pr)
+                r2 = Runner(z, n2, b2, A2, pr)
                 for _ in range(2):
                     r2.step()
                 torch.cuda.synchronize()
@@ -444,7 +446,8 @@ def main():
                 ts, _, c2, se2, _ = measure(torch, z, r2, k, flush, barrier, 1, with_e2e=False)
                 ms = sum(ts0) / len(ts0)
                 rf = [r for r in roofline_objects(c2, se2, imad_peak, dfma_peak, k, sum(ts), nm) if r["share_of_step"] >= 0.1]
-                extra[f"{nm}x{b2}"] = {"matrices_per_s": b2 / (ms * 1e-3), "ms_per_step": ms, "ms_per_step_events_armed": sum(ts) / len(ts),
+                extra[f"{nm}x{b2}" + ("" if pr == 768 else f"@{pr}bit")] = {
+                                       "matrices_per_s": b2 / (ms * 1e-3), "ms_per_step": ms, "ms_per_step_events_armed": sum(ts) / len(ts),
                                        "kernels": [{"kernel": r["kernel"], "share_of_step": round(r["share_of_step"], 4),
                                                     "frac": r["frac"], "bound": r["bound"]} for r in rf]}
                 del r2

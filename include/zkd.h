@@ -37,7 +37,7 @@ extern "C" {
 
 #define ZKD_OK 0
 #define ZKD_ERR_INVALID_ARG (-1)      /* N < 1, batch < 1, NULL or misaligned pointer, N > ZKD_MAX_N */
-#define ZKD_ERR_UNSUPPORTED_PREC (-2) /* this build: prec_bits == 768 only */
+#define ZKD_ERR_UNSUPPORTED_PREC (-2) /* prec_bits is not a multiple of 64 in 128 .. 768 */
 #define ZKD_ERR_WORKSPACE (-3)        /* workspace too small / allocation failed */
 #define ZKD_ERR_CUDA (-4)             /* a CUDA call failed (the sticky error is cleared) */
 #define ZKD_ERR_ARCH (-5)             /* device is not sm_100 */
@@ -64,7 +64,11 @@ typedef struct {
                           not below -800 */
 } zkd_info;
 
-/* ---- the hot path ------------------------------------------------------------- */
+/* ---- the hot path -------------------------------------------------------------
+ * prec_bits: the significand length of the API numbers, a multiple of 64 from 128 to 768 (the paper's settings: 768
+ * PAPER.md:41, 256 PAPER.md:61, 128 PAPER.md:65).  Results are accurate to 2^-(prec_bits - 28) ||A||_F (eigenvalues,
+ * residuals; 2^-(prec_bits - 28) for orthonormality) and rounded to prec_bits on export; internally every precision
+ * runs on the same 840-bit fixed-point planes, with everything below 2^-(prec_bits + 44) left uncomputed. */
 
 /* Bytes of one real in the API layout at `prec_bits` of significand ("The 768-bit precision was used", PAPER.md:41,
  * section 2.1; 256 bit: section 3.1; 128 bit: section 3.2): 16 + prec_bits/8.  Returns 0 if

@@ -412,10 +412,11 @@ static double log2_mpfr(mpfr_srcptr x) {
  *  out[0] = log2 max_j |lam_j - lam0_j| / F                          (i)
  *  out[1] = log2 max_{j in cols} ||A x_j - lam_j x_j||_2 / F         (ii)
  *  out[2] = log2 max_{j in cols, all i} |x_i^H x_j - delta_ij|       (iii)
- *  out[3] = max over groups of  log2 ||E_G||_F - log2 (2^-730 F / gap_G)   (iv)  (<= 0 passes)
+ *  out[3] = max over groups of  log2 ||E_G||_F - log2 (2^-(prec-38) F / gap_G)   (iv)  (<= 0 passes; 2^-730 at 768 bit)
  *  out[4] = log2 F;  out[5] = number of groups;  out[6] = largest group;  out[7] = log2 of worst ||E_G||_F
  * Groups (reading A10): reference eigenvalues sorted ascending; a new group starts where the gap exceeds
- * 2^-666 F.  gap_G = distance from the group's extreme members to the nearest eigenvalue outside.
+ * 2^-(prec-102) F (2^-666 F at 768 bit; the two constants follow the precision for the paper's 256- and 128-bit
+ * settings, PAPER.md:61, :65 - DESIGN.md section 3, reading A18; at 768 bit nothing changes).  gap_G = distance from the group's extreme members to the nearest eigenvalue outside.
  * E_G = X_G - X0_G (X0_G^H X_G)  (= ||sin Theta||_F; for |G| = 1 the phase-aligned difference). */
 int zkd_oracle_compare(int N, int prec, int nthreads, const uint8_t *A_api, const uint8_t *lam_api,
                        const uint8_t *X_api, const uint8_t *lam0_api, const uint8_t *X0_api, const int *cols,
@@ -501,7 +502,7 @@ int zkd_oracle_compare(int N, int prec, int nthreads, const uint8_t *A_api, cons
       load_cmat(&X0, X0_api, N, prec, tmpP, 0);
       mpfr_t gthr, gap, g2;
       mpfr_init2(gthr, Pc); mpfr_init2(gap, Pc); mpfr_init2(g2, Pc);
-      mpfr_div_2si(gthr, F, 666, RN);
+      mpfr_div_2si(gthr, F, prec - 102, RN);
       int *gstart = (int *)malloc(sizeof(int) * (size_t)(N + 1));
       int ng = 0;
       gstart[ng++] = 0;
@@ -557,7 +558,7 @@ int zkd_oracle_compare(int N, int prec, int nthreads, const uint8_t *A_api, cons
             }
           mpfr_sqrt(e2, e2, RN);
           eabs[g] = log2_mpfr(e2);
-          double ltol = have ? (-730.0 + lF - log2_mpfr(gp)) : 1.0e9; /* single group spanning everything: any basis */
+          double ltol = have ? (-(double)(prec - 38) + lF - log2_mpfr(gp)) : 1.0e9; /* single group spanning everything: any basis */
           margin[g] = eabs[g] - ltol;
           cmat_free(&Mm);
         }

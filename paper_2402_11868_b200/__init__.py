@@ -192,7 +192,7 @@ def diag_herm_bufsize(N: int, batch: int, prec_bits: int = PREC) -> int:
 def diag_herm_ws(N: int, batch: int, A, eigvals, eigvecs, workspace, info=None, prec_bits: int = PREC, stream=None) -> None:
     """zkd_diag_herm_ws on device tensors (uint8, API layout).  `info`: optional uint8/int32 CUDA tensor of
     batch * sizeof(zkd_info) bytes."""
-    rb = REAL_BYTES
+    rb = 16 + prec_bits // 8
     a = _dev_u8(A, batch * N * N * 2 * rb, "A")
     lam = _dev_u8(eigvals, batch * N * rb, "eigvals")
     x = _dev_u8(eigvecs, batch * N * N * 2 * rb, "eigvecs")
@@ -204,7 +204,7 @@ def diag_herm_ws(N: int, batch: int, A, eigvals, eigvecs, workspace, info=None, 
 
 
 def diag_herm(N: int, batch: int, A, eigvals, eigvecs, prec_bits: int = PREC, stream=None) -> None:
-    rb = REAL_BYTES
+    rb = 16 + prec_bits // 8
     a = _dev_u8(A, batch * N * N * 2 * rb, "A")
     lam = _dev_u8(eigvals, batch * N * rb, "eigvals")
     x = _dev_u8(eigvecs, batch * N * N * 2 * rb, "eigvecs")
@@ -228,15 +228,15 @@ def read_info(info_tensor, batch: int) -> list[dict]:
 
 # ---- building blocks -------------------------------------------------------------------------------------------
 
-def fx_from_api(count: int, src_api, dst_fx, scale_bits: int = 0, stream=None) -> None:
-    _check(lib().zkd_fx_from_api(count, PREC, _dev_u8(src_api, count * REAL_BYTES, "src_api"),
+def fx_from_api(count: int, src_api, dst_fx, scale_bits: int = 0, stream=None, prec_bits: int = PREC) -> None:
+    _check(lib().zkd_fx_from_api(count, prec_bits, _dev_u8(src_api, count * (16 + prec_bits // 8), "src_api"),
                                  _dev_u8(dst_fx, count * FX_DIGITS * 4, "dst_fx"), scale_bits, _stream_ptr(stream)),
            "zkd_fx_from_api")
 
 
-def fx_to_api(count: int, src_fx, dst_api, scale_bits: int = 0, stream=None) -> None:
-    _check(lib().zkd_fx_to_api(count, PREC, _dev_u8(src_fx, count * FX_DIGITS * 4, "src_fx"),
-                               _dev_u8(dst_api, count * REAL_BYTES, "dst_api"), scale_bits, _stream_ptr(stream)),
+def fx_to_api(count: int, src_fx, dst_api, scale_bits: int = 0, stream=None, prec_bits: int = PREC) -> None:
+    _check(lib().zkd_fx_to_api(count, prec_bits, _dev_u8(src_fx, count * FX_DIGITS * 4, "src_fx"),
+                               _dev_u8(dst_api, count * (16 + prec_bits // 8), "dst_api"), scale_bits, _stream_ptr(stream)),
            "zkd_fx_to_api")
 
 

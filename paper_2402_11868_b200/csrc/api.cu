@@ -172,13 +172,13 @@ using namespace zkd;
 
 extern "C" {
 
-size_t zkd_real_bytes(int prec_bits) { return prec_bits == kPrec ? (size_t)kApiRealBytes : 0; }
+size_t zkd_real_bytes(int prec_bits) { return prec_supported(prec_bits) ? api_real_bytes(prec_bits) : 0; }
 
 const char* zkd_strerror(int code) {
   switch (code) {
     case ZKD_OK: return "ok";
     case ZKD_ERR_INVALID_ARG: return "invalid argument";
-    case ZKD_ERR_UNSUPPORTED_PREC: return "unsupported precision (768 only)";
+    case ZKD_ERR_UNSUPPORTED_PREC: return "unsupported precision (multiples of 64 from 128 to 768 bits)";
     case ZKD_ERR_WORKSPACE: return "workspace too small or allocation failed";
     case ZKD_ERR_CUDA: return "CUDA error";
     case ZKD_ERR_ARCH: return "device is not sm_100";
@@ -234,19 +234,19 @@ int zkd_get_option(const char* key, double* value) {
 
 // ---- host-side number helpers -------------------------------------------------------------------------------------
 int zkd_pack(void* dst, int prec_bits, int sign, int64_t exp, const uint64_t* limbs_le) {
-  if (!dst || prec_bits != kPrec || sign < -1 || sign > 1) return ZKD_ERR_INVALID_ARG;
+  if (!dst || !prec_supported(prec_bits) || sign < -1 || sign > 1) return ZKD_ERR_INVALID_ARG;
   unsigned char* o = (unsigned char*)dst;
-  memset(o, 0, kApiRealBytes);
+  memset(o, 0, api_real_bytes(prec_bits));
   if (sign == 0) return ZKD_OK;
-  if (!limbs_le || !(limbs_le[kPrec / 64 - 1] >> 63)) return ZKD_ERR_INVALID_ARG;
+  if (!limbs_le || !(limbs_le[prec_bits / 64 - 1] >> 63)) return ZKD_ERR_INVALID_ARG;
   int32_t s32 = sign;
   memcpy(o, &s32, 4);
   memcpy(o + 8, &exp, 8);
-  memcpy(o + 16, limbs_le, kPrec / 8);
+  memcpy(o + 16, limbs_le, prec_bits / 8);
   return ZKD_OK;
 }
 int zkd_unpack(const void* src, int prec_bits, int* sign, int64_t* exp, uint64_t* limbs_le) {
-  if (!src || prec_bits != kPrec) return ZKD_ERR_INVALID_ARG;
+  if (!src || !prec_supported(prec_bits)) return ZKD_ERR_INVALID_ARG;
   const unsigned char* s = (const unsigned char*)src;
   int32_t s32, fl;
   int64_t e;
@@ -255,20 +255,20 @@ int zkd_unpack(const void* src, int prec_bits, int* sign, int64_t* exp, uint64_t
   memcpy(&e, s + 8, 8);
   if (fl != 0 || s32 < -1 || s32 > 1) return ZKD_ERR_INVALID_ARG;
   uint64_t top;
-  memcpy(&top, s + 16 + kPrec / 8 - 8, 8);
+  memcpy(&top, s + 16 + prec_bits / 8 - 8, 8);
   if (s32 != 0 && !(top >> 63)) return ZKD_ERR_INVALID_ARG;
   if (sign) *sign = s32;
   if (exp) *exp = e;
-  if (limbs_le) memcpy(limbs_le, s + 16, kPrec / 8);
+  if (limbs_le) memcpy(limbs_le, s + 16, prec_bits / 8);
   return ZKD_OK;
 }
 int zkd_from_double(void* dst, int prec_bits, double v) {
-  if (!dst || prec_bits != kPrec || !std::isfinite(v)) return ZKD_ERR_INVALID_ARG;
+  if (!dst || !prec_supported(prec_bits) || !std::isfinite(v)) return ZKD_ERR_INVALID_ARG;
   uint64_t limbs[kPrec / 64] = {0};
   if (v == 0.0) return zkd_pack(dst, prec_bits, 0, 0, nullptr);
   int e;
   double m = frexp(fabs(v), &e);  // m in [1/2, 1)
-  limbs[kPrec / 64 - 1] = (uint64_t)ldexp(m, 64);  // exact: m has 53 bits
+  limbs[prec_bits / 64 - 1] = (uint64_t)ldexp(m, 64);  // exact: m has 53 bits
   return zkd_pack(dst, prec_bits, v < 0 ? -1 : 1, e, limbs);
 }
 double zkd_to_double(const void* src, int prec_bits) {
@@ -278,9 +278,9 @@ double zkd_to_double(const void* src, int prec_bits) {
   if (zkd_unpack(src, prec_bits, &sign, &e, limbs) != ZKD_OK) return NAN;
   if (sign == 0) return 0.0;
   // round to nearest even on the top 64 bits + sticky
-  uint64_t top = limbs[kPrec / 64 - 1];
+  uint64_t top = limbs[prec_bits / 64 - 1];
   bool sticky = false;
-  for (int k = 0; k < kPrec / 64 - 1; ++k) sticky |= limbs[k] != 0;
+  for (int k = 0; k < prec_bits / 64 - 1; ++k) sticky |= limbs[k] != 0;
   uint64_t keep = top >> 11, rem = top & 0x7ff;
   if (rem > 0x400 || (rem == 0x400 && (sticky || (keep & 1)))) keep += 1;
   double m = ldexp((double)keep, -53);
@@ -290,16 +290,16 @@ double zkd_to_double(const void* src, int prec_bits) {
 
 // ---- building blocks ----------------------------------------------------------------------------------------------
 int zkd_fx_from_api(int count, int prec_bits, const void* src_api, int32_t* dst_fx, int scale_bits, void* stream) {
-  if (prec_bits != kPrec) return ZKD_ERR_UNSUPPORTED_PREC;
+  if (!prec_supported(prec_bits)) return ZKD_ERR_UNSUPPORTED_PREC;
   if (count < 0 || !src_api || !dst_fx) return ZKD_ERR_INVALID_ARG;
   ZKD_TRY(check_device());
-  return fx_from_api(count, src_api, dst_fx, scale_bits, (cudaStream_t)stream);
+  return fx_from_api(count, src_api, dst_fx, scale_bits, (cudaStream_t)stream, prec_bits);
 }
 int zkd_fx_to_api(int count, int prec_bits, const int32_t* src_fx, void* dst_api, int scale_bits, void* stream) {
-  if (prec_bits != kPrec) return ZKD_ERR_UNSUPPORTED_PREC;
+  if (!prec_supported(prec_bits)) return ZKD_ERR_UNSUPPORTED_PREC;
   if (count < 0 || !src_fx || !dst_api) return ZKD_ERR_INVALID_ARG;
   ZKD_TRY(check_device());
-  return fx_to_api(count, src_fx, dst_api, scale_bits, (cudaStream_t)stream);
+  return fx_to_api(count, src_fx, dst_api, scale_bits, (cudaStream_t)stream, prec_bits);
 }
 int zkd_fx_prim(int op, int count, const int32_t* a_fx, const int32_t* b_fx, int32_t* out_fx, void* stream) {
   if (count < 0 || !a_fx || !out_fx || op < 0 || op > ZKD_PRIM_FROM_DOUBLE) return ZKD_ERR_INVALID_ARG;
@@ -364,7 +364,7 @@ int zkd_kernel_timing_read_i8(double* gemm_ms, uint64_t* gemm_launches, uint64_t
 
 // ---- the hot path -------------------------------------------------------------------------------------------------
 static int check_diag_args(int N, int batch, int prec_bits) {
-  if (prec_bits != kPrec) return ZKD_ERR_UNSUPPORTED_PREC;
+  if (!prec_supported(prec_bits)) return ZKD_ERR_UNSUPPORTED_PREC;
   if (N < 1 || N > ZKD_MAX_N || batch < 1 || batch > 65535) return ZKD_ERR_INVALID_ARG;  // batch is a grid dimension (y / z)
   return ZKD_OK;
 }
@@ -381,7 +381,7 @@ int zkd_diag_herm_ws(int N, int batch, int prec_bits, const void* A, void* eigva
   if (((uintptr_t)A | (uintptr_t)eigvals | (uintptr_t)eigvecs | (uintptr_t)workspace) & 15) return ZKD_ERR_INVALID_ARG;
   if (workspace_bytes < diag_workspace_bytes(N, batch)) return ZKD_ERR_WORKSPACE;
   ZKD_TRY(check_device());
-  return diag_herm_device(N, batch, A, eigvals, eigvecs, workspace, workspace_bytes, info, (cudaStream_t)stream);
+  return diag_herm_device(N, batch, prec_bits, A, eigvals, eigvecs, workspace, workspace_bytes, info, (cudaStream_t)stream);
 }
 int zkd_diag_herm(int N, int batch, int prec_bits, const void* A, void* eigvals, void* eigvecs, void* stream) {
   ZKD_TRY(check_diag_args(N, batch, prec_bits));
@@ -403,7 +403,7 @@ int zkd_diag_herm_host(int N, int batch, int prec_bits, const void* A_host, void
   ZKD_TRY(check_diag_args(N, batch, prec_bits));
   if (!A_host || !eigvals_host || !eigvecs_host) return ZKD_ERR_INVALID_ARG;
   ZKD_TRY(check_device());
-  const size_t nA = (size_t)batch * N * N * 2 * kApiRealBytes, nL = (size_t)batch * N * kApiRealBytes;
+  const size_t nA = (size_t)batch * N * N * 2 * api_real_bytes(prec_bits), nL = (size_t)batch * N * api_real_bytes(prec_bits);
   const size_t wsb = diag_workspace_bytes(N, batch);
   const size_t offL = (nA + 255) / 256 * 256, offX = offL + (nL + 255) / 256 * 256, offI = offX + offL,
                offW = offI + ((sizeof(zkd_info) * batch + 255) / 256 * 256);

@@ -25,7 +25,8 @@ int ecalc(int n, int nb, const int32_t* theta, const int* cl, int32_t* C, int pr
 
 // finalize.cu
 // S0: per-matrix scale (max exponent over the upper triangle) and ingest with Hermitian mirroring
-int ingest_herm(int N, int batch, const void* A_api, int32_t* A_fx, int* scale /*[2 * batch]: scales, then scratch*/, int* status /*[batch]*/, cudaStream_t s);
+int ingest_herm(int N, int batch, const void* A_api, int32_t* A_fx, int* scale /*[2 * batch]: scales, then scratch*/, int* status /*[batch]*/, cudaStream_t s,
+                int prec = kPrec);
 // S5 plumbing: gather cluster blocks of S into a batch of m x m sub-problems scaled by 2^k, and back
 struct SubProblem { int b, col0; };  // matrix index and first column of the cluster
 int sub_gather(int n, int nb, int m, int nsub, const SubProblem* subs_dev, const int32_t* S, int32_t* H /*nsub m m*/,
@@ -47,6 +48,6 @@ int fold_sub_stats(int nsub, const SubProblem* subs_dev, const int* kshift, cons
 // S6: sort ascending, phase-normalise, export
 int finalize_export(int N, int batch, const int32_t* X, const int32_t* lam, const int* scale, void* eigvals_api, void* eigvecs_api,
                     int32_t* scratch /* FxC batch N N */, int32_t* lam_sorted /* FxR batch N */, int* rank /* batch N */,
-                    cudaStream_t s);
+                    cudaStream_t s, int prec = kPrec);
 
 }  // namespace zkd

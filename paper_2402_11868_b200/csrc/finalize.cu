@@ -15,7 +15,9 @@ namespace zkd {
 // Pass 1 (grid: chunks x batch): rawmax[b] <- max exponent (clamped to +-2^30; kNoExp when every entry is zero),
 // status[b] |= 3 on a malformed number.  The ingest kernel turns rawmax into the scale.
 constexpr int kNoExp = (int)0x80808080;  // what cudaMemsetAsync(.., 0x80, ..) leaves: below every clamped exponent
-__global__ void __launch_bounds__(256) maxexp_kernel(int N, const uint8_t* __restrict__ A, int* __restrict__ rawmax, int* __restrict__ status) {
+__global__ void __launch_bounds__(256) maxexp_kernel(int N, const uint8_t* __restrict__ A, int* __restrict__ rawmax, int* __restrict__ status,
+                                                     int prec) {
+  const int kApiRealBytes = 16 + (prec >> 3);
   __shared__ int s_max, s_bad;
   const int b = blockIdx.y;
   if (threadIdx.x == 0) { s_max = kNoExp; s_bad = 0; }
@@ -28,7 +30,7 @@ __global__ void __launch_bounds__(256) maxexp_kernel(int N, const uint8_t* __res
     if (i > j) continue;
     int64_t ex;
     for (int part = 0; part < (i < j ? 2 : 1); ++part) {
-      if (api_real_exp(Ab + (e * 2 + part) * kApiRealBytes, &ex, &bad)) {
+      if (api_real_exp(Ab + (e * 2 + part) * kApiRealBytes, &ex, &bad, prec)) {
         const int ec = ex > (1 << 30) ? (1 << 30) : ex < -(1 << 30) ? -(1 << 30) : (int)ex;
         if (ec > mx) mx = ec;
       }
@@ -45,7 +47,8 @@ __global__ void __launch_bounds__(256) maxexp_kernel(int N, const uint8_t* __res
 __device__ __forceinline__ int scale_from_rawmax(int rawmax) { return rawmax == kNoExp ? 0 : -rawmax - 2; }
 
 __global__ void __launch_bounds__(128) ingest_kernel(int N, int batch, const uint8_t* __restrict__ A, const int* __restrict__ rawmax,
-                                                     int* __restrict__ scale, int32_t* __restrict__ dst, int* __restrict__ status) {
+                                                     int* __restrict__ scale, int32_t* __restrict__ dst, int* __restrict__ status, int prec) {
+  const int kApiRealBytes = 16 + (prec >> 3);
   const size_t per = (size_t)N * N, count = per * batch;
   const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= 2 * count) return;
@@ -59,13 +62,13 @@ __global__ void __launch_bounds__(128) ingest_kernel(int N, int batch, const uin
   if (!(part == 1 && i == j) && status[b] == 0) {
     const int si = i <= j ? i : j, sj = i <= j ? j : i;
     const uint8_t* s = A + (((size_t)b * per + (size_t)si * N + sj) * 2 + part) * kApiRealBytes;
-    const int st = api_real_to_fx(s, sc, part == 1 && i > j, d);
+    const int st = api_real_to_fx(s, sc, part == 1 && i > j, d, prec);
     if (st) { atomicOr(&status[b], 3); fx_zero(d); }
   }
   fx_store(dst + (part ? (size_t)ND * count : 0), count, e, d);
 }
 
-int ingest_herm(int N, int batch, const void* A_api, int32_t* A_fx, int* scale /* 2 * batch ints */, int* status, cudaStream_t s) {
+int ingest_herm(int N, int batch, const void* A_api, int32_t* A_fx, int* scale /* 2 * batch ints */, int* status, cudaStream_t s, int prec) {
   KtScope kt_scope(KC_IO, s);
   int* rawmax = scale + batch;
   ZKD_CUDA_TRY(cudaMemsetAsync(rawmax, 0x80, sizeof(int) * batch, s));
@@ -73,9 +76,9 @@ int ingest_herm(int N, int batch, const void* A_api, int32_t* A_fx, int* scale /
   // enough CTAs per matrix to fill the machine when the batch is small
   const size_t per = (size_t)N * N;
   unsigned chunks = (unsigned)std::min<size_t>((per + 255) / 256, (size_t)std::max(1, 592 / batch));
-  maxexp_kernel<<<dim3(chunks, batch), 256, 0, s>>>(N, (const uint8_t*)A_api, rawmax, status);
+  maxexp_kernel<<<dim3(chunks, batch), 256, 0, s>>>(N, (const uint8_t*)A_api, rawmax, status, prec);
   const size_t t = 2 * (size_t)N * N * batch;
-  ingest_kernel<<<(unsigned)((t + 127) / 128), 128, 0, s>>>(N, batch, (const uint8_t*)A_api, rawmax, scale, A_fx, status);
+  ingest_kernel<<<(unsigned)((t + 127) / 128), 128, 0, s>>>(N, batch, (const uint8_t*)A_api, rawmax, scale, A_fx, status, prec);
   count_launch(2);
   return launch_check();
 }
@@ -450,15 +453,15 @@ __global__ void __launch_bounds__(128) phase_kernel(int N, int batch, const int3
 }
 
 int finalize_export(int N, int batch, const int32_t* X, const int32_t* lam, const int* scale, void* eigvals_api, void* eigvecs_api,
-                    int32_t* scratch, int32_t* lam_sorted, int* rank, cudaStream_t s) {
+                    int32_t* scratch, int32_t* lam_sorted, int* rank, cudaStream_t s, int prec) {
   KtScope kt_scope(KC_IO, s);
   const size_t nl = (size_t)N * batch;
   rank_kernel<<<(unsigned)((nl + 127) / 128), 128, 0, s>>>(N, batch, lam, rank, lam_sorted);
   phase_kernel<<<(unsigned)((nl * 32 + 127) / 128), 128, 0, s>>>(N, batch, X, rank, scratch);
   count_launch(2);
   ZKD_TRY(launch_check());
-  ZKD_TRY(fx_to_api_scaled(nl, lam_sorted, eigvals_api, 0, scale, 1, (size_t)N, s));
-  return fxc_to_api((size_t)N * N * batch, scratch, eigvecs_api, s);
+  ZKD_TRY(fx_to_api_scaled(nl, lam_sorted, eigvals_api, 0, scale, 1, (size_t)N, s, prec));
+  return fxc_to_api((size_t)N * N * batch, scratch, eigvecs_api, s, prec);
 }
 
 }  // namespace zkd

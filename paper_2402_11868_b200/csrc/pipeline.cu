@@ -63,6 +63,9 @@ struct Arena {
 enum { S_ERR = 0, S_MSB_R = 1, S_MSB_G = 2, S_MSB_E = 3, S_MSB_T = 4, S_GAP_INV = 5, S_NUM = 8 };
 
 struct Ctx {
+  // API precision of the call and what follows from it (NEXT-2, other precisions): results are wanted to 2^-(prec + 2) in the
+  // scaled units, so nothing below FX bit fb = 812 - (prec + 44) has to be computed (fb = 0 at 768 bit: the FX floor itself).
+  int prec = kPrec, fb = 0, tol_bits = 770;
   cudaStream_t s;
   Arena ar;
   void* gemm_ws;
@@ -191,7 +194,7 @@ int cluster_pass(Ctx& c, int n, int nb, const ClusterPlan& plan, const int* cl, 
     // These two must be exact to the FX floor, whatever the pass's precision: W = A X is kept incrementally, so an error
     // made here would stay in W for good.  Exact = all digits of X / W times all nonzero digits of M (those above cutG - 1).
     const int topM = msb_m + 1, nwM = std::max(1, std::min(kND, ceil_div(topM - (cutG - 1), kDB)));
-    const int nwXm = kND, nwWm = kND;
+    const int nwXm = digits_for(topX, c.fb), nwWm = digits_for(topW, c.fb);
     for (const ClusterGroup& g : plan.groups) {
       ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(X, n, g.m, false, topX, nwXm, g.offX), view(Gm, g.m, g.m, false, topM, nwM, g.offB), X,
                    GemmMode::Add, g.offX, nullptr));
@@ -298,7 +301,7 @@ int try_split(Ctx& c, int n, int nb, const ClusterPlan& plan, const int32_t* Sm,
     const size_t cnt = (size_t)n * n * nb;
     auto view = [&](const int32_t* fx, int rows, int cols, bool ct, int top, const int* off) {
       GemmSide g;
-      g.fx = fx; g.rows = rows; g.cols = cols; g.conj_transpose = ct; g.top_bit = top; g.nw = kND;
+      g.fx = fx; g.rows = rows; g.cols = cols; g.conj_transpose = ct; g.top_bit = top; g.nw = digits_for(top, c.fb);
       g.ld = n; g.off = off; g.plane_count = cnt;
       return g;
     };
@@ -313,7 +316,7 @@ int try_split(Ctx& c, int n, int nb, const ClusterPlan& plan, const int32_t* Sm,
     // Iteration `it` starts from an error of about 2^-(48 2^it): U^H U is needed to twice that many bits only, and the
     // correction M = (I - U^H U)/2 is then a short number (bits below the cut cleared).
     for (int it = 0; it < 6; ++it) {
-      const int cutU = std::max(1, 812 - (100 << it) - 30);
+      const int cutU = std::max(c.fb + 1, 812 - (100 << it) - 30);
       const int nwU = digits_for(815, cutU);
       for (const ClusterGroup& g : plan.groups) {
         GemmSide P = view(Um, g.m, g.m, true, 815, g.offB), Q = view(Um, g.m, g.m, false, 815, g.offB);
@@ -329,7 +332,7 @@ int try_split(Ctx& c, int n, int nb, const ClusterPlan& plan, const int32_t* Sm,
       ZKD_TRY(read_scalars(c, scal, S_NUM, hs));
       if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
       const int msb_m = hs[S_MSB_T];
-      if (msb_m <= 20 && cutU <= 1) break;  // |U^H U - I| < 2^-792
+      if (msb_m <= c.fb + 20 && cutU <= c.fb + 1) break;  // |U^H U - I| < 2^-792 (768 bit)
       if (msb_m == 0) continue;
       for (const ClusterGroup& g : plan.groups) {
         GemmSide Q = view(G2, g.m, g.m, false, msb_m + 1, g.offB);
@@ -416,7 +419,7 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
     return g;
   };
   // W = A X0 : X0 has digits 27..29 only
-  ZKD_TRY(gemm_complex(n, n, n, nb, side(A, topA, kND, false), side(Xc, topX, 3, false), Wc, GemmMode::Assign, -1, opt.gemm_path,
+  ZKD_TRY(gemm_complex(n, n, n, nb, side(A, topA, digits_for(topA, c.fb), false), side(Xc, topX, 3, false), Wc, GemmMode::Assign, -1, opt.gemm_path,
                        c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s));
 
   ZKD_CUDA_TRY(cudaMemcpyAsync(cl0, cl, sizeof(int) * n * nb, cudaMemcpyDeviceToDevice, s));
@@ -439,14 +442,16 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
   int status = 2, steps = 0, prev_msb_r = 1 << 30;
   int e_prev = 15, last_cut = 0;  // error level of the previous pass (2^-e_prev), precision of the current one
   int hs[S_NUM];
-  const int tol_msb = 812 - opt.tol_bits;
+  const int tol_msb = 812 - c.tol_bits;
+  const int orth_ok = 812 - (c.tol_bits / 2 + 15);  // Newton-Schulz squares the deviation: 2^-400 -> 2^-800 at 768 bit
+  const int fb = c.fb;
   for (int step = 0; step < opt.max_steps; ++step) {
     if (singletons) {
       // S4f + S4c fused: normalise columns, Rayleigh quotients, residual (X, W in place)
       ZKD_TRY(singleton_step(n, nb, Xc, Wc, R, Sm, theta, scal + S_MSB_G, scal + S_MSB_R, s, nullptr, nullptr, pm + nb));
     } else {
       // S4f + S4c on cluster views.  Results are needed to about 2^-(2 e_now + 40) and e_now <= 2 e_prev + 45.
-      last_cut = 812 - (4 * e_prev + 130);
+      last_cut = std::max(fb, 812 - (4 * e_prev + 130));
       ZKD_TRY(cluster_pass(c, n, nb, plan, cl, cle, Xc, Wc, R, Sm, Gm, theta, scal, last_cut, fxc, pm + nb));
     }
     ZKD_TRY(min_gap(n, nb, theta, cl, scal + S_GAP_INV, s));
@@ -459,9 +464,9 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
     if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
     steps = step;
     if (st) { st->msb_r = msb_r; st->msb_g = msb_g; }
-    const bool exact_pass = singletons || last_cut <= 0;  // a windowed pass cannot certify convergence
-    if (exact_pass && msb_r <= tol_msb && msb_g <= 812 - 400) { status = 0; break; }
-    if (exact_pass && step > 0 && msb_r > tol_msb && msb_r >= prev_msb_r - 2 && msb_g <= 812 - 400) { status = 1; break; }
+    const bool exact_pass = singletons || last_cut <= fb;  // a windowed pass cannot certify convergence
+    if (exact_pass && msb_r <= tol_msb && msb_g <= orth_ok) { status = 0; break; }
+    if (exact_pass && step > 0 && msb_r > tol_msb && msb_r >= prev_msb_r - 2 && msb_g <= orth_ok) { status = 1; break; }
     e_prev = std::max(15, 812 - msb_r);
     if (step + 1 == opt.max_steps) break;
     prev_msb_r = msb_r;
@@ -490,7 +495,7 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
 
     // S4d: C = X^H R on windows sized for this step's gain
     const int e = 812 - msb_r;                        // residual ~ 2^-e
-    const int pb = std::max(40, std::min(e + 40, msb_r + 30)) + gap_extra;  // relative bits worth computing for the correction
+    const int pb = std::max(40, std::min(e + 40, msb_r - fb + 30)) + gap_extra;  // relative bits worth computing for the correction
     const int nwX = ceil_div(pb + 3, 28);
     const int topR = msb_r + 2, nwR = ceil_div(pb + 2, 28);
     ZKD_TRY(gemm_complex(n, n, n, nb, side(Xc, topX, nwX, true), side(R, topR, nwR, false), Cc, GemmMode::Assign, -1, opt.gemm_path,
@@ -503,13 +508,13 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
     const int pbE = pb + 8;
     // S4e: T = X E (bits below cutT cleared so that W += A T tracks A X exactly), X += T, W += A T
     const int topE = msb_e + 2, nwE = ceil_div(pbE + 2, 28);
-    const int cutT = std::max(0, msb_e - pbE - 4);
+    const int cutT = std::max(fb, msb_e - pbE - 4);
     ZKD_TRY(gemm_complex(n, n, n, nb, side(Xc, topX, nwX, false), side(Cc, topE, nwE, false), Tc, GemmMode::Assign, cutT, opt.gemm_path,
                          c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s));
     ZKD_TRY(fxc_add_inplace(cnt, Xc, Tc, s));
     const int topT = msb_e + ilog2_ceil(n) + 2;
     const int nwT = ceil_div(topT - cutT, 28);
-    const int nwA = std::min(kND, ceil_div(topT, 28));
+    const int nwA = std::max(1, std::min(kND, ceil_div(topT - fb, 28)));
     ZKD_TRY(gemm_complex(n, n, n, nb, side(A, topA, nwA, false), side(Tc, topT, nwT, false), Wc, GemmMode::Add, -1, opt.gemm_path,
                          c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s));
   }
@@ -539,16 +544,16 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
       };
       ZKD_CUDA_TRY(cudaMemsetAsync(scal, 0, sizeof(int) * S_NUM, s));
       for (const ClusterGroup& g : plan0.groups)
-        ZKD_TRY(gemm(g.m, g.m, n, g.nsub, view(Xc, n, g.m, true, topX, kND, g.offX), view(Xc, n, g.m, false, topX, kND, g.offX), Gm,
-                     GemmMode::Assign, g.offB));
+        ZKD_TRY(gemm(g.m, g.m, n, g.nsub, view(Xc, n, g.m, true, topX, digits_for(topX, fb), g.offX),
+                     view(Xc, n, g.m, false, topX, digits_for(topX, fb), g.offX), Gm, GemmMode::Assign, g.offB));
       ZKD_TRY(ns_build(n, nb, cl0, Gm, scal + S_MSB_G, s, cle0));
       ZKD_TRY(read_scalars(c, scal, S_NUM, hs));
       if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
       const int msb_m = hs[S_MSB_G];
       if (msb_m > 0) {
-        const int topM = msb_m + 1, nwM = std::max(1, std::min(kND, ceil_div(topM, kDB)));
+        const int topM = msb_m + 1, nwM = std::max(1, std::min(kND, ceil_div(topM - fb, kDB)));
         for (const ClusterGroup& g : plan0.groups)
-          ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(Xc, n, g.m, false, topX, kND, g.offX), view(Gm, g.m, g.m, false, topM, nwM, g.offB), Xc,
+          ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(Xc, n, g.m, false, topX, digits_for(topX, fb), g.offX), view(Gm, g.m, g.m, false, topM, nwM, g.offB), Xc,
                        GemmMode::Add, g.offX));
       }
     }
@@ -602,8 +607,8 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
       const size_t cntf = (size_t)n * n * nb;
       for (const ClusterGroup& g : planf.groups) {
         GemmSide P, Q;
-        P.fx = X; P.rows = n; P.cols = g.m; P.conj_transpose = false; P.top_bit = topX; P.nw = kND; P.ld = n; P.off = g.offX; P.plane_count = cntf;
-        Q.fx = Um; Q.rows = g.m; Q.cols = g.m; Q.conj_transpose = false; Q.top_bit = topX; Q.nw = kND; Q.ld = n; Q.off = g.offB; Q.plane_count = cntf;
+        P.fx = X; P.rows = n; P.cols = g.m; P.conj_transpose = false; P.top_bit = topX; P.nw = digits_for(topX, fb); P.ld = n; P.off = g.offX; P.plane_count = cntf;
+        Q.fx = Um; Q.rows = g.m; Q.cols = g.m; Q.conj_transpose = false; Q.top_bit = topX; Q.nw = digits_for(topX, fb); Q.ld = n; Q.off = g.offB; Q.plane_count = cntf;
         GemmDstView dv;
         dv.ld = n; dv.off = g.offX; dv.plane_count = cntf;
         ZKD_TRY(gemm_complex(n, g.m, g.m, g.nsub, P, Q, X, GemmMode::Assign, -1, opt.gemm_path, c.gemm_ws, c.gemm_ws_bytes, nullptr, nullptr,
@@ -665,9 +670,12 @@ size_t diag_workspace_bytes(int N, int batch) {
   return 2 * level_bytes(N, batch) + gemm_workspace_bytes(N, N, N, batch) + (32u << 20);
 }
 
-int diag_herm_device(int N, int batch, const void* A_api, void* eigvals_api, void* eigvecs_api, void* ws, size_t ws_bytes,
+int diag_herm_device(int N, int batch, int prec, const void* A_api, void* eigvals_api, void* eigvecs_api, void* ws, size_t ws_bytes,
                      zkd_info* info, cudaStream_t s) {
   Ctx c;
+  c.prec = prec;
+  c.tol_bits = std::min(options().tol_bits, 790) - (kPrec - prec);  // "tol_bits" is quoted at 768 bit: prec + 2 by default
+  c.fb = std::max(0, kFRAC - (c.tol_bits + 42));
   c.s = s;
   c.ar.base = (char*)ws;
   c.ar.size = ws_bytes;
@@ -688,7 +696,7 @@ int diag_herm_device(int N, int batch, const void* A_api, void* eigvals_api, voi
   int* pm = c.ar.get<int>((size_t)2 * batch);
   if (!c.gemm_ws || !A || !X || !lam || !lam_sorted || !scale || !status || !rank || !cl_stats_dev || !pm) return ZKD_ERR_WORKSPACE;
 
-  ZKD_TRY(ingest_herm(N, batch, A_api, A, scale, status, s));
+  ZKD_TRY(ingest_herm(N, batch, A_api, A, scale, status, s, prec));
   LevelStats st;
   {
     const int rc = solve_level(c, N, batch, A, X, lam, 0, nullptr, &st, pm);
@@ -697,14 +705,14 @@ int diag_herm_device(int N, int batch, const void* A_api, void* eigvals_api, voi
       return rc;
     }
   }
-  ZKD_TRY(finalize_export(N, batch, X, lam, scale, eigvals_api, eigvecs_api, A /* scratch: A is dead */, lam_sorted, rank, s));
+  ZKD_TRY(finalize_export(N, batch, X, lam, scale, eigvals_api, eigvecs_api, A /* scratch: A is dead */, lam_sorted, rank, s, prec));
   if (info) {
     const int* cs = nullptr;
     if (!st.cl_stats.empty()) {
       ZKD_CUDA_TRY(cudaMemcpyAsync(cl_stats_dev, st.cl_stats.data(), sizeof(int) * 2 * batch, cudaMemcpyHostToDevice, s));
       cs = cl_stats_dev;
     }
-    info_kernel<<<(batch + 127) / 128, 128, 0, s>>>(batch, status, st.status, st.steps, 812 - options().tol_bits, pm, cs, info);
+    info_kernel<<<(batch + 127) / 128, 128, 0, s>>>(batch, status, st.status, st.steps, 812 - c.tol_bits, pm, cs, info);
     count_launch();
     ZKD_TRY(launch_check());
     // st.cl_stats must outlive the async copy

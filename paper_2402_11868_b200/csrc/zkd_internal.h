@@ -12,8 +12,8 @@ constexpr int kND = ZKD_FX_DIGITS;   // 30
 constexpr int kDB = 28;
 constexpr int kFRAC = ZKD_FX_FRAC_BITS;
 constexpr int kFxBits = kND * kDB;   // 840 (the top digit really has 32 bits)
-constexpr int kPrec = 768;
-constexpr int kApiRealBytes = 16 + kPrec / 8;  // 112
+constexpr int kPrec = 768;                      // the largest (and default) API precision
+constexpr int kApiRealBytes = 16 + kPrec / 8;  // 112, at kPrec
 
 // ---- error plumbing ---------------------------------------------------------------------------------------------
 #define ZKD_CUDA_TRY(expr)                         \
@@ -105,22 +105,25 @@ int gemm_complex(int M, int N, int K, int batch, const GemmSide& P, const GemmSi
 uint64_t gemm_complex_macs(int M, int N, int K, int batch, int nwP, int nwQ, int* inst_np, int* inst_nq);
 
 // ---- pipeline pieces --------------------------------------------------------------------------------------------
-int fx_from_api(int count, const void* src_api, int32_t* dst_fx, int scale_bits, cudaStream_t s);
-int fx_to_api(int count, const int32_t* src_fx, void* dst_api, int scale_bits, cudaStream_t s);
+int fx_from_api(int count, const void* src_api, int32_t* dst_fx, int scale_bits, cudaStream_t s, int prec = kPrec);
+int fx_to_api(int count, const int32_t* src_fx, void* dst_api, int scale_bits, cudaStream_t s, int prec = kPrec);
+// supported API precisions: multiples of 64 from 128 to 768 bits (PAPER.md:41 768, :61 256, :65 128)
+inline bool prec_supported(int prec) { return prec >= 128 && prec <= kPrec && (prec & 63) == 0; }
+inline size_t api_real_bytes(int prec) { return 16 + (size_t)prec / 8; }
 int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int max_sweeps, cudaStream_t s);
 
 size_t diag_workspace_bytes(int N, int batch);
-int diag_herm_device(int N, int batch, const void* A_api, void* eigvals_api, void* eigvecs_api, void* ws, size_t ws_bytes,
+int diag_herm_device(int N, int batch, int prec, const void* A_api, void* eigvals_api, void* eigvecs_api, void* ws, size_t ws_bytes,
                      zkd_info* info, cudaStream_t s);
 
 }  // namespace zkd
 
 namespace zkd {
 int fx_from_api_scaled(size_t count, const void* src_api, int32_t* dst_fx, int scale_bits, const int* scale_dev,
-                       int scale_stride, size_t per_scale, int* status, cudaStream_t s);
+                       int scale_stride, size_t per_scale, int* status, cudaStream_t s, int prec = kPrec);
 int fx_to_api_scaled(size_t count, const int32_t* src_fx, void* dst_api, int scale_bits, const int* scale_dev, int scale_stride,
-                     size_t per_scale, cudaStream_t s);
-int fxc_to_api(size_t count, const int32_t* src_fxc, void* dst_api, cudaStream_t s);
+                     size_t per_scale, cudaStream_t s, int prec = kPrec);
+int fxc_to_api(size_t count, const int32_t* src_fxc, void* dst_api, cudaStream_t s, int prec = kPrec);
 int fx_prim(int op, size_t count, const int32_t* a, const int32_t* b, int32_t* out, cudaStream_t s);
 int measure_imad_peak(double millis, double* per_sec, cudaStream_t s);
 int measure_dfma_peak(double millis, double* flops_per_sec, cudaStream_t s);

@@ -326,7 +326,7 @@ def test_argument_errors(zkd):
     t = torch.zeros(1 << 16, dtype=torch.uint8, device="cuda")
     L = zkd.lib()
     assert L.zkd_diag_herm_ws(0, 1, 768, t.data_ptr(), t.data_ptr(), t.data_ptr(), t.data_ptr(), 1 << 16, None, None) == -1
-    assert L.zkd_diag_herm_ws(4, 1, 512, t.data_ptr(), t.data_ptr(), t.data_ptr(), t.data_ptr(), 1 << 16, None, None) == -2
+    assert L.zkd_diag_herm_ws(4, 1, 100, t.data_ptr(), t.data_ptr(), t.data_ptr(), t.data_ptr(), 1 << 16, None, None) == -2
     assert L.zkd_diag_herm_ws(4, 1, 768, t.data_ptr(), t.data_ptr(), t.data_ptr(), t.data_ptr(), 16, None, None) == -3
     assert L.zkd_diag_herm_ws(4, 1, 768, t.data_ptr() + 4, t.data_ptr(), t.data_ptr(), t.data_ptr(), 1 << 16, None, None) == -1
     assert L.zkd_diag_herm_ws(4, 1, 768, None, t.data_ptr(), t.data_ptr(), t.data_ptr(), 1 << 16, None, None) == -1

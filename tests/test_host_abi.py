@@ -59,6 +59,24 @@ def test_real_bytes_and_strerror(L):
     assert len({L.zkd_strerror(-k) for k in range(1, 6)}) >= 4
 
 
+def test_other_precisions_host_helpers(L):
+    """NEXT-2: multiples of 64 bits from 128 to 768 (PAPER.md:61 256 bit, :65 128 bit)."""
+    import paper_2402_11868_b200 as z
+
+    for prec in (128, 192, 256, 512, 768):
+        assert L.zkd_real_bytes(prec) == 16 + prec // 8
+        n = prec // 64
+        limbs = [(0x9E3779B97F4A7C15 * (k + 3)) & 0xFFFFFFFFFFFFFFFF for k in range(n)]
+        limbs[-1] |= 1 << 63
+        raw = z.pack(1, 5, limbs, prec)
+        assert len(raw) == 16 + prec // 8
+        assert z.unpack(raw, prec) == (1, 5, limbs)
+        for v in (0.0, 1.0, -0.3125, 3.0e-200, -7.5e250):
+            assert z.to_double(z.from_double(v, prec), prec) == v
+    for prec in (0, 64, 100, 832, 1024):
+        assert L.zkd_real_bytes(prec) == 0
+
+
 def test_pack_unpack_layout(L):
     # layout of one real (DESIGN.md 2): int32 sign, int32 flags, int64 exp, uint64 limb[12] little-endian
     limbs = [(0x0123456789ABCDEF * (k + 1)) & 0xFFFFFFFFFFFFFFFF for k in range(12)]
@@ -104,7 +122,7 @@ def test_argument_validation_needs_no_gpu(L):
     assert L.zkd_diag_herm_bufsize(64, 4, 768, ctypes.byref(n)) == 0 and n.value > small
     assert L.zkd_diag_herm_bufsize(0, 1, 768, ctypes.byref(n)) < 0
     assert L.zkd_diag_herm_bufsize(8, 0, 768, ctypes.byref(n)) < 0
-    assert L.zkd_diag_herm_bufsize(8, 1, 512, ctypes.byref(n)) < 0
+    assert L.zkd_diag_herm_bufsize(8, 1, 100, ctypes.byref(n)) == -2  # unsupported precision
     assert L.zkd_diag_herm_bufsize(8, 1, 768, None) < 0
     # NULL pointers are refused before anything touches CUDA
     assert L.zkd_diag_herm_ws(8, 1, 768, None, None, None, None, 0, None, None) < 0
