@@ -44,6 +44,10 @@ def lib():
                                            ctypes.c_long, vp, vp, vp, vp]
         L.zkd_oracle_compare.restype = ctypes.c_int
         L.zkd_oracle_compare.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, vp, vp, vp, vp, vp, ctypes.c_int, vp]
+        L.zkd_oracle_svd.restype = ctypes.c_int
+        L.zkd_oracle_svd.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, vp, vp, vp, vp]
+        L.zkd_oracle_svd_compare.restype = ctypes.c_int
+        L.zkd_oracle_svd_compare.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, vp, vp, vp, vp, vp, vp, vp]
         L.zkd_oracle_api_to_double.restype = ctypes.c_double
         L.zkd_oracle_api_to_double.argtypes = [vp, ctypes.c_int]
         L.zkd_oracle_api_from_double.argtypes = [vp, ctypes.c_int, ctypes.c_double]
@@ -95,6 +99,33 @@ def compare(A: np.ndarray, N: int, lam: np.ndarray, X: np.ndarray, lam0: np.ndar
     return {"log2_dlam_rel": out[0], "log2_resid_rel": out[1], "log2_orth": out[2], "vec_margin_bits": out[3],
             "log2_F": out[4], "groups": int(out[5]) if out[5] > -1e8 else 0,
             "max_group": int(out[6]) if out[6] > -1e8 else 0, "log2_vec_err": out[7]}
+
+
+def svd(A: np.ndarray, M: int, N: int, prec: int = PREC, guard_bits: int = GUARD_BITS):
+    """One-sided Jacobi SVD of ONE M x N complex matrix in the API layout (NEXT-1).
+    Returns (S uint8[K*rb] descending, U uint8[M*K*2*rb], V uint8[N*K*2*rb], info dict), K = min(M, N)."""
+    rb = real_bytes(prec)
+    K = min(M, N)
+    A = np.ascontiguousarray(A, dtype=np.uint8)
+    assert A.size == M * N * 2 * rb, (A.size, M, N)
+    S = np.zeros(K * rb, dtype=np.uint8)
+    U = np.zeros(M * K * 2 * rb, dtype=np.uint8)
+    V = np.zeros(N * K * 2 * rb, dtype=np.uint8)
+    info = (ctypes.c_long * 3)()
+    rc = lib().zkd_oracle_svd(M, N, prec, guard_bits, A.ctypes.data, S.ctypes.data, U.ctypes.data, V.ctypes.data, info)
+    return S, U, V, {"status": rc, "sweeps": info[0], "rotations": info[1]}
+
+
+def svd_compare(A: np.ndarray, M: int, N: int, S, U, V, S0=None, U0=None, V0=None, prec: int = PREC) -> dict:
+    """Comparator for singular value decompositions (see zkd_oracle_svd_compare)."""
+    out = np.zeros(8, dtype=np.float64)
+    def p(x):
+        return np.ascontiguousarray(x).ctypes.data if x is not None else None
+    keep = [np.ascontiguousarray(x) for x in (A, S, U, V)] + [np.ascontiguousarray(x) for x in (S0, U0, V0) if x is not None]
+    lib().zkd_oracle_svd_compare(M, N, prec, keep[0].ctypes.data, keep[1].ctypes.data, keep[2].ctypes.data, keep[3].ctypes.data,
+                                 p(S0), p(U0), p(V0), out.ctypes.data)
+    return {"log2_dsig_rel": out[0], "log2_resid_rel": out[1], "log2_orth": out[2], "vec_margin_bits": out[3], "log2_F": out[4],
+            "groups": int(out[5]) if out[5] > -1e8 else 0, "max_group": int(out[6]) if out[6] > -1e8 else 0, "log2_vec_err": out[7]}
 
 
 def api_to_double(buf, prec: int = PREC) -> float:

@@ -71,6 +71,7 @@ int mpfr_cmp(mpfr_srcptr, mpfr_srcptr);
 int mpfr_cmpabs(mpfr_srcptr, mpfr_srcptr);
 int mpfr_cmp_ui(mpfr_srcptr, unsigned long);
 int mpfr_cmp_si(mpfr_srcptr, long);
+int mpfr_cmp_d(mpfr_srcptr, double);
 int mpfr_sgn(mpfr_srcptr);
 int mpfr_zero_p(mpfr_srcptr);
 void mpfr_swap(mpfr_ptr, mpfr_ptr);

@@ -595,3 +595,395 @@ void zkd_oracle_api_from_double(uint8_t *dst, int prec, double v) {
 }
 const char *zkd_oracle_mpfr_version(void) { return mpfr_get_version(); }
 int zkd_oracle_max_threads(void) { return omp_get_max_threads(); }
+
+/* ================================================================================================ */
+/* Singular value decomposition                                              */
+/* ================================================================================================ */
+/* PAPER.md:31, :33 (section 2): ZKCM_CUS ships two routines, Hermitian diagonalisation and "singular value decomposition";
+ * PAPER.md:49 (section 2.2): ZKCM_QC switches both.  Result definition (plain): for A in C^{M x N}, K = min(M, N):
+ * sigma_1 >= ... >= sigma_K >= 0, U (M x K) and V (N x K) with orthonormal columns, A V = U diag(sigma),
+ * A^H U = V diag(sigma).  Computed by the textbook one-sided Jacobi method (Hestenes) on MPFR:
+ *   1. working precision P_o = prec + guard_bits.  If M < N work on A^H and swap U and V at the end.  B = A, W = I (N x N).
+ *   2. sweeps over all column pairs p < q (row-cyclic): alpha = ||b_p||^2, beta = ||b_q||^2, gamma = b_p^H b_q;
+ *      skip if |gamma| <= 2^-(P_o-8) sqrt(alpha beta) (the computed gamma carries rounding noise of about 2^-P_o sqrt(alpha
+ *      beta): a threshold below that would rotate on noise for ever); else rotate with the SAME formulas as the eigenvalue oracle applied
+ *      to the 2 x 2 Gram matrix [[alpha, gamma], [conj gamma, beta]]:  zeta = (beta - alpha) / (2|gamma|),
+ *      t = sgn(zeta) / (|zeta| + sqrt(1 + zeta^2)), c = 1/sqrt(1 + t^2), s = t c, sg = s gamma/|gamma|,
+ *      (b_p, b_q) <- (c b_p - conj(sg) b_q, sg b_p + c b_q), same on (w_p, w_q).
+ *      Stop when a sweep applied no rotation; fail after 80 sweeps.
+ *   3. sigma_j = ||b_j||; sort descending (stable); v_j = w_j; u_j = b_j / sigma_j; when sigma_j <= 2^-(prec+32) F the
+ *      direction of b_j is noise: sigma_j is kept as computed and u_j is completed by Gram-Schmidt (twice) of the unit
+ *      vectors e_0, e_1, ... against the columns already fixed.
+ *   4. phase: the first component of largest modulus of v_j is made real positive (the same factor on u_j); unit norm;
+ *      round to prec bits.
+ * Layout: A[i][j] row-major complex (M x N); S[j] real; U[i][j] (M x K), V[i][j] (N x K) row-major complex.
+ * info[0] = sweeps, info[1] = rotations, info[2] = status (0 ok, 2 not converged, 3 malformed).
+ * Parity status: pinned (tests/test_oracle_pins.py, section "SVD": 2 x 2 closed form, constructed U S V^H, sigma^2 =
+ * eigenvalues of A^H A by the eigenvalue oracle, ||A||_F^2 = sum sigma^2, diagonal / rank-deficient / zero inputs,
+ * mpmath.svd_c as a third opinion). */
+
+typedef struct { int r, c; __mpfr_struct *re, *im; } rmat;
+static rmat rmat_alloc(int r, int c, long prec) {
+  rmat m; m.r = r; m.c = c;
+  m.re = vec_alloc((size_t)r * c, prec); m.im = vec_alloc((size_t)r * c, prec);
+  return m;
+}
+static void rmat_free(rmat *m) { vec_free(m->re, (size_t)m->r * m->c); vec_free(m->im, (size_t)m->r * m->c); }
+#define RRE(m, i, j) (&(m).re[(size_t)(i) * (m).c + (j)])
+#define RIM(m, i, j) (&(m).im[(size_t)(i) * (m).c + (j)])
+
+/* acc <- x_p^H x_q over the rows of m (ar + i ai) */
+static void col_dot(mpfr_ptr ar, mpfr_ptr ai, const rmat *m, int p, int q, mpfr_ptr w) {
+  mpfr_set_zero(ar, +1); mpfr_set_zero(ai, +1);
+  for (int k = 0; k < m->r; ++k) {
+    /* conj(x_p) x_q = (pr qr + pi qi) + i (pr qi - pi qr) */
+    mpfr_fmma(w, RRE(*m, k, p), RRE(*m, k, q), RIM(*m, k, p), RIM(*m, k, q), RN); mpfr_add(ar, ar, w, RN);
+    mpfr_fmms(w, RRE(*m, k, p), RIM(*m, k, q), RIM(*m, k, p), RRE(*m, k, q), RN); mpfr_add(ai, ai, w, RN);
+  }
+}
+
+int zkd_oracle_svd(int M, int N, int prec, int guard_bits, const uint8_t *A_api, uint8_t *S_api, uint8_t *U_api,
+                   uint8_t *V_api, long *info) {
+  const long Po = (long)prec + guard_bits;
+  const size_t rb = api_real_bytes(prec);
+  long sweeps = 0, rotations = 0;
+  int status = 0;
+  if (info) info[0] = info[1] = info[2] = 0;
+  if (M < 1 || N < 1 || prec < 64 || prec % 64) { if (info) info[2] = 3; return 3; }
+  const int tr = M < N;              /* work on A^H */
+  const int R = tr ? N : M, C = tr ? M : N, K = C;
+  mpfr_t tmpP, F, w, al, be, gr, gi, thr2, zt;
+  mpfr_init2(tmpP, prec); mpfr_init2(F, Po); mpfr_init2(w, Po); mpfr_init2(al, Po); mpfr_init2(be, Po);
+  mpfr_init2(gr, Po); mpfr_init2(gi, Po); mpfr_init2(thr2, Po); mpfr_init2(zt, Po);
+  rmat B = rmat_alloc(R, C, Po), W = rmat_alloc(C, C, Po), Uo = rmat_alloc(R, K, Po);
+  __mpfr_struct *sig = vec_alloc((size_t)C, Po);
+  rot_t rt; rot_init(&rt, Po);
+  int *ord = (int *)malloc(sizeof(int) * (size_t)C);
+
+  for (int i = 0; i < M && !status; ++i)
+    for (int j = 0; j < N; ++j) {
+      const uint8_t *src = A_api + ((size_t)i * N + j) * 2 * rb;
+      mpfr_ptr dr = tr ? RRE(B, j, i) : RRE(B, i, j), di = tr ? RIM(B, j, i) : RIM(B, i, j);
+      if (api_get(dr, src, prec, tmpP) || api_get(di, src + rb, prec, tmpP)) { status = 3; break; }
+      if (tr) mpfr_neg(di, di, RN);
+    }
+  if (status) goto done;
+  for (int i = 0; i < C; ++i) mpfr_set_ui(RRE(W, i, i), 1, RN);
+  mpfr_set_zero(F, +1);
+  for (int i = 0; i < R; ++i)
+    for (int j = 0; j < C; ++j) {
+      mpfr_sqr(w, RRE(B, i, j), RN); mpfr_add(F, F, w, RN);
+      mpfr_sqr(w, RIM(B, i, j), RN); mpfr_add(F, F, w, RN);
+    }
+  mpfr_sqrt(F, F, RN);
+
+  /* step 2 */
+  for (;;) {
+    if (sweeps >= 80) { status = 2; break; }
+    long applied = 0;
+    for (int p = 0; p < C - 1; ++p)
+      for (int q = p + 1; q < C; ++q) {
+        col_dot(al, w, &B, p, p, zt);
+        col_dot(be, w, &B, q, q, zt);
+        col_dot(gr, gi, &B, p, q, zt);
+        /* skip if |gamma|^2 <= 2^-(2 Po - 16) alpha beta */
+        mpfr_sqr(rt.w1, gr, RN); mpfr_sqr(rt.w2, gi, RN); mpfr_add(rt.w1, rt.w1, rt.w2, RN); /* |gamma|^2 */
+        mpfr_mul(thr2, al, be, RN); mpfr_div_2si(thr2, thr2, 2 * Po - 16, RN);
+        if (mpfr_zero_p(rt.w1) || mpfr_cmp(rt.w1, thr2) <= 0) continue;
+        mpfr_sqrt(rt.absb, rt.w1, RN);
+        mpfr_sub(rt.w1, be, al, RN);
+        mpfr_mul_2si(rt.w2, rt.absb, 1, RN);
+        mpfr_div(rt.zeta, rt.w1, rt.w2, RN);
+        int neg = mpfr_sgn(rt.zeta) < 0;
+        mpfr_sqr(rt.w1, rt.zeta, RN); mpfr_add_ui(rt.w1, rt.w1, 1, RN); mpfr_sqrt(rt.w1, rt.w1, RN);
+        mpfr_abs(rt.w2, rt.zeta, RN); mpfr_add(rt.w1, rt.w1, rt.w2, RN);
+        mpfr_ui_div(rt.t, 1, rt.w1, RN);
+        if (neg) mpfr_neg(rt.t, rt.t, RN);
+        mpfr_sqr(rt.w1, rt.t, RN); mpfr_add_ui(rt.w1, rt.w1, 1, RN); mpfr_sqrt(rt.w1, rt.w1, RN);
+        mpfr_ui_div(rt.c, 1, rt.w1, RN);
+        mpfr_mul(rt.w2, rt.t, rt.c, RN); mpfr_div(rt.w2, rt.w2, rt.absb, RN);
+        mpfr_mul(rt.sr, rt.w2, gr, RN); mpfr_mul(rt.si, rt.w2, gi, RN);
+        for (int k = 0; k < R; ++k) rot_apply(&rt, RRE(B, k, p), RIM(B, k, p), RRE(B, k, q), RIM(B, k, q), +1);
+        for (int k = 0; k < C; ++k) rot_apply(&rt, RRE(W, k, p), RIM(W, k, p), RRE(W, k, q), RIM(W, k, q), +1);
+        ++applied;
+      }
+    rotations += applied;
+    ++sweeps;
+    if (applied == 0) break;
+  }
+
+  /* step 3 */
+  for (int j = 0; j < C; ++j) { col_dot(&sig[j], w, &B, j, j, zt); mpfr_sqrt(&sig[j], &sig[j], RN); ord[j] = j; }
+  for (int i = 1; i < C; ++i) { /* insertion sort, descending, stable */
+    int k = ord[i], j = i - 1;
+    while (j >= 0 && mpfr_cmp(&sig[ord[j]], &sig[k]) < 0) { ord[j + 1] = ord[j]; --j; }
+    ord[j + 1] = k;
+  }
+  mpfr_div_2si(thr2, F, prec + 32, RN); /* directions of columns shorter than this are noise */
+  {
+    int next_e = 0;
+    for (int jj = 0; jj < K; ++jj) {
+      int j = ord[jj];
+      if (mpfr_cmp(&sig[j], thr2) > 0) {
+        for (int k = 0; k < R; ++k) { mpfr_div(RRE(Uo, k, jj), RRE(B, k, j), &sig[j], RN); mpfr_div(RIM(Uo, k, jj), RIM(B, k, j), &sig[j], RN); }
+        continue;
+      }
+      for (; next_e < R; ++next_e) { /* complete by Gram-Schmidt of unit vectors (only reached for rank-deficient input) */
+        for (int k = 0; k < R; ++k) { mpfr_set_zero(RRE(Uo, k, jj), +1); mpfr_set_zero(RIM(Uo, k, jj), +1); }
+        mpfr_set_ui(RRE(Uo, next_e, jj), 1, RN);
+        for (int pass = 0; pass < 2; ++pass)
+          for (int c2 = 0; c2 < K; ++c2) {
+            /* orthogonalise against every column already fixed: earlier ones and all later non-noise ones */
+            int fixed = c2 < jj || (c2 > jj && mpfr_cmp(&sig[ord[c2]], thr2) > 0);
+            if (!fixed) continue;
+            if (c2 > jj) { /* later non-noise column: its u is b / sigma, not stored yet */
+              for (int k = 0; k < R; ++k) { mpfr_div(RRE(Uo, k, c2), RRE(B, k, ord[c2]), &sig[ord[c2]], RN); mpfr_div(RIM(Uo, k, c2), RIM(B, k, ord[c2]), &sig[ord[c2]], RN); }
+            }
+            col_dot(gr, gi, &Uo, c2, jj, zt); /* u_c2^H x */
+            for (int k = 0; k < R; ++k) {
+              mpfr_fmms(w, RRE(Uo, k, c2), gr, RIM(Uo, k, c2), gi, RN); mpfr_sub(RRE(Uo, k, jj), RRE(Uo, k, jj), w, RN);
+              mpfr_fmma(w, RRE(Uo, k, c2), gi, RIM(Uo, k, c2), gr, RN); mpfr_sub(RIM(Uo, k, jj), RIM(Uo, k, jj), w, RN);
+            }
+          }
+        col_dot(al, w, &Uo, jj, jj, zt);
+        if (mpfr_cmp_d(al, 0.25) > 0) {
+          mpfr_sqrt(al, al, RN);
+          for (int k = 0; k < R; ++k) { mpfr_div(RRE(Uo, k, jj), RRE(Uo, k, jj), al, RN); mpfr_div(RIM(Uo, k, jj), RIM(Uo, k, jj), al, RN); }
+          ++next_e;
+          break;
+        }
+      }
+    }
+  }
+  /* step 4: phase from v_j (in the caller's orientation: V is W unless the problem was transposed, then V is Uo) */
+  for (int jj = 0; jj < K; ++jj) {
+    int j = ord[jj];
+    const rmat *Vsrc = tr ? &Uo : &W;
+    int vcol = tr ? jj : j, vrows = tr ? R : C;
+    int kstar = 0;
+    mpfr_set_si(be, -1, RN);
+    mpfr_set_zero(al, +1);
+    for (int k = 0; k < vrows; ++k) {
+      mpfr_sqr(gr, RRE(*Vsrc, k, vcol), RN); mpfr_sqr(w, RIM(*Vsrc, k, vcol), RN); mpfr_add(gr, gr, w, RN);
+      mpfr_add(al, al, gr, RN);
+      if (mpfr_cmp(gr, be) > 0) { mpfr_set(be, gr, RN); kstar = k; }
+    }
+    mpfr_sqrt(be, be, RN);
+    /* phase factor f = conj(x_k*) / |x_k*| */
+    mpfr_div(gr, RRE(*Vsrc, kstar, vcol), be, RN);
+    mpfr_div(gi, RIM(*Vsrc, kstar, vcol), be, RN); mpfr_neg(gi, gi, RN);
+    if (S_api) api_put(S_api + (size_t)jj * rb, &sig[j], prec, tmpP);
+    for (int side = 0; side < 2; ++side) {
+      /* side 0: the caller's U, side 1: the caller's V */
+      const int from_uo = tr ? side == 1 : side == 0;
+      const rmat *src = from_uo ? &Uo : &W;
+      const int col = from_uo ? jj : j, rows = from_uo ? R : C;
+      uint8_t *dst0 = side == 0 ? U_api : V_api;
+      if (!dst0) continue;
+      col_dot(al, w, src, col, col, zt); mpfr_sqrt(al, al, RN); /* unit norm */
+      for (int k = 0; k < rows; ++k) {
+        mpfr_fmms(be, RRE(*src, k, col), gr, RIM(*src, k, col), gi, RN); mpfr_div(be, be, al, RN);
+        mpfr_fmma(w, RRE(*src, k, col), gi, RIM(*src, k, col), gr, RN); mpfr_div(w, w, al, RN);
+        if (side == 1 && k == kstar) mpfr_set_zero(w, +1);
+        uint8_t *dst = dst0 + ((size_t)k * K + jj) * 2 * rb;
+        api_put(dst, be, prec, tmpP);
+        api_put(dst + rb, w, prec, tmpP);
+      }
+    }
+  }
+
+done:
+  rmat_free(&B); rmat_free(&W); rmat_free(&Uo); vec_free(sig, (size_t)C); rot_clear(&rt); free(ord);
+  mpfr_clear(tmpP); mpfr_clear(F); mpfr_clear(w); mpfr_clear(al); mpfr_clear(be); mpfr_clear(gr); mpfr_clear(gi);
+  mpfr_clear(thr2); mpfr_clear(zt);
+  if (info) { info[0] = sweeps; info[1] = rotations; info[2] = status; }
+  return status;
+}
+
+static void load_rmat(rmat *m, const uint8_t *api, int prec, mpfr_ptr tmpP) {
+  size_t rb = api_real_bytes(prec);
+  for (int i = 0; i < m->r; ++i)
+    for (int j = 0; j < m->c; ++j) {
+      const uint8_t *src = api + ((size_t)i * m->c + j) * 2 * rb;
+      api_get(RRE(*m, i, j), src, prec, tmpP);
+      api_get(RIM(*m, i, j), src + rb, prec, tmpP);
+    }
+}
+
+/* ||X_G - X0_G (X0_G^H X_G)||_F^2 over the columns [g0, g1) (the projector distance of comparator (iv)); X, X0: rows x K */
+static void proj_dist2(mpfr_ptr out, const rmat *X, const rmat *X0, int g0, int g1, long Pc) {
+  const int m = g1 - g0, rows = X->r;
+  mpfr_t sr, si, t1, t2;
+  mpfr_init2(sr, Pc); mpfr_init2(si, Pc); mpfr_init2(t1, Pc); mpfr_init2(t2, Pc);
+  rmat Mm = rmat_alloc(m, m, Pc);
+  for (int a = 0; a < m; ++a)
+    for (int b = 0; b < m; ++b) {
+      mpfr_set_zero(sr, +1); mpfr_set_zero(si, +1);
+      for (int k = 0; k < rows; ++k) { /* conj(X0[k][g0+a]) X[k][g0+b] */
+        mpfr_fmma(t1, RRE(*X0, k, g0 + a), RRE(*X, k, g0 + b), RIM(*X0, k, g0 + a), RIM(*X, k, g0 + b), RN); mpfr_add(sr, sr, t1, RN);
+        mpfr_fmms(t1, RRE(*X0, k, g0 + a), RIM(*X, k, g0 + b), RIM(*X0, k, g0 + a), RRE(*X, k, g0 + b), RN); mpfr_add(si, si, t1, RN);
+      }
+      mpfr_set(RRE(Mm, a, b), sr, RN); mpfr_set(RIM(Mm, a, b), si, RN);
+    }
+  mpfr_set_zero(out, +1);
+  for (int k = 0; k < rows; ++k)
+    for (int b = 0; b < m; ++b) {
+      mpfr_set(sr, RRE(*X, k, g0 + b), RN); mpfr_set(si, RIM(*X, k, g0 + b), RN);
+      for (int a = 0; a < m; ++a) {
+        mpfr_fmms(t1, RRE(*X0, k, g0 + a), RRE(Mm, a, b), RIM(*X0, k, g0 + a), RIM(Mm, a, b), RN); mpfr_sub(sr, sr, t1, RN);
+        mpfr_fmma(t1, RRE(*X0, k, g0 + a), RIM(Mm, a, b), RIM(*X0, k, g0 + a), RRE(Mm, a, b), RN); mpfr_sub(si, si, t1, RN);
+      }
+      mpfr_sqr(t1, sr, RN); mpfr_sqr(t2, si, RN); mpfr_add(out, out, t1, RN); mpfr_add(out, out, t2, RN);
+    }
+  rmat_free(&Mm);
+  mpfr_clear(sr); mpfr_clear(si); mpfr_clear(t1); mpfr_clear(t2);
+}
+
+/* Comparator for a candidate SVD (S, U, V) of A, optionally against a reference (S0, U0, V0).  K = min(M, N).
+ *  out[0] = log2 max_j |sigma_j - sigma0_j| / F
+ *  out[1] = log2 max_j max(||A v_j - sigma_j u_j||_2, ||A^H u_j - sigma_j v_j||_2) / F
+ *  out[2] = log2 max(max |U^H U - I|, max |V^H V - I|)
+ *  out[3] = max over groups of log2 err_G - log2 (2^-(prec-38) F / gap_G)      (<= 0 passes)
+ *  out[4] = log2 F;  out[5] = groups;  out[6] = largest group;  out[7] = worst log2 err_G
+ * Groups: reference sigma sorted descending, a new group where the gap exceeds 2^-(prec-102) F (the rule of
+ * zkd_oracle_compare).  For a group of nonzero sigma the pairs are compared as stacked vectors z_j = (u_j; v_j)/sqrt 2 -
+ * the eigenvectors of [[0, A], [A^H, 0]] for +sigma_j, so that the common phase of (u_j, v_j) is aligned by the projector -
+ * with gap_G = min(distance to the nearest sigma outside the group, 2 sigma_min(G)) (the mirrored eigenvalue -sigma).  For
+ * the group of sigma <= 2^-(prec-102) F, u and v decouple: the spans of V_G (when N <= M) and of U_G (when M <= N) are
+ * compared separately, gap_G = distance to the smallest sigma outside the group. */
+int zkd_oracle_svd_compare(int M, int N, int prec, const uint8_t *A_api, const uint8_t *S_api, const uint8_t *U_api,
+                           const uint8_t *V_api, const uint8_t *S0_api, const uint8_t *U0_api, const uint8_t *V0_api,
+                           double *out) {
+  const long Pc = (long)prec + 256;
+  const size_t rb = api_real_bytes(prec);
+  const int K = M < N ? M : N;
+  mpfr_t tmpP, F, w, sr, si, acc, worst, t1;
+  mpfr_init2(tmpP, prec); mpfr_init2(F, Pc); mpfr_init2(w, Pc); mpfr_init2(sr, Pc); mpfr_init2(si, Pc);
+  mpfr_init2(acc, Pc); mpfr_init2(worst, Pc); mpfr_init2(t1, Pc);
+  rmat A = rmat_alloc(M, N, Pc), U = rmat_alloc(M, K, Pc), V = rmat_alloc(N, K, Pc);
+  __mpfr_struct *S = vec_alloc((size_t)K, Pc);
+  load_rmat(&A, A_api, prec, tmpP); load_rmat(&U, U_api, prec, tmpP); load_rmat(&V, V_api, prec, tmpP);
+  for (int j = 0; j < K; ++j) api_get(&S[j], S_api + (size_t)j * rb, prec, tmpP);
+  for (int i = 0; i < 8; ++i) out[i] = -1.0e9;
+  mpfr_set_zero(F, +1);
+  for (int i = 0; i < M; ++i)
+    for (int j = 0; j < N; ++j) {
+      mpfr_sqr(w, RRE(A, i, j), RN); mpfr_add(F, F, w, RN);
+      mpfr_sqr(w, RIM(A, i, j), RN); mpfr_add(F, F, w, RN);
+    }
+  mpfr_sqrt(F, F, RN);
+  const double lF = log2_mpfr(F);
+  out[4] = lF;
+  /* (ii) residuals */
+  mpfr_set_zero(worst, +1);
+  for (int j = 0; j < K; ++j) {
+    mpfr_set_zero(acc, +1);
+    for (int i = 0; i < M; ++i) { /* (A v_j - sigma_j u_j)_i */
+      mpfr_set_zero(sr, +1); mpfr_set_zero(si, +1);
+      for (int k = 0; k < N; ++k) {
+        mpfr_fmms(t1, RRE(A, i, k), RRE(V, k, j), RIM(A, i, k), RIM(V, k, j), RN); mpfr_add(sr, sr, t1, RN);
+        mpfr_fmma(t1, RRE(A, i, k), RIM(V, k, j), RIM(A, i, k), RRE(V, k, j), RN); mpfr_add(si, si, t1, RN);
+      }
+      mpfr_mul(t1, &S[j], RRE(U, i, j), RN); mpfr_sub(sr, sr, t1, RN);
+      mpfr_mul(t1, &S[j], RIM(U, i, j), RN); mpfr_sub(si, si, t1, RN);
+      mpfr_sqr(t1, sr, RN); mpfr_add(acc, acc, t1, RN); mpfr_sqr(t1, si, RN); mpfr_add(acc, acc, t1, RN);
+    }
+    if (mpfr_cmp(acc, worst) > 0) mpfr_set(worst, acc, RN);
+    mpfr_set_zero(acc, +1);
+    for (int k = 0; k < N; ++k) { /* (A^H u_j - sigma_j v_j)_k */
+      mpfr_set_zero(sr, +1); mpfr_set_zero(si, +1);
+      for (int i = 0; i < M; ++i) { /* conj(a_ik) u_ij */
+        mpfr_fmma(t1, RRE(A, i, k), RRE(U, i, j), RIM(A, i, k), RIM(U, i, j), RN); mpfr_add(sr, sr, t1, RN);
+        mpfr_fmms(t1, RRE(A, i, k), RIM(U, i, j), RIM(A, i, k), RRE(U, i, j), RN); mpfr_add(si, si, t1, RN);
+      }
+      mpfr_mul(t1, &S[j], RRE(V, k, j), RN); mpfr_sub(sr, sr, t1, RN);
+      mpfr_mul(t1, &S[j], RIM(V, k, j), RN); mpfr_sub(si, si, t1, RN);
+      mpfr_sqr(t1, sr, RN); mpfr_add(acc, acc, t1, RN); mpfr_sqr(t1, si, RN); mpfr_add(acc, acc, t1, RN);
+    }
+    if (mpfr_cmp(acc, worst) > 0) mpfr_set(worst, acc, RN);
+  }
+  mpfr_sqrt(worst, worst, RN);
+  out[1] = log2_mpfr(worst) - lF;
+  /* (iii) orthonormality */
+  mpfr_set_zero(worst, +1);
+  for (int side = 0; side < 2; ++side) {
+    const rmat *X = side ? &V : &U;
+    for (int a = 0; a < K; ++a)
+      for (int b = a; b < K; ++b) {
+        mpfr_set_zero(sr, +1); mpfr_set_zero(si, +1);
+        for (int k = 0; k < X->r; ++k) {
+          mpfr_fmma(t1, RRE(*X, k, a), RRE(*X, k, b), RIM(*X, k, a), RIM(*X, k, b), RN); mpfr_add(sr, sr, t1, RN);
+          mpfr_fmms(t1, RRE(*X, k, a), RIM(*X, k, b), RIM(*X, k, a), RRE(*X, k, b), RN); mpfr_add(si, si, t1, RN);
+        }
+        if (a == b) mpfr_sub_ui(sr, sr, 1, RN);
+        mpfr_abs(sr, sr, RN); mpfr_abs(si, si, RN);
+        if (mpfr_cmp(sr, worst) > 0) mpfr_set(worst, sr, RN);
+        if (mpfr_cmp(si, worst) > 0) mpfr_set(worst, si, RN);
+      }
+  }
+  out[2] = log2_mpfr(worst);
+  if (S0_api) {
+    __mpfr_struct *S0 = vec_alloc((size_t)K, Pc);
+    for (int j = 0; j < K; ++j) api_get(&S0[j], S0_api + (size_t)j * rb, prec, tmpP);
+    mpfr_set_zero(worst, +1);
+    for (int j = 0; j < K; ++j) { mpfr_sub(w, &S[j], &S0[j], RN); mpfr_abs(w, w, RN); if (mpfr_cmp(w, worst) > 0) mpfr_set(worst, w, RN); }
+    out[0] = log2_mpfr(worst) - lF;
+    if (U0_api && V0_api) {
+      rmat U0 = rmat_alloc(M, K, Pc), V0 = rmat_alloc(N, K, Pc);
+      load_rmat(&U0, U0_api, prec, tmpP); load_rmat(&V0, V0_api, prec, tmpP);
+      /* stacked vectors (u; v), norm^2 = 2 */
+      rmat Z = rmat_alloc(M + N, K, Pc), Z0 = rmat_alloc(M + N, K, Pc);
+      for (int j = 0; j < K; ++j) {
+        for (int i = 0; i < M; ++i) { mpfr_set(RRE(Z, i, j), RRE(U, i, j), RN); mpfr_set(RIM(Z, i, j), RIM(U, i, j), RN);
+                                      mpfr_set(RRE(Z0, i, j), RRE(U0, i, j), RN); mpfr_set(RIM(Z0, i, j), RIM(U0, i, j), RN); }
+        for (int i = 0; i < N; ++i) { mpfr_set(RRE(Z, M + i, j), RRE(V, i, j), RN); mpfr_set(RIM(Z, M + i, j), RIM(V, i, j), RN);
+                                      mpfr_set(RRE(Z0, M + i, j), RRE(V0, i, j), RN); mpfr_set(RIM(Z0, M + i, j), RIM(V0, i, j), RN); }
+      }
+      /* scale the stacked vectors by 1/sqrt(2) so that proj_dist2's X0 X0^H is a projector */
+      mpfr_set_ui(w, 2, RN); mpfr_sqrt(w, w, RN);
+      for (size_t e = 0; e < (size_t)(M + N) * K; ++e) {
+        mpfr_div(&Z.re[e], &Z.re[e], w, RN); mpfr_div(&Z.im[e], &Z.im[e], w, RN);
+        mpfr_div(&Z0.re[e], &Z0.re[e], w, RN); mpfr_div(&Z0.im[e], &Z0.im[e], w, RN);
+      }
+      mpfr_t gthr, gap, g2, e2;
+      mpfr_init2(gthr, Pc); mpfr_init2(gap, Pc); mpfr_init2(g2, Pc); mpfr_init2(e2, Pc);
+      mpfr_div_2si(gthr, F, prec - 102, RN);
+      int ng = 0, maxg = 0;
+      double worst_margin = -1.0e9, worst_err = -1.0e9;
+      int g0 = 0;
+      while (g0 < K) {
+        int g1 = g0 + 1;
+        while (g1 < K) { mpfr_sub(w, &S0[g1 - 1], &S0[g1], RN); if (mpfr_cmp(w, gthr) > 0) break; ++g1; }
+        ++ng; if (g1 - g0 > maxg) maxg = g1 - g0;
+        const int zero_group = mpfr_cmp(&S0[g0], gthr) <= 0; /* its largest member is (numerically) zero */
+        int have = 0;
+        if (g0 > 0) { mpfr_sub(gap, &S0[g0 - 1], &S0[g0], RN); have = 1; }
+        if (g1 < K) { mpfr_sub(g2, &S0[g1 - 1], &S0[g1], RN); if (!have || mpfr_cmp(g2, gap) < 0) mpfr_set(gap, g2, RN); have = 1; }
+        double err;
+        if (!zero_group) {
+          mpfr_mul_2si(g2, &S0[g1 - 1], 1, RN); /* distance to the mirrored -sigma */
+          if (!have || mpfr_cmp(g2, gap) < 0) mpfr_set(gap, g2, RN);
+          have = 1;
+          proj_dist2(e2, &Z, &Z0, g0, g1, Pc);
+          mpfr_sqrt(e2, e2, RN);
+          err = log2_mpfr(e2);
+        } else {
+          err = -1.0e9;
+          if (N <= M) { proj_dist2(e2, &V, &V0, g0, g1, Pc); mpfr_sqrt(e2, e2, RN); if (log2_mpfr(e2) > err) err = log2_mpfr(e2); }
+          if (M <= N) { proj_dist2(e2, &U, &U0, g0, g1, Pc); mpfr_sqrt(e2, e2, RN); if (log2_mpfr(e2) > err) err = log2_mpfr(e2); }
+        }
+        const double ltol = have ? (-(double)(prec - 38) + lF - log2_mpfr(gap)) : 1.0e9;
+        if (err - ltol > worst_margin) worst_margin = err - ltol;
+        if (err > worst_err) worst_err = err;
+        g0 = g1;
+      }
+      out[3] = worst_margin; out[5] = ng; out[6] = maxg; out[7] = worst_err;
+      mpfr_clear(gthr); mpfr_clear(gap); mpfr_clear(g2); mpfr_clear(e2);
+      rmat_free(&U0); rmat_free(&V0); rmat_free(&Z); rmat_free(&Z0);
+    }
+    vec_free(S0, (size_t)K);
+  }
+  rmat_free(&A); rmat_free(&U); rmat_free(&V); vec_free(S, (size_t)K);
+  mpfr_clear(tmpP); mpfr_clear(F); mpfr_clear(w); mpfr_clear(sr); mpfr_clear(si); mpfr_clear(acc); mpfr_clear(worst); mpfr_clear(t1);
+  return 0;
+}
