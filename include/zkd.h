@@ -102,6 +102,22 @@ int zkd_diag_herm(int N, int batch, int prec_bits, const void *A, void *eigvals,
 int zkd_diag_herm_host(int N, int batch, int prec_bits, const void *A_host, void *eigvals_host, void *eigvecs_host,
                        zkd_info *info_host);
 
+/* ---- singular value decomposition ----------------------------------------------------
+ * The second routine of the paper's ZKCM_CUS: "Hermitian matrix diagonalization and singular value decomposition"
+ * (section 2; switched by ZKCM_QC, section 2.2).  Thin SVD of `batch` complex M x N
+ * matrices, K = min(M, N):  A V = U diag(S), A^H U = V diag(S), S descending and >= 0, U (M x K) and V (N x K) with
+ * orthonormal columns; phase: the first component of largest modulus of every v_j is real positive.  Computed through
+ * the same hot path on the Hermitian matrix [[0, A], [A^H, 0]], so singular values are good to ABSOLUTE
+ * 2^-(prec_bits - 28) ||A||_F: Schmidt weights far below sqrt(epsilon) are resolved.  Rank-deficient input is fine.
+ *   A[b][i][j] (M x N), U[b][i][j] (M x K), V[b][i][j] (N x K): row-major complex API numbers; S[b][j]: real.
+ *   All pointers DEVICE, 16-byte aligned, caller-owned; info (device, `batch` records, may be NULL) as for
+ *   zkd_diag_herm_ws (clusters and residual refer to the (M+N) x (M+N) eigenproblem).  M + N <= ZKD_MAX_N.
+ *   Errors as for zkd_diag_herm_ws.  zkd_svd obtains its workspace from the stream-ordered allocator. */
+int zkd_svd_bufsize(int M, int N, int batch, int prec_bits, size_t *workspace_bytes);
+int zkd_svd_ws(int M, int N, int batch, int prec_bits, const void *A, void *S, void *U, void *V, void *workspace,
+               size_t workspace_bytes, zkd_info *info, void *stream);
+int zkd_svd(int M, int N, int batch, int prec_bits, const void *A, void *S, void *U, void *V, void *stream);
+
 /* Tunables.  PROCESS-WIDE and unsynchronised: set them before, not during, calls of zkd_diag_herm* from
  * other threads; the library may be used from several host threads with distinct workspaces as long as the options, the
  * counters and the kernel timing are left alone meanwhile, and it serves ONE device per process (the device current at

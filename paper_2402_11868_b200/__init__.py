@@ -49,6 +49,9 @@ def lib() -> ctypes.CDLL:
     L.zkd_diag_herm_ws.argtypes = [ci, ci, ci, vp, vp, vp, vp, cs, vp, vp]
     L.zkd_diag_herm.argtypes = [ci, ci, ci, vp, vp, vp, vp]
     L.zkd_diag_herm_host.argtypes = [ci, ci, ci, vp, vp, vp, vp]
+    L.zkd_svd_bufsize.argtypes = [ci, ci, ci, ci, ctypes.POINTER(cs)]
+    L.zkd_svd_ws.argtypes = [ci, ci, ci, ci, vp, vp, vp, vp, vp, cs, vp, vp]
+    L.zkd_svd.argtypes = [ci, ci, ci, ci, vp, vp, vp, vp, vp]
     L.zkd_set_option.argtypes = [ctypes.c_char_p, cd]
     L.zkd_get_option.argtypes = [ctypes.c_char_p, ctypes.POINTER(cd)]
     L.zkd_strerror.restype = ctypes.c_char_p
@@ -218,6 +221,29 @@ def diag_herm_host(N: int, batch: int, A_host, eigvals_host, eigvecs_host, info_
     ip = ctypes.addressof(info_host) if info_host is not None else None
     _check(lib().zkd_diag_herm_host(N, batch, prec_bits, ptr(A_host), ptr(eigvals_host), ptr(eigvecs_host), ip),
            "zkd_diag_herm_host")
+
+
+def svd_bufsize(M: int, N: int, batch: int, prec_bits: int = PREC) -> int:
+    n = ctypes.c_size_t()
+    _check(lib().zkd_svd_bufsize(M, N, batch, prec_bits, ctypes.byref(n)), "zkd_svd_bufsize")
+    return int(n.value)
+
+
+def svd_ws(M: int, N: int, batch: int, A, S, U, V, workspace, info=None, prec_bits: int = PREC, stream=None) -> None:
+    """zkd_svd_ws on device tensors (uint8, API layout): thin SVD, K = min(M, N) (NEXT-1)."""
+    rb, K = 16 + prec_bits // 8, min(M, N)
+    i = _dev_u8(info, batch * ctypes.sizeof(zkd_info), "info") if info is not None else None
+    _check(lib().zkd_svd_ws(M, N, batch, prec_bits, _dev_u8(A, batch * M * N * 2 * rb, "A"), _dev_u8(S, batch * K * rb, "S"),
+                            _dev_u8(U, batch * M * K * 2 * rb, "U"), _dev_u8(V, batch * N * K * 2 * rb, "V"),
+                            _dev_u8(workspace, svd_bufsize(M, N, batch, prec_bits), "workspace"),
+                            workspace.numel() * workspace.element_size(), i, _stream_ptr(stream)), "zkd_svd_ws")
+
+
+def svd(M: int, N: int, batch: int, A, S, U, V, prec_bits: int = PREC, stream=None) -> None:
+    rb, K = 16 + prec_bits // 8, min(M, N)
+    _check(lib().zkd_svd(M, N, batch, prec_bits, _dev_u8(A, batch * M * N * 2 * rb, "A"), _dev_u8(S, batch * K * rb, "S"),
+                         _dev_u8(U, batch * M * K * 2 * rb, "U"), _dev_u8(V, batch * N * K * 2 * rb, "V"), _stream_ptr(stream)),
+           "zkd_svd")
 
 
 def read_info(info_tensor, batch: int) -> list[dict]:

@@ -398,6 +398,41 @@ int zkd_diag_herm(int N, int batch, int prec_bits, const void* A, void* eigvals,
   cudaFreeAsync(ws, s);
   return rc;
 }
+static int check_svd_args(int M, int N, int batch, int prec_bits) {
+  if (!prec_supported(prec_bits)) return ZKD_ERR_UNSUPPORTED_PREC;
+  if (M < 1 || N < 1 || M + N > ZKD_MAX_N || batch < 1 || batch > 65535) return ZKD_ERR_INVALID_ARG;
+  return ZKD_OK;
+}
+int zkd_svd_bufsize(int M, int N, int batch, int prec_bits, size_t* workspace_bytes) {
+  ZKD_TRY(check_svd_args(M, N, batch, prec_bits));
+  if (!workspace_bytes) return ZKD_ERR_INVALID_ARG;
+  *workspace_bytes = svd_workspace_bytes(M, N, batch);
+  return ZKD_OK;
+}
+int zkd_svd_ws(int M, int N, int batch, int prec_bits, const void* A, void* S, void* U, void* V, void* workspace, size_t workspace_bytes,
+               zkd_info* info, void* stream) {
+  ZKD_TRY(check_svd_args(M, N, batch, prec_bits));
+  if (!A || !S || !U || !V || !workspace) return ZKD_ERR_INVALID_ARG;
+  if (((uintptr_t)A | (uintptr_t)S | (uintptr_t)U | (uintptr_t)V | (uintptr_t)workspace) & 15) return ZKD_ERR_INVALID_ARG;
+  if (workspace_bytes < svd_workspace_bytes(M, N, batch)) return ZKD_ERR_WORKSPACE;
+  ZKD_TRY(check_device());
+  return svd_device(M, N, batch, prec_bits, A, S, U, V, workspace, workspace_bytes, info, (cudaStream_t)stream);
+}
+int zkd_svd(int M, int N, int batch, int prec_bits, const void* A, void* S, void* U, void* V, void* stream) {
+  ZKD_TRY(check_svd_args(M, N, batch, prec_bits));
+  if (!A || !S || !U || !V) return ZKD_ERR_INVALID_ARG;
+  ZKD_TRY(check_device());
+  const size_t bytes = svd_workspace_bytes(M, N, batch);
+  void* ws = nullptr;
+  cudaStream_t s = (cudaStream_t)stream;
+  if (cudaMallocAsync(&ws, bytes, s) != cudaSuccess) {
+    (void)cudaGetLastError();
+    return ZKD_ERR_WORKSPACE;
+  }
+  int rc = zkd_svd_ws(M, N, batch, prec_bits, A, S, U, V, ws, bytes, nullptr, stream);
+  cudaFreeAsync(ws, s);
+  return rc;
+}
 int zkd_diag_herm_host(int N, int batch, int prec_bits, const void* A_host, void* eigvals_host, void* eigvecs_host,
                        zkd_info* info_host) {
   ZKD_TRY(check_diag_args(N, batch, prec_bits));

@@ -50,4 +50,18 @@ int finalize_export(int N, int batch, const int32_t* X, const int32_t* lam, cons
                     int32_t* scratch /* FxC batch N N */, int32_t* lam_sorted /* FxR batch N */, int* rank /* batch N */,
                     cudaStream_t s, int prec = kPrec);
 
+// rank[b][j] = number of eigenvalues of matrix b that sort before lam[b][j] (ascending, stable); lam_sorted[b][rank] = lam[b][j]
+int rank_sort(int N, int batch, const int32_t* lam, int* rank, int32_t* lam_sorted, cudaStream_t s);
+
+// svd.cu (NEXT-1)
+int ingest_general(int M, int N, int batch, const void* A_api, int32_t* A_fx, int* scale /*[2 batch]*/, int* status /*[batch]*/, cudaStream_t s,
+                   int prec);
+int jw_build(int M, int N, int batch, const int32_t* A_fx, int32_t* H_fx, cudaStream_t s);
+int svd_plan(int n, int batch, const int* rank, const int32_t* lam_sorted, int zero_msb, int* col_of, int* r_out, cudaStream_t s);
+int svd_gather(int M, int N, int batch, const int32_t* X, const int* col_of, const int* r, const int32_t* lam_sorted, int32_t* U, int32_t* V,
+               int32_t* S, cudaStream_t s);
+int svd_zgather(int n, int batch, int d0, int r, int g, const int* mats_dev, const int32_t* X, const int* col_of, int32_t* Z, cudaStream_t s);
+int fxc_shr(size_t count, int32_t* X, int bits, cudaStream_t s);
+int svd_phase(int M, int N, int batch, int32_t* U, int32_t* V, cudaStream_t s);
+
 }  // namespace zkd

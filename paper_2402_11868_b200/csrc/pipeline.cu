@@ -721,4 +721,192 @@ int diag_herm_device(int N, int batch, int prec, const void* A_api, void* eigval
   return ZKD_OK;
 }
 
+// ---- NEXT-1: singular value decomposition through the same path (svd.cu) ---------------------------------
+size_t svd_workspace_bytes(int M, int N, int batch) {
+  const int n = M + N;
+  const size_t cnt = (size_t)n * n * batch;
+  return diag_workspace_bytes(n, batch) + 8 * (FxC::bytes(cnt) + 4096) + 64 * (size_t)n * batch + (8u << 20);
+}
+
+int svd_device(int M, int N, int batch, int prec, const void* A_api, void* S_api, void* U_api, void* V_api, void* ws, size_t ws_bytes,
+               zkd_info* info, cudaStream_t s) {
+  const Options& opt = options();
+  const int n = M + N, K = std::min(M, N);
+  Ctx c;
+  c.prec = prec;
+  c.tol_bits = std::min(opt.tol_bits, 790) - (kPrec - prec);
+  c.fb = std::max(0, kFRAC - (c.tol_bits + 42));
+  c.s = s;
+  c.ar.base = (char*)ws;
+  c.ar.size = ws_bytes;
+  c.ar.stream = s;
+  c.h_pin = pinned_staging();
+  if (!c.h_pin) return ZKD_ERR_CUDA;
+  c.gemm_ws_bytes = gemm_workspace_bytes(n, n, n, batch) + (32u << 20);
+  c.gemm_ws = c.ar.alloc(c.gemm_ws_bytes);
+  const size_t cnt = (size_t)n * n * batch;
+  int32_t* A = (int32_t*)c.ar.alloc(FxC::bytes((size_t)M * N * batch));
+  int32_t* H = (int32_t*)c.ar.alloc(FxC::bytes(cnt));
+  int32_t* X = (int32_t*)c.ar.alloc(FxC::bytes(cnt));
+  int32_t* lam = (int32_t*)c.ar.alloc(FxR::bytes((size_t)n * batch));
+  int32_t* lam_sorted = (int32_t*)c.ar.alloc(FxR::bytes((size_t)n * batch));
+  int32_t* Uf = (int32_t*)c.ar.alloc(FxC::bytes((size_t)M * K * batch));
+  int32_t* Vf = (int32_t*)c.ar.alloc(FxC::bytes((size_t)N * K * batch));
+  int32_t* Sf = (int32_t*)c.ar.alloc(FxR::bytes((size_t)K * batch));
+  int32_t* Gm = (int32_t*)c.ar.alloc(FxC::bytes((size_t)K * K * batch));
+  int* scale = c.ar.get<int>((size_t)2 * batch);
+  int* status = c.ar.get<int>((size_t)batch);
+  int* rank = c.ar.get<int>((size_t)n * batch);
+  int* col_of = c.ar.get<int>((size_t)n * batch);
+  int* r_dev = c.ar.get<int>((size_t)batch);
+  int* cl0 = c.ar.get<int>((size_t)K * batch);
+  int* cl_stats_dev = c.ar.get<int>((size_t)2 * batch);
+  int* pm = c.ar.get<int>((size_t)2 * batch);
+  int* scal = c.ar.get<int>(S_NUM);
+  if (!c.gemm_ws || !A || !H || !X || !lam || !lam_sorted || !Uf || !Vf || !Sf || !Gm || !scale || !status || !rank || !col_of || !r_dev ||
+      !cl0 || !cl_stats_dev || !pm || !scal)
+    return ZKD_ERR_WORKSPACE;
+
+  ZKD_TRY(ingest_general(M, N, batch, A_api, A, scale, status, s, prec));
+  ZKD_TRY(jw_build(M, N, batch, A, H, s));
+  LevelStats st;
+  {
+    const int rc = solve_level(c, n, batch, H, X, lam, 0, nullptr, &st, pm);
+    if (rc != ZKD_OK) {
+      c.ar.release(Arena::Mark{c.ar.off, 0});
+      return rc;
+    }
+  }
+  ZKD_TRY(rank_sort(n, batch, lam, rank, lam_sorted, s));
+  // eigenvalues of H up to 2^-(prec - 10) (scaled units) count as zero: their eigenvectors mix null(A^H) and null(A)
+  const int zero_msb = 812 - c.tol_bits + 12;
+  ZKD_TRY(svd_plan(n, batch, rank, lam_sorted, zero_msb, col_of, r_dev, s));
+  std::vector<int> h_r((size_t)batch);
+  ZKD_CUDA_TRY(cudaMemcpyAsync(h_r.data(), r_dev, sizeof(int) * batch, cudaMemcpyDeviceToHost, s));
+  ZKD_CUDA_TRY(cudaStreamSynchronize(s));
+  ZKD_TRY(svd_gather(M, N, batch, X, col_of, r_dev, lam_sorted, Uf, Vf, Sf, s));
+
+  // rank-deficient matrices (and M != N): the K - r missing pairs come from the zero cluster Z of H (dimension d0 = n - 2r).
+  // P = Z_u^H Z_u (Z_u = the upper M rows) is an orthogonal projector on span(Z): eigenvalue 1 on the vectors that live in
+  // null(A^H) (u-type, M - r of them), 0 on those in null(A) (v-type, N - r).  Diagonalising P / 8 with the same path separates
+  // the two, whatever basis of the zero cluster the eigensolver returned.
+  std::map<int, std::vector<int>> groups;
+  for (int b = 0; b < batch; ++b) {
+    if (h_r[b] > K) return ZKD_ERR_INTERNAL;  // more positive eigenvalues than min(M, N): cannot happen for a Jordan-Wielandt matrix
+    if (h_r[b] < K) groups[h_r[b]].push_back(b);
+  }
+  const Arena::Mark markg = c.ar.mark();
+  for (const auto& kv : groups) {
+    c.ar.release(markg);
+    const int r = kv.first, g = (int)kv.second.size(), d0 = n - 2 * r, nz = K - r;
+    const size_t zc = (size_t)n * d0 * g, pc = (size_t)d0 * d0 * g;
+    int* ints = c.ar.get<int>((size_t)8 * g);
+    int32_t* Z = (int32_t*)c.ar.alloc(FxC::bytes(zc));
+    int32_t* Pm = (int32_t*)c.ar.alloc(FxC::bytes(pc));
+    int32_t* Y = (int32_t*)c.ar.alloc(FxC::bytes(pc));
+    int32_t* lamY = (int32_t*)c.ar.alloc(FxR::bytes((size_t)d0 * g));
+    int* pm2 = c.ar.get<int>((size_t)2 * g);
+    if (!ints || !Z || !Pm || !Y || !lamY || !pm2) return ZKD_ERR_WORKSPACE;
+    std::vector<int> h((size_t)8 * g);
+    for (int v = 0; v < g; ++v) {
+      const int b = kv.second[v];
+      h[v] = b;                                           // mats
+      h[g + v] = v * n * d0;                              // Z_u of element v
+      h[2 * g + v] = v * n * d0 + M * d0;                 // Z_v
+      h[3 * g + v] = v * d0 * d0 + (N - r);               // Y columns of the u-type vectors (eigenvalue 1/8: after the N - r zeros)
+      h[4 * g + v] = v * d0 * d0;                         // Y columns of the v-type vectors
+      h[5 * g + v] = b * M * K + r;                       // destination columns r .. K-1 of U
+      h[6 * g + v] = b * N * K + r;                       // ... of V
+      h[7 * g + v] = v * d0 * d0;                         // P of element v
+    }
+    ZKD_CUDA_TRY(cudaMemcpyAsync(ints, h.data(), sizeof(int) * h.size(), cudaMemcpyHostToDevice, s));
+    ZKD_CUDA_TRY(cudaStreamSynchronize(s));  // h is a local
+    ZKD_TRY(svd_zgather(n, batch, d0, r, g, ints, X, col_of, Z, s));
+    ZKD_CUDA_TRY(cudaMemsetAsync(scal, 0, sizeof(int) * S_NUM, s));
+    const int nwZ = digits_for(815, c.fb);
+    auto zside = [&](const int* off, int rows, bool ct) {
+      GemmSide sd;
+      sd.fx = Z; sd.rows = rows; sd.cols = d0; sd.conj_transpose = ct; sd.top_bit = 815; sd.nw = nwZ; sd.ld = d0; sd.off = off; sd.plane_count = zc;
+      return sd;
+    };
+    {
+      GemmDstView dv;
+      dv.ld = d0; dv.off = ints + 7 * g; dv.plane_count = pc;
+      ZKD_TRY(gemm_complex(d0, d0, M, g, zside(ints + g, M, true), zside(ints + g, M, false), Pm, GemmMode::Assign, -1, opt.gemm_path, c.gemm_ws,
+                           c.gemm_ws_bytes, scal + S_ERR, nullptr, s, &dv));
+    }
+    ZKD_TRY(fxc_shr(pc, Pm, 3, s));
+    LevelStats st2;
+    ZKD_TRY(solve_level(c, d0, g, Pm, Y, lamY, 1, nullptr, &st2, pm2));
+    if (st2.status > st.status) st.status = st2.status;
+    if (nz > 0) {
+      auto yside = [&](const int* off) {
+        GemmSide sd;
+        sd.fx = Y; sd.rows = d0; sd.cols = nz; sd.conj_transpose = false; sd.top_bit = 815; sd.nw = nwZ; sd.ld = d0; sd.off = off; sd.plane_count = pc;
+        return sd;
+      };
+      GemmDstView du, dvv;
+      du.ld = K; du.off = ints + 5 * g; du.plane_count = (size_t)M * K * batch;
+      dvv.ld = K; dvv.off = ints + 6 * g; dvv.plane_count = (size_t)N * K * batch;
+      ZKD_TRY(gemm_complex(M, nz, d0, g, zside(ints + g, M, false), yside(ints + 3 * g), Uf, GemmMode::Assign, -1, opt.gemm_path, c.gemm_ws,
+                           c.gemm_ws_bytes, scal + S_ERR, nullptr, s, &du));
+      ZKD_TRY(gemm_complex(N, nz, d0, g, zside(ints + 2 * g, N, false), yside(ints + 4 * g), Vf, GemmMode::Assign, -1, opt.gemm_path, c.gemm_ws,
+                           c.gemm_ws_bytes, scal + S_ERR, nullptr, s, &dvv));
+    }
+    int hs[S_NUM];
+    ZKD_TRY(read_scalars(c, scal, S_NUM, hs));  // synchronises: the group's buffers are reused by the next group
+    if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
+  }
+  c.ar.release(markg);
+
+  // every pair: unit norm of u and of v separately, common phase from v (the oracle's convention)
+  ZKD_TRY(svd_phase(M, N, batch, Uf, Vf, s));
+  // One symmetric (Loewdin / Newton-Schulz) orthonormalisation of U and of V.  The parts of eigenvectors of H for a tiny sigma are
+  // orthogonal to the others only to residual / sigma (the mirrored eigenvalue -sigma is 2 sigma away); the step squares that
+  // and moves A v - sigma u by sigma times it, i.e. by less than the residual.
+  ZKD_CUDA_TRY(cudaMemsetAsync(cl0, 0, sizeof(int) * K * batch, s));
+  for (int side = 0; side < 2; ++side) {
+    int32_t* Xs = side ? Vf : Uf;
+    const int rows = side ? N : M;
+    const int nwX = digits_for(815, c.fb);
+    // each pass squares the deviation (2^-170 when a sigma of 2^-600 sits next to the zero cluster): iterate to the tolerance
+    for (int it = 0; it < 10; ++it) {
+      GemmSide P, Q;
+      P.fx = Xs; P.rows = rows; P.cols = K; P.conj_transpose = true; P.top_bit = 815; P.nw = nwX;
+      Q.fx = Xs; Q.rows = rows; Q.cols = K; Q.conj_transpose = false; Q.top_bit = 815; Q.nw = nwX;
+      ZKD_CUDA_TRY(cudaMemsetAsync(scal, 0, sizeof(int) * S_NUM, s));
+      ZKD_TRY(gemm_complex(K, K, rows, batch, P, Q, Gm, GemmMode::Assign, -1, opt.gemm_path, c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s));
+      ZKD_TRY(ns_build(K, batch, cl0, Gm, scal + S_MSB_G, s));
+      int hs[S_NUM];
+      ZKD_TRY(read_scalars(c, scal, S_NUM, hs));
+      if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
+      const int msb_m = hs[S_MSB_G];
+      if (msb_m <= c.fb + 8) break;                          // orthonormal to the working floor
+      if (msb_m >= 812 - 2) return ZKD_ERR_INTERNAL;         // not a near-orthonormal set: the iteration would not converge
+      GemmSide Pm2, Qm;
+      Pm2.fx = Xs; Pm2.rows = rows; Pm2.cols = K; Pm2.top_bit = 815; Pm2.nw = nwX;
+      Qm.fx = Gm; Qm.rows = K; Qm.cols = K; Qm.top_bit = msb_m + 1; Qm.nw = std::max(1, std::min(kND, ceil_div(msb_m + 1 - c.fb, kDB)));
+      ZKD_TRY(gemm_complex(rows, K, K, batch, Pm2, Qm, Xs, GemmMode::Add, -1, opt.gemm_path, c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s));
+      if (2 * (812 - msb_m) >= c.tol_bits + 30) break;       // the pass just applied squared the deviation below the tolerance
+    }
+  }
+  // the orthonormalisation moved every vector by about the residual: restore the exact phase convention (Im v_k* = 0)
+  ZKD_TRY(svd_phase(M, N, batch, Uf, Vf, s));
+  ZKD_TRY(fx_to_api_scaled((size_t)K * batch, Sf, S_api, 0, scale, 1, (size_t)K, s, prec));
+  ZKD_TRY(fxc_to_api((size_t)M * K * batch, Uf, U_api, s, prec));
+  ZKD_TRY(fxc_to_api((size_t)N * K * batch, Vf, V_api, s, prec));
+  if (info) {
+    const int* cs = nullptr;
+    if (!st.cl_stats.empty()) {
+      ZKD_CUDA_TRY(cudaMemcpyAsync(cl_stats_dev, st.cl_stats.data(), sizeof(int) * 2 * batch, cudaMemcpyHostToDevice, s));
+      cs = cl_stats_dev;
+    }
+    info_kernel<<<(batch + 127) / 128, 128, 0, s>>>(batch, status, st.status, st.steps, 812 - c.tol_bits, pm, cs, info);
+    count_launch();
+    ZKD_TRY(launch_check());
+  }
+  ZKD_CUDA_TRY(cudaStreamSynchronize(s));
+  return ZKD_OK;
+}
+
 }  // namespace zkd

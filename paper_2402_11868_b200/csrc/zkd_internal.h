@@ -116,6 +116,10 @@ size_t diag_workspace_bytes(int N, int batch);
 int diag_herm_device(int N, int batch, int prec, const void* A_api, void* eigvals_api, void* eigvecs_api, void* ws, size_t ws_bytes,
                      zkd_info* info, cudaStream_t s);
 
+size_t svd_workspace_bytes(int M, int N, int batch);
+int svd_device(int M, int N, int batch, int prec, const void* A_api, void* S_api, void* U_api, void* V_api, void* ws, size_t ws_bytes,
+               zkd_info* info, cudaStream_t s);
+
 }  // namespace zkd
 
 namespace zkd {
