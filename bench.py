@@ -48,6 +48,8 @@ def parse_args():
     ap.add_argument("--workload", default="c5", choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="zkd", choices=["zkd", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
+                    help="zkd_set_option before the run (route experiments; the defaults are the measured-fastest ones)")
     ap.add_argument("--no-extra", action="store_true", help="skip the context rows (other configs, saturating batch)")
     return ap.parse_args()
 
@@ -370,6 +372,9 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     z.lib()
+    for kv in args.opt:
+        k, v = kv.split("=")
+        z.set_option(k, float(v))
 
     def barrier():
         if world > 1:
@@ -415,7 +420,8 @@ def main():
         "data": "synthetic",
         "config": {"workload": WORKLOADS[args.workload], "N": N, "batch": b, "prec_bits": 768, "parallelism": "replicas only",
                    "l2": "flushed before every step (192 MiB write), device-timed and e2e legs alike",
-                   "kernel_events": "armed in both legs (one CUDA event pair per kernel launch inside the library)"},
+                   "kernel_events": "armed in both legs (one CUDA event pair per kernel launch inside the library)",
+                   **({"options": args.opt} if args.opt else {})},
         "eigenpairs_per_s": value * N,
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": run.h2d_bytes, "d2h_bytes_per_step": run.d2h_bytes,

@@ -128,7 +128,11 @@ int zkd_svd(int M, int N, int batch, int prec_bits, const void *A, void *S, void
  * "min_split_ctas" (split-K target, default 296; every split keeps at least 32 of K), "early_split" (S4h: split clusters whose internal structure stands
  * above the noise of the projected matrix; default 1; 0 leaves every cluster to the S5 recursion),
  * "split_margin_bits" (that margin, default 40), "seed_sweeps" (cap on the fp64 Jacobi sweeps, default 12),
- * "seed_path" / "seed_cluster" (seed kernel selection), "combine_path" (epilogue of the IMAD GEMM: 0 automatic,
+ * "seed_path" / "seed_cluster" (seed kernel selection), "cluster_tiles" (default 1: on levels where
+ * no cluster straddles a multiple of 128 columns, most columns are clustered and the clusters average more than 51 columns,
+ * the cluster-block products of a pass run as 128-column tile products on the int8 tcgen05 engine; 0: always per cluster on
+ * the IMAD engine; 2: tiles wherever they can be formed),
+ * "combine_path" (epilogue of the IMAD GEMM: 0 automatic,
  * 1 digit-serial, 2 warp-cooperative), "sstep_cpb" (matrix columns per CTA of the fused singleton step, 0 automatic), "sstep_warp" (1: its
  * warp-per-element variant for N <= 64, default 0), "sstep_cache" (shared-memory staging of the column, default 1),
  * "verbose" (1: one line per refinement pass on stderr).  All routes give the same results to the stated tolerances;

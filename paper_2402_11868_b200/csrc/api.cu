@@ -209,6 +209,7 @@ static int* option_slot(const char* key) {
   if (!strcmp(key, "seed_sweeps")) return &o.seed_sweeps;
   if (!strcmp(key, "seed_path")) return &o.seed_path;
   if (!strcmp(key, "seed_dbuf")) return &o.seed_dbuf;
+  if (!strcmp(key, "seed_block_warps")) return &o.seed_block_warps;
   if (!strcmp(key, "seed_cluster")) return &o.seed_cluster;
   if (!strcmp(key, "early_split")) return &o.early_split;
   if (!strcmp(key, "split_margin_bits")) return &o.split_margin_bits;
@@ -216,6 +217,7 @@ static int* option_slot(const char* key) {
   if (!strcmp(key, "sstep_cache")) return &o.sstep_cache;
   if (!strcmp(key, "sstep_warp")) return &o.sstep_warp;
   if (!strcmp(key, "combine_path")) return &o.combine_path;
+  if (!strcmp(key, "cluster_tiles")) return &o.cluster_tiles;
   if (!strcmp(key, "verbose")) return &o.verbose;
   return nullptr;
 }

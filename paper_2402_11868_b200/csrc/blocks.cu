@@ -111,17 +111,21 @@ int init_x(size_t count, const double2* V, int32_t* X, cudaStream_t s) {
 
 // ---- M := (I - G)/2 on cluster blocks (Newton-Schulz orthonormalisation step), msb of (G - I) ---------------------------
 __global__ void __launch_bounds__(256) ns_build_kernel(int n, int nb, const int* __restrict__ cl, const int* __restrict__ cle_skip1,
-                                                       int32_t* __restrict__ G, int* __restrict__ msb_out, int* __restrict__ msb_b) {
+                                                       int32_t* __restrict__ G, int* __restrict__ msb_out, int* __restrict__ msb_b,
+                                                       int zero_rest) {
   const size_t per = (size_t)n * n, count = per * nb;
   const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= count * 2) return;
   const int part = (int)(t / count);
   const size_t e = t % count;
   const int b = (int)(e / per), i = (int)((e % per) / n), j = (int)(e % n);
-  if (cl[(size_t)b * n + i] != cl[(size_t)b * n + j]) return;
-  if (cle_skip1 && cle_skip1[(size_t)b * n + j] - cl[(size_t)b * n + j] == 1) return;  // singletons are handled elsewhere
   int32_t* p = G + (part ? (size_t)ND * count : 0);
   int32_t g[ND], r[ND];
+  if (cl[(size_t)b * n + i] != cl[(size_t)b * n + j] ||
+      (cle_skip1 && cle_skip1[(size_t)b * n + j] - cl[(size_t)b * n + j] == 1)) {  // singletons are handled elsewhere
+    if (zero_rest) { fx_zero(g); fx_store(p, count, e, g); }
+    return;
+  }
   fx_load(g, p, count, e);
   if (part == 0 && i == j) g[ND - 1] -= 1;  // G - I
   const int msb = fx_msb(g);
@@ -131,27 +135,50 @@ __global__ void __launch_bounds__(256) ns_build_kernel(int n, int nb, const int*
   fx_half(g, r);                            // (I - G)/2
   fx_store(p, count, e, g);
 }
-int ns_build(int n, int nb, const int* cl, int32_t* G, int* msb_out, cudaStream_t s, const int* cle_skip1, int* msb_b) {
+int ns_build(int n, int nb, const int* cl, int32_t* G, int* msb_out, cudaStream_t s, const int* cle_skip1, int* msb_b, bool zero_rest) {
   KtScope kt_scope(KC_OTHER, s);
   const size_t t = (size_t)n * n * nb * 2;
-  ns_build_kernel<<<(unsigned)((t + 255) / 256), 256, 0, s>>>(n, nb, cl, cle_skip1, G, msb_out, msb_b);
+  ns_build_kernel<<<(unsigned)((t + 255) / 256), 256, 0, s>>>(n, nb, cl, cle_skip1, G, msb_out, msb_b, zero_rest ? 1 : 0);
   count_launch();
   return launch_check();
 }
 
 // ---- theta_j = Re S_jj ---------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) theta_kernel(int n, int nb, const int32_t* __restrict__ S, int32_t* __restrict__ theta) {
+__global__ void __launch_bounds__(256) mask_offcluster_kernel(int n, int nb, const int* __restrict__ cl, const int* __restrict__ cle,
+                                                              int32_t* __restrict__ S) {
+  const size_t per = (size_t)n * n, count = per * nb;
+  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= count * 2) return;
+  const size_t e = t % count;
+  const int b = (int)(e / per), i = (int)((e % per) / n), j = (int)(e % n);
+  const bool keep = cl[(size_t)b * n + i] == cl[(size_t)b * n + j] && cle[(size_t)b * n + j] - cl[(size_t)b * n + j] > 1;
+  if (keep) return;
+  int32_t z[ND];
+  fx_zero(z);
+  fx_store(S + (t / count) * (size_t)ND * count, count, e, z);
+}
+int mask_offcluster(int n, int nb, const int* cl, const int* cle, int32_t* S, cudaStream_t s) {
+  KtScope kt_scope(KC_OTHER, s);
+  const size_t t = (size_t)n * n * nb * 2;
+  mask_offcluster_kernel<<<(unsigned)((t + 255) / 256), 256, 0, s>>>(n, nb, cl, cle, S);
+  count_launch();
+  return launch_check();
+}
+
+__global__ void __launch_bounds__(128) theta_kernel(int n, int nb, const int32_t* __restrict__ S, int32_t* __restrict__ theta,
+                                                    const int* __restrict__ cl, const int* __restrict__ cle) {
   const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= (size_t)n * nb) return;
+  if (cl && cle[t] - cl[t] == 1) return;
   const int b = (int)(t / n), j = (int)(t % n);
   const size_t count = (size_t)n * n * nb;
   int32_t d[ND];
   fx_load(d, S, count, (size_t)b * n * n + (size_t)j * n + j);
   fx_store(theta, (size_t)n * nb, t, d);
 }
-int theta_from_diag(int n, int nb, const int32_t* S, int32_t* theta, cudaStream_t s) {
+int theta_from_diag(int n, int nb, const int32_t* S, int32_t* theta, cudaStream_t s, const int* cl, const int* cle) {
   KtScope kt_scope(KC_OTHER, s);
-  theta_kernel<<<(unsigned)(((size_t)n * nb + 127) / 128), 128, 0, s>>>(n, nb, S, theta);
+  theta_kernel<<<(unsigned)(((size_t)n * nb + 127) / 128), 128, 0, s>>>(n, nb, S, theta, cl, cle);
   count_launch();
   return launch_check();
 }

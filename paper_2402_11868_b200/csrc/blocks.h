@@ -10,7 +10,11 @@ int cluster_detect(int n, int nb, const double2* A64, const double* mu, int tau_
 int init_x(size_t count, const double2* V, int32_t* X, cudaStream_t s);
 // cle_skip1 != null: blocks of singleton clusters are left untouched
 // msb_b != null: the same maximum per matrix (atomicMax into msb_b[b])
-int ns_build(int n, int nb, const int* cl, int32_t* G, int* msb_out, cudaStream_t s, const int* cle_skip1 = nullptr, int* msb_b = nullptr);
+// zero_rest: entries outside the cluster blocks (and the skipped singleton diagonals) are set to zero instead of left alone
+int ns_build(int n, int nb, const int* cl, int32_t* G, int* msb_out, cudaStream_t s, const int* cle_skip1 = nullptr, int* msb_b = nullptr,
+             bool zero_rest = false);
+// S_ij := 0 unless i and j belong to the same cluster of more than one member
+int mask_offcluster(int n, int nb, const int* cl, const int* cle, int32_t* S, cudaStream_t s);
 // fused S4f + S4c when every cluster of the level is a singleton: X, W updated in place, R, diag(S), theta written
 // cl / cle != null: only the columns whose cluster is a singleton are processed
 int singleton_step(int n, int nb, int32_t* X, int32_t* W, int32_t* R, int32_t* S, int32_t* theta, int* msb_g_out, int* msb_r_out,
@@ -19,7 +23,8 @@ int singleton_step(int n, int nb, int32_t* X, int32_t* W, int32_t* R, int32_t* S
 int resid_per_matrix(int n, int nb, const int32_t* R, int* msb_r_b, cudaStream_t s);
 // gap_inv_out (device int, zeroed by the caller) <- max over neighbouring columns of different clusters of 1024 - msb(gap)
 int min_gap(int n, int nb, const int32_t* theta, const int* cl, int* gap_inv_out, cudaStream_t s);
-int theta_from_diag(int n, int nb, const int32_t* S, int32_t* theta, cudaStream_t s);
+// cl / cle != null: singleton columns are skipped (their theta comes from the fused singleton kernel)
+int theta_from_diag(int n, int nb, const int32_t* S, int32_t* theta, cudaStream_t s, const int* cl = nullptr, const int* cle = nullptr);
 int fxc_add_inplace(size_t count, int32_t* X, const int32_t* T, cudaStream_t s);
 int ecalc(int n, int nb, const int32_t* theta, const int* cl, int32_t* C, int prec_bits, int* msb_out, int* err_flag, cudaStream_t s);
 

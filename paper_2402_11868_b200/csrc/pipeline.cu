@@ -19,6 +19,7 @@
 #include <vector>
 
 #include "blocks.h"
+#include "gemm_i8.h"
 #include "timing.h"
 
 namespace zkd {
@@ -125,6 +126,12 @@ struct ClusterPlan {
   std::vector<ClusterGroup> groups;
   bool has_singletons = false;
   int max_m = 1, max_nsub = 0;
+  // Tiled form of the same pass for the int8 tcgen05 engine (S4b): when no cluster straddles a multiple of 128 columns, the
+  // cluster-block products of a pass are taken over whole 128-column tiles (X_t^H X_t, X_t^H W_t: 128 x 128 x n; X_t M_t, X_t S_t:
+  // n x 128 x 128 with M_t, S_t masked to their cluster blocks).  A tile computes 128 / m times the entries a cluster needs, on
+  // an engine that is far more than that factor faster than the IMAD path on m x m x n products.
+  bool tiled = false;
+  std::vector<ClusterGroup> tile;  // one entry: m = 128, nsub = tiles that hold a cluster
 };
 
 int build_plan(Ctx& c, int n, int nb, const std::vector<int>& h_cl, int* plan_dev /* 2 n nb ints */, ClusterPlan* plan) {
@@ -148,6 +155,46 @@ int build_plan(Ctx& c, int n, int nb, const std::vector<int>& h_cl, int* plan_de
     clustered += (size_t)g.m * g.nsub;
   }
   plan->has_singletons = clustered < (size_t)n * nb;
+  plan->tiled = false;
+  plan->tile.clear();
+  constexpr int TW = 128;
+  // worth it only when the clusters fill most of a tile: a tile computes 128 / m times the entries a cluster of m needs, and the
+  // int8 engine is about 2 x 128 / m ... faster than the IMAD engine per entry (measured on c5, m = 16: tiles 97 ms against 81 ms
+  // per cluster); cluster_tiles = 2 forces tiles wherever they can be formed (tests)
+  size_t sum_m2 = 0;
+  for (const auto& kv : groups) sum_m2 += (size_t)kv.first * kv.first * kv.second.size();
+  const bool tiles_pay = options().cluster_tiles == 2 || (options().cluster_tiles == 1 && 5 * sum_m2 >= 2 * (size_t)TW * clustered);
+  if (options().gemm_path != 1 && tiles_pay && n >= TW && n % TW == 0 && 2 * clustered >= (size_t)n * nb &&
+      gemm_i8_eligible(options().gemm_path, TW, TW, n, 1)) {
+    bool ok = true;
+    std::vector<char> used((size_t)(n / TW) * nb, 0);
+    for (const auto& kv : groups)
+      for (const SubProblem& sp : kv.second) {
+        if (sp.col0 / TW != (sp.col0 + kv.first - 1) / TW) ok = false;
+        used[(size_t)sp.b * (n / TW) + sp.col0 / TW] = 1;
+      }
+    if (ok) {
+      ClusterGroup g;
+      g.m = TW;
+      g.nsub = 0;
+      std::vector<int> ox, ob;
+      for (int b = 0; b < nb; ++b)
+        for (int t = 0; t < n / TW; ++t)
+          if (used[(size_t)b * (n / TW) + t]) {
+            ox.push_back(b * n * n + t * TW);
+            ob.push_back(b * n * n + t * TW * n + t * TW);
+            ++g.nsub;
+          }
+      if (g.nsub > 0 && h.size() + 2 * (size_t)g.nsub <= (size_t)2 * n * nb) {
+        g.offX = plan_dev + h.size();
+        h.insert(h.end(), ox.begin(), ox.end());
+        g.offB = plan_dev + h.size();
+        h.insert(h.end(), ob.begin(), ob.end());
+        plan->tile.push_back(g);
+        plan->tiled = true;
+      }
+    }
+  }
   if (!h.empty()) {
     ZKD_CUDA_TRY(cudaMemcpyAsync(plan_dev, h.data(), sizeof(int) * h.size(), cudaMemcpyHostToDevice, c.s));
     ZKD_CUDA_TRY(cudaStreamSynchronize(c.s));  // h is a local
@@ -179,12 +226,14 @@ int cluster_pass(Ctx& c, int n, int nb, const ClusterPlan& plan, const int* cl, 
                         &dv);
   };
   const int nwX = digits_for(topX, cut), nwW = digits_for(topW, cut);
+  // the products of this pass run per cluster (IMAD engine) or per 128-column tile (int8 tcgen05 engine), see ClusterPlan
+  const std::vector<ClusterGroup>& groups = plan.tiled ? plan.tile : plan.groups;
   // S4f: G_c = X_c^H X_c, bits below cutG cleared so that M = (I - G)/2 is a short number
   const int cutG = std::max(1, cut);
-  for (const ClusterGroup& g : plan.groups)
+  for (const ClusterGroup& g : groups)
     ZKD_TRY(gemm(g.m, g.m, n, g.nsub, view(X, n, g.m, true, topX, nwX, g.offX), view(X, n, g.m, false, topX, nwX, g.offX), Gm,
                  GemmMode::Assign, g.offB, nullptr, cutG));
-  ZKD_TRY(ns_build(n, nb, cl, Gm, scal + S_MSB_G, s, cle, pm_orth));
+  ZKD_TRY(ns_build(n, nb, cl, Gm, scal + S_MSB_G, s, cle, pm_orth, plan.tiled));
   int hs[S_NUM];
   ZKD_TRY(read_scalars(c, scal, S_NUM, hs));
   if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
@@ -195,7 +244,7 @@ int cluster_pass(Ctx& c, int n, int nb, const ClusterPlan& plan, const int* cl, 
     // made here would stay in W for good.  Exact = all digits of X / W times all nonzero digits of M (those above cutG - 1).
     const int topM = msb_m + 1, nwM = std::max(1, std::min(kND, ceil_div(topM - (cutG - 1), kDB)));
     const int nwXm = digits_for(topX, c.fb), nwWm = digits_for(topW, c.fb);
-    for (const ClusterGroup& g : plan.groups) {
+    for (const ClusterGroup& g : groups) {
       ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(X, n, g.m, false, topX, nwXm, g.offX), view(Gm, g.m, g.m, false, topM, nwM, g.offB), X,
                    GemmMode::Add, g.offX, nullptr));
       ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(W, n, g.m, false, topW, nwWm, g.offX), view(Gm, g.m, g.m, false, topM, nwM, g.offB), W,
@@ -208,11 +257,12 @@ int cluster_pass(Ctx& c, int n, int nb, const ClusterPlan& plan, const int* cl, 
     ZKD_CUDA_TRY(cudaMemcpyAsync(R, W, fxc, cudaMemcpyDeviceToDevice, s));
   }
   if (plan.has_singletons) ZKD_TRY(singleton_step(n, nb, X, W, R, Sm, theta, scal + S_MSB_G, scal + S_MSB_R, s, cl, cle, pm_orth));
-  for (const ClusterGroup& g : plan.groups)
+  for (const ClusterGroup& g : groups)
     ZKD_TRY(gemm(g.m, g.m, n, g.nsub, view(X, n, g.m, true, topX, nwX, g.offX), view(W, n, g.m, false, topW, nwW, g.offX), Sm,
                  GemmMode::Assign, g.offB, nullptr));
-  ZKD_TRY(theta_from_diag(n, nb, Sm, theta, s));
-  for (const ClusterGroup& g : plan.groups)
+  if (plan.tiled) ZKD_TRY(mask_offcluster(n, nb, cl, cle, Sm, s));  // keep the cluster blocks of the tiles only (singletons: theta, R are the fused kernel's)
+  ZKD_TRY(theta_from_diag(n, nb, Sm, theta, s, plan.tiled ? cl : nullptr, plan.tiled ? cle : nullptr));
+  for (const ClusterGroup& g : groups)
     ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(X, n, g.m, false, topX, nwX, g.offX), view(Sm, g.m, g.m, false, topW, nwW, g.offB), R,
                  GemmMode::Sub, g.offX, scal + S_MSB_R));
   return ZKD_OK;

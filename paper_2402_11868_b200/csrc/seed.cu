@@ -590,12 +590,12 @@ __device__ __forceinline__ double rotate_pair_smem(double2* __restrict__ gp, dou
   return cos2;
 }
 
-template <int W>
-__global__ void __launch_bounds__(256) seed_block_kernel(int n, const double2* __restrict__ A, double2* __restrict__ G,
+template <int W, int NWARPS>
+__global__ void __launch_bounds__(32 * NWARPS) seed_block_kernel(int n, const double2* __restrict__ A, double2* __restrict__ G,
                                                          const double* __restrict__ sigma_p, int* __restrict__ rot_flags,
                                                          double* __restrict__ mu_unsorted, int max_sweeps, double tol2) {
   extern __shared__ double2 s_cols[];  // [2 W][n]
-  constexpr int WPP = 8 / W;           // warps per pair: all 8 warps of the CTA rotate in every sub-round
+  constexpr int WPP = NWARPS / W;      // warps per pair: all warps of the CTA rotate in every sub-round
   __shared__ double s_red[W][4 * WPP];
   cg::grid_group grid = cg::this_grid();
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -621,15 +621,15 @@ __global__ void __launch_bounds__(256) seed_block_kernel(int n, const double2* _
         for (int pi = blockIdx.x; pi < npairs; pi += gridDim.x) {
           int bp, bq;
           rr_pair(MB, r, pi, bp, bq);
-          // load (absent columns, beyond n or in the padding block, are zero: rot_params leaves zero columns alone)
-          for (int c = 0; c < 2 * W; ++c) {
-            const int col = (c < W ? bp : bq) * W + (c % W);
-            double2* dst = s_cols + (size_t)c * n;
-            if (col < n) {
-              const double2* src = G + (size_t)col * n;
-              for (int i = tid; i < n; i += blockDim.x) dst[i] = __ldcg(src + i);
-            } else {
-              for (int i = tid; i < n; i += blockDim.x) dst[i] = make_double2(0.0, 0.0);
+          // load (absent columns, beyond n or in the padding block, are zero: rot_params leaves zero columns alone);
+          // one flat loop over the 2 W columns, unrolled, so that many independent L2 loads are in flight per thread
+          {
+            const int tot = 2 * W * n;
+#pragma unroll 8
+            for (int e = tid; e < tot; e += 32 * NWARPS) {
+              const int c = e / n, i = e - c * n;
+              const int col = (c < W ? bp : bq) * W + (c % W);
+              s_cols[e] = col < n ? __ldcg(G + (size_t)col * n + i) : make_double2(0.0, 0.0);
             }
           }
           __syncthreads();
@@ -649,12 +649,13 @@ __global__ void __launch_bounds__(256) seed_block_kernel(int n, const double2* _
             cmax = fmax(cmax, rotate_pair_smem<WPP>(s_cols + (size_t)p * n, s_cols + (size_t)q * n, n, lane, part, s_red[pr], tol2, nchk, nrot));
             __syncthreads();
           }
-          for (int c = 0; c < 2 * W; ++c) {
-            const int col = (c < W ? bp : bq) * W + (c % W);
-            if (col < n) {
-              const double2* src = s_cols + (size_t)c * n;
-              double2* dst = G + (size_t)col * n;
-              for (int i = tid; i < n; i += blockDim.x) __stcg(dst + i, src[i]);
+          {
+            const int tot = 2 * W * n;
+#pragma unroll 8
+            for (int e = tid; e < tot; e += 32 * NWARPS) {
+              const int c = e / n, i = e - c * n;
+              const int col = (c < W ? bp : bq) * W + (c % W);
+              if (col < n) __stcg(G + (size_t)col * n + i, s_cols[e]);
             }
           }
           __syncthreads();
@@ -674,16 +675,16 @@ __global__ void __launch_bounds__(256) seed_block_kernel(int n, const double2* _
   }
 }
 
-template <int W>
+template <int W, int NWARPS>
 static int launch_block(int n, int sms, const double2* Ab, double2* G, double* sigma, int* flags, double* mu_uns, int ms, double t2,
                         cudaStream_t s) {
   const size_t smem = sizeof(double2) * 2 * W * (size_t)n;
-  if (cudaFuncSetAttribute(seed_block_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess) {
+  if (cudaFuncSetAttribute(seed_block_kernel<W, NWARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess) {
     (void)cudaGetLastError();
     return ZKD_ERR_CUDA;
   }
   int maxb = 0;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&maxb, seed_block_kernel<W>, 256, smem) != cudaSuccess || maxb < 1) {
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&maxb, seed_block_kernel<W, NWARPS>, 32 * NWARPS, smem) != cudaSuccess || maxb < 1) {
     (void)cudaGetLastError();
     return ZKD_ERR_CUDA;
   }
@@ -691,7 +692,7 @@ static int launch_block(int n, int sms, const double2* Ab, double2* G, double* s
   int nblocks = MB / 2;
   if (nblocks > maxb * sms) nblocks = maxb * sms;
   void* args[] = {&n, (void*)&Ab, &G, &sigma, &flags, &mu_uns, &ms, &t2};
-  if (cudaLaunchCooperativeKernel((void*)seed_block_kernel<W>, dim3(nblocks), dim3(256), args, smem, s) != cudaSuccess) {
+  if (cudaLaunchCooperativeKernel((void*)seed_block_kernel<W, NWARPS>, dim3(nblocks), dim3(32 * NWARPS), args, smem, s) != cudaSuccess) {
     (void)cudaGetLastError();
     return ZKD_ERR_CUDA;
   }
@@ -730,7 +731,7 @@ int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int ma
   int dev = 0, sms = 0;
   ZKD_CUDA_TRY(cudaGetDevice(&dev));
   ZKD_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-  if (N <= 256) {
+  if (N <= 256 && !(options().seed_path == 4 && N > 96 && batch == 1)) {
     // ring: as many CTAs as give every processor (pair of columns) its own warp, with at most 16 (n > 128) or 32 warps per CTA;
     // fewer CTAs when the batch alone fills the machine.  A cluster of 16 is "non-portable": fall back to 8 when refused.
     const int P = (N + 1) / 2;
@@ -800,9 +801,13 @@ int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int ma
     // blocked kernel with the widest column blocks whose pair fits shared memory; plain kernel beyond that
     const size_t col_bytes = sizeof(double2) * (size_t)n;
     const size_t smem_budget = 200 * 1024;
-    if (options().seed_path != 3 && 16 * col_bytes <= smem_budget) rc = launch_block<8>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, s);
-    else if (options().seed_path != 3 && 8 * col_bytes <= smem_budget) rc = launch_block<4>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, s);
-    else if (options().seed_path != 3 && 4 * col_bytes <= smem_budget) rc = launch_block<2>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, s);
+    const bool w16 = options().seed_block_warps == 16;  // 16 warps per CTA: twice the loads in flight, half the rows per warp
+    if (options().seed_path != 3 && 16 * col_bytes <= smem_budget)
+      rc = w16 ? launch_block<8, 16>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, s) : launch_block<8, 8>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, s);
+    else if (options().seed_path != 3 && 8 * col_bytes <= smem_budget)
+      rc = w16 ? launch_block<4, 16>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, s) : launch_block<4, 8>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, s);
+    else if (options().seed_path != 3 && 4 * col_bytes <= smem_budget)
+      rc = w16 ? launch_block<2, 16>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, s) : launch_block<2, 8>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, s);
     else {
       void* args[] = {&n, (void*)&Ab, &G, &sigma, &flags, &mu_uns, &ms, &t2};
       if (cudaLaunchCooperativeKernel((void*)seed_large_kernel, dim3(nblocks), dim3(128), args, 0, s) != cudaSuccess) {

@@ -45,10 +45,12 @@ struct Options {
   int min_split_ctas = 296;  // split K until a product has about this many CTAs (two per SM), see pick_splits
   int seed_sweeps = 12;
   int seed_cluster = 0;  // ring seed: largest cluster size to use (0 = 16, falling back to 8 when refused)
+  int seed_block_warps = 8;   // blocked seed (N > 256): warps per CTA (8 or 16)
   int seed_dbuf = 1;     // ring seed: two slot sets, one cluster barrier per round (when they fit shared memory)
   int seed_path = 0;     // 0: auto; 2: always the ring kernel for N <= 256; 3: unblocked cooperative kernel for N > 256
   int early_split = 1;        // S4h: split clusters as soon as their internal structure stands above the noise
   int split_margin_bits = 40; // ... by this many bits
+  int cluster_tiles = 1;      // cluster passes as 128-column tile products on the int8 engine when no cluster straddles a tile
   int combine_path = 0;       // IMAD GEMM epilogue: 0 auto, 1 digit-serial thread per element, 2 warp-cooperative (digit per lane)
   int sstep_warp = 0;         // singleton_step: 1: warp-per-element kernel (digit per lane) when one column per CTA and n <= 64; measured 1 % faster at N = 16, 3 % slower at N = 64: off by default
   int sstep_cache = 1;        // singleton_step: stage the column's x, w digits in shared memory (one column per CTA, n <= 96)
