@@ -48,6 +48,8 @@ def lib():
         L.zkd_oracle_svd.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, vp, vp, vp, vp]
         L.zkd_oracle_svd_compare.restype = ctypes.c_int
         L.zkd_oracle_svd_compare.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, vp, vp, vp, vp, vp, vp, vp]
+        L.zkd_oracle_lu_solve.restype = ctypes.c_int
+        L.zkd_oracle_lu_solve.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, vp, vp]
         L.zkd_oracle_api_to_double.restype = ctypes.c_double
         L.zkd_oracle_api_to_double.argtypes = [vp, ctypes.c_int]
         L.zkd_oracle_api_from_double.argtypes = [vp, ctypes.c_int, ctypes.c_double]
@@ -126,6 +128,17 @@ def svd_compare(A: np.ndarray, M: int, N: int, S, U, V, S0=None, U0=None, V0=Non
                                  p(S0), p(U0), p(V0), out.ctypes.data)
     return {"log2_dsig_rel": out[0], "log2_resid_rel": out[1], "log2_orth": out[2], "vec_margin_bits": out[3], "log2_F": out[4],
             "groups": int(out[5]) if out[5] > -1e8 else 0, "max_group": int(out[6]) if out[6] > -1e8 else 0, "log2_vec_err": out[7]}
+
+
+def lu_solve(A: np.ndarray, B: np.ndarray, N: int, nrhs: int, prec: int = PREC, guard_bits: int = GUARD_BITS):
+    """Gaussian elimination with partial pivoting on MPFR (NEXT-3): X with A X = B.  Returns (X, status)."""
+    rb = real_bytes(prec)
+    A = np.ascontiguousarray(A, dtype=np.uint8)
+    B = np.ascontiguousarray(B, dtype=np.uint8)
+    assert A.size == N * N * 2 * rb and B.size == N * nrhs * 2 * rb
+    X = np.zeros(N * nrhs * 2 * rb, dtype=np.uint8)
+    rc = lib().zkd_oracle_lu_solve(N, nrhs, prec, guard_bits, A.ctypes.data, B.ctypes.data, X.ctypes.data)
+    return X, rc
 
 
 def api_to_double(buf, prec: int = PREC) -> float:

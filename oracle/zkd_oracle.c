@@ -987,3 +987,92 @@ int zkd_oracle_svd_compare(int M, int N, int prec, const uint8_t *A_api, const u
   mpfr_clear(tmpP); mpfr_clear(F); mpfr_clear(w); mpfr_clear(sr); mpfr_clear(si); mpfr_clear(acc); mpfr_clear(worst); mpfr_clear(t1);
   return 0;
 }
+
+/* ================================================================================================ */
+/* Linear solve by Gaussian elimination (8(a) S4a')                           */
+/* ================================================================================================ */
+/* PAPER.md:31 (section 2): ZKCM_OMP's main routines include "Gaussian elimination, LU decomposition".  Result definition
+ * (plain): X with A X = B for a nonsingular complex N x N matrix A and N x nrhs right-hand sides B.  Computed by the
+ * textbook method at working precision P_o = prec + guard_bits:
+ *   for k = 0 .. N-1: p = first row index >= k attaining max |a_ik|^2 (partial pivoting); swap rows k and p of A and B;
+ *                     for i > k: l = a_ik / a_kk; row_i(A) -= l row_k(A) (columns > k); row_i(B) -= l row_k(B);
+ *   back substitution: x_i = (b_i - sum_{j>i} a_ij x_j) / a_ii, i = N-1 .. 0;  round to prec bits.
+ * Layout: A[i][j] (N x N), B[i][j], X[i][j] (N x nrhs) row-major complex API numbers.
+ * Returns 0, 1 when a pivot is exactly zero (singular to working precision), 3 for malformed input.
+ * Parity status: pinned (tests/test_oracle_lu_pins.py: 2 x 2 Cramer closed form, B = A X0 with chosen X0, residual, exact
+ * permutation / diagonal / triangular cases, mpmath.lu_solve as a third opinion). */
+int zkd_oracle_lu_solve(int N, int nrhs, int prec, int guard_bits, const uint8_t *A_api, const uint8_t *B_api, uint8_t *X_api) {
+  const long Po = (long)prec + guard_bits;
+  const size_t rb = api_real_bytes(prec);
+  if (N < 1 || nrhs < 1 || prec < 64 || prec % 64) return 3;
+  int status = 0;
+  mpfr_t tmpP, best, m2, w, lr, li, dr, di, t1, t2;
+  mpfr_init2(tmpP, prec); mpfr_init2(best, Po); mpfr_init2(m2, Po); mpfr_init2(w, Po); mpfr_init2(lr, Po); mpfr_init2(li, Po);
+  mpfr_init2(dr, Po); mpfr_init2(di, Po); mpfr_init2(t1, Po); mpfr_init2(t2, Po);
+  rmat A = rmat_alloc(N, N, Po), B = rmat_alloc(N, nrhs, Po);
+  for (int i = 0; i < N && !status; ++i) {
+    for (int j = 0; j < N; ++j) {
+      const uint8_t *src = A_api + ((size_t)i * N + j) * 2 * rb;
+      if (api_get(RRE(A, i, j), src, prec, tmpP) || api_get(RIM(A, i, j), src + rb, prec, tmpP)) { status = 3; break; }
+    }
+    for (int j = 0; j < nrhs && !status; ++j) {
+      const uint8_t *src = B_api + ((size_t)i * nrhs + j) * 2 * rb;
+      if (api_get(RRE(B, i, j), src, prec, tmpP) || api_get(RIM(B, i, j), src + rb, prec, tmpP)) { status = 3; break; }
+    }
+  }
+  /* (x + i y) / (c + i d) = ((x c + y d) + i (y c - x d)) / (c^2 + d^2) */
+#define CDIV(outr, outi, xr, xi, cr, ci)                                   \
+  do {                                                                     \
+    mpfr_sqr(t1, cr, RN); mpfr_sqr(t2, ci, RN); mpfr_add(w, t1, t2, RN);   \
+    mpfr_fmma(t1, xr, cr, xi, ci, RN); mpfr_fmms(t2, xi, cr, xr, ci, RN);  \
+    mpfr_div(outr, t1, w, RN); mpfr_div(outi, t2, w, RN);                  \
+  } while (0)
+  for (int k = 0; k < N && !status; ++k) {
+    int p = k;
+    mpfr_set_si(best, -1, RN);
+    for (int i = k; i < N; ++i) {
+      mpfr_sqr(m2, RRE(A, i, k), RN); mpfr_sqr(w, RIM(A, i, k), RN); mpfr_add(m2, m2, w, RN);
+      if (mpfr_cmp(m2, best) > 0) { mpfr_set(best, m2, RN); p = i; }
+    }
+    if (mpfr_zero_p(best)) { status = 1; break; }
+    if (p != k) {
+      for (int j = 0; j < N; ++j) { mpfr_swap(RRE(A, k, j), RRE(A, p, j)); mpfr_swap(RIM(A, k, j), RIM(A, p, j)); }
+      for (int j = 0; j < nrhs; ++j) { mpfr_swap(RRE(B, k, j), RRE(B, p, j)); mpfr_swap(RIM(B, k, j), RIM(B, p, j)); }
+    }
+    for (int i = k + 1; i < N; ++i) {
+      CDIV(lr, li, RRE(A, i, k), RIM(A, i, k), RRE(A, k, k), RIM(A, k, k));
+      for (int j = k + 1; j < N; ++j) {
+        mpfr_fmms(t1, lr, RRE(A, k, j), li, RIM(A, k, j), RN); mpfr_sub(RRE(A, i, j), RRE(A, i, j), t1, RN);
+        mpfr_fmma(t1, lr, RIM(A, k, j), li, RRE(A, k, j), RN); mpfr_sub(RIM(A, i, j), RIM(A, i, j), t1, RN);
+      }
+      for (int j = 0; j < nrhs; ++j) {
+        mpfr_fmms(t1, lr, RRE(B, k, j), li, RIM(B, k, j), RN); mpfr_sub(RRE(B, i, j), RRE(B, i, j), t1, RN);
+        mpfr_fmma(t1, lr, RIM(B, k, j), li, RRE(B, k, j), RN); mpfr_sub(RIM(B, i, j), RIM(B, i, j), t1, RN);
+      }
+      mpfr_set_zero(RRE(A, i, k), +1); mpfr_set_zero(RIM(A, i, k), +1);
+    }
+  }
+  if (!status)
+    for (int c = 0; c < nrhs; ++c)
+      for (int i = N - 1; i >= 0; --i) {
+        mpfr_set(dr, RRE(B, i, c), RN); mpfr_set(di, RIM(B, i, c), RN);
+        for (int j = i + 1; j < N; ++j) {
+          mpfr_fmms(t1, RRE(A, i, j), RRE(B, j, c), RIM(A, i, j), RIM(B, j, c), RN); mpfr_sub(dr, dr, t1, RN);
+          mpfr_fmma(t1, RRE(A, i, j), RIM(B, j, c), RIM(A, i, j), RRE(B, j, c), RN); mpfr_sub(di, di, t1, RN);
+        }
+        CDIV(lr, li, dr, di, RRE(A, i, i), RIM(A, i, i));
+        mpfr_set(RRE(B, i, c), lr, RN); mpfr_set(RIM(B, i, c), li, RN); /* x_i overwrites b_i */
+      }
+#undef CDIV
+  if (!status)
+    for (int i = 0; i < N; ++i)
+      for (int j = 0; j < nrhs; ++j) {
+        uint8_t *dst = X_api + ((size_t)i * nrhs + j) * 2 * rb;
+        api_put(dst, RRE(B, i, j), prec, tmpP);
+        api_put(dst + rb, RIM(B, i, j), prec, tmpP);
+      }
+  rmat_free(&A); rmat_free(&B);
+  mpfr_clear(tmpP); mpfr_clear(best); mpfr_clear(m2); mpfr_clear(w); mpfr_clear(lr); mpfr_clear(li);
+  mpfr_clear(dr); mpfr_clear(di); mpfr_clear(t1); mpfr_clear(t2);
+  return status;
+}
