@@ -41,6 +41,7 @@ extern "C" {
 #define ZKD_ERR_WORKSPACE (-3)        /* workspace too small / allocation failed */
 #define ZKD_ERR_CUDA (-4)             /* a CUDA call failed (the sticky error is cleared) */
 #define ZKD_ERR_ARCH (-5)             /* device is not sm_100 */
+#define ZKD_ERR_CLUSTERED (-7)        /* zkd_diag_herm_rqi_lu only: the spectrum has clusters, which per-vector RQI cannot separate */
 #define ZKD_ERR_INTERNAL (-6)         /* internal consistency check failed (window overflow that could not be repaired) */
 
 #define ZKD_MAX_N 2048
@@ -117,6 +118,26 @@ int zkd_svd_bufsize(int M, int N, int batch, int prec_bits, size_t *workspace_by
 int zkd_svd_ws(int M, int N, int batch, int prec_bits, const void *A, void *S, void *U, void *V, void *workspace,
                size_t workspace_bytes, zkd_info *info, void *stream);
 int zkd_svd(int M, int N, int batch, int prec_bits, const void *A, void *S, void *U, void *V, void *stream);
+
+/* ---- linear systems by multiprecision LU and exact RQI on top of it (8(a) S4a') --------
+ * "Gaussian elimination, LU decomposition" are among ZKCM_OMP's main routines (section 2).
+ * zkd_lu_solve: X with A X = B for `batch` complex N x N systems with nrhs right-hand sides each, by LU with partial
+ * pivoting in the library's block fixed point: A and B are scaled by powers of two (max entry in [1/8, 1/4)), so the
+ * accuracy is ABSOLUTE, about cond(A) 2^-(prec_bits+2) relative to ||X||-scale, and pivots below 2^-26 max|a_ij| cannot
+ * be inverted.  A[b][i][j] (N x N), B[b][i][j], X[b][i][j] (N x nrhs): row-major complex API numbers, DEVICE pointers,
+ * 16-byte aligned, caller-owned; status (device int[batch], may be NULL): 0 solved, 1 singular to working precision,
+ * 2 pivot too small for the format, 3 malformed input number.  N <= ZKD_MAX_N. */
+int zkd_lu_solve_bufsize(int N, int nrhs, int batch, int prec_bits, size_t *workspace_bytes);
+int zkd_lu_solve(int N, int nrhs, int batch, int prec_bits, const void *A, const void *B, void *X, void *workspace,
+                 size_t workspace_bytes, int *status, void *stream);
+/* zkd_diag_herm_rqi_lu: the operation of zkd_diag_herm_ws by the paper's route taken literally:
+ * fp64 eigendecomposition, then for every eigenpair the Rayleigh quotient iteration sigma = x^H A x,
+ * y = (A - sigma I)^-1 x by one multiprecision LU per eigenpair and iteration, x = y / ||y|| (cubic: three iterations from
+ * an fp64 start).  O(N^4); isolated eigenvalues only (returns ZKD_ERR_CLUSTERED otherwise); N <= 64.  It exists as the
+ * in-product cross-check of the production path.  Arguments as zkd_diag_herm_ws. */
+int zkd_diag_herm_rqi_lu_bufsize(int N, int batch, int prec_bits, size_t *workspace_bytes);
+int zkd_diag_herm_rqi_lu(int N, int batch, int prec_bits, const void *A, void *eigvals, void *eigvecs, void *workspace,
+                         size_t workspace_bytes, zkd_info *info, void *stream);
 
 /* Tunables.  PROCESS-WIDE and unsynchronised: set them before, not during, calls of zkd_diag_herm* from
  * other threads; the library may be used from several host threads with distinct workspaces as long as the options, the

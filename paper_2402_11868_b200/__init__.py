@@ -52,6 +52,10 @@ def lib() -> ctypes.CDLL:
     L.zkd_svd_bufsize.argtypes = [ci, ci, ci, ci, ctypes.POINTER(cs)]
     L.zkd_svd_ws.argtypes = [ci, ci, ci, ci, vp, vp, vp, vp, vp, cs, vp, vp]
     L.zkd_svd.argtypes = [ci, ci, ci, ci, vp, vp, vp, vp, vp]
+    L.zkd_lu_solve_bufsize.argtypes = [ci, ci, ci, ci, ctypes.POINTER(cs)]
+    L.zkd_lu_solve.argtypes = [ci, ci, ci, ci, vp, vp, vp, vp, cs, vp, vp]
+    L.zkd_diag_herm_rqi_lu_bufsize.argtypes = [ci, ci, ci, ctypes.POINTER(cs)]
+    L.zkd_diag_herm_rqi_lu.argtypes = [ci, ci, ci, vp, vp, vp, vp, cs, vp, vp]
     L.zkd_set_option.argtypes = [ctypes.c_char_p, cd]
     L.zkd_get_option.argtypes = [ctypes.c_char_p, ctypes.POINTER(cd)]
     L.zkd_strerror.restype = ctypes.c_char_p
@@ -244,6 +248,37 @@ def svd(M: int, N: int, batch: int, A, S, U, V, prec_bits: int = PREC, stream=No
     _check(lib().zkd_svd(M, N, batch, prec_bits, _dev_u8(A, batch * M * N * 2 * rb, "A"), _dev_u8(S, batch * K * rb, "S"),
                          _dev_u8(U, batch * M * K * 2 * rb, "U"), _dev_u8(V, batch * N * K * 2 * rb, "V"), _stream_ptr(stream)),
            "zkd_svd")
+
+
+def lu_solve_bufsize(N: int, nrhs: int, batch: int, prec_bits: int = PREC) -> int:
+    n = ctypes.c_size_t()
+    _check(lib().zkd_lu_solve_bufsize(N, nrhs, batch, prec_bits, ctypes.byref(n)), "zkd_lu_solve_bufsize")
+    return int(n.value)
+
+
+def lu_solve(N: int, nrhs: int, batch: int, A, B, X, workspace, status=None, prec_bits: int = PREC, stream=None) -> None:
+    """zkd_lu_solve on device tensors (uint8, API layout): X with A X = B by multiprecision LU (NEXT-3)."""
+    rb = 16 + prec_bits // 8
+    _check(lib().zkd_lu_solve(N, nrhs, batch, prec_bits, _dev_u8(A, batch * N * N * 2 * rb, "A"), _dev_u8(B, batch * N * nrhs * 2 * rb, "B"),
+                              _dev_u8(X, batch * N * nrhs * 2 * rb, "X"), _dev_u8(workspace, lu_solve_bufsize(N, nrhs, batch, prec_bits), "workspace"),
+                              workspace.numel() * workspace.element_size(),
+                              _dev_u8(status, batch * 4, "status") if status is not None else None, _stream_ptr(stream)), "zkd_lu_solve")
+
+
+def diag_herm_rqi_lu_bufsize(N: int, batch: int, prec_bits: int = PREC) -> int:
+    n = ctypes.c_size_t()
+    _check(lib().zkd_diag_herm_rqi_lu_bufsize(N, batch, prec_bits, ctypes.byref(n)), "zkd_diag_herm_rqi_lu_bufsize")
+    return int(n.value)
+
+
+def diag_herm_rqi_lu(N: int, batch: int, A, eigvals, eigvecs, workspace, info=None, prec_bits: int = PREC, stream=None) -> None:
+    """zkd_diag_herm_rqi_lu: the exact-RQI-by-LU cross-check route (S4a'), arguments as diag_herm_ws."""
+    rb = 16 + prec_bits // 8
+    i = _dev_u8(info, batch * ctypes.sizeof(zkd_info), "info") if info is not None else None
+    _check(lib().zkd_diag_herm_rqi_lu(N, batch, prec_bits, _dev_u8(A, batch * N * N * 2 * rb, "A"), _dev_u8(eigvals, batch * N * rb, "eigvals"),
+                                      _dev_u8(eigvecs, batch * N * N * 2 * rb, "eigvecs"),
+                                      _dev_u8(workspace, diag_herm_rqi_lu_bufsize(N, batch, prec_bits), "workspace"),
+                                      workspace.numel() * workspace.element_size(), i, _stream_ptr(stream)), "zkd_diag_herm_rqi_lu")
 
 
 def read_info(info_tensor, batch: int) -> list[dict]:

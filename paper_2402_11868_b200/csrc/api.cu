@@ -183,6 +183,7 @@ const char* zkd_strerror(int code) {
     case ZKD_ERR_CUDA: return "CUDA error";
     case ZKD_ERR_ARCH: return "device is not sm_100";
     case ZKD_ERR_INTERNAL: return "internal consistency check failed";
+    case ZKD_ERR_CLUSTERED: return "clustered spectrum: exact per-vector RQI does not apply";
     default: return "unknown error";
   }
 }
@@ -434,6 +435,36 @@ int zkd_svd(int M, int N, int batch, int prec_bits, const void* A, void* S, void
   int rc = zkd_svd_ws(M, N, batch, prec_bits, A, S, U, V, ws, bytes, nullptr, stream);
   cudaFreeAsync(ws, s);
   return rc;
+}
+int zkd_lu_solve_bufsize(int N, int nrhs, int batch, int prec_bits, size_t* workspace_bytes) {
+  if (!prec_supported(prec_bits)) return ZKD_ERR_UNSUPPORTED_PREC;
+  if (N < 1 || N > ZKD_MAX_N || nrhs < 1 || batch < 1 || batch > 65535 || !workspace_bytes) return ZKD_ERR_INVALID_ARG;
+  *workspace_bytes = lu_workspace_bytes(N, nrhs, batch);
+  return ZKD_OK;
+}
+int zkd_lu_solve(int N, int nrhs, int batch, int prec_bits, const void* A, const void* B, void* X, void* workspace, size_t workspace_bytes,
+                 int* status, void* stream) {
+  if (!prec_supported(prec_bits)) return ZKD_ERR_UNSUPPORTED_PREC;
+  if (N < 1 || N > ZKD_MAX_N || nrhs < 1 || batch < 1 || batch > 65535 || !A || !B || !X || !workspace) return ZKD_ERR_INVALID_ARG;
+  if (((uintptr_t)A | (uintptr_t)B | (uintptr_t)X | (uintptr_t)workspace) & 15) return ZKD_ERR_INVALID_ARG;
+  if (workspace_bytes < lu_workspace_bytes(N, nrhs, batch)) return ZKD_ERR_WORKSPACE;
+  ZKD_TRY(check_device());
+  return lu_solve_device(N, nrhs, batch, prec_bits, A, B, X, workspace, workspace_bytes, status, (cudaStream_t)stream);
+}
+int zkd_diag_herm_rqi_lu_bufsize(int N, int batch, int prec_bits, size_t* workspace_bytes) {
+  ZKD_TRY(check_diag_args(N, batch, prec_bits));
+  if (N > 64 || !workspace_bytes) return ZKD_ERR_INVALID_ARG;
+  *workspace_bytes = rqi_lu_workspace_bytes(N, batch);
+  return ZKD_OK;
+}
+int zkd_diag_herm_rqi_lu(int N, int batch, int prec_bits, const void* A, void* eigvals, void* eigvecs, void* workspace,
+                         size_t workspace_bytes, zkd_info* info, void* stream) {
+  ZKD_TRY(check_diag_args(N, batch, prec_bits));
+  if (N > 64 || !A || !eigvals || !eigvecs || !workspace) return ZKD_ERR_INVALID_ARG;
+  if (((uintptr_t)A | (uintptr_t)eigvals | (uintptr_t)eigvecs | (uintptr_t)workspace) & 15) return ZKD_ERR_INVALID_ARG;
+  if (workspace_bytes < rqi_lu_workspace_bytes(N, batch)) return ZKD_ERR_WORKSPACE;
+  ZKD_TRY(check_device());
+  return diag_herm_rqi_lu_device(N, batch, prec_bits, A, eigvals, eigvecs, workspace, workspace_bytes, info, (cudaStream_t)stream);
 }
 int zkd_diag_herm_host(int N, int batch, int prec_bits, const void* A_host, void* eigvals_host, void* eigvecs_host,
                        zkd_info* info_host) {

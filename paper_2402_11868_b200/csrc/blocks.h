@@ -69,4 +69,15 @@ int svd_zgather(int n, int batch, int d0, int r, int g, const int* mats_dev, con
 int fxc_shr(size_t count, int32_t* X, int bits, cudaStream_t s);
 int svd_phase(int M, int N, int batch, int32_t* U, int32_t* V, cudaStream_t s);
 
+
+// lu.cu (NEXT-3, S4a')
+// P A = L U in place for nprob N x N problems stored consecutively (complex FX planes over nprob N N elements); perm: [nprob][N];
+// invd: complex FX [nprob][N] (1 / u_kk); flags: [nprob] (1 singular, 2 a pivot too small to invert, 4 the last pivot too small)
+int lu_factor(int N, int nprob, int32_t* Mx, int* perm, int32_t* invd, int* flags, cudaStream_t s);
+// B (complex FX planes over nprob N nrhs elements) <- A^-1 B (mode 0) or the unit-norm direction of A^-1 b (mode 1, nrhs = 1)
+int lu_solve(int N, int nrhs, int nprob, int mode, const int32_t* Mx, const int* perm, const int32_t* invd, int32_t* B, int* flags,
+             cudaStream_t s);
+int rqi_setup(int N, int batch, const int32_t* A, const int32_t* theta, const int32_t* X, int32_t* Mx, int32_t* rhs, cudaStream_t s);
+int rqi_scatter(int N, int batch, const int32_t* rhs, const int* flags, int32_t* X, cudaStream_t s);
+
 }  // namespace zkd

@@ -140,6 +140,16 @@ int fxc_to_api(size_t count, const int32_t* src_fxc, void* dst_api, cudaStream_t
   count_launch(2);
   return launch_check();
 }
+// the same with one power-of-two scale per `per_scale` complex elements (value = fx 2^-scale)
+int fxc_to_api_scaled(size_t count, const int32_t* src_fxc, void* dst_api, const int* scale_dev, size_t per_scale, cudaStream_t s, int prec) {
+  KtScope kt_scope(KC_IO, s);
+  if (count == 0) return ZKD_OK;
+  for (int part = 0; part < 2; ++part)
+    fx_to_api_kernel<<<(unsigned)((count + 127) / 128), 128, 0, s>>>(count, src_fxc + (size_t)part * ND * count, (uint8_t*)dst_api,
+                                                                     2, part, 0, scale_dev, 1, per_scale ? per_scale : 1, prec);
+  count_launch(2);
+  return launch_check();
+}
 int fx_from_api(int count, const void* src_api, int32_t* dst_fx, int scale_bits, cudaStream_t s, int prec) {
   return fx_from_api_scaled((size_t)count, src_api, dst_fx, scale_bits, nullptr, 0, 1, nullptr, s, prec);
 }

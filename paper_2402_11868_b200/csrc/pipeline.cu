@@ -959,4 +959,101 @@ int svd_device(int M, int N, int batch, int prec, const void* A_api, void* S_api
   return ZKD_OK;
 }
 
+// ---- S4a': exact Rayleigh quotient iteration by multiprecision LU (lu.cu), the cross-check route for isolated spectra ---------------
+size_t rqi_lu_workspace_bytes(int N, int batch) {
+  const size_t cnt = (size_t)N * N * batch;
+  return FxC::bytes(cnt * N) + 8 * (FxC::bytes(cnt) + 4096) + 3 * 16 * cnt + 64 * (size_t)N * batch + gemm_workspace_bytes(N, N, N, batch) +
+         (34u << 20);
+}
+
+int diag_herm_rqi_lu_device(int N, int batch, int prec, const void* A_api, void* eigvals_api, void* eigvecs_api, void* ws, size_t ws_bytes,
+                            zkd_info* info, cudaStream_t s) {
+  const Options& opt = options();
+  Ctx c;
+  c.prec = prec;
+  c.tol_bits = std::min(opt.tol_bits, 790) - (kPrec - prec);
+  c.fb = 0;  // full width: this route is the cross-check, not the fast path
+  c.s = s;
+  c.ar.base = (char*)ws;
+  c.ar.size = ws_bytes;
+  c.ar.stream = s;
+  c.h_pin = pinned_staging();
+  if (!c.h_pin) return ZKD_ERR_CUDA;
+  c.gemm_ws_bytes = gemm_workspace_bytes(N, N, N, batch) + (32u << 20);
+  c.gemm_ws = c.ar.alloc(c.gemm_ws_bytes);
+  const size_t cnt = (size_t)N * N * batch, P = (size_t)N * batch;
+  int32_t* A = (int32_t*)c.ar.alloc(FxC::bytes(cnt));
+  int32_t* X = (int32_t*)c.ar.alloc(FxC::bytes(cnt));
+  int32_t* W = (int32_t*)c.ar.alloc(FxC::bytes(cnt));
+  int32_t* R = (int32_t*)c.ar.alloc(FxC::bytes(cnt));
+  int32_t* Sm = (int32_t*)c.ar.alloc(FxC::bytes(cnt));
+  int32_t* Mx = (int32_t*)c.ar.alloc(FxC::bytes(cnt * N));
+  int32_t* rhs = (int32_t*)c.ar.alloc(FxC::bytes(cnt));
+  int32_t* invd = (int32_t*)c.ar.alloc(FxC::bytes(cnt));
+  int32_t* lam = (int32_t*)c.ar.alloc(FxR::bytes(P));
+  int32_t* lam_sorted = (int32_t*)c.ar.alloc(FxR::bytes(P));
+  double2* A64 = c.ar.get<double2>(cnt);
+  double2* V = c.ar.get<double2>(cnt);
+  double* mu = c.ar.get<double>(P);
+  int* perm = c.ar.get<int>(cnt);
+  int* flags = c.ar.get<int>(P);
+  int* scale = c.ar.get<int>((size_t)2 * batch);
+  int* status = c.ar.get<int>((size_t)batch);
+  int* rank = c.ar.get<int>(P);
+  int* cl = c.ar.get<int>(P);
+  int* cle = c.ar.get<int>(P);
+  int* stats = c.ar.get<int>((size_t)2 * batch);
+  int* pm = c.ar.get<int>((size_t)2 * batch);
+  int* scal = c.ar.get<int>(S_NUM);
+  if (!c.gemm_ws || !A || !X || !W || !R || !Sm || !Mx || !rhs || !invd || !lam || !lam_sorted || !A64 || !V || !mu || !perm || !flags ||
+      !scale || !status || !rank || !cl || !cle || !stats || !pm || !scal)
+    return ZKD_ERR_WORKSPACE;
+  ZKD_TRY(ingest_herm(N, batch, A_api, A, scale, status, s, prec));
+  ZKD_TRY(fxc_to_c64(cnt, A, A64, s));
+  ZKD_TRY(seed_fp64(N, batch, (const double*)A64, mu, (double*)V, opt.seed_sweeps, s));
+  ZKD_TRY(cluster_detect(N, batch, A64, mu, opt.tau_bits, nullptr, cl, cle, stats, s));
+  std::vector<int> h_stats((size_t)2 * batch);
+  ZKD_CUDA_TRY(cudaMemcpyAsync(h_stats.data(), stats, sizeof(int) * 2 * batch, cudaMemcpyDeviceToHost, s));
+  ZKD_CUDA_TRY(cudaStreamSynchronize(s));
+  for (int b = 0; b < batch; ++b)
+    if (h_stats[2 * b + 1] > 1) return ZKD_ERR_CLUSTERED;  // per-vector RQI cannot separate clustered eigenvalues
+  ZKD_TRY(init_x(cnt, V, X, s));
+  auto side = [&](const int32_t* fx, int top, int nw) {
+    GemmSide g;
+    g.fx = fx; g.rows = N; g.cols = N; g.top_bit = top; g.nw = nw;
+    return g;
+  };
+  const int tol_msb = 812 - c.tol_bits;
+  int status_level = 2, steps = 0, hs[S_NUM], prev = 1 << 30;
+  for (int it = 0; it < 8; ++it) {
+    ZKD_CUDA_TRY(cudaMemsetAsync(scal, 0, sizeof(int) * S_NUM, s));
+    ZKD_CUDA_TRY(cudaMemsetAsync(pm, 0, sizeof(int) * 2 * batch, s));
+    // sigma_j = x_j^H A x_j (and the residual that decides convergence): W = A X at full width, then the fused singleton step
+    ZKD_TRY(gemm_complex(N, N, N, batch, side(A, 812, kND), side(X, 815, it == 0 ? 3 : kND), W, GemmMode::Assign, -1, opt.gemm_path, c.gemm_ws,
+                         c.gemm_ws_bytes, scal + S_ERR, nullptr, s));
+    ZKD_TRY(singleton_step(N, batch, X, W, R, Sm, lam, scal + S_MSB_G, scal + S_MSB_R, s, nullptr, nullptr, pm + batch));
+    ZKD_TRY(read_scalars(c, scal, S_NUM, hs));
+    if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
+    steps = it + 1;
+    if (opt.verbose) fprintf(stderr, "[zkd] exact RQI it %d: msbR %d (2^%d) msbG %d\n", it, hs[S_MSB_R], hs[S_MSB_R] - 812, hs[S_MSB_G]);
+    if (hs[S_MSB_R] <= tol_msb && hs[S_MSB_G] <= 812 - (c.tol_bits / 2 + 15)) { status_level = 0; break; }
+    if (it > 1 && hs[S_MSB_R] >= prev - 2 && hs[S_MSB_R] > tol_msb) { status_level = 1; break; }
+    prev = hs[S_MSB_R];
+    // y_j = (A - sigma_j I)^-1 x_j, normalised: one LU per eigenpair
+    ZKD_TRY(rqi_setup(N, batch, A, lam, X, Mx, rhs, s));
+    ZKD_TRY(lu_factor(N, (int)P, Mx, perm, invd, flags, s));
+    ZKD_TRY(lu_solve(N, 1, (int)P, 1, Mx, perm, invd, rhs, flags, s));
+    ZKD_TRY(rqi_scatter(N, batch, rhs, flags, X, s));
+  }
+  ZKD_TRY(resid_per_matrix(N, batch, R, pm, s));
+  ZKD_TRY(finalize_export(N, batch, X, lam, scale, eigvals_api, eigvecs_api, A /* scratch */, lam_sorted, rank, s, prec));
+  if (info) {
+    info_kernel<<<(batch + 127) / 128, 128, 0, s>>>(batch, status, status_level, steps, tol_msb, pm, stats, info);
+    count_launch();
+    ZKD_TRY(launch_check());
+  }
+  ZKD_CUDA_TRY(cudaStreamSynchronize(s));
+  return ZKD_OK;
+}
+
 }  // namespace zkd

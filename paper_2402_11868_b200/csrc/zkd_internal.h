@@ -118,6 +118,12 @@ size_t diag_workspace_bytes(int N, int batch);
 int diag_herm_device(int N, int batch, int prec, const void* A_api, void* eigvals_api, void* eigvecs_api, void* ws, size_t ws_bytes,
                      zkd_info* info, cudaStream_t s);
 
+size_t lu_workspace_bytes(int N, int nrhs, int batch);
+int lu_solve_device(int N, int nrhs, int batch, int prec, const void* A_api, const void* B_api, void* X_api, void* ws, size_t ws_bytes,
+                    int* status_dev, cudaStream_t s);
+size_t rqi_lu_workspace_bytes(int N, int batch);
+int diag_herm_rqi_lu_device(int N, int batch, int prec, const void* A_api, void* eigvals_api, void* eigvecs_api, void* ws, size_t ws_bytes,
+                            zkd_info* info, cudaStream_t s);
 size_t svd_workspace_bytes(int M, int N, int batch);
 int svd_device(int M, int N, int batch, int prec, const void* A_api, void* S_api, void* U_api, void* V_api, void* ws, size_t ws_bytes,
                zkd_info* info, cudaStream_t s);
@@ -130,6 +136,7 @@ int fx_from_api_scaled(size_t count, const void* src_api, int32_t* dst_fx, int s
 int fx_to_api_scaled(size_t count, const int32_t* src_fx, void* dst_api, int scale_bits, const int* scale_dev, int scale_stride,
                      size_t per_scale, cudaStream_t s, int prec = kPrec);
 int fxc_to_api(size_t count, const int32_t* src_fxc, void* dst_api, cudaStream_t s, int prec = kPrec);
+int fxc_to_api_scaled(size_t count, const int32_t* src_fxc, void* dst_api, const int* scale_dev, size_t per_scale, cudaStream_t s, int prec = kPrec);
 int fx_prim(int op, size_t count, const int32_t* a, const int32_t* b, int32_t* out, cudaStream_t s);
 int measure_imad_peak(double millis, double* per_sec, cudaStream_t s);
 int measure_dfma_peak(double millis, double* flops_per_sec, cudaStream_t s);
