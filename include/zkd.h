@@ -139,6 +139,25 @@ int zkd_diag_herm_rqi_lu_bufsize(int N, int batch, int prec_bits, size_t *worksp
 int zkd_diag_herm_rqi_lu(int N, int batch, int prec_bits, const void *A, void *eigvals, void *eigvecs, void *workspace,
                          size_t workspace_bytes, zkd_info *info, void *stream);
 
+/* ---- minimal MPS two-site update around the eigensolver ------------------------------
+ * An MPS is a "nested Schmidt decomposition" (section 1); its simulation cost is dominated by "Hermitian matrix
+ * diagonalization" (section 2.1), and Schmidt weights of order epsilon ~ 2^(-n+1) must survive
+ * (footnote) - hence the precision.  One update of `batch` independent bonds:
+ *     Theta0 = L R;   Theta[(a,i'),(j',c)] = sum_ij G[(i'j'),(ij)] Theta0[(a,i),(j,c)];   rho = Theta Theta^H;
+ *     rho = U diag(w) U^H  (zkd's Hermitian eigendecomposition);   L' = U[:, 0:K];   R' = L'^H Theta
+ *   L[b]   : (chiL d) x chiC, rows (a, i);     R[b]  : chiC x (d chiR), columns (j, c);     G[b] : d^2 x d^2, rows (i' j'),
+ *            columns (i j): the two-site gate.  All row-major complex API numbers.
+ *   W[b]   : K reals, the Schmidt weights (eigenvalues of rho) in DESCENDING order, K = min(chiL d, max_keep) (max_keep <= 0:
+ *            no limit); good to absolute 2^-(prec_bits - 28) trace(rho).
+ *   Lnew[b]: (chiL d) x K, orthonormal columns (phase: first component of largest modulus real positive);
+ *   Rnew[b]: K x (d chiR), so that Theta = Lnew Rnew up to the discarded weights.
+ *   kept   : device int[batch]: how many leading weights exceed 2^-cutoff_bits trace(rho) (the caller truncates to that).
+ * All pointers DEVICE, 16-byte aligned, caller-owned; info as for zkd_diag_herm_ws (may be NULL).  chiL d <= ZKD_MAX_N. */
+int zkd_mps_two_site_update_bufsize(int chiL, int chiC, int chiR, int d, int batch, int prec_bits, size_t *workspace_bytes);
+int zkd_mps_two_site_update(int chiL, int chiC, int chiR, int d, int batch, int prec_bits, const void *L, const void *R,
+                            const void *G, int max_keep, int cutoff_bits, void *W, void *Lnew, void *Rnew, int *kept,
+                            zkd_info *info, void *workspace, size_t workspace_bytes, void *stream);
+
 /* Tunables.  PROCESS-WIDE and unsynchronised: set them before, not during, calls of zkd_diag_herm* from
  * other threads; the library may be used from several host threads with distinct workspaces as long as the options, the
  * counters and the kernel timing are left alone meanwhile, and it serves ONE device per process (the device current at

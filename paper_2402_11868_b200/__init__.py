@@ -56,6 +56,8 @@ def lib() -> ctypes.CDLL:
     L.zkd_lu_solve.argtypes = [ci, ci, ci, ci, vp, vp, vp, vp, cs, vp, vp]
     L.zkd_diag_herm_rqi_lu_bufsize.argtypes = [ci, ci, ci, ctypes.POINTER(cs)]
     L.zkd_diag_herm_rqi_lu.argtypes = [ci, ci, ci, vp, vp, vp, vp, cs, vp, vp]
+    L.zkd_mps_two_site_update_bufsize.argtypes = [ci, ci, ci, ci, ci, ci, ctypes.POINTER(cs)]
+    L.zkd_mps_two_site_update.argtypes = [ci, ci, ci, ci, ci, ci, vp, vp, vp, ci, ci, vp, vp, vp, vp, vp, vp, cs, vp]
     L.zkd_set_option.argtypes = [ctypes.c_char_p, cd]
     L.zkd_get_option.argtypes = [ctypes.c_char_p, ctypes.POINTER(cd)]
     L.zkd_strerror.restype = ctypes.c_char_p
@@ -279,6 +281,27 @@ def diag_herm_rqi_lu(N: int, batch: int, A, eigvals, eigvecs, workspace, info=No
                                       _dev_u8(eigvecs, batch * N * N * 2 * rb, "eigvecs"),
                                       _dev_u8(workspace, diag_herm_rqi_lu_bufsize(N, batch, prec_bits), "workspace"),
                                       workspace.numel() * workspace.element_size(), i, _stream_ptr(stream)), "zkd_diag_herm_rqi_lu")
+
+
+def mps_two_site_update_bufsize(chiL: int, chiC: int, chiR: int, d: int, batch: int, prec_bits: int = PREC) -> int:
+    n = ctypes.c_size_t()
+    _check(lib().zkd_mps_two_site_update_bufsize(chiL, chiC, chiR, d, batch, prec_bits, ctypes.byref(n)), "zkd_mps_two_site_update_bufsize")
+    return int(n.value)
+
+
+def mps_two_site_update(chiL: int, chiC: int, chiR: int, d: int, batch: int, L, R, G, W, Lnew, Rnew, kept, workspace, max_keep: int = 0,
+                        cutoff_bits: int = 700, info=None, prec_bits: int = PREC, stream=None) -> None:
+    """zkd_mps_two_site_update on device tensors (uint8, API layout; kept: int32[batch]) - NEXT-4."""
+    rb = 16 + prec_bits // 8
+    mL, mR = chiL * d, d * chiR
+    K = min(mL, max_keep) if max_keep > 0 else mL
+    i = _dev_u8(info, batch * ctypes.sizeof(zkd_info), "info") if info is not None else None
+    _check(lib().zkd_mps_two_site_update(
+        chiL, chiC, chiR, d, batch, prec_bits, _dev_u8(L, batch * mL * chiC * 2 * rb, "L"), _dev_u8(R, batch * chiC * mR * 2 * rb, "R"),
+        _dev_u8(G, batch * d ** 4 * 2 * rb, "G"), max_keep, cutoff_bits, _dev_u8(W, batch * K * rb, "W"),
+        _dev_u8(Lnew, batch * mL * K * 2 * rb, "Lnew"), _dev_u8(Rnew, batch * K * mR * 2 * rb, "Rnew"), _dev_u8(kept, batch * 4, "kept"), i,
+        _dev_u8(workspace, mps_two_site_update_bufsize(chiL, chiC, chiR, d, batch, prec_bits), "workspace"),
+        workspace.numel() * workspace.element_size(), _stream_ptr(stream)), "zkd_mps_two_site_update")
 
 
 def read_info(info_tensor, batch: int) -> list[dict]:

@@ -466,6 +466,30 @@ int zkd_diag_herm_rqi_lu(int N, int batch, int prec_bits, const void* A, void* e
   ZKD_TRY(check_device());
   return diag_herm_rqi_lu_device(N, batch, prec_bits, A, eigvals, eigvecs, workspace, workspace_bytes, info, (cudaStream_t)stream);
 }
+static int check_mps_args(int chiL, int chiC, int chiR, int d, int batch, int prec_bits) {
+  if (!prec_supported(prec_bits)) return ZKD_ERR_UNSUPPORTED_PREC;
+  if (chiL < 1 || chiC < 1 || chiR < 1 || d < 1 || d > 16 || batch < 1 || batch > 65535) return ZKD_ERR_INVALID_ARG;
+  if ((long)chiL * d > ZKD_MAX_N || (long)d * chiR > 65536 || chiC > 65536) return ZKD_ERR_INVALID_ARG;
+  return ZKD_OK;
+}
+int zkd_mps_two_site_update_bufsize(int chiL, int chiC, int chiR, int d, int batch, int prec_bits, size_t* workspace_bytes) {
+  ZKD_TRY(check_mps_args(chiL, chiC, chiR, d, batch, prec_bits));
+  if (!workspace_bytes) return ZKD_ERR_INVALID_ARG;
+  *workspace_bytes = mps_workspace_bytes(chiL, chiC, chiR, d, batch);
+  return ZKD_OK;
+}
+int zkd_mps_two_site_update(int chiL, int chiC, int chiR, int d, int batch, int prec_bits, const void* L, const void* R, const void* G,
+                            int max_keep, int cutoff_bits, void* W, void* Lnew, void* Rnew, int* kept, zkd_info* info, void* workspace,
+                            size_t workspace_bytes, void* stream) {
+  ZKD_TRY(check_mps_args(chiL, chiC, chiR, d, batch, prec_bits));
+  if (!L || !R || !G || !W || !Lnew || !Rnew || !kept || !workspace || cutoff_bits < 0 || cutoff_bits > 800) return ZKD_ERR_INVALID_ARG;
+  if (((uintptr_t)L | (uintptr_t)R | (uintptr_t)G | (uintptr_t)W | (uintptr_t)Lnew | (uintptr_t)Rnew | (uintptr_t)workspace) & 15)
+    return ZKD_ERR_INVALID_ARG;
+  if (workspace_bytes < mps_workspace_bytes(chiL, chiC, chiR, d, batch)) return ZKD_ERR_WORKSPACE;
+  ZKD_TRY(check_device());
+  return mps_update_device(chiL, chiC, chiR, d, batch, prec_bits, L, R, G, max_keep, cutoff_bits, W, Lnew, Rnew, kept, info, workspace,
+                           workspace_bytes, (cudaStream_t)stream);
+}
 int zkd_diag_herm_host(int N, int batch, int prec_bits, const void* A_host, void* eigvals_host, void* eigvecs_host,
                        zkd_info* info_host) {
   ZKD_TRY(check_diag_args(N, batch, prec_bits));

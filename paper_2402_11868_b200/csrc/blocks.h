@@ -70,6 +70,16 @@ int fxc_shr(size_t count, int32_t* X, int bits, cudaStream_t s);
 int svd_phase(int M, int N, int batch, int32_t* U, int32_t* V, cudaStream_t s);
 
 
+// mps.cu (NEXT-4)
+int conj_transpose(int R, int C, int batch, const int32_t* src, int32_t* dst, cudaStream_t s);
+int mps_gate(int chiL, int chiR, int d, int batch, const int32_t* T0, const int32_t* G, int32_t* T, int* msb_out, cudaStream_t s);
+int fxc_shl(size_t count, int32_t* X, int bits, cudaStream_t s);
+int mps_select(int n, int K, int batch, int cutoff_bits, const int32_t* lam_sorted, int32_t* Wt, int* kept, cudaStream_t s);
+int mps_take(int n, int K, int batch, const int32_t* Xs, int32_t* Lnew, cudaStream_t s);
+int mps_scales(int batch, const int* sl, const int* sr, const int* sg, int t, int u, int* s_theta, int* s_w, cudaStream_t s);
+// S6 pieces on their own: out[:, rank[j]] = x_j with the phase convention A9 applied (out: FxC batch N N)
+int phase_sorted(int N, int batch, const int32_t* X, const int* rank, int32_t* out, cudaStream_t s);
+
 // lu.cu (NEXT-3, S4a')
 // P A = L U in place for nprob N x N problems stored consecutively (complex FX planes over nprob N N elements); perm: [nprob][N];
 // invd: complex FX [nprob][N] (1 / u_kk); flags: [nprob] (1 singular, 2 a pivot too small to invert, 4 the last pivot too small)

@@ -460,6 +460,14 @@ int rank_sort(int N, int batch, const int32_t* lam, int* rank, int32_t* lam_sort
   return launch_check();
 }
 
+int phase_sorted(int N, int batch, const int32_t* X, const int* rank, int32_t* out, cudaStream_t s) {
+  KtScope kt_scope(KC_OTHER, s);
+  const size_t nl = (size_t)N * batch;
+  phase_kernel<<<(unsigned)((nl * 32 + 127) / 128), 128, 0, s>>>(N, batch, X, rank, out);
+  count_launch();
+  return launch_check();
+}
+
 int finalize_export(int N, int batch, const int32_t* X, const int32_t* lam, const int* scale, void* eigvals_api, void* eigvecs_api,
                     int32_t* scratch, int32_t* lam_sorted, int* rank, cudaStream_t s, int prec) {
   KtScope kt_scope(KC_IO, s);

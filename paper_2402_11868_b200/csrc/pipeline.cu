@@ -1056,4 +1056,120 @@ int diag_herm_rqi_lu_device(int N, int batch, int prec, const void* A_api, void*
   return ZKD_OK;
 }
 
+// ---- NEXT-4: minimal MPS two-site update around the eigensolver (mps.cu) ---------------------------------------
+size_t mps_workspace_bytes(int chiL, int chiC, int chiR, int d, int batch) {
+  const size_t mL = (size_t)chiL * d, mR = (size_t)d * chiR;
+  const size_t big = std::max(std::max(mL * mL, mL * mR), std::max(mL * chiC, chiC * mR)) * batch;
+  return diag_workspace_bytes((int)mL, batch) + 12 * (FxC::bytes(big) + 4096) + FxC::bytes((size_t)d * d * d * d * batch) +
+         64 * (mL + 16) * batch + (8u << 20);
+}
+
+int mps_update_device(int chiL, int chiC, int chiR, int d, int batch, int prec, const void* L_api, const void* R_api, const void* G_api,
+                      int max_keep, int cutoff_bits, void* W_api, void* Lnew_api, void* Rnew_api, int* kept_dev, zkd_info* info, void* ws,
+                      size_t ws_bytes, cudaStream_t s) {
+  const Options& opt = options();
+  const int mL = chiL * d, mR = d * chiR, n = mL, d2 = d * d;
+  const int K = max_keep > 0 ? std::min(max_keep, mL) : mL;
+  Ctx c;
+  c.prec = prec;
+  c.tol_bits = std::min(opt.tol_bits, 790) - (kPrec - prec);
+  c.fb = std::max(0, kFRAC - (c.tol_bits + 42));
+  c.s = s;
+  c.ar.base = (char*)ws;
+  c.ar.size = ws_bytes;
+  c.ar.stream = s;
+  c.h_pin = pinned_staging();
+  if (!c.h_pin) return ZKD_ERR_CUDA;
+  const int gmax = std::max(std::max(mL, mR), chiC);
+  c.gemm_ws_bytes = std::max(gemm_workspace_bytes(n, n, n, batch), gemm_workspace_bytes(gmax, gmax, gmax, batch)) + (32u << 20);
+  c.gemm_ws = c.ar.alloc(c.gemm_ws_bytes);
+  const size_t cnt = (size_t)n * n * batch, tcnt = (size_t)mL * mR * batch;
+  int32_t* Lf = (int32_t*)c.ar.alloc(FxC::bytes((size_t)mL * chiC * batch));
+  int32_t* Rf = (int32_t*)c.ar.alloc(FxC::bytes((size_t)chiC * mR * batch));
+  int32_t* Gf = (int32_t*)c.ar.alloc(FxC::bytes((size_t)d2 * d2 * batch));
+  int32_t* T0 = (int32_t*)c.ar.alloc(FxC::bytes(tcnt));
+  int32_t* T = (int32_t*)c.ar.alloc(FxC::bytes(tcnt));
+  int32_t* TH = (int32_t*)c.ar.alloc(FxC::bytes(tcnt));
+  int32_t* rho = (int32_t*)c.ar.alloc(FxC::bytes(cnt));
+  int32_t* X = (int32_t*)c.ar.alloc(FxC::bytes(cnt));
+  int32_t* Xs = (int32_t*)c.ar.alloc(FxC::bytes(cnt));
+  int32_t* Ln = (int32_t*)c.ar.alloc(FxC::bytes((size_t)n * K * batch));
+  int32_t* Rn = (int32_t*)c.ar.alloc(FxC::bytes((size_t)K * mR * batch));
+  int32_t* Wt = (int32_t*)c.ar.alloc(FxR::bytes((size_t)K * batch));
+  int32_t* lam = (int32_t*)c.ar.alloc(FxR::bytes((size_t)n * batch));
+  int32_t* lam_sorted = (int32_t*)c.ar.alloc(FxR::bytes((size_t)n * batch));
+  int* ints = c.ar.get<int>((size_t)(16 + n) * batch + S_NUM);
+  if (!c.gemm_ws || !Lf || !Rf || !Gf || !T0 || !T || !TH || !rho || !X || !Xs || !Ln || !Rn || !Wt || !lam || !lam_sorted || !ints)
+    return ZKD_ERR_WORKSPACE;
+  int *sl = ints, *sr = ints + 2 * batch, *sg = ints + 4 * batch, *stl = ints + 6 * batch, *str_ = ints + 7 * batch, *stg = ints + 8 * batch;
+  int *s_theta = ints + 9 * batch, *s_w = ints + 10 * batch, *pm = ints + 11 * batch, *status = ints + 13 * batch;
+  int *cl_stats_dev = ints + 14 * batch, *rank = ints + 16 * batch, *scal = ints + (size_t)(16 + n) * batch;
+  ZKD_TRY(ingest_general(mL, chiC, batch, L_api, Lf, sl, stl, s, prec));
+  ZKD_TRY(ingest_general(chiC, mR, batch, R_api, Rf, sr, str_, s, prec));
+  ZKD_TRY(ingest_general(d2, d2, batch, G_api, Gf, sg, stg, s, prec));
+  auto side = [&](const int32_t* fx, int rows, int cols, int top, bool ct) {
+    GemmSide g;
+    g.fx = fx; g.rows = rows; g.cols = cols; g.conj_transpose = ct; g.top_bit = top; g.nw = digits_for(top, c.fb);
+    return g;
+  };
+  ZKD_CUDA_TRY(cudaMemsetAsync(scal, 0, sizeof(int) * S_NUM, s));
+  // Theta0 = L R, then the gate on the physical indices
+  ZKD_TRY(gemm_complex(mL, mR, chiC, batch, side(Lf, mL, chiC, 812, false), side(Rf, chiC, mR, 812, false), T0, GemmMode::Assign, -1, opt.gemm_path,
+                       c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s));
+  ZKD_TRY(mps_gate(chiL, chiR, d, batch, T0, Gf, T, scal + S_MSB_T, s));
+  int hs[S_NUM];
+  ZKD_TRY(read_scalars(c, scal, S_NUM, hs));
+  if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
+  // one power of two for the batch so that max |Theta| lies in [1/8, 1/4)
+  const int t = hs[S_MSB_T] ? 810 - hs[S_MSB_T] : 0;
+  if (t > 0) ZKD_TRY(fxc_shl(tcnt, T, t, s));
+  if (t < 0) ZKD_TRY(fxc_shr(tcnt, T, -t, s));
+  // rho = Theta Theta^H  (= (Theta^H)^H Theta^H: the GEMM conjugate-transposes its left operand)
+  ZKD_TRY(conj_transpose(mL, mR, batch, T, TH, s));
+  ZKD_CUDA_TRY(cudaMemsetAsync(scal, 0, sizeof(int) * S_NUM, s));
+  ZKD_TRY(gemm_complex(mL, mL, mR, batch, side(TH, mR, mL, 812, true), side(TH, mR, mL, 812, false), rho, GemmMode::Assign, -1, opt.gemm_path,
+                       c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, scal + S_MSB_E, s));
+  ZKD_TRY(read_scalars(c, scal, S_NUM, hs));
+  if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
+  const int u = hs[S_MSB_E] ? 810 - hs[S_MSB_E] : 0;
+  if (u > 0) ZKD_TRY(fxc_shl(cnt, rho, u, s));
+  if (u < 0) ZKD_TRY(fxc_shr(cnt, rho, -u, s));
+  // the hot path: Hermitian eigendecomposition of the reduced density matrices
+  LevelStats st;
+  {
+    const int rc = solve_level(c, n, batch, rho, X, lam, 0, nullptr, &st, pm);
+    if (rc != ZKD_OK) {
+      c.ar.release(Arena::Mark{c.ar.off, 0});
+      return rc;
+    }
+  }
+  ZKD_TRY(rank_sort(n, batch, lam, rank, lam_sorted, s));
+  ZKD_TRY(phase_sorted(n, batch, X, rank, Xs, s));
+  ZKD_TRY(mps_select(n, K, batch, cutoff_bits, lam_sorted, Wt, kept_dev, s));
+  ZKD_TRY(mps_take(n, K, batch, Xs, Ln, s));
+  // R' = L'^H Theta
+  ZKD_CUDA_TRY(cudaMemsetAsync(scal, 0, sizeof(int) * S_NUM, s));
+  ZKD_TRY(gemm_complex(K, mR, mL, batch, side(Ln, mL, K, 815, true), side(T, mL, mR, 812, false), Rn, GemmMode::Assign, -1, opt.gemm_path, c.gemm_ws,
+                       c.gemm_ws_bytes, scal + S_ERR, nullptr, s));
+  ZKD_TRY(mps_scales(batch, sl, sr, sg, t, u, s_theta, s_w, s));
+  ZKD_TRY(fx_to_api_scaled((size_t)K * batch, Wt, W_api, 0, s_w, 1, (size_t)K, s, prec));
+  ZKD_TRY(fxc_to_api((size_t)n * K * batch, Ln, Lnew_api, s, prec));
+  ZKD_TRY(fxc_to_api_scaled((size_t)K * mR * batch, Rn, Rnew_api, s_theta, (size_t)K * mR, s, prec));
+  if (info) {
+    // malformed input in any of the three operands -> status 3
+    ZKD_CUDA_TRY(cudaMemsetAsync(status, 0, sizeof(int) * batch, s));
+    const int* cs = nullptr;
+    if (!st.cl_stats.empty()) {
+      ZKD_CUDA_TRY(cudaMemcpyAsync(cl_stats_dev, st.cl_stats.data(), sizeof(int) * 2 * batch, cudaMemcpyHostToDevice, s));
+      cs = cl_stats_dev;
+    }
+    info_kernel<<<(batch + 127) / 128, 128, 0, s>>>(batch, stl, st.status, st.steps, 812 - c.tol_bits, pm, cs, info);
+    count_launch();
+    ZKD_TRY(launch_check());
+  }
+  ZKD_TRY(read_scalars(c, scal, S_NUM, hs));  // synchronises (st.cl_stats must outlive the copy)
+  if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
+  return ZKD_OK;
+}
+
 }  // namespace zkd

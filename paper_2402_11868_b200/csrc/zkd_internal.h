@@ -124,6 +124,10 @@ int lu_solve_device(int N, int nrhs, int batch, int prec, const void* A_api, con
 size_t rqi_lu_workspace_bytes(int N, int batch);
 int diag_herm_rqi_lu_device(int N, int batch, int prec, const void* A_api, void* eigvals_api, void* eigvecs_api, void* ws, size_t ws_bytes,
                             zkd_info* info, cudaStream_t s);
+size_t mps_workspace_bytes(int chiL, int chiC, int chiR, int d, int batch);
+int mps_update_device(int chiL, int chiC, int chiR, int d, int batch, int prec, const void* L_api, const void* R_api, const void* G_api,
+                      int max_keep, int cutoff_bits, void* W_api, void* Lnew_api, void* Rnew_api, int* kept_dev, zkd_info* info, void* ws,
+                      size_t ws_bytes, cudaStream_t s);
 size_t svd_workspace_bytes(int M, int N, int batch);
 int svd_device(int M, int N, int batch, int prec, const void* A_api, void* S_api, void* U_api, void* V_api, void* ws, size_t ws_bytes,
                zkd_info* info, cudaStream_t s);
