@@ -219,6 +219,7 @@ static int* option_slot(const char* key) {
   if (!strcmp(key, "sstep_warp")) return &o.sstep_warp;
   if (!strcmp(key, "combine_path")) return &o.combine_path;
   if (!strcmp(key, "cluster_tiles")) return &o.cluster_tiles;
+  if (!strcmp(key, "block_correction")) return &o.block_correction;
   if (!strcmp(key, "verbose")) return &o.verbose;
   return nullptr;
 }

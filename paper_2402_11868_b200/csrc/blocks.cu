@@ -236,7 +236,34 @@ int resid_per_matrix(int n, int nb, const int32_t* R, int* msb_r_b, cudaStream_t
 }
 
 // ---- complex FX add: X += T ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) fx_add_kernel(size_t reals, int32_t* __restrict__ X, const int32_t* __restrict__ T) {
+__global__ void __launch_bounds__(256) offdiag_blocks_kernel(int n, int nb, const int* __restrict__ cl, const int32_t* __restrict__ S,
+                                                             int32_t* __restrict__ O, int* __restrict__ msb_out) {
+  const size_t per = (size_t)n * n, count = per * nb;
+  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int m = 0;
+  if (t < 2 * count) {
+    const size_t e = t % count;
+    const int b = (int)(e / per), i = (int)((e % per) / n), j = (int)(e % n);
+    int32_t d[ND];
+    fx_zero(d);
+    if (i != j && cl[(size_t)b * n + i] == cl[(size_t)b * n + j]) {
+      fx_load(d, S + (t / count) * (size_t)ND * count, count, e);
+      m = fx_msb(d);
+    }
+    fx_store(O + (t / count) * (size_t)ND * count, count, e, d);
+  }
+  for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0 && m) atomicMax(msb_out, m);
+}
+int offdiag_blocks(int n, int nb, const int* cl, const int32_t* S, int32_t* O, int* msb_out, cudaStream_t s) {
+  KtScope kt_scope(KC_OTHER, s);
+  const size_t t = 2 * (size_t)n * n * nb;
+  offdiag_blocks_kernel<<<(unsigned)((t + 255) / 256), 256, 0, s>>>(n, nb, cl, S, O, msb_out);
+  count_launch();
+  return launch_check();
+}
+
+__global__ void __launch_bounds__(256) fx_add_kernel(size_t reals, int32_t* __restrict__ X, const int32_t* __restrict__ T, int subtract) {
   const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= reals) return;
   // planes of re and im are laid out [2][ND][count]; treat as 2*count reals with plane stride `count`
@@ -247,12 +274,12 @@ __global__ void __launch_bounds__(256) fx_add_kernel(size_t reals, int32_t* __re
   int32_t a[ND], c[ND], r[ND];
   fx_load(a, xp, count, idx);
   fx_load(c, tp, count, idx);
-  fx_add(r, a, c);
+  if (subtract) fx_sub(r, a, c); else fx_add(r, a, c);
   fx_store(xp, count, idx, r);
 }
-int fxc_add_inplace(size_t count, int32_t* X, const int32_t* T, cudaStream_t s) {
+int fxc_add_inplace(size_t count, int32_t* X, const int32_t* T, cudaStream_t s, bool subtract) {
   KtScope kt_scope(KC_OTHER, s);
-  fx_add_kernel<<<(unsigned)((2 * count + 255) / 256), 256, 0, s>>>(2 * count, X, T);
+  fx_add_kernel<<<(unsigned)((2 * count + 255) / 256), 256, 0, s>>>(2 * count, X, T, subtract ? 1 : 0);
   count_launch();
   return launch_check();
 }

@@ -25,7 +25,9 @@ int resid_per_matrix(int n, int nb, const int32_t* R, int* msb_r_b, cudaStream_t
 int min_gap(int n, int nb, const int32_t* theta, const int* cl, int* gap_inv_out, cudaStream_t s);
 // cl / cle != null: singleton columns are skipped (their theta comes from the fused singleton kernel)
 int theta_from_diag(int n, int nb, const int32_t* S, int32_t* theta, cudaStream_t s, const int* cl = nullptr, const int* cle = nullptr);
-int fxc_add_inplace(size_t count, int32_t* X, const int32_t* T, cudaStream_t s);
+int fxc_add_inplace(size_t count, int32_t* X, const int32_t* T, cudaStream_t s, bool subtract = false);
+// O_ij := S_ij for i != j in the same cluster, 0 elsewhere (the off-diagonal parts of the cluster blocks of S); msb_out <- max msb
+int offdiag_blocks(int n, int nb, const int* cl, const int32_t* S, int32_t* O, int* msb_out, cudaStream_t s);
 int ecalc(int n, int nb, const int32_t* theta, const int* cl, int32_t* C, int prec_bits, int* msb_out, int* err_flag, cudaStream_t s);
 
 // finalize.cu

@@ -22,6 +22,8 @@ struct GemmShape {
   static constexpr int LOW = NQ >= 2 ? NQ - 2 : 0;
   static constexpr int NC = NP + NQ + 1 - LOW;  // kept columns LOW .. NP+NQ
   static constexpr size_t SMEM = sizeof(int32_t) * (NP + NQ) * GT * GT;
+  static constexpr int COST = NP * NQ - (LOW * (LOW + 1)) / 2;  // digit products per (i, j, k) (valid while LOW <= min(NP, NQ))
+  static constexpr int KUNROLL = COST <= 64 ? 8 : COST <= 160 ? 4 : COST <= 400 ? 2 : 1;
 };
 
 struct GemmKArgs {
@@ -62,7 +64,9 @@ __global__ void __launch_bounds__(GT * GT) gemm_digits_kernel(GemmKArgs a) {
       for (int d = 0; d < NQ; ++d) Qs[(d * GT + ty) * GT + tx] = qin ? Qg[(size_t)d * a.q_dstride + qo] : 0;
     }
     __syncthreads();
-#pragma unroll 1
+    // unrolled for the small instances: with one kk per iteration ptxas shuffles the 64-bit accumulator pairs around the back
+    // edge (~0.5 IMAD.MOV per product at <8,8>), which costs issue slots on the pipe the products need
+#pragma unroll S::KUNROLL
     for (int kk = 0; kk < GT; ++kk) {
       int32_t p[NP], q[NQ];
 #pragma unroll

@@ -121,7 +121,7 @@ Groups build_groups(const std::vector<int>& h_cl, int n, int nb) {
 // For every cluster size m > 1 the clusters of that size form one batched product over views into X, W, S (column slices
 // X_c = X[:, c0:c0+m] and diagonal blocks); singleton columns go through the fused singleton kernel.  All products carry
 // only the bits above `cut` (an absolute FX bit position chosen from the previous pass's error level).
-struct ClusterGroup { int m, nsub; const int* offX; const int* offB; };
+struct ClusterGroup { int m, nsub; const int* offX; const int* offB; const int* offR = nullptr; };  // column slice, diagonal block, row slice
 struct ClusterPlan {
   std::vector<ClusterGroup> groups;
   bool has_singletons = false;
@@ -149,6 +149,8 @@ int build_plan(Ctx& c, int n, int nb, const std::vector<int>& h_cl, int* plan_de
     for (const SubProblem& sp : kv.second) h.push_back(sp.b * n * n + sp.col0);
     g.offB = plan_dev + h.size();
     for (const SubProblem& sp : kv.second) h.push_back(sp.b * n * n + sp.col0 * n + sp.col0);
+    g.offR = plan_dev + h.size();
+    for (const SubProblem& sp : kv.second) h.push_back(sp.b * n * n + sp.col0 * n);
     plan->groups.push_back(g);
     plan->max_m = std::max(plan->max_m, g.m);
     plan->max_nsub = std::max(plan->max_nsub, g.nsub);
@@ -551,10 +553,47 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
     ZKD_TRY(gemm_complex(n, n, n, nb, side(Xc, topX, nwX, true), side(R, topR, nwR, false), Cc, GemmMode::Assign, -1, opt.gemm_path,
                          c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s));
     ZKD_TRY(ecalc(n, nb, theta, cl, Cc, pb + 8, scal + S_MSB_E, scal + S_ERR, s));
+    // Second-order treatment of the cluster blocks.  The correction solves E_dc S_c - S_d E_dc = C_dc for every pair of
+    // clusters; the division above takes S = diag(theta) only, which leaves an error of (spread of a cluster / gap) relative
+    // to E and so caps the gain of a pass at log2(gap / spread) bits once the residual is below the spread (c5: 186 bits per
+    // pass from 2^-405 on).  One fixed-point step with the off-diagonal parts O of the cluster blocks,
+    //     E <- E - (E O - O E) ./ (theta_j - theta_i),
+    // squares that factor; the two products are short (their result matters only above the cut of T) and run over the cluster
+    // views like the products of the cluster pass.
+    if (!singletons && opt.block_correction) {
+      ZKD_CUDA_TRY(cudaMemsetAsync(scal + S_MSB_T, 0, sizeof(int), s));
+      ZKD_TRY(offdiag_blocks(n, nb, cl, Sm, Gm, scal + S_MSB_T, s));
+      ZKD_TRY(read_scalars(c, scal, S_NUM, hs));
+      if (hs[S_ERR]) return ZKD_ERR_INTERNAL;
+      const int msb_o = hs[S_MSB_T];
+      const int msb_e0 = std::min(838, msb_r + (ilog2_ceil(n) + 1) / 2 + 1 + 813 - gap_msb);
+      const int nbk = msb_o ? (pb + 8) - (gap_msb - msb_o) + 12 : 0;  // bits of the correction that lie above the cut of T
+      if (nbk >= 8) {
+        const int nwk = std::min(kND, ceil_div(nbk + 2, 28) + 1);
+        const size_t cntv = (size_t)n * n * nb;
+        auto vw = [&](const int32_t* fx, int rows, int cols, int top, const int* off) {
+          GemmSide g;
+          g.fx = fx; g.rows = rows; g.cols = cols; g.top_bit = top; g.nw = nwk; g.ld = n; g.off = off; g.plane_count = cntv;
+          return g;
+        };
+        ZKD_CUDA_TRY(cudaMemsetAsync(R, 0, fxc, s));  // R is free from here to the next pass: K = E O - O E goes there
+        for (const ClusterGroup& g : plan.groups) {
+          GemmDstView dc, dr;
+          dc.ld = n; dc.off = g.offX; dc.plane_count = cntv;
+          dr.ld = n; dr.off = g.offR; dr.plane_count = cntv;
+          ZKD_TRY(gemm_complex(n, g.m, g.m, g.nsub, vw(Cc, n, g.m, msb_e0 + 2, g.offX), vw(Gm, g.m, g.m, msb_o + 2, g.offB), R, GemmMode::Add, -1,
+                               opt.gemm_path, c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s, &dc));
+          ZKD_TRY(gemm_complex(g.m, n, g.m, g.nsub, vw(Gm, g.m, g.m, msb_o + 2, g.offB), vw(Cc, g.m, n, msb_e0 + 2, g.offR), R, GemmMode::Sub, -1,
+                               opt.gemm_path, c.gemm_ws, c.gemm_ws_bytes, scal + S_ERR, nullptr, s, &dr));
+        }
+        ZKD_TRY(ecalc(n, nb, theta, cl, R, nbk + 8, nullptr, scal + S_ERR, s));
+        ZKD_TRY(fxc_add_inplace(cnt, Cc, R, s, true));
+      }
+    }
     // No host read of msb(E): a rigorous bound sizes the windows instead.  |C_ij| = |x_i^H r_j| <= |x_i| |r_j| <= sqrt(n) max|R|
     // (columns are normalised), and |theta_j - theta_i| >= the smallest gap between neighbouring clusters, which the same
     // read as msb(R) delivered.  The bound is a few bits loose; the E / T windows get those bits back (pbE).
-    const int msb_e = std::min(838, msb_r + (ilog2_ceil(n) + 1) / 2 + 1 + 813 - gap_msb);
+    const int msb_e = std::min(838, msb_r + (ilog2_ceil(n) + 1) / 2 + 1 + 813 - gap_msb + ((!singletons && opt.block_correction) ? 1 : 0));
     const int pbE = pb + 8;
     // S4e: T = X E (bits below cutT cleared so that W += A T tracks A X exactly), X += T, W += A T
     const int topE = msb_e + 2, nwE = ceil_div(pbE + 2, 28);

@@ -746,7 +746,9 @@ int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int ma
       while (csize > 1 && (long)batch * csize > 2L * sms) csize /= 2;
       while ((P + csize - 1) / csize > maxw) csize *= 2;
       int rc;
-      if (csize == 1 && N <= 96 && options().seed_path != 2) {
+      // a whole matrix in one CTA: batches (one SM per matrix), and single tiny matrices, where a round of 8 pairs is cheaper behind
+      // __syncthreads than behind a cluster barrier (measured: N = 16 0.109 -> 0.083 ms; N = 64 is 2.3 x slower that way)
+      if ((csize == 1 || N <= 24 || options().seed_path == 5) && N <= 96 && options().seed_path != 2) {
         // a whole matrix per SM: plain CTA kernel (__syncthreads instead of cluster barriers)
         if (N <= 32) rc = launch_cta<1>(N, batch, A, mu, Vv, max_sweeps, tol2, s);
         else if (N <= 64) rc = launch_cta<2>(N, batch, A, mu, Vv, max_sweeps, tol2, s);
