@@ -461,6 +461,23 @@ def main():
                 torch.cuda.empty_cache()
             except Exception as e:  # context only; never fails the bench line
                 extra[f"{nm}x{bb}"] = {"error": str(e)[:200]}
+        # the paper's route taken literally on the same GPU (S4a': exact RQI, one multiprecision LU per eigenpair and iteration)
+        for nm in ("c1", "c2"):
+            try:
+                n2, b2, A2 = make_workload(nm, 0)
+                r2 = Runner(z, n2, b2, A2)
+                ws2 = torch.empty(z.diag_herm_rqi_lu_bufsize(n2, b2), dtype=torch.uint8, device="cuda")
+                step2 = lambda: z.diag_herm_rqi_lu(n2, b2, r2.A, r2.lam, r2.X, ws2, r2.info)
+                step2()
+                torch.cuda.synchronize()
+                ts0 = timed_steps(torch, step2, 3, flush)
+                ms = sum(ts0) / len(ts0)
+                extra[f"{nm}x1@exact_rqi_lu"] = {"matrices_per_s": b2 / (ms * 1e-3), "ms_per_step": ms,
+                                                 "note": "zkd_diag_herm_rqi_lu: fp64 seed + exact RQI by LU (PAPER.md:33 route), cross-check path"}
+                del r2, ws2
+                torch.cuda.empty_cache()
+            except Exception as e:
+                extra[f"{nm}x1@exact_rqi_lu"] = {"error": str(e)[:200]}
         line["other_configs"] = extra
 
     if not args.no_cpu_baseline:

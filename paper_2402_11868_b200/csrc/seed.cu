@@ -590,13 +590,35 @@ __device__ __forceinline__ double rotate_pair_smem(double2* __restrict__ gp, dou
   return cos2;
 }
 
+// 1-D bulk copies of whole columns between global memory (L2) and shared memory through the TMA engine (cp.async.bulk): one
+// elected thread issues 2 W copies of 16 n bytes, all in flight at once, instead of every thread walking the columns with 16-byte
+// loads (a handful of dependent L2 round trips per thread).
+__device__ __forceinline__ uint32_t seed_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void seed_mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "SW_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra SD_%=;\n\t"
+      "bra SW_%=;\n\t"
+      "SD_%=:\n\t}" ::"r"(seed_smem_u32(bar)), "r"(parity)
+      : "memory");
+}
+
 template <int W, int NWARPS>
 __global__ void __launch_bounds__(32 * NWARPS) seed_block_kernel(int n, const double2* __restrict__ A, double2* __restrict__ G,
                                                          const double* __restrict__ sigma_p, int* __restrict__ rot_flags,
-                                                         double* __restrict__ mu_unsorted, int max_sweeps, double tol2) {
+                                                         double* __restrict__ mu_unsorted, int max_sweeps, double tol2, int use_tma) {
   extern __shared__ double2 s_cols[];  // [2 W][n]
   constexpr int WPP = NWARPS / W;      // warps per pair: all warps of the CTA rotate in every sub-round
   __shared__ double s_red[W][4 * WPP];
+  __shared__ __align__(8) uint64_t s_bar;
+  uint32_t bar_phase = 0;
+  if (threadIdx.x == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(seed_smem_u32(&s_bar)), "r"(1));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
   cg::grid_group grid = cg::this_grid();
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int pr = warp % W, part = warp / W;
@@ -623,7 +645,30 @@ __global__ void __launch_bounds__(32 * NWARPS) seed_block_kernel(int n, const do
           rr_pair(MB, r, pi, bp, bq);
           // load (absent columns, beyond n or in the padding block, are zero: rot_params leaves zero columns alone);
           // one flat loop over the 2 W columns, unrolled, so that many independent L2 loads are in flight per thread
-          {
+          if (use_tma) {
+            int present = 0;
+            for (int c = 0; c < 2 * W; ++c) {
+              const int col = (c < W ? bp : bq) * W + (c % W);
+              if (col < n) ++present;
+              else
+                for (int i = tid; i < n; i += 32 * NWARPS) s_cols[(size_t)c * n + i] = make_double2(0.0, 0.0);
+            }
+            if (tid == 0) {
+              const uint32_t colb = (uint32_t)n * (uint32_t)sizeof(double2);
+              asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(seed_smem_u32(&s_bar)), "r"(colb * (uint32_t)present)
+                           : "memory");
+              for (int c = 0; c < 2 * W; ++c) {
+                const int col = (c < W ? bp : bq) * W + (c % W);
+                if (col < n)
+                  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                                   seed_smem_u32(s_cols + (size_t)c * n)),
+                               "l"(G + (size_t)col * n), "r"(colb), "r"(seed_smem_u32(&s_bar))
+                               : "memory");
+              }
+            }
+            seed_mbar_wait(&s_bar, bar_phase);
+            bar_phase ^= 1;
+          } else {
             const int tot = 2 * W * n;
 #pragma unroll 8
             for (int e = tid; e < tot; e += 32 * NWARPS) {
@@ -649,7 +694,24 @@ __global__ void __launch_bounds__(32 * NWARPS) seed_block_kernel(int n, const do
             cmax = fmax(cmax, rotate_pair_smem<WPP>(s_cols + (size_t)p * n, s_cols + (size_t)q * n, n, lane, part, s_red[pr], tol2, nchk, nrot));
             __syncthreads();
           }
-          {
+          if (use_tma) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // the rotated columns (generic-proxy writes) to the TMA engine
+            __syncthreads();
+            if (tid == 0) {
+              const uint32_t colb = (uint32_t)n * (uint32_t)sizeof(double2);
+              for (int c = 0; c < 2 * W; ++c) {
+                const int col = (c < W ? bp : bq) * W + (c % W);
+                if (col < n)
+                  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(G + (size_t)col * n),
+                               "r"(seed_smem_u32(s_cols + (size_t)c * n)), "r"(colb)
+                               : "memory");
+              }
+              asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+              asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");  // complete: the grid barrier below publishes the columns
+              asm volatile("fence.proxy.async.global;" ::: "memory");
+              __threadfence();
+            }
+          } else {
             const int tot = 2 * W * n;
 #pragma unroll 8
             for (int e = tid; e < tot; e += 32 * NWARPS) {
@@ -661,7 +723,7 @@ __global__ void __launch_bounds__(32 * NWARPS) seed_block_kernel(int n, const do
           __syncthreads();
         }
         if (r == MB - 2 && cmax > kSeedStopCos2 && lane == 0) rot_flags[sweep] = 1;
-        grid.sync();
+        grid.sync();  // (a hand-written atomic-counter barrier measured no faster: 48.0 vs 46.4 ms per N = 1024 seed)
       }
       if (!rot_flags[sweep]) break;
     }
@@ -691,7 +753,8 @@ static int launch_block(int n, int sms, const double2* Ab, double2* G, double* s
   const int NB = (n + W - 1) / W, MB = NB + (NB & 1);
   int nblocks = MB / 2;
   if (nblocks > maxb * sms) nblocks = maxb * sms;
-  void* args[] = {&n, (void*)&Ab, &G, &sigma, &flags, &mu_uns, &ms, &t2};
+  int use_tma = options().seed_tma ? 1 : 0;
+  void* args[] = {&n, (void*)&Ab, &G, &sigma, &flags, &mu_uns, &ms, &t2, &use_tma};
   if (cudaLaunchCooperativeKernel((void*)seed_block_kernel<W, NWARPS>, dim3(nblocks), dim3(32 * NWARPS), args, smem, s) != cudaSuccess) {
     (void)cudaGetLastError();
     return ZKD_ERR_CUDA;
@@ -771,7 +834,7 @@ int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int ma
   if (nblocks > maxb * sms) nblocks = maxb * sms;
   char* buf = nullptr;
   const size_t nn = (size_t)N * N;
-  const size_t bytes = sizeof(double2) * nn + sizeof(double) * (N + 8) + sizeof(int) * 64;
+  const size_t bytes = sizeof(double2) * nn + sizeof(double) * (N + 8) + sizeof(int) * 128;
   // grow-only scratch of the calling thread (N^2 double2: 16 MB at N = 1024): a stream-ordered allocation here costs a pool
   // re-growth after every synchronisation of the caller (the default pool trims at sync points)
   {
