@@ -317,49 +317,49 @@ __device__ __forceinline__ bool fx_less(const int32_t (&a)[ND], const int32_t (&
   return lt;
 }
 
-// rank[j] = number of eigenvalues that sort before lambda_j (ascending, stable); also writes lambda sorted
+// rank[j] = number of eigenvalues that sort before lambda_j (ascending, stable); also writes lambda sorted.
+// One WARP per eigenvalue: the lanes share the N comparisons (a thread per eigenvalue is a chain of N dependent 3-digit loads on
+// a few hundred threads: 25 us at N = 16, 150 us at N = 256).
 __global__ void __launch_bounds__(128) rank_kernel(int N, int batch, const int32_t* __restrict__ lam, int* __restrict__ rank,
                                                    int32_t* __restrict__ lam_sorted) {
-  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= (size_t)N * batch) return;
+  const size_t t = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (t >= (size_t)N * batch) return;  // the whole warp leaves together
   const int b = (int)(t / N), j = (int)(t % N);
   const size_t cnt = (size_t)N * batch;
   int32_t lj[ND];
   fx_load(lj, lam, cnt, t);
   int r = 0;
-  // The top three digits (integer part and 56 fractional bits) decide almost every comparison: fetch them for four
-  // candidates at a time (independent loads), and walk the remaining digits only on a tie.
+  // The top three digits (integer part and 56 fractional bits) decide almost every comparison; the remaining digits are walked
+  // only on a tie.
   const int32_t* base = lam + (size_t)b * N;
-  for (int i0 = 0; i0 < N; i0 += 4) {
-    int32_t d2[4], d1[4], d0[4];
+  for (int i = lane; i < N; i += 32) {
+    const int32_t d2 = base[(size_t)(ND - 1) * cnt + i], d1 = base[(size_t)(ND - 2) * cnt + i], d0 = base[(size_t)(ND - 3) * cnt + i];
+    int cmp = d2 < lj[ND - 1] ? -1 : d2 > lj[ND - 1] ? 1 : 0;  // sign of (lambda_i - lambda_j)
+    if (cmp == 0) cmp = d1 < lj[ND - 2] ? -1 : d1 > lj[ND - 2] ? 1 : 0;
+    if (cmp == 0) cmp = d0 < lj[ND - 3] ? -1 : d0 > lj[ND - 3] ? 1 : 0;
+    if (cmp == 0) {
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const int i = i0 + u < N ? i0 + u : N - 1;
-      d2[u] = base[(size_t)(ND - 1) * cnt + i];
-      d1[u] = base[(size_t)(ND - 2) * cnt + i];
-      d0[u] = base[(size_t)(ND - 3) * cnt + i];
-    }
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const int i = i0 + u;
-      if (i >= N) continue;
-      int cmp = d2[u] < lj[ND - 1] ? -1 : d2[u] > lj[ND - 1] ? 1 : 0;  // sign of (lambda_i - lambda_j)
-      if (cmp == 0) cmp = d1[u] < lj[ND - 2] ? -1 : d1[u] > lj[ND - 2] ? 1 : 0;
-      if (cmp == 0) cmp = d0[u] < lj[ND - 3] ? -1 : d0[u] > lj[ND - 3] ? 1 : 0;
-      if (cmp == 0) {
-#pragma unroll
-        for (int k = ND - 4; k >= 0; --k) {
-          if (cmp == 0) {
-            const int32_t d = base[(size_t)k * cnt + i];
-            cmp = d < lj[k] ? -1 : d > lj[k] ? 1 : 0;
-          }
+      for (int k = ND - 4; k >= 0; --k) {
+        if (cmp == 0) {
+          const int32_t d = base[(size_t)k * cnt + i];
+          cmp = d < lj[k] ? -1 : d > lj[k] ? 1 : 0;
         }
       }
-      r += cmp < 0 || (cmp == 0 && i < j);
     }
+    r += cmp < 0 || (cmp == 0 && i < j);
   }
-  rank[t] = r;
-  fx_store(lam_sorted, cnt, (size_t)b * N + r, lj);
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) r += __shfl_xor_sync(0xffffffffu, r, off);
+  if (lane == 0) rank[t] = r;
+  // every lane holds lambda_j: lane k stores digit k
+  if (lane < ND) {
+    int32_t v = 0;
+#pragma unroll
+    for (int k = 0; k < ND; ++k)
+      if (k == lane) v = lj[k];
+    lam_sorted[(size_t)lane * cnt + (size_t)b * N + r] = v;
+  }
 }
 
 // one warp per column: k* = first index of max |x_k|^2 (exact FX comparison), u = conj(x_k*) / |x_k*|,
@@ -455,7 +455,7 @@ __global__ void __launch_bounds__(128) phase_kernel(int N, int batch, const int3
 int rank_sort(int N, int batch, const int32_t* lam, int* rank, int32_t* lam_sorted, cudaStream_t s) {
   KtScope kt_scope(KC_OTHER, s);
   const size_t nl = (size_t)N * batch;
-  rank_kernel<<<(unsigned)((nl + 127) / 128), 128, 0, s>>>(N, batch, lam, rank, lam_sorted);
+  rank_kernel<<<(unsigned)((nl * 32 + 127) / 128), 128, 0, s>>>(N, batch, lam, rank, lam_sorted);
   count_launch();
   return launch_check();
 }
@@ -472,7 +472,7 @@ int finalize_export(int N, int batch, const int32_t* X, const int32_t* lam, cons
                     int32_t* scratch, int32_t* lam_sorted, int* rank, cudaStream_t s, int prec) {
   KtScope kt_scope(KC_IO, s);
   const size_t nl = (size_t)N * batch;
-  rank_kernel<<<(unsigned)((nl + 127) / 128), 128, 0, s>>>(N, batch, lam, rank, lam_sorted);
+  rank_kernel<<<(unsigned)((nl * 32 + 127) / 128), 128, 0, s>>>(N, batch, lam, rank, lam_sorted);
   phase_kernel<<<(unsigned)((nl * 32 + 127) / 128), 128, 0, s>>>(N, batch, X, rank, scratch);
   count_launch(2);
   ZKD_TRY(launch_check());
