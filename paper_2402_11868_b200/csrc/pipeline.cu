@@ -568,7 +568,9 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
       const int msb_o = hs[S_MSB_T];
       const int msb_e0 = std::min(838, msb_r + (ilog2_ceil(n) + 1) / 2 + 1 + 813 - gap_msb);
       const int nbk = msb_o ? (pb + 8) - (gap_msb - msb_o) + 12 : 0;  // bits of the correction that lie above the cut of T
-      if (nbk >= 8) {
+      // worth it only when the fixed-point step converges fast (spread / gap <= 2^-24: a cluster with structure near its gap, like c4's
+      // 29-dimensional one before S4h has split it, gains a bit per step at the price of two products) and when the cap binds (nbk)
+      if (nbk >= 8 && gap_msb - msb_o >= 24) {
         const int nwk = std::min(kND, ceil_div(nbk + 2, 28) + 1);
         const size_t cntv = (size_t)n * n * nb;
         auto vw = [&](const int32_t* fx, int rows, int cols, int top, const int* off) {
