@@ -174,7 +174,8 @@ int zkd_mps_two_site_update(int chiL, int chiC, int chiR, int d, int batch, int 
  * the IMAD engine; 2: tiles wherever they can be formed),
  * "block_correction" (default 1: the correction between clusters takes
  * one fixed-point step with the off-diagonal parts of the cluster blocks of X^H A X, which squares the spread / gap factor
- * that otherwise caps the gain of a pass), "seed_tma" (default 1: the blocked fp64 seed moves its columns by TMA bulk copies),
+ * that otherwise caps the gain of a pass), "seed_ring_block" (columns per block of the block-ring fp64 seed for N <= 256:
+ * 2 or 4, 0 = the column ring, default -1 = 4 from N = 96 on), "seed_tma" (default 1: the blocked fp64 seed moves its columns by TMA bulk copies),
  * "seed_block_warps" (8 or 16), "combine_path" (epilogue of the IMAD GEMM: 0 automatic,
  * 1 digit-serial, 2 warp-cooperative), "sstep_cpb" (matrix columns per CTA of the fused singleton step, 0 automatic), "sstep_warp" (1: its
  * warp-per-element variant for N <= 64, default 0), "sstep_cache" (shared-memory staging of the column, default 1),

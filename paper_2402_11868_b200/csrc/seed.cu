@@ -320,6 +320,284 @@ static int launch_ring(int N, int batch, int csize, const double2* A, double* mu
   return launch_check();
 }
 
+// ---- n <= 256, BLOCK ring: a processor = W warps holds two blocks of W columns ------------------------------------------------------
+// Same Brent-Luk ring, but over blocks of W columns: per ring step a processor rotates all W^2 cross pairs of its two blocks in W
+// sub-steps of W disjoint pairs (one warp each, in place in its own shared-memory slots, a named barrier of the processor's W warps
+// between sub-steps) and only then hands the blocks on: (n / W - 1) cluster barriers and DSMEM hand-overs per sweep instead of (n - 1).
+// The pairs inside a block meet once per sweep, in step 0.  Blocks keep their columns for the whole run.
+__device__ __forceinline__ void proc_barrier(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+
+template <int EPL>
+__device__ __forceinline__ void ring_load(double2 (&a)[EPL], const double2* __restrict__ col, int n, int lane) {
+#pragma unroll
+  for (int q = 0; q < EPL; ++q) {
+    const int i = lane + 32 * q;
+    a[q] = i < n ? col[i] : make_double2(0, 0);
+  }
+}
+template <int EPL>
+__device__ __forceinline__ void ring_store(double2* __restrict__ col, const double2 (&a)[EPL], int n, int lane) {
+#pragma unroll
+  for (int q = 0; q < EPL; ++q) {
+    const int i = lane + 32 * q;
+    if (i < n) col[i] = a[q];
+  }
+}
+// orthogonalise the register-held columns a, bb; returns |cos|^2 before the rotation (0 when skipped)
+template <int EPL>
+__device__ __forceinline__ double ring_rotate(double2 (&a)[EPL], double2 (&bb)[EPL], double tol2, bool& rotated) {
+  double al = 0, be = 0, gr = 0, gi = 0;
+#pragma unroll
+  for (int q = 0; q < EPL; ++q) {
+    al = fma(a[q].x, a[q].x, fma(a[q].y, a[q].y, al));
+    be = fma(bb[q].x, bb[q].x, fma(bb[q].y, bb[q].y, be));
+    gr = fma(a[q].x, bb[q].x, fma(a[q].y, bb[q].y, gr));
+    gi = fma(a[q].x, bb[q].y, fma(-a[q].y, bb[q].x, gi));
+  }
+  al = warp_sum(al); be = warp_sum(be); gr = warp_sum(gr); gi = warp_sum(gi);
+  double c, sr, si, cos2;
+  rotated = rot_params(al, be, gr, gi, tol2, c, sr, si, cos2);
+  if (rotated) {
+#pragma unroll
+    for (int q = 0; q < EPL; ++q) {
+      const double2 x = a[q], y = bb[q];
+      a[q] = make_double2(c * x.x - (sr * y.x + si * y.y), c * x.y - (sr * y.y - si * y.x));
+      bb[q] = make_double2(sr * x.x - si * x.y + c * y.x, sr * x.y + si * x.x + c * y.y);
+    }
+  }
+  return cos2;
+}
+
+constexpr int kRingbMaxProc = 8;   // processors per CTA
+constexpr int kRingbMaxCols = 288;  // columns incl. padding
+
+template <int EPL, int W>
+__global__ void __launch_bounds__(512)
+seed_ringb_kernel(int n, int ppc, const double2* __restrict__ A, double* __restrict__ mu, double2* __restrict__ V, int max_sweeps, double tol2) {
+  extern __shared__ double2 slots[];                 // [2 sets][ppc][2 blocks][W][n]
+  __shared__ int s_id2[2][kRingbMaxProc][2][W];      // column ids held by the local slots (per set)
+  __shared__ double s_mu[kRingbMaxCols];             // by position (2k + which) W + w (every CTA holds a full copy)
+  __shared__ int s_pid[kRingbMaxCols];
+  __shared__ unsigned long long s_cmax[2];
+  __shared__ double s_rmax;
+  __shared__ double s_red[32];
+  cg::cluster_group cluster = cg::this_cluster();
+  const int csize = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
+  const int b = blockIdx.x / csize;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int pl = warp / W, w = warp % W;             // local processor, warp inside the processor
+  const double2* Ab = A + (size_t)b * n * n;
+  const int NBk = (n + W - 1) / W, MB = NBk + (NBk & 1), P = MB / 2;  // blocks (even), processors
+  const int k = rank * ppc + pl;                     // global processor
+  const bool act = k < P;
+  const size_t blk = (size_t)W * n;                  // double2 elements of a block
+  const size_t bufstride = (size_t)ppc * 2 * blk;    // between the two slot sets
+  double2* my_top = slots + (size_t)(pl * 2 + 0) * blk;
+  double2* my_bot = slots + (size_t)(pl * 2 + 1) * blk;
+  int cur = 0;
+
+  // own columns: warp w of processor k loads column w of both blocks (ids (2k) W + w and (2k + 1) W + w); Gershgorin radius
+  double rmax = 0;
+  if (act) {
+    for (int which = 0; which < 2; ++which) {
+      const int j = (2 * k + which) * W + w;
+      double2* g = (which ? my_bot : my_top) + (size_t)w * n;
+      double rs = 0;
+      for (int i = lane; i < n; i += 32) {
+        double2 a = make_double2(0, 0);
+        if (j < n) {
+          a = (i <= j) ? Ab[(size_t)i * n + j] : Ab[(size_t)j * n + i];
+          if (i > j) a.y = -a.y;
+          if (i == j) a.y = 0;
+        }
+        g[i] = a;
+        rs += (i == j) ? fabs(a.x) : sqrt(a.x * a.x + a.y * a.y);
+      }
+      rmax = fmax(rmax, warp_sum(rs));
+      if (lane == 0) s_id2[0][pl][which][w] = j;
+    }
+  }
+  if (lane == 0) s_red[warp] = rmax;
+  if (tid == 0) { s_cmax[0] = 0ull; s_cmax[1] = 0ull; }
+  __syncthreads();
+  if (tid == 0) {
+    double m = 0;
+    for (int x = 0; x < (int)(blockDim.x >> 5); ++x) m = fmax(m, s_red[x]);
+    s_rmax = m;
+  }
+  cluster.sync();
+  double sigma = 0;
+  for (int r = 0; r < csize; ++r) sigma = fmax(sigma, *cluster.map_shared_rank(&s_rmax, r));
+  sigma *= 1.5;
+  if (act && lane == 0) {
+    const int jt = (2 * k) * W + w, jb = (2 * k + 1) * W + w;
+    if (jt < n) my_top[(size_t)w * n + jt].x += sigma;
+    if (jb < n) my_bot[(size_t)w * n + jb].x += sigma;
+  }
+  // destinations of this processor's blocks (fixed for the whole run), set 0 addresses
+  double2* dst_top = my_top;
+  double2* dst_bot = my_bot;
+  int* dst_top_id = &s_id2[0][pl][0][0];
+  int* dst_bot_id = &s_id2[0][pl][1][0];
+  if (act && P > 1) {
+    auto slot_of = [&](int kk, int which) -> double2* {
+      double2* local = slots + (size_t)((kk % ppc) * 2 + which) * blk;
+      return (kk / ppc == rank) ? local : cluster.map_shared_rank(local, kk / ppc);
+    };
+    auto id_of = [&](int kk, int which) -> int* {
+      int* local = &s_id2[0][kk % ppc][which][0];
+      return (kk / ppc == rank) ? local : cluster.map_shared_rank(local, kk / ppc);
+    };
+    if (k == 0) { dst_bot = slot_of(1, 0); dst_bot_id = id_of(1, 0); }
+    else {
+      if (k < P - 1) { dst_top = slot_of(k + 1, 0); dst_top_id = id_of(k + 1, 0); }
+      else { dst_top = my_bot; dst_top_id = &s_id2[0][pl][1][0]; }
+      dst_bot = slot_of(k - 1, 1); dst_bot_id = id_of(k - 1, 1);
+    }
+  }
+  constexpr int kIdSet = kRingbMaxProc * 2 * W;      // ints between the two id sets
+  cluster.sync();
+
+  unsigned long long nchk = 0, nrot = 0;
+  if (n > 1 && sigma > 0) {
+    for (int sweep = 0; sweep < max_sweeps; ++sweep) {
+      double cmax = 0;
+      for (int r = 0; r < MB - 1; ++r) {
+        const int nxt = cur ^ 1;
+        if (act) {
+          double2* T = my_top + (size_t)cur * bufstride;
+          double2* B = my_bot + (size_t)cur * bufstride;
+          double2 a[EPL], bb[EPL];
+          bool rot;
+          if (r == 0 && W > 1) {
+            // pairs inside each block, once per sweep: round-robin over W columns, W / 2 pairs per block and sub-step
+            for (int t = 0; t < W - 1; ++t) {
+              const int which = w / (W / 2), i = w % (W / 2);
+              int p, q;
+              rr_pair(W, t, i, p, q);
+              double2* X = which ? B : T;
+              ring_load<EPL>(a, X + (size_t)p * n, n, lane);
+              ring_load<EPL>(bb, X + (size_t)q * n, n, lane);
+              cmax = fmax(cmax, ring_rotate<EPL>(a, bb, tol2, rot));
+              nchk += n;
+              if (rot) {
+                nrot += n;
+                ring_store<EPL>(X + (size_t)p * n, a, n, lane);
+                ring_store<EPL>(X + (size_t)q * n, bb, n, lane);
+              }
+              proc_barrier(1 + pl, 32 * W);
+            }
+          }
+          const int ida = s_id2[cur][pl][0][w];
+          ring_load<EPL>(a, T + (size_t)w * n, n, lane);  // column w of the top block stays in this warp's registers
+          for (int t = 0; t < W; ++t) {
+            const int q = (w + t) % W;
+            ring_load<EPL>(bb, B + (size_t)q * n, n, lane);
+            cmax = fmax(cmax, ring_rotate<EPL>(a, bb, tol2, rot));
+            nchk += n;
+            if (rot) nrot += n;
+            if (t < W - 1) {
+              if (rot) ring_store<EPL>(B + (size_t)q * n, bb, n, lane);
+              proc_barrier(1 + pl, 32 * W);
+            } else {
+              // last sub-step: straight into the slots where the blocks are needed next (set nxt of the neighbours)
+              const int idb = s_id2[cur][pl][1][q];
+              ring_store<EPL>(dst_top + (size_t)nxt * bufstride + (size_t)w * n, a, n, lane);
+              ring_store<EPL>(dst_bot + (size_t)nxt * bufstride + (size_t)q * n, bb, n, lane);
+              if (lane == 0) { dst_top_id[nxt * kIdSet + w] = ida; dst_bot_id[nxt * kIdSet + q] = idb; }
+            }
+          }
+        }
+        cur = nxt;
+        if (r == MB - 2 && lane == 0 && cmax > 0) atomicMax(&s_cmax[sweep & 1], (unsigned long long)__double_as_longlong(cmax));
+        cluster_arrive();
+        cluster_wait();
+      }
+      double worst = 0;
+      for (int r = 0; r < csize; ++r)
+        worst = fmax(worst, __longlong_as_double((long long)*cluster.map_shared_rank(&s_cmax[sweep & 1], r)));
+      if (tid == 0) s_cmax[(sweep + 1) & 1] = 0ull;
+      __syncthreads();
+      if (!(worst > kSeedStopCos2)) break;
+    }
+    if (lane == 0) seed_count(nchk, nrot);
+  }
+  cluster.sync();
+  my_top += (size_t)cur * bufstride;
+  my_bot += (size_t)cur * bufstride;
+
+  // mu = ||g|| - sigma per position, broadcast to every CTA; normalise in place
+  if (act) {
+    for (int which = 0; which < 2; ++which) {
+      double2* g = (which ? my_bot : my_top) + (size_t)w * n;
+      double sq = 0;
+      for (int i = lane; i < n; i += 32) { const double2 x = g[i]; sq += x.x * x.x + x.y * x.y; }
+      sq = warp_sum(sq);
+      const double nrm = sqrt(sq);
+      const double inv = nrm > 0 ? 1.0 / nrm : 0.0;
+      const int id = s_id2[cur][pl][which][w];
+      for (int i = lane; i < n; i += 32) {
+        double2 x = g[i];
+        if (nrm > 0) { x.x *= inv; x.y *= inv; } else { x = make_double2(i == id ? 1.0 : 0.0, 0.0); }
+        g[i] = x;
+      }
+      const int pos = (2 * k + which) * W + w;
+      if (lane < csize) {
+        *cluster.map_shared_rank(&s_mu[pos], lane) = nrm - sigma;
+        *cluster.map_shared_rank(&s_pid[pos], lane) = id;
+      }
+    }
+  }
+  cluster.sync();
+  if (act) {
+    const int Mc = MB * W;
+    for (int which = 0; which < 2; ++which) {
+      const int pos = (2 * k + which) * W + w;
+      const int id = s_pid[pos];
+      if (id >= n) continue;  // a padding column
+      const double mj = s_mu[pos];
+      int rk = 0;
+      for (int i = lane; i < Mc; i += 32) {
+        const double mi = s_mu[i];
+        const int idi = s_pid[i];
+        rk += (idi < n) && ((mi < mj) || (mi == mj && idi < id));
+      }
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) rk += __shfl_xor_sync(0xffffffffu, rk, off);
+      if (lane == 0) mu[(size_t)b * n + rk] = mj;
+      const double2* g = (which ? my_bot : my_top) + (size_t)w * n;
+      for (int i = lane; i < n; i += 32) V[(size_t)b * n * n + (size_t)i * n + rk] = g[i];
+    }
+  }
+  cluster.sync();
+}
+
+template <int EPL, int W>
+static int launch_ringb(int N, int batch, int csize, int ppc, const double2* A, double* mu, double2* V, int max_sweeps, double tol2,
+                        cudaStream_t s) {
+  const size_t smem = sizeof(double2) * 2 * (size_t)ppc * 2 * W * N;
+  if (smem > 48 * 1024) ZKD_CUDA_TRY(cudaFuncSetAttribute(seed_ringb_kernel<EPL, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  if (csize > 8) ZKD_CUDA_TRY(cudaFuncSetAttribute(seed_ringb_kernel<EPL, W>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(batch * csize));
+  cfg.blockDim = dim3((unsigned)(32 * W * ppc));
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = (unsigned)csize;
+  at[0].val.clusterDim.y = 1;
+  at[0].val.clusterDim.z = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  {
+    KtScope kt(KC_SEED, s);
+    ZKD_CUDA_TRY(cudaLaunchKernelEx(&cfg, seed_ringb_kernel<EPL, W>, N, ppc, A, mu, V, max_sweeps, tol2));
+  }
+  count_launch();
+  return launch_check();
+}
+
 // ---- n <= 96: one CTA per matrix, G in this CTA's shared memory -----------------------------------------------------------
 // One warp per pair of a round (npairs <= 48 warps would not fit, so a warp takes ceil(npairs / nwarps) pairs), one
 // __syncthreads per round: no cluster barrier and no DSMEM latency on the critical path, and a batch uses one SM per matrix.
@@ -802,6 +1080,35 @@ int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int ma
     const double2* A = (const double2*)A64;
     double2* Vv = (double2*)V;
     static int max_cluster = 16;
+    // block ring (W columns per block): whenever its slots fit and the batch leaves room for one cluster per matrix
+    // measured (N: column ring / W = 2 / W = 4, ms): 64: 0.50 / 0.64 / 0.57; 100: 1.54 / 1.38 / 1.19; 128: 2.00 / 1.88 / 1.51;
+    // 256: 4.11 / 3.69 / 3.34 - a rotation's own dependent chain (load, dot, reduce, parameters, update, store: ~1.3 us) bounds both
+    const int Wb = options().seed_ring_block < 0 ? (N >= 96 ? 4 : 0) : options().seed_ring_block;
+    if ((Wb == 2 || Wb == 4) && N > 2 * Wb && options().seed_path != 2 && options().seed_path != 5 && N > 24) {
+      const int NBk = (N + Wb - 1) / Wb, MB = NBk + (NBk & 1), Pb = MB / 2;
+      const int ppc_max = std::min(std::min(16 / Wb, kRingbMaxProc), (int)(200 * 1024 / (64 * (size_t)Wb * N)));
+      if (ppc_max >= 1) {
+        int csize = 1;
+        while (csize < 16 && (Pb + csize - 1) / csize > ppc_max) csize *= 2;
+        const int ppc = (Pb + csize - 1) / csize;
+        if (ppc <= ppc_max && csize <= max_cluster && (long)batch * csize <= 2L * sms) {
+          int rc;
+          if (Wb == 2) {
+            if (N <= 32) rc = launch_ringb<1, 2>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, s);
+            else if (N <= 64) rc = launch_ringb<2, 2>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, s);
+            else if (N <= 128) rc = launch_ringb<4, 2>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, s);
+            else rc = launch_ringb<8, 2>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, s);
+          } else {
+            if (N <= 32) rc = launch_ringb<1, 4>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, s);
+            else if (N <= 64) rc = launch_ringb<2, 4>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, s);
+            else if (N <= 128) rc = launch_ringb<4, 4>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, s);
+            else rc = launch_ringb<8, 4>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, s);
+          }
+          if (!(rc == ZKD_ERR_CUDA && csize > 8)) return rc;
+          max_cluster = 8;  // a cluster of 16 was refused: the column ring below copes with 8
+        }
+      }
+    }
     const int want = options().seed_cluster > 0 ? options().seed_cluster : max_cluster;
     for (;;) {
       int csize = 1;

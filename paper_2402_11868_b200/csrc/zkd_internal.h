@@ -45,6 +45,7 @@ struct Options {
   int min_split_ctas = 296;  // split K until a product has about this many CTAs (two per SM), see pick_splits
   int seed_sweeps = 12;
   int seed_cluster = 0;  // ring seed: largest cluster size to use (0 = 16, falling back to 8 when refused)
+  int seed_ring_block = -1;   // ring seed (N <= 256): columns per block of the block ring (2 or 4); 0: the column ring; -1: 4 for N >= 96
   int seed_tma = 1;           // blocked seed: columns move between L2 and shared memory by 1-D TMA bulk copies
   int seed_block_warps = 8;   // blocked seed (N > 256): warps per CTA (8 or 16)
   int seed_dbuf = 1;     // ring seed: two slot sets, one cluster barrier per round (when they fit shared memory)
