@@ -50,6 +50,9 @@ def lib():
         L.zkd_oracle_svd_compare.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, vp, vp, vp, vp, vp, vp, vp]
         L.zkd_oracle_lu_solve.restype = ctypes.c_int
         L.zkd_oracle_lu_solve.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, vp, vp]
+        L.zkd_oracle_rqi.restype = ctypes.c_int
+        L.zkd_oracle_rqi.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                     ctypes.c_int, ctypes.c_int, vp, vp]
         L.zkd_oracle_api_to_double.restype = ctypes.c_double
         L.zkd_oracle_api_to_double.argtypes = [vp, ctypes.c_int]
         L.zkd_oracle_api_from_double.argtypes = [vp, ctypes.c_int, ctypes.c_double]
@@ -139,6 +142,43 @@ def lu_solve(A: np.ndarray, B: np.ndarray, N: int, nrhs: int, prec: int = PREC, 
     X = np.zeros(N * nrhs * 2 * rb, dtype=np.uint8)
     rc = lib().zkd_oracle_lu_solve(N, nrhs, prec, guard_bits, A.ctypes.data, B.ctypes.data, X.ctypes.data)
     return X, rc
+
+
+def api_matrix_to_complex128(A: np.ndarray, N: int, prec: int = PREC) -> np.ndarray:
+    """Hermitian API matrix (upper triangle authoritative) rounded to complex128, for the fp64 stage of rqi_refine."""
+    rb = real_bytes(prec)
+    flat = np.ascontiguousarray(A, dtype=np.uint8).reshape(N, N, 2, rb)
+    out = np.zeros((N, N), dtype=np.complex128)
+    for i in range(N):
+        for j in range(i, N):
+            re = lib().zkd_oracle_api_to_double(flat[i, j, 0].ctypes.data, prec)
+            im = lib().zkd_oracle_api_to_double(flat[i, j, 1].ctypes.data, prec) if i != j else 0.0
+            out[i, j] = complex(re, im)
+            out[j, i] = complex(re, -im)
+    return out
+
+
+def rqi_refine(A: np.ndarray, N: int, first: int = 0, count: int | None = None, iters: int = 3, max_pivots: int = 0,
+               threads: int | None = None, prec: int = PREC, guard_bits: int = GUARD_BITS, V64: np.ndarray | None = None):
+    """CPU restatement of the paper's route: LAPACK fp64 eigendecomposition (numpy.linalg.eigh), then Rayleigh
+    quotient iteration in MPFR (one Gaussian elimination per eigenpair and iteration).  Timed CPU baseline only.
+    Returns (lam uint8[count*rb], X uint8[N*count*2*rb], seconds of the fp64 stage, V64)."""
+    import time
+
+    rb = real_bytes(prec)
+    count = N - first if count is None else count
+    A = np.ascontiguousarray(A, dtype=np.uint8)
+    t0 = time.perf_counter()
+    if V64 is None:
+        _, V64 = np.linalg.eigh(api_matrix_to_complex128(A, N, prec))
+    t64 = time.perf_counter() - t0
+    Vc = np.ascontiguousarray(V64.astype(np.complex128)).view(np.float64)
+    lam = np.zeros(count * rb, dtype=np.uint8)
+    X = np.zeros(N * count * 2 * rb, dtype=np.uint8)
+    rc = lib().zkd_oracle_rqi(N, prec, guard_bits, A.ctypes.data, Vc.ctypes.data, first, count, iters, max_pivots,
+                              threads or host_threads(), lam.ctypes.data, X.ctypes.data)
+    assert rc == 0, rc
+    return lam, X, t64, V64
 
 
 def api_to_double(buf, prec: int = PREC) -> float:

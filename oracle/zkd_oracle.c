@@ -1076,3 +1076,156 @@ int zkd_oracle_lu_solve(int N, int nrhs, int prec, int guard_bits, const uint8_t
   mpfr_clear(dr); mpfr_clear(di); mpfr_clear(t1); mpfr_clear(t2);
   return status;
 }
+
+/* ================================================================================================ */
+/* CPU restatement of the paper's own route: fp64 eigendecomposition + Rayleigh quotient iteration   */
+/* ================================================================================================ */
+/* PAPER.md:33 (section 2): "the Rayleigh quotient iteration was employed to recover the precision from the result of
+ * double-precision calculations".  Used ONLY as a timed CPU baseline beside the GPU numbers (bench.py) and cross-checked
+ * against the Jacobi oracle in tests/test_oracle_pins.py (P12); the checker of the CUDA path stays the Jacobi oracle.
+ * For every eigenpair j in [first, first + count): start x = column j of the supplied fp64 eigenvector matrix; repeat `iters`
+ * times: sigma = x^H A x (x has unit norm); solve (A - sigma I) y = x by Gaussian elimination with partial pivoting at
+ * P_o = prec + guard_bits (a pivot that is exactly zero - sigma has converged to the working precision - is replaced by
+ * 2^-P_o ||A||_F, the usual inverse-iteration safeguard); x = y / ||y||.  Output lambda_j = x^H A x and x, phase-normalised like
+ * the Jacobi oracle (first component of largest modulus real positive).  Isolated eigenvalues only.
+ *   max_pivots > 0: every elimination stops after that many pivot columns (bench sampling hook: the result is then
+ *   meaningless; the caller extrapolates the time by the flop count sum_{k < max_pivots} (N-1-k)^2 / sum_{k < N-1} (N-1-k)^2).
+ * OpenMP over eigenpairs.  Layout: V64[i][j] complex double, row-major (component i of vector j); lam_api[count],
+ * X_api[i][c] (N x count) row-major complex API numbers.  Returns 0, or 3 for malformed input. */
+int zkd_oracle_rqi(int N, int prec, int guard_bits, const uint8_t *A_api, const double *V64, int first, int count, int iters,
+                   int max_pivots, int nthreads, uint8_t *lam_api, uint8_t *X_api) {
+  const long Po = (long)prec + guard_bits;
+  const size_t rb = api_real_bytes(prec);
+  if (N < 1 || count < 1 || first < 0 || first + count > N || prec < 64 || prec % 64) return 3;
+  if (nthreads < 1) nthreads = 1;
+  int status = 0;
+  mpfr_t tmpP0, F, w0;
+  mpfr_init2(tmpP0, prec); mpfr_init2(F, Po); mpfr_init2(w0, Po);
+  cmat A = cmat_alloc(N, Po);
+  for (int i = 0; i < N && !status; ++i)
+    for (int j = i; j < N; ++j) {
+      const uint8_t *src = A_api + ((size_t)i * N + j) * 2 * rb;
+      if (api_get(RE(A, i, j), src, prec, tmpP0) || api_get(IM(A, i, j), src + rb, prec, tmpP0)) { status = 3; break; }
+      if (i == j) mpfr_set_zero(IM(A, i, j), +1);
+      else { mpfr_set(RE(A, j, i), RE(A, i, j), RN); mpfr_neg(IM(A, j, i), IM(A, i, j), RN); }
+    }
+  mpfr_set_zero(F, +1);
+  for (int i = 0; i < N && !status; ++i)
+    for (int j = 0; j < N; ++j) {
+      mpfr_sqr(w0, RE(A, i, j), RN); mpfr_add(F, F, w0, RN);
+      mpfr_sqr(w0, IM(A, i, j), RN); mpfr_add(F, F, w0, RN);
+    }
+  mpfr_sqrt(F, F, RN);
+  if (!status) {
+#pragma omp parallel for num_threads(nthreads) schedule(dynamic, 1)
+    for (int c = 0; c < count; ++c) {
+      const int j = first + c;
+      mpfr_t tmpP, sg, best, m2, w, lr, li, t1, t2, nr;
+      mpfr_init2(tmpP, prec); mpfr_init2(sg, Po); mpfr_init2(best, Po); mpfr_init2(m2, Po); mpfr_init2(w, Po);
+      mpfr_init2(lr, Po); mpfr_init2(li, Po); mpfr_init2(t1, Po); mpfr_init2(t2, Po); mpfr_init2(nr, Po);
+      rmat M = rmat_alloc(N, N, Po), x = rmat_alloc(N, 1, Po), y = rmat_alloc(N, 1, Po);
+      for (int i = 0; i < N; ++i) {
+        mpfr_set_d(RRE(x, i, 0), V64[((size_t)i * N + j) * 2], RN);
+        mpfr_set_d(RIM(x, i, 0), V64[((size_t)i * N + j) * 2 + 1], RN);
+      }
+      for (int it = 0; it <= iters; ++it) {
+        /* unit norm, then sigma = x^H A x */
+        col_dot(nr, w, &x, 0, 0, t1);
+        mpfr_sqrt(nr, nr, RN);
+        for (int i = 0; i < N; ++i) { mpfr_div(RRE(x, i, 0), RRE(x, i, 0), nr, RN); mpfr_div(RIM(x, i, 0), RIM(x, i, 0), nr, RN); }
+        mpfr_set_zero(sg, +1);
+        for (int i = 0; i < N; ++i) {
+          mpfr_set_zero(lr, +1); mpfr_set_zero(li, +1); /* (A x)_i */
+          for (int k = 0; k < N; ++k) {
+            mpfr_fmms(t1, RE(A, i, k), RRE(x, k, 0), IM(A, i, k), RIM(x, k, 0), RN); mpfr_add(lr, lr, t1, RN);
+            mpfr_fmma(t1, RE(A, i, k), RIM(x, k, 0), IM(A, i, k), RRE(x, k, 0), RN); mpfr_add(li, li, t1, RN);
+          }
+          mpfr_fmma(t1, RRE(x, i, 0), lr, RIM(x, i, 0), li, RN); /* Re conj(x_i) (A x)_i */
+          mpfr_add(sg, sg, t1, RN);
+        }
+        if (it == iters) break;
+        /* M = A - sigma I, y = x; Gaussian elimination with partial pivoting (same steps as zkd_oracle_lu_solve) */
+        for (int i = 0; i < N; ++i) {
+          for (int k = 0; k < N; ++k) { mpfr_set(RRE(M, i, k), RE(A, i, k), RN); mpfr_set(RIM(M, i, k), IM(A, i, k), RN); }
+          mpfr_sub(RRE(M, i, i), RRE(M, i, i), sg, RN);
+          mpfr_set(RRE(y, i, 0), RRE(x, i, 0), RN); mpfr_set(RIM(y, i, 0), RIM(x, i, 0), RN);
+        }
+#define CDIV2(outr, outi, xr, xi, cr, ci)                                  \
+  do {                                                                     \
+    mpfr_sqr(t1, cr, RN); mpfr_sqr(t2, ci, RN); mpfr_add(w, t1, t2, RN);   \
+    mpfr_fmma(t1, xr, cr, xi, ci, RN); mpfr_fmms(t2, xi, cr, xr, ci, RN);  \
+    mpfr_div(outr, t1, w, RN); mpfr_div(outi, t2, w, RN);                  \
+  } while (0)
+        const int kmax = (max_pivots > 0 && max_pivots < N) ? max_pivots : N;
+        for (int k = 0; k < kmax; ++k) {
+          int p = k;
+          mpfr_set_si(best, -1, RN);
+          for (int i = k; i < N; ++i) {
+            mpfr_sqr(m2, RRE(M, i, k), RN); mpfr_sqr(w, RIM(M, i, k), RN); mpfr_add(m2, m2, w, RN);
+            if (mpfr_cmp(m2, best) > 0) { mpfr_set(best, m2, RN); p = i; }
+          }
+          if (mpfr_zero_p(best)) { mpfr_div_2si(RRE(M, k, k), F, Po, RN); mpfr_set_zero(RIM(M, k, k), +1); p = k; }
+          if (p != k) {
+            for (int c2 = 0; c2 < N; ++c2) { mpfr_swap(RRE(M, k, c2), RRE(M, p, c2)); mpfr_swap(RIM(M, k, c2), RIM(M, p, c2)); }
+            mpfr_swap(RRE(y, k, 0), RRE(y, p, 0)); mpfr_swap(RIM(y, k, 0), RIM(y, p, 0));
+          }
+          for (int i = k + 1; i < N; ++i) {
+            CDIV2(lr, li, RRE(M, i, k), RIM(M, i, k), RRE(M, k, k), RIM(M, k, k));
+            for (int c2 = k + 1; c2 < N; ++c2) {
+              mpfr_fmms(t1, lr, RRE(M, k, c2), li, RIM(M, k, c2), RN); mpfr_sub(RRE(M, i, c2), RRE(M, i, c2), t1, RN);
+              mpfr_fmma(t1, lr, RIM(M, k, c2), li, RRE(M, k, c2), RN); mpfr_sub(RIM(M, i, c2), RIM(M, i, c2), t1, RN);
+            }
+            mpfr_fmms(t1, lr, RRE(y, k, 0), li, RIM(y, k, 0), RN); mpfr_sub(RRE(y, i, 0), RRE(y, i, 0), t1, RN);
+            mpfr_fmma(t1, lr, RIM(y, k, 0), li, RRE(y, k, 0), RN); mpfr_sub(RIM(y, i, 0), RIM(y, i, 0), t1, RN);
+          }
+        }
+        if (kmax == N) {
+          for (int i = N - 1; i >= 0; --i) {
+            mpfr_set(lr, RRE(y, i, 0), RN); mpfr_set(li, RIM(y, i, 0), RN);
+            for (int c2 = i + 1; c2 < N; ++c2) {
+              mpfr_fmms(t1, RRE(M, i, c2), RRE(y, c2, 0), RIM(M, i, c2), RIM(y, c2, 0), RN); mpfr_sub(lr, lr, t1, RN);
+              mpfr_fmma(t1, RRE(M, i, c2), RIM(y, c2, 0), RIM(M, i, c2), RRE(y, c2, 0), RN); mpfr_sub(li, li, t1, RN);
+            }
+            CDIV2(RRE(y, i, 0), RIM(y, i, 0), lr, li, RRE(M, i, i), RIM(M, i, i));
+          }
+          /* scale by 2^-exp of the largest component before the norm (y is huge once sigma has converged) */
+          long emax = LONG_MIN;
+          for (int i = 0; i < N; ++i) {
+            if (!mpfr_zero_p(RRE(y, i, 0)) && mpfr_get_exp(RRE(y, i, 0)) > emax) emax = mpfr_get_exp(RRE(y, i, 0));
+            if (!mpfr_zero_p(RIM(y, i, 0)) && mpfr_get_exp(RIM(y, i, 0)) > emax) emax = mpfr_get_exp(RIM(y, i, 0));
+          }
+          for (int i = 0; i < N; ++i) {
+            mpfr_div_2si(RRE(x, i, 0), RRE(y, i, 0), emax, RN); mpfr_div_2si(RIM(x, i, 0), RIM(y, i, 0), emax, RN);
+          }
+        }
+#undef CDIV2
+      }
+      /* output: lambda_j = sigma; x phase-normalised (first component of largest modulus real positive), unit norm */
+      if (lam_api) api_put(lam_api + (size_t)c * rb, sg, prec, tmpP);
+      if (X_api) {
+        int kstar = 0;
+        mpfr_set_si(best, -1, RN);
+        for (int i = 0; i < N; ++i) {
+          mpfr_sqr(m2, RRE(x, i, 0), RN); mpfr_sqr(w, RIM(x, i, 0), RN); mpfr_add(m2, m2, w, RN);
+          if (mpfr_cmp(m2, best) > 0) { mpfr_set(best, m2, RN); kstar = i; }
+        }
+        mpfr_sqrt(best, best, RN);
+        mpfr_div(lr, RRE(x, kstar, 0), best, RN); mpfr_div(li, RIM(x, kstar, 0), best, RN); mpfr_neg(li, li, RN);
+        for (int i = 0; i < N; ++i) {
+          mpfr_fmms(t1, RRE(x, i, 0), lr, RIM(x, i, 0), li, RN);
+          mpfr_fmma(t2, RRE(x, i, 0), li, RIM(x, i, 0), lr, RN);
+          if (i == kstar) mpfr_set_zero(t2, +1);
+          uint8_t *dst = X_api + ((size_t)i * count + c) * 2 * rb;
+          api_put(dst, t1, prec, tmpP);
+          api_put(dst + rb, t2, prec, tmpP);
+        }
+      }
+      rmat_free(&M); rmat_free(&x); rmat_free(&y);
+      mpfr_clear(tmpP); mpfr_clear(sg); mpfr_clear(best); mpfr_clear(m2); mpfr_clear(w); mpfr_clear(lr); mpfr_clear(li);
+      mpfr_clear(t1); mpfr_clear(t2); mpfr_clear(nr);
+    }
+  }
+  cmat_free(&A);
+  mpfr_clear(tmpP0); mpfr_clear(F); mpfr_clear(w0);
+  return status;
+}

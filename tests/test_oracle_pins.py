@@ -474,3 +474,27 @@ def test_P11_comparator_multi_member_groups(mp):
     c = oracle.compare(cI, 5, lamI, XI, lamI, zi.cmatrix_from_mp(mp.eye(5), 5))
     assert c["groups"] == 1 and c["max_group"] == 5 and c["vec_margin_bits"] < -1e8
     assert c["log2_resid_rel"] <= -760 and c["log2_orth"] <= -760
+
+
+def test_P12_rqi_restatement_agrees_with_jacobi_and_mpmath(mp):
+    """oracle.rqi_refine - the CPU restatement of the paper's own route (fp64 LAPACK eigendecomposition + Rayleigh quotient
+    iteration in MPFR), used only as a timed baseline - gives the eigenpairs of the pinned Jacobi oracle, and its
+    residual, computed here in mpmath, is at the working precision; three iterations from the fp64 start are cubic."""
+    N = 12
+    A = zi.random_hermitian(N, 1212)
+    lam, X, _, _ = oracle.rqi_refine(A, N, iters=3, threads=2)
+    l0, X0, info = oracle.diag_herm(A, N)
+    assert info["status"] == 0
+    c = oracle.compare(A, N, lam, X, l0, X0)
+    assert c["log2_dlam_rel"] <= -750 and c["log2_resid_rel"] <= -750 and c["log2_orth"] <= -745 and c["vec_margin_bits"] <= 0, c
+    Am = herm_from_upper(mp, zi.cmatrix_to_mp(A, N), N)
+    lam_m, Xm = decode(mp, lam, X, N)
+    F = fro(mp, Am)
+    j = 5
+    r = mp.sqrt(sum(abs(sum(Am[i, k] * Xm[k, j] for k in range(N)) - lam_m[j] * Xm[i, j]) ** 2 for i in range(N)))
+    assert log2abs(mp, r / F) <= -755
+    # one iteration is not enough (vector 2^-50 -> 2^-150, eigenvalue error its square), a subset of pairs works, the sampling hook returns
+    lam2, X2, _, _ = oracle.rqi_refine(A, N, first=3, count=4, iters=1, threads=1)
+    d = max(abs(zi.to_fraction(lam2.reshape(4, -1)[t]) - zi.to_fraction(l0.reshape(N, -1)[3 + t])) for t in range(4))
+    assert Fraction(1, 2 ** 420) < d < Fraction(1, 2 ** 200), float(d)
+    oracle.rqi_refine(A, N, first=0, count=2, iters=1, max_pivots=3, threads=1)
