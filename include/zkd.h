@@ -177,7 +177,8 @@ int zkd_mps_two_site_update(int chiL, int chiC, int chiR, int d, int batch, int 
  * that otherwise caps the gain of a pass), "seed_ring_block" (columns per block of the block-ring fp64 seed for N <= 256:
  * 2 or 4, 0 = the column ring, default -1 = 4 from N = 96 on), "seed_tma" (default 1: the blocked fp64 seed moves its columns by TMA bulk copies),
  * "seed_block_warps" (8 or 16), "combine_path" (epilogue of the IMAD GEMM: 0 automatic,
- * 1 digit-serial, 2 warp-cooperative), "sstep_cpb" (matrix columns per CTA of the fused singleton step, 0 automatic), "sstep_warp" (1: its
+ * 1 digit-serial, 2 warp-cooperative), "sstep_cpb" (matrix columns per CTA of the fused singleton step, 0 automatic), "sstep_par" (default 1: for N <= 96 and
+ * one column per CTA the products of a row are spread over four threads), "sstep_warp" (1: its
  * warp-per-element variant for N <= 64, default 0), "sstep_cache" (shared-memory staging of the column, default 1),
  * "verbose" (1: one line per refinement pass on stderr).  All routes give the same results to the stated tolerances;
  * the defaults are the measured-fastest ones.  Returns ZKD_ERR_INVALID_ARG for an unknown key. */

@@ -218,6 +218,7 @@ static int* option_slot(const char* key) {
   if (!strcmp(key, "split_margin_bits")) return &o.split_margin_bits;
   if (!strcmp(key, "sstep_cpb")) return &o.sstep_cpb;
   if (!strcmp(key, "sstep_cache")) return &o.sstep_cache;
+  if (!strcmp(key, "sstep_par")) return &o.sstep_par;
   if (!strcmp(key, "sstep_warp")) return &o.sstep_warp;
   if (!strcmp(key, "combine_path")) return &o.combine_path;
   if (!strcmp(key, "cluster_tiles")) return &o.cluster_tiles;

@@ -472,6 +472,137 @@ __global__ void __launch_bounds__(256) singleton_step_kernel(int n, int nb, int3
   __syncthreads();
   if (tid == 0 && msb_r_out && s_msb) atomicMax(msb_r_out, s_msb);
 }
+// ---- the same step with the 14 products of a row spread over several threads (small n, one column per CTA) ------------------------
+// singleton_step_kernel gives every thread whole rows: 14 dependent 30 x 30-digit products (~500 IMAD.WIDE each) per row, on as many
+// threads as the column has rows - at n = 64 that is two warps per CTA walking a 7000-multiply chain (the kernel was the largest item of
+// c2: 6 x 70 us).  Here the work items are (row, plane) / (row, term) pairs, so a thread's chain is 6 products: |x|^2 (1), the
+// normalisation of one plane (1), one term of Re s and of Im s (2), one part of the residual (2).  Same integer sums, same
+// roundings: bit-identical results.  The column's x, w digits live in shared memory throughout.
+__global__ void __launch_bounds__(256) singleton_step_par_kernel(int n, int nb, int32_t* __restrict__ X, int32_t* __restrict__ W,
+                                                                 int32_t* __restrict__ R, int32_t* __restrict__ S,
+                                                                 int32_t* __restrict__ theta, int* __restrict__ msb_g_out,
+                                                                 int* __restrict__ msb_r_out, const int* __restrict__ cl,
+                                                                 const int* __restrict__ cle, int* __restrict__ msb_g_b) {
+  __shared__ int64_t s_part[16 * FXP_NACC];
+  __shared__ int s_msb;
+  extern __shared__ int32_t s_cache[];  // [4][ND][n]: xr, xi, wr, wi
+  const int b = blockIdx.x / n, j = blockIdx.x % n;
+  const int tid = threadIdx.x, T = blockDim.x, nwarps = T >> 5;
+  const bool act = !(cl && cle[(size_t)b * n + j] - cl[(size_t)b * n + j] > 1);  // columns of larger clusters take the GEMM path
+  const size_t per = (size_t)n * n, count = per * nb;
+  int32_t* const gplane[4] = {X, X + (size_t)ND * count, W, W + (size_t)ND * count};
+  if (tid == 0) s_msb = 0;
+  if (act) {
+    for (int it = tid; it < 4 * n; it += T) {
+      const int pl = it / n, k = it - pl * n;
+      int32_t a[ND];
+      fx_load(a, gplane[pl], count, (size_t)b * per + (size_t)k * n + j);
+      fx_store(s_cache + (size_t)pl * ND * n, (size_t)n, (size_t)k, a);
+    }
+  }
+  __syncthreads();
+  // g = sum_k |x_kj|^2
+  int64_t acc[FXP_NACC];
+  fxp_zero(acc);
+  if (act) {
+    for (int it = tid; it < 2 * n; it += T) {
+      const int pl = it / n, k = it - pl * n;
+      int32_t a[ND];
+      fx_load(a, s_cache + (size_t)pl * ND * n, (size_t)n, (size_t)k);
+      fx_mac<false>(acc, a, a);
+      fxp_relax(acc);
+    }
+  }
+  block_sum_cols<1>(acc, s_part, nwarps);
+  int32_t g[ND], m[ND];
+  fxp_finish(g, acc);
+  g[ND - 1] -= 1;  // g - 1
+  if (act && tid == 0 && msb_g_out) {
+    const int mg = fx_msb(g);
+    atomicMax(msb_g_out, mg);
+    if (msb_g_b && mg) atomicMax(msb_g_b + b, mg);
+  }
+  {
+    int32_t t[ND];
+    fx_neg(t, g);
+    fx_half(m, t);  // m = (1 - g)/2
+  }
+  // x <- x + x m, w <- w + w m
+  if (act) {
+    for (int it = tid; it < 4 * n; it += T) {
+      const int pl = it / n, k = it - pl * n;
+      int32_t u[ND], t[ND], o[ND];
+      fx_load(u, s_cache + (size_t)pl * ND * n, (size_t)n, (size_t)k);
+      fx_mul(t, u, m);
+      fx_add(o, u, t);
+      fx_store(s_cache + (size_t)pl * ND * n, (size_t)n, (size_t)k, o);
+      fx_store(gplane[pl], count, (size_t)b * per + (size_t)k * n + j, o);
+    }
+  }
+  __syncthreads();
+  // s = x^H w : real part, then imaginary part (items: (term, row))
+  int32_t sr[ND], si[ND];
+#pragma unroll 1
+  for (int part = 0; part < 2; ++part) {
+    fxp_zero(acc);
+    if (act) {
+      for (int it = tid; it < 2 * n; it += T) {
+        const int term = it / n, k = it - term * n;
+        // part 0: xr wr + xi wi ;  part 1: xr wi - xi wr
+        int32_t a[ND], c[ND];
+        fx_load(a, s_cache + (size_t)term * ND * n, (size_t)n, (size_t)k);
+        fx_load(c, s_cache + (size_t)(2 + (term ^ part)) * ND * n, (size_t)n, (size_t)k);
+        if (part == 1 && term == 1) {
+#pragma unroll
+          for (int q = 0; q < ND; ++q) a[q] = -a[q];  // digit-wise negation: a valid (non-canonical) operand of fx_mac
+        }
+        fx_mac<false>(acc, a, c);
+        fxp_relax(acc);
+      }
+    }
+    block_sum_cols<1>(acc, s_part, nwarps);
+    if (part == 0) fxp_finish(sr, acc); else fxp_finish(si, acc);
+  }
+  if (act && tid == 0) {
+    fx_store(theta, (size_t)n * nb, (size_t)b * n + j, sr);
+    const size_t ejj = (size_t)b * per + (size_t)j * n + j;
+    fx_store(S, count, ejj, sr);
+    fx_store(S + (size_t)ND * count, count, ejj, si);
+  }
+  // r = w - x s (items: (part, row))
+  int mymsb = 0;
+  if (act) {
+    for (int it = tid; it < 2 * n; it += T) {
+      const int part = it / n, k = it - part * n;
+      int32_t a[ND], t[ND];
+      fxp_zero(acc);
+      // part 0: xr sr - xi si ;  part 1: xr si + xi sr
+#pragma unroll 1
+      for (int term = 0; term < 2; ++term) {
+        int32_t mm[ND];
+        const bool use_si = (term ^ part) != 0, neg = part == 0 && term == 1;
+#pragma unroll
+        for (int q = 0; q < ND; ++q) {
+          const int32_t v = use_si ? si[q] : sr[q];
+          mm[q] = neg ? -v : v;
+        }
+        fx_load(a, s_cache + (size_t)term * ND * n, (size_t)n, (size_t)k);
+        fx_mac<false>(acc, a, mm);
+      }
+      fxp_finish(t, acc);
+      fx_load(a, s_cache + (size_t)(2 + part) * ND * n, (size_t)n, (size_t)k);
+      int32_t o[ND];
+      fx_sub(o, a, t);
+      fx_store(R + (part ? (size_t)ND * count : 0), count, (size_t)b * per + (size_t)k * n + j, o);
+      mymsb = max(mymsb, fx_msb(o));
+    }
+  }
+  for (int off = 16; off > 0; off >>= 1) mymsb = max(mymsb, __shfl_xor_sync(0xffffffffu, mymsb, off));
+  if ((tid & 31) == 0 && mymsb) atomicMax(&s_msb, mymsb);
+  __syncthreads();
+  if (tid == 0 && msb_r_out && s_msb) atomicMax(msb_r_out, s_msb);
+}
+
 // ---- warp-cooperative variant for small n (north_star (b): "warp-cooperative limb add, multiply, normalise ... carry chains
 // via warp shuffles") -------------------------------------------------------------------------------------------------------
 // One CTA per matrix column, one WARP per element: lane L holds digit L of an FX number (lanes 0..29) and, in a product,
@@ -712,6 +843,11 @@ int singleton_step(int n, int nb, int32_t* X, int32_t* W, int32_t* R, int32_t* S
   if (cpb == 1 && n <= 16 * SW_RPW && options().sstep_warp) {
     const int nw = (n + SW_RPW - 1) / SW_RPW;
     singleton_step_warp_kernel<<<grid, 32 * nw, 0, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle, msb_g_b);
+  } else if (cpb == 1 && options().sstep_par && n <= 96 && sizeof(int32_t) * 4 * ND * (size_t)n <= 40 * 1024) {
+    int threads = (4 * n + 31) / 32 * 32;
+    if (threads > 256) threads = 256;  // 255 registers per thread: the digit arrays of g, m, s and one accumulator set stay in registers
+    singleton_step_par_kernel<<<grid, threads, sizeof(int32_t) * 4 * ND * (size_t)n, s>>>(n, nb, X, W, R, S, theta, msb_g_out, msb_r_out, cl, cle,
+                                                                                       msb_g_b);
   } else if (cpb == 1) {
     int threads = (n + 31) / 32 * 32;
     if (threads > 256) threads = 256;

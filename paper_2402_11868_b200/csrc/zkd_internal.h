@@ -56,6 +56,7 @@ struct Options {
   int cluster_tiles = 1;      // cluster passes as 128-column tile products on the int8 engine when no cluster straddles a tile
   int combine_path = 0;       // IMAD GEMM epilogue: 0 auto, 1 digit-serial thread per element, 2 warp-cooperative (digit per lane)
   int sstep_warp = 0;         // singleton_step: 1: warp-per-element kernel (digit per lane) when one column per CTA and n <= 64; measured 1 % faster at N = 16, 3 % slower at N = 64: off by default
+  int sstep_par = 1;          // singleton_step, one column per CTA, n <= 96: the products of a row spread over several threads
   int sstep_cache = 1;        // singleton_step: stage the column's x, w digits in shared memory (one column per CTA, n <= 96)
   int sstep_cpb = 0;          // singleton_step: matrix columns per CTA (0: auto)
   int verbose = 0;

@@ -128,7 +128,7 @@ def test_parity_public_entry_points(zkd, name, batch):
 @pytest.mark.parametrize("name,opt,val", [("c4small", "early_split", 0), ("c5small", "split_margin_bits", 20),
                                           ("c4small", "tau_bits", 12), ("c5small", "tau_bits", 30), ("c4small", "sstep_cpb", 8),
                                           ("c2", "sstep_cpb", 4), ("c1", "sstep_cpb", 2), ("c2", "sstep_warp", 1), ("c1", "sstep_warp", 1),
-                                          ("c4small", "sstep_warp", 1), ("c2", "sstep_cache", 0), ("c5mid", "cluster_tiles", 2), ("c5small", "block_correction", 0),
+                                          ("c4small", "sstep_warp", 1), ("c2", "sstep_cache", 0), ("c5mid", "cluster_tiles", 2), ("c5small", "block_correction", 0), ("c2", "sstep_par", 0), ("c1", "sstep_par", 0),
                                           ("c4small", "block_correction", 0)])
 def test_parity_alternative_paths(zkd, name, opt, val):
     """The same results through the other routes of the method: clusters left to the S5 recursion (S4h off), a different
