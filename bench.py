@@ -469,7 +469,7 @@ def main():
     if not args.no_extra and world == 1:
         extra = {}
         # (the last two rows: the paper's other precisions, 256 bit = Deutsch-Jozsa runs PAPER.md:61, 128 bit = Shor runs :65)
-        for nm, bb, k, pr in (("c1", 1, 5, 768), ("c2", 1, 5, 768), ("c2", 256, 3, 768), ("c3", 1, 5, 768), ("c4", 512, 3, 768),
+        for nm, bb, k, pr in (("c1", 1, 5, 768), ("c1", 4096, 3, 768), ("c2", 1, 5, 768), ("c2", 256, 3, 768), ("c3", 1, 5, 768), ("c4", 512, 3, 768),
                               ("c5", 1, 3, 768), ("c4", 512, 3, 256), ("c4", 512, 3, 128)):
             if nm == args.workload and bb == b and pr == 768:
                 continue

@@ -165,7 +165,8 @@ int zkd_mps_two_site_update(int chiL, int chiC, int chiR, int d, int batch, int 
  * default 20), "tol_bits" (stop when max|R_ij| <= 2^-tol, default 770), "max_steps" (default 120),
  * "gemm_path" (engine of the digit GEMM: 0 = automatic [default]: limb-sliced int8 tcgen05 MMAs when M, N, K >= 128,
  * the IMAD kernel otherwise; 1 = IMAD only; 2 = int8 tcgen05 wherever its tiles can be formed),
- * "min_split_ctas" (split-K target, default 296; every split keeps at least 32 of K), "early_split" (S4h: split clusters whose internal structure stands
+ * "gemm_tile" (tile of the IMAD digit GEMM: 0 automatic - 8 x 8 x 8 where 16-wide tiles
+ * would be filled more than 1.25 x worse, e.g. 24- or 29-dimensional cluster blocks -, 8, 16), "min_split_ctas" (split-K target, default 296; every split keeps at least 32 of K), "early_split" (S4h: split clusters whose internal structure stands
  * above the noise of the projected matrix; default 1; 0 leaves every cluster to the S5 recursion),
  * "split_margin_bits" (that margin, default 40), "seed_sweeps" (cap on the fp64 Jacobi sweeps, default 12),
  * "seed_path" / "seed_cluster" (seed kernel selection), "cluster_tiles" (default 1: on levels where

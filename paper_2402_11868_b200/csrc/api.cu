@@ -207,6 +207,7 @@ static int* option_slot(const char* key) {
   if (!strcmp(key, "max_steps")) return &o.max_steps;
   if (!strcmp(key, "gemm_path")) return &o.gemm_path;
   if (!strcmp(key, "min_split_ctas")) return &o.min_split_ctas;
+  if (!strcmp(key, "gemm_tile")) return &o.gemm_tile;
   if (!strcmp(key, "seed_sweeps")) return &o.seed_sweeps;
   if (!strcmp(key, "seed_path")) return &o.seed_path;
   if (!strcmp(key, "seed_dbuf")) return &o.seed_dbuf;

@@ -5,6 +5,7 @@
 // Complex product by 3 real products (3M):  with P = pr + i pi and Q = qr + i qi,
 //     k1 = (pr + pi) qr,  k2 = pr (qi - qr),  k3 = pi (qr + qi);   Re = k1 - k3,  Im = k1 + k2.
 // In fixed point the operand sums are exact, so 3M costs nothing in accuracy.
+#include <algorithm>
 #include <cstdio>
 #include <vector>
 
@@ -535,15 +536,25 @@ int kernel_timing_read(double* ms, uint64_t* launches, uint64_t* macs) { return 
 
 static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
-static int pick_splits(int M, int N, int K, int batch) {
+// tile size for a shape: 8 when 16-wide tiles would be filled much worse (see gemm_digits.cuh)
+static int pick_tile(int M, int N, int K) {
+  if (options().gemm_tile == 8 || options().gemm_tile == 16) return options().gemm_tile;
+  auto fill = [&](int t) {
+    auto up = [&](int x) { return (double)((x + t - 1) / t * t); };
+    return (double)M * N * K / (up(M) * up(N) * up(K));
+  };
+  return fill(8) > 1.25 * fill(16) ? 8 : 16;
+}
+
+static int pick_splits(int M, int N, int K, int batch, int tg = GT) {
   // Split K until the product has about min_split_ctas CTAs, but leave every split at least two 16-deep K tiles: a CTA
   // that does a single tile is all prologue and epilogue, and every split adds a raw plane for the epilogue to sum
   // (measured: N = 64, K = 64: 2 splits 2.27 ms per matrix, 4 splits 2.37, none 2.46; K = 1024 wants its splits).
-  const long tiles = (long)((M + GT - 1) / GT) * ((N + GT - 1) / GT) * 3 * batch;
+  const long tiles = std::max(1L, (long)((M + tg - 1) / tg) * ((N + tg - 1) / tg) * 3 * batch / (tg == 8 ? 4 : 1));  // in units of 256 threads
   const int want = options().min_split_ctas;
   if (tiles >= want) return 1;
   int s = (int)((want + tiles - 1) / tiles);
-  const int kmax = ((K + GT - 1) / GT) / 2;
+  const int kmax = ((K + 15) / 16) / 2;  // at least 32 of K per split, whatever the tile
   if (s > kmax) s = kmax;
   if (s > 32) s = 32;
   return s < 1 ? 1 : s;
@@ -552,7 +563,7 @@ static int pick_splits(int M, int N, int K, int batch) {
 size_t gemm_workspace_bytes(int M, int N, int K, int batch) {
   const size_t pc = align_up(sizeof(int32_t) * 3 * (size_t)batch * kND * M * K);
   const size_t qc = align_up(sizeof(int32_t) * 3 * (size_t)batch * kND * K * N);
-  const int sp = pick_splits(M, N, K, batch);
+  const int sp = std::max(pick_splits(M, N, K, batch, 16), pick_splits(M, N, K, batch, 8));
   const size_t raw = align_up(sizeof(int32_t) * (size_t)sp * 3 * batch * (2 * kND + 3) * M * N);
   const size_t i8 = gemm_i8_eligible(options().gemm_path, M, N, K, batch) ? gemm_i8_workspace_bytes(M, N, K, batch) : 0;
   return pc + qc + (raw > i8 ? raw : i8);
@@ -611,20 +622,21 @@ int gemm_complex(int M, int N, int K, int batch, const GemmSide& P, const GemmSi
   if (use_i8)
     return gemm_i8_finish(M, N, K, batch, Pc, Qc, npad, nqad, lsbP, lsbQ, dst_fx, (int)mode, out_cut_bit, raw,
                           workspace_bytes - (size_t)((char*)raw - (char*)workspace), err_flag, msb_out, stream, dv);
-  const int nsplit = pick_splits(M, N, K, batch);
+  const int tg = pick_tile(M, N, K);
+  const int nsplit = pick_splits(M, N, K, batch, tg);
   int ksplit = (K + nsplit - 1) / nsplit;
-  ksplit = (ksplit + GT - 1) / GT * GT;
+  ksplit = (ksplit + tg - 1) / tg * tg;
   const int nsp = (K + ksplit - 1) / ksplit;
   GemmKArgs ka{};
   ka.P = Pc; ka.Q = Qc; ka.Out = raw;
   ka.p_dstride = (size_t)M * K; ka.p_gstride = (size_t)in->np * M * K;
   ka.q_dstride = (size_t)K * N; ka.q_gstride = (size_t)in->nq * K * N;
   ka.M = M; ka.N = N; ka.K = K; ka.G = 3 * batch; ka.ksplit = ksplit; ka.nsplit = nsp;
-  dim3 grid((N + GT - 1) / GT, (M + GT - 1) / GT, (unsigned)(3 * batch * nsp));
+  dim3 grid((N + tg - 1) / tg, (M + tg - 1) / tg, (unsigned)(3 * batch * nsp));
   const uint64_t nmacs = inst_cost(*in) * 3ull * (uint64_t)batch * M * N * K;
   {
     KtScope kt(KC_GEMM_DIGITS, stream, nmacs, request_cost(P.nw, Q.nw) * 3ull * (uint64_t)batch * M * N * K);
-    if (in->launch(ka, grid, stream) != cudaSuccess) return ZKD_ERR_CUDA;
+    if ((tg == 8 ? in->launch8 : in->launch)(ka, grid, stream) != cudaSuccess) return ZKD_ERR_CUDA;
   }
   count_launch();
   count_macs(nmacs);

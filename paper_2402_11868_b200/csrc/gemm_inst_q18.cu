@@ -3,7 +3,7 @@
 #include "gemm_digits.cuh"
 
 namespace zkd {
-#define ZKD_INST(NP, NQ) {NP, NQ, GemmShape<NP, NQ>::LOW, GemmShape<NP, NQ>::NC, &gemm_digits_launch<NP, NQ>}
+#define ZKD_INST(NP, NQ) {NP, NQ, GemmShape<NP, NQ>::LOW, GemmShape<NP, NQ>::NC, &gemm_digits_launch<NP, NQ, 16>, &gemm_digits_launch<NP, NQ, 8>}
 extern const GemmInstance kGemmInstQ18[] = {
     ZKD_INST(18, 18),
     ZKD_INST(24, 18),

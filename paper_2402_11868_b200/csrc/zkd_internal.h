@@ -42,6 +42,7 @@ struct Options {
   int tol_bits = 770;
   int max_steps = 120;
   int gemm_path = 0;
+  int gemm_tile = 0;         // IMAD digit GEMM: 0 automatic (8 x 8 x 8 tiles where 16-wide tiles fill badly), 8, 16
   int min_split_ctas = 296;  // split K until a product has about this many CTAs (two per SM), see pick_splits
   int seed_sweeps = 12;
   int seed_cluster = 0;  // ring seed: largest cluster size to use (0 = 16, falling back to 8 when refused)

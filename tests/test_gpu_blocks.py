@@ -125,6 +125,17 @@ def test_gemm_fx_epilogues_match_python_integers(zkd, case, combine):
 
 
 @pytest.mark.parametrize("case", GEMM_CASES)
+@pytest.mark.parametrize("tile", [8, 16])
+def test_gemm_fx_tile_sizes_match_python_integers(zkd, case, tile):
+    """the IMAD kernel built with 8 x 8 x 8 and with 16 x 16 x 16 tiles (option gemm_tile; automatic by tile fill otherwise)"""
+    zkd.set_option("gemm_tile", tile)
+    try:
+        test_gemm_fx_matches_python_integers(zkd, case, path=1)
+    finally:
+        zkd.set_option("gemm_tile", 0)
+
+
+@pytest.mark.parametrize("case", GEMM_CASES)
 def test_gemm_fx_matches_python_integers(zkd, case, path=1):
     import torch
 
