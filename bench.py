@@ -193,6 +193,9 @@ def load_traffic(workload: str) -> dict:
         return {}
 
 
+I8_MMA_PEAK = None  # int8 op/s, measured live in main()
+
+
 def roofline_objects(cats: dict, seed_elems, imad_peak, dfma_peak, steps, total_ms, workload) -> list[dict]:
     """One roofline object per kernel category that took part, largest share of the step first.
     achieved = ALGORITHMIC work of the launches / their summed CUDA-event time; achieved_executed = the same with the
@@ -221,6 +224,12 @@ def roofline_objects(cats: dict, seed_elems, imad_peak, dfma_peak, steps, total_
                 peak, src = 4500.0, "fallback: nominal dense int8 4.5 POP/s (B200_PROFILING.md); MEASURED_PEAKS.json absent"
             o.update({"bound": "tensor", "unit": "TOP/s (int8)", "achieved": 2.0 * walg / sec / 1e12,
                       "achieved_executed": 2.0 * wexec / sec / 1e12, "peak": peak, "work_per_step": walg / steps, "peak_source": src})
+            if I8_MMA_PEAK:
+                # the peak above is cuBLAS bf16 x the nominal int8 : bf16 ratio, which this kernel can exceed; the live
+                # figure is the issue rate of the kernel's own MMA shape with operands resident in shared memory
+                o.update({"mma_issue_peak": I8_MMA_PEAK / 1e12, "frac_of_mma_issue_peak": o["achieved"] / (I8_MMA_PEAK / 1e12),
+                          "mma_issue_peak_source": "measured live (zkd_measure_i8_mma_peak): tcgen05.mma kind::i8 128x128x32, "
+                                                   "one CTA per SM, no loads"})
         elif name == "seed_fp64":
             chk, rot = seed_elems
             flops = 2.0 * (8.0 * chk + 12.0 * rot)
@@ -440,6 +449,8 @@ def main():
     # ---- rooflines: every kernel category of the step, measured peaks ------------------------------------------------
     imad_peak = z.measure_imad_peak(60.0)  # register-only IMAD.WIDE loop on all SMs
     dfma_peak = z.measure_dfma_peak(40.0)  # register-only DFMA loop on all SMs
+    global I8_MMA_PEAK
+    I8_MMA_PEAK = z.measure_i8_mma_peak(30.0)  # resident-operand tcgen05.mma kind::i8 loop on all SMs
     roofs = roofline_objects(cats, seed_elems, imad_peak, dfma_peak, args.steps, total_ms, args.workload)
     listed = [r for r in roofs if r["share_of_step"] >= 0.02]
 

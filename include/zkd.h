@@ -284,6 +284,10 @@ int zkd_seed_fp64(int N, int batch, const double *A64, double *mu, double *V, vo
 int zkd_measure_imad_peak(double millis, double *imad_wide_per_sec, void *stream);
 /* Measured fp64 peak (roofline denominator of the seed): register-only DFMA loop on every SM; returns flop/s (2 per FMA). */
 int zkd_measure_dfma_peak(double millis, double *fp64_flops_per_sec, void *stream);
+/* Measured issue peak of the int8 tensor-core shape S4b uses (tcgen05.mma kind::i8, 128 x 128 x 32, one CTA per SM, operands
+ * resident in shared memory, no loads): returns int8 op/s (2 per multiply-add).  Reported by bench.py beside the bf16-derived
+ * peak of MEASURED_PEAKS.json. */
+int zkd_measure_i8_mma_peak(double millis, double *int8_ops_per_sec, void *stream);
 
 #ifdef __cplusplus
 }

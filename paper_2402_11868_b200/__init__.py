@@ -82,6 +82,7 @@ def lib() -> ctypes.CDLL:
     L.zkd_seed_fp64.argtypes = [ci, ci, vp, vp, vp, vp]
     L.zkd_measure_imad_peak.argtypes = [cd, ctypes.POINTER(cd), vp]
     L.zkd_measure_dfma_peak.argtypes = [cd, ctypes.POINTER(cd), vp]
+    L.zkd_measure_i8_mma_peak.argtypes = [cd, ctypes.POINTER(cd), vp]
     L.zkd_seed_stats.argtypes = [ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint64), ci]
     L.zkd_kernel_timing_categories.restype = ci
     L.zkd_kernel_timing_name.restype = ctypes.c_char_p
@@ -364,6 +365,12 @@ def measure_imad_peak(millis: float = 50.0, stream=None) -> float:
     v = ctypes.c_double()
     _check(lib().zkd_measure_imad_peak(millis, ctypes.byref(v), _stream_ptr(stream)), "zkd_measure_imad_peak")
     return v.value
+
+
+def measure_i8_mma_peak(millis: float = 50.0, stream=None) -> float:
+    v = ctypes.c_double()
+    _check(lib().zkd_measure_i8_mma_peak(millis, ctypes.byref(v), _stream_ptr(stream)), "zkd_measure_i8_mma_peak")
+    return float(v.value)
 
 
 def measure_dfma_peak(millis: float = 50.0, stream=None) -> float:

@@ -223,6 +223,7 @@ static int* option_slot(const char* key) {
   if (!strcmp(key, "sstep_warp")) return &o.sstep_warp;
   if (!strcmp(key, "combine_path")) return &o.combine_path;
   if (!strcmp(key, "cluster_tiles")) return &o.cluster_tiles;
+  if (!strcmp(key, "i8_step")) return &o.i8_step;
   if (!strcmp(key, "block_correction")) return &o.block_correction;
   if (!strcmp(key, "verbose")) return &o.verbose;
   return nullptr;
@@ -342,6 +343,11 @@ int zkd_measure_imad_peak(double millis, double* imad_wide_per_sec, void* stream
   if (!imad_wide_per_sec || !(millis > 0)) return ZKD_ERR_INVALID_ARG;
   ZKD_TRY(check_device());
   return measure_imad_peak(millis, imad_wide_per_sec, (cudaStream_t)stream);
+}
+
+int zkd_measure_i8_mma_peak(double millis, double* int8_ops_per_sec, void* stream) {
+  if (!int8_ops_per_sec || !(millis > 0) || millis > 10000) return ZKD_ERR_INVALID_ARG;
+  return measure_i8_mma_peak(millis, int8_ops_per_sec, (cudaStream_t)stream);
 }
 
 int zkd_measure_dfma_peak(double millis, double* fp64_flops_per_sec, void* stream) {

@@ -25,10 +25,11 @@ namespace {
 
 constexpr int I8_BM = 128, I8_BN = 128, I8_BK = 128;  // BK in int8 elements = bytes = one 128B swizzle row
 constexpr int I8_D = 4;                               // accumulators (columns d) per CTA: 4 x 128 TMEM columns
-constexpr int I8_RP = 3, I8_RQ = 6;                   // ring depths (tiles of 16 KB)
+// ring depths (tiles of 16 KB) are template parameters <RP, RQ>: a step keeps 1 P tile and up to 4 Q tiles live, so the
+// producer runs RP - 1 / RQ - 4 steps ahead of the MMAs
 constexpr int I8_TILE_BYTES = I8_BM * I8_BK;          // 16384
 constexpr int I8_THREADS = 192;                       // warps 0-3 epilogue, 4 TMA producer, 5 MMA issuer
-constexpr size_t I8_SMEM = (size_t)(I8_RP + I8_RQ) * I8_TILE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+constexpr size_t i8_smem(int rp, int rq) { return (size_t)(rp + rq) * I8_TILE_BYTES + 1024 /*align*/ + 512 /*barriers*/; }
 
 // ---- PTX wrappers --------------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -75,6 +76,13 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
   d |= (uint64_t)1 << 46;                       // descriptor version (sm_100)
   d |= (uint64_t)2 << 61;                       // SWIZZLE_128B
   return d;
+}
+// one lane of a converged warp; unlike "lane == 0" the compiler knows the branch holds exactly one thread, so tcgen05 / TMA
+// instructions inside it are issued straight from uniform registers (no per-instruction election loop)
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.b32 %0, 1, 0, P;\n\t}" : "=r"(pred));
+  return pred != 0;
 }
 __device__ __forceinline__ void tmem_ld_32x32b_x32(uint32_t taddr, uint32_t (&v)[32]) {
   asm volatile(
@@ -168,18 +176,26 @@ __device__ __forceinline__ GroupRange group_range(const I8Args& a, int dg) {
   return r;
 }
 
+// One CTA = one 128 x 128 output tile x D columns.  Work proceeds in macro-steps of S consecutive slices a of one K block:
+// the producer loads the S P tiles and the (at most S, or S + D - 1 at the start of a K block) new Q tiles of the window under
+// ONE transaction barrier, the issuing thread waits once, issues up to S x D x 4 MMAs back to back and commits ONCE; the
+// producer learns from that commit which macro-steps are complete and reuses the slots of the tiles that died in them.  (The
+// issuing thread's waits and commits are not hidden behind the MMAs - the tensor pipe's queue is short - so the count of
+// barrier operations per MMA is what sets the kernel's speed: see profiles/r02_summary.md.)
+constexpr int I8_RF = 8;  // transaction ("full") and completion ("done") barrier rings, indexed by macro-step
+
+template <int I8_RP, int I8_RQ, int I8_S>
 __global__ void __launch_bounds__(I8_THREADS, 1)
 gemm_i8_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__ CUtensorMap mapQ, const I8Args a) {
+  static_assert(I8_RQ >= I8_S + I8_D - 1 + I8_S && I8_RP >= 2 * I8_S && I8_RP < I8_RF, "ring depths");
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   uint8_t* p_tiles = smem;                                  // [RP][16 KB]
   uint8_t* q_tiles = smem + (size_t)I8_RP * I8_TILE_BYTES;  // [RQ][16 KB]
   uint64_t* bars = (uint64_t*)(smem + (size_t)(I8_RP + I8_RQ) * I8_TILE_BYTES);
-  uint64_t* full_p = bars;
-  uint64_t* empty_p = bars + I8_RP;
-  uint64_t* full_q = bars + 2 * I8_RP;
-  uint64_t* empty_q = bars + 2 * I8_RP + I8_RQ;
-  uint64_t* tmem_full = bars + 2 * I8_RP + 2 * I8_RQ;
+  uint64_t* full = bars;            // [RF] all tiles of macro-step m have landed
+  uint64_t* done = bars + I8_RF;    // [RF] all MMAs of macro-step m have completed
+  uint64_t* tmem_full = bars + 2 * I8_RF;
   uint32_t* tmem_base_slot = (uint32_t*)(tmem_full + 1);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -191,10 +207,10 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__
   const int g = z / a.nsplit;
   const GroupRange gr = group_range(a, dg);
   const int kb0 = sp * a.kb_per_split, kb1 = min(a.nkb, kb0 + a.kb_per_split);
+  const int nm = (gr.nA + I8_S - 1) / I8_S;  // macro-steps per K block
 
   if (threadIdx.x == 0) {
-    for (int i = 0; i < I8_RP; ++i) { mbar_init(full_p + i, 1); mbar_init(empty_p + i, 1); }
-    for (int i = 0; i < I8_RQ; ++i) { mbar_init(full_q + i, 1); mbar_init(empty_q + i, 1); }
+    for (int i = 0; i < I8_RF; ++i) { mbar_init(full + i, 1); mbar_init(done + i, 1); }
     mbar_init(tmem_full, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -210,71 +226,80 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__
 
   if (warp == 4) {
     // ===== TMA producer =====
-    if (lane == 0) {
-      uint32_t pseq = 0, qseq = 0;
+    if (elect_one()) {
+      int pdeath[I8_RP], qdeath[I8_RQ];  // macro-step in which the tile now in the slot is used last
+      for (int i = 0; i < I8_RP; ++i) pdeath[i] = -1;
+      for (int i = 0; i < I8_RQ; ++i) qdeath[i] = -1;
+      int known_done = -1;  // macro-steps <= known_done are complete
+      auto wait_done = [&](int upto) {
+        while (known_done < upto) {
+          ++known_done;
+          mbar_wait(done + (known_done % I8_RF), (uint32_t)(known_done / I8_RF) & 1u);
+        }
+      };
+      int M = 0;
+      uint32_t pslot = 0, qslot = 0;
       for (int kb = kb0; kb < kb1; ++kb) {
         int q_next = gr.b_max;
-        for (int aa = gr.a_min; aa <= gr.a_max; ++aa) {
-          const int lowest = max(gr.b_min, gr.d0 - aa);
+        for (int m = 0; m < nm; ++m, ++M) {
+          const int aa0 = gr.a_min + m * I8_S, aa1 = min(gr.a_max, aa0 + I8_S - 1);
+          const int lowest = max(gr.b_min, gr.d0 - aa1);
+          const int nq_new = max(0, q_next - lowest + 1), np_new = aa1 - aa0 + 1;
+          uint64_t* fb = full + (M % I8_RF);
+          mbar_expect_tx(fb, (uint32_t)nq_new * a.q_tile_bytes + (uint32_t)np_new * a.p_tile_bytes);
           while (q_next >= lowest) {
-            const uint32_t s = qseq % I8_RQ, ph = (qseq / I8_RQ) & 1;
-            mbar_wait(empty_q + s, ph ^ 1);
-            mbar_expect_tx(full_q + s, a.q_tile_bytes);
-            tma_load_3d(q_tiles + (size_t)s * I8_TILE_BYTES, &mapQ, full_q + s, kb * I8_BK, j0, g * a.nsQ + q_next);
-            ++qseq;
+            wait_done(qdeath[qslot]);
+            tma_load_3d(q_tiles + (size_t)qslot * I8_TILE_BYTES, &mapQ, fb, kb * I8_BK, j0, g * a.nsQ + q_next);
+            // Q_b is used last by the slice a = d0 + D - 1 - b (the group's highest column), clipped to the K block's range
+            qdeath[qslot] = M - m + (min(gr.a_max, gr.d0 + I8_D - 1 - q_next) - gr.a_min) / I8_S;
+            qslot = qslot + 1 == I8_RQ ? 0 : qslot + 1;
             --q_next;
           }
-          const uint32_t s = pseq % I8_RP, ph = (pseq / I8_RP) & 1;
-          mbar_wait(empty_p + s, ph ^ 1);
-          mbar_expect_tx(full_p + s, a.p_tile_bytes);
-          tma_load_3d(p_tiles + (size_t)s * I8_TILE_BYTES, &mapP, full_p + s, kb * I8_BK, i0, g * a.nsP + aa);
-          ++pseq;
+          for (int aa = aa0; aa <= aa1; ++aa) {
+            wait_done(pdeath[pslot]);
+            tma_load_3d(p_tiles + (size_t)pslot * I8_TILE_BYTES, &mapP, fb, kb * I8_BK, i0, g * a.nsP + aa);
+            pdeath[pslot] = M;
+            pslot = pslot + 1 == I8_RP ? 0 : pslot + 1;
+          }
         }
       }
     }
   } else if (warp == 5) {
     // ===== MMA issuer =====
-    if (lane == 0) {
+    if (elect_one()) {
       // S32 accumulate, S8 x S8, both K-major, M = 128, N = 128
       constexpr uint32_t idesc = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(I8_BN >> 3) << 17) | ((uint32_t)(I8_BM >> 4) << 24);
+      const uint32_t p_base = smem_u32(p_tiles), q_base = smem_u32(q_tiles);
       uint32_t started = 0;
-      uint32_t pseq = 0;
+      uint32_t pslot = 0;
+      int M = 0;
       for (int kb = kb0; kb < kb1; ++kb) {
-        const uint32_t qbase = (uint32_t)(kb - kb0) * gr.nQ;  // sequence number of tile b_max of this K block
-        int q_next = gr.b_max;
-        for (int aa = gr.a_min; aa <= gr.a_max; ++aa) {
-          const int lowest = max(gr.b_min, gr.d0 - aa);
-          while (q_next >= lowest) {
-            const uint32_t qs = qbase + (gr.b_max - q_next);
-            mbar_wait(full_q + qs % I8_RQ, (qs / I8_RQ) & 1);
-            --q_next;
-          }
-          const uint32_t s = pseq % I8_RP;
-          mbar_wait(full_p + s, (pseq / I8_RP) & 1);
+        // ring slot of tile b_max of this K block (tiles enter the ring in the order b_max, b_max - 1, ...)
+        const uint32_t qslot0 = (uint32_t)(((long long)(kb - kb0) * gr.nQ) % I8_RQ);
+        for (int m = 0; m < nm; ++m, ++M) {
+          const int aa0 = gr.a_min + m * I8_S, aa1 = min(gr.a_max, aa0 + I8_S - 1);
+          mbar_wait(full + (M % I8_RF), (uint32_t)(M / I8_RF) & 1u);
           asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-          const uint32_t pa = smem_u32(p_tiles + (size_t)s * I8_TILE_BYTES);
+          for (int aa = aa0; aa <= aa1; ++aa) {
+            const uint32_t pa = p_base + pslot * I8_TILE_BYTES;
+            // slot of Q_b, b = d0 + dd - aa: (qslot0 + b_max - b) mod RQ
+            const uint32_t s0 = (qslot0 + (uint32_t)(gr.b_max - (gr.d0 - aa) + I8_RQ * 16)) % I8_RQ;  // dd = 0 (b may lie outside the range)
 #pragma unroll
-          for (int dd = 0; dd < I8_D; ++dd) {
-            const int b = gr.d0 + dd - aa;
-            if (b < gr.b_min || b > gr.b_max) continue;
-            const uint32_t qs = qbase + (gr.b_max - b);
-            const uint32_t qa = smem_u32(q_tiles + (size_t)(qs % I8_RQ) * I8_TILE_BYTES);
+            for (int dd = 0; dd < I8_D; ++dd) {
+              const int b = gr.d0 + dd - aa;
+              if (b < gr.b_min || b > gr.b_max) continue;
+              const uint32_t sq = s0 >= (uint32_t)dd ? s0 - dd : s0 + I8_RQ - dd;
+              const uint32_t qa = q_base + sq * I8_TILE_BYTES;
 #pragma unroll
-            for (int k = 0; k < I8_BK / 32; ++k) {
-              umma_i8(tmem_base + dd * I8_BN, umma_desc_sw128(pa + k * 32), umma_desc_sw128(qa + k * 32), idesc,
-                      ((started >> dd) & 1) | (k > 0));
+              for (int k = 0; k < I8_BK / 32; ++k) {
+                umma_i8(tmem_base + dd * I8_BN, umma_desc_sw128(pa + k * 32), umma_desc_sw128(qa + k * 32), idesc,
+                        ((started >> dd) & 1) | (k > 0));
+              }
+              started |= 1u << dd;
             }
-            started |= 1u << dd;
+            pslot = pslot + 1 == I8_RP ? 0 : pslot + 1;
           }
-          umma_commit(empty_p + s);
-          ++pseq;
-          // Q tiles that no later step of this K block uses
-          const int dead_hi = gr.d0 + I8_D - 1 - aa;
-          const int dead_lo = (aa == gr.a_max) ? gr.b_min : dead_hi;
-          for (int b = min(dead_hi, gr.b_max); b >= max(dead_lo, gr.b_min); --b) {
-            const uint32_t qs = qbase + (gr.b_max - b);
-            umma_commit(empty_q + qs % I8_RQ);
-          }
+          umma_commit(done + (M % I8_RF));
         }
       }
       umma_commit(tmem_full);
@@ -288,17 +313,12 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__
     for (int dd = 0; dd < I8_D; ++dd) {
       const int c = I8_D * dg + dd;  // column index relative to dcut
       if (c >= a.ncol) break;
+      // every kept column d <= nsP + nsQ - 2 receives at least one slice pair, so its accumulator has been written
       int32_t* o = a.out + ((size_t)(sp * a.G + g) * a.ncol + c) * mn + (size_t)i * a.N + j0;
-      const bool has = true;  // every kept column d <= nsP + nsQ - 2 receives at least one slice pair
 #pragma unroll 1
       for (int cc = 0; cc < I8_BN; cc += 32) {
         uint32_t v[32];
-        if (has) {
-          tmem_ld_32x32b_x32(tmem_base + ((uint32_t)(warp * 32) << 16) + dd * I8_BN + cc, v);
-        } else {
-#pragma unroll
-          for (int t = 0; t < 32; ++t) v[t] = 0;
-        }
+        tmem_ld_32x32b_x32(tmem_base + ((uint32_t)(warp * 32) << 16) + dd * I8_BN + cc, v);
         if (i < a.M) {
           if (j0 + cc + 32 <= a.N && (a.N & 3) == 0) {
 #pragma unroll
@@ -321,6 +341,98 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__
 }
 
 }  // namespace
+
+namespace {
+
+// ---- measured issue peak of the MMA shape the kernel uses (roofline denominator next to the bf16-derived one) ----------
+// One CTA per SM, operands resident in shared memory (no TMA), one elected thread issuing 128 x 128 x 32 kind::i8 MMAs back
+// to back into four accumulators exactly as gemm_i8_kernel does, one commit at the end.
+__global__ void __launch_bounds__(128, 1) i8_peak_kernel(int niter) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  uint64_t* bar = (uint64_t*)(smem + 5 * I8_TILE_BYTES);
+  uint32_t* slot = (uint32_t*)(bar + 1);
+  for (int i = threadIdx.x; i < 5 * I8_TILE_BYTES / 4; i += blockDim.x) ((uint32_t*)smem)[i] = ((uint32_t)i * 2654435761u) ^ ((uint32_t)i >> 3);
+  if (threadIdx.x == 0) {
+    mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  const int warp = threadIdx.x >> 5;
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(slot)), "n"(512));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t tm = *slot;
+  if (warp == 0) {
+    if (elect_one()) {
+      constexpr uint32_t idesc = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(I8_BN >> 3) << 17) | ((uint32_t)(I8_BM >> 4) << 24);
+      const uint32_t pa = smem_u32(smem), qa = pa + I8_TILE_BYTES;
+      for (int it = 0; it < niter; ++it) {
+#pragma unroll
+        for (int dd = 0; dd < I8_D; ++dd) {
+#pragma unroll
+          for (int k = 0; k < I8_BK / 32; ++k)
+            umma_i8(tm + dd * I8_BN, umma_desc_sw128(pa + k * 32), umma_desc_sw128(qa + dd * I8_TILE_BYTES + k * 32), idesc, 1);
+        }
+      }
+      umma_commit(bar);
+      mbar_wait(bar, 0);
+    }
+    __syncwarp();
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (warp == 0) {
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm), "n"(512));
+  }
+}
+
+}  // namespace
+
+int measure_i8_mma_peak(double millis, double* ops_per_sec, cudaStream_t s) {
+  int dev = 0, sms = 0;
+  ZKD_CUDA_TRY(cudaGetDevice(&dev));
+  ZKD_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const size_t smem = 5 * (size_t)I8_TILE_BYTES + 1024 + 64;
+  ZKD_CUDA_TRY(cudaFuncSetAttribute(i8_peak_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  cudaEvent_t e0, e1;
+  ZKD_CUDA_TRY(cudaEventCreate(&e0));
+  ZKD_CUDA_TRY(cudaEventCreate(&e1));
+  int iters = 2000;
+  double best = 0;
+  const int reps = millis > 20 ? 5 : 3;
+  int rc = ZKD_OK;
+  i8_peak_kernel<<<sms, 128, smem, s>>>(100);  // warm-up
+  for (int r = 0; r < reps + 1; ++r) {
+    cudaEventRecord(e0, s);
+    i8_peak_kernel<<<sms, 128, smem, s>>>(iters);
+    cudaEventRecord(e1, s);
+    if (cudaEventSynchronize(e1) != cudaSuccess) {
+      (void)cudaGetLastError();
+      rc = ZKD_ERR_CUDA;
+      break;
+    }
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double ops = 2.0 * I8_BM * I8_BN * 32.0 * (I8_BK / 32) * I8_D * (double)iters * sms;
+    if (r > 0 && ops / (ms * 1e-3) > best) best = ops / (ms * 1e-3);
+    if (r == 0 && ms > 0) {
+      double scale = (millis / reps) / ms;
+      if (scale > 50) scale = 50;
+      if (scale < 0.05) scale = 0.05;
+      iters = (int)(iters * scale) + 1;
+    }
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (rc == ZKD_OK) *ops_per_sec = best;
+  return rc;
+}
 
 namespace {
 
@@ -546,7 +658,11 @@ int gemm_i8_finish(int M, int N, int K, int batch, const int32_t* Pc, const int3
   ka.nsplit = (ka.nkb + ka.kb_per_split - 1) / ka.kb_per_split;
   ka.p_tile_bytes = (uint32_t)boxP * I8_BK;
   ka.q_tile_bytes = (uint32_t)boxQ * I8_BK;
-  ZKD_CUDA_TRY(cudaFuncSetAttribute(gemm_i8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)I8_SMEM));  // per device, cheap
+  // macro-step of 2 slices with rings <4, 9> by default; i8_step = 1: one slice per step, rings <5, 8>
+  const bool step1 = options().i8_step == 1;
+  auto kern = step1 ? gemm_i8_kernel<5, 8, 1> : gemm_i8_kernel<4, 9, 2>;
+  const size_t smem = i8_smem(4, 9);
+  ZKD_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));  // per device, cheap
   const dim3 grid((N + I8_BN - 1) / I8_BN, (M + I8_BM - 1) / I8_BM, (unsigned)(G * ka.nsplit * ka.ngroups));
   if (grid.z > 65535) return ZKD_ERR_INTERNAL;
   // int8 MACs actually issued: every (a, b) pair with a + b >= dcut, on full 128 x 128 x 128 blocks
@@ -558,7 +674,7 @@ int gemm_i8_finish(int M, int N, int K, int batch, const int32_t* Pc, const int3
   {
     // algorithmic: the same slice pairs on the matrices as they are (no padding of M, N, K to 128)
     KtScope kt(KC_GEMM_I8, stream, macs, pairs * (uint64_t)G * M * N * K);
-    gemm_i8_kernel<<<grid, I8_THREADS, I8_SMEM, stream>>>(mapP, mapQ, ka);
+    kern<<<grid, I8_THREADS, smem, stream>>>(mapP, mapQ, ka);
   }
   count_launch();
   count_i8_macs(macs);

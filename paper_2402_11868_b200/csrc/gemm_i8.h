@@ -15,5 +15,7 @@ int gemm_i8_finish(int M, int N, int K, int batch, const int32_t* Pc, const int3
 void kernel_timing_enable_i8(bool on);
 int kernel_timing_read_i8(double* ms, uint64_t* launches, uint64_t* i8_macs);
 void count_i8_macs(uint64_t n);
+// issue peak of the kernel's MMA shape (128 x 128 x 32 kind::i8, one CTA per SM, operands resident): int8 op/s
+int measure_i8_mma_peak(double millis, double* ops_per_sec, cudaStream_t s);
 
 }  // namespace zkd

@@ -300,6 +300,12 @@ def test_measured_imad_peak_is_plausible(zkd):
     assert 148 * 28 * 1.0e9 < p < 148 * 33 * 2.1e9, p
 
 
+def test_measured_i8_mma_peak_is_plausible(zkd):
+    p = zkd.measure_i8_mma_peak(20.0)
+    # 128 x 128 x 32 kind::i8 per >= 64 clocks per SM: at most 148 x 16384 op/clk x 2.1 GHz; at least half of that at 1 GHz
+    assert 148 * 8192 * 1.0e9 < p < 148 * 16384 * 2.1e9 * 1.02, p
+
+
 def test_measured_dfma_peak_is_plausible(zkd):
     p = zkd.measure_dfma_peak(30.0)
     # fp64 FMA: 148 SMs x (32 .. 64 lanes/clk) x 2 flop x (1.0 .. 2.1 GHz)
