@@ -42,9 +42,11 @@ extern "C" {
 #define ZKD_ERR_CUDA (-4)             /* a CUDA call failed (the sticky error is cleared) */
 #define ZKD_ERR_ARCH (-5)             /* device is not sm_100 */
 #define ZKD_ERR_CLUSTERED (-7)        /* zkd_diag_herm_rqi_lu only: the spectrum has clusters, which per-vector RQI cannot separate */
+#define ZKD_ERR_STATIC_LIMIT (-8)     /* zkd_seed_fp64_static only: N > ZKD_SEED_STATIC_MAX_N (its scratch is a fixed device array) */
 #define ZKD_ERR_INTERNAL (-6)         /* internal consistency check failed (window overflow that could not be repaired) */
 
 #define ZKD_MAX_N 2048
+#define ZKD_SEED_STATIC_MAX_N 512 /* largest N of zkd_seed_fp64_static */
 
 /* Per-matrix outcome, written to device memory by the call (one record per matrix of the batch).
  * status, n_clusters, max_cluster, log2_resid and log2_orth are per matrix.  `steps` is per CALL: the refinement loop runs
@@ -278,6 +280,17 @@ int zkd_gemm_fx(int M, int N, int K, int batch, int op_a, const int32_t *A_fx, i
  * Hermitian eigendecomposition of batch N x N matrices given as complex doubles (row-major,
  * interleaved re/im); mu ascending, V[i][j] = component i of vector j. */
 int zkd_seed_fp64(int N, int batch, const double *A64, double *mu, double *V, void *stream);
+/* The same seed for callers that must not allocate (code under CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): same arguments, layouts and result as zkd_seed_fp64, but the call makes no cudaMalloc / cudaFree / event or
+ * stream creation.  zkd_seed_fp64 keeps G = A + sigma I (N^2 complex doubles), sigma, the unsorted eigenvalues and the sweep
+ * flags in a cudaMalloc'ed buffer when N > 256; this entry point runs that same blocked one-sided Jacobi kernel for every
+ * 1 <= N <= ZKD_SEED_STATIC_MAX_N (= 512) with that scratch in a static __device__ array of 4 MiB + 8 KiB, which every GPU that
+ * loads libzkd.so holds until the process exits.  Errors: ZKD_ERR_STATIC_LIMIT for N > 512 (nothing is launched),
+ * ZKD_ERR_INVALID_ARG, ZKD_ERR_ARCH, ZKD_ERR_CUDA.  A64, mu, V: device pointers owned by the caller; the batch is processed
+ * one matrix at a time on `stream`.  ALL calls on a device share the one array: calls on the same stream are ordered and
+ * safe, calls that overlap on the GPU (different streams, different host threads without ordering) race on it and give
+ * undefined results.  The array keeps the previous call's contents; the call clears what has to start at zero itself. */
+int zkd_seed_fp64_static(int N, int batch, const double *A64, double *mu, double *V, void *stream);
 
 /* Measured integer-multiply peak: runs a register-only IMAD.WIDE loop on every SM for about `millis`
  * milliseconds and returns wide (32x32+64) multiply-adds per second (host double). */

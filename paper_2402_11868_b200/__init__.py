@@ -80,6 +80,7 @@ def lib() -> ctypes.CDLL:
     L.zkd_gemm_fx_bufsize.argtypes = [ci, ci, ci, ci, ctypes.POINTER(cs)]
     L.zkd_gemm_fx.argtypes = [ci, ci, ci, ci, ci, vp, ci, ci, vp, ci, ci, vp, ci, ci, ci, vp, cs, vp, vp, vp]
     L.zkd_seed_fp64.argtypes = [ci, ci, vp, vp, vp, vp]
+    L.zkd_seed_fp64_static.argtypes = [ci, ci, vp, vp, vp, vp]
     L.zkd_measure_imad_peak.argtypes = [cd, ctypes.POINTER(cd), vp]
     L.zkd_measure_dfma_peak.argtypes = [cd, ctypes.POINTER(cd), vp]
     L.zkd_measure_i8_mma_peak.argtypes = [cd, ctypes.POINTER(cd), vp]
@@ -359,6 +360,15 @@ def gemm_fx(M, N, K, batch, op_a, A_fx, a_top_bit, a_digits, B_fx, b_top_bit, b_
 def seed_fp64(N: int, batch: int, A64, mu, V, stream=None) -> None:
     _check(lib().zkd_seed_fp64(N, batch, _dev_u8(A64, batch * N * N * 16, "A64"), _dev_u8(mu, batch * N * 8, "mu"),
                                _dev_u8(V, batch * N * N * 16, "V"), _stream_ptr(stream)), "zkd_seed_fp64")
+
+
+SEED_STATIC_MAX_N = 512
+
+
+def seed_fp64_static(N: int, batch: int, A64, mu, V, stream=None) -> None:
+    """zkd_seed_fp64 without any allocation (scratch in a static device array; N <= SEED_STATIC_MAX_N)"""
+    _check(lib().zkd_seed_fp64_static(N, batch, _dev_u8(A64, batch * N * N * 16, "A64"), _dev_u8(mu, batch * N * 8, "mu"),
+                                      _dev_u8(V, batch * N * N * 16, "V"), _stream_ptr(stream)), "zkd_seed_fp64_static")
 
 
 def measure_imad_peak(millis: float = 50.0, stream=None) -> float:

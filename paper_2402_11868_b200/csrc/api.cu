@@ -184,6 +184,7 @@ const char* zkd_strerror(int code) {
     case ZKD_ERR_ARCH: return "device is not sm_100";
     case ZKD_ERR_INTERNAL: return "internal consistency check failed";
     case ZKD_ERR_CLUSTERED: return "clustered spectrum: exact per-vector RQI does not apply";
+    case ZKD_ERR_STATIC_LIMIT: return "size exceeds the static scratch of the no-allocation entry point (N <= 512)";
     default: return "unknown error";
   }
 }
@@ -338,6 +339,12 @@ int zkd_seed_fp64(int N, int batch, const double* A64, double* mu, double* V, vo
   if (N < 1 || N > ZKD_MAX_N || batch < 1 || !A64 || !mu || !V) return ZKD_ERR_INVALID_ARG;
   ZKD_TRY(check_device());
   return seed_fp64(N, batch, A64, mu, V, options().seed_sweeps, (cudaStream_t)stream);
+}
+int zkd_seed_fp64_static(int N, int batch, const double* A64, double* mu, double* V, void* stream) {
+  if (N < 1 || batch < 1 || !A64 || !mu || !V) return ZKD_ERR_INVALID_ARG;
+  if (N > ZKD_SEED_STATIC_MAX_N) return ZKD_ERR_STATIC_LIMIT;
+  ZKD_TRY(check_device());
+  return seed_fp64_static(N, batch, A64, mu, V, options().seed_sweeps, (cudaStream_t)stream);
 }
 int zkd_measure_imad_peak(double millis, double* imad_wide_per_sec, void* stream) {
   if (!imad_wide_per_sec || !(millis > 0)) return ZKD_ERR_INVALID_ARG;

@@ -17,10 +17,21 @@
 // The seed only has to be good to ~2^-40 (the refinement squares the error every step).
 #include <cooperative_groups.h>
 
+#include <mutex>
+
 #include "timing.h"
 #include "zkd_internal.h"
 
 namespace cg = cooperative_groups;
+
+// Scratch of zkd_seed_fp64_static (the entry point that allocates nothing; bottom of this file): the rotated matrix G of one
+// N x N problem, N <= ZKD_SEED_STATIC_MAX_N = 512 (4 MiB of complex doubles), followed by sigma, the unsorted eigenvalues and
+// the sweep flags (8 KiB).  Every GPU that loads the library holds these 4 MiB + 8 KiB until the process exits.  In host code
+// this name is a host-side stand-in, not a device address: host code takes the address with cudaGetSymbolAddress, once per
+// device (seed_static_scratch below).
+constexpr size_t kSeedStaticGBytes = sizeof(double2) * (size_t)ZKD_SEED_STATIC_MAX_N * ZKD_SEED_STATIC_MAX_N;
+constexpr size_t kSeedStaticBytes = kSeedStaticGBytes + 8192;
+static __device__ __align__(256) unsigned char g_seed_static_scratch[kSeedStaticBytes];
 
 namespace zkd {
 
@@ -1205,6 +1216,68 @@ int seed_stats(uint64_t* elems_checked, uint64_t* elems_rotated, bool reset) {
     ZKD_CUDA_TRY(cudaMemcpyToSymbol(g_seed_stats, z, sizeof(z)));
   }
   return ZKD_OK;
+}
+
+// ---- the seed without any allocation (zkd_seed_fp64_static, include/zkd.h) ----------------------------------------------
+// For callers that cannot call cudaMalloc (stream capture, serving loops, harnesses that forbid it).  Same kernels as the
+// large-matrix branch of seed_fp64 above (seed_sigma_kernel, seed_block_kernel<8, 8>, seed_sort_kernel), for every N up to
+// ZKD_SEED_STATIC_MAX_N, one matrix of the batch at a time, with G / sigma / unsorted eigenvalues / sweep flags in
+// g_seed_static_scratch instead of a cudaMalloc'ed buffer.  No cudaMalloc, cudaFree, event or stream creation in here.
+namespace {
+
+constexpr int kSeedStaticMaxDevices = 64;
+
+// device address of g_seed_static_scratch on the CURRENT device: looked up once per device, with that device current
+int seed_static_scratch(unsigned char** out) {
+  static unsigned char* addr[kSeedStaticMaxDevices] = {};
+  static std::mutex mu;
+  int dev = 0;
+  ZKD_CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kSeedStaticMaxDevices) return ZKD_ERR_INVALID_ARG;
+  std::lock_guard<std::mutex> lk(mu);
+  if (!addr[dev]) {
+    unsigned char* p = nullptr;
+    if (cudaGetSymbolAddress((void**)&p, g_seed_static_scratch) != cudaSuccess || !p) {
+      (void)cudaGetLastError();
+      return ZKD_ERR_CUDA;
+    }
+    addr[dev] = p;
+  }
+  *out = addr[dev];
+  return ZKD_OK;
+}
+
+}  // namespace
+
+int seed_fp64_static(int N, int batch, const double* A64, double* mu, double* V, int max_sweeps, cudaStream_t s) {
+  if (N > ZKD_SEED_STATIC_MAX_N) return ZKD_ERR_STATIC_LIMIT;
+  const double tol = ldexp(1.0, -50);
+  int dev = 0, sms = 0;
+  ZKD_CUDA_TRY(cudaGetDevice(&dev));
+  ZKD_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  unsigned char* buf = nullptr;
+  ZKD_TRY(seed_static_scratch(&buf));
+  const size_t nn = (size_t)N * N;
+  double2* G = (double2*)buf;
+  double* sigma = (double*)(buf + kSeedStaticGBytes);  // 8 doubles
+  double* mu_uns = sigma + 8;                          // N <= 512 doubles
+  int* flags = (int*)(mu_uns + ZKD_SEED_STATIC_MAX_N);  // 128 ints (the kernel clears the ones it uses)
+  static_assert(sizeof(double) * (8 + ZKD_SEED_STATIC_MAX_N) + sizeof(int) * 128 <= 8192, "tail of the static scratch");
+  static_assert(sizeof(double2) * 16 * ZKD_SEED_STATIC_MAX_N <= 200 * 1024, "two blocks of 8 columns fit shared memory");
+  // the array keeps the last call's contents: sigma, the eigenvalues and the flags start from zero (G is overwritten from A)
+  ZKD_CUDA_TRY(cudaMemsetAsync(buf + kSeedStaticGBytes, 0, 8192, s));
+  int rc = ZKD_OK;
+  for (int b = 0; b < batch && rc == ZKD_OK; ++b) {
+    const double2* Ab = (const double2*)A64 + (size_t)b * nn;
+    seed_sigma_kernel<<<1, 1024, 0, s>>>(N, Ab, sigma);
+    const int ms = max_sweeps > 64 ? 64 : max_sweeps;
+    rc = launch_block<8, 8>(N, sms, Ab, G, sigma, flags, mu_uns, ms, tol * tol, s);
+    if (rc != ZKD_OK) break;
+    seed_sort_kernel<<<sms, 256, 0, s>>>(N, mu_uns, G, sigma, mu + (size_t)b * N, (double2*)V + (size_t)b * nn);
+    count_launch(3);
+    rc = launch_check();
+  }
+  return rc;
 }
 
 }  // namespace zkd

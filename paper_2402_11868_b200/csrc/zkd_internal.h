@@ -119,6 +119,8 @@ int fx_to_api(int count, const int32_t* src_fx, void* dst_api, int scale_bits, c
 inline bool prec_supported(int prec) { return prec >= 128 && prec <= kPrec && (prec & 63) == 0; }
 inline size_t api_real_bytes(int prec) { return 16 + (size_t)prec / 8; }
 int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int max_sweeps, cudaStream_t s);
+// the same with its scratch in a static device array (N <= ZKD_SEED_STATIC_MAX_N): allocates nothing
+int seed_fp64_static(int N, int batch, const double* A64, double* mu, double* V, int max_sweeps, cudaStream_t s);
 
 size_t diag_workspace_bytes(int N, int batch);
 int diag_herm_device(int N, int batch, int prec, const void* A_api, void* eigvals_api, void* eigvecs_api, void* ws, size_t ws_bytes,
