@@ -148,6 +148,111 @@ __global__ void __launch_bounds__(256) slice_i8_kernel(SliceArgs a) {
   if (bad && a.err_flag) atomicOr(a.err_flag, 4);
 }
 
+
+// The same re-slicing, four consecutive k per thread and two digits (56 bits = seven slices) per step.  The balanced
+// slices of a value x are the plain bytes of x + 0x80...80 with their top bits flipped, and what is left above them is the
+// carry: one 64-bit add, one xor and one shift per seven slices instead of a carry step per slice; the slices of the
+// thread's four elements are transposed with byte permutes and leave as one 32-bit store per slice plane.  Lanes of a warp
+// cover 128 consecutive k of one row (TRANS = false: the source is read with 16-byte loads) or 8 rows x 16 k (TRANS = true:
+// the source is k-major there, so 8 consecutive rows make one 32-byte sector).  Bit-identical to slice_i8_kernel.
+template <bool TRANS>
+__global__ void __launch_bounds__(256) slice4_i8_kernel(SliceArgs a) {
+  const int KG = a.Kp >> 2;  // groups of four k per row (a multiple of 32)
+  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int g, row, kg;
+  if (!TRANS) {
+    kg = (int)(t % KG);
+    const size_t rest = t / KG;
+    row = (int)(rest % a.rows);
+    g = (int)(rest / a.rows);
+  } else {
+    const int lane = threadIdx.x & 31;
+    const size_t wid = t >> 5;
+    const int KT = KG >> 2, RT = (a.rows + 7) >> 3;
+    kg = (int)(wid % KT) * 4 + (lane & 3);
+    const size_t rest = wid / KT;
+    row = (int)(rest % RT) * 8 + (lane >> 2);
+    g = (int)(rest / RT);
+  }
+  if (g >= a.G || row >= a.rows) return;
+  const int kk = kg << 2;
+  const size_t per = (size_t)a.rows * a.Kp;
+  uint32_t* __restrict__ dst = (uint32_t*)(a.dst + (size_t)g * a.ns * per + (size_t)row * a.Kp + kk);
+  const size_t dstride = per >> 2;
+  const size_t RC = (size_t)a.R * a.C;
+  const int32_t* __restrict__ src = a.src + (size_t)g * a.nw * RC + (TRANS ? ((size_t)kk * a.C + row) : ((size_t)row * a.C + kk));
+  const size_t estride = TRANS ? (size_t)a.C : 1;  // between the thread's four elements
+  const int nvalid = a.K - kk;                      // elements kk + i with i < nvalid exist
+  const bool vec = !TRANS && (a.C & 3) == 0 && nvalid >= 4 && (((uintptr_t)a.src & 15) == 0);
+  auto load4 = [&](int k, int32_t (&d)[4]) {
+    const int32_t* p = src + (size_t)k * RC;
+    if (vec) {
+      const int4 v = *(const int4*)p;
+      d[0] = v.x; d[1] = v.y; d[2] = v.z; d[3] = v.w;
+    } else {
+#pragma unroll
+      for (int i = 0; i < 4; ++i) d[i] = i < nvalid ? p[(size_t)i * estride] : 0;
+    }
+  };
+  constexpr int64_t BIAS7 = 0x0080808080808080ll;
+  int64_t cy[4] = {0, 0, 0, 0};
+  int j = 0;
+  const int npair = a.nw >> 1;
+  for (int pr = 0; pr < npair; ++pr) {
+    int32_t d0[4], d1[4];
+    load4(2 * pr, d0);
+    load4(2 * pr + 1, d1);
+    uint32_t lo[4], hi[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int64_t tt = cy[i] + (int64_t)d0[i] + ((int64_t)d1[i] << DB) + BIAS7;
+      const uint64_t x = (uint64_t)tt ^ (uint64_t)BIAS7;
+      cy[i] = tt >> 56;
+      lo[i] = (uint32_t)x;
+      hi[i] = (uint32_t)(x >> 32);
+    }
+    const uint32_t la = __byte_perm(lo[0], lo[1], 0x5140), lb = __byte_perm(lo[2], lo[3], 0x5140);
+    const uint32_t lc = __byte_perm(lo[0], lo[1], 0x7362), ld = __byte_perm(lo[2], lo[3], 0x7362);
+    const uint32_t ha = __byte_perm(hi[0], hi[1], 0x5140), hb = __byte_perm(hi[2], hi[3], 0x5140);
+    const uint32_t hc = __byte_perm(hi[0], hi[1], 0x7362), hd = __byte_perm(hi[2], hi[3], 0x7362);
+    uint32_t* o = dst + (size_t)j * dstride;
+    o[0] = __byte_perm(la, lb, 0x5410);
+    o[dstride] = __byte_perm(la, lb, 0x7632);
+    o[2 * dstride] = __byte_perm(lc, ld, 0x5410);
+    o[3 * dstride] = __byte_perm(lc, ld, 0x7632);
+    o[4 * dstride] = __byte_perm(ha, hb, 0x5410);
+    o[5 * dstride] = __byte_perm(ha, hb, 0x7632);
+    o[6 * dstride] = __byte_perm(hc, hd, 0x5410);
+    j += 7;
+  }
+  // what is left: the odd last digit (if any) on top of the carry; ns - j - 1 more balanced slices, then the top slice takes the rest
+  if (a.nw & 1) {
+    int32_t d[4];
+    load4(a.nw - 1, d);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) cy[i] += d[i];
+  }
+  bool bad = false;
+  for (; j < a.ns; ++j) {
+    uint32_t w = 0;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      int64_t byte;
+      if (j < a.ns - 1) {
+        const int64_t c = (cy[i] + 128) >> 8;
+        byte = cy[i] - (c << 8);
+        cy[i] = c;
+      } else {
+        byte = cy[i];
+        if (byte < -128 || byte > 127) bad = true;
+      }
+      w |= ((uint32_t)byte & 255u) << (8 * i);
+    }
+    dst[(size_t)j * dstride] = w;
+  }
+  if (bad && a.err_flag) atomicOr(a.err_flag, 4);
+}
+
 }  // namespace
 
 namespace {
@@ -633,14 +738,17 @@ int gemm_i8_finish(int M, int N, int K, int batch, const int32_t* Pc, const int3
     size_t tot = (size_t)G * M * Kp;
     {
       KtScope kt(KC_SLICE_I8, stream, (uint64_t)G * M * K * 4ull * np + (uint64_t)tot * nsP);
-      slice_i8_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(sa);
+      if (options().i8_slice == 1) slice_i8_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(sa);
+      else slice4_i8_kernel<false><<<(unsigned)((tot / 4 + 255) / 256), 256, 0, stream>>>(sa);
     }
     count_launch();
     sa.src = Qc; sa.dst = Q8; sa.R = K; sa.C = N; sa.nw = nq; sa.ns = nsQ; sa.rows = N; sa.transpose = 1;
     tot = (size_t)G * N * Kp;
     {
       KtScope kt(KC_SLICE_I8, stream, (uint64_t)G * N * K * 4ull * nq + (uint64_t)tot * nsQ);
-      slice_i8_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(sa);
+      const size_t thr = (size_t)G * ((N + 7) / 8) * (Kp / 16) * 32;  // warps of 8 rows x 16 k
+      if (options().i8_slice == 1) slice_i8_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(sa);
+      else slice4_i8_kernel<true><<<(unsigned)((thr + 255) / 256), 256, 0, stream>>>(sa);
     }
     count_launch();
   }
