@@ -160,12 +160,13 @@ int build_plan(Ctx& c, int n, int nb, const std::vector<int>& h_cl, int* plan_de
   plan->tiled = false;
   plan->tile.clear();
   constexpr int TW = 128;
-  // worth it only when the clusters fill most of a tile: a tile computes 128 / m times the entries a cluster of m needs, and the
-  // int8 engine is about 2 x 128 / m ... faster than the IMAD engine per entry (measured on c5, m = 16: tiles 97 ms against 81 ms
-  // per cluster); cluster_tiles = 2 forces tiles wherever they can be formed (tests)
+  // a tile computes 128 / m times the entries a cluster of m needs, but the int8 engine is that much faster per entry than the
+  // IMAD engine down to m of about 10 (measured on c5, m = 16, after the issue-side and re-slicing work of round 2: cluster
+  // passes 55 ms as tiles against 85 ms per cluster; before it, 97 against 81); the weighted mean cluster size decides.
+  // cluster_tiles = 2 forces tiles wherever they can be formed (tests), 0 never uses them
   size_t sum_m2 = 0;
   for (const auto& kv : groups) sum_m2 += (size_t)kv.first * kv.first * kv.second.size();
-  const bool tiles_pay = options().cluster_tiles == 2 || (options().cluster_tiles == 1 && 5 * sum_m2 >= 2 * (size_t)TW * clustered);
+  const bool tiles_pay = options().cluster_tiles == 2 || (options().cluster_tiles == 1 && sum_m2 >= 10 * clustered);
   if (options().gemm_path != 1 && tiles_pay && n >= TW && n % TW == 0 && 2 * clustered >= (size_t)n * nb &&
       gemm_i8_eligible(options().gemm_path, TW, TW, n, 1)) {
     bool ok = true;
