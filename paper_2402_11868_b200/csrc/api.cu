@@ -226,6 +226,7 @@ static int* option_slot(const char* key) {
   if (!strcmp(key, "cluster_tiles")) return &o.cluster_tiles;
   if (!strcmp(key, "i8_step")) return &o.i8_step;
   if (!strcmp(key, "i8_slice")) return &o.i8_slice;
+  if (!strcmp(key, "i8_packed")) return &o.i8_packed;
   if (!strcmp(key, "block_correction")) return &o.block_correction;
   if (!strcmp(key, "verbose")) return &o.verbose;
   return nullptr;

@@ -77,6 +77,14 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
   d |= (uint64_t)2 << 61;                       // SWIZZLE_128B
   return d;
 }
+__device__ __forceinline__ void tmem_ld_32x32b_x16_nowait(uint32_t taddr, uint32_t (&v)[16]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+        "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+      : "r"(taddr));
+}
 // one lane of a converged warp; unlike "lane == 0" the compiler knows the branch holds exactly one thread, so tcgen05 / TMA
 // instructions inside it are issued straight from uniform registers (no per-instruction election loop)
 __device__ __forceinline__ bool elect_one() {
@@ -259,7 +267,8 @@ namespace {
 
 // ---- the tcgen05 kernel ----------------------------------------------------------------------------------------------
 struct I8Args {
-  int32_t* out;  // [nsplit][G][ncol][M][N]
+  int32_t* out;  // [nsplit][G][ncol][M][N] int32, or (packed) [nsplit][G][ngroups][M][N] int64 = sum_dd S_(4 dg + dd) 2^(8 dd)
+  int packed;
   int M, N, G, nsP, nsQ, dcut, ncol, ngroups, nkb, kb_per_split, nsplit;
   uint32_t p_tile_bytes, q_tile_bytes;  // bytes one TMA box delivers (rows may be < 128 for small matrices)
 };
@@ -415,6 +424,41 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const int i = i0 + warp * 32 + lane;
     const size_t mn = (size_t)a.M * a.N;
+    if (a.packed) {
+      // the group's columns leave as ONE 64-bit word per entry, sum_dd S_(d0 + dd) 2^(8 dd) (|S| < 2^31: below 2^56): half the
+      // bytes of four int32 columns and a quarter of the words combine_i8_packed_kernel has to walk
+      const int ncv = min(I8_D, a.ncol - I8_D * dg);  // columns of this group that exist (their accumulators were written)
+      int64_t* o = (int64_t*)a.out + ((size_t)(sp * a.G + g) * a.ngroups + dg) * mn + (size_t)i * a.N + j0;
+#pragma unroll 1
+      for (int cc = 0; cc < I8_BN; cc += 16) {
+        uint32_t v[I8_D][16];
+#pragma unroll
+        for (int dd = 0; dd < I8_D; ++dd) {
+          if (dd < ncv) {
+            tmem_ld_32x32b_x16_nowait(tmem_base + ((uint32_t)(warp * 32) << 16) + dd * I8_BN + cc, v[dd]);
+          } else {
+#pragma unroll
+            for (int t = 0; t < 16; ++t) v[dd][t] = 0;
+          }
+        }
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        int64_t r[16];
+#pragma unroll
+        for (int t = 0; t < 16; ++t)
+          r[t] = (int64_t)(int32_t)v[0][t] + ((int64_t)(int32_t)v[1][t] << 8) + ((int64_t)(int32_t)v[2][t] << 16) +
+                 ((int64_t)(int32_t)v[3][t] << 24);
+        if (i < a.M) {
+          if (j0 + cc + 16 <= a.N && (a.N & 1) == 0) {
+#pragma unroll
+            for (int t = 0; t < 16; t += 2) *(longlong2*)(o + cc + t) = make_longlong2(r[t], r[t + 1]);
+          } else {
+#pragma unroll
+            for (int t = 0; t < 16; ++t)
+              if (j0 + cc + t < a.N) o[cc + t] = r[t];
+          }
+        }
+      }
+    } else
     for (int dd = 0; dd < I8_D; ++dd) {
       const int c = I8_D * dg + dd;  // column index relative to dcut
       if (c >= a.ncol) break;
@@ -639,6 +683,87 @@ __global__ void __launch_bounds__(256) combine_i8_kernel(CombineI8Args a) {
     for (int kk = 0; kk < kstart && kk < ND; ++kk) dst[(size_t)kk * tot_d] = 0;
 }
 
+// The same fold for the packed output of gemm_i8_kernel (one int64 per entry and group of four columns).  The groups are
+// first normalised into a stream of 32-bit words of the two's complement value V = sum_g G_g 2^(32 g) (one 64-bit add and one
+// shift per group: w = G_g + carry, word = low 32 bits, carry = w >> 32; beyond the last group the words are the sign); FX digit
+// k is then the bit field [28 k - base_bit, +28) of that stream (one funnel shift), the signed top digit the 32 bits from its
+// position.  No per-column 64-bit shifts and a quarter of the loads of combine_i8_kernel; bit-identical to it.
+__global__ void __launch_bounds__(256) combine_i8_packed_kernel(CombineI8Args a) {
+  const size_t tot = a.mn * a.batch;
+  const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int part = blockIdx.y;
+  if (e >= tot) return;
+  const int b = (int)(e / a.mn);
+  const size_t ij = e % a.mn;
+  const int ng = a.ncol;  // here: number of groups
+  const size_t gstride = (size_t)ng * a.mn;
+  const size_t sstride = (size_t)3 * a.batch * gstride;
+  const int64_t* __restrict__ r1 = (const int64_t*)a.raw + (size_t)(b * 3 + 0) * gstride + ij;
+  const int64_t* __restrict__ r2 = (const int64_t*)a.raw + (size_t)(b * 3 + (part == 0 ? 2 : 1)) * gstride + ij;
+  const bool neg2 = part == 0;
+  const size_t tot_d = a.plane_count;
+  int32_t* dst = a.dst + (part ? (size_t)ND * tot_d : 0) + (a.off ? (size_t)a.off[b] : (size_t)b * a.mn) +
+                 (size_t)(ij / a.N) * a.ld + (ij % a.N);
+
+  // word stream: index -1 is a zero word (bits below base_bit), 0 .. ng - 1 the normalised groups, then the sign
+  int gi = 0;
+  int64_t carry = 0;
+  auto next_word = [&]() -> uint32_t {
+    int64_t w = carry;
+    if (gi < ng) {
+      for (int s = 0; s < a.nsplit; ++s) {
+        const int64_t x1 = r1[(size_t)s * sstride + (size_t)gi * a.mn], x2 = r2[(size_t)s * sstride + (size_t)gi * a.mn];
+        w += neg2 ? x1 - x2 : x1 + x2;
+      }
+      ++gi;
+    }
+    carry = w >> 32;
+    return (uint32_t)w;
+  };
+  const int kstart = a.base_bit >= 0 ? a.base_bit / DB : -((-a.base_bit + DB - 1) / DB);
+  const int k0 = kstart > 0 ? kstart : 0;
+  const int cutq = a.cut_bit > 0 ? a.cut_bit / DB : 0, cutr = a.cut_bit > 0 ? a.cut_bit % DB : 0;
+  // bit offset of digit k0 in the stream that starts with the zero word: >= 4
+  long p = (long)DB * k0 - a.base_bit + 32;
+  uint32_t wa = 0, wb = next_word();  // stream words q, q + 1 with q = 0
+  long q = 0;
+  int64_t cy2 = 0;
+  int msb_pos = 0, msb_neg = 0;
+  if (a.mode == 0)
+    for (int kk = 0; kk < k0 && kk < ND; ++kk) dst[(size_t)kk * tot_d] = 0;
+  for (int k = k0; k <= ND - 1; ++k, p += DB) {
+    while (q < (p >> 5)) {
+      wa = wb;
+      wb = next_word();
+      ++q;
+    }
+    const uint32_t f = __funnelshift_r(wa, wb, (uint32_t)(p & 31));
+    int32_t digit = k < ND - 1 ? (int32_t)(f & (uint32_t)DMASK) : (int32_t)f;
+    if (k < cutq) digit = 0;
+    else if (k == cutq && cutr) digit &= ~((1 << cutr) - 1);
+    int32_t* dp = dst + (size_t)k * tot_d;
+    int32_t outd = digit;
+    if (a.mode != 0) {
+      const int64_t t = (int64_t)*dp + (a.mode == 1 ? (int64_t)digit : -(int64_t)digit) + cy2;
+      if (k < ND - 1) {
+        cy2 = t >> DB;
+        outd = (int32_t)(t & DMASK);
+      } else {
+        outd = (int32_t)t;
+      }
+    }
+    *dp = outd;
+    if (k < ND - 1) {
+      if (outd != 0) msb_pos = k * DB + (32 - __clz(outd));
+      if (outd != DMASK) msb_neg = k * DB + (32 - __clz((~outd) & DMASK));
+    } else {
+      if (outd > 0) msb_pos = k * DB + (32 - __clz(outd));
+      if (outd < -1) msb_neg = k * DB + (32 - __clz(~outd));
+      if (a.msb_out) atomicMax(a.msb_out, outd < 0 ? msb_neg : msb_pos);
+    }
+  }
+}
+
 }  // namespace
 
 // ---- host side -----------------------------------------------------------------------------------------------------
@@ -758,6 +883,8 @@ int gemm_i8_finish(int M, int N, int K, int batch, const int32_t* Pc, const int3
   ZKD_TRY(make_map(&mapQ, Q8, Kp, N, G * nsQ, boxQ));
 
   I8Args ka{};
+  const bool packed = options().i8_packed != 0;
+  ka.packed = packed ? 1 : 0;
   ka.out = raw; ka.M = M; ka.N = N; ka.G = G; ka.nsP = nsP; ka.nsQ = nsQ; ka.dcut = dcut; ka.ncol = ncol;
   ka.ngroups = (ncol + I8_D - 1) / I8_D;
   ka.nkb = Kp / I8_BK;
@@ -795,8 +922,14 @@ int gemm_i8_finish(int M, int N, int K, int batch, const int32_t* Pc, const int3
   ca.base_bit = lsbP + lsbQ - FRAC + 8 * dcut;
   ca.cut_bit = cut_bit; ca.mode = mode; ca.msb_out = msb_out;
   const size_t tot = (size_t)batch * M * N;
-  KtScope kt(KC_COMBINE_I8, stream, 4ull * tot * ((uint64_t)ka.nsplit * 3 * ncol + 2ull * ND * (mode == 0 ? 1 : 2)));
-  combine_i8_kernel<<<dim3((unsigned)((tot + 255) / 256), 2), 256, 0, stream>>>(ca);
+  if (packed) {
+    ca.ncol = ka.ngroups;
+    KtScope kt(KC_COMBINE_I8, stream, 4ull * tot * ((uint64_t)ka.nsplit * 3 * 2 * ka.ngroups + 2ull * ND * (mode == 0 ? 1 : 2)));
+    combine_i8_packed_kernel<<<dim3((unsigned)((tot + 255) / 256), 2), 256, 0, stream>>>(ca);
+  } else {
+    KtScope kt(KC_COMBINE_I8, stream, 4ull * tot * ((uint64_t)ka.nsplit * 3 * ncol + 2ull * ND * (mode == 0 ? 1 : 2)));
+    combine_i8_kernel<<<dim3((unsigned)((tot + 255) / 256), 2), 256, 0, stream>>>(ca);
+  }
   count_launch();
   return launch_check();
 }

@@ -54,6 +54,7 @@ struct Options {
   int early_split = 1;        // S4h: split clusters as soon as their internal structure stands above the noise
   int split_margin_bits = 40; // ... by this many bits
   int block_correction = 1;   // S4d: one fixed-point step with the off-diagonal parts of the cluster blocks (second order in spread / gap)
+  int i8_packed = 1;          // int8 GEMM output: 1 = one int64 per entry and group of four columns (combine_i8_packed_kernel), 0 = int32 columns
   int i8_slice = 0;           // int8 GEMM re-slicing kernel: 0 = four k per thread, seven slices per step; 1 = one element per thread
   int i8_step = 0;            // int8 GEMM: slices a per barrier round trip: 0 / 2 = two (rings <4, 9>), 1 = one (rings <5, 8>)
   int cluster_tiles = 1;      // cluster passes as 128-column tile products on the int8 engine when no cluster straddles a tile
