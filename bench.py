@@ -228,6 +228,7 @@ def roofline_objects(cats: dict, seed_elems, imad_peak, dfma_peak, steps, total_
                 # the peak above is cuBLAS bf16 x the nominal int8 : bf16 ratio, which this kernel can exceed; the live
                 # figure is the issue rate of the kernel's own MMA shape with operands resident in shared memory
                 o.update({"mma_issue_peak": I8_MMA_PEAK / 1e12, "frac_of_mma_issue_peak": o["achieved"] / (I8_MMA_PEAK / 1e12),
+                          "frac_executed_of_mma_issue_peak": o["achieved_executed"] / (I8_MMA_PEAK / 1e12),
                           "mma_issue_peak_source": "measured live (zkd_measure_i8_mma_peak): tcgen05.mma kind::i8 128x128x32, "
                                                    "one CTA per SM, no loads"})
         elif name == "seed_fp64":

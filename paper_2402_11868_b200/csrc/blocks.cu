@@ -868,9 +868,11 @@ int singleton_step(int n, int nb, int32_t* X, int32_t* W, int32_t* R, int32_t* S
 }
 
 // ---- E_ij = C_ij / (theta_j - theta_i) across clusters, 0 inside ---------------------------------------------------------------
-// One thread per pair i < j (and the diagonal, which is zeroed).  d = theta_j - theta_i is normalised to
-// d' = d 2^s in [1/4, 1/2) with a static barrel shifter, r = 1/d' by Newton from an fp64 start on W-digit fixed point
-// (r in (2,4], FX-like with 29 - (30-W) fractional digits), then E_ij = (C_ij r) 2^s, E_ji = -(C_ji r) 2^s.
+// One thread per entry (i, j) (the diagonal and the entries inside a cluster are zeroed).  d = theta_j - theta_i is normalised
+// to d' = |d| 2^s in [1/4, 1/2) with a static barrel shifter, r = 1/d' by Newton from an fp64 start on W-digit fixed point
+// (r in (2,4], FX-like with 29 - (30-W) fractional digits), then E_ij = sgn(d) (C_ij r) 2^s.  (i, j) and (j, i) each compute
+// the reciprocal of the same |d|: a thread that served both entries read and wrote the (j, i) one with stride n (12.5
+// sectors per request, half the threads idle: 0.76 ms per launch at n = 1024); per entry every access is coalesced.
 template <int W>
 __global__ void __launch_bounds__(128) ecalc_kernel(int n, int nb, const int32_t* __restrict__ theta, const int* __restrict__ cl,
                                                     int32_t* __restrict__ C, int newton_iters, int* __restrict__ msb_out,
@@ -879,15 +881,13 @@ __global__ void __launch_bounds__(128) ecalc_kernel(int n, int nb, const int32_t
   const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= count) return;
   const int b = (int)(t / per), i = (int)((t % per) / n), j = (int)(t % n);
-  if (i > j) return;
   int32_t* Cr = C;
   int32_t* Ci = C + (size_t)ND * count;
-  const size_t eij = (size_t)b * per + (size_t)i * n + j, eji = (size_t)b * per + (size_t)j * n + i;
+  const size_t eij = (size_t)b * per + (size_t)i * n + j;
   int32_t z[ND];
   fx_zero(z);
   if (cl[(size_t)b * n + i] == cl[(size_t)b * n + j]) {
     fx_store(Cr, count, eij, z); fx_store(Ci, count, eij, z);
-    if (i != j) { fx_store(Cr, count, eji, z); fx_store(Ci, count, eji, z); }
     return;
   }
   int32_t ti[ND], tj[ND], d[ND];
@@ -902,7 +902,6 @@ __global__ void __launch_bounds__(128) ecalc_kernel(int n, int nb, const int32_t
   if (msb < 812 - 400) {      // different clusters must be apart; anything this close is a planning error
     if (err_flag) atomicOr(err_flag, 2);
     fx_store(Cr, count, eij, z); fx_store(Ci, count, eij, z);
-    fx_store(Cr, count, eji, z); fx_store(Ci, count, eji, z);
     return;
   }
   // d' = d 2^s with msb(d') = 811  (value in [1/4,1/2))
@@ -917,10 +916,10 @@ __global__ void __launch_bounds__(128) ecalc_kernel(int n, int nb, const int32_t
   // E = (C r) 2^s, with sign
   int mymsb = 0;
 #pragma unroll 1
-  for (int which = 0; which < 4; ++which) {
+  for (int which = 0; which < 2; ++which) {
     int32_t* plane = (which & 1) ? Ci : Cr;
-    const size_t e = (which & 2) ? eji : eij;
-    const bool neg = dneg ^ ((which & 2) != 0);
+    const size_t e = eij;
+    const bool neg = dneg;
     int32_t c[ND], o[ND];
     fx_load(c, plane, count, e);
     {
@@ -946,9 +945,11 @@ int ecalc(int n, int nb, const int32_t* theta, const int* cl, int32_t* C, int pr
   // Newton doubles the ~50 correct bits of the fp64 start each iteration
   int iters = 0;
   for (int have = 48; have < prec_bits; have *= 2) ++iters;
-  // digit products per pair i < j: two (W+1)^2-digit products per Newton iteration (half of them kept) and four 30 x (W+1) products
+  // digit products per entry i != j: two (W+1)^2-digit products per Newton iteration (half of them kept) and two 30 x (W+1)
+  // products (executed); algorithmic: the reciprocal once per pair
   const uint64_t Wd = prec_bits <= 28 * 4 - 8 ? 5 : prec_bits <= 28 * 8 - 8 ? 9 : prec_bits <= 28 * 16 - 8 ? 17 : 30;
-  KtScope kt_scope(KC_ECALC, s, (uint64_t)n * (n - 1) / 2 * nb * ((uint64_t)iters * Wd * (Wd + 3) + 4ull * ND * Wd));
+  KtScope kt_scope(KC_ECALC, s, (uint64_t)n * (n - 1) * nb * ((uint64_t)iters * Wd * (Wd + 3) + 2ull * ND * Wd),
+                   (uint64_t)n * (n - 1) / 2 * nb * ((uint64_t)iters * Wd * (Wd + 3) + 4ull * ND * Wd));
   if (prec_bits <= 28 * 4 - 8) ecalc_kernel<4><<<blocks, 128, 0, s>>>(n, nb, theta, cl, C, iters, msb_out, err_flag);
   else if (prec_bits <= 28 * 8 - 8) ecalc_kernel<8><<<blocks, 128, 0, s>>>(n, nb, theta, cl, C, iters, msb_out, err_flag);
   else if (prec_bits <= 28 * 16 - 8) ecalc_kernel<16><<<blocks, 128, 0, s>>>(n, nb, theta, cl, C, iters, msb_out, err_flag);

@@ -635,7 +635,8 @@ int gemm_complex(int M, int N, int K, int batch, const GemmSide& P, const GemmSi
   dim3 grid((N + tg - 1) / tg, (M + tg - 1) / tg, (unsigned)(3 * batch * nsp));
   const uint64_t nmacs = inst_cost(*in) * 3ull * (uint64_t)batch * M * N * K;
   {
-    KtScope kt(KC_GEMM_DIGITS, stream, nmacs, request_cost(P.nw, Q.nw) * 3ull * (uint64_t)batch * M * N * K);
+    KtScope kt(KC_GEMM_DIGITS, stream, nmacs,
+               (uint64_t)((double)(request_cost(P.nw, Q.nw) * 3ull * (uint64_t)batch * M * N * K) * gemm_useful_fraction()));
     if ((tg == 8 ? in->launch8 : in->launch)(ka, grid, stream) != cudaSuccess) return ZKD_ERR_CUDA;
   }
   count_launch();

@@ -818,6 +818,13 @@ int pick_nsplit(int K, int nsmin) {
 
 }  // namespace
 
+namespace {
+thread_local double t_useful = 1.0;
+}
+double gemm_useful_fraction() { return t_useful; }
+GemmUsefulScope::GemmUsefulScope(double f) : old_(t_useful) { t_useful = f; }
+GemmUsefulScope::~GemmUsefulScope() { t_useful = old_; }
+
 void kernel_timing_enable_i8(bool on) { (void)on; }
 int kernel_timing_read_i8(double* ms, uint64_t* launches, uint64_t* macs) { return kt_read(KC_GEMM_I8, ms, launches, macs, nullptr); }
 
@@ -908,7 +915,7 @@ int gemm_i8_finish(int M, int N, int K, int batch, const int32_t* Pc, const int3
   const uint64_t macs = pairs * (uint64_t)G * grid.x * grid.y * ka.nkb * I8_BM * I8_BN * I8_BK;
   {
     // algorithmic: the same slice pairs on the matrices as they are (no padding of M, N, K to 128)
-    KtScope kt(KC_GEMM_I8, stream, macs, pairs * (uint64_t)G * M * N * K);
+    KtScope kt(KC_GEMM_I8, stream, macs, (uint64_t)((double)(pairs * (uint64_t)G * M * N * K) * gemm_useful_fraction()));
     kern<<<grid, I8_THREADS, smem, stream>>>(mapP, mapQ, ka);
   }
   count_launch();

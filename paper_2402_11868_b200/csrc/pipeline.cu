@@ -132,6 +132,7 @@ struct ClusterPlan {
   // an engine that is far more than that factor faster than the IMAD path on m x m x n products.
   bool tiled = false;
   std::vector<ClusterGroup> tile;  // one entry: m = 128, nsub = tiles that hold a cluster
+  double tile_useful = 1.0;        // sum of m^2 over the clusters / (128^2 x tiles): the share of a tile product the clusters need
 };
 
 int build_plan(Ctx& c, int n, int nb, const std::vector<int>& h_cl, int* plan_dev /* 2 n nb ints */, ClusterPlan* plan) {
@@ -195,6 +196,7 @@ int build_plan(Ctx& c, int n, int nb, const std::vector<int>& h_cl, int* plan_de
         h.insert(h.end(), ob.begin(), ob.end());
         plan->tile.push_back(g);
         plan->tiled = true;
+        plan->tile_useful = (double)sum_m2 / ((double)TW * TW * g.nsub);
       }
     }
   }
@@ -231,6 +233,8 @@ int cluster_pass(Ctx& c, int n, int nb, const ClusterPlan& plan, const int* cl, 
   const int nwX = digits_for(topX, cut), nwW = digits_for(topW, cut);
   // the products of this pass run per cluster (IMAD engine) or per 128-column tile (int8 tcgen05 engine), see ClusterPlan
   const std::vector<ClusterGroup>& groups = plan.tiled ? plan.tile : plan.groups;
+  // timing only: the ALGORITHMIC work of a tile product is the share its cluster blocks need (the rest is executed padding)
+  GemmUsefulScope useful(plan.tiled ? plan.tile_useful : 1.0);
   // S4f: G_c = X_c^H X_c, bits below cutG cleared so that M = (I - G)/2 is a short number
   const int cutG = std::max(1, cut);
   for (const ClusterGroup& g : groups)

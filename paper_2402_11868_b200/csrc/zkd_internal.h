@@ -103,6 +103,18 @@ struct GemmDstView {         // the same for the destination (M x N per batch el
   size_t plane_count = 0;
 };
 enum class GemmMode : int { Assign = 0, Add = 1, Sub = 2 };
+// Timing bookkeeping only (KtScope work counters): the share of the products issued inside the scope that the caller needs
+// (cluster passes run as 128-column tiles need sum m^2 / 128^2 per tile); thread-local, nests by restoring the old value.
+double gemm_useful_fraction();
+struct GemmUsefulScope {
+  explicit GemmUsefulScope(double f);
+  ~GemmUsefulScope();
+  GemmUsefulScope(const GemmUsefulScope&) = delete;
+  GemmUsefulScope& operator=(const GemmUsefulScope&) = delete;
+
+ private:
+  double old_;
+};
 
 size_t gemm_workspace_bytes(int M, int N, int K, int batch);
 // dst (+)= op(P) * Q ; bits of the product below out_cut_bit are cleared (use a negative value for none).
