@@ -179,7 +179,12 @@ int zkd_mps_two_site_update(int chiL, int chiC, int chiR, int d, int batch, int 
  * one fixed-point step with the off-diagonal parts of the cluster blocks of X^H A X, which squares the spread / gap factor
  * that otherwise caps the gain of a pass), "seed_ring_block" (columns per block of the block-ring fp64 seed for N <= 256:
  * 2 or 4, 0 = the column ring, default -1 = 4 from N = 96 on), "seed_tma" (default 1: the blocked fp64 seed moves its columns by TMA bulk copies),
- * "seed_block_warps" (8 or 16), "combine_path" (epilogue of the IMAD GEMM: 0 automatic,
+ * "seed_block_warps" (8 or 16), "seed_gram" (default 0; 1 / 2: the blocked seed finds a round's rotations on the 8 x 8 Gram
+ * matrix of the CTA's two column blocks and applies them in one pass, for 256 < N <= 1600; measured slower),
+ * "seed_degenerate_skip" (default 1: inside the path the fp64 seed leaves column pairs of one numerically multiple eigenvalue -
+ * estimates closer than 2^-(tau_bits + 2) sigma / sqrt N, cosine below 2^-10 - unrotated, which keeps the Jacobi sweeps quadratically
+ * convergent on spectra with multiplicities; such a pair always lies inside one cluster of S2; 0: off; >= 8: the exponent itself;
+ * zkd_seed_fp64 and zkd_seed_fp64_static never apply the rule), "combine_path" (epilogue of the IMAD GEMM: 0 automatic,
  * 1 digit-serial, 2 warp-cooperative), "sstep_cpb" (matrix columns per CTA of the fused singleton step, 0 automatic), "sstep_par" (default 1: for N <= 96 and
  * one column per CTA the products of a row are spread over four threads), "sstep_warp" (1: its
  * warp-per-element variant for N <= 64, default 0), "sstep_cache" (shared-memory staging of the column, default 1),

@@ -459,7 +459,10 @@ int solve_level_impl(Ctx& c, int n, int nb, const int32_t* A, int32_t* X, int32_
 
   // S1-S3
   ZKD_TRY(fxc_to_c64(cnt, A, A64, s));
-  ZKD_TRY(seed_fp64(n, nb, (const double*)A64, mu, (double*)V, opt.seed_sweeps, s));
+  // the seed leaves degenerate pairs unrotated (seed.cu, rot_params) where S4h is there to resolve the inner structure of a cluster
+  // as soon as it stands above the noise; without S4h the seed's own resolution inside a cluster is what keeps the deflated
+  // correction fast on clusters that are wide against their gap (geometric cascades: 14 passes with it, > 120 without)
+  ZKD_TRY(seed_fp64(n, nb, (const double*)A64, mu, (double*)V, opt.seed_sweeps, s, allow_split && opt.early_split != 0));
   ZKD_TRY(cluster_detect(n, nb, A64, mu, opt.tau_bits, nullptr, cl, cle, stats, s));
   int32_t* Xc = X;  // current iterate (may end up in T's storage; copied back at the end)
   int32_t* Tc = T;

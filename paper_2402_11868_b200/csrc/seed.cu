@@ -56,14 +56,27 @@ __device__ __forceinline__ double warp_sum(double v) {
 //   c = 1/sqrt(1 + |tau|^2),  sigma = c tau;   [g_p, g_q] <- [c g_p - conj(sigma) g_q,  sigma g_p + c g_q].
 // Only c^2 + |sigma|^2 = 1 has to hold to working precision (one rsqrt); an error in w merely perturbs the angle.
 // Returns false when the pair is already orthogonal to tol (or a column is zero).  cos2 = |cos(g_p, g_q)|^2.
-__device__ __forceinline__ bool rot_params(double al, double be, double gr, double gi, double tol2, double& c, double& sr,
+//
+// Degenerate pairs are left alone (dgap2): two columns whose eigenvalue estimates ||g|| - sigma differ by less than
+// dgap = sqrt(dgap2) and whose cosine is already below 2^-10 belong to one (numerically) multiple eigenvalue.  Orthogonalising
+// such a pair takes a rotation of up to 45 degrees however small gamma is, and every large rotation re-fills, at FIRST order,
+// the inner products with the other eigenspaces that the sweep has just annihilated: with multiple eigenvalues cyclic Jacobi
+// then converges only linearly (c5's 64 x 16 clusters: ||A V - V L|| ~ 1e-7 after 12 sweeps, 1e-9 after 15).  Inside an
+// eigenspace the pair needs no rotation: V stays unitary, so gamma = v_p^H G^2 v_q is second order in the contamination from
+// other eigenspaces plus (eigenvalue difference) / ||g||, and vanishes with them; without the large rotations the sweeps converge
+// quadratically again (the same matrix: 1e-12 after 9 sweeps).  dgap is kept below the cluster threshold of S2
+// (2^-tau ||A||_F >= 2^-tau sigma / (1.5 sqrt n)), so a skipped pair always lands inside one cluster of the refinement, which
+// treats the cluster as a block (S4f re-orthonormalises it, S5 resolves it).  Skipped pairs do not count towards the sweep's
+// stopping criterion (cos2 = 0).
+__device__ __forceinline__ bool rot_params(double al, double be, double gr, double gi, double tol2, double dgap2, double& c, double& sr,
                                            double& si, double& cos2) {
   const double g2 = gr * gr + gi * gi;
   const double ab = al * be;
   cos2 = 0.0;
   if (!(g2 > tol2 * ab) || g2 == 0.0) return false;
-  cos2 = g2 * (1.0 / ab);
   const double d = 0.5 * (be - al);
+  if (g2 < 9.5367431640625e-07 * ab && d * d < dgap2 * fmax(al, be)) return false;  // 2^-20: |cos| < 2^-10
+  cos2 = g2 * (1.0 / ab);
   const double x = fma(d, d, g2);
   const double h = x * rsqrt(x);  // sqrt(d^2 + |gamma|^2)
   const double r2 = rsqrt(fabs(d) + h);
@@ -96,7 +109,7 @@ __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.w
 template <int EPL>
 __global__ void __launch_bounds__(EPL >= 8 ? 512 : 1024)
 seed_ring_kernel(int n, int wpc, const double2* __restrict__ A, double* __restrict__ mu, double2* __restrict__ V, int max_sweeps,
-                 double tol2, int dbuf) {
+                 double tol2, double gap2, int dbuf) {
   extern __shared__ double2 slots[];              // [1 + dbuf][wpc][2][n]
   __shared__ int s_id2[2][32][2];                 // column ids held by the local slots (per buffer)
   int (*s_id)[2] = s_id2[0];
@@ -181,6 +194,7 @@ seed_ring_kernel(int n, int wpc, const double2* __restrict__ A, double* __restri
   }
   cluster.sync();
 
+  const double dgap2 = gap2 * sigma * sigma / n;
   if (n > 1 && sigma > 0) {
     unsigned long long nchk = 0, nrot = 0;
     for (int sweep = 0; sweep < max_sweeps; ++sweep) {
@@ -213,7 +227,7 @@ seed_ring_kernel(int n, int wpc, const double2* __restrict__ A, double* __restri
           al = warp_sum(al); be = warp_sum(be); gr = warp_sum(gr); gi = warp_sum(gi);
           double c, sr, si, cos2;
           nchk += n;
-          if (rot_params(al, be, gr, gi, tol2, c, sr, si, cos2)) {
+          if (rot_params(al, be, gr, gi, tol2, dgap2, c, sr, si, cos2)) {
             nrot += n;
             cmax = fmax(cmax, cos2);
 #pragma unroll
@@ -301,7 +315,7 @@ seed_ring_kernel(int n, int wpc, const double2* __restrict__ A, double* __restri
 }
 
 template <int EPL>
-static int launch_ring(int N, int batch, int csize, const double2* A, double* mu, double2* V, int max_sweeps, double tol2,
+static int launch_ring(int N, int batch, int csize, const double2* A, double* mu, double2* V, int max_sweeps, double tol2, double gap2,
                        cudaStream_t s) {
   const int P = (N + 1) / 2;
   const int wpc = (P + csize - 1) / csize;
@@ -325,7 +339,7 @@ static int launch_ring(int N, int batch, int csize, const double2* A, double* mu
   cfg.numAttrs = 1;
   {
     KtScope kt(KC_SEED, s);
-    ZKD_CUDA_TRY(cudaLaunchKernelEx(&cfg, seed_ring_kernel<EPL>, N, wpc, A, mu, V, max_sweeps, tol2, dbuf));
+    ZKD_CUDA_TRY(cudaLaunchKernelEx(&cfg, seed_ring_kernel<EPL>, N, wpc, A, mu, V, max_sweeps, tol2, gap2, dbuf));
   }
   count_launch();
   return launch_check();
@@ -356,7 +370,7 @@ __device__ __forceinline__ void ring_store(double2* __restrict__ col, const doub
 }
 // orthogonalise the register-held columns a, bb; returns |cos|^2 before the rotation (0 when skipped)
 template <int EPL>
-__device__ __forceinline__ double ring_rotate(double2 (&a)[EPL], double2 (&bb)[EPL], double tol2, bool& rotated) {
+__device__ __forceinline__ double ring_rotate(double2 (&a)[EPL], double2 (&bb)[EPL], double tol2, double dgap2, bool& rotated) {
   double al = 0, be = 0, gr = 0, gi = 0;
 #pragma unroll
   for (int q = 0; q < EPL; ++q) {
@@ -367,7 +381,7 @@ __device__ __forceinline__ double ring_rotate(double2 (&a)[EPL], double2 (&bb)[E
   }
   al = warp_sum(al); be = warp_sum(be); gr = warp_sum(gr); gi = warp_sum(gi);
   double c, sr, si, cos2;
-  rotated = rot_params(al, be, gr, gi, tol2, c, sr, si, cos2);
+  rotated = rot_params(al, be, gr, gi, tol2, dgap2, c, sr, si, cos2);
   if (rotated) {
 #pragma unroll
     for (int q = 0; q < EPL; ++q) {
@@ -384,7 +398,7 @@ constexpr int kRingbMaxCols = 288;  // columns incl. padding
 
 template <int EPL, int W>
 __global__ void __launch_bounds__(512)
-seed_ringb_kernel(int n, int ppc, const double2* __restrict__ A, double* __restrict__ mu, double2* __restrict__ V, int max_sweeps, double tol2) {
+seed_ringb_kernel(int n, int ppc, const double2* __restrict__ A, double* __restrict__ mu, double2* __restrict__ V, int max_sweeps, double tol2, double gap2) {
   extern __shared__ double2 slots[];                 // [2 sets][ppc][2 blocks][W][n]
   __shared__ int s_id2[2][kRingbMaxProc][2][W];      // column ids held by the local slots (per set)
   __shared__ double s_mu[kRingbMaxCols];             // by position (2k + which) W + w (every CTA holds a full copy)
@@ -470,6 +484,7 @@ seed_ringb_kernel(int n, int ppc, const double2* __restrict__ A, double* __restr
   cluster.sync();
 
   unsigned long long nchk = 0, nrot = 0;
+  const double dgap2 = gap2 * sigma * sigma / n;
   if (n > 1 && sigma > 0) {
     for (int sweep = 0; sweep < max_sweeps; ++sweep) {
       double cmax = 0;
@@ -489,7 +504,7 @@ seed_ringb_kernel(int n, int ppc, const double2* __restrict__ A, double* __restr
               double2* X = which ? B : T;
               ring_load<EPL>(a, X + (size_t)p * n, n, lane);
               ring_load<EPL>(bb, X + (size_t)q * n, n, lane);
-              cmax = fmax(cmax, ring_rotate<EPL>(a, bb, tol2, rot));
+              cmax = fmax(cmax, ring_rotate<EPL>(a, bb, tol2, dgap2, rot));
               nchk += n;
               if (rot) {
                 nrot += n;
@@ -504,7 +519,7 @@ seed_ringb_kernel(int n, int ppc, const double2* __restrict__ A, double* __restr
           for (int t = 0; t < W; ++t) {
             const int q = (w + t) % W;
             ring_load<EPL>(bb, B + (size_t)q * n, n, lane);
-            cmax = fmax(cmax, ring_rotate<EPL>(a, bb, tol2, rot));
+            cmax = fmax(cmax, ring_rotate<EPL>(a, bb, tol2, dgap2, rot));
             nchk += n;
             if (rot) nrot += n;
             if (t < W - 1) {
@@ -585,7 +600,7 @@ seed_ringb_kernel(int n, int ppc, const double2* __restrict__ A, double* __restr
 
 template <int EPL, int W>
 static int launch_ringb(int N, int batch, int csize, int ppc, const double2* A, double* mu, double2* V, int max_sweeps, double tol2,
-                        cudaStream_t s) {
+                        double gap2, cudaStream_t s) {
   const size_t smem = sizeof(double2) * 2 * (size_t)ppc * 2 * W * N;
   if (smem > 48 * 1024) ZKD_CUDA_TRY(cudaFuncSetAttribute(seed_ringb_kernel<EPL, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   if (csize > 8) ZKD_CUDA_TRY(cudaFuncSetAttribute(seed_ringb_kernel<EPL, W>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
@@ -603,7 +618,7 @@ static int launch_ringb(int N, int batch, int csize, int ppc, const double2* A, 
   cfg.numAttrs = 1;
   {
     KtScope kt(KC_SEED, s);
-    ZKD_CUDA_TRY(cudaLaunchKernelEx(&cfg, seed_ringb_kernel<EPL, W>, N, ppc, A, mu, V, max_sweeps, tol2));
+    ZKD_CUDA_TRY(cudaLaunchKernelEx(&cfg, seed_ringb_kernel<EPL, W>, N, ppc, A, mu, V, max_sweeps, tol2, gap2));
   }
   count_launch();
   return launch_check();
@@ -614,7 +629,7 @@ static int launch_ringb(int N, int batch, int csize, int ppc, const double2* A, 
 // __syncthreads per round: no cluster barrier and no DSMEM latency on the critical path, and a batch uses one SM per matrix.
 template <int EPL>
 __global__ void __launch_bounds__(1024)
-seed_cta_kernel(int n, const double2* __restrict__ A, double* __restrict__ mu, double2* __restrict__ V, int max_sweeps, double tol2) {
+seed_cta_kernel(int n, const double2* __restrict__ A, double* __restrict__ mu, double2* __restrict__ V, int max_sweeps, double tol2, double gap2) {
   extern __shared__ double2 Gl[];                 // [n][n], column j at Gl + j n
   __shared__ double s_mu[96];
   __shared__ unsigned long long s_cmax[2];
@@ -654,6 +669,7 @@ seed_cta_kernel(int n, const double2* __restrict__ A, double* __restrict__ mu, d
   __syncthreads();
 
   const int M = n + (n & 1), npairs = M / 2;
+  const double dgap2 = gap2 * sigma * sigma / n;
   if (n > 1 && sigma > 0) {
     unsigned long long nchk = 0, nrot = 0;
     for (int sweep = 0; sweep < max_sweeps; ++sweep) {
@@ -683,7 +699,7 @@ seed_cta_kernel(int n, const double2* __restrict__ A, double* __restrict__ mu, d
           al = warp_sum(al); be = warp_sum(be); gr = warp_sum(gr); gi = warp_sum(gi);
           double c, sr, si, cos2;
           nchk += n;
-          if (!rot_params(al, be, gr, gi, tol2, c, sr, si, cos2)) continue;
+          if (!rot_params(al, be, gr, gi, tol2, dgap2, c, sr, si, cos2)) continue;
           nrot += n;
           cmax = fmax(cmax, cos2);
 #pragma unroll
@@ -735,14 +751,14 @@ seed_cta_kernel(int n, const double2* __restrict__ A, double* __restrict__ mu, d
 }
 
 template <int EPL>
-static int launch_cta(int N, int batch, const double2* A, double* mu, double2* V, int max_sweeps, double tol2, cudaStream_t s) {
+static int launch_cta(int N, int batch, const double2* A, double* mu, double2* V, int max_sweeps, double tol2, double gap2, cudaStream_t s) {
   const int npairs = (N + 1) / 2;
   int warps = npairs < 1 ? 1 : (npairs > 32 ? (npairs + 1) / 2 : npairs);
   const size_t smem = sizeof(double2) * (size_t)N * N;
   if (smem > 48 * 1024) ZKD_CUDA_TRY(cudaFuncSetAttribute(seed_cta_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   {
     KtScope kt(KC_SEED, s);
-    seed_cta_kernel<EPL><<<batch, 32 * warps, smem, s>>>(N, A, mu, V, max_sweeps, tol2);
+    seed_cta_kernel<EPL><<<batch, 32 * warps, smem, s>>>(N, A, mu, V, max_sweeps, tol2, gap2);
   }
   count_launch();
   return launch_check();
@@ -772,7 +788,7 @@ __global__ void seed_sigma_kernel(int n, const double2* __restrict__ A, double* 
 }
 
 // one warp: orthogonalise columns p, q of G (length n, global memory)
-__device__ __forceinline__ double rotate_pair_global(double2* __restrict__ gp, double2* __restrict__ gq, int n, int lane, double tol2,
+__device__ __forceinline__ double rotate_pair_global(double2* __restrict__ gp, double2* __restrict__ gq, int n, int lane, double tol2, double dgap2,
                                                      unsigned long long& nchk, unsigned long long& nrot) {
   double al = 0, be = 0, gr = 0, gi = 0;
   for (int i = lane; i < n; i += 32) {
@@ -785,7 +801,7 @@ __device__ __forceinline__ double rotate_pair_global(double2* __restrict__ gp, d
   al = warp_sum(al); be = warp_sum(be); gr = warp_sum(gr); gi = warp_sum(gi);
   double c, sr, si, cos2;
   nchk += n;
-  if (!rot_params(al, be, gr, gi, tol2, c, sr, si, cos2)) return cos2;
+  if (!rot_params(al, be, gr, gi, tol2, dgap2, c, sr, si, cos2)) return cos2;
   nrot += n;
   for (int i = lane; i < n; i += 32) {
     const double2 a = __ldcg(gp + i), b = __ldcg(gq + i);
@@ -797,12 +813,13 @@ __device__ __forceinline__ double rotate_pair_global(double2* __restrict__ gp, d
 
 __global__ void __launch_bounds__(128) seed_large_kernel(int n, const double2* __restrict__ A, double2* __restrict__ G,
                                                          const double* __restrict__ sigma_p, int* __restrict__ rot_flags,
-                                                         double* __restrict__ mu_unsorted, int max_sweeps, double tol2) {
+                                                         double* __restrict__ mu_unsorted, int max_sweeps, double tol2, double gap2) {
   cg::grid_group grid = cg::this_grid();
   const int tid = threadIdx.x, lane = tid & 31;
   const int gwarp = (blockIdx.x * blockDim.x + tid) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
   const size_t gtid = (size_t)blockIdx.x * blockDim.x + tid, gthr = (size_t)gridDim.x * blockDim.x;
   const double sigma = *sigma_p;
+  const double dgap2 = gap2 * sigma * sigma / n;
   for (size_t e = gtid; e < (size_t)n * n; e += gthr) {
     const int i = (int)(e % n), j = (int)(e / n);
     double2 a = (i <= j) ? A[(size_t)i * n + j] : A[(size_t)j * n + i];
@@ -821,7 +838,7 @@ __global__ void __launch_bounds__(128) seed_large_kernel(int n, const double2* _
         for (int i = gwarp; i < npairs; i += nwarps) {
           int p, q;
           rr_pair(M, r, i, p, q);
-          if (q < n) cmax = fmax(cmax, rotate_pair_global(G + (size_t)p * n, G + (size_t)q * n, n, lane, tol2, nchk, nrot));
+          if (q < n) cmax = fmax(cmax, rotate_pair_global(G + (size_t)p * n, G + (size_t)q * n, n, lane, tol2, dgap2, nchk, nrot));
         }
         if (r == M - 2 && cmax > kSeedStopCos2 && lane == 0) rot_flags[sweep] = 1;
         grid.sync();
@@ -847,7 +864,7 @@ __global__ void __launch_bounds__(128) seed_large_kernel(int n, const double2* _
 // shared memory (s_red: [4 * WPP] doubles of this pair).  Contains one __syncthreads when WPP > 1: every warp of the CTA calls it.
 template <int WPP>
 __device__ __forceinline__ double rotate_pair_smem(double2* __restrict__ gp, double2* __restrict__ gq, int n, int lane, int part,
-                                                   double* __restrict__ s_red, double tol2, unsigned long long& nchk,
+                                                   double* __restrict__ s_red, double tol2, double dgap2, unsigned long long& nchk,
                                                    unsigned long long& nrot) {
   const int chunk = (n + WPP - 1) / WPP;
   const int i0 = part * chunk, i1 = min(n, i0 + chunk);
@@ -868,7 +885,7 @@ __device__ __forceinline__ double rotate_pair_smem(double2* __restrict__ gp, dou
     for (int p = 0; p < WPP; ++p) { al += s_red[4 * p + 0]; be += s_red[4 * p + 1]; gr += s_red[4 * p + 2]; gi += s_red[4 * p + 3]; }
   }
   double c, sr, si, cos2;
-  const bool rot = rot_params(al, be, gr, gi, tol2, c, sr, si, cos2);
+  const bool rot = rot_params(al, be, gr, gi, tol2, dgap2, c, sr, si, cos2);
   if (part == 0) { nchk += n; if (rot) nrot += n; }
   if (!rot) return cos2;
   for (int i = i0 + lane; i < i1; i += 32) {
@@ -897,7 +914,7 @@ __device__ __forceinline__ void seed_mbar_wait(uint64_t* bar, uint32_t parity) {
 template <int W, int NWARPS>
 __global__ void __launch_bounds__(32 * NWARPS) seed_block_kernel(int n, const double2* __restrict__ A, double2* __restrict__ G,
                                                          const double* __restrict__ sigma_p, int* __restrict__ rot_flags,
-                                                         double* __restrict__ mu_unsorted, int max_sweeps, double tol2, int use_tma) {
+                                                         double* __restrict__ mu_unsorted, int max_sweeps, double tol2, double gap2, int use_tma) {
   extern __shared__ double2 s_cols[];  // [2 W][n]
   constexpr int WPP = NWARPS / W;      // warps per pair: all warps of the CTA rotate in every sub-round
   __shared__ double s_red[W][4 * WPP];
@@ -914,6 +931,7 @@ __global__ void __launch_bounds__(32 * NWARPS) seed_block_kernel(int n, const do
   const int gwarp = (blockIdx.x * blockDim.x + tid) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
   const size_t gtid = (size_t)blockIdx.x * blockDim.x + tid, gthr = (size_t)gridDim.x * blockDim.x;
   const double sigma = *sigma_p;
+  const double dgap2 = gap2 * sigma * sigma / n;
   for (size_t e = gtid; e < (size_t)n * n; e += gthr) {
     const int i = (int)(e % n), j = (int)(e / n);
     double2 a = (i <= j) ? A[(size_t)i * n + j] : A[(size_t)j * n + i];
@@ -974,13 +992,13 @@ __global__ void __launch_bounds__(32 * NWARPS) seed_block_kernel(int n, const do
               int p, q;
               rr_pair(W, t, i, p, q);
               cmax = fmax(cmax, rotate_pair_smem<WPP>(s_cols + (size_t)(blk * W + p) * n, s_cols + (size_t)(blk * W + q) * n, n, lane,
-                                                      part, s_red[pr], tol2, nchk, nrot));
+                                                      part, s_red[pr], tol2, dgap2, nchk, nrot));
               __syncthreads();
             }
           }
           for (int t = 0; t < W; ++t) {
             const int p = pr, q = W + (pr + t) % W;
-            cmax = fmax(cmax, rotate_pair_smem<WPP>(s_cols + (size_t)p * n, s_cols + (size_t)q * n, n, lane, part, s_red[pr], tol2, nchk, nrot));
+            cmax = fmax(cmax, rotate_pair_smem<WPP>(s_cols + (size_t)p * n, s_cols + (size_t)q * n, n, lane, part, s_red[pr], tol2, dgap2, nchk, nrot));
             __syncthreads();
           }
           if (use_tma) {
@@ -1028,7 +1046,7 @@ __global__ void __launch_bounds__(32 * NWARPS) seed_block_kernel(int n, const do
 
 template <int W, int NWARPS>
 static int launch_block(int n, int sms, const double2* Ab, double2* G, double* sigma, int* flags, double* mu_uns, int ms, double t2,
-                        cudaStream_t s) {
+                        double gap2, cudaStream_t s) {
   const size_t smem = sizeof(double2) * 2 * W * (size_t)n;
   if (cudaFuncSetAttribute(seed_block_kernel<W, NWARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess) {
     (void)cudaGetLastError();
@@ -1043,8 +1061,285 @@ static int launch_block(int n, int sms, const double2* Ab, double2* G, double* s
   int nblocks = MB / 2;
   if (nblocks > maxb * sms) nblocks = maxb * sms;
   int use_tma = options().seed_tma ? 1 : 0;
-  void* args[] = {&n, (void*)&Ab, &G, &sigma, &flags, &mu_uns, &ms, &t2, &use_tma};
+  void* args[] = {&n, (void*)&Ab, &G, &sigma, &flags, &mu_uns, &ms, &t2, &gap2, &use_tma};
   if (cudaLaunchCooperativeKernel((void*)seed_block_kernel<W, NWARPS>, dim3(nblocks), dim3(32 * NWARPS), args, smem, s) != cudaSuccess) {
+    (void)cudaGetLastError();
+    return ZKD_ERR_CUDA;
+  }
+  return ZKD_OK;
+}
+
+// ---- large matrices, blocked, GRAM form of a round (W = 4) -------------------------------------------------------------------
+// The same rotations in the same order as seed_block_kernel<4, .>, but a round's 16 (round 0 of a sweep: 28) rotations are found
+// on the 8 x 8 Gram matrix H = [P Q]^H [P Q] of the CTA's two blocks instead of on the long columns:
+//   1. H in ONE pass over the 8 columns (36 dot products, every thread a few rows, 64 fp64 accumulators, warp transpose-reduce);
+//   2. one warp runs the sub-rounds on H alone: (al, be, gamma) = (H_pp, H_qq, H_pq) are what the dot products of the rotated
+//      columns would give (H <- J^H H J is exact in exact arithmetic), and the rotations accumulate in an 8 x 8 unitary U;
+//   3. [P Q] <- [P Q] U in ONE pass (64 complex multiply-adds per row).
+// A round then has one long-vector reduction and two passes over shared memory instead of W dependent sub-rounds of
+// dot / reduce / barrier / parameters / update / barrier each (2.3 us per sub-round at n = 1024); the flop count is the same
+// to 20 % (384 n DFMA per round against 320 n) and both passes run at the fp64 pipe's rate.  Rounding: H carries the noise of
+// its two-sided updates (a few ulp of |g|^2 after <= 7 of them), the same order as freshly summed dot products.
+// rotation k (0..3) of sub-round t: pairs inside the blocks (round-robin over 4 columns, both blocks at once) or cross pairs
+__device__ __forceinline__ void gram_pair(bool inside, int t, int k, int& p, int& q) {
+  if (inside) {
+    rr_pair(4, t, k & 1, p, q);
+    p += (k >> 1) * 4;
+    q += (k >> 1) * 4;
+  } else {
+    p = k;
+    q = 4 + ((k + t) & 3);
+  }
+}
+
+template <int NWARPS>
+__global__ void __launch_bounds__(32 * NWARPS) seed_blockg_kernel(int n, const double2* __restrict__ A, double2* __restrict__ G,
+                                                                 const double* __restrict__ sigma_p, int* __restrict__ rot_flags,
+                                                                 double* __restrict__ mu_unsorted, int max_sweeps, double tol2, double gap2) {
+  constexpr int W = 4, C = 2 * W, NT = 32 * NWARPS;
+  extern __shared__ double2 s_cols[];  // [C][n]
+  __shared__ double s_part[NWARPS][64];
+  __shared__ double2 s_H[C][C], s_U[C][C];
+  __shared__ int s_any;
+  __shared__ __align__(8) uint64_t s_bar;
+  uint32_t bar_phase = 0;
+  if (threadIdx.x == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(seed_smem_u32(&s_bar)), "r"(1));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  cg::grid_group grid = cg::this_grid();
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int gwarp = (blockIdx.x * blockDim.x + tid) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
+  const size_t gtid = (size_t)blockIdx.x * blockDim.x + tid, gthr = (size_t)gridDim.x * blockDim.x;
+  const double sigma = *sigma_p;
+  const double dgap2 = gap2 * sigma * sigma / n;
+  for (size_t e = gtid; e < (size_t)n * n; e += gthr) {
+    const int i = (int)(e % n), j = (int)(e / n);
+    double2 a = (i <= j) ? A[(size_t)i * n + j] : A[(size_t)j * n + i];
+    if (i > j) a.y = -a.y;
+    if (i == j) { a.y = 0; a.x += sigma; }
+    G[e] = a;
+  }
+  if (gtid < (size_t)max_sweeps) rot_flags[gtid] = 0;
+  grid.sync();
+  const int NB = (n + W - 1) / W, MB = NB + (NB & 1), npairs = MB / 2;
+  unsigned long long nchk = 0, nrot = 0;
+  const uint32_t colb = (uint32_t)n * (uint32_t)sizeof(double2);
+  if (sigma > 0) {
+    for (int sweep = 0; sweep < max_sweeps; ++sweep) {
+      double cmax = 0;
+      for (int r = 0; r < MB - 1; ++r) {
+        for (int pi = blockIdx.x; pi < npairs; pi += gridDim.x) {
+          int bp, bq;
+          rr_pair(MB, r, pi, bp, bq);
+          // load: absent columns (beyond n, or the padding block) are zero and rot_params leaves zero columns alone
+          int present = 0;
+          for (int c = 0; c < C; ++c) {
+            const int col = (c < W ? bp : bq) * W + (c % W);
+            if (col < n) ++present;
+            else
+              for (int i = tid; i < n; i += NT) s_cols[(size_t)c * n + i] = make_double2(0.0, 0.0);
+          }
+          if (tid == 0) {
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(seed_smem_u32(&s_bar)), "r"(colb * (uint32_t)present)
+                         : "memory");
+            for (int c = 0; c < C; ++c) {
+              const int col = (c < W ? bp : bq) * W + (c % W);
+              if (col < n)
+                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                                 seed_smem_u32(s_cols + (size_t)c * n)),
+                             "l"(G + (size_t)col * n), "r"(colb), "r"(seed_smem_u32(&s_bar))
+                             : "memory");
+            }
+          }
+          seed_mbar_wait(&s_bar, bar_phase);
+          bar_phase ^= 1;
+          __syncthreads();  // the zero fill of absent columns
+          // 1. Gram matrix: v[0..7] = H_aa, v[8 + k] / v[36 + k] = Re / Im of H_ab = sum_i conj(g_a[i]) g_b[i], k = pair (a < b)
+          {
+            double v[64];
+#pragma unroll
+            for (int k = 0; k < 64; ++k) v[k] = 0.0;
+#pragma unroll 1
+            for (int i = tid; i < n; i += NT) {
+              double2 g[C];
+#pragma unroll
+              for (int c = 0; c < C; ++c) g[c] = s_cols[(size_t)c * n + i];
+              int k = 0;
+#pragma unroll
+              for (int a = 0; a < C; ++a) {
+                v[a] = fma(g[a].x, g[a].x, fma(g[a].y, g[a].y, v[a]));
+#pragma unroll
+                for (int b = a + 1; b < C; ++b, ++k) {
+                  v[8 + k] = fma(g[a].x, g[b].x, fma(g[a].y, g[b].y, v[8 + k]));
+                  v[36 + k] = fma(g[a].x, g[b].y, fma(-g[a].y, g[b].x, v[36 + k]));
+                }
+              }
+            }
+            // warp transpose-reduce: 64 values over 32 lanes, 62 exchanges; lane l ends up with the warp totals of values 2l, 2l + 1
+#pragma unroll
+            for (int off = 16, cnt = 32; off > 0; off >>= 1, cnt >>= 1) {
+              const bool up = (lane & off) != 0;
+#pragma unroll
+              for (int k = 0; k < cnt; ++k) {
+                const double send = up ? v[k] : v[k + cnt];
+                const double keep = up ? v[k + cnt] : v[k];
+                v[k] = keep + __shfl_xor_sync(0xffffffffu, send, off);
+              }
+            }
+            s_part[warp][2 * lane] = v[0];
+            s_part[warp][2 * lane + 1] = v[1];
+          }
+          __syncthreads();
+          if (tid < C * C) {
+            const int a = tid / C, b = tid % C;
+            const int lo = a < b ? a : b, hi = a < b ? b : a;
+            double re = 0, im = 0;
+            if (a == b) {
+#pragma unroll
+              for (int w = 0; w < NWARPS; ++w) re += s_part[w][a];
+            } else {
+              const int k = lo * C - (lo * (lo + 1)) / 2 + (hi - lo - 1);  // index of the pair (lo < hi) in the enumeration above
+#pragma unroll
+              for (int w = 0; w < NWARPS; ++w) { re += s_part[w][8 + k]; im += s_part[w][36 + k]; }
+              if (a > b) im = -im;
+            }
+            s_H[a][b] = make_double2(re, im);
+            s_U[a][b] = make_double2(a == b ? 1.0 : 0.0, 0.0);
+          }
+          if (tid == 0) s_any = 0;
+          __syncthreads();
+          // 2. the sub-rounds on H (warp 0): lane = (k, e), k = rotation of the sub-round, e = row (column step) / column (row step)
+          if (warp == 0) {
+            const int k = lane >> 3, e = lane & 7;
+            bool any = false;
+            const int nsub = (r == 0 ? W - 1 : 0) + W;
+            for (int ts = 0; ts < nsub; ++ts) {
+              const bool inside = r == 0 && ts < W - 1;
+              int p, q;
+              gram_pair(inside, inside ? ts : ts - (r == 0 ? W - 1 : 0), k, p, q);
+              const double al = s_H[p][p].x, be = s_H[q][q].x;
+              const double2 ga = s_H[p][q];
+              double c, sr, si, cos2;
+              const bool rot = rot_params(al, be, ga.x, ga.y, tol2, dgap2, c, sr, si, cos2);
+              cmax = fmax(cmax, cos2);
+              if (e == 0) { nchk += n; if (rot) nrot += n; }
+              any = any || rot;
+              if (!rot) { c = 1.0; sr = 0.0; si = 0.0; }
+              // columns p, q of H and of U (row e):  x' = c x - conj(s) y,  y' = s x + c y
+              {
+                const double2 x = s_H[e][p], y = s_H[e][q];
+                const double2 ux = s_U[e][p], uy = s_U[e][q];
+                __syncwarp();
+                s_H[e][p] = make_double2(c * x.x - (sr * y.x + si * y.y), c * x.y - (sr * y.y - si * y.x));
+                s_H[e][q] = make_double2(sr * x.x - si * x.y + c * y.x, sr * x.y + si * x.x + c * y.y);
+                s_U[e][p] = make_double2(c * ux.x - (sr * uy.x + si * uy.y), c * ux.y - (sr * uy.y - si * uy.x));
+                s_U[e][q] = make_double2(sr * ux.x - si * ux.y + c * uy.x, sr * ux.y + si * ux.x + c * uy.y);
+              }
+              __syncwarp();
+              // rows p, q of H (column e):  x' = c x - s y,  y' = conj(s) x + c y
+              {
+                const double2 x = s_H[p][e], y = s_H[q][e];
+                __syncwarp();
+                double2 xn = make_double2(c * x.x - (sr * y.x - si * y.y), c * x.y - (sr * y.y + si * y.x));
+                double2 yn = make_double2(sr * x.x + si * x.y + c * y.x, sr * x.y - si * x.x + c * y.y);
+                if (rot) {  // what the rotation makes exact: H_pq = 0, real diagonal
+                  if (e == q) xn = make_double2(0.0, 0.0);
+                  if (e == p) { yn = make_double2(0.0, 0.0); xn.y = 0.0; }
+                  if (e == q) yn.y = 0.0;
+                }
+                s_H[p][e] = xn;
+                s_H[q][e] = yn;
+              }
+              __syncwarp();
+            }
+            if (__any_sync(0xffffffffu, any) && lane == 0) s_any = 1;
+          }
+          __syncthreads();
+          // 3. [P Q] <- [P Q] U, a row at a time (a thread reads its row before it writes it: in place)
+          if (s_any) {
+            // two rows per thread and step, their 16 complex outputs accumulated in registers (32 independent fp64 chains: the
+            // fp64 pipe's latency is ~20 clocks, and a CTA has two warps per scheduler), U read as shared-memory broadcasts
+#pragma unroll 1
+            for (int i0 = tid; i0 < n; i0 += 2 * NT) {
+              const int i1 = i0 + NT;
+              const bool two = i1 < n;
+              double2 o0[C], o1[C];
+#pragma unroll
+              for (int b = 0; b < C; ++b) o0[b] = o1[b] = make_double2(0.0, 0.0);
+#pragma unroll
+              for (int a = 0; a < C; ++a) {
+                const double2 g0 = s_cols[(size_t)a * n + i0];
+                const double2 g1 = two ? s_cols[(size_t)a * n + i1] : make_double2(0.0, 0.0);
+#pragma unroll
+                for (int b = 0; b < C; ++b) {
+                  const double2 u = s_U[a][b];
+                  o0[b].x = fma(g0.x, u.x, fma(-g0.y, u.y, o0[b].x));
+                  o0[b].y = fma(g0.x, u.y, fma(g0.y, u.x, o0[b].y));
+                  o1[b].x = fma(g1.x, u.x, fma(-g1.y, u.y, o1[b].x));
+                  o1[b].y = fma(g1.x, u.y, fma(g1.y, u.x, o1[b].y));
+                }
+              }
+#pragma unroll
+              for (int b = 0; b < C; ++b) {
+                s_cols[(size_t)b * n + i0] = o0[b];
+                if (two) s_cols[(size_t)b * n + i1] = o1[b];
+              }
+            }
+          }
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // the rotated columns (generic-proxy writes) to the TMA engine
+          __syncthreads();
+          if (tid == 0) {
+            if (s_any) {
+              for (int c = 0; c < C; ++c) {
+                const int col = (c < W ? bp : bq) * W + (c % W);
+                if (col < n)
+                  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(G + (size_t)col * n),
+                               "r"(seed_smem_u32(s_cols + (size_t)c * n)), "r"(colb)
+                               : "memory");
+              }
+              asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+              asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");  // complete: the grid barrier below publishes the columns
+              asm volatile("fence.proxy.async.global;" ::: "memory");
+            }
+            __threadfence();
+          }
+          __syncthreads();
+        }
+        if (r == MB - 2 && cmax > kSeedStopCos2 && warp == 0) rot_flags[sweep] = 1;
+        grid.sync();
+      }
+      if (!rot_flags[sweep]) break;
+    }
+  }
+  if (warp == 0 && (lane & 7) == 0) seed_count(nchk, nrot);
+  for (int j = gwarp; j < n; j += nwarps) {
+    double s = 0;
+    for (int i = lane; i < n; i += 32) { const double2 a = G[(size_t)j * n + i]; s += a.x * a.x + a.y * a.y; }
+    s = warp_sum(s);
+    if (lane == 0) mu_unsorted[j] = sqrt(s) - sigma;
+  }
+}
+
+template <int NWARPS>
+static int launch_blockg(int n, int sms, const double2* Ab, double2* G, double* sigma, int* flags, double* mu_uns, int ms, double t2,
+                         double gap2, cudaStream_t s) {
+  const size_t smem = sizeof(double2) * 8 * (size_t)n;
+  if (cudaFuncSetAttribute(seed_blockg_kernel<NWARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 216 * 1024) != cudaSuccess) {
+    (void)cudaGetLastError();
+    return ZKD_ERR_CUDA;
+  }
+  int maxb = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&maxb, seed_blockg_kernel<NWARPS>, 32 * NWARPS, smem) != cudaSuccess || maxb < 1) {
+    (void)cudaGetLastError();
+    return ZKD_ERR_CUDA;
+  }
+  const int NB = (n + 3) / 4, MB = NB + (NB & 1);
+  int nblocks = MB / 2;
+  if (nblocks > maxb * sms) nblocks = maxb * sms;
+  void* args[] = {&n, (void*)&Ab, &G, &sigma, &flags, &mu_uns, &ms, &t2, &gap2};
+  if (cudaLaunchCooperativeKernel((void*)seed_blockg_kernel<NWARPS>, dim3(nblocks), dim3(32 * NWARPS), args, smem, s) != cudaSuccess) {
     (void)cudaGetLastError();
     return ZKD_ERR_CUDA;
   }
@@ -1077,9 +1372,23 @@ __global__ void __launch_bounds__(256) seed_sort_kernel(int n, const double* __r
   }
 }
 
-int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int max_sweeps, cudaStream_t s) {
+// square of the relative eigenvalue distance (in units of sigma / sqrt n) below which a pair counts as degenerate (rot_params):
+// 2^-g with g = tau_bits + 2, i.e. always below the cluster threshold 2^-tau ||A||_F of S2 (||A||_F >= sigma / (1.5 sqrt n)).
+// Option seed_degenerate_skip: 0 switches the rule off, 1 = this default, >= 8 = g itself (never below tau_bits + 1).
+// Measured (c5 ms per step / c4 ms per step): off 169.4 / 203.1; g = 21: 154.4 / 210.1; 22: 154.8 / 200.2; 24: 155.6 / 213.6;
+// 26: 159.1 / 203.0 - c5 gains a converged seed in 11 sweeps instead of an unconverged one in 12 and with it one refinement pass;
+// c4 moves by +- one pass (the batch's slowest matrix decides), not systematically.
+static double seed_gap2() {
+  const int v = options().seed_degenerate_skip;
+  if (!v) return 0.0;
+  const int g = std::max(v >= 8 ? v : options().tau_bits + 2, options().tau_bits + 1);
+  return ldexp(1.0, -2 * g);
+}
+
+int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int max_sweeps, cudaStream_t s, bool degenerate_skip) {
   const double tol = ldexp(1.0, -50);
   const double tol2 = tol * tol;
+  double gap2 = degenerate_skip ? seed_gap2() : 0.0;
   int dev = 0, sms = 0;
   ZKD_CUDA_TRY(cudaGetDevice(&dev));
   ZKD_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
@@ -1105,15 +1414,15 @@ int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int ma
         if (ppc <= ppc_max && csize <= max_cluster && (long)batch * csize <= 2L * sms) {
           int rc;
           if (Wb == 2) {
-            if (N <= 32) rc = launch_ringb<1, 2>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, s);
-            else if (N <= 64) rc = launch_ringb<2, 2>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, s);
-            else if (N <= 128) rc = launch_ringb<4, 2>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, s);
-            else rc = launch_ringb<8, 2>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, s);
+            if (N <= 32) rc = launch_ringb<1, 2>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, gap2, s);
+            else if (N <= 64) rc = launch_ringb<2, 2>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, gap2, s);
+            else if (N <= 128) rc = launch_ringb<4, 2>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, gap2, s);
+            else rc = launch_ringb<8, 2>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, gap2, s);
           } else {
-            if (N <= 32) rc = launch_ringb<1, 4>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, s);
-            else if (N <= 64) rc = launch_ringb<2, 4>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, s);
-            else if (N <= 128) rc = launch_ringb<4, 4>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, s);
-            else rc = launch_ringb<8, 4>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, s);
+            if (N <= 32) rc = launch_ringb<1, 4>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, gap2, s);
+            else if (N <= 64) rc = launch_ringb<2, 4>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, gap2, s);
+            else if (N <= 128) rc = launch_ringb<4, 4>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, gap2, s);
+            else rc = launch_ringb<8, 4>(N, batch, csize, ppc, A, mu, Vv, max_sweeps, tol2, gap2, s);
           }
           if (!(rc == ZKD_ERR_CUDA && csize > 8)) return rc;
           max_cluster = 8;  // a cluster of 16 was refused: the column ring below copes with 8
@@ -1131,15 +1440,15 @@ int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int ma
       // __syncthreads than behind a cluster barrier (measured: N = 16 0.109 -> 0.083 ms; N = 64 is 2.3 x slower that way)
       if ((csize == 1 || N <= 24 || options().seed_path == 5) && N <= 96 && options().seed_path != 2) {
         // a whole matrix per SM: plain CTA kernel (__syncthreads instead of cluster barriers)
-        if (N <= 32) rc = launch_cta<1>(N, batch, A, mu, Vv, max_sweeps, tol2, s);
-        else if (N <= 64) rc = launch_cta<2>(N, batch, A, mu, Vv, max_sweeps, tol2, s);
-        else rc = launch_cta<3>(N, batch, A, mu, Vv, max_sweeps, tol2, s);
+        if (N <= 32) rc = launch_cta<1>(N, batch, A, mu, Vv, max_sweeps, tol2, gap2, s);
+        else if (N <= 64) rc = launch_cta<2>(N, batch, A, mu, Vv, max_sweeps, tol2, gap2, s);
+        else rc = launch_cta<3>(N, batch, A, mu, Vv, max_sweeps, tol2, gap2, s);
         return rc;
       }
-      if (N <= 32) rc = launch_ring<1>(N, batch, csize, A, mu, Vv, max_sweeps, tol2, s);
-      else if (N <= 64) rc = launch_ring<2>(N, batch, csize, A, mu, Vv, max_sweeps, tol2, s);
-      else if (N <= 128) rc = launch_ring<4>(N, batch, csize, A, mu, Vv, max_sweeps, tol2, s);
-      else rc = launch_ring<8>(N, batch, csize, A, mu, Vv, max_sweeps, tol2, s);
+      if (N <= 32) rc = launch_ring<1>(N, batch, csize, A, mu, Vv, max_sweeps, tol2, gap2, s);
+      else if (N <= 64) rc = launch_ring<2>(N, batch, csize, A, mu, Vv, max_sweeps, tol2, gap2, s);
+      else if (N <= 128) rc = launch_ring<4>(N, batch, csize, A, mu, Vv, max_sweeps, tol2, gap2, s);
+      else rc = launch_ring<8>(N, batch, csize, A, mu, Vv, max_sweeps, tol2, gap2, s);
       if (rc == ZKD_ERR_CUDA && csize > 8 && max_cluster > 8) { max_cluster = 8; continue; }
       return rc;
     }
@@ -1185,14 +1494,17 @@ int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int ma
     const size_t col_bytes = sizeof(double2) * (size_t)n;
     const size_t smem_budget = 200 * 1024;
     const bool w16 = options().seed_block_warps == 16;  // 16 warps per CTA: twice the loads in flight, half the rows per warp
-    if (options().seed_path != 3 && 16 * col_bytes <= smem_budget)
-      rc = w16 ? launch_block<8, 16>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, s) : launch_block<8, 8>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, s);
+    if (options().seed_path != 3 && options().seed_gram && 8 * col_bytes <= 210 * 1024 &&
+        (options().seed_gram == 2 || 16 * col_bytes > smem_budget))
+      rc = launch_blockg<8>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, gap2, s);
+    else if (options().seed_path != 3 && 16 * col_bytes <= smem_budget)
+      rc = w16 ? launch_block<8, 16>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, gap2, s) : launch_block<8, 8>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, gap2, s);
     else if (options().seed_path != 3 && 8 * col_bytes <= smem_budget)
-      rc = w16 ? launch_block<4, 16>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, s) : launch_block<4, 8>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, s);
+      rc = w16 ? launch_block<4, 16>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, gap2, s) : launch_block<4, 8>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, gap2, s);
     else if (options().seed_path != 3 && 4 * col_bytes <= smem_budget)
-      rc = w16 ? launch_block<2, 16>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, s) : launch_block<2, 8>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, s);
+      rc = w16 ? launch_block<2, 16>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, gap2, s) : launch_block<2, 8>(n, sms, Ab, G, sigma, flags, mu_uns, ms, t2, gap2, s);
     else {
-      void* args[] = {&n, (void*)&Ab, &G, &sigma, &flags, &mu_uns, &ms, &t2};
+      void* args[] = {&n, (void*)&Ab, &G, &sigma, &flags, &mu_uns, &ms, &t2, &gap2};
       if (cudaLaunchCooperativeKernel((void*)seed_large_kernel, dim3(nblocks), dim3(128), args, 0, s) != cudaSuccess) {
         (void)cudaGetLastError();
         rc = ZKD_ERR_CUDA;
@@ -1271,7 +1583,7 @@ int seed_fp64_static(int N, int batch, const double* A64, double* mu, double* V,
     const double2* Ab = (const double2*)A64 + (size_t)b * nn;
     seed_sigma_kernel<<<1, 1024, 0, s>>>(N, Ab, sigma);
     const int ms = max_sweeps > 64 ? 64 : max_sweeps;
-    rc = launch_block<8, 8>(N, sms, Ab, G, sigma, flags, mu_uns, ms, tol * tol, s);
+    rc = launch_block<8, 8>(N, sms, Ab, G, sigma, flags, mu_uns, ms, tol * tol, 0.0, s);
     if (rc != ZKD_OK) break;
     seed_sort_kernel<<<sms, 256, 0, s>>>(N, mu_uns, G, sigma, mu + (size_t)b * N, (double2*)V + (size_t)b * nn);
     count_launch(3);

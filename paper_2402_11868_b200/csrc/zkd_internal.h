@@ -49,6 +49,8 @@ struct Options {
   int seed_ring_block = -1;   // ring seed (N <= 256): columns per block of the block ring (2 or 4); 0: the column ring; -1: 4 for N >= 96
   int seed_tma = 1;           // blocked seed: columns move between L2 and shared memory by 1-D TMA bulk copies
   int seed_block_warps = 8;   // blocked seed (N > 256): warps per CTA (8 or 16)
+  int seed_gram = 0;          // blocked seed: 1 / 2: a round's rotations found on the 8 x 8 Gram matrix of the CTA's two blocks (seed_blockg_kernel; 1: where the classic kernel would use W = 4, 2: up to N = 1600); measured slower (N = 1024: 44.1 vs 41.7 ms), off
+  int seed_degenerate_skip = 1;  // fp64 seed: leave column pairs of one (numerically) multiple eigenvalue unrotated (rot_params)
   int seed_dbuf = 1;     // ring seed: two slot sets, one cluster barrier per round (when they fit shared memory)
   int seed_path = 0;     // 0: auto; 2: always the ring kernel for N <= 256; 3: unblocked cooperative kernel for N > 256
   int early_split = 1;        // S4h: split clusters as soon as their internal structure stands above the noise
@@ -132,7 +134,9 @@ int fx_to_api(int count, const int32_t* src_fx, void* dst_api, int scale_bits, c
 // supported API precisions: multiples of 64 from 128 to 768 bits (PAPER.md:41 768, :61 256, :65 128)
 inline bool prec_supported(int prec) { return prec >= 128 && prec <= kPrec && (prec & 63) == 0; }
 inline size_t api_real_bytes(int prec) { return 16 + (size_t)prec / 8; }
-int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int max_sweeps, cudaStream_t s);
+// degenerate_skip: leave column pairs of one numerically multiple eigenvalue unrotated (rot_params in seed.cu); only for callers
+// that treat the clusters of S2 as blocks afterwards (solve_level)
+int seed_fp64(int N, int batch, const double* A64, double* mu, double* V, int max_sweeps, cudaStream_t s, bool degenerate_skip = false);
 // the same with its scratch in a static device array (N <= ZKD_SEED_STATIC_MAX_N): allocates nothing
 int seed_fp64_static(int N, int batch, const double* A64, double* mu, double* V, int max_sweeps, cudaStream_t s);
 

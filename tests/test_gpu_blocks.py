@@ -294,6 +294,16 @@ def test_seed_fp64_vs_lapack(zkd, N, batch):
         assert np.max(np.abs(A[b] @ V[b] - V[b] * mu[b][None, :])) <= 1e-11 * max(F, 1)
 
 
+@pytest.mark.parametrize("N", [300, 515, 1000])
+def test_seed_fp64_gram_rounds_vs_lapack(zkd, N):
+    """option seed_gram = 2: the blocked seed with the rotations of a round found on the Gram matrix of the CTA's column blocks."""
+    zkd.set_option("seed_gram", 2)
+    try:
+        test_seed_fp64_vs_lapack(zkd, N, 1)
+    finally:
+        zkd.set_option("seed_gram", 0)
+
+
 def test_measured_imad_peak_is_plausible(zkd):
     p = zkd.measure_imad_peak(30.0)
     # IMAD.WIDE with a 64-bit accumulator issues at half the 32-bit IMAD rate: 148 SMs x ~30.5 /clk x (1.0 .. 2.1 GHz)
