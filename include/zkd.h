@@ -174,7 +174,9 @@ int zkd_mps_two_site_update(int chiL, int chiC, int chiR, int d, int batch, int 
  * "seed_path" / "seed_cluster" (seed kernel selection), "cluster_tiles" (default 1: on levels where
  * no cluster straddles a multiple of 128 columns, most columns are clustered and the clusters average more than 51 columns,
  * the cluster-block products of a pass run as 128-column tile products on the int8 tcgen05 engine; 0: always per cluster on
- * the IMAD engine; 2: tiles wherever they can be formed),
+ * the IMAD engine; 2: tiles wherever they can be formed), "i8_bdiag" (default 1: in those tile products the block-diagonal
+ * operand M_t / S_t - no cluster straddling a multiple of 32 columns - is multiplied with 128 x 32 x 32 MMAs, one per 32-column
+ * block, instead of full-width ones; 0: full width; same integers either way),
  * "block_correction" (default 1: the correction between clusters takes
  * one fixed-point step with the off-diagonal parts of the cluster blocks of X^H A X, which squares the spread / gap factor
  * that otherwise caps the gain of a pass), "seed_ring_block" (columns per block of the block-ring fp64 seed for N <= 256:

@@ -215,6 +215,7 @@ static int* option_slot(const char* key) {
   if (!strcmp(key, "seed_block_warps")) return &o.seed_block_warps;
   if (!strcmp(key, "seed_tma")) return &o.seed_tma;
   if (!strcmp(key, "seed_gram")) return &o.seed_gram;
+  if (!strcmp(key, "i8_bdiag")) return &o.i8_bdiag;
   if (!strcmp(key, "seed_degenerate_skip")) return &o.seed_degenerate_skip;
   if (!strcmp(key, "seed_ring_block")) return &o.seed_ring_block;
   if (!strcmp(key, "seed_cluster")) return &o.seed_cluster;

@@ -621,7 +621,7 @@ int gemm_complex(int M, int N, int K, int batch, const GemmSide& P, const GemmSi
   }
   if (use_i8)
     return gemm_i8_finish(M, N, K, batch, Pc, Qc, npad, nqad, lsbP, lsbQ, dst_fx, (int)mode, out_cut_bit, raw,
-                          workspace_bytes - (size_t)((char*)raw - (char*)workspace), err_flag, msb_out, stream, dv);
+                          workspace_bytes - (size_t)((char*)raw - (char*)workspace), err_flag, msb_out, stream, dv, Q.bdiag32);
   const int tg = pick_tile(M, N, K);
   const int nsplit = pick_splits(M, N, K, batch, tg);
   int ksplit = (K + nsplit - 1) / nsplit;

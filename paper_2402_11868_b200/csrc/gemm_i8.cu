@@ -271,6 +271,7 @@ struct I8Args {
   int packed;
   int M, N, G, nsP, nsQ, dcut, ncol, ngroups, nkb, kb_per_split, nsplit;
   uint32_t p_tile_bytes, q_tile_bytes;  // bytes one TMA box delivers (rows may be < 128 for small matrices)
+  int bdiag;  // Q (128 x 128, one K block) is block diagonal in 32 x 32 blocks: K chunk k only feeds output columns 32 k .. 32 k + 31
 };
 
 // the slice ranges of one column group [d0, d0 + D)
@@ -404,10 +405,22 @@ gemm_i8_kernel(const __grid_constant__ CUtensorMap mapP, const __grid_constant__
               if (b < gr.b_min || b > gr.b_max) continue;
               const uint32_t sq = s0 >= (uint32_t)dd ? s0 - dd : s0 + I8_RQ - dd;
               const uint32_t qa = q_base + sq * I8_TILE_BYTES;
+              if (a.bdiag) {
+                // block-diagonal Q (cluster-tile products X_t M_t of a cluster pass): the 32 K values of chunk k meet only the 32 rows
+                // 32 k .. 32 k + 31 of the K-major Q tile (4096 bytes apart: whole 1024-byte swizzle atoms), so the MMA is 128 x 32 x 32
+                // into its own 32 accumulator columns - a quarter of the multiply-adds of the full-width instruction
+                constexpr uint32_t idesc32 = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(32 >> 3) << 17) | ((uint32_t)(I8_BM >> 4) << 24);
 #pragma unroll
-              for (int k = 0; k < I8_BK / 32; ++k) {
-                umma_i8(tmem_base + dd * I8_BN, umma_desc_sw128(pa + k * 32), umma_desc_sw128(qa + k * 32), idesc,
-                        ((started >> dd) & 1) | (k > 0));
+                for (int k = 0; k < I8_BK / 32; ++k) {
+                  umma_i8(tmem_base + dd * I8_BN + 32 * k, umma_desc_sw128(pa + k * 32), umma_desc_sw128(qa + k * 4096 + k * 32), idesc32,
+                          (started >> dd) & 1);
+                }
+              } else {
+#pragma unroll
+                for (int k = 0; k < I8_BK / 32; ++k) {
+                  umma_i8(tmem_base + dd * I8_BN, umma_desc_sw128(pa + k * 32), umma_desc_sw128(qa + k * 32), idesc,
+                          ((started >> dd) & 1) | (k > 0));
+                }
               }
               started |= 1u << dd;
             }
@@ -847,7 +860,7 @@ size_t gemm_i8_workspace_bytes(int M, int N, int K, int batch) {
 
 int gemm_i8_finish(int M, int N, int K, int batch, const int32_t* Pc, const int32_t* Qc, int np, int nq, int lsbP, int lsbQ,
                    int32_t* dst_fx, int mode, int cut_bit, void* ws, size_t ws_bytes, int* err_flag, int* msb_out,
-                   cudaStream_t stream, const GemmDstView* dv) {
+                   cudaStream_t stream, const GemmDstView* dv, bool q_bdiag32) {
   if (ws_bytes < gemm_i8_workspace_bytes(M, N, K, batch)) return ZKD_ERR_WORKSPACE;
   const int Kp = (K + I8_BK - 1) / I8_BK * I8_BK;
   const int G = 3 * batch;
@@ -900,6 +913,7 @@ int gemm_i8_finish(int M, int N, int K, int batch, const int32_t* Pc, const int3
   ka.nsplit = (ka.nkb + ka.kb_per_split - 1) / ka.kb_per_split;
   ka.p_tile_bytes = (uint32_t)boxP * I8_BK;
   ka.q_tile_bytes = (uint32_t)boxQ * I8_BK;
+  ka.bdiag = (q_bdiag32 && options().i8_bdiag && K == I8_BK && N == I8_BN) ? 1 : 0;
   // macro-step of 2 slices with rings <4, 9> by default; i8_step = 1: one slice per step, rings <5, 8>
   const bool step1 = options().i8_step == 1;
   auto kern = step1 ? gemm_i8_kernel<5, 8, 1> : gemm_i8_kernel<4, 9, 2>;
@@ -912,7 +926,7 @@ int gemm_i8_finish(int M, int N, int K, int batch, const int32_t* Pc, const int3
   for (int x = 0; x < nsP; ++x)
     for (int y = 0; y < nsQ; ++y)
       if (x + y >= dcut) ++pairs;
-  const uint64_t macs = pairs * (uint64_t)G * grid.x * grid.y * ka.nkb * I8_BM * I8_BN * I8_BK;
+  const uint64_t macs = pairs * (uint64_t)G * grid.x * grid.y * ka.nkb * I8_BM * I8_BN * I8_BK / (ka.bdiag ? 4 : 1);
   {
     // algorithmic: the same slice pairs on the matrices as they are (no padding of M, N, K to 128)
     KtScope kt(KC_GEMM_I8, stream, macs, (uint64_t)((double)(pairs * (uint64_t)G * M * N * K) * gemm_useful_fraction()));

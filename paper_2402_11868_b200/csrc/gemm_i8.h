@@ -11,7 +11,7 @@ size_t gemm_i8_workspace_bytes(int M, int N, int K, int batch);
 // sits at FX bit lsbP / lsbQ.  Writes dst (+)= P*Q like combine_kernel.
 int gemm_i8_finish(int M, int N, int K, int batch, const int32_t* Pc, const int32_t* Qc, int np, int nq, int lsbP, int lsbQ,
                    int32_t* dst_fx, int mode, int cut_bit, void* ws, size_t ws_bytes, int* err_flag, int* msb_out,
-                   cudaStream_t stream, const GemmDstView* dst_view = nullptr);
+                   cudaStream_t stream, const GemmDstView* dst_view = nullptr, bool q_bdiag32 = false);
 void kernel_timing_enable_i8(bool on);
 int kernel_timing_read_i8(double* ms, uint64_t* launches, uint64_t* i8_macs);
 void count_i8_macs(uint64_t n);

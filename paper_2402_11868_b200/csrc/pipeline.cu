@@ -133,6 +133,7 @@ struct ClusterPlan {
   bool tiled = false;
   std::vector<ClusterGroup> tile;  // one entry: m = 128, nsub = tiles that hold a cluster
   double tile_useful = 1.0;        // sum of m^2 over the clusters / (128^2 x tiles): the share of a tile product the clusters need
+  bool tile_bdiag32 = false;       // no cluster straddles a multiple of 32 columns: M_t, S_t are block diagonal in aligned 32 x 32 blocks
 };
 
 int build_plan(Ctx& c, int n, int nb, const std::vector<int>& h_cl, int* plan_dev /* 2 n nb ints */, ClusterPlan* plan) {
@@ -159,6 +160,7 @@ int build_plan(Ctx& c, int n, int nb, const std::vector<int>& h_cl, int* plan_de
   }
   plan->has_singletons = clustered < (size_t)n * nb;
   plan->tiled = false;
+  plan->tile_bdiag32 = false;
   plan->tile.clear();
   constexpr int TW = 128;
   // a tile computes 128 / m times the entries a cluster of m needs, but the int8 engine is that much faster per entry than the
@@ -170,11 +172,12 @@ int build_plan(Ctx& c, int n, int nb, const std::vector<int>& h_cl, int* plan_de
   const bool tiles_pay = options().cluster_tiles == 2 || (options().cluster_tiles == 1 && sum_m2 >= 10 * clustered);
   if (options().gemm_path != 1 && tiles_pay && n >= TW && n % TW == 0 && 2 * clustered >= (size_t)n * nb &&
       gemm_i8_eligible(options().gemm_path, TW, TW, n, 1)) {
-    bool ok = true;
+    bool ok = true, ok32 = true;
     std::vector<char> used((size_t)(n / TW) * nb, 0);
     for (const auto& kv : groups)
       for (const SubProblem& sp : kv.second) {
         if (sp.col0 / TW != (sp.col0 + kv.first - 1) / TW) ok = false;
+        if (sp.col0 / 32 != (sp.col0 + kv.first - 1) / 32) ok32 = false;
         used[(size_t)sp.b * (n / TW) + sp.col0 / TW] = 1;
       }
     if (ok) {
@@ -197,6 +200,7 @@ int build_plan(Ctx& c, int n, int nb, const std::vector<int>& h_cl, int* plan_de
         plan->tile.push_back(g);
         plan->tiled = true;
         plan->tile_useful = (double)sum_m2 / ((double)TW * TW * g.nsub);
+        plan->tile_bdiag32 = ok32;
       }
     }
   }
@@ -231,6 +235,8 @@ int cluster_pass(Ctx& c, int n, int nb, const ClusterPlan& plan, const int* cl, 
                         &dv);
   };
   const int nwX = digits_for(topX, cut), nwW = digits_for(topW, cut);
+  // M_t / S_t of a tiled pass are masked to their cluster blocks (ns_build with zero_rest, mask_offcluster): block diagonal
+  auto bd = [&](GemmSide g) { g.bdiag32 = plan.tiled && plan.tile_bdiag32; return g; };
   // the products of this pass run per cluster (IMAD engine) or per 128-column tile (int8 tcgen05 engine), see ClusterPlan
   const std::vector<ClusterGroup>& groups = plan.tiled ? plan.tile : plan.groups;
   // timing only: the ALGORITHMIC work of a tile product is the share its cluster blocks need (the rest is executed padding)
@@ -252,9 +258,9 @@ int cluster_pass(Ctx& c, int n, int nb, const ClusterPlan& plan, const int* cl, 
     const int topM = msb_m + 1, nwM = std::max(1, std::min(kND, ceil_div(topM - (cutG - 1), kDB)));
     const int nwXm = digits_for(topX, c.fb), nwWm = digits_for(topW, c.fb);
     for (const ClusterGroup& g : groups) {
-      ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(X, n, g.m, false, topX, nwXm, g.offX), view(Gm, g.m, g.m, false, topM, nwM, g.offB), X,
+      ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(X, n, g.m, false, topX, nwXm, g.offX), bd(view(Gm, g.m, g.m, false, topM, nwM, g.offB)), X,
                    GemmMode::Add, g.offX, nullptr));
-      ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(W, n, g.m, false, topW, nwWm, g.offX), view(Gm, g.m, g.m, false, topM, nwM, g.offB), W,
+      ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(W, n, g.m, false, topW, nwWm, g.offX), bd(view(Gm, g.m, g.m, false, topM, nwM, g.offB)), W,
                    GemmMode::Add, g.offX, nullptr));
     }
   }
@@ -270,7 +276,7 @@ int cluster_pass(Ctx& c, int n, int nb, const ClusterPlan& plan, const int* cl, 
   if (plan.tiled) ZKD_TRY(mask_offcluster(n, nb, cl, cle, Sm, s));  // keep the cluster blocks of the tiles only (singletons: theta, R are the fused kernel's)
   ZKD_TRY(theta_from_diag(n, nb, Sm, theta, s, plan.tiled ? cl : nullptr, plan.tiled ? cle : nullptr));
   for (const ClusterGroup& g : groups)
-    ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(X, n, g.m, false, topX, nwX, g.offX), view(Sm, g.m, g.m, false, topW, nwW, g.offB), R,
+    ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(X, n, g.m, false, topX, nwX, g.offX), bd(view(Sm, g.m, g.m, false, topW, nwW, g.offB)), R,
                  GemmMode::Sub, g.offX, scal + S_MSB_R));
   return ZKD_OK;
 }

@@ -59,6 +59,7 @@ struct Options {
   int i8_packed = 1;          // int8 GEMM output: 1 = one int64 per entry and group of four columns (combine_i8_packed_kernel), 0 = int32 columns
   int i8_slice = 0;           // int8 GEMM re-slicing kernel: 0 = four k per thread, seven slices per step; 1 = one element per thread
   int i8_step = 0;            // int8 GEMM: slices a per barrier round trip: 0 / 2 = two (rings <4, 9>), 1 = one (rings <5, 8>)
+  int i8_bdiag = 1;           // int8 GEMM: quarter-width MMAs for block-diagonal Q tiles (GemmSide::bdiag32)
   int cluster_tiles = 1;      // cluster passes as 128-column tile products on the int8 engine when no cluster straddles a tile
   int combine_path = 0;       // IMAD GEMM epilogue: 0 auto, 1 digit-serial thread per element, 2 warp-cooperative (digit per lane)
   int sstep_warp = 0;         // singleton_step: 1: warp-per-element kernel (digit per lane) when one column per CTA and n <= 64; measured 1 % faster at N = 16, 3 % slower at N = 64: off by default
@@ -98,6 +99,9 @@ struct GemmSide {
   int ld = 0;                // 0: cols
   const int* off = nullptr;  // device, [batch]; null: v * rows * cols
   size_t plane_count = 0;    // 0: batch * rows * cols
+  // Q only, a promise of the caller: the 128 x 128 matrices are block diagonal in aligned 32 x 32 blocks (cluster-tile products);
+  // the int8 engine then issues 128 x 32 x 32 MMAs (gemm_i8.cu)
+  bool bdiag32 = false;
 };
 struct GemmDstView {         // the same for the destination (M x N per batch element)
   int ld = 0;

@@ -131,13 +131,14 @@ def test_parity_public_entry_points(zkd, name, batch):
                                           ("c4small", "sstep_warp", 1), ("c2", "sstep_cache", 0), ("c5mid", "cluster_tiles", 2), ("c5small", "block_correction", 0), ("c2", "sstep_par", 0), ("c1", "sstep_par", 0),
                                           ("c4small", "block_correction", 0), ("c5small", "seed_degenerate_skip", 0),
                                           ("c5mid", "seed_degenerate_skip", 0), ("c4small", "seed_degenerate_skip", 0),
-                                          ("c4small", "seed_degenerate_skip", 30), ("c5small", "seed_degenerate_skip", 40)])
+                                          ("c4small", "seed_degenerate_skip", 30), ("c5small", "seed_degenerate_skip", 40), ("c5mid", "i8_bdiag", 0)])
 def test_parity_alternative_paths(zkd, name, opt, val):
     """The same results through the other routes of the method: clusters left to the S5 recursion (S4h off), a different
     cluster threshold (other cluster tables, splits and recursion depths), several matrix columns per CTA in the fused
     singleton kernel, its warp-per-element variant (digit per lane, carries by shuffles and ballots), no shared-memory
     staging, the cluster passes as 128-column tile products on the int8 tcgen05 engine, the correction without its second-order
-    block step, the fp64 seed rotating degenerate pairs too (the rule is on by default) or with another degeneracy threshold."""
+    block step, the fp64 seed rotating degenerate pairs too (the rule is on by default) or with another degeneracy threshold, the
+    cluster-tile products with full-width MMAs on their block-diagonal operand (quarter-width by default)."""
     cfg = zi.config(name, batch=2 if name == "c4small" else None)
     N, b = cfg["N"], cfg["batch"]
     old = zkd.get_option(opt)
