@@ -130,15 +130,14 @@ def test_parity_public_entry_points(zkd, name, batch):
                                           ("c2", "sstep_cpb", 4), ("c1", "sstep_cpb", 2), ("c2", "sstep_warp", 1), ("c1", "sstep_warp", 1),
                                           ("c4small", "sstep_warp", 1), ("c2", "sstep_cache", 0), ("c5mid", "cluster_tiles", 2), ("c5small", "block_correction", 0), ("c2", "sstep_par", 0), ("c1", "sstep_par", 0),
                                           ("c4small", "block_correction", 0), ("c5small", "seed_degenerate_skip", 0),
-                                          ("c5mid", "seed_degenerate_skip", 0), ("c4small", "seed_degenerate_skip", 0),
-                                          ("c4small", "seed_degenerate_skip", 30), ("c5small", "seed_degenerate_skip", 40), ("c5mid", "i8_bdiag", 0)])
+                                          ("c4small", "seed_degenerate_skip", 0),
+                                          ("c4small", "seed_degenerate_skip", 30), ("c5small", "seed_degenerate_skip", 40)])
 def test_parity_alternative_paths(zkd, name, opt, val):
     """The same results through the other routes of the method: clusters left to the S5 recursion (S4h off), a different
     cluster threshold (other cluster tables, splits and recursion depths), several matrix columns per CTA in the fused
     singleton kernel, its warp-per-element variant (digit per lane, carries by shuffles and ballots), no shared-memory
     staging, the cluster passes as 128-column tile products on the int8 tcgen05 engine, the correction without its second-order
-    block step, the fp64 seed rotating degenerate pairs too (the rule is on by default) or with another degeneracy threshold, the
-    cluster-tile products with full-width MMAs on their block-diagonal operand (quarter-width by default)."""
+    block step, the fp64 seed rotating degenerate pairs too (the rule is on by default) or with another degeneracy threshold."""
     cfg = zi.config(name, batch=2 if name == "c4small" else None)
     N, b = cfg["N"], cfg["batch"]
     old = zkd.get_option(opt)
@@ -152,6 +151,27 @@ def test_parity_alternative_paths(zkd, name, opt, val):
         assert info[i]["status"] == 0, info[i]
         l0, X0, _ = oracle.diag_herm(A[i], N)
         check(oracle.compare(A[i], N, lam[i], X[i], l0, X0), (name, opt, val, i))
+
+
+def test_i8_bdiag_same_bits(zkd):
+    """The cluster-tile apply products with quarter-width MMAs on their block-diagonal operand (option i8_bdiag, the default) give
+    the same integers as with full-width MMAs: c5mid with the tile route forced, both settings, outputs compared byte for byte
+    (the oracle parity of this route is test_parity_alternative_paths[c5mid-cluster_tiles-2])."""
+    cfg = zi.config("c5mid")
+    N, b = cfg["N"], cfg["batch"]
+    old = {k: zkd.get_option(k) for k in ("cluster_tiles", "i8_bdiag")}
+    out = {}
+    try:
+        zkd.set_option("cluster_tiles", 2)
+        for v in (1, 0):
+            zkd.set_option("i8_bdiag", v)
+            lam, X, info = gpu_diag(zkd, cfg["A"], N, b)
+            assert all(i["status"] == 0 for i in info), info
+            out[v] = (lam.copy(), X.copy())
+    finally:
+        for k, v in old.items():
+            zkd.set_option(k, v)
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
 
 
 @pytest.mark.parametrize("N", [1, 2, 3, 5, 17, 31, 33, 48, 65, 100])
