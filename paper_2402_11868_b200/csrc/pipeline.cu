@@ -256,7 +256,10 @@ int cluster_pass(Ctx& c, int n, int nb, const ClusterPlan& plan, const int* cl, 
     // These two must be exact to the FX floor, whatever the pass's precision: W = A X is kept incrementally, so an error
     // made here would stay in W for good.  Exact = all digits of X / W times all nonzero digits of M (those above cutG - 1).
     const int topM = msb_m + 1, nwM = std::max(1, std::min(kND, ceil_div(topM - (cutG - 1), kDB)));
-    const int nwXm = digits_for(topX, c.fb), nwWm = digits_for(topW, c.fb);
+    // ... of X / W only the digits whose product with the TOP bit of M still reaches the floor (one digit of guard below it), as for
+    // A in W += A T: |M| < 2^(topM - 812), so a digit of X below FX bit fb + 784 - topM contributes less than 2^(fb - 28)
+    const int lowXM = c.fb + std::max(0, 784 - topM);
+    const int nwXm = digits_for(topX, lowXM), nwWm = digits_for(topW, lowXM);
     for (const ClusterGroup& g : groups) {
       ZKD_TRY(gemm(n, g.m, g.m, g.nsub, view(X, n, g.m, false, topX, nwXm, g.offX), bd(view(Gm, g.m, g.m, false, topM, nwM, g.offB)), X,
                    GemmMode::Add, g.offX, nullptr));
