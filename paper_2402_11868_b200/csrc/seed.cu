@@ -14,6 +14,10 @@
 //              cross distributed shared memory; rounds are separated by the hardware cluster barrier.  With many matrices
 //              in the batch the cluster shrinks to 1 CTA (one SM per matrix, plain CTA kernel).
 //   n  > 256 : cooperative grid, G in global memory (L2 resident), grid.sync between rounds.
+//              (seed_block_kernel: blocks of W columns per CTA in shared memory, TMA bulk copies; seed_blockg_kernel: the same
+//              rounds on the 8 x 8 Gram matrix of the CTA's blocks, measured slower, option seed_gram)
+// Column pairs of one numerically multiple eigenvalue are left unrotated when the caller treats clusters as blocks afterwards
+// (rot_params, dgap2): this keeps the sweeps quadratically convergent on spectra with multiplicities.
 // The seed only has to be good to ~2^-40 (the refinement squares the error every step).
 #include <cooperative_groups.h>
 
